@@ -1,0 +1,679 @@
+// ORACLE -- TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, obviously-correct CPU implementation of the batched tactile readout of
+// Tactile Genesis (arxiv/paper_2606_22332), written from /root/reference/PAPER.md
+// ("P:NNN" = PAPER.md line NNN) and the readings fixed in DESIGN.md / SURVEY.md 8(c)
+// ("O0".."O8", "D1".."D5", "Q1".."Q24").  Every floating-point step is evaluated in
+// double precision on the fp32 input values, in the paper's order and notation; there
+// is no blocking, fusion, table or reordering.  It shares no code with the CUDA path
+// (paper_2606_22332_b200/csrc/), includes none of its headers and is never imported by
+// the product.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference legs may load it.
+//
+// Pins (tests/test_oracle_pins.py, all -m "not gpu"):
+//   philox4x32_10            known-answer vectors (P15)
+//   primitive SDFs           closed forms + brute-force surface sampling (P1, P5)
+//   grid SDF                 affine field exact, star grid vs analytic, brute-force mesh (P6, P7, P9)
+//   depth / contact          worked sphere example, Schmitt hand sequence (P1, P10)
+//   kinematic force/torque   closed-form spring / damping / cap values (P2-P4)
+//   marker                   single-source closed form at r* (P11)
+//   march                    plane closed form t_k = D/cos(th) (1-(1-cos th)^k) (P12)
+//   noise                    Maxwell / asym closed forms, crosstalk patch-sum, drift moments, dead (P13-P16)
+//   whole path               rigid-frame invariance, filler slots, no-contact zeros (P8, P17)
+// parity unpinned: none of the functions; the *joint* output on star grids with all
+// stages on (configs 4-5) is pinned only through the per-stage pins above (P18).
+//
+// Build: g++ -O2 -std=c++17 -fPIC -shared -fopenmp oracle.cpp -o liboracle.so
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+struct V3 { double x, y, z; };
+inline V3 operator+(V3 a, V3 b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+inline V3 operator-(V3 a, V3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+inline V3 operator*(double s, V3 a) { return {s * a.x, s * a.y, s * a.z}; }
+inline double dot(V3 a, V3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+inline V3 cross(V3 a, V3 b) { return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x}; }
+inline double norm(V3 a) { return std::sqrt(dot(a, a)); }
+inline V3 ld3(const float* p) { return {(double)p[0], (double)p[1], (double)p[2]}; }
+
+// O0: rotation matrix of a quaternion (w,x,y,z), used as given (no renormalisation).
+struct M3 { double m[3][3]; };
+inline M3 quat_to_R(const float* q) {
+  double w = q[0], x = q[1], y = q[2], z = q[3];
+  M3 R;
+  R.m[0][0] = 1 - 2 * (y * y + z * z); R.m[0][1] = 2 * (x * y - w * z);     R.m[0][2] = 2 * (x * z + w * y);
+  R.m[1][0] = 2 * (x * y + w * z);     R.m[1][1] = 1 - 2 * (x * x + z * z); R.m[1][2] = 2 * (y * z - w * x);
+  R.m[2][0] = 2 * (x * z - w * y);     R.m[2][1] = 2 * (y * z + w * x);     R.m[2][2] = 1 - 2 * (x * x + y * y);
+  return R;
+}
+inline V3 mul(const M3& R, V3 v) {
+  return {R.m[0][0] * v.x + R.m[0][1] * v.y + R.m[0][2] * v.z,
+          R.m[1][0] * v.x + R.m[1][1] * v.y + R.m[1][2] * v.z,
+          R.m[2][0] * v.x + R.m[2][1] * v.y + R.m[2][2] * v.z};
+}
+inline V3 mulT(const M3& R, V3 v) {  // R^T v
+  return {R.m[0][0] * v.x + R.m[1][0] * v.y + R.m[2][0] * v.z,
+          R.m[0][1] * v.x + R.m[1][1] * v.y + R.m[2][1] * v.z,
+          R.m[0][2] * v.x + R.m[1][2] * v.y + R.m[2][2] * v.z};
+}
+
+// ---------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al. 2011).  O8 "Random draws".
+// ---------------------------------------------------------------------------------
+void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+  uint32_t k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+    uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+    uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    uint32_t n0 = hi1 ^ c1 ^ k0;
+    uint32_t n1 = lo1;
+    uint32_t n2 = hi0 ^ c3 ^ k1;
+    uint32_t n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// O8: u = (2 (w >> 9) + 1) 2^-24, in (0,1), exact in fp32.
+inline double word_to_uniform(uint32_t w) { return (2.0 * (double)(w >> 9) + 1.0) * (1.0 / 16777216.0); }
+
+// O8: Box-Muller on a word pair.
+inline void box_muller(uint32_t wa, uint32_t wb, double* z0, double* z1) {
+  const double two_pi = 6.283185307179586476925286766559;
+  double ua = word_to_uniform(wa), ub = word_to_uniform(wb);
+  double r = std::sqrt(-2.0 * std::log(ua));
+  *z0 = r * std::cos(two_pi * ub);
+  *z1 = r * std::sin(two_pi * ub);
+}
+
+// ---------------------------------------------------------------------------------
+// O2: geometry queries.  Types: 0 none, 1 sphere, 2 box, 3 capsule, 4 SDF grid.
+// ---------------------------------------------------------------------------------
+enum { G_NONE = 0, G_SPHERE = 1, G_BOX = 2, G_CAPSULE = 3, G_GRID = 4 };
+
+struct Query {
+  double phi;      // signed distance
+  V3 g;            // object-frame gradient, NOT normalised
+  double face;     // grid only: min over axes of the distance (voxels) of u to an integer
+  double boxgap;   // box interior only: gap between the two largest w_i
+};
+
+// sphere: phi = |x| - r, g = x/|x|  (Q7: g = e_z at the centre)
+Query sdf_sphere(V3 x, double r) {
+  Query q; q.face = INFINITY; q.boxgap = INFINITY;
+  double n = norm(x);
+  q.phi = n - r;
+  q.g = (n < 1e-12) ? V3{0, 0, 1} : (1.0 / n) * x;
+  return q;
+}
+
+// box, half-extents b (Q7)
+Query sdf_box(V3 x, V3 b) {
+  Query q; q.face = INFINITY; q.boxgap = INFINITY;
+  double w[3] = {std::fabs(x.x) - b.x, std::fabs(x.y) - b.y, std::fabs(x.z) - b.z};
+  double sgn[3] = {x.x < 0 ? -1.0 : 1.0, x.y < 0 ? -1.0 : 1.0, x.z < 0 ? -1.0 : 1.0};
+  double p[3] = {std::fmax(w[0], 0.0), std::fmax(w[1], 0.0), std::fmax(w[2], 0.0)};
+  double lp = std::sqrt(p[0] * p[0] + p[1] * p[1] + p[2] * p[2]);
+  double wmax = std::fmax(w[0], std::fmax(w[1], w[2]));
+  q.phi = lp + std::fmin(wmax, 0.0);
+  bool outside = (w[0] > 0) || (w[1] > 0) || (w[2] > 0);
+  if (outside) {
+    q.g = {sgn[0] * p[0] / lp, sgn[1] * p[1] / lp, sgn[2] * p[2] / lp};
+  } else {
+    int i = 0;                       // argmax w_i, ties -> lowest index
+    if (w[1] > w[i]) i = 1;
+    if (w[2] > w[i]) i = 2;
+    double second = -INFINITY;
+    for (int a = 0; a < 3; ++a) if (a != i) second = std::fmax(second, w[a]);
+    q.boxgap = w[i] - second;
+    q.g = {0, 0, 0};
+    if (i == 0) q.g.x = sgn[0]; else if (i == 1) q.g.y = sgn[1]; else q.g.z = sgn[2];
+  }
+  return q;
+}
+
+// capsule, radius r, half-length h along local z
+Query sdf_capsule(V3 x, double r, double h) {
+  Query q; q.face = INFINITY; q.boxgap = INFINITY;
+  double zc = std::fmin(std::fmax(x.z, -h), h);
+  V3 y = {x.x, x.y, x.z - zc};
+  double n = norm(y);
+  q.phi = n - r;
+  q.g = (n < 1e-12) ? V3{0, 0, 1} : (1.0 / n) * y;
+  return q;
+}
+
+// grid: N^3 nodes, voxel hv, node i at origin + i hv with origin = -(N-1)/2 hv; data
+// index (k N + j) N + i, i <-> x fastest.  Trilinear value, exact gradient of the
+// interpolant in cell i0, outside-grid extension phi = phi_tri(u_c) + |x - x(u_c)|.
+Query sdf_grid(V3 x, const float* data, int N, double hv) {
+  Query q; q.boxgap = INFINITY;
+  double origin = -0.5 * (N - 1) * hv;
+  double xs[3] = {x.x, x.y, x.z};
+  double uc[3], f[3];
+  int i0[3];
+  double face = INFINITY, out2 = 0.0;
+  for (int a = 0; a < 3; ++a) {
+    double u = (xs[a] - origin) / hv;
+    double c = std::fmin(std::fmax(u, 0.0), (double)(N - 1));
+    uc[a] = c;
+    int i = (int)std::floor(c);
+    if (i > N - 2) i = N - 2;
+    i0[a] = i;
+    f[a] = c - i;
+    double xc = origin + c * hv;
+    out2 += (xs[a] - xc) * (xs[a] - xc);
+    face = std::fmin(face, std::fabs(u - std::round(u)));
+  }
+  auto at = [&](int di, int dj, int dk) -> double {
+    size_t idx = ((size_t)(i0[2] + dk) * N + (size_t)(i0[1] + dj)) * N + (size_t)(i0[0] + di);
+    return (double)data[idx];
+  };
+  double c000 = at(0, 0, 0), c100 = at(1, 0, 0), c010 = at(0, 1, 0), c110 = at(1, 1, 0);
+  double c001 = at(0, 0, 1), c101 = at(1, 0, 1), c011 = at(0, 1, 1), c111 = at(1, 1, 1);
+  double fx = f[0], fy = f[1], fz = f[2];
+  double gx0 = 1 - fx, gy0 = 1 - fy, gz0 = 1 - fz;
+  double tri = c000 * gx0 * gy0 * gz0 + c100 * fx * gy0 * gz0 + c010 * gx0 * fy * gz0 + c110 * fx * fy * gz0 +
+               c001 * gx0 * gy0 * fz + c101 * fx * gy0 * fz + c011 * gx0 * fy * fz + c111 * fx * fy * fz;
+  double dx = ((c100 - c000) * gy0 * gz0 + (c110 - c010) * fy * gz0 + (c101 - c001) * gy0 * fz + (c111 - c011) * fy * fz) / hv;
+  double dy = ((c010 - c000) * gx0 * gz0 + (c110 - c100) * fx * gz0 + (c011 - c001) * gx0 * fz + (c111 - c101) * fx * fz) / hv;
+  double dz = ((c001 - c000) * gx0 * gy0 + (c101 - c100) * fx * gy0 + (c011 - c010) * gx0 * fy + (c111 - c110) * fx * fy) / hv;
+  q.phi = tri + std::sqrt(out2);
+  q.g = {dx, dy, dz};
+  q.face = face;
+  return q;
+}
+
+struct Geom {
+  int type;
+  double p[4];
+  const float* grid;  // type 4
+  int N;
+  double hv;
+};
+
+Query sdf_eval(const Geom& g, V3 x) {
+  switch (g.type) {
+    case G_SPHERE: return sdf_sphere(x, g.p[0]);
+    case G_BOX: return sdf_box(x, {g.p[0], g.p[1], g.p[2]});
+    case G_CAPSULE: return sdf_capsule(x, g.p[0], g.p[1]);
+    case G_GRID: return sdf_grid(x, g.grid, g.N, g.hv);
+    default: {
+      Query q; q.phi = INFINITY; q.g = {0, 0, 1}; q.face = INFINITY; q.boxgap = INFINITY;
+      return q;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------
+// Parameters and patches (plain C structs, mirrored by ctypes in oracle/oracle.py)
+// ---------------------------------------------------------------------------------
+extern "C" {
+typedef struct orc_patch {
+  int32_t link;
+  float origin[3];
+  float u_axis[3];
+  float v_axis[3];
+  float size_u, size_v;
+  int32_t nu, nv;
+  float radius;
+  int32_t marker_nu, marker_nv;
+} orc_patch;
+
+typedef struct orc_params {
+  float k_n, c_n, alpha, k_t, k_omega, mu, eta_on, eta_off;
+  int32_t use_velocity;
+  float s_d, lambda_d, alpha_e, c_e;
+  float r_prox;
+  int32_t march_steps;
+  float dt;
+  int32_t noise_enable;
+  uint32_t seed_lo, seed_hi;
+  float sigma_rw_force, sigma_rw_torque;
+  int32_t hyst_mode;  // 0 off, 1 Maxwell (Eq. 29-30), 2 asymmetric first-order (D3)
+  float beta, tau, alpha_load, alpha_unload;
+  float p_dead, chi;
+} orc_params;
+}
+
+struct Oracle {
+  int E, L, K, T, P, M;
+  std::vector<int64_t> env_id;  // global env ids (Philox counters use these)
+  orc_params prm;
+  // S0 layout; values are the fp32-rounded ones, held in double.
+  std::vector<V3> pos, nrm, mpos, mnrm;
+  std::vector<double> radius;
+  std::vector<int> link, patch, iu, iv, mpatch;
+  std::vector<int> p_start, p_nu, p_nv, p_link, p_mstart, p_mcount;
+  std::vector<double> p_eps;
+  std::vector<int> nbr;  // [T,4]: -u, +u, -v, +v; -1 = none
+  // geometry
+  std::vector<Geom> geom;  // [E,K]
+  std::vector<float> bank;
+  int bank_n = 0, bank_N = 0;
+  double bank_hv = 0;
+  // state
+  std::vector<uint8_t> ybit;                // Schmitt state [E,T]
+  std::vector<double> hyst_a, hyst_b, drift;  // [E,T,6]: (xi, x_prev) or (y, -)
+  std::vector<uint32_t> n_step, episode;      // [E]
+};
+
+inline double f32(double v) { return (double)(float)v; }
+
+// S0 (Q19): cell-centred regular grid on each patch.
+void build_layout(Oracle& o, const orc_patch* patches, int P, int T, const uint8_t* link_mask) {
+  o.P = P; o.T = T;
+  o.pos.assign(T, {0, 0, 0}); o.nrm.assign(T, {0, 0, 1}); o.radius.assign(T, 0.0);
+  o.link.assign(T, 0); o.patch.assign(T, -1); o.iu.assign(T, 0); o.iv.assign(T, 0);
+  o.nbr.assign((size_t)T * 4, -1);
+  o.mpos.clear(); o.mnrm.clear(); o.mpatch.clear();
+  o.p_start.clear(); o.p_nu.clear(); o.p_nv.clear(); o.p_link.clear(); o.p_mstart.clear(); o.p_mcount.clear(); o.p_eps.clear();
+  int t = 0;
+  for (int p = 0; p < P; ++p) {
+    const orc_patch& d = patches[p];
+    V3 org = ld3(d.origin), ua = ld3(d.u_axis), va = ld3(d.v_axis);
+    V3 n = cross(ua, va);
+    bool keep = (link_mask == nullptr) || link_mask[d.link];
+    o.p_start.push_back(t); o.p_nu.push_back(d.nu); o.p_nv.push_back(d.nv); o.p_link.push_back(d.link);
+    o.p_eps.push_back(f32((double)d.size_u / d.nu));
+    for (int v = 0; v < d.nv; ++v)
+      for (int u = 0; u < d.nu; ++u, ++t) {
+        double su = ((u + 0.5) / d.nu - 0.5) * (double)d.size_u;
+        double sv = ((v + 0.5) / d.nv - 0.5) * (double)d.size_v;
+        V3 x = org + su * ua + sv * va;
+        o.pos[t] = {f32(x.x), f32(x.y), f32(x.z)};
+        o.nrm[t] = {f32(n.x), f32(n.y), f32(n.z)};
+        o.radius[t] = keep ? (double)d.radius : 0.0;   // link filter -> filler
+        o.link[t] = d.link; o.patch[t] = p; o.iu[t] = u; o.iv[t] = v;
+        o.nbr[(size_t)t * 4 + 0] = (u > 0) ? t - 1 : -1;
+        o.nbr[(size_t)t * 4 + 1] = (u < d.nu - 1) ? t + 1 : -1;
+        o.nbr[(size_t)t * 4 + 2] = (v > 0) ? t - d.nu : -1;
+        o.nbr[(size_t)t * 4 + 3] = (v < d.nv - 1) ? t + d.nu : -1;
+      }
+    o.p_mstart.push_back((int)o.mpos.size());
+    o.p_mcount.push_back(d.marker_nu * d.marker_nv);
+    for (int v = 0; v < d.marker_nv; ++v)
+      for (int u = 0; u < d.marker_nu; ++u) {
+        double su = ((u + 0.5) / d.marker_nu - 0.5) * (double)d.size_u;
+        double sv = ((v + 0.5) / d.marker_nv - 0.5) * (double)d.size_v;
+        V3 x = org + su * ua + sv * va;
+        o.mpos.push_back({f32(x.x), f32(x.y), f32(x.z)});
+        o.mnrm.push_back({f32(n.x), f32(n.y), f32(n.z)});
+        o.mpatch.push_back(p);
+      }
+  }
+  o.M = (int)o.mpos.size();
+  // slots t..T-1 stay fillers with R = 0 (Q18)
+}
+
+// O5 (Eq. 4-10, D2, Q4-Q6): kinematic force / torque of one taxel, link frame.
+void kinematic_ft(const orc_params& pr, double d, V3 m_world, V3 q, V3 x_j, const M3& RL, V3 pL, V3 vL, V3 wL,
+                  V3 pO, V3 vO, V3 wO, double out[6]) {
+  for (int c = 0; c < 6; ++c) out[c] = 0.0;
+  if (!(d > 0.0)) return;                                    // Q5: every term gated on d > 0
+  V3 mbar = mulT(RL, m_world);                               // m_bar = R_L^T m
+  double s = std::pow(d, (double)pr.alpha);                  // s_j = d^alpha
+  V3 f, tau;
+  if (pr.use_velocity) {
+    V3 vC = vO + cross(wO, q - pO);                          // Eq. 4, r_C = p_O (Q4)
+    V3 vLq = vL + cross(wL, q - pL);                         // Eq. 5, r_L = p_L
+    V3 vrel = mulT(RL, vC - vLq);                            // Eq. 6
+    double vn_s = dot(vrel, mbar);
+    V3 vn = vn_s * mbar;                                     // Eq. 7
+    V3 vt = vrel - vn;
+    V3 fn = ((double)pr.k_n * s) * mbar + ((double)pr.c_n * s) * vn;  // Eq. 8 normal part
+    V3 ft = (-(double)pr.k_t) * vt;                          // Eq. 8 tangential part
+    double lim = (double)pr.mu * norm(fn);                   // D2: Coulomb cap (mu = inf -> Eq. 8)
+    double nft = norm(ft);
+    if (nft > lim) ft = (lim / nft) * ft;
+    f = fn + ft;
+    tau = cross(x_j, f) - ((double)pr.k_omega * dot(wO - wL, m_world)) * mbar;   // Eq. 9
+  } else {
+    f = ((double)pr.k_n * s) * mbar;
+    tau = cross(x_j, f);
+  }
+  out[0] = f.x; out[1] = f.y; out[2] = f.z; out[3] = tau.x; out[4] = tau.y; out[5] = tau.z;
+}
+
+// O7 (D1): bounded march along a from q through phi = min_k phi_k.
+template <class PhiFn>
+double march(PhiFn phi, double r_prox, int steps) {
+  double t = 0.0;
+  for (int i = 0; i < steps; ++i) {
+    double s = phi(t);
+    t = std::fmin(t + std::fmax(s, 0.0), r_prox);
+  }
+  return r_prox - t;
+}
+
+}  // namespace
+
+// =================================================================================
+// C interface (ctypes)
+// =================================================================================
+extern "C" {
+
+void orc_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
+
+double orc_uniform(uint32_t w) { return word_to_uniform(w); }
+
+void orc_box_muller(uint32_t wa, uint32_t wb, double* z) { box_muller(wa, wb, &z[0], &z[1]); }
+
+// One geometry query in the object frame: out = {phi, gx, gy, gz (unnormalised), face, boxgap}.
+void orc_sdf_query(int type, const double* params, const float* grid, int N, double hv, const double* x, double* out) {
+  Geom g; g.type = type; for (int i = 0; i < 4; ++i) g.p[i] = params ? params[i] : 0.0;
+  g.grid = grid; g.N = N; g.hv = hv;
+  Query q = sdf_eval(g, {x[0], x[1], x[2]});
+  out[0] = q.phi; out[1] = q.g.x; out[2] = q.g.y; out[3] = q.g.z; out[4] = q.face; out[5] = q.boxgap;
+}
+
+void* orc_create(const orc_params* prm, const orc_patch* patches, int n_patches, int n_taxels, const uint8_t* link_mask,
+                 int n_envs, const int64_t* env_ids, int n_links, int objs_per_env) {
+  int need = 0;
+  for (int p = 0; p < n_patches; ++p) need += patches[p].nu * patches[p].nv;
+  if (need > n_taxels || n_envs <= 0) return nullptr;
+  Oracle* o = new Oracle();
+  o->prm = *prm;
+  o->E = n_envs; o->L = n_links; o->K = objs_per_env;
+  o->env_id.resize(n_envs);
+  for (int e = 0; e < n_envs; ++e) o->env_id[e] = env_ids ? env_ids[e] : e;
+  build_layout(*o, patches, n_patches, n_taxels, link_mask);
+  size_t ET = (size_t)o->E * o->T;
+  o->ybit.assign(ET, 0);
+  o->hyst_a.assign(ET * 6, 0.0); o->hyst_b.assign(ET * 6, 0.0); o->drift.assign(ET * 6, 0.0);   // Q12
+  o->n_step.assign(o->E, 0); o->episode.assign(o->E, 0);
+  Geom none; none.type = G_NONE; none.grid = nullptr; none.N = 0; none.hv = 0; for (double& v : none.p) v = 0;
+  o->geom.assign((size_t)o->E * o->K, none);
+  return o;
+}
+
+void orc_destroy(void* h) { delete (Oracle*)h; }
+
+int orc_n_markers(void* h) { return ((Oracle*)h)->M; }
+
+// Copies the S0 layout out for inspection (any pointer may be NULL).
+void orc_get_layout(void* h, double* pos, double* nrm, double* radius, int32_t* link, int32_t* patch, int32_t* nbr,
+                    double* mpos, double* mnrm, int32_t* mpatch) {
+  Oracle& o = *(Oracle*)h;
+  for (int t = 0; t < o.T; ++t) {
+    if (pos) { pos[3 * t] = o.pos[t].x; pos[3 * t + 1] = o.pos[t].y; pos[3 * t + 2] = o.pos[t].z; }
+    if (nrm) { nrm[3 * t] = o.nrm[t].x; nrm[3 * t + 1] = o.nrm[t].y; nrm[3 * t + 2] = o.nrm[t].z; }
+    if (radius) radius[t] = o.radius[t];
+    if (link) link[t] = o.link[t];
+    if (patch) patch[t] = o.patch[t];
+    if (nbr) for (int a = 0; a < 4; ++a) nbr[4 * t + a] = o.nbr[(size_t)4 * t + a];
+  }
+  for (int j = 0; j < o.M; ++j) {
+    if (mpos) { mpos[3 * j] = o.mpos[j].x; mpos[3 * j + 1] = o.mpos[j].y; mpos[3 * j + 2] = o.mpos[j].z; }
+    if (mnrm) { mnrm[3 * j] = o.mnrm[j].x; mnrm[3 * j + 1] = o.mnrm[j].y; mnrm[3 * j + 2] = o.mnrm[j].z; }
+    if (mpatch) mpatch[j] = o.mpatch[j];
+  }
+}
+
+// Geometry: type[E,K], params[E,K,4] (sphere r; box hx,hy,hz; capsule r,h; grid id in params[0]),
+// bank[n_grids,N,N,N] fp32 x-fastest (copied).
+int orc_set_geometry(void* h, const int32_t* type, const float* params, int n_grids, int N, float voxel, const float* bank) {
+  Oracle& o = *(Oracle*)h;
+  o.bank_n = n_grids; o.bank_N = N; o.bank_hv = (double)voxel;
+  size_t per = (size_t)N * N * N;
+  o.bank.assign(bank, bank + per * (size_t)n_grids);
+  for (size_t i = 0; i < (size_t)o.E * o.K; ++i) {
+    Geom g; g.type = type[i]; g.grid = nullptr; g.N = N; g.hv = (double)voxel;
+    for (int a = 0; a < 4; ++a) g.p[a] = (double)params[4 * i + a];
+    if (g.type == G_GRID) {
+      int id = (int)params[4 * i];
+      if (id < 0 || id >= n_grids) return 1;
+      g.grid = o.bank.data() + per * (size_t)id;
+    }
+    o.geom[i] = g;
+  }
+  return 0;
+}
+
+// ts_reset semantics (8b): zero the state of the masked envs, restart their step count,
+// advance their episode (which re-draws the dead mask).
+void orc_reset(void* h, const uint8_t* env_mask) {
+  Oracle& o = *(Oracle*)h;
+  for (int e = 0; e < o.E; ++e) {
+    if (env_mask && !env_mask[e]) continue;
+    for (int t = 0; t < o.T; ++t) {
+      size_t i = (size_t)e * o.T + t;
+      o.ybit[i] = 0;
+      for (int c = 0; c < 6; ++c) { o.hyst_a[i * 6 + c] = 0; o.hyst_b[i * 6 + c] = 0; o.drift[i * 6 + c] = 0; }
+    }
+    o.n_step[e] = 0;
+    o.episode[e] += 1;
+  }
+}
+
+// O8 dead mask (Eq. 28, D5): stream 2, n = 0, word0 < floor(p_dead 2^32).
+static bool is_dead(const Oracle& o, int e, int t) {
+  if (!o.prm.noise_enable) return false;
+  uint32_t thr = (uint32_t)std::floor((double)o.prm.p_dead * 4294967296.0);
+  uint32_t ctr[4] = {(uint32_t)o.env_id[e], (uint32_t)t, 0u, (o.episode[e] << 4) | 2u};
+  uint32_t key[2] = {o.prm.seed_lo, o.prm.seed_hi};
+  uint32_t w[4];
+  philox4x32_10(ctr, key, w);
+  return w[0] < thr;
+}
+
+// One step of the whole path.  Inputs fp32 [E,L,*] / [E,K,*]; outputs double (NULL = skip).
+// aux (all optional): aux_phi[E,T] = min_k phi_k(q_j); aux_face[E,T] = voxel-face distance of the
+// winner if it is a grid (else +inf); aux_boxgap[E,T]; aux_asym[E,T,6] = |x|-|y_prev| where the
+// signs of x and y_prev differ (else +inf) -- used only for the comparator's band accounting.
+void orc_step(void* h, const float* link_pos, const float* link_quat, const float* link_linvel, const float* link_angvel,
+              const float* obj_pos, const float* obj_quat, const float* obj_linvel, const float* obj_angvel,
+              uint8_t* contact, double* depth, double* ft, double* marker, double* prox, double* ft_noisy, uint8_t* dead,
+              double* aux_phi, double* aux_face, double* aux_boxgap, double* aux_asym, int n_threads) {
+  Oracle& o = *(Oracle*)h;
+  const orc_params& pr = o.prm;
+  const int T = o.T, L = o.L, K = o.K, M = o.M;
+  (void)n_threads;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 1) num_threads(n_threads > 0 ? n_threads : 1)
+#endif
+  for (int e = 0; e < o.E; ++e) {
+    std::vector<double> phi_min(T), dep(T), ftc((size_t)T * 6), hcl((size_t)T * 6);
+    std::vector<uint8_t> deadv(T, 0);
+    for (int j = 0; j < T; ++j) {
+      size_t ej = (size_t)e * T + j;
+      bool active = o.radius[j] > 0.0;                       // R_j = 0 -> filler
+      int l = o.link[j];
+      const float* lp = link_pos + ((size_t)e * L + l) * 3;
+      M3 RL = quat_to_R(link_quat + ((size_t)e * L + l) * 4);
+      V3 pL = ld3(lp);
+      V3 q = pL + mul(RL, o.pos[j]);                         // Eq. 1
+      V3 a = mul(RL, o.nrm[j]);
+      // O2/O3: query all K objects, winner = max_k [R - phi_k]_+, ties -> lowest k
+      double best_phi = INFINITY; int kstar = -1; Query qstar{}; M3 RO_star{};
+      for (int k = 0; k < K; ++k) {
+        const Geom& g = o.geom[(size_t)e * K + k];
+        if (g.type == G_NONE) continue;
+        V3 pO = ld3(obj_pos + ((size_t)e * K + k) * 3);
+        M3 RO = quat_to_R(obj_quat + ((size_t)e * K + k) * 4);
+        V3 xo = mulT(RO, q - pO);
+        Query r = sdf_eval(g, xo);
+        if (r.phi < best_phi) { best_phi = r.phi; kstar = k; qstar = r; RO_star = RO; }
+      }
+      phi_min[j] = best_phi;
+      double d = (active && kstar >= 0) ? std::fmax(0.0, o.radius[j] - best_phi) : 0.0;   // Eq. 2
+      dep[j] = d;
+      if (aux_phi) aux_phi[ej] = best_phi;
+      if (aux_face) aux_face[ej] = kstar >= 0 ? qstar.face : INFINITY;
+      if (aux_boxgap) aux_boxgap[ej] = kstar >= 0 ? qstar.boxgap : INFINITY;
+      // O4 (Eq. 3): Schmitt trigger, strict >
+      uint8_t y = 0;
+      if (active) y = (d > (double)pr.eta_on) || (o.ybit[ej] == 1 && d > (double)pr.eta_off);
+      o.ybit[ej] = y;
+      deadv[j] = active && is_dead(o, e, j);
+      if (contact) contact[ej] = deadv[j] ? 0 : y;
+      if (dead) dead[ej] = deadv[j];
+      if (depth) depth[ej] = d;
+      // O5
+      double f6[6] = {0, 0, 0, 0, 0, 0};
+      if (active && d > 0.0) {
+        double gn = norm(qstar.g);
+        V3 m = (gn < 1e-12) ? (-1.0) * a : (1.0 / gn) * mul(RO_star, qstar.g);   // Q2
+        V3 pO = ld3(obj_pos + ((size_t)e * K + kstar) * 3);
+        kinematic_ft(pr, d, m, q, o.pos[j], RL, pL, ld3(link_linvel + ((size_t)e * L + l) * 3),
+                     ld3(link_angvel + ((size_t)e * L + l) * 3), pO, ld3(obj_linvel + ((size_t)e * K + kstar) * 3),
+                     ld3(obj_angvel + ((size_t)e * K + kstar) * 3), f6);
+      }
+      for (int c = 0; c < 6; ++c) { ftc[(size_t)j * 6 + c] = f6[c]; if (ft) ft[ej * 6 + c] = f6[c]; }
+      // O7
+      if (prox) {
+        double P = 0.0;
+        if (active) {
+          auto phi_at = [&](double t) {
+            double best = INFINITY;
+            V3 x = q + t * a;
+            for (int k = 0; k < K; ++k) {
+              const Geom& g = o.geom[(size_t)e * K + k];
+              if (g.type == G_NONE) continue;
+              V3 pO = ld3(obj_pos + ((size_t)e * K + k) * 3);
+              M3 RO = quat_to_R(obj_quat + ((size_t)e * K + k) * 4);
+              best = std::fmin(best, sdf_eval(g, mulT(RO, x - pO)).phi);
+            }
+            return best;
+          };
+          P = march(phi_at, (double)pr.r_prox, pr.march_steps);
+        }
+        prox[ej] = P;
+      }
+    }
+    // O6 (Eq. 18-21, 23 first sum; Q15-Q17): dilation of each patch's markers by its active taxels
+    if (marker) {
+      double lam = (double)pr.lambda_d, cE = (double)pr.c_e;
+      double gbar = std::exp(-0.5) / std::sqrt(2.0 * lam);
+      for (int jm = 0; jm < M; ++jm) {
+        int p = o.mpatch[jm];
+        double eps = o.p_eps[p], rhobar = 1.0 / (2.0 * eps);
+        V3 u = {0, 0, 0};
+        V3 nj = o.mnrm[jm];
+        int n = o.p_nu[p] * o.p_nv[p];
+        for (int i = o.p_start[p]; i < o.p_start[p] + n; ++i) {
+          if (!(o.radius[i] > 0.0)) continue;
+          double hi = std::fmax(0.0, -phi_min[i]);                       // Eq. 19
+          V3 z = o.mpos[jm] - o.pos[i];
+          V3 r = z - dot(z, nj) * nj;                                   // Eq. 18
+          double r2 = dot(r, r);
+          double g = std::exp(-lam * r2);
+          double rho = 1.0 / (r2 + eps * eps);
+          double w = hi * (cE * g / gbar + (1.0 - cE) * rho / rhobar);   // Eq. 20
+          double bulge = (hi > 0.0) ? std::pow(hi, (double)pr.alpha_e) * g : 0.0;
+          u = u + (double)pr.s_d * (w * r + bulge * nj);                 // Eq. 21
+        }
+        size_t o3 = ((size_t)e * M + jm) * 3;
+        marker[o3] = u.x; marker[o3 + 1] = u.y; marker[o3 + 2] = u.z;
+      }
+    }
+    // O8: hysteresis -> crosstalk -> drift -> dead
+    if (pr.noise_enable) {
+      uint32_t n = o.n_step[e];
+      double decay = std::exp(-(double)pr.dt / (double)pr.tau);
+      for (int j = 0; j < T; ++j) {
+        size_t ej = (size_t)e * T + j;
+        for (int c = 0; c < 6; ++c) {
+          double x = ftc[(size_t)j * 6 + c], hval = x;
+          if (aux_asym) aux_asym[ej * 6 + c] = INFINITY;
+          if (o.radius[j] > 0.0) {
+            if (pr.hyst_mode == 1) {                                      // Eq. 29-30
+              double xi = decay * o.hyst_a[ej * 6 + c] + (x - o.hyst_b[ej * 6 + c]);
+              o.hyst_a[ej * 6 + c] = xi; o.hyst_b[ej * 6 + c] = x;
+              hval = x + (double)pr.beta * xi;
+            } else if (pr.hyst_mode == 2) {                               // D3, Q14
+              double yp = o.hyst_a[ej * 6 + c];
+              if (aux_asym && x * yp < 0.0) aux_asym[ej * 6 + c] = std::fabs(x) - std::fabs(yp);
+              double al = (std::fabs(x) > std::fabs(yp)) ? (double)pr.alpha_load : (double)pr.alpha_unload;
+              double y = yp + al * (x - yp);
+              o.hyst_a[ej * 6 + c] = y;
+              hval = y;
+            }
+          }
+          hcl[(size_t)j * 6 + c] = hval;
+        }
+      }
+      for (int j = 0; j < T; ++j) {
+        size_t ej = (size_t)e * T + j;
+        bool active = o.radius[j] > 0.0;
+        // draws: stream 0 -> channels 0-3, stream 1 words 0-1 -> channels 4-5
+        double z[6] = {0, 0, 0, 0, 0, 0};
+        if (active) {
+          uint32_t key[2] = {pr.seed_lo, pr.seed_hi}, w0[4], w1[4];
+          uint32_t c0[4] = {(uint32_t)o.env_id[e], (uint32_t)j, n, (o.episode[e] << 4) | 0u};
+          uint32_t c1[4] = {(uint32_t)o.env_id[e], (uint32_t)j, n, (o.episode[e] << 4) | 1u};
+          philox4x32_10(c0, key, w0);
+          philox4x32_10(c1, key, w1);
+          box_muller(w0[0], w0[1], &z[0], &z[1]);
+          box_muller(w0[2], w0[3], &z[2], &z[3]);
+          box_muller(w1[0], w1[1], &z[4], &z[5]);
+        }
+        for (int c = 0; c < 6; ++c) {
+          double out = 0.0;
+          if (active) {
+            double hj = hcl[(size_t)j * 6 + c];
+            double acc = 0.0;                                             // D4, Q11
+            for (int a = 0; a < 4; ++a) {
+              int k = o.nbr[(size_t)j * 4 + a];
+              if (k >= 0 && o.radius[k] > 0.0) acc += hcl[(size_t)k * 6 + c] - hj;
+            }
+            double cj = hj + ((double)pr.chi / 4.0) * acc;
+            double sig = (c < 3) ? (double)pr.sigma_rw_force : (double)pr.sigma_rw_torque;
+            double D = o.drift[ej * 6 + c] + sig * z[c];                  // Eq. 25 drift
+            o.drift[ej * 6 + c] = D;
+            out = deadv[j] ? 0.0 : cj + D;                                // Eq. 28, D5
+          }
+          if (ft_noisy) ft_noisy[ej * 6 + c] = out;
+        }
+      }
+    }
+    o.n_step[e] += 1;
+  }
+}
+
+// Stand-alone pieces for the pins -------------------------------------------------
+
+// O5 on explicit arguments (all double[3] except quat float[4]); out[6].
+void orc_kinematic_ft(const orc_params* pr, double d, const double* m_world, const double* x_j, const float* quat_L,
+                      const double* pL, const double* vL, const double* wL, const double* pO, const double* vO,
+                      const double* wO, double* out) {
+  M3 RL = quat_to_R(quat_L);
+  V3 xj = {x_j[0], x_j[1], x_j[2]};
+  V3 pl = {pL[0], pL[1], pL[2]};
+  V3 q = pl + mul(RL, xj);
+  kinematic_ft(*pr, d, {m_world[0], m_world[1], m_world[2]}, q, xj, RL, pl, {vL[0], vL[1], vL[2]}, {wL[0], wL[1], wL[2]},
+               {pO[0], pO[1], pO[2]}, {vO[0], vO[1], vO[2]}, {wO[0], wO[1], wO[2]}, out);
+}
+
+// O7 on one geometry in its own frame: start x0, direction a (object frame).
+double orc_march(int type, const double* params, const float* grid, int N, double hv, const double* x0, const double* a,
+                 double r_prox, int steps) {
+  Geom g; g.type = type; for (int i = 0; i < 4; ++i) g.p[i] = params ? params[i] : 0.0;
+  g.grid = grid; g.N = N; g.hv = hv;
+  V3 x = {x0[0], x0[1], x0[2]}, d = {a[0], a[1], a[2]};
+  return march([&](double t) { return sdf_eval(g, x + t * d).phi; }, r_prox, steps);
+}
+
+int orc_max_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"
