@@ -654,7 +654,7 @@ def test_transform_eq1():
     assert out["depth"][0, 0] == pytest.approx(0.0005, abs=3e-9)
     assert out["prox"][0, 0] == pytest.approx(0.020 - 0.0015, abs=3e-9)
     f = out["ft"][0, 0]
-    assert f[2] < 0 and abs(f[0]) < 1e-9 and abs(f[1]) < 1e-9
+    assert f[2] < 0 and abs(f[0]) < 1e-7 and abs(f[1]) < 1e-7     # quaternion is fp32
     np.testing.assert_allclose(f[3:], np.cross([0.01, 0, 0], f[:3]), atol=1e-12)   # lever arm is x_j (link frame)
     # the wrong rotation sense would put the taxel at (0,-0.01,0): no contact there
     out = o.step(inputs(link_pos=pL, link_quat=(s, 0, 0, s), obj_pos=pL + [0, -0.01, 0.0065]))
