@@ -1,0 +1,232 @@
+/* ts.h -- C ABI of the B200-native batched tactile readout (after Tactile Genesis,
+ * arxiv/paper_2606_22332; "P:NNN" = line NNN of the paper text, App. A = P:172-359).
+ *
+ * One context (ts_ctx) serves E environments x T taxel slots on ONE CUDA device.  Each
+ * ts_step() runs, for every (environment, taxel):
+ *   Eq. 1      q_j = p_L + R_L x_j,  a_j = R_L n_j
+ *   Eq. 2      d_j = max_g [R_j - phi_g(q_j)]_+ , normal m_j = grad phi_g*
+ *   Eq. 3      Schmitt-trigger contact bit
+ *   Eq. 4-9  kinematic force / torque (+ Coulomb cap, D2)
+ *   Eq. 18-21, 23  elastomer marker dilation
+ *   bounded SDF march along a_j (D1; output form of Eq. 12)
+ *   App. A.8 noise: hysteresis (Eq. 29-30) -> crosstalk (Eq. 31) -> random-walk
+ *                        drift (Eq. 25) -> dead taxels (Eq. 28)
+ * All device work is hand-written CUDA for sm_100a; there is no CPU fallback.
+ *
+ * Conventions: SI units; quaternions (w,x,y,z), used as given (never renormalised); each
+ * environment has its own world frame; force/torque and marker outputs are expressed in the
+ * sensor-link frame.  All arrays are dense, row-major, fp32 unless stated.
+ *
+ * Threading: calls on one ctx are not thread-safe.  Streams: every device operation of
+ * ts_set_geometry / ts_step / ts_reset is enqueued on the caller's stream (a cudaStream_t
+ * passed as void*; NULL = the legacy default stream); none of them synchronises except where
+ * stated.  Errors: every call returns a ts_status; nothing throws, aborts or prints.
+ */
+#ifndef TS_H_
+#define TS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ts_ctx ts_ctx;       /* opaque; owned by the library */
+typedef struct ts_layout ts_layout; /* opaque host object: the taxel-layout builder (S0) */
+
+typedef enum ts_status {
+  TS_OK = 0,
+  TS_ERR_INVALID_ARG = 1, /* NULL pointer, size out of range, inconsistent layout, ... */
+  TS_ERR_CUDA = 2,        /* a CUDA runtime call or a kernel launch failed; see ts_last_error */
+  TS_ERR_OOM = 3,         /* host or device allocation failed */
+  TS_ERR_STATE = 4,       /* call order violated (e.g. ts_step before ts_set_geometry) */
+  TS_ERR_UNSUPPORTED = 5  /* device is not sm_100 or a requested mode is not built */
+} ts_status;
+
+/* ---------------------------------------------------------------------------------------
+ * S0 -- taxel-layout builder (host).  P:178 (probe = link-frame position, unit normal,
+ * radius), P:182 (R_j = 0 filler slots keep batched tensors regular), P:72 / P:234 (regular
+ * planar grids), P:510 (placement subsets = link filters).
+ *
+ * A patch is a regular nu x nv cell-centred grid of taxels on one link:
+ *   x(iu,iv) = origin + ((iu+.5)/nu - .5) size_u u_axis + ((iv+.5)/nv - .5) size_v v_axis,
+ *   n = u_axis x v_axis,  slot index = patch_start + iv*nu + iu  (u fastest),
+ * plus an optional marker_nu x marker_nv grid of elastomer markers placed the same way
+ * (marker_nu = 0: none; markers = taxels reproduces the paper's (N,3) output, Q16).
+ * Limits: nu*nv <= 64 and marker_nu*marker_nv <= 64 per patch (one warp owns a patch).
+ * u_axis, v_axis must be unit and orthogonal to 1e-3.
+ * ------------------------------------------------------------------------------------- */
+typedef struct ts_patch_desc {
+  int32_t link;       /* sensor link index, 0 <= link < n_links */
+  float origin[3];    /* patch centre, link frame [m] */
+  float u_axis[3];
+  float v_axis[3];
+  float size_u, size_v; /* patch extent [m] */
+  int32_t nu, nv;
+  float radius;       /* probe radius R_j > 0 [m] */
+  int32_t marker_nu, marker_nv;
+} ts_patch_desc;
+
+/* Read-only view of a finalised layout (host pointers owned by the layout). */
+typedef struct ts_layout_view {
+  int32_t n_taxels, n_patches, n_markers;
+  const float* pos;       /* [T,3] link-frame positions */
+  const float* nrm;       /* [T,3] link-frame unit normals */
+  const float* radius;    /* [T]   0 = inactive filler */
+  const int32_t* link;    /* [T] */
+  const int32_t* patch;   /* [T]   -1 for trailing fillers */
+  const int32_t* nbr;     /* [T,4] in-patch neighbours (-u,+u,-v,+v), -1 = none */
+  const int32_t* patch_start; /* [P] */
+  const int32_t* patch_nu;    /* [P] */
+  const int32_t* patch_nv;    /* [P] */
+  const int32_t* patch_link;  /* [P] */
+  const int32_t* marker_start; /* [P] */
+  const int32_t* marker_count; /* [P] */
+  const float* marker_pos; /* [M,3] */
+  const float* marker_nrm; /* [M,3] */
+  const int32_t* marker_patch; /* [M] */
+} ts_layout_view;
+
+ts_status ts_layout_create(ts_layout** out);
+/* Appends a patch; its taxels take the next nu*nv slots.  TS_ERR_INVALID_ARG on bad sizes/axes. */
+ts_status ts_layout_add_patch(ts_layout* lay, const ts_patch_desc* desc);
+/* Link filter: taxels (and markers' sources) on links whose mask byte is 0 become fillers
+ * (radius 0).  link_mask has n_links entries.  May be called before or after finalize. */
+ts_status ts_layout_filter_links(ts_layout* lay, const uint8_t* link_mask, int32_t n_links);
+/* Pads with trailing filler slots up to n_taxels (>= slots used) and builds the adjacency. */
+ts_status ts_layout_finalize(ts_layout* lay, int32_t n_taxels);
+ts_status ts_layout_get(const ts_layout* lay, ts_layout_view* out);
+ts_status ts_layout_destroy(ts_layout* lay); /* NULL is a no-op */
+
+/* ---------------------------------------------------------------------------------------
+ * Configuration (host POD, copied by ts_create).
+ * ------------------------------------------------------------------------------------- */
+enum { TS_HYST_OFF = 0, TS_HYST_MAXWELL = 1 /* Eq. 29-30 */, TS_HYST_ASYM = 2 /* DESIGN.md D3 */ };
+
+enum {                      /* output_mask bits; a bit set with a NULL pointer is an error */
+  TS_OUT_CONTACT = 1 << 0,  /* Eq. 3   uint8 [E,T] */
+  TS_OUT_DEPTH = 1 << 1,    /* Eq. 2   f32   [E,T] */
+  TS_OUT_FT = 1 << 2,       /* Eq. 8-9 f32   [E,T,6] (f_x,f_y,f_z,tau_x,tau_y,tau_z), link frame */
+  TS_OUT_MARKER = 1 << 3,   /* Eq. 21  f32   [E,M,3] link frame */
+  TS_OUT_PROX = 1 << 4,     /* march   f32   [E,T]  P_j = r_prox - t */
+  TS_OUT_FT_NOISY = 1 << 5, /* A.8     f32   [E,T,6]; needs noise_enable */
+  TS_OUT_DEAD = 1 << 6      /* Eq. 28  uint8 [E,T];   needs noise_enable */
+};
+
+typedef struct ts_config {
+  int32_t n_envs;        /* E >= 1 */
+  int32_t n_links;       /* L >= 1 */
+  int32_t objs_per_env;  /* K >= 1 */
+  int64_t env_id_base;   /* global id of env 0 (Philox counters use env_id_base + e; multi-GPU sharding) */
+  const ts_layout* layout; /* finalised; copied to the device, may be destroyed afterwards */
+  /* KinematicTaxel, Eq. 10: k_n=500 c_n=1 alpha=1.2 k_t=2 k_omega=2; mu = Coulomb cap
+   * (INFINITY reproduces Eq. 8 exactly); use_velocity = 0 drops the velocity terms. */
+  float k_n, c_n, alpha, k_t, k_omega, mu;
+  int32_t use_velocity;
+  float eta_on, eta_off; /* Eq. 3 thresholds, eta_off <= eta_on (5e-4 / 2e-4) */
+  /* ElastomerTaxel dilation: s_d=100 lambda_d=8000 alpha_e=1.2 c_e=1 */
+  float s_d, lambda_d, alpha_e, c_e;
+  float r_prox;          /* march range [m] */
+  int32_t march_steps;   /* 0..64 SDF evaluations per taxel */
+  float dt;              /* physics step [s] (0.005) */
+  /* noise model (App. A.8) */
+  int32_t noise_enable;
+  uint64_t seed;         /* Philox4x32-10 key */
+  float sigma_rw_force, sigma_rw_torque; /* Eq. 25 random-walk sigma per step, channels 0-2 / 3-5 */
+  int32_t hyst_mode;     /* TS_HYST_* */
+  float beta, tau;       /* Maxwell (Table 12: 0.5, 0.05 s) */
+  float alpha_load, alpha_unload; /* asymmetric first-order */
+  float p_dead;          /* Eq. 28 Bernoulli probability, 0 <= p < 1 */
+  float chi;             /* Eq. 31 crosstalk strength (4-neighbour kernel, D4) */
+  uint32_t output_mask;  /* TS_OUT_* the ctx will be asked for (upper bound per step) */
+} ts_config;
+
+/* Fills *cfg with the paper's constants and everything else zero / off. */
+void ts_config_default(ts_config* cfg);
+
+/* ---------------------------------------------------------------------------------------
+ * Geometry (per-geometry SDFs).  Arrays are HOST pointers, read before the call
+ * returns (the uploads are enqueued on `stream` from a staging copy the ctx owns).
+ * ------------------------------------------------------------------------------------- */
+enum { TS_GEOM_NONE = 0, TS_GEOM_SPHERE = 1, TS_GEOM_BOX = 2, TS_GEOM_CAPSULE = 3, TS_GEOM_SDF = 4 };
+
+typedef struct ts_geometry {
+  const int32_t* type;  /* [E,K] TS_GEOM_* */
+  const float* params;  /* [E,K,4] sphere: r | box: half-extents hx,hy,hz | capsule: r, half-length
+                           (axis = local z) | SDF: grid id in params[0] */
+  int32_t n_grids;      /* G >= 0 */
+  int32_t grid_n;       /* N: nodes per axis, 2 <= N <= 512 (all grids alike) */
+  float voxel;          /* h_v [m]; node i sits at (i - (N-1)/2) h_v on each axis */
+  const float* grids;   /* [G,N,N,N] fp32 signed distance, x fastest: index (k*N + j)*N + i */
+} ts_geometry;
+
+/* Per-step inputs: DEVICE pointers, caller-owned, read-only.  Velocities are those of the
+ * frame origin, in world axes (Eq. 4-5 with r_C, r_L = frame origins, Q4). */
+typedef struct ts_step_in {
+  const float* link_pos;    /* [E,L,3] */
+  const float* link_quat;   /* [E,L,4] */
+  const float* link_linvel; /* [E,L,3] */
+  const float* link_angvel; /* [E,L,3] */
+  const float* obj_pos;     /* [E,K,3] */
+  const float* obj_quat;    /* [E,K,4] */
+  const float* obj_linvel;  /* [E,K,3] */
+  const float* obj_angvel;  /* [E,K,3] */
+} ts_step_in;
+
+/* Per-step outputs: DEVICE pointers, caller-owned, fully overwritten.  NULL = not produced.
+ * Requirements: 16-byte aligned base pointers (torch / cudaMalloc allocations are). */
+typedef struct ts_step_out {
+  uint8_t* contact; /* [E,T]   */
+  float* depth;     /* [E,T]   */
+  float* ft;        /* [E,T,6] */
+  float* marker;    /* [E,M,3] */
+  float* prox;      /* [E,T]   */
+  float* ft_noisy;  /* [E,T,6] */
+  uint8_t* dead;    /* [E,T]   */
+} ts_step_out;
+
+/* Creates a context on `cuda_device` (must be sm_100).  Allocates every device buffer the
+ * path needs (layout copy, state: Schmitt bit + dead flag 1 B, hysteresis 24/48 B, drift 24 B
+ * per taxel slot); nothing is allocated later except the geometry bank in ts_set_geometry. */
+ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out);
+
+/* Uploads object descriptors and the SDF bank (re-tiled into the internal gather layout by a
+ * kernel on `stream`).  May be called again to replace the geometry.  Synchronises `stream`
+ * once before returning, so host arrays may be freed immediately. */
+ts_status ts_set_geometry(ts_ctx* ctx, const ts_geometry* geo, void* stream);
+
+/* One pass of the whole hot path over all envs.  Asynchronous; never allocates. */
+ts_status ts_step(ts_ctx* ctx, const ts_step_in* in, const ts_step_out* out, void* stream);
+
+/* The same step on HOST buffers (pinned memory recommended): copies the eight inputs to
+ * ctx-owned device staging, runs ts_step, and copies every non-NULL output back, all enqueued
+ * on `stream` in that order.  Host buffers must stay valid until the stream reaches the end
+ * of the call.  The staging (inputs + requested outputs) is allocated on the first call. */
+ts_status ts_step_host(ts_ctx* ctx, const ts_step_in* host_in, const ts_step_out* host_out, void* stream);
+
+/* Zeroes drift / hysteresis / contact state and the step count of the masked envs
+ * (env_mask: DEVICE uint8 [E], NULL = all) and advances their episode, which re-draws the
+ * dead-taxel mask.  Asynchronous. */
+ts_status ts_reset(ts_ctx* ctx, const uint8_t* env_mask_dev, void* stream);
+
+ts_status ts_destroy(ts_ctx* ctx); /* NULL is a no-op returning TS_OK */
+
+/* Last error text of this ctx (or of the last failed ts_create when ctx is NULL).  Never NULL. */
+const char* ts_last_error(const ts_ctx* ctx);
+
+/* Introspection used by the binding and the bench. */
+int32_t ts_n_taxels(const ts_ctx* ctx);
+int32_t ts_n_markers(const ts_ctx* ctx);
+/* Number of kernel launches one ts_step enqueues with the ctx's current configuration. */
+int32_t ts_launches_per_step(const ts_ctx* ctx);
+/* Records CUDA events around the main kernel of every subsequent ts_step (on the step's own
+ * stream) and returns the mean duration in ms of the steps since the last call (after
+ * synchronising those events).  enable = 0 switches recording off.  *n_steps gets the count. */
+ts_status ts_kernel_time_ms(ts_ctx* ctx, int32_t enable, float* mean_ms, int32_t* n_steps);
+
+const char* ts_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TS_H_ */

@@ -1,0 +1,390 @@
+// C ABI of include/ts.h: context, validation, uploads, launches.  No compute happens here.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "ts_internal.h"
+
+struct ts_ctx {
+  int device = 0;
+  ts_config cfg{};
+  int T = 0, P = 0, M = 0, nh = 0;
+  bool have_geometry = false;
+  uint32_t gstep = 0;
+  uint32_t dead_thr = 0;
+  // device buffers
+  float4 *tx_pos = nullptr, *tx_nrm = nullptr, *mk_pos = nullptr, *mk_nrm = nullptr;
+  TsPatch* patches = nullptr;
+  int32_t* g_type = nullptr;
+  float4* g_params = nullptr;
+  float4* bank = nullptr;
+  size_t bank_bytes = 0;
+  int grid_n = 2, n_grids = 0;
+  float voxel = 1.f;
+  uint8_t* st_flags = nullptr;
+  float4 *st_hyst = nullptr, *st_drift = nullptr;
+  uint32_t *reset_step = nullptr, *episode = nullptr;
+  // device staging of ts_step_host
+  float* stage_in[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  void* stage_out[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  // timing of the main kernel
+  bool timing = false;
+  std::vector<cudaEvent_t> ev;  // pairs
+  size_t ev_used = 0;
+  std::string err;
+};
+
+namespace {
+thread_local std::string g_create_err;
+
+ts_status fail(ts_ctx* c, ts_status s, const std::string& msg) {
+  if (c) c->err = msg; else g_create_err = msg;
+  return s;
+}
+ts_status cuda_fail(ts_ctx* c, cudaError_t e, const char* what) {
+  return fail(c, e == cudaErrorMemoryAllocation ? TS_ERR_OOM : TS_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define TS_CUDA(ctx, call)                                   \
+  do {                                                       \
+    cudaError_t e_ = (call);                                 \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); \
+  } while (0)
+
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+void free_all(ts_ctx* c) {
+  cudaFree(c->tx_pos); cudaFree(c->tx_nrm); cudaFree(c->mk_pos); cudaFree(c->mk_nrm); cudaFree(c->patches);
+  cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->bank); cudaFree(c->st_flags); cudaFree(c->st_hyst);
+  cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode);
+  for (float* q : c->stage_in) cudaFree(q);
+  for (void* q : c->stage_out) cudaFree(q);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+}
+
+void fill_params(const ts_ctx* c, TsStepParams& p) {
+  const ts_config& g = c->cfg;
+  std::memset(&p, 0, sizeof(p));
+  p.E = g.n_envs; p.L = g.n_links; p.K = g.objs_per_env; p.T = c->T; p.P = c->P; p.M = c->M;
+  p.env_id_base = (uint32_t)g.env_id_base;
+  p.tx_pos = c->tx_pos; p.tx_nrm = c->tx_nrm; p.patches = c->patches; p.mk_pos = c->mk_pos; p.mk_nrm = c->mk_nrm;
+  p.g_type = c->g_type; p.g_params = c->g_params; p.bank = c->bank;
+  p.grid_n = c->grid_n; p.voxel = c->voxel; p.inv_voxel = 1.0f / c->voxel;
+  p.grid_origin = -0.5f * (c->grid_n - 1) * c->voxel;
+  p.grid_stride = ts_bank_elems_per_grid(c->grid_n);
+  p.st_flags = c->st_flags; p.st_hyst = c->st_hyst; p.st_drift = c->st_drift;
+  p.reset_step = c->reset_step; p.episode = c->episode; p.gstep = c->gstep;
+  p.k_n = g.k_n; p.c_n = g.c_n; p.alpha = g.alpha; p.k_t = g.k_t; p.k_omega = g.k_omega; p.mu = g.mu;
+  p.eta_on = g.eta_on; p.eta_off = g.eta_off; p.use_velocity = g.use_velocity;
+  p.s_d = g.s_d; p.lambda_d = g.lambda_d; p.alpha_e = g.alpha_e; p.c_e = g.c_e;
+  // 1 / g_bar, g_bar = e^{-1/2} / sqrt(2 lambda_d)
+  p.inv_gbar = (float)(std::sqrt(2.0 * (double)g.lambda_d) / std::exp(-0.5));
+  p.r_prox = g.r_prox; p.march_steps = g.march_steps;
+  p.noise_enable = g.noise_enable; p.hyst_mode = g.noise_enable ? g.hyst_mode : TS_HYST_OFF;
+  p.seed_lo = (uint32_t)(g.seed & 0xffffffffu); p.seed_hi = (uint32_t)(g.seed >> 32);
+  p.sigma_f = g.sigma_rw_force; p.sigma_t = g.sigma_rw_torque; p.beta = g.beta;
+  p.decay = (g.tau > 0.f) ? (float)std::exp(-(double)g.dt / (double)g.tau) : 0.f;   // Eq. 29
+  p.alpha_load = g.alpha_load; p.alpha_unload = g.alpha_unload; p.chi = g.chi;
+}
+}  // namespace
+
+extern "C" {
+
+const char* ts_version(void) { return "ts 0.1 (sm_100a)"; }
+
+void ts_config_default(ts_config* c) {
+  if (!c) return;
+  std::memset(c, 0, sizeof(*c));
+  c->n_envs = 1; c->n_links = 1; c->objs_per_env = 1;
+  c->k_n = 500.f; c->c_n = 1.f; c->alpha = 1.2f; c->k_t = 2.f; c->k_omega = 2.f;  // Eq. 10
+  c->mu = 1.0f;                                                                    // D2
+  c->use_velocity = 1;
+  c->eta_on = 5e-4f; c->eta_off = 5e-4f;
+  c->s_d = 100.f; c->lambda_d = 8000.f; c->alpha_e = 1.2f; c->c_e = 1.f;
+  c->r_prox = 0.020f; c->march_steps = 16;                                         // D1
+  c->dt = 0.005f;
+  c->tau = 0.05f; c->beta = 0.5f; c->alpha_load = 1.f; c->alpha_unload = 1.f;
+  c->output_mask = TS_OUT_CONTACT | TS_OUT_DEPTH | TS_OUT_FT | TS_OUT_MARKER | TS_OUT_PROX;
+}
+
+const char* ts_last_error(const ts_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+int32_t ts_n_taxels(const ts_ctx* ctx) { return ctx ? ctx->T : 0; }
+int32_t ts_n_markers(const ts_ctx* ctx) { return ctx ? ctx->M : 0; }
+int32_t ts_launches_per_step(const ts_ctx* ctx) { return ctx ? 1 : 0; }
+
+ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
+  if (!cfg || !out) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: NULL argument");
+  *out = nullptr;
+  const ts_layout* lay = cfg->layout;
+  if (!lay || !lay->finalized) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: layout missing or not finalised");
+  if (cfg->n_envs < 1 || cfg->n_links < 1 || cfg->objs_per_env < 1)
+    return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: n_envs, n_links, objs_per_env must be >= 1");
+  if (!(cfg->eta_off <= cfg->eta_on)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: eta_off > eta_on");
+  if (cfg->march_steps < 0 || cfg->march_steps > 64) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: march_steps not in 0..64");
+  if (!(cfg->alpha > 0.f) || !(cfg->r_prox >= 0.f) || !(cfg->lambda_d > 0.f) || !(cfg->c_e >= 0.f && cfg->c_e <= 1.f))
+    return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: physics parameter out of range");
+  if (cfg->noise_enable) {
+    if (cfg->hyst_mode < TS_HYST_OFF || cfg->hyst_mode > TS_HYST_ASYM) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: hyst_mode");
+    if (!(cfg->p_dead >= 0.f && cfg->p_dead < 1.f)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: p_dead not in [0,1)");
+    if (cfg->hyst_mode == TS_HYST_MAXWELL && !(cfg->tau > 0.f)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: tau <= 0");
+  } else if (cfg->output_mask & (TS_OUT_FT_NOISY | TS_OUT_DEAD)) {
+    return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: ft_noisy / dead need noise_enable");
+  }
+  for (size_t t = 0; t < lay->link.size(); ++t)
+    if (lay->link[t] >= cfg->n_links) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: layout link index >= n_links");
+  if ((long long)cfg->n_envs * lay->n_taxels > (1LL << 40)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: too large");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev)
+    return fail(nullptr, TS_ERR_CUDA, "ts_create: no such CUDA device");
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) return fail(nullptr, TS_ERR_CUDA, "ts_create: cudaGetDeviceProperties");
+  if (prop.major != 10) return fail(nullptr, TS_ERR_UNSUPPORTED, "ts_create: kernels are built for sm_100a only");
+
+  ts_ctx* c = new (std::nothrow) ts_ctx();
+  if (!c) return fail(nullptr, TS_ERR_OOM, "ts_create: host allocation");
+  c->device = cuda_device;
+  c->cfg = *cfg;
+  c->cfg.layout = nullptr;
+  DeviceGuard guard(cuda_device);
+
+  // ---- layout -> device records; trailing filler slots are covered by filler patches ----
+  const int T = lay->n_taxels;
+  std::vector<float4> pos(T), nrm(T);
+  for (int t = 0; t < T; ++t) {
+    pos[t] = make_float4(lay->pos[3 * t], lay->pos[3 * t + 1], lay->pos[3 * t + 2], lay->radius[t]);
+    nrm[t] = make_float4(lay->nrm[3 * t], lay->nrm[3 * t + 1], lay->nrm[3 * t + 2], 0.f);
+  }
+  std::vector<TsPatch> pts;
+  int used = 0;
+  for (size_t p = 0; p < lay->patch_start.size(); ++p) {
+    TsPatch q{};
+    q.start = lay->patch_start[p]; q.nu = lay->patch_nu[p]; q.n = lay->patch_nu[p] * lay->patch_nv[p];
+    q.link = lay->patch_link[p]; q.mstart = lay->marker_start[p]; q.mcount = lay->marker_count[p];
+    q.eps = lay->patch_eps[p];
+    pts.push_back(q);
+    used = q.start + q.n;
+  }
+  for (int t = used; t < T; t += TS_MAX_PATCH_TAXELS) {
+    TsPatch q{};
+    q.start = t; q.n = (T - t < TS_MAX_PATCH_TAXELS) ? T - t : TS_MAX_PATCH_TAXELS; q.nu = q.n; q.link = -1;
+    pts.push_back(q);
+  }
+  const int M = (int)lay->marker_patch.size();
+  std::vector<float4> mpos(M > 0 ? M : 1), mnrm(M > 0 ? M : 1);
+  for (int j = 0; j < M; ++j) {
+    mpos[j] = make_float4(lay->marker_pos[3 * j], lay->marker_pos[3 * j + 1], lay->marker_pos[3 * j + 2], 0.f);
+    mnrm[j] = make_float4(lay->marker_nrm[3 * j], lay->marker_nrm[3 * j + 1], lay->marker_nrm[3 * j + 2], 0.f);
+  }
+  c->T = T; c->P = (int)pts.size(); c->M = M;
+  c->nh = !cfg->noise_enable ? 0 : (cfg->hyst_mode == TS_HYST_MAXWELL ? 6 : (cfg->hyst_mode == TS_HYST_ASYM ? 3 : 0));
+  c->dead_thr = (uint32_t)std::floor((double)cfg->p_dead * 4294967296.0);
+
+  const size_t E = (size_t)cfg->n_envs, EK = E * cfg->objs_per_env, EP = E * c->P;
+#define TS_ALLOC(ptr, bytes)                                                          \
+  do {                                                                                \
+    cudaError_t e_ = cudaMalloc((void**)&(ptr), (bytes));                             \
+    if (e_ != cudaSuccess) { ts_status s_ = cuda_fail(nullptr, e_, "cudaMalloc " #ptr); free_all(c); delete c; return s_; } \
+  } while (0)
+  TS_ALLOC(c->tx_pos, sizeof(float4) * T);
+  TS_ALLOC(c->tx_nrm, sizeof(float4) * T);
+  TS_ALLOC(c->mk_pos, sizeof(float4) * mpos.size());
+  TS_ALLOC(c->mk_nrm, sizeof(float4) * mnrm.size());
+  TS_ALLOC(c->patches, sizeof(TsPatch) * pts.size());
+  TS_ALLOC(c->g_type, sizeof(int32_t) * EK);
+  TS_ALLOC(c->g_params, sizeof(float4) * EK);
+  TS_ALLOC(c->st_flags, E * T);
+  TS_ALLOC(c->reset_step, sizeof(uint32_t) * E);
+  TS_ALLOC(c->episode, sizeof(uint32_t) * E);
+  if (cfg->noise_enable) {
+    if (c->nh) TS_ALLOC(c->st_hyst, sizeof(float4) * EP * c->nh * 32);
+    TS_ALLOC(c->st_drift, sizeof(float4) * EP * 3 * 32);
+  }
+#undef TS_ALLOC
+  cudaError_t e = cudaSuccess;
+  auto cp = [&](void* d, const void* h, size_t b) { if (e == cudaSuccess) e = cudaMemcpy(d, h, b, cudaMemcpyHostToDevice); };
+  cp(c->tx_pos, pos.data(), sizeof(float4) * T);
+  cp(c->tx_nrm, nrm.data(), sizeof(float4) * T);
+  cp(c->mk_pos, mpos.data(), sizeof(float4) * mpos.size());
+  cp(c->mk_nrm, mnrm.data(), sizeof(float4) * mnrm.size());
+  cp(c->patches, pts.data(), sizeof(TsPatch) * pts.size());
+  if (e == cudaSuccess) e = cudaMemset(c->g_type, 0, sizeof(int32_t) * EK);
+  if (e == cudaSuccess) e = cudaMemset(c->g_params, 0, sizeof(float4) * EK);
+  if (e == cudaSuccess) e = cudaMemset(c->reset_step, 0, sizeof(uint32_t) * E);
+  if (e == cudaSuccess) e = cudaMemset(c->episode, 0, sizeof(uint32_t) * E);
+  if (e == cudaSuccess) {  // episode 0: zero state, draw the dead mask
+    TsStepParams p;
+    fill_params(c, p);
+    e = (cudaError_t)ts_launch_reset_state(p, nullptr, c->dead_thr, c->nh, nullptr);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  }
+  if (e != cudaSuccess) { ts_status s = cuda_fail(nullptr, e, "ts_create: upload"); free_all(c); delete c; return s; }
+  *out = c;
+  return TS_OK;
+}
+
+ts_status ts_set_geometry(ts_ctx* c, const ts_geometry* geo, void* stream) {
+  if (!c) return TS_ERR_INVALID_ARG;
+  if (!geo || !geo->type || !geo->params) return fail(c, TS_ERR_INVALID_ARG, "ts_set_geometry: NULL argument");
+  const size_t EK = (size_t)c->cfg.n_envs * c->cfg.objs_per_env;
+  if (geo->n_grids < 0 || (geo->n_grids > 0 && (!geo->grids || geo->grid_n < 2 || geo->grid_n > 512 || !(geo->voxel > 0.f))))
+    return fail(c, TS_ERR_INVALID_ARG, "ts_set_geometry: bad grid bank");
+  for (size_t i = 0; i < EK; ++i) {
+    const int t = geo->type[i];
+    if (t < TS_GEOM_NONE || t > TS_GEOM_SDF) return fail(c, TS_ERR_INVALID_ARG, "ts_set_geometry: unknown type");
+    if (t == TS_GEOM_SDF) {
+      const float id = geo->params[4 * i];
+      if (!(id >= 0.f) || id >= (float)geo->n_grids || id != std::floor(id)) return fail(c, TS_ERR_INVALID_ARG, "ts_set_geometry: grid id out of range");
+    }
+  }
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  TS_CUDA(c, cudaMemcpyAsync(c->g_type, geo->type, sizeof(int32_t) * EK, cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaMemcpyAsync(c->g_params, geo->params, sizeof(float4) * EK, cudaMemcpyHostToDevice, st));
+  if (geo->n_grids > 0) {
+    const int N = geo->grid_n;
+    const size_t need = sizeof(float4) * ts_bank_elems_per_grid(N) * geo->n_grids;
+    if (need > c->bank_bytes) {
+      TS_CUDA(c, cudaStreamSynchronize(st));
+      cudaFree(c->bank); c->bank = nullptr; c->bank_bytes = 0;
+      TS_CUDA(c, cudaMalloc((void**)&c->bank, need));
+      c->bank_bytes = need;
+    }
+    float* staging = nullptr;
+    const size_t lin = sizeof(float) * (size_t)N * N * N * geo->n_grids;
+    TS_CUDA(c, cudaMalloc((void**)&staging, lin));
+    cudaError_t e = cudaMemcpyAsync(staging, geo->grids, lin, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = (cudaError_t)ts_launch_retile(staging, c->bank, geo->n_grids, N, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(staging);
+    if (e != cudaSuccess) return cuda_fail(c, e, "ts_set_geometry: bank upload");
+    c->grid_n = N; c->voxel = geo->voxel; c->n_grids = geo->n_grids;
+  } else {
+    c->n_grids = 0;
+  }
+  TS_CUDA(c, cudaStreamSynchronize(st));
+  c->have_geometry = true;
+  return TS_OK;
+}
+
+ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void* stream) {
+  if (!c) return TS_ERR_INVALID_ARG;
+  if (!in || !out) return fail(c, TS_ERR_INVALID_ARG, "ts_step: NULL argument");
+  if (!c->have_geometry) return fail(c, TS_ERR_STATE, "ts_step before ts_set_geometry");
+  if (!in->link_pos || !in->link_quat || !in->link_linvel || !in->link_angvel || !in->obj_pos || !in->obj_quat ||
+      !in->obj_linvel || !in->obj_angvel)
+    return fail(c, TS_ERR_INVALID_ARG, "ts_step: NULL input pointer");
+  if ((out->ft_noisy || out->dead) && !c->cfg.noise_enable) return fail(c, TS_ERR_INVALID_ARG, "ts_step: ft_noisy / dead need noise_enable");
+  if (out->marker && c->M == 0) return fail(c, TS_ERR_INVALID_ARG, "ts_step: marker requested but the layout has no markers");
+  const uintptr_t al = (uintptr_t)out->contact | (uintptr_t)out->depth | (uintptr_t)out->ft | (uintptr_t)out->marker |
+                       (uintptr_t)out->prox | (uintptr_t)out->ft_noisy | (uintptr_t)out->dead | (uintptr_t)in->link_quat |
+                       (uintptr_t)in->obj_quat;
+  if (al & 15) return fail(c, TS_ERR_INVALID_ARG, "ts_step: pointers must be 16-byte aligned");
+  DeviceGuard guard(c->device);
+  TsStepParams p;
+  fill_params(c, p);
+  p.link_pos = in->link_pos; p.link_quat = in->link_quat; p.link_linvel = in->link_linvel; p.link_angvel = in->link_angvel;
+  p.obj_pos = in->obj_pos; p.obj_quat = in->obj_quat; p.obj_linvel = in->obj_linvel; p.obj_angvel = in->obj_angvel;
+  p.contact = out->contact; p.depth = out->depth; p.ft = out->ft; p.marker = out->marker; p.prox = out->prox;
+  p.ft_noisy = out->ft_noisy; p.dead = out->dead;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (c->timing) {
+    if (c->ev_used + 2 > c->ev.size()) {
+      cudaEvent_t a, b;
+      TS_CUDA(c, cudaEventCreate(&a));
+      TS_CUDA(c, cudaEventCreate(&b));
+      c->ev.push_back(a); c->ev.push_back(b);
+    }
+    e0 = c->ev[c->ev_used]; e1 = c->ev[c->ev_used + 1];
+    c->ev_used += 2;
+    TS_CUDA(c, cudaEventRecord(e0, st));
+  }
+  const cudaError_t e = (cudaError_t)ts_launch_step(p, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: launch");
+  if (c->timing) TS_CUDA(c, cudaEventRecord(e1, st));
+  c->gstep += 1;
+  return TS_OK;
+}
+
+ts_status ts_step_host(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void* stream) {
+  if (!c) return TS_ERR_INVALID_ARG;
+  if (!in || !out) return fail(c, TS_ERR_INVALID_ARG, "ts_step_host: NULL argument");
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t E = (size_t)c->cfg.n_envs, L = (size_t)c->cfg.n_links, K = (size_t)c->cfg.objs_per_env, T = (size_t)c->T;
+  const float* hin[8] = {in->link_pos, in->link_quat, in->link_linvel, in->link_angvel,
+                         in->obj_pos, in->obj_quat, in->obj_linvel, in->obj_angvel};
+  const size_t in_bytes[8] = {E * L * 12, E * L * 16, E * L * 12, E * L * 12, E * K * 12, E * K * 16, E * K * 12, E * K * 12};
+  void* hout[7] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead};
+  const size_t out_bytes[7] = {E * T, E * T * 4, E * T * 24, E * (size_t)c->M * 12, E * T * 4, E * T * 24, E * T};
+  for (int i = 0; i < 8; ++i) {
+    if (!hin[i]) return fail(c, TS_ERR_INVALID_ARG, "ts_step_host: NULL input pointer");
+    if (!c->stage_in[i]) TS_CUDA(c, cudaMalloc((void**)&c->stage_in[i], in_bytes[i]));
+    TS_CUDA(c, cudaMemcpyAsync(c->stage_in[i], hin[i], in_bytes[i], cudaMemcpyHostToDevice, st));
+  }
+  for (int i = 0; i < 7; ++i)
+    if (hout[i] && !c->stage_out[i]) TS_CUDA(c, cudaMalloc(&c->stage_out[i], out_bytes[i] ? out_bytes[i] : 16));
+  ts_step_in din = {c->stage_in[0], c->stage_in[1], c->stage_in[2], c->stage_in[3],
+                    c->stage_in[4], c->stage_in[5], c->stage_in[6], c->stage_in[7]};
+  ts_step_out dout = {hout[0] ? (uint8_t*)c->stage_out[0] : nullptr, hout[1] ? (float*)c->stage_out[1] : nullptr,
+                      hout[2] ? (float*)c->stage_out[2] : nullptr,   hout[3] ? (float*)c->stage_out[3] : nullptr,
+                      hout[4] ? (float*)c->stage_out[4] : nullptr,   hout[5] ? (float*)c->stage_out[5] : nullptr,
+                      hout[6] ? (uint8_t*)c->stage_out[6] : nullptr};
+  const ts_status s = ts_step(c, &din, &dout, stream);
+  if (s != TS_OK) return s;
+  for (int i = 0; i < 7; ++i)
+    if (hout[i]) TS_CUDA(c, cudaMemcpyAsync(hout[i], c->stage_out[i], out_bytes[i], cudaMemcpyDeviceToHost, st));
+  return TS_OK;
+}
+
+ts_status ts_reset(ts_ctx* c, const uint8_t* env_mask_dev, void* stream) {
+  if (!c) return TS_ERR_INVALID_ARG;
+  DeviceGuard guard(c->device);
+  TsStepParams p;
+  fill_params(c, p);
+  cudaError_t e = (cudaError_t)ts_launch_reset_counters(c->reset_step, c->episode, env_mask_dev, c->cfg.n_envs, c->gstep, stream);
+  if (e == cudaSuccess) e = (cudaError_t)ts_launch_reset_state(p, env_mask_dev, c->dead_thr, c->nh, stream);
+  if (e != cudaSuccess) return cuda_fail(c, e, "ts_reset: launch");
+  return TS_OK;
+}
+
+ts_status ts_kernel_time_ms(ts_ctx* c, int32_t enable, float* mean_ms, int32_t* n_steps) {
+  if (!c) return TS_ERR_INVALID_ARG;
+  DeviceGuard guard(c->device);
+  double sum = 0.0;
+  int n = 0;
+  for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
+    TS_CUDA(c, cudaEventSynchronize(c->ev[i + 1]));
+    float ms = 0.f;
+    TS_CUDA(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
+    sum += ms;
+    ++n;
+  }
+  c->ev_used = 0;
+  c->timing = enable != 0;
+  if (mean_ms) *mean_ms = n ? (float)(sum / n) : 0.f;
+  if (n_steps) *n_steps = n;
+  return TS_OK;
+}
+
+ts_status ts_destroy(ts_ctx* c) {
+  if (!c) return TS_OK;
+  {
+    DeviceGuard guard(c->device);
+    cudaDeviceSynchronize();
+    free_all(c);
+  }
+  delete c;
+  return TS_OK;
+}
+
+}  // extern "C"
