@@ -77,7 +77,7 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.env_id_base = (uint32_t)g.env_id_base;
   p.tx_pos = c->tx_pos; p.tx_nrm = c->tx_nrm; p.patches = c->patches; p.mk_pos = c->mk_pos; p.mk_nrm = c->mk_nrm;
   p.g_type = c->g_type; p.g_params = c->g_params; p.bank = c->bank;
-  p.grid_n = c->grid_n; p.voxel = c->voxel; p.inv_voxel = 1.0f / c->voxel;
+  p.grid_n = c->grid_n; p.voxel = c->voxel; p.inv_voxel = 1.0f / c->voxel; p.inv_voxel_d = 1.0 / (double)c->voxel;
   p.grid_origin = -0.5f * (c->grid_n - 1) * c->voxel;
   p.grid_stride = ts_bank_elems_per_grid(c->grid_n);
   p.st_flags = c->st_flags; p.st_hyst = c->st_hyst; p.st_drift = c->st_drift;

@@ -51,6 +51,7 @@ struct TsStepParams {
   const float4* bank;      // re-tiled SDF bank (see ts_kernels.cu, "bank layout")
   int32_t grid_n;
   float voxel, inv_voxel, grid_origin;
+  double inv_voxel_d;  // 1 / (double)voxel, for the fp64 first query
   unsigned long long grid_stride;  // float4 elements per grid
   // inputs
   const float *link_pos, *link_quat, *link_linvel, *link_angvel;

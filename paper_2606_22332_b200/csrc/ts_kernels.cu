@@ -37,16 +37,6 @@ __device__ __forceinline__ F3 ld3(const float* p) { return F3{__ldg(p), __ldg(p 
 struct Rot {  // row-major 3x3
   float a[9];
 };
-// O0: rotation of a quaternion (w,x,y,z), used as given.
-__device__ __forceinline__ Rot quat_R(const float* q4) {
-  const float4 q = __ldg(reinterpret_cast<const float4*>(q4));
-  const float w = q.x, x = q.y, y = q.z, z = q.w;
-  Rot R;
-  R.a[0] = 1.f - 2.f * (y * y + z * z); R.a[1] = 2.f * (x * y - w * z);       R.a[2] = 2.f * (x * z + w * y);
-  R.a[3] = 2.f * (x * y + w * z);       R.a[4] = 1.f - 2.f * (x * x + z * z); R.a[5] = 2.f * (y * z - w * x);
-  R.a[6] = 2.f * (x * z - w * y);       R.a[7] = 2.f * (y * z + w * x);       R.a[8] = 1.f - 2.f * (x * x + y * y);
-  return R;
-}
 __device__ __forceinline__ F3 mul(const Rot& R, F3 v) {
   return F3{fmaf(R.a[0], v.x, fmaf(R.a[1], v.y, R.a[2] * v.z)), fmaf(R.a[3], v.x, fmaf(R.a[4], v.y, R.a[5] * v.z)),
             fmaf(R.a[6], v.x, fmaf(R.a[7], v.y, R.a[8] * v.z))};
@@ -56,50 +46,103 @@ __device__ __forceinline__ F3 mulT(const Rot& R, F3 v) {
             fmaf(R.a[2], v.x, fmaf(R.a[5], v.y, R.a[8] * v.z))};
 }
 
+// Double-precision twins used ONLY for the relative pose and the first geometry query (DESIGN.md
+// "fp64 frame"): the contact normal of a box edge/corner is max(|x|-b,0)/|.|, a ratio of
+// millimetre differences of centimetre numbers, and the stiff force law amplifies d; with fp32
+// positions (error ~4e-9 m) neither meets rtol 1e-4.  B200 issues DFMA at half the FFMA rate
+// and this is ~60 DFMA per taxel, so the cost hides under the state streams.
+template <typename S>
+struct X3 {
+  S x, y, z;
+};
+typedef X3<double> D3;
+struct RotD {
+  double a[9];
+};
+// O0: rotation of a quaternion (w,x,y,z), used as given.
+__device__ __forceinline__ RotD quat_Rd(const float* q4) {
+  const float4 q = __ldg(reinterpret_cast<const float4*>(q4));
+  const double w = q.x, x = q.y, y = q.z, z = q.w;
+  RotD R;
+  R.a[0] = 1.0 - 2.0 * (y * y + z * z); R.a[1] = 2.0 * (x * y - w * z);       R.a[2] = 2.0 * (x * z + w * y);
+  R.a[3] = 2.0 * (x * y + w * z);       R.a[4] = 1.0 - 2.0 * (x * x + z * z); R.a[5] = 2.0 * (y * z - w * x);
+  R.a[6] = 2.0 * (x * z - w * y);       R.a[7] = 2.0 * (y * z + w * x);       R.a[8] = 1.0 - 2.0 * (x * x + y * y);
+  return R;
+}
+__device__ __forceinline__ Rot to_float(const RotD& R) {
+  Rot r;
+#pragma unroll
+  for (int i = 0; i < 9; ++i) r.a[i] = (float)R.a[i];
+  return r;
+}
+__device__ __forceinline__ F3 to_float(const D3& v) { return F3{(float)v.x, (float)v.y, (float)v.z}; }
+__device__ __forceinline__ X3<float> as_x3(F3 v) { return X3<float>{v.x, v.y, v.z}; }
+
 // Object k seen from the sensor link: x_o = c + M x_j (object frame <- link frame).
-// Forming p_L - p_O BEFORE rotating keeps the small relative offsets accurate in fp32.
+// Forming p_L - p_O BEFORE rotating keeps the small relative offsets accurate.
 struct ObjFrame {
   Rot M;  // R_O^T R_L
   F3 c;   // R_O^T (p_L - p_O)
   int type;
   float4 prm;
 };
+struct ObjFrameD {
+  RotD M;
+  D3 c;
+};
 
-__device__ __forceinline__ ObjFrame make_frame(const TsStepParams& p, int e, int k, const Rot& RL, F3 pL) {
+__device__ __forceinline__ ObjFrame make_frame(const TsStepParams& p, int e, int k, const RotD& RL, D3 pL, ObjFrameD& fd) {
   const size_t ek = (size_t)e * p.K + k;
   ObjFrame f;
   f.type = __ldg(p.g_type + ek);
   f.prm = __ldg(p.g_params + ek);
-  const Rot RO = quat_R(p.obj_quat + ek * 4);
-  const F3 pO = ld3(p.obj_pos + ek * 3);
+  const RotD RO = quat_Rd(p.obj_quat + ek * 4);
+  const double dx = pL.x - (double)__ldg(p.obj_pos + ek * 3), dy = pL.y - (double)__ldg(p.obj_pos + ek * 3 + 1),
+               dz = pL.z - (double)__ldg(p.obj_pos + ek * 3 + 2);
 #pragma unroll
   for (int r = 0; r < 3; ++r)
 #pragma unroll
     for (int c = 0; c < 3; ++c)
-      f.M.a[r * 3 + c] = fmaf(RO.a[r], RL.a[c], fmaf(RO.a[3 + r], RL.a[3 + c], RO.a[6 + r] * RL.a[6 + c]));
-  f.c = mulT(RO, pL - pO);
+      fd.M.a[r * 3 + c] = fma(RO.a[r], RL.a[c], fma(RO.a[3 + r], RL.a[3 + c], RO.a[6 + r] * RL.a[6 + c]));
+  fd.c.x = fma(RO.a[0], dx, fma(RO.a[3], dy, RO.a[6] * dz));
+  fd.c.y = fma(RO.a[1], dx, fma(RO.a[4], dy, RO.a[7] * dz));
+  fd.c.z = fma(RO.a[2], dx, fma(RO.a[5], dy, RO.a[8] * dz));
+  f.M = to_float(fd.M);
+  f.c = to_float(fd.c);
   return f;
+}
+__device__ __forceinline__ D3 mul(const ObjFrameD& f, F3 v) {
+  const double x = v.x, y = v.y, z = v.z;
+  return D3{fma(f.M.a[0], x, fma(f.M.a[1], y, fma(f.M.a[2], z, f.c.x))), fma(f.M.a[3], x, fma(f.M.a[4], y, fma(f.M.a[5], z, f.c.y))),
+            fma(f.M.a[6], x, fma(f.M.a[7], y, fma(f.M.a[8], z, f.c.z)))};
 }
 
 // ---------------------------------------------------------------------------------------
 // O2: signed distance (and object-frame gradient) of one geometry at object-frame point x.
 // ---------------------------------------------------------------------------------------
-template <bool GRAD>
-__device__ __forceinline__ float sdf_grid(const TsStepParams& p, int gid, F3 x, F3& g) {
+__device__ __forceinline__ float inv_vox(const TsStepParams& p, float) { return p.inv_voxel; }
+__device__ __forceinline__ double inv_vox(const TsStepParams& p, double) { return p.inv_voxel_d; }
+__device__ __forceinline__ float fma_s(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_s(double a, double b, double c) { return fma(a, b, c); }
+
+// S = double for the first query (cell index and fractions exact to fp32 rounding), float in the march.
+template <bool GRAD, typename S>
+__device__ __forceinline__ float sdf_grid(const TsStepParams& p, int gid, X3<S> x, F3& g) {
   const int N = p.grid_n;
-  const float top = (float)(N - 1);
-  const float half = 0.5f * top;
-  const float ux = fmaf(x.x, p.inv_voxel, half), uy = fmaf(x.y, p.inv_voxel, half), uz = fmaf(x.z, p.inv_voxel, half);
-  const float cx = fminf(fmaxf(ux, 0.f), top), cy = fminf(fmaxf(uy, 0.f), top), cz = fminf(fmaxf(uz, 0.f), top);
+  const S top = (S)(N - 1);
+  const S half = (S)0.5 * top;
+  const S iv = inv_vox(p, S());
+  const S ux = fma_s(x.x, iv, half), uy = fma_s(x.y, iv, half), uz = fma_s(x.z, iv, half);
+  const S cx = min(max(ux, (S)0), top), cy = min(max(uy, (S)0), top), cz = min(max(uz, (S)0), top);
   const int i0 = min((int)cx, N - 2), j0 = min((int)cy, N - 2), k0 = min((int)cz, N - 2);
-  const float fx = cx - (float)i0, fy = cy - (float)j0, fz = cz - (float)k0;
+  const float fx = (float)(cx - (S)i0), fy = (float)(cy - (S)j0), fz = (float)(cz - (S)k0);
   const float4* q = p.bank + (size_t)gid * p.grid_stride + ((size_t)(j0 * (N - 1) + i0) * N + k0);
   const float4 A = __ldg(q), B = __ldg(q + 1);  // (c000,c100,c010,c110), (c001,c101,c011,c111)
   const float a0 = fmaf(fx, A.y - A.x, A.x), a1 = fmaf(fx, A.w - A.z, A.z);
   const float b0 = fmaf(fx, B.y - B.x, B.x), b1 = fmaf(fx, B.w - B.z, B.z);
   const float lo = fmaf(fy, a1 - a0, a0), hi = fmaf(fy, b1 - b0, b0);
   float phi = fmaf(fz, hi - lo, lo);
-  const float ox = ux - cx, oy = uy - cy, oz = uz - cz;   // outside-grid extension (O2)
+  const float ox = (float)(ux - cx), oy = (float)(uy - cy), oz = (float)(uz - cz);   // outside-grid extension (O2)
   const float o2 = fmaf(ox, ox, fmaf(oy, oy, oz * oz));
   if (o2 > 0.f) phi += p.voxel * sqrtf(o2);
   if (GRAD) {  // exact derivative of the trilinear interpolant in cell (i0,j0,k0); 1/h_v dropped (normalised later)
@@ -112,16 +155,17 @@ __device__ __forceinline__ float sdf_grid(const TsStepParams& p, int gid, F3 x, 
   return phi;
 }
 
-template <bool GRAD>
-__device__ __forceinline__ float sdf_eval(const TsStepParams& p, const ObjFrame& f, F3 x, F3& g) {
+template <bool GRAD, typename S>
+__device__ __forceinline__ float sdf_eval(const TsStepParams& p, const ObjFrame& f, X3<S> xs, F3& g) {
+  const F3 x = mk3((float)xs.x, (float)xs.y, (float)xs.z);
   switch (f.type) {
     case TS_GEOM_SPHERE: {
       const float n = sqrtf(dot(x, x));
       if (GRAD) g = (n < 1e-12f) ? mk3(0.f, 0.f, 1.f) : (1.f / n) * x;
       return n - f.prm.x;
     }
-    case TS_GEOM_BOX: {
-      const float wx = fabsf(x.x) - f.prm.x, wy = fabsf(x.y) - f.prm.y, wz = fabsf(x.z) - f.prm.z;
+    case TS_GEOM_BOX: {  // w = |x| - b formed in S: the edge/corner normal is a ratio of these small differences
+      const float wx = (float)(abs(xs.x) - (S)f.prm.x), wy = (float)(abs(xs.y) - (S)f.prm.y), wz = (float)(abs(xs.z) - (S)f.prm.z);
       const float px = fmaxf(wx, 0.f), py = fmaxf(wy, 0.f), pz = fmaxf(wz, 0.f);
       const float lp = sqrtf(fmaf(px, px, fmaf(py, py, pz * pz)));
       const float wmax = fmaxf(wx, fmaxf(wy, wz));
@@ -147,7 +191,7 @@ __device__ __forceinline__ float sdf_eval(const TsStepParams& p, const ObjFrame&
       return n - f.prm.x;
     }
     case TS_GEOM_SDF:
-      return sdf_grid<GRAD>(p, (int)f.prm.x, x, g);
+      return sdf_grid<GRAD, S>(p, (int)f.prm.x, xs, g);
     default:
       if (GRAD) g = mk3(0.f, 0.f, 1.f);
       return __int_as_float(0x7f800000);
@@ -216,11 +260,14 @@ __global__ void __launch_bounds__(TS_BLOCK) ts_step_kernel(const __grid_constant
   // ---- S1: link pose (warp-uniform) ---------------------------------------------------
   const int lk = max(link, 0);
   const size_t el = (size_t)e * p.L + lk;
-  const Rot RL = quat_R(p.link_quat + el * 4);
+  const RotD RLd = quat_Rd(p.link_quat + el * 4);
+  const Rot RL = to_float(RLd);
   const F3 pL = ld3(p.link_pos + el * 3);
+  const D3 pLd = D3{(double)pL.x, (double)pL.y, (double)pL.z};
 
   // ---- S2/S3: geometry query, winner = smallest phi (= max_k [R - phi_k]_+, Eq. 2) ------
-  ObjFrame fr = make_frame(p, e, 0, RL, pL);
+  ObjFrameD frd;
+  ObjFrame fr = make_frame(p, e, 0, RLd, pLd, frd);
   float phi[2];
   F3 mbar[2];  // contact normal in the link frame, m_bar = R_L^T m = M^T g/|g|
   int kst[2] = {0, 0};
@@ -231,13 +278,13 @@ __global__ void __launch_bounds__(TS_BLOCK) ts_step_kernel(const __grid_constant
     mbar[s] = mk3(0.f, 0.f, 0.f);
   }
   for (int k = 0; k < (SINGLE ? 1 : p.K); ++k) {
-    if (!SINGLE && k > 0) fr = make_frame(p, e, k, RL, pL);
+    if (!SINGLE && k > 0) fr = make_frame(p, e, k, RLd, pLd, frd);
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
-      const F3 x = fr.c + mul(fr.M, xj[s]);
-      if (SINGLE) { xo[s] = x; dro[s] = mul(fr.M, nj[s]); }
+      const D3 xd = mul(frd, xj[s]);
+      if (SINGLE) { xo[s] = to_float(xd); dro[s] = mul(fr.M, nj[s]); }
       F3 g;
-      const float ph = sdf_eval<true>(p, fr, x, g);
+      const float ph = sdf_eval<true, double>(p, fr, xd, g);
       if (ph < phi[s]) {  // strict: ties -> lowest k (Q3)
         phi[s] = ph;
         kst[s] = k;
@@ -570,12 +617,13 @@ __global__ void __launch_bounds__(TS_BLOCK) ts_step_kernel(const __grid_constant
           float sv;
           F3 dummy;
           if (SINGLE) {
-            sv = sdf_eval<false>(p, fr, xo[s] + t[s] * dro[s], dummy);
+            sv = sdf_eval<false, float>(p, fr, as_x3(xo[s] + t[s] * dro[s]), dummy);
           } else {
             sv = __int_as_float(0x7f800000);
             for (int k = 0; k < p.K; ++k) {
-              const ObjFrame f2 = make_frame(p, e, k, RL, pL);
-              sv = fminf(sv, sdf_eval<false>(p, f2, f2.c + mul(f2.M, xj[s] + t[s] * nj[s]), dummy));
+              ObjFrameD f2d;
+              const ObjFrame f2 = make_frame(p, e, k, RLd, pLd, f2d);
+              sv = fminf(sv, sdf_eval<false, float>(p, f2, as_x3(f2.c + mul(f2.M, xj[s] + t[s] * nj[s])), dummy));
             }
           }
           const float tn = fminf(t[s] + fmaxf(sv, 0.f), p.r_prox);
