@@ -53,8 +53,9 @@ typedef enum ts_status {
  *   n = u_axis x v_axis,  slot index = patch_start + iv*nu + iu  (u fastest),
  * plus an optional marker_nu x marker_nv grid of elastomer markers placed the same way
  * (marker_nu = 0: none; markers = taxels reproduces the paper's (N,3) output, Q16).
- * Limits: nu*nv <= 64 and marker_nu*marker_nv <= 64 per patch (one warp owns a patch).
- * u_axis, v_axis must be unit and orthogonal to 1e-3.
+ * Limits: nu*nv <= 64 and marker_nu*marker_nv <= 64 per patch (whole patches are packed into
+ * 256-slot thread blocks).  u_axis, v_axis must be unit and orthogonal to 1e-5 (the marker sum
+ * is evaluated separably along u and v).
  * ------------------------------------------------------------------------------------- */
 typedef struct ts_patch_desc {
   int32_t link;       /* sensor link index, 0 <= link < n_links */

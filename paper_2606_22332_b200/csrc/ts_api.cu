@@ -13,13 +13,18 @@
 struct ts_ctx {
   int device = 0;
   ts_config cfg{};
-  int T = 0, P = 0, M = 0, nh = 0;
+  int T = 0, P = 0, M = 0, nh = 0, G = 0, Tp = 0, frames_per_group = 1;
   bool have_geometry = false;
   uint32_t gstep = 0;
   uint32_t dead_thr = 0;
   // device buffers
   float4 *tx_pos = nullptr, *tx_nrm = nullptr, *mk_pos = nullptr, *mk_nrm = nullptr;
+  int4* tx_nbr = nullptr;
   TsPatch* patches = nullptr;
+  TsGroup* groups = nullptr;
+  TsChunk* chunks = nullptr;
+  int32_t *mk_item1 = nullptr, *mk_item2 = nullptr;
+  double* mk_tab = nullptr;
   int32_t* g_type = nullptr;
   float4* g_params = nullptr;
   float4* bank = nullptr;
@@ -27,7 +32,7 @@ struct ts_ctx {
   int grid_n = 2, n_grids = 0;
   float voxel = 1.f;
   uint8_t* st_flags = nullptr;
-  float4 *st_hyst = nullptr, *st_drift = nullptr;
+  float *st_hyst = nullptr, *st_drift = nullptr;
   uint32_t *reset_step = nullptr, *episode = nullptr;
   // device staging of ts_step_host
   float* stage_in[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -63,6 +68,7 @@ struct DeviceGuard {
 
 void free_all(ts_ctx* c) {
   cudaFree(c->tx_pos); cudaFree(c->tx_nrm); cudaFree(c->mk_pos); cudaFree(c->mk_nrm); cudaFree(c->patches);
+  cudaFree(c->tx_nbr); cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab);
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->bank); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode);
   for (float* q : c->stage_in) cudaFree(q);
@@ -74,11 +80,13 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   const ts_config& g = c->cfg;
   std::memset(&p, 0, sizeof(p));
   p.E = g.n_envs; p.L = g.n_links; p.K = g.objs_per_env; p.T = c->T; p.P = c->P; p.M = c->M;
+  p.G = c->G; p.Tp = c->Tp; p.frames_per_group = c->frames_per_group;
+  p.tx_nbr = c->tx_nbr; p.groups = c->groups; p.chunks = c->chunks; p.mk_item1 = c->mk_item1; p.mk_item2 = c->mk_item2;
+  p.mk_tab = c->mk_tab;
   p.env_id_base = (uint32_t)g.env_id_base;
   p.tx_pos = c->tx_pos; p.tx_nrm = c->tx_nrm; p.patches = c->patches; p.mk_pos = c->mk_pos; p.mk_nrm = c->mk_nrm;
   p.g_type = c->g_type; p.g_params = c->g_params; p.bank = c->bank;
   p.grid_n = c->grid_n; p.voxel = c->voxel; p.inv_voxel = 1.0f / c->voxel; p.inv_voxel_d = 1.0 / (double)c->voxel;
-  p.grid_origin = -0.5f * (c->grid_n - 1) * c->voxel;
   p.grid_stride = ts_bank_elems_per_grid(c->grid_n);
   p.st_flags = c->st_flags; p.st_hyst = c->st_hyst; p.st_drift = c->st_drift;
   p.reset_step = c->reset_step; p.episode = c->episode; p.gstep = c->gstep;
@@ -86,7 +94,7 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.eta_on = g.eta_on; p.eta_off = g.eta_off; p.use_velocity = g.use_velocity;
   p.s_d = g.s_d; p.lambda_d = g.lambda_d; p.alpha_e = g.alpha_e; p.c_e = g.c_e;
   // 1 / g_bar, g_bar = e^{-1/2} / sqrt(2 lambda_d)
-  p.inv_gbar = (float)(std::sqrt(2.0 * (double)g.lambda_d) / std::exp(-0.5));
+  p.inv_gbar = std::sqrt(2.0 * (double)g.lambda_d) / std::exp(-0.5);
   p.r_prox = g.r_prox; p.march_steps = g.march_steps;
   p.noise_enable = g.noise_enable; p.hyst_mode = g.noise_enable ? g.hyst_mode : TS_HYST_OFF;
   p.seed_lo = (uint32_t)(g.seed & 0xffffffffu); p.seed_hi = (uint32_t)(g.seed >> 32);
@@ -159,36 +167,129 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   // ---- layout -> device records; trailing filler slots are covered by filler patches ----
   const int T = lay->n_taxels;
   std::vector<float4> pos(T), nrm(T);
+  std::vector<int4> nbr(T);
   for (int t = 0; t < T; ++t) {
     pos[t] = make_float4(lay->pos[3 * t], lay->pos[3 * t + 1], lay->pos[3 * t + 2], lay->radius[t]);
     nrm[t] = make_float4(lay->nrm[3 * t], lay->nrm[3 * t + 1], lay->nrm[3 * t + 2], 0.f);
+    nbr[t] = make_int4(lay->nbr[4 * t], lay->nbr[4 * t + 1], lay->nbr[4 * t + 2], lay->nbr[4 * t + 3]);
   }
+  const int M = (int)lay->marker_patch.size();
   std::vector<TsPatch> pts;
+  std::vector<double> tab;
+  std::vector<int32_t> item1, item2(M > 0 ? M : 1, 0);
   int used = 0;
-  for (size_t p = 0; p < lay->patch_start.size(); ++p) {
+  for (size_t pi = 0; pi < lay->patch_start.size(); ++pi) {
+    const ts_patch_desc& d = lay->desc[pi];
     TsPatch q{};
-    q.start = lay->patch_start[p]; q.nu = lay->patch_nu[p]; q.n = lay->patch_nu[p] * lay->patch_nv[p];
-    q.link = lay->patch_link[p]; q.mstart = lay->marker_start[p]; q.mcount = lay->marker_count[p];
-    q.eps = lay->patch_eps[p];
+    q.start = lay->patch_start[pi]; q.nu = d.nu; q.nv = d.nv; q.n = d.nu * d.nv;
+    q.link = d.link; q.mstart = lay->marker_start[pi]; q.mnu = d.marker_nu; q.mnv = d.marker_nv;
+    q.eps = lay->patch_eps[pi];
+    const double u[3] = {d.u_axis[0], d.u_axis[1], d.u_axis[2]}, v[3] = {d.v_axis[0], d.v_axis[1], d.v_axis[2]};
+    q.ua = make_float4(d.u_axis[0], d.u_axis[1], d.u_axis[2], 0.f);
+    q.va = make_float4(d.v_axis[0], d.v_axis[1], d.v_axis[2], 0.f);
+    q.na = q.mnu > 0 ? make_float4(lay->marker_nrm[3 * q.mstart], lay->marker_nrm[3 * q.mstart + 1], lay->marker_nrm[3 * q.mstart + 2], 0.f)
+                     : make_float4(0.f, 0.f, 1.f, 0.f);
+    q.direct = (cfg->c_e != 1.0f || q.mnu * q.nv > TS_BLOCK) ? 1 : 0;
+    q.tab = (int32_t)tab.size();
+    q.i1off = (int32_t)item1.size();
+    if (q.mnu > 0 && !q.direct) {
+      // separable tables from the fp32 layout coordinates (the oracle's inputs), evaluated in double:
+      // su(a,p) = u^.(x^m(a,0) - x(p,0)) / u^.u^,  GU = exp(-lambda su^2 u^.u^),  DU = su GU; same along v.
+      const double lam = (double)cfg->lambda_d;
+      const double uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2], vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+      auto coef = [&](int m, int t, const double* ax, double aa) {
+        double s = 0.0;
+        for (int k = 0; k < 3; ++k) s += ax[k] * ((double)lay->marker_pos[3 * m + k] - (double)lay->pos[3 * t + k]);
+        return s / aa;
+      };
+      std::vector<double> GU(q.mnu * q.nu), DU(q.mnu * q.nu), GV(q.mnv * q.nv), DV(q.mnv * q.nv);
+      for (int a = 0; a < q.mnu; ++a)
+        for (int ip = 0; ip < q.nu; ++ip) {
+          const double su = coef(q.mstart + a, q.start + ip, u, uu);
+          GU[a * q.nu + ip] = std::exp(-lam * su * su * uu);
+          DU[a * q.nu + ip] = su * GU[a * q.nu + ip];
+        }
+      for (int b = 0; b < q.mnv; ++b)
+        for (int iq = 0; iq < q.nv; ++iq) {
+          const double sv = coef(q.mstart + b * q.mnu, q.start + iq * q.nu, v, vv);
+          GV[b * q.nv + iq] = std::exp(-lam * sv * sv * vv);
+          DV[b * q.nv + iq] = sv * GV[b * q.nv + iq];
+        }
+      tab.insert(tab.end(), GU.begin(), GU.end());
+      tab.insert(tab.end(), DU.begin(), DU.end());
+      tab.insert(tab.end(), GV.begin(), GV.end());
+      tab.insert(tab.end(), DV.begin(), DV.end());
+      for (int iq = 0; iq < q.nv; ++iq)
+        for (int a = 0; a < q.mnu; ++a) item1.push_back(0);  // packed below, once the group-local index is known
+    }
     pts.push_back(q);
     used = q.start + q.n;
   }
-  for (int t = used; t < T; t += TS_MAX_PATCH_TAXELS) {
+  for (int t = used; t < T; t += TS_BLOCK) {
     TsPatch q{};
-    q.start = t; q.n = (T - t < TS_MAX_PATCH_TAXELS) ? T - t : TS_MAX_PATCH_TAXELS; q.nu = q.n; q.link = -1;
+    q.start = t; q.n = (T - t < TS_BLOCK) ? T - t : TS_BLOCK; q.nu = q.n; q.nv = 1; q.link = -1; q.mstart = M;
+    q.tab = (int32_t)tab.size(); q.i1off = (int32_t)item1.size();
+    q.ua = q.va = q.na = make_float4(0.f, 0.f, 0.f, 0.f);
     pts.push_back(q);
   }
-  const int M = (int)lay->marker_patch.size();
+  // ---- pack whole patches into groups of <= TS_BLOCK slots; markers of a group into chunks ----
+  std::vector<TsGroup> groups;
+  std::vector<TsChunk> chunks;
+  int fpg = 1;
+  for (size_t pi = 0; pi < pts.size();) {
+    TsGroup g{};
+    g.start = pts[pi].start; g.patch0 = (int32_t)pi; g.mstart = pts[pi].mstart; g.chunk0 = (int32_t)chunks.size();
+    while (pi < pts.size() && g.count + pts[pi].n <= TS_BLOCK && g.npatch < TS_MAX_GROUP_PATCHES) {
+      g.count += pts[pi].n; g.npatch += 1; g.mcount += pts[pi].mnu * pts[pi].mnv; ++pi;
+    }
+    if (g.npatch > fpg) fpg = g.npatch;
+    for (int l = 0; l < g.npatch;) {  // chunks: pass-1 items and markers both fit one block
+      TsChunk ck{};
+      const TsPatch& f = pts[g.patch0 + l];
+      ck.i1_begin = ck.i1_end = f.i1off; ck.m_begin = ck.m_end = f.mstart; ck.lp_begin = l;
+      while (l < g.npatch) {
+        const TsPatch& q = pts[g.patch0 + l];
+        const int n1 = (q.mnu > 0 && !q.direct) ? q.mnu * q.nv : 0, nm = q.mnu * q.mnv;
+        if (l > ck.lp_begin && ((ck.i1_end - ck.i1_begin) + n1 > TS_BLOCK || (ck.m_end - ck.m_begin) + nm > TS_BLOCK)) break;
+        ck.i1_end += n1; ck.m_end += nm; ++l;
+      }
+      ck.lp_end = l;
+      if (ck.m_end > ck.m_begin) chunks.push_back(ck);
+    }
+    g.nchunk = (int32_t)chunks.size() - g.chunk0;
+    for (int l = 0; l < g.npatch; ++l) {  // group-local patch index: per taxel (in nrm.w) and per marker item
+      const TsPatch& q = pts[g.patch0 + l];
+      for (int t = q.start; t < q.start + q.n; ++t) std::memcpy(&nrm[t].w, &l, sizeof(int));
+      if (q.mnu > 0 && !q.direct)
+        for (int iq = 0; iq < q.nv; ++iq)
+          for (int a = 0; a < q.mnu; ++a) item1[q.i1off + iq * q.mnu + a] = l | (a << 8) | (iq << 16);
+      for (int b = 0; b < q.mnv; ++b)
+        for (int a = 0; a < q.mnu; ++a) item2[q.mstart + b * q.mnu + a] = l | (a << 8) | (b << 16);
+    }
+    groups.push_back(g);
+  }
+  if (item1.empty()) item1.push_back(0);
+  if (tab.empty()) tab.push_back(0.0);
+  if (chunks.empty()) chunks.push_back(TsChunk{});
   std::vector<float4> mpos(M > 0 ? M : 1), mnrm(M > 0 ? M : 1);
   for (int j = 0; j < M; ++j) {
     mpos[j] = make_float4(lay->marker_pos[3 * j], lay->marker_pos[3 * j + 1], lay->marker_pos[3 * j + 2], 0.f);
     mnrm[j] = make_float4(lay->marker_nrm[3 * j], lay->marker_nrm[3 * j + 1], lay->marker_nrm[3 * j + 2], 0.f);
   }
-  c->T = T; c->P = (int)pts.size(); c->M = M;
-  c->nh = !cfg->noise_enable ? 0 : (cfg->hyst_mode == TS_HYST_MAXWELL ? 6 : (cfg->hyst_mode == TS_HYST_ASYM ? 3 : 0));
+  c->T = T; c->P = (int)pts.size(); c->M = M; c->G = (int)groups.size(); c->Tp = (T + 31) / 32 * 32;
+  c->frames_per_group = fpg;
+  c->nh = !cfg->noise_enable ? 0 : (cfg->hyst_mode == TS_HYST_MAXWELL ? 12 : (cfg->hyst_mode == TS_HYST_ASYM ? 6 : 0));
   c->dead_thr = (uint32_t)std::floor((double)cfg->p_dead * 4294967296.0);
+  {
+    TsStepParams sp;
+    fill_params(c, sp);
+    const unsigned long long smem = ts_step_smem_bytes(sp);
+    if (smem > 200 * 1024) { delete c; return fail(nullptr, TS_ERR_UNSUPPORTED, "ts_create: objs_per_env too large for the shared-memory frames"); }
+    const cudaError_t ea = (cudaError_t)ts_prepare_kernels((int)smem);
+    if (ea != cudaSuccess) { ts_status s_ = cuda_fail(nullptr, ea, "cudaFuncSetAttribute"); delete c; return s_; }
+  }
 
-  const size_t E = (size_t)cfg->n_envs, EK = E * cfg->objs_per_env, EP = E * c->P;
+  const size_t E = (size_t)cfg->n_envs, EK = E * cfg->objs_per_env;
 #define TS_ALLOC(ptr, bytes)                                                          \
   do {                                                                                \
     cudaError_t e_ = cudaMalloc((void**)&(ptr), (bytes));                             \
@@ -196,26 +297,38 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   } while (0)
   TS_ALLOC(c->tx_pos, sizeof(float4) * T);
   TS_ALLOC(c->tx_nrm, sizeof(float4) * T);
+  TS_ALLOC(c->tx_nbr, sizeof(int4) * T);
   TS_ALLOC(c->mk_pos, sizeof(float4) * mpos.size());
   TS_ALLOC(c->mk_nrm, sizeof(float4) * mnrm.size());
   TS_ALLOC(c->patches, sizeof(TsPatch) * pts.size());
+  TS_ALLOC(c->groups, sizeof(TsGroup) * groups.size());
+  TS_ALLOC(c->chunks, sizeof(TsChunk) * chunks.size());
+  TS_ALLOC(c->mk_item1, sizeof(int32_t) * item1.size());
+  TS_ALLOC(c->mk_item2, sizeof(int32_t) * item2.size());
+  TS_ALLOC(c->mk_tab, sizeof(double) * tab.size());
   TS_ALLOC(c->g_type, sizeof(int32_t) * EK);
   TS_ALLOC(c->g_params, sizeof(float4) * EK);
   TS_ALLOC(c->st_flags, E * T);
   TS_ALLOC(c->reset_step, sizeof(uint32_t) * E);
   TS_ALLOC(c->episode, sizeof(uint32_t) * E);
   if (cfg->noise_enable) {
-    if (c->nh) TS_ALLOC(c->st_hyst, sizeof(float4) * EP * c->nh * 32);
-    TS_ALLOC(c->st_drift, sizeof(float4) * EP * 3 * 32);
+    if (c->nh) TS_ALLOC(c->st_hyst, sizeof(float) * E * c->nh * c->Tp);
+    TS_ALLOC(c->st_drift, sizeof(float) * E * 6 * c->Tp);
   }
 #undef TS_ALLOC
   cudaError_t e = cudaSuccess;
   auto cp = [&](void* d, const void* h, size_t b) { if (e == cudaSuccess) e = cudaMemcpy(d, h, b, cudaMemcpyHostToDevice); };
   cp(c->tx_pos, pos.data(), sizeof(float4) * T);
   cp(c->tx_nrm, nrm.data(), sizeof(float4) * T);
+  cp(c->tx_nbr, nbr.data(), sizeof(int4) * T);
   cp(c->mk_pos, mpos.data(), sizeof(float4) * mpos.size());
   cp(c->mk_nrm, mnrm.data(), sizeof(float4) * mnrm.size());
   cp(c->patches, pts.data(), sizeof(TsPatch) * pts.size());
+  cp(c->groups, groups.data(), sizeof(TsGroup) * groups.size());
+  cp(c->chunks, chunks.data(), sizeof(TsChunk) * chunks.size());
+  cp(c->mk_item1, item1.data(), sizeof(int32_t) * item1.size());
+  cp(c->mk_item2, item2.data(), sizeof(int32_t) * item2.size());
+  cp(c->mk_tab, tab.data(), sizeof(double) * tab.size());
   if (e == cudaSuccess) e = cudaMemset(c->g_type, 0, sizeof(int32_t) * EK);
   if (e == cudaSuccess) e = cudaMemset(c->g_params, 0, sizeof(float4) * EK);
   if (e == cudaSuccess) e = cudaMemset(c->reset_step, 0, sizeof(uint32_t) * E);

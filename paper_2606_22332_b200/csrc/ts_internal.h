@@ -10,11 +10,14 @@
 
 #include "../../include/ts.h"
 
-#define TS_MAX_PATCH_TAXELS 64  // one warp owns a patch: 2 taxel slots per lane
+#define TS_MAX_PATCH_TAXELS 64   // taxels (and markers) per patch
+#define TS_BLOCK 256             // threads per block = taxel slots per patch group
+#define TS_MAX_GROUP_PATCHES 32  // patches per group
 
 struct ts_layout {
   bool finalized = false;
   int n_taxels = 0;
+  std::vector<ts_patch_desc> desc;  // as given to ts_layout_add_patch
   std::vector<float> pos, nrm, radius, radius_cfg;
   std::vector<int32_t> link, patch, nbr;
   std::vector<int32_t> patch_start, patch_nu, patch_nv, patch_link, marker_start, marker_count;
@@ -23,35 +26,61 @@ struct ts_layout {
   std::vector<int32_t> marker_patch;
 };
 
-// Device-side patch record (two 16-byte loads per warp).
+// Device-side patch record (96 bytes).
 struct TsPatch {
   int32_t start;   // first taxel slot
-  int32_t n;       // taxel slots in the patch (<= 64)
-  int32_t nu;      // grid width (u fastest); fillers: nu = n
+  int32_t n;       // taxel slots in the patch
+  int32_t nu, nv;  // taxel grid (u fastest); fillers: nu = n, nv = 1
   int32_t link;    // sensor link, -1 = filler patch (all slots inactive)
   int32_t mstart;  // first marker
-  int32_t mcount;  // markers (<= 64)
+  int32_t mnu, mnv;  // marker grid (0 = none)
   float eps;       // Eq. 20 epsilon
-  int32_t pad;
+  int32_t tab;     // offset (doubles) of this patch's separable tables in mk_tab
+  int32_t i1off;   // first pass-1 item of this patch (index into mk_item1)
+  int32_t direct;  // 1 = direct (non-separable) marker sum
+  float4 ua, va, na;  // u axis, v axis, normal (link frame)
+};
+
+// A group = consecutive patches whose taxel slots fit one block.
+struct TsGroup {
+  int32_t start, count;    // taxel slots [start, start + count)
+  int32_t patch0, npatch;  // patches [patch0, patch0 + npatch)
+  int32_t chunk0, nchunk;  // marker chunks [chunk0, chunk0 + nchunk)
+  int32_t mstart, mcount;  // markers of the group (contiguous)
+};
+
+// A marker chunk = consecutive patches of one group whose pass-1 items and markers fit one block.
+struct TsChunk {
+  int32_t i1_begin, i1_end;  // pass-1 items (a, q) in mk_item1
+  int32_t m_begin, m_end;    // markers (pass-2 items) in mk_item2
+  int32_t lp_begin, lp_end;  // group-local patch range
+  int32_t pad0, pad1;
 };
 
 // Kernel parameters of one step (passed by value).
 struct TsStepParams {
-  int32_t E, L, K, T, P, M;
+  int32_t E, L, K, T, P, M, G, Tp;
+  int32_t frames_per_group;  // max patches per group (shared-memory frames = this * K)
   uint32_t env_id_base;
   // layout
-  const float4* tx_pos;  // [T] (x, y, z, R_j)
-  const float4* tx_nrm;  // [T] (nx, ny, nz, 0)
-  const TsPatch* patches;  // [P]
-  const float4* mk_pos;  // [M]
-  const float4* mk_nrm;  // [M]
+  const float4* tx_pos;   // [T] (x, y, z, R_j); R_j = 0 for every inactive slot
+  const float4* tx_nrm;   // [T] (nx, ny, nz, bits: group-local patch index)
+  const int4* tx_nbr;     // [T] neighbour slots (-u,+u,-v,+v), -1 = none
+  const TsPatch* patches; // [P]
+  const TsGroup* groups;  // [G]
+  const TsChunk* chunks;
+  const int32_t* mk_item1;  // packed lp | a << 8 | q << 16
+  const int32_t* mk_item2;  // [M] packed lp | a << 8 | b << 16
+  const double* mk_tab;     // per patch: GU[mnu][nu], DU[mnu][nu], GV[mnv][nv], DV[mnv][nv]
+  const float4* mk_pos;   // [M]
+  const float4* mk_nrm;   // [M]
   // geometry
   const int32_t* g_type;   // [E,K]
   const float4* g_params;  // [E,K]
   const float4* bank;      // re-tiled SDF bank (see ts_kernels.cu, "bank layout")
   int32_t grid_n;
-  float voxel, inv_voxel, grid_origin;
-  double inv_voxel_d;  // 1 / (double)voxel, for the fp64 first query
+  float voxel, inv_voxel;
+  double inv_voxel_d;      // 1 / (double)voxel
   unsigned long long grid_stride;  // float4 elements per grid
   // inputs
   const float *link_pos, *link_quat, *link_linvel, *link_angvel;
@@ -66,15 +95,16 @@ struct TsStepParams {
   uint8_t* dead;
   // state
   uint8_t* st_flags;          // [E,T] bit0 Schmitt, bit1 dead
-  float4* st_hyst;            // [E,P,nh,32] float4, nh = 3 (asym) / 6 (maxwell)
-  float4* st_drift;           // [E,P,3,32] float4
+  float* st_hyst;             // [E,nh,Tp], nh = 6 (asym: y) / 12 (maxwell: xi then x_prev)
+  float* st_drift;            // [E,6,Tp]
   const uint32_t* reset_step; // [E]
   const uint32_t* episode;    // [E]
   uint32_t gstep;
   // physics
   float k_n, c_n, alpha, k_t, k_omega, mu, eta_on, eta_off;
   int32_t use_velocity;
-  float s_d, lambda_d, alpha_e, c_e, inv_gbar;
+  float s_d, lambda_d, alpha_e, c_e;
+  double inv_gbar;            // 1 / g_bar = sqrt(2 lambda_d) e^{1/2}
   float r_prox;
   int32_t march_steps;
   // noise
@@ -90,5 +120,7 @@ int ts_launch_reset_counters(uint32_t* reset_step, uint32_t* episode, const uint
                              void* stream);
 int ts_launch_reset_state(const TsStepParams& p, const uint8_t* mask, uint32_t dead_threshold, int nh, void* stream);
 unsigned long long ts_bank_elems_per_grid(int N);
+unsigned long long ts_step_smem_bytes(const TsStepParams& p);
+int ts_prepare_kernels(int max_smem_bytes);
 
 #endif  // TS_INTERNAL_H_

@@ -1,11 +1,24 @@
 // Hand-written sm_100a kernels of the batched tactile readout.  Citations: "P:NNN" = line of
 // the paper text (App. A = P:172-359); "D*/Q*/O*" = readings listed in DESIGN.md.
 //
-// Mapping: ONE WARP PER (environment, patch).  A patch has <= 64 taxel slots; lane l owns the
-// two consecutive slots i = 2l and 2l+1 (so every per-taxel stream is read/written as one
-// 8-, 16- or 48-byte vector per lane) and the two markers l and l+32.  The link pose, the
-// link->object transform and the velocity terms are warp-uniform; crosstalk neighbours are
-// fetched with __shfl_sync, marker sources are broadcast with __shfl_sync.
+// Mapping: ONE THREAD PER (environment, taxel slot); a block owns one "patch group" of one
+// environment: up to TS_BLOCK consecutive taxel slots made of whole patches (packed on the
+// host, ts_api.cu).  Per block:
+//   phase 0  threads < npatch*K build the relative pose of every (patch link, object) pair in
+//            DOUBLE and park it in shared memory (frames);
+//   phase 1  per taxel: x_o = c + M x_j (double), phi (double), depth, Schmitt contact bit;
+//   phase 2  proximity march along a_j (fp32; evaluation 0 is the phase-1 query);
+//   phase 3  kinematic force/torque in double for warps that touch anything, rounded once;
+//   phase 4  noise chain: hysteresis -> crosstalk (neighbours through shared memory) ->
+//            Philox/Box-Muller random-walk drift -> dead taxels;
+//   phase 5  elastomer marker dilation as two separable passes over shared memory (double).
+// [E,T,6] and [E,M,3] outputs are staged in shared memory and written as coalesced float4.
+//
+// Why double in phases 0/1/3/5: outputs are compared element by
+// element at rtol 1e-4 / atol 1e-6.  d = R - phi feeds f ~ d^1.2, the marker sum multiplies
+// h = -phi by s_d = 100 over up to 64 sources, and a small component of a 3 N force needs the
+// contact normal to ~1e-7.  fp32 positions (ulp 4e-9 m at 5 cm) give neither.  B200 issues DFMA
+// at half the FFMA rate; the double chain is ~250 instructions per touching taxel.
 //
 // Bank layout ("quad"): for every grid, Q[(j*(N-1) + i)*N + k] = float4(phi(i,j,k), phi(i+1,j,k),
 // phi(i,j+1,k), phi(i+1,j+1,k)), i,j in [0,N-2], k in [0,N-1].  The 8 corners of cell (i,j,k) are
@@ -17,185 +30,289 @@
 
 #include "ts_internal.h"
 
-#define TS_BLOCK 128
-
 namespace {
 
 struct F3 {
   float x, y, z;
+};
+struct D3 {
+  double x, y, z;
 };
 __device__ __forceinline__ F3 mk3(float x, float y, float z) { return F3{x, y, z}; }
 __device__ __forceinline__ F3 operator+(F3 a, F3 b) { return F3{a.x + b.x, a.y + b.y, a.z + b.z}; }
 __device__ __forceinline__ F3 operator-(F3 a, F3 b) { return F3{a.x - b.x, a.y - b.y, a.z - b.z}; }
 __device__ __forceinline__ F3 operator*(float s, F3 a) { return F3{s * a.x, s * a.y, s * a.z}; }
 __device__ __forceinline__ float dot(F3 a, F3 b) { return fmaf(a.x, b.x, fmaf(a.y, b.y, a.z * b.z)); }
-__device__ __forceinline__ F3 cross(F3 a, F3 b) {
-  return F3{a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
-}
-__device__ __forceinline__ F3 ld3(const float* p) { return F3{__ldg(p), __ldg(p + 1), __ldg(p + 2)}; }
 
-struct Rot {  // row-major 3x3
-  float a[9];
-};
-__device__ __forceinline__ F3 mul(const Rot& R, F3 v) {
-  return F3{fmaf(R.a[0], v.x, fmaf(R.a[1], v.y, R.a[2] * v.z)), fmaf(R.a[3], v.x, fmaf(R.a[4], v.y, R.a[5] * v.z)),
-            fmaf(R.a[6], v.x, fmaf(R.a[7], v.y, R.a[8] * v.z))};
+__device__ __forceinline__ D3 operator+(D3 a, D3 b) { return D3{a.x + b.x, a.y + b.y, a.z + b.z}; }
+__device__ __forceinline__ D3 operator-(D3 a, D3 b) { return D3{a.x - b.x, a.y - b.y, a.z - b.z}; }
+__device__ __forceinline__ D3 operator*(double s, D3 a) { return D3{s * a.x, s * a.y, s * a.z}; }
+__device__ __forceinline__ double dot(D3 a, D3 b) { return fma(a.x, b.x, fma(a.y, b.y, a.z * b.z)); }
+__device__ __forceinline__ D3 cross(D3 a, D3 b) {
+  return D3{fma(a.y, b.z, -a.z * b.y), fma(a.z, b.x, -a.x * b.z), fma(a.x, b.y, -a.y * b.x)};
 }
-__device__ __forceinline__ F3 mulT(const Rot& R, F3 v) {
-  return F3{fmaf(R.a[0], v.x, fmaf(R.a[3], v.y, R.a[6] * v.z)), fmaf(R.a[1], v.x, fmaf(R.a[4], v.y, R.a[7] * v.z)),
-            fmaf(R.a[2], v.x, fmaf(R.a[5], v.y, R.a[8] * v.z))};
+__device__ __forceinline__ D3 ld3d(const float* p) { return D3{(double)__ldg(p), (double)__ldg(p + 1), (double)__ldg(p + 2)}; }
+__device__ __forceinline__ D3 ldv(const double* p) { return D3{p[0], p[1], p[2]}; }
+// y = R v, y = R^T v for a row-major 3x3 of doubles
+__device__ __forceinline__ D3 mulR(const double* R, D3 v) {
+  return D3{fma(R[0], v.x, fma(R[1], v.y, R[2] * v.z)), fma(R[3], v.x, fma(R[4], v.y, R[5] * v.z)),
+            fma(R[6], v.x, fma(R[7], v.y, R[8] * v.z))};
+}
+__device__ __forceinline__ D3 mulRT(const double* R, D3 v) {
+  return D3{fma(R[0], v.x, fma(R[3], v.y, R[6] * v.z)), fma(R[1], v.x, fma(R[4], v.y, R[7] * v.z)),
+            fma(R[2], v.x, fma(R[5], v.y, R[8] * v.z))};
 }
 
-// Double-precision twins used ONLY for the relative pose and the first geometry query (DESIGN.md
-// "fp64 frame"): the contact normal of a box edge/corner is max(|x|-b,0)/|.|, a ratio of
-// millimetre differences of centimetre numbers, and the stiff force law amplifies d; with fp32
-// positions (error ~4e-9 m) neither meets rtol 1e-4.  B200 issues DFMA at half the FFMA rate
-// and this is ~60 DFMA per taxel, so the cost hides under the state streams.
-template <typename S>
-struct X3 {
-  S x, y, z;
-};
-typedef X3<double> D3;
-struct RotD {
-  double a[9];
-};
+// sqrt / reciprocal sqrt of a double to ~1e-13 relative: MUFU.RSQ seed + one Newton step in
+// double (a correctly rounded DSQRT costs ~4x more and its last bits are not needed).
+__device__ __forceinline__ double dsqrt_n(double s) {
+  const float sf = (float)s;
+  if (!(sf > 0.f)) return 0.0;
+  const float rs = rsqrtf(sf);
+  const double r0 = (double)(sf * rs);
+  const double e = fma(-r0, r0, s);
+  return fma(e, (double)(0.5f * rs), r0);
+}
+__device__ __forceinline__ double drsqrt_n(double s) {  // s > 0
+  const double y0 = (double)rsqrtf((float)s);
+  const double e = fma(-s * y0, y0, 1.0);
+  return fma(0.5 * y0, e, y0);
+}
+
 // O0: rotation of a quaternion (w,x,y,z), used as given.
-__device__ __forceinline__ RotD quat_Rd(const float* q4) {
+__device__ __forceinline__ void quat_Rd(const float* q4, double* R) {
   const float4 q = __ldg(reinterpret_cast<const float4*>(q4));
   const double w = q.x, x = q.y, y = q.z, z = q.w;
-  RotD R;
-  R.a[0] = 1.0 - 2.0 * (y * y + z * z); R.a[1] = 2.0 * (x * y - w * z);       R.a[2] = 2.0 * (x * z + w * y);
-  R.a[3] = 2.0 * (x * y + w * z);       R.a[4] = 1.0 - 2.0 * (x * x + z * z); R.a[5] = 2.0 * (y * z - w * x);
-  R.a[6] = 2.0 * (x * z - w * y);       R.a[7] = 2.0 * (y * z + w * x);       R.a[8] = 1.0 - 2.0 * (x * x + y * y);
-  return R;
+  R[0] = 1.0 - 2.0 * (y * y + z * z); R[1] = 2.0 * (x * y - w * z);       R[2] = 2.0 * (x * z + w * y);
+  R[3] = 2.0 * (x * y + w * z);       R[4] = 1.0 - 2.0 * (x * x + z * z); R[5] = 2.0 * (y * z - w * x);
+  R[6] = 2.0 * (x * z - w * y);       R[7] = 2.0 * (y * z + w * x);       R[8] = 1.0 - 2.0 * (x * x + y * y);
 }
-__device__ __forceinline__ Rot to_float(const RotD& R) {
-  Rot r;
-#pragma unroll
-  for (int i = 0; i < 9; ++i) r.a[i] = (float)R.a[i];
-  return r;
-}
-__device__ __forceinline__ F3 to_float(const D3& v) { return F3{(float)v.x, (float)v.y, (float)v.z}; }
-__device__ __forceinline__ X3<float> as_x3(F3 v) { return X3<float>{v.x, v.y, v.z}; }
 
-// Object k seen from the sensor link: x_o = c + M x_j (object frame <- link frame).
-// Forming p_L - p_O BEFORE rotating keeps the small relative offsets accurate.
-struct ObjFrame {
-  Rot M;  // R_O^T R_L
-  F3 c;   // R_O^T (p_L - p_O)
+// Relative pose of (sensor link of a patch, object k), in shared memory.  x_o = c + M x_j maps
+// link-frame points to the object frame; p_L - p_O is formed BEFORE rotating.
+struct FrameS {
+  double M[9];     // R_O^T R_L
+  double c[3];     // R_O^T (p_L - p_O)
+  double wO[3];    // R_L^T w_O   (link-frame velocity terms of Eq. 4-6)
+  double wL[3];    // R_L^T w_L
+  double vbar[3];  // R_L^T (v_O - v_L)
+  double cbar[3];  // R_L^T (p_L - p_O)
+  float Mf[9];     // fp32 copies for the march
+  float cf[3];
+  float prm[4];
   int type;
-  float4 prm;
-};
-struct ObjFrameD {
-  RotD M;
-  D3 c;
+  int pad[3];
 };
 
-__device__ __forceinline__ ObjFrame make_frame(const TsStepParams& p, int e, int k, const RotD& RL, D3 pL, ObjFrameD& fd) {
+__device__ void build_frame(const TsStepParams& p, int e, int link, int k, FrameS& F) {
   const size_t ek = (size_t)e * p.K + k;
-  ObjFrame f;
-  f.type = __ldg(p.g_type + ek);
-  f.prm = __ldg(p.g_params + ek);
-  const RotD RO = quat_Rd(p.obj_quat + ek * 4);
-  const double dx = pL.x - (double)__ldg(p.obj_pos + ek * 3), dy = pL.y - (double)__ldg(p.obj_pos + ek * 3 + 1),
-               dz = pL.z - (double)__ldg(p.obj_pos + ek * 3 + 2);
+  F.type = (link >= 0) ? __ldg(p.g_type + ek) : TS_GEOM_NONE;
+  const float4 prm = __ldg(p.g_params + ek);
+  F.prm[0] = prm.x; F.prm[1] = prm.y; F.prm[2] = prm.z; F.prm[3] = prm.w;
+  if (link < 0) return;
+  const size_t el = (size_t)e * p.L + link;
+  double RL[9], RO[9];
+  quat_Rd(p.link_quat + el * 4, RL);
+  quat_Rd(p.obj_quat + ek * 4, RO);
+  const D3 d = ld3d(p.link_pos + el * 3) - ld3d(p.obj_pos + ek * 3);
 #pragma unroll
   for (int r = 0; r < 3; ++r)
 #pragma unroll
-    for (int c = 0; c < 3; ++c)
-      fd.M.a[r * 3 + c] = fma(RO.a[r], RL.a[c], fma(RO.a[3 + r], RL.a[3 + c], RO.a[6 + r] * RL.a[6 + c]));
-  fd.c.x = fma(RO.a[0], dx, fma(RO.a[3], dy, RO.a[6] * dz));
-  fd.c.y = fma(RO.a[1], dx, fma(RO.a[4], dy, RO.a[7] * dz));
-  fd.c.z = fma(RO.a[2], dx, fma(RO.a[5], dy, RO.a[8] * dz));
-  f.M = to_float(fd.M);
-  f.c = to_float(fd.c);
-  return f;
-}
-__device__ __forceinline__ D3 mul(const ObjFrameD& f, F3 v) {
-  const double x = v.x, y = v.y, z = v.z;
-  return D3{fma(f.M.a[0], x, fma(f.M.a[1], y, fma(f.M.a[2], z, f.c.x))), fma(f.M.a[3], x, fma(f.M.a[4], y, fma(f.M.a[5], z, f.c.y))),
-            fma(f.M.a[6], x, fma(f.M.a[7], y, fma(f.M.a[8], z, f.c.z)))};
+    for (int c = 0; c < 3; ++c) {
+      const double m = fma(RO[r], RL[c], fma(RO[3 + r], RL[3 + c], RO[6 + r] * RL[6 + c]));
+      F.M[r * 3 + c] = m;
+      F.Mf[r * 3 + c] = (float)m;
+    }
+  const D3 c = mulRT(RO, d), cb = mulRT(RL, d);
+  F.c[0] = c.x; F.c[1] = c.y; F.c[2] = c.z;
+  F.cf[0] = (float)c.x; F.cf[1] = (float)c.y; F.cf[2] = (float)c.z;
+  F.cbar[0] = cb.x; F.cbar[1] = cb.y; F.cbar[2] = cb.z;
+  const D3 wO = mulRT(RL, ld3d(p.obj_angvel + ek * 3)), wL = mulRT(RL, ld3d(p.link_angvel + el * 3));
+  const D3 vb = mulRT(RL, ld3d(p.obj_linvel + ek * 3) - ld3d(p.link_linvel + el * 3));
+  F.wO[0] = wO.x; F.wO[1] = wO.y; F.wO[2] = wO.z;
+  F.wL[0] = wL.x; F.wL[1] = wL.y; F.wL[2] = wL.z;
+  F.vbar[0] = vb.x; F.vbar[1] = vb.y; F.vbar[2] = vb.z;
 }
 
 // ---------------------------------------------------------------------------------------
-// O2: signed distance (and object-frame gradient) of one geometry at object-frame point x.
+// O2 in double: signed distance and (unnormalised, object-frame) gradient of one geometry at
+// the object-frame point x.  Used once per taxel (the first query).
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ float inv_vox(const TsStepParams& p, float) { return p.inv_voxel; }
-__device__ __forceinline__ double inv_vox(const TsStepParams& p, double) { return p.inv_voxel_d; }
-__device__ __forceinline__ float fma_s(float a, float b, float c) { return fmaf(a, b, c); }
-__device__ __forceinline__ double fma_s(double a, double b, double c) { return fma(a, b, c); }
+struct CellD {  // trilinear cell around x: corners, in-cell fractions, outside-grid offset (voxels)
+  float4 A, B;  // (c000,c100,c010,c110), (c001,c101,c011,c111)
+  double fx, fy, fz;
+  double ox, oy, oz;
+  bool outside;
+};
 
-// S = double for the first query (cell index and fractions exact to fp32 rounding), float in the march.
-template <bool GRAD, typename S>
-__device__ __forceinline__ float sdf_grid(const TsStepParams& p, int gid, X3<S> x, F3& g) {
-  const int N = p.grid_n;
-  const S top = (S)(N - 1);
-  const S half = (S)0.5 * top;
-  const S iv = inv_vox(p, S());
-  const S ux = fma_s(x.x, iv, half), uy = fma_s(x.y, iv, half), uz = fma_s(x.z, iv, half);
-  const S cx = min(max(ux, (S)0), top), cy = min(max(uy, (S)0), top), cz = min(max(uz, (S)0), top);
-  const int i0 = min((int)cx, N - 2), j0 = min((int)cy, N - 2), k0 = min((int)cz, N - 2);
-  const float fx = (float)(cx - (S)i0), fy = (float)(cy - (S)j0), fz = (float)(cz - (S)k0);
-  const float4* q = p.bank + (size_t)gid * p.grid_stride + ((size_t)(j0 * (N - 1) + i0) * N + k0);
-  const float4 A = __ldg(q), B = __ldg(q + 1);  // (c000,c100,c010,c110), (c001,c101,c011,c111)
-  const float a0 = fmaf(fx, A.y - A.x, A.x), a1 = fmaf(fx, A.w - A.z, A.z);
-  const float b0 = fmaf(fx, B.y - B.x, B.x), b1 = fmaf(fx, B.w - B.z, B.z);
-  const float lo = fmaf(fy, a1 - a0, a0), hi = fmaf(fy, b1 - b0, b0);
-  float phi = fmaf(fz, hi - lo, lo);
-  const float ox = (float)(ux - cx), oy = (float)(uy - cy), oz = (float)(uz - cz);   // outside-grid extension (O2)
-  const float o2 = fmaf(ox, ox, fmaf(oy, oy, oz * oz));
-  if (o2 > 0.f) phi += p.voxel * sqrtf(o2);
-  if (GRAD) {  // exact derivative of the trilinear interpolant in cell (i0,j0,k0); 1/h_v dropped (normalised later)
-    const float gy0 = 1.f - fy, gz0 = 1.f - fz;
-    const float dxa = fmaf(fy, A.w - A.z, gy0 * (A.y - A.x)), dxb = fmaf(fy, B.w - B.z, gy0 * (B.y - B.x));
-    g.x = fmaf(fz, dxb, gz0 * dxa);
-    g.y = fmaf(fz, b1 - b0, gz0 * (a1 - a0));
-    g.z = hi - lo;
+__device__ __forceinline__ void clamp01(double& f, double& o, bool& outside) {
+  const float ff = (float)f;
+  o = 0.0;
+  if (ff < 0.f || ff > 1.f) {  // outside the grid on this axis (O2 extension); rare
+    const double c = ff < 0.f ? 0.0 : 1.0;
+    o = f - c;
+    f = c;
+    outside = true;
   }
+}
+
+__device__ __forceinline__ void grid_cell_d(const TsStepParams& p, int gid, D3 x, CellD& C) {
+  const int N = p.grid_n;
+  const double half = 0.5 * (double)(N - 1);
+  const double ux = fma(x.x, p.inv_voxel_d, half), uy = fma(x.y, p.inv_voxel_d, half), uz = fma(x.z, p.inv_voxel_d, half);
+  // cell index from the fp32 image of u: a one-ulp slip across a face only moves the (continuous)
+  // interpolant by ~1e-11 m and lands in the comparator's voxel-face band for the gradient.
+  const int i0 = min(max(__float2int_rd((float)ux), 0), N - 2);
+  const int j0 = min(max(__float2int_rd((float)uy), 0), N - 2);
+  const int k0 = min(max(__float2int_rd((float)uz), 0), N - 2);
+  C.fx = ux - (double)i0; C.fy = uy - (double)j0; C.fz = uz - (double)k0;
+  C.outside = false;
+  clamp01(C.fx, C.ox, C.outside);
+  clamp01(C.fy, C.oy, C.outside);
+  clamp01(C.fz, C.oz, C.outside);
+  const float4* q = p.bank + (size_t)gid * p.grid_stride + ((size_t)(j0 * (N - 1) + i0) * N + k0);
+  C.A = __ldg(q);
+  C.B = __ldg(q + 1);
+}
+
+__device__ __forceinline__ double grid_value_d(const TsStepParams& p, const CellD& C) {
+  const double c000 = C.A.x, c100 = C.A.y, c010 = C.A.z, c110 = C.A.w;
+  const double c001 = C.B.x, c101 = C.B.y, c011 = C.B.z, c111 = C.B.w;
+  const double a0 = fma(C.fx, c100 - c000, c000), a1 = fma(C.fx, c110 - c010, c010);
+  const double b0 = fma(C.fx, c101 - c001, c001), b1 = fma(C.fx, c111 - c011, c011);
+  const double lo = fma(C.fy, a1 - a0, a0), hi = fma(C.fy, b1 - b0, b0);
+  double phi = fma(C.fz, hi - lo, lo);
+  if (C.outside) phi += (double)p.voxel * dsqrt_n(fma(C.ox, C.ox, fma(C.oy, C.oy, C.oz * C.oz)));
   return phi;
 }
 
-template <bool GRAD, typename S>
-__device__ __forceinline__ float sdf_eval(const TsStepParams& p, const ObjFrame& f, X3<S> xs, F3& g) {
-  const F3 x = mk3((float)xs.x, (float)xs.y, (float)xs.z);
-  switch (f.type) {
-    case TS_GEOM_SPHERE: {
-      const float n = sqrtf(dot(x, x));
-      if (GRAD) g = (n < 1e-12f) ? mk3(0.f, 0.f, 1.f) : (1.f / n) * x;
-      return n - f.prm.x;
-    }
-    case TS_GEOM_BOX: {  // w = |x| - b formed in S: the edge/corner normal is a ratio of these small differences
-      const float wx = (float)(abs(xs.x) - (S)f.prm.x), wy = (float)(abs(xs.y) - (S)f.prm.y), wz = (float)(abs(xs.z) - (S)f.prm.z);
-      const float px = fmaxf(wx, 0.f), py = fmaxf(wy, 0.f), pz = fmaxf(wz, 0.f);
-      const float lp = sqrtf(fmaf(px, px, fmaf(py, py, pz * pz)));
-      const float wmax = fmaxf(wx, fmaxf(wy, wz));
-      if (GRAD) {
-        const float sx = x.x < 0.f ? -1.f : 1.f, sy = x.y < 0.f ? -1.f : 1.f, sz = x.z < 0.f ? -1.f : 1.f;
-        if (wmax > 0.f) {
-          const float il = 1.f / lp;
-          g = mk3(sx * px * il, sy * py * il, sz * pz * il);
-        } else {  // interior: axis of the largest w, ties -> lowest index (Q7)
-          g = mk3(0.f, 0.f, 0.f);
-          if (wx >= wy && wx >= wz) g.x = sx;
-          else if (wy >= wz) g.y = sy;
-          else g.z = sz;
-        }
-      }
-      return lp + fminf(wmax, 0.f);
+// exact derivative of the trilinear interpolant in the cell; the common factor 1/h_v is dropped
+__device__ __forceinline__ D3 grid_grad_d(const CellD& C) {
+  const double c000 = C.A.x, c100 = C.A.y, c010 = C.A.z, c110 = C.A.w;
+  const double c001 = C.B.x, c101 = C.B.y, c011 = C.B.z, c111 = C.B.w;
+  const double a0 = fma(C.fx, c100 - c000, c000), a1 = fma(C.fx, c110 - c010, c010);
+  const double b0 = fma(C.fx, c101 - c001, c001), b1 = fma(C.fx, c111 - c011, c011);
+  const double lo = fma(C.fy, a1 - a0, a0), hi = fma(C.fy, b1 - b0, b0);
+  const double gy0 = 1.0 - C.fy, gz0 = 1.0 - C.fz;
+  const double dxa = fma(C.fy, c110 - c010, gy0 * (c100 - c000)), dxb = fma(C.fy, c111 - c011, gy0 * (c101 - c001));
+  return D3{fma(C.fz, dxb, gz0 * dxa), fma(C.fz, b1 - b0, gz0 * (a1 - a0)), hi - lo};
+}
+
+__device__ __forceinline__ double phi_d(const TsStepParams& p, int type, const float* prm, D3 x) {
+  switch (type) {
+    case TS_GEOM_SPHERE:
+      return dsqrt_n(dot(x, x)) - (double)prm[0];
+    case TS_GEOM_BOX: {
+      const double wx = fabs(x.x) - (double)prm[0], wy = fabs(x.y) - (double)prm[1], wz = fabs(x.z) - (double)prm[2];
+      const double px = fmax(wx, 0.0), py = fmax(wy, 0.0), pz = fmax(wz, 0.0);
+      return dsqrt_n(fma(px, px, fma(py, py, pz * pz))) + fmin(fmax(wx, fmax(wy, wz)), 0.0);
     }
     case TS_GEOM_CAPSULE: {
-      const float zc = fminf(fmaxf(x.z, -f.prm.y), f.prm.y);
-      const F3 y = mk3(x.x, x.y, x.z - zc);
-      const float n = sqrtf(dot(y, y));
-      if (GRAD) g = (n < 1e-12f) ? mk3(0.f, 0.f, 1.f) : (1.f / n) * y;
-      return n - f.prm.x;
+      const double h = (double)prm[1];
+      const double zc = fmin(fmax(x.z, -h), h);
+      const D3 y = D3{x.x, x.y, x.z - zc};
+      return dsqrt_n(dot(y, y)) - (double)prm[0];
     }
-    case TS_GEOM_SDF:
-      return sdf_grid<GRAD, S>(p, (int)f.prm.x, xs, g);
+    case TS_GEOM_SDF: {
+      CellD C;
+      grid_cell_d(p, (int)prm[0], x, C);
+      return grid_value_d(p, C);
+    }
     default:
-      if (GRAD) g = mk3(0.f, 0.f, 1.f);
+      return __longlong_as_double(0x7ff0000000000000LL);
+  }
+}
+
+// unnormalised gradient; the zero vector flags a singular point (Q2/Q7 handled by the caller)
+__device__ __forceinline__ D3 grad_d(const TsStepParams& p, int type, const float* prm, D3 x) {
+  switch (type) {
+    case TS_GEOM_SPHERE:
+      return dot(x, x) < 1e-24 ? D3{0.0, 0.0, 1.0} : x;
+    case TS_GEOM_BOX: {
+      const double wx = fabs(x.x) - (double)prm[0], wy = fabs(x.y) - (double)prm[1], wz = fabs(x.z) - (double)prm[2];
+      const double sx = x.x < 0.0 ? -1.0 : 1.0, sy = x.y < 0.0 ? -1.0 : 1.0, sz = x.z < 0.0 ? -1.0 : 1.0;
+      if (fmax(wx, fmax(wy, wz)) > 0.0) return D3{sx * fmax(wx, 0.0), sy * fmax(wy, 0.0), sz * fmax(wz, 0.0)};
+      if (wx >= wy && wx >= wz) return D3{sx, 0.0, 0.0};  // interior: axis of the largest w, ties -> lowest index (Q7)
+      if (wy >= wz) return D3{0.0, sy, 0.0};
+      return D3{0.0, 0.0, sz};
+    }
+    case TS_GEOM_CAPSULE: {
+      const double h = (double)prm[1];
+      const double zc = fmin(fmax(x.z, -h), h);
+      const D3 y = D3{x.x, x.y, x.z - zc};
+      return dot(y, y) < 1e-24 ? D3{0.0, 0.0, 1.0} : y;
+    }
+    case TS_GEOM_SDF: {
+      CellD C;
+      grid_cell_d(p, (int)prm[0], x, C);
+      return grid_grad_d(C);
+    }
+    default:
+      return D3{0.0, 0.0, 0.0};
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// O2 in fp32, value only: the march evaluations (prox tolerance 1e-6 m; fp32 gives ~1e-8).
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ float trilerp(float4 A, float4 B, float fx, float fy, float fz) {
+  const float a0 = fmaf(fx, A.y - A.x, A.x), a1 = fmaf(fx, A.w - A.z, A.z);
+  const float b0 = fmaf(fx, B.y - B.x, B.x), b1 = fmaf(fx, B.w - B.z, B.z);
+  const float lo = fmaf(fy, a1 - a0, a0), hi = fmaf(fy, b1 - b0, b0);
+  return fmaf(fz, hi - lo, lo);
+}
+
+// general point (clamps + outside-grid extension); u = voxel coordinates
+__device__ __forceinline__ float grid_value_f(const TsStepParams& p, const float4* bank_g, F3 u) {
+  const int N = p.grid_n;
+  const float top = (float)(N - 1);
+  const float cx = fminf(fmaxf(u.x, 0.f), top), cy = fminf(fmaxf(u.y, 0.f), top), cz = fminf(fmaxf(u.z, 0.f), top);
+  const int i0 = min((int)cx, N - 2), j0 = min((int)cy, N - 2), k0 = min((int)cz, N - 2);
+  const float4* q = bank_g + ((size_t)(j0 * (N - 1) + i0) * N + k0);
+  float phi = trilerp(__ldg(q), __ldg(q + 1), cx - (float)i0, cy - (float)j0, cz - (float)k0);
+  const float ox = u.x - cx, oy = u.y - cy, oz = u.z - cz;
+  const float o2 = fmaf(ox, ox, fmaf(oy, oy, oz * oz));
+  if (o2 > 0.f) phi += p.voxel * sqrtf(o2);
+  return phi;
+}
+
+// interior point, um = u - 0.5 with u in [0.75, N-1.75]: floor and fraction by the 1.5*2^23 trick
+// (FADDs on the FMA pipe instead of F2I/I2F on the quarter-rate conversion pipe).
+__device__ __forceinline__ float grid_value_fast(const float4* bank_g, int N, F3 um) {
+  const float MAGIC = 12582912.f;  // 1.5 * 2^23
+  const float tx = um.x + MAGIC, ty = um.y + MAGIC, tz = um.z + MAGIC;
+  const int i0 = __float_as_int(tx) - 0x4B400000, j0 = __float_as_int(ty) - 0x4B400000, k0 = __float_as_int(tz) - 0x4B400000;
+  const float fx = (um.x - (tx - MAGIC)) + 0.5f, fy = (um.y - (ty - MAGIC)) + 0.5f, fz = (um.z - (tz - MAGIC)) + 0.5f;
+  const float4* q = bank_g + ((j0 * (N - 1) + i0) * N + k0);
+  return trilerp(__ldg(q), __ldg(q + 1), fx, fy, fz);
+}
+
+__device__ __forceinline__ float prim_value_f(int type, const float* prm, F3 x) {
+  switch (type) {
+    case TS_GEOM_SPHERE:
+      return sqrtf(dot(x, x)) - prm[0];
+    case TS_GEOM_BOX: {
+      const float wx = fabsf(x.x) - prm[0], wy = fabsf(x.y) - prm[1], wz = fabsf(x.z) - prm[2];
+      const float px = fmaxf(wx, 0.f), py = fmaxf(wy, 0.f), pz = fmaxf(wz, 0.f);
+      return sqrtf(fmaf(px, px, fmaf(py, py, pz * pz))) + fminf(fmaxf(wx, fmaxf(wy, wz)), 0.f);
+    }
+    case TS_GEOM_CAPSULE: {
+      const float zc = fminf(fmaxf(x.z, -prm[1]), prm[1]);
+      const F3 y = mk3(x.x, x.y, x.z - zc);
+      return sqrtf(dot(y, y)) - prm[0];
+    }
+    default:
       return __int_as_float(0x7f800000);
   }
+}
+
+__device__ __forceinline__ float phi_f(const TsStepParams& p, int type, const float* prm, F3 x) {
+  if (type == TS_GEOM_SDF) {
+    const float half = 0.5f * (float)(p.grid_n - 1);
+    const F3 u = mk3(fmaf(x.x, p.inv_voxel, half), fmaf(x.y, p.inv_voxel, half), fmaf(x.z, p.inv_voxel, half));
+    return grid_value_f(p, p.bank + (size_t)(int)prm[0] * p.grid_stride, u);
+  }
+  return prim_value_f(type, prm, x);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -204,442 +321,408 @@ __device__ __forceinline__ float sdf_eval(const TsStepParams& p, const ObjFrame&
 __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1) {
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
-    const uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
-    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
-    c = make_uint4(hi1 ^ c.y ^ k0, lo1, hi0 ^ c.w ^ k1, lo0);
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c.x, p1 = (uint64_t)0xCD9E8D57u * c.z;
+    c = make_uint4((uint32_t)(p1 >> 32) ^ c.y ^ k0, (uint32_t)p1, (uint32_t)(p0 >> 32) ^ c.w ^ k1, (uint32_t)p0);
     k0 += 0x9E3779B9u;
     k1 += 0xBB67AE85u;
   }
   return c;
 }
-// u = (2 (w >> 9) + 1) 2^-24: exact in fp32, never 0 or 1.
-__device__ __forceinline__ float u01(uint32_t w) { return (float)(2u * (w >> 9) + 1u) * 5.9604644775390625e-8f; }
+
+// Box-Muller on a word pair (O8): u = (2 (w >> 9) + 1) 2^-24 (exact in fp32, never 0 or 1),
+// z0 = sqrt(-2 ln u_a) cos(2 pi u_b), z1 = ... sin(...).
+//  * -2 ln u_a: MUFU.LG2 has an ABSOLUTE error of ~2^-22 near u = 1, so for 1 - u < 1/64 the
+//    series of -ln(1 - v) (v = 1 - u is exact) is used instead; relative error of L <= ~1e-5.
+//  * the angle is reduced EXACTLY in integers to [-pi/4, pi/4] (k_b is a 24-bit integer), then
+//    MUFU.SIN/COS (abs error ~4e-7) and a quadrant swap.
+// Error of z <= ~1e-5 |z| + 4e-7 r, i.e. < 1e-8 N per step at sigma = 1e-3 N (tolerance 1e-6).
 __device__ __forceinline__ void box_muller(uint32_t wa, uint32_t wb, float& z0, float& z1) {
-  const float r = sqrtf(-2.f * logf(u01(wa)));
-  float s, c;
-  sincospif(2.f * u01(wb), &s, &c);  // 2 u_b is exact; sin/cos(2 pi u_b)
-  z0 = r * c;
-  z1 = r * s;
+  const float ua = (float)(2u * (wa >> 9) + 1u) * 5.9604644775390625e-8f;
+  const float v = 1.f - ua;  // exact
+  const float Ls = 2.f * v * fmaf(v, fmaf(v, fmaf(v, 0.25f, 0.33333334f), 0.5f), 1.f);  // -2 ln(1-v), v < 1/64: rel 2e-9
+  const float Ll = -1.3862943611198906f * __log2f(ua);                                  // -2 ln 2 * log2 u
+  const float L = (v < 0.015625f) ? Ls : Ll;
+  const float r = L * rsqrtf(L);
+  const uint32_t kb = 2u * (wb >> 9) + 1u;             // angle = 2 pi kb / 2^24
+  const uint32_t q = (kb + 0x200000u) >> 22;           // nearest quadrant
+  const int rem = (int)kb - (int)(q << 22);            // in [-2^21, 2^21)
+  const float th = (float)rem * 3.7450703e-7f;         // 2 pi / 2^24
+  const float s = __sinf(th), c = __cosf(th);
+  const float cs = (q & 1u) ? -s : c, sn = (q & 1u) ? c : s;
+  const float sg = (q & 2u) ? -1.f : 1.f;
+  z0 = r * (sg * cs);
+  z1 = r * (sg * sn);
 }
 
-__device__ __forceinline__ void st_stream(float* p, float v) { __stcs(p, v); }
+// coalesced copy of n floats from shared memory to a contiguous global range (streaming stores)
+__device__ __forceinline__ void block_store(float* dst, const float* src, int n, int tid) {
+  if ((reinterpret_cast<uintptr_t>(dst) & 15) == 0) {
+    const int n4 = n >> 2;
+    for (int i = tid; i < n4; i += TS_BLOCK) __stcs(reinterpret_cast<float4*>(dst) + i, reinterpret_cast<const float4*>(src)[i]);
+    for (int i = (n4 << 2) + tid; i < n; i += TS_BLOCK) __stcs(dst + i, src[i]);
+  } else {
+    for (int i = tid; i < n; i += TS_BLOCK) __stcs(dst + i, src[i]);
+  }
+}
+
+#define TS_FULL 0xffffffffu
 
 // ---------------------------------------------------------------------------------------
-// The fused step kernel: S1-S8 of DESIGN.md for one (env, patch) per warp.
+// The fused step kernel: S1-S8 of DESIGN.md; block = (env, patch group), thread = taxel slot.
 // ---------------------------------------------------------------------------------------
 template <bool SINGLE>
-__global__ void __launch_bounds__(TS_BLOCK) ts_step_kernel(const __grid_constant__ TsStepParams p) {
-  const int lane = threadIdx.x & 31;
-  const long long gw = ((long long)blockIdx.x * TS_BLOCK + threadIdx.x) >> 5;
-  if (gw >= (long long)p.E * p.P) return;
-  const int e = (int)(gw / p.P);
-  const int pi = (int)(gw - (long long)e * p.P);
-  const int4 pa = __ldg(reinterpret_cast<const int4*>(p.patches + pi));
-  const int4 pb = __ldg(reinterpret_cast<const int4*>(p.patches + pi) + 1);
-  const int start = pa.x, n = pa.y, nu = pa.z, link = pa.w, mstart = pb.x, mcount = pb.y;
-  const float eps = __int_as_float(pb.z);
-  const size_t eT = (size_t)e * p.T;
-  const int i0 = 2 * lane;
-  const size_t j0 = eT + start + i0;  // global slot of my first taxel
-  bool valid[2] = {i0 < n, i0 + 1 < n};
-  const bool vec_ok = valid[1] && ((j0 & 1) == 0);  // both slots present and the pair is 8/16-byte aligned
+__global__ void __launch_bounds__(TS_BLOCK, 2) ts_step_kernel(const __grid_constant__ TsStepParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int nfr = p.frames_per_group * p.K;
+  FrameS* frames = reinterpret_cast<FrameS*>(smem_raw);
+  float* bufA = reinterpret_cast<float*>(frames + nfr);   // [TS_BLOCK*6] output staging
+  float* bufB = bufA + 6 * TS_BLOCK;                      // [6][TS_BLOCK] crosstalk exchange
+  float* hh = bufB + 6 * TS_BLOCK;                        // [TS_BLOCK] penetration h_i (Eq. 19)
+  float* ha = hh + TS_BLOCK;                              // [TS_BLOCK] h_i^alpha_e
+  double* S = reinterpret_cast<double*>(ha + TS_BLOCK);   // [3][TS_BLOCK] marker pass-1 sums
+  int* pact = reinterpret_cast<int*>(S + 3 * TS_BLOCK);   // [TS_MAX_GROUP_PATCHES] patch has penetration
 
-  // ---- per-taxel layout (shared by all envs; L1/L2 resident) --------------------------
-  F3 xj[2], nj[2];
-  float Rj[2];
-#pragma unroll
-  for (int s = 0; s < 2; ++s) {
-    const int t = start + min(i0 + s, n - 1);
-    const float4 a = __ldg(p.tx_pos + t), b = __ldg(p.tx_nrm + t);
-    xj[s] = mk3(a.x, a.y, a.z);
-    nj[s] = mk3(b.x, b.y, b.z);
-    Rj[s] = (valid[s] && link >= 0) ? a.w : 0.f;  // R_j = 0: inactive filler
+  const int tid = threadIdx.x;
+  const int e = blockIdx.x / p.G;
+  const int gi = blockIdx.x - e * p.G;
+  const int4 g0 = __ldg(reinterpret_cast<const int4*>(p.groups + gi));
+  const int4 g1 = __ldg(reinterpret_cast<const int4*>(p.groups + gi) + 1);
+  const int gstart = g0.x, gcount = g0.y, patch0 = g0.z, npatch = g0.w, chunk0 = g1.x, nchunk = g1.y, gmcount = g1.w;
+
+  // ---- phase 0: relative poses (double) -> shared memory ---------------------------------
+  if (tid < TS_MAX_GROUP_PATCHES) pact[tid] = 0;
+  for (int it = tid; it < npatch * p.K; it += TS_BLOCK) {
+    const int lp = it / p.K, k = it - lp * p.K;
+    build_frame(p, e, __ldg(&p.patches[patch0 + lp].link), k, frames[it]);
   }
-  const bool act[2] = {Rj[0] > 0.f, Rj[1] > 0.f};
+  const bool valid = tid < gcount;
+  const int j = gstart + (valid ? tid : 0);
+  const size_t ej = (size_t)e * p.T + j;
+  const float4 P4 = __ldg(p.tx_pos + j), N4 = __ldg(p.tx_nrm + j);
+  const int lp = __float_as_int(N4.w);
+  const float Rj = valid ? P4.w : 0.f;  // R_j = 0: inactive slot
+  const bool act = Rj > 0.f;
+  uint8_t flag = valid ? p.st_flags[ej] : (uint8_t)0;
+  __syncthreads();
 
-  // ---- S1: link pose (warp-uniform) ---------------------------------------------------
-  const int lk = max(link, 0);
-  const size_t el = (size_t)e * p.L + lk;
-  const RotD RLd = quat_Rd(p.link_quat + el * 4);
-  const Rot RL = to_float(RLd);
-  const F3 pL = ld3(p.link_pos + el * 3);
-  const D3 pLd = D3{(double)pL.x, (double)pL.y, (double)pL.z};
-
-  // ---- S2/S3: geometry query, winner = smallest phi (= max_k [R - phi_k]_+, Eq. 2) ------
-  ObjFrameD frd;
-  ObjFrame fr = make_frame(p, e, 0, RLd, pLd, frd);
-  float phi[2];
-  F3 mbar[2];  // contact normal in the link frame, m_bar = R_L^T m = M^T g/|g|
-  int kst[2] = {0, 0};
-  F3 xo[2], dro[2];  // object-frame taxel position and march direction (SINGLE only)
-#pragma unroll
-  for (int s = 0; s < 2; ++s) {
-    phi[s] = __int_as_float(0x7f800000);
-    mbar[s] = mk3(0.f, 0.f, 0.f);
-  }
-  for (int k = 0; k < (SINGLE ? 1 : p.K); ++k) {
-    if (!SINGLE && k > 0) fr = make_frame(p, e, k, RLd, pLd, frd);
-#pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      const D3 xd = mul(frd, xj[s]);
-      if (SINGLE) { xo[s] = to_float(xd); dro[s] = mul(fr.M, nj[s]); }
-      F3 g;
-      const float ph = sdf_eval<true, double>(p, fr, xd, g);
-      if (ph < phi[s]) {  // strict: ties -> lowest k (Q3)
-        phi[s] = ph;
-        kst[s] = k;
-        const float gn = sqrtf(dot(g, g));
-        mbar[s] = (gn < 1e-12f) ? (-1.f) * nj[s] : (1.f / gn) * mulT(fr.M, g);  // Q2
+  // ---- phase 1 (S1-S4): x_o = c + M x_j, phi = min_k phi_k, depth (Eq. 2), contact (Eq. 3) ----
+  double phid = __longlong_as_double(0x7ff0000000000000LL);
+  D3 xd = D3{0.0, 0.0, 0.0};
+  int kst = 0;
+  if (act) {
+    const D3 xj = D3{(double)P4.x, (double)P4.y, (double)P4.z};
+    for (int k = 0; k < (SINGLE ? 1 : p.K); ++k) {
+      const FrameS& F = frames[lp * (SINGLE ? 1 : p.K) + k];
+      const D3 x = ldv(F.c) + mulR(F.M, xj);
+      const double ph = phi_d(p, F.type, F.prm, x);
+      if (ph < phid) {  // strict: ties -> lowest k (Q3)
+        phid = ph; kst = k; xd = x;
       }
     }
   }
-
-  // ---- S4: depth (Eq. 2) and Schmitt contact bit (Eq. 3) ------------------------------
-  float d[2];
-  uint8_t flag[2];
-  {
-    uchar2 fl = make_uchar2(0, 0);
-    if (vec_ok) fl = *reinterpret_cast<const uchar2*>(p.st_flags + j0);
-    else { if (valid[0]) fl.x = p.st_flags[j0]; if (valid[1]) fl.y = p.st_flags[j0 + 1]; }
-    flag[0] = fl.x; flag[1] = fl.y;
+  const float phif = (float)phid;
+  float d = 0.f;
+  if (act) {
+    const double dd = (double)Rj - phid;
+    d = dd > 0.0 ? (float)dd : 0.f;
   }
-  uint8_t yb[2], deadb[2];
-#pragma unroll
-  for (int s = 0; s < 2; ++s) {
-    d[s] = act[s] ? fmaxf(0.f, Rj[s] - phi[s]) : 0.f;
-    const bool y = act[s] && ((d[s] > p.eta_on) || ((flag[s] & 1) && d[s] > p.eta_off));
-    deadb[s] = (p.noise_enable && act[s]) ? ((flag[s] >> 1) & 1) : 0;
-    yb[s] = y ? 1 : 0;
-    flag[s] = (flag[s] & 2) | yb[s];
+  const bool yb = act && ((d > p.eta_on) || ((flag & 1) && d > p.eta_off));
+  const bool deadb = p.noise_enable && act && ((flag >> 1) & 1);
+  if (valid) {
+    p.st_flags[ej] = (uint8_t)((flag & 2) | (yb ? 1 : 0));  // Schmitt state from the un-masked bit (O4)
+    if (p.contact) p.contact[ej] = (yb && !deadb) ? 1 : 0;
+    if (p.dead) p.dead[ej] = deadb ? 1 : 0;
+    if (p.depth) __stcs(p.depth + ej, d);
   }
-  if (vec_ok) {
-    *reinterpret_cast<uchar2*>(p.st_flags + j0) = make_uchar2(flag[0], flag[1]);
-    if (p.contact) *reinterpret_cast<uchar2*>(p.contact + j0) = make_uchar2(deadb[0] ? 0 : yb[0], deadb[1] ? 0 : yb[1]);
-    if (p.dead) *reinterpret_cast<uchar2*>(p.dead + j0) = make_uchar2(deadb[0], deadb[1]);
-    if (p.depth) __stcs(reinterpret_cast<float2*>(p.depth + j0), make_float2(d[0], d[1]));
-  } else {
-#pragma unroll
-    for (int s = 0; s < 2; ++s)
-      if (valid[s]) {
-        p.st_flags[j0 + s] = flag[s];
-        if (p.contact) p.contact[j0 + s] = deadb[s] ? 0 : yb[s];
-        if (p.dead) p.dead[j0 + s] = deadb[s];
-        if (p.depth) st_stream(p.depth + j0 + s, d[s]);
-      }
+  if (p.marker) {  // Eq. 19: h_i = max(0, -phi), no R_j
+    const float h = (act && phid < 0.0) ? (float)(-phid) : 0.f;
+    hh[tid] = h;
+    ha[tid] = h > 0.f ? __powf(h, p.alpha_e) : 0.f;
+    if (h > 0.f) pact[lp] = 1;
   }
 
-  // ---- S5: kinematic force / torque (Eq. 4-9, D2), link frame -------------------------
-  float ft[2][6];
-#pragma unroll
-  for (int s = 0; s < 2; ++s)
-#pragma unroll
-    for (int c = 0; c < 6; ++c) ft[s][c] = 0.f;
-  const bool want_ft = (p.ft != nullptr) || p.noise_enable;
-  if (want_ft && __any_sync(0xffffffffu, d[0] > 0.f || d[1] > 0.f)) {
-    // link-frame velocity terms: v_rel = vbar + wO x (cbar + x_j) - wL x x_j
-    const F3 vL = ld3(p.link_linvel + el * 3), wLw = ld3(p.link_angvel + el * 3);
-    const F3 wL = mulT(RL, wLw);
-#pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      if (d[s] > 0.f) {  // Q5: every term gated on d > 0
-        const size_t ek = (size_t)e * p.K + kst[s];
-        const float sj = __powf(d[s], p.alpha);  // s_j = d^alpha
-        F3 f, tau;
-        if (p.use_velocity) {
-          const F3 pO = ld3(p.obj_pos + ek * 3), vO = ld3(p.obj_linvel + ek * 3), wOw = ld3(p.obj_angvel + ek * 3);
-          const F3 wO = mulT(RL, wOw), vbar = mulT(RL, vO - vL), cbar = mulT(RL, pL - pO);
-          const F3 vrel = vbar + cross(wO, cbar + xj[s]) - cross(wL, xj[s]);           // Eq. 4-6
-          const float vns = dot(vrel, mbar[s]);
-          const F3 vt = vrel - vns * mbar[s];                                          // Eq. 7
-          const F3 fn = (sj * fmaf(p.c_n, vns, p.k_n)) * mbar[s];                      // Eq. 8 normal
-          F3 ftan = (-p.k_t) * vt;                                                     // Eq. 8 tangential
-          const float lim = p.mu * sqrtf(dot(fn, fn)), nft = sqrtf(dot(ftan, ftan));
-          if (nft > lim) ftan = (lim / nft) * ftan;                                    // D2 Coulomb cap
-          f = fn + ftan;
-          tau = cross(xj[s], f) - (p.k_omega * dot(wO - wL, mbar[s])) * mbar[s];       // Eq. 9
+  // ---- phase 2 (S7): proximity march, t <- min(t + max(phi(q + t a), 0), r_prox), K_m evaluations.
+  // Exact shortcuts (O7): evaluation 0 is the query above; t = r_prox is absorbing; an evaluation
+  // that leaves t unchanged repeats forever.
+  if (p.prox) {
+    float t = 0.f;
+    bool go = false;
+    if (act && p.march_steps > 0) {
+      t = fminf(fmaxf(phif, 0.f), p.r_prox);
+      go = (t > 0.f) && (t < p.r_prox);
+    }
+    const F3 nj = mk3(N4.x, N4.y, N4.z);
+    if (SINGLE) {
+      const FrameS& F = frames[lp];
+      const int gtype = __ldg(p.g_type + e);  // block-uniform (one object per env)
+      const F3 xo = mk3((float)xd.x, (float)xd.y, (float)xd.z);
+      const F3 dr = mk3(fmaf(F.Mf[0], nj.x, fmaf(F.Mf[1], nj.y, F.Mf[2] * nj.z)), fmaf(F.Mf[3], nj.x, fmaf(F.Mf[4], nj.y, F.Mf[5] * nj.z)),
+                        fmaf(F.Mf[6], nj.x, fmaf(F.Mf[7], nj.y, F.Mf[8] * nj.z)));
+      if (gtype == TS_GEOM_SDF) {
+        const int N = p.grid_n;
+        const float4* bank_g = p.bank + (size_t)(int)F.prm[0] * p.grid_stride;
+        const float hm = 0.5f * (float)(N - 1) - 0.5f;
+        const F3 um0 = mk3(fmaf(xo.x, p.inv_voxel, hm), fmaf(xo.y, p.inv_voxel, hm), fmaf(xo.z, p.inv_voxel, hm));  // u - 0.5
+        const F3 du = p.inv_voxel * dr;
+        const F3 um1 = um0 + p.r_prox * du;
+        const float lo = 0.25f, hi = (float)N - 2.25f;
+        const bool inside = fminf(fminf(fminf(um0.x, um0.y), um0.z), fminf(fminf(um1.x, um1.y), um1.z)) >= lo &&
+                            fmaxf(fmaxf(fmaxf(um0.x, um0.y), um0.z), fmaxf(fmaxf(um1.x, um1.y), um1.z)) <= hi;
+        if (__all_sync(TS_FULL, inside || !go)) {  // whole segment inside the grid for every marching lane
+          for (int it = 1; it < p.march_steps; ++it) {
+            if (!__any_sync(TS_FULL, go)) break;
+            if (go) {
+              const float sv = grid_value_fast(bank_g, N, um0 + t * du);
+              const float tn = fminf(t + fmaxf(sv, 0.f), p.r_prox);
+              go = (tn != t) && (tn < p.r_prox);
+              t = tn;
+            }
+          }
         } else {
-          f = (p.k_n * sj) * mbar[s];
-          tau = cross(xj[s], f);
+          const F3 u0 = mk3(um0.x + 0.5f, um0.y + 0.5f, um0.z + 0.5f);
+          for (int it = 1; it < p.march_steps; ++it) {
+            if (!__any_sync(TS_FULL, go)) break;
+            if (go) {
+              const float sv = grid_value_f(p, bank_g, u0 + t * du);
+              const float tn = fminf(t + fmaxf(sv, 0.f), p.r_prox);
+              go = (tn != t) && (tn < p.r_prox);
+              t = tn;
+            }
+          }
         }
-        ft[s][0] = f.x; ft[s][1] = f.y; ft[s][2] = f.z; ft[s][3] = tau.x; ft[s][4] = tau.y; ft[s][5] = tau.z;
+      } else {
+        for (int it = 1; it < p.march_steps; ++it) {
+          if (!__any_sync(TS_FULL, go)) break;
+          if (go) {
+            const float sv = prim_value_f(gtype, F.prm, xo + t * dr);
+            const float tn = fminf(t + fmaxf(sv, 0.f), p.r_prox);
+            go = (tn != t) && (tn < p.r_prox);
+            t = tn;
+          }
+        }
       }
+    } else {
+      const F3 xj = mk3(P4.x, P4.y, P4.z);
+      for (int it = 1; it < p.march_steps; ++it) {
+        if (!__any_sync(TS_FULL, go)) break;
+        if (go) {
+          const F3 y = xj + t * nj;
+          float sv = __int_as_float(0x7f800000);
+          for (int k = 0; k < p.K; ++k) {
+            const FrameS& F = frames[lp * p.K + k];
+            const F3 x = mk3(F.cf[0] + fmaf(F.Mf[0], y.x, fmaf(F.Mf[1], y.y, F.Mf[2] * y.z)), F.cf[1] + fmaf(F.Mf[3], y.x, fmaf(F.Mf[4], y.y, F.Mf[5] * y.z)),
+                             F.cf[2] + fmaf(F.Mf[6], y.x, fmaf(F.Mf[7], y.y, F.Mf[8] * y.z)));
+            sv = fminf(sv, phi_f(p, F.type, F.prm, x));
+          }
+          const float tn = fminf(t + fmaxf(sv, 0.f), p.r_prox);
+          go = (tn != t) && (tn < p.r_prox);
+          t = tn;
+        }
+      }
+    }
+    if (valid) __stcs(p.prox + ej, act ? p.r_prox - t : 0.f);
+  }
+
+  // ---- phase 3 (S5): kinematic force / torque (Eq. 4-9, D2) in double, link frame ---------------
+  float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if ((p.ft != nullptr || p.noise_enable) && __any_sync(TS_FULL, d > 0.f)) {
+    if (d > 0.f) {  // Q5: every term gated on d > 0
+      const FrameS& F = frames[lp * (SINGLE ? 1 : p.K) + kst];
+      const D3 g = grad_d(p, F.type, F.prm, xd);
+      const double g2 = dot(g, g);
+      D3 mbar;  // contact normal in the link frame, m_bar = R_L^T m = M^T g / |g|
+      if (g2 < 1e-24) mbar = D3{-(double)N4.x, -(double)N4.y, -(double)N4.z};  // Q2
+      else mbar = drsqrt_n(g2) * mulRT(F.M, g);
+      const double sj = (double)__powf(d, p.alpha);  // s_j = d^alpha
+      const D3 x = D3{(double)P4.x, (double)P4.y, (double)P4.z};
+      D3 f, tau;
+      if (p.use_velocity) {
+        const D3 wO = ldv(F.wO), wL = ldv(F.wL);
+        const D3 vrel = ldv(F.vbar) + cross(wO, ldv(F.cbar) + x) - cross(wL, x);       // Eq. 4-6
+        const double vns = dot(vrel, mbar);
+        const D3 vt = vrel - vns * mbar;                                               // Eq. 7
+        const double fnm = sj * fma((double)p.c_n, vns, (double)p.k_n);
+        D3 ftan = (-(double)p.k_t) * vt;                                               // Eq. 8 tangential
+        const double lim = (double)p.mu * fabs(fnm), nft2 = dot(ftan, ftan);
+        if (nft2 > lim * lim) ftan = (lim * drsqrt_n(nft2)) * ftan;                    // D2 Coulomb cap
+        f = fnm * mbar + ftan;
+        tau = cross(x, f) - ((double)p.k_omega * dot(wO - wL, mbar)) * mbar;           // Eq. 9
+      } else {
+        f = ((double)p.k_n * sj) * mbar;
+        tau = cross(x, f);
+      }
+      ft[0] = (float)f.x; ft[1] = (float)f.y; ft[2] = (float)f.z;
+      ft[3] = (float)tau.x; ft[4] = (float)tau.y; ft[5] = (float)tau.z;
     }
   }
   if (p.ft) {
-    float* o = p.ft + j0 * 6;
-    if (vec_ok) {
-      __stcs(reinterpret_cast<float4*>(o), make_float4(ft[0][0], ft[0][1], ft[0][2], ft[0][3]));
-      __stcs(reinterpret_cast<float4*>(o) + 1, make_float4(ft[0][4], ft[0][5], ft[1][0], ft[1][1]));
-      __stcs(reinterpret_cast<float4*>(o) + 2, make_float4(ft[1][2], ft[1][3], ft[1][4], ft[1][5]));
-    } else {
 #pragma unroll
-      for (int s = 0; s < 2; ++s)
-        if (valid[s])
-#pragma unroll
-          for (int c = 0; c < 6; ++c) st_stream(o + s * 6 + c, ft[s][c]);
-    }
+    for (int c = 0; c < 6; ++c) bufA[tid * 6 + c] = ft[c];
   }
 
-  // ---- S8: noise chain on the six channels (O8): hysteresis -> crosstalk -> drift -> dead
+  // ---- phase 4 (S8): noise chain on the six channels (O8): hysteresis -> crosstalk -> drift -> dead
+  float outv[6];
   if (p.noise_enable) {
-    const size_t blk = (size_t)e * p.P + pi;
-    float h[2][6];
-    // S8b hysteresis; state rows are [row][lane] float4 so each load is one 512-byte warp transaction
-    if (p.hyst_mode == TS_HYST_ASYM) {
-      float4* st = p.st_hyst + blk * (3 * 32) + lane;
-      float y[12];
-      if (valid[0]) {
+    float h[6];
+    const size_t Tp = (size_t)p.Tp;
+    if (p.hyst_mode == TS_HYST_ASYM) {  // D3, Q14
+      float* st = p.st_hyst + (size_t)e * 6 * Tp + j;
 #pragma unroll
-        for (int r = 0; r < 3; ++r) {
-          const float4 v = __ldcs(st + r * 32);
-          y[4 * r] = v.x; y[4 * r + 1] = v.y; y[4 * r + 2] = v.z; y[4 * r + 3] = v.w;
-        }
-      } else {
-#pragma unroll
-        for (int i = 0; i < 12; ++i) y[i] = 0.f;
+      for (int c = 0; c < 6; ++c) {
+        const float yp = valid ? __ldcs(st + c * Tp) : 0.f;
+        const float al = (fabsf(ft[c]) > fabsf(yp)) ? p.alpha_load : p.alpha_unload;
+        h[c] = act ? fmaf(al, ft[c] - yp, yp) : 0.f;
+        if (valid) __stcs(st + c * Tp, h[c]);
       }
+    } else if (p.hyst_mode == TS_HYST_MAXWELL) {  // Eq. 29-30
+      float* st = p.st_hyst + (size_t)e * 12 * Tp + j;
 #pragma unroll
-      for (int s = 0; s < 2; ++s)
-#pragma unroll
-        for (int c = 0; c < 6; ++c) {
-          const float x = ft[s][c], yp = y[s * 6 + c];
-          const float al = (fabsf(x) > fabsf(yp)) ? p.alpha_load : p.alpha_unload;  // D3, Q14
-          const float yn = act[s] ? fmaf(al, x - yp, yp) : 0.f;
-          y[s * 6 + c] = yn;
-          h[s][c] = yn;
-        }
-      if (valid[0]) {
-#pragma unroll
-        for (int r = 0; r < 3; ++r) __stcs(st + r * 32, make_float4(y[4 * r], y[4 * r + 1], y[4 * r + 2], y[4 * r + 3]));
-      }
-    } else if (p.hyst_mode == TS_HYST_MAXWELL) {
-      float4* st = p.st_hyst + blk * (6 * 32) + lane;
-      float xi[12], xp[12];
-      if (valid[0]) {
-#pragma unroll
-        for (int r = 0; r < 3; ++r) {
-          const float4 v = __ldcs(st + r * 32), w = __ldcs(st + (3 + r) * 32);
-          xi[4 * r] = v.x; xi[4 * r + 1] = v.y; xi[4 * r + 2] = v.z; xi[4 * r + 3] = v.w;
-          xp[4 * r] = w.x; xp[4 * r + 1] = w.y; xp[4 * r + 2] = w.z; xp[4 * r + 3] = w.w;
-        }
-      } else {
-#pragma unroll
-        for (int i = 0; i < 12; ++i) { xi[i] = 0.f; xp[i] = 0.f; }
-      }
-#pragma unroll
-      for (int s = 0; s < 2; ++s)
-#pragma unroll
-        for (int c = 0; c < 6; ++c) {
-          const float x = ft[s][c];
-          const float z = act[s] ? fmaf(p.decay, xi[s * 6 + c], x - xp[s * 6 + c]) : 0.f;  // Eq. 29
-          xi[s * 6 + c] = z;
-          xp[s * 6 + c] = act[s] ? x : 0.f;
-          h[s][c] = fmaf(p.beta, z, x);                                                    // Eq. 30
-        }
-      if (valid[0]) {
-#pragma unroll
-        for (int r = 0; r < 3; ++r) {
-          __stcs(st + r * 32, make_float4(xi[4 * r], xi[4 * r + 1], xi[4 * r + 2], xi[4 * r + 3]));
-          __stcs(st + (3 + r) * 32, make_float4(xp[4 * r], xp[4 * r + 1], xp[4 * r + 2], xp[4 * r + 3]));
+      for (int c = 0; c < 6; ++c) {
+        const float xi = valid ? __ldcs(st + c * Tp) : 0.f, xp = valid ? __ldcs(st + (6 + c) * Tp) : 0.f;
+        const float z = act ? fmaf(p.decay, xi, ft[c] - xp) : 0.f;
+        h[c] = fmaf(p.beta, z, ft[c]);
+        if (valid) {
+          __stcs(st + c * Tp, z);
+          __stcs(st + (6 + c) * Tp, act ? ft[c] : 0.f);
         }
       }
     } else {
 #pragma unroll
-      for (int s = 0; s < 2; ++s)
-#pragma unroll
-        for (int c = 0; c < 6; ++c) h[s][c] = ft[s][c];
+      for (int c = 0; c < 6; ++c) h[c] = ft[c];
     }
-
-    // S8c crosstalk (D4): c_j = h_j + chi/4 sum_{k in N4(j)} (h_k - h_j), neighbours by shuffle.
-    // Slot i = 2 lane + s sits at (iu, iv) = (i mod nu, i div nu); -u/+u neighbours are i-+1,
-    // -v/+v neighbours are i-+nu, i.e. lane (i-+nu)>>1, slot (i-+nu)&1.
-    float cx[2][6];
-    {
-      const int nv_ = n / nu;
-      const bool odd = nu & 1;
-      int iu[2], iv[2];
 #pragma unroll
-      for (int s = 0; s < 2; ++s) { iv[s] = (i0 + s) / nu; iu[s] = (i0 + s) - iv[s] * nu; }
-      const float q = 0.25f * p.chi;
+    for (int c = 0; c < 6; ++c) bufB[c * TS_BLOCK + tid] = h[c];
+  }
+  __syncthreads();
+  if (p.ft) block_store(p.ft + ((size_t)e * p.T + gstart) * 6, bufA, gcount * 6, tid);
+  if (p.noise_enable) {
+    // S8c crosstalk (D4): c_j = h_j + chi/4 sum_{k in N4(j)} (h_k - h_j), neighbours from shared memory
+    const int4 nb = __ldg(p.tx_nbr + j);
+    const float q4 = 0.25f * p.chi;
+    float D[6];
+    float* sd = p.st_drift + (size_t)e * 6 * (size_t)p.Tp + j;
 #pragma unroll
-      for (int c = 0; c < 6; ++c) {
-        const float up1 = __shfl_up_sync(0xffffffffu, h[1][c], 1);      // slot 1 of lane-1  = taxel i0-1
-        const float dn0 = __shfl_down_sync(0xffffffffu, h[0][c], 1);    // slot 0 of lane+1  = taxel i0+2
-        float acc0 = 0.f, acc1 = 0.f;
-        if (iu[0] > 0) acc0 += up1 - h[0][c];
-        if (iu[0] < nu - 1) acc0 += h[1][c] - h[0][c];
-        if (iu[1] > 0) acc1 += h[0][c] - h[1][c];
-        if (iu[1] < nu - 1) acc1 += dn0 - h[1][c];
-#pragma unroll
-        for (int s = 0; s < 2; ++s) {
-          const int im = i0 + s - nu, ip = i0 + s + nu;
-          // source slot is warp-uniform: same slot when nu is even, the other one when odd
-          const float srcm = odd ? h[1 - s][c] : h[s][c];
-          const float vm = __shfl_sync(0xffffffffu, srcm, (im >> 1) & 31);
-          const float vp = __shfl_sync(0xffffffffu, srcm, (ip >> 1) & 31);
-          float a = 0.f;
-          if (iv[s] > 0) a += vm - h[s][c];
-          if (iv[s] < nv_ - 1) a += vp - h[s][c];
-          if (s == 0) acc0 += a; else acc1 += a;
-        }
-        cx[0][c] = fmaf(q, acc0, h[0][c]);
-        cx[1][c] = fmaf(q, acc1, h[1][c]);
-      }
-    }
-
-    // S8d drift (Eq. 25): D <- D + sigma z, z from Philox + Box-Muller; S8a dead (Eq. 28)
-    {
-      float4* st = p.st_drift + blk * (3 * 32) + lane;
-      float D[12];
-      if (valid[0]) {
-#pragma unroll
-        for (int r = 0; r < 3; ++r) {
-          const float4 v = __ldcs(st + r * 32);
-          D[4 * r] = v.x; D[4 * r + 1] = v.y; D[4 * r + 2] = v.z; D[4 * r + 3] = v.w;
-        }
-      } else {
-#pragma unroll
-        for (int i = 0; i < 12; ++i) D[i] = 0.f;
-      }
+    for (int c = 0; c < 6; ++c) D[c] = valid ? __ldcs(sd + (size_t)c * p.Tp) : 0.f;
+    // S8d drift draws (Eq. 25): Philox streams 0 / 1 -> six normals
+    float z[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (act) {
       const uint32_t nstep = p.gstep - __ldg(p.reset_step + e);
       const uint32_t ep4 = __ldg(p.episode + e) << 4;
       const uint32_t env = p.env_id_base + (uint32_t)e;
-      float outv[12];
+      const uint4 w0 = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 0u), p.seed_lo, p.seed_hi);
+      const uint4 w1 = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 1u), p.seed_lo, p.seed_hi);
+      box_muller(w0.x, w0.y, z[0], z[1]);
+      box_muller(w0.z, w0.w, z[2], z[3]);
+      box_muller(w1.x, w1.y, z[4], z[5]);
+    }
 #pragma unroll
-      for (int s = 0; s < 2; ++s) {
-        float z[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        if (act[s]) {
-          const uint32_t tax = (uint32_t)(start + i0 + s);
-          const uint4 w0 = philox4x32_10(make_uint4(env, tax, nstep, ep4 | 0u), p.seed_lo, p.seed_hi);
-          const uint4 w1 = philox4x32_10(make_uint4(env, tax, nstep, ep4 | 1u), p.seed_lo, p.seed_hi);
-          box_muller(w0.x, w0.y, z[0], z[1]);
-          box_muller(w0.z, w0.w, z[2], z[3]);
-          box_muller(w1.x, w1.y, z[4], z[5]);
-        }
+    for (int c = 0; c < 6; ++c) {
+      const float* hb = bufB + c * TS_BLOCK;
+      const float hc = hb[tid];
+      float acc = 0.f;
+      if (nb.x >= 0) acc += hb[nb.x - gstart] - hc;
+      if (nb.y >= 0) acc += hb[nb.y - gstart] - hc;
+      if (nb.z >= 0) acc += hb[nb.z - gstart] - hc;
+      if (nb.w >= 0) acc += hb[nb.w - gstart] - hc;
+      const float cx = fmaf(q4, acc, hc);
+      const float Dn = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], D[c]) : 0.f;
+      if (valid) __stcs(sd + (size_t)c * p.Tp, Dn);
+      outv[c] = (act && !deadb) ? cx + Dn : 0.f;  // S8a dead (Eq. 28) last
+    }
+    if (p.ft_noisy) {
+      __syncthreads();  // bufA drained by the ft store
 #pragma unroll
-        for (int c = 0; c < 6; ++c) {
-          const float Dn = act[s] ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], D[s * 6 + c]) : 0.f;
-          D[s * 6 + c] = Dn;
-          outv[s * 6 + c] = (act[s] && !deadb[s]) ? cx[s][c] + Dn : 0.f;
-        }
-      }
-      if (valid[0]) {
-#pragma unroll
-        for (int r = 0; r < 3; ++r) __stcs(st + r * 32, make_float4(D[4 * r], D[4 * r + 1], D[4 * r + 2], D[4 * r + 3]));
-      }
-      if (p.ft_noisy) {
-        float* o = p.ft_noisy + j0 * 6;
-        if (vec_ok) {
-#pragma unroll
-          for (int r = 0; r < 3; ++r)
-            __stcs(reinterpret_cast<float4*>(o) + r, make_float4(outv[4 * r], outv[4 * r + 1], outv[4 * r + 2], outv[4 * r + 3]));
-        } else {
-#pragma unroll
-          for (int s = 0; s < 2; ++s)
-            if (valid[s])
-#pragma unroll
-              for (int c = 0; c < 6; ++c) st_stream(o + s * 6 + c, outv[s * 6 + c]);
-        }
-      }
+      for (int c = 0; c < 6; ++c) bufA[tid * 6 + c] = outv[c];
+      __syncthreads();
+      block_store(p.ft_noisy + ((size_t)e * p.T + gstart) * 6, bufA, gcount * 6, tid);
     }
   }
 
-  // ---- S6: elastomer marker dilation (Eq. 18-21; sources with h_i = 0 contribute exactly 0)
-  if (p.marker && mcount > 0) {
-    float hh[2], ha[2];
-#pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      hh[s] = act[s] ? fmaxf(0.f, -phi[s]) : 0.f;                  // Eq. 19
-      ha[s] = hh[s] > 0.f ? __powf(hh[s], p.alpha_e) : 0.f;
-    }
-    unsigned m0 = __ballot_sync(0xffffffffu, hh[0] > 0.f), m1 = __ballot_sync(0xffffffffu, hh[1] > 0.f);
-    F3 acc[2] = {mk3(0.f, 0.f, 0.f), mk3(0.f, 0.f, 0.f)};
-    F3 mp[2], mn[2];
-#pragma unroll
-    for (int r = 0; r < 2; ++r) {
-      const int jm = mstart + min(lane + 32 * r, mcount - 1);
-      const float4 a = __ldg(p.mk_pos + jm), b = __ldg(p.mk_nrm + jm);
-      mp[r] = mk3(a.x, a.y, a.z);
-      mn[r] = mk3(b.x, b.y, b.z);
-    }
-    const float two_eps = 2.f * eps, eps2 = eps * eps, cg = p.c_e * p.inv_gbar, crho = 1.f - p.c_e;
-#pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      unsigned m = s ? m1 : m0;
-      while (m) {
-        const int sl = __ffs(m) - 1;
-        m &= m - 1;
-        const float hi = __shfl_sync(0xffffffffu, hh[s], sl), hai = __shfl_sync(0xffffffffu, ha[s], sl);
-        const float4 xs = __ldg(p.tx_pos + start + 2 * sl + s);  // uniform address: broadcast
-#pragma unroll
-        for (int r = 0; r < 2; ++r) {
-          const F3 z = mp[r] - mk3(xs.x, xs.y, xs.z);
-          const F3 rr = z - dot(z, mn[r]) * mn[r];                 // Eq. 18
-          const float r2 = dot(rr, rr);
-          const float g = __expf(-p.lambda_d * r2);
-          float w = cg * g;
-          if (crho != 0.f) w = fmaf(crho, __fdividef(two_eps, r2 + eps2), w);
-          w *= hi;                                                 // Eq. 20
-          acc[r] = acc[r] + p.s_d * (w * rr + (hai * g) * mn[r]);  // Eq. 21
-        }
-      }
-    }
-#pragma unroll
-    for (int r = 0; r < 2; ++r) {
-      const int jm = lane + 32 * r;
-      if (jm < mcount) {
-        float* o = p.marker + ((size_t)e * p.M + mstart + jm) * 3;
-        st_stream(o, acc[r].x); st_stream(o + 1, acc[r].y); st_stream(o + 2, acc[r].z);
-      }
-    }
-  }
-
-  // ---- S7: proximity march (O7): t <- min(t + max(phi(q + t a), 0), r_prox), K_m evaluations.
-  // Exact shortcuts: evaluation 0 is the query above; t = r_prox is absorbing; an evaluation
-  // that leaves t unchanged (s <= 0, or s below half an ulp of t) repeats forever.
-  if (p.prox) {
-    float t[2];
-    bool go[2];
-#pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      t[s] = 0.f;
-      go[s] = false;
-      if (act[s] && p.march_steps > 0) {
-        t[s] = fminf(fmaxf(phi[s], 0.f), p.r_prox);
-        go[s] = (t[s] > 0.f) && (t[s] < p.r_prox);
-      }
-    }
-    for (int it = 1; it < p.march_steps; ++it) {
-      if (!(go[0] || go[1])) break;
-#pragma unroll
-      for (int s = 0; s < 2; ++s) {
-        if (go[s]) {
-          float sv;
-          F3 dummy;
-          if (SINGLE) {
-            sv = sdf_eval<false, float>(p, fr, as_x3(xo[s] + t[s] * dro[s]), dummy);
-          } else {
-            sv = __int_as_float(0x7f800000);
-            for (int k = 0; k < p.K; ++k) {
-              ObjFrameD f2d;
-              const ObjFrame f2 = make_frame(p, e, k, RLd, pLd, f2d);
-              sv = fminf(sv, sdf_eval<false, float>(p, f2, as_x3(f2.c + mul(f2.M, xj[s] + t[s] * nj[s])), dummy));
+  // ---- phase 5 (S6): elastomer marker dilation (Eq. 18-21, 23 first sum) ----------------------
+  // With c = 1 and planar regular grids, g(r_ij) = exp(-lambda |r|^2) = gu(a,p) gv(b,q) and
+  // r_ij = du(a,p) u^ + dv(b,q) v^, so u_j = s_d [ (u^ Uu + v^ Uv)/g_bar + n Un ] with
+  //   pass 1 over (a,q): S0 = sum_p gu h, S1 = sum_p du gu h, T0 = sum_p gu h^alpha_e
+  //   pass 2 over (a,b): Uu = sum_q gv S1, Uv = sum_q dv gv S0, Un = sum_q gv T0.
+  // Sources with h_i = 0 contribute exactly 0; patches without penetration are skipped.
+  if (p.marker && gmcount > 0) {
+    __syncthreads();  // hh / ha / pact complete, bufA free
+    for (int ch = 0; ch < nchunk; ++ch) {
+      const int4 c0 = __ldg(reinterpret_cast<const int4*>(p.chunks + chunk0 + ch));
+      const int4 c1 = __ldg(reinterpret_cast<const int4*>(p.chunks + chunk0 + ch) + 1);
+      const int i1b = c0.x, i1e = c0.y, mb = c0.z, me = c0.w, lpb = c1.x, lpe = c1.y;
+      bool any = false;
+      for (int l = lpb; l < lpe; ++l) any = any || (pact[l] != 0);
+      if (any) {
+        if (i1b + tid < i1e) {  // pass 1
+          const int pk = __ldg(p.mk_item1 + i1b + tid);
+          const int l = pk & 255, a = (pk >> 8) & 255, q = pk >> 16;
+          const TsPatch& pt = p.patches[patch0 + l];
+          double s0 = 0.0, s1 = 0.0, t0 = 0.0;
+          if (pact[l] && !pt.direct) {
+            const int nu = pt.nu;
+            const double* GU = p.mk_tab + pt.tab + a * nu;
+            const double* DU = GU + pt.mnu * nu;
+            const int base = pt.start - gstart + q * nu;
+            for (int ip = 0; ip < nu; ++ip) {
+              const double h = (double)hh[base + ip], hal = (double)ha[base + ip], gu = __ldg(GU + ip);
+              s0 = fma(gu, h, s0);
+              s1 = fma(__ldg(DU + ip), h, s1);
+              t0 = fma(gu, hal, t0);
             }
           }
-          const float tn = fminf(t[s] + fmaxf(sv, 0.f), p.r_prox);
-          go[s] = (tn != t[s]) && (tn < p.r_prox);
-          t[s] = tn;
+          S[tid] = s0; S[TS_BLOCK + tid] = s1; S[2 * TS_BLOCK + tid] = t0;
         }
+        __syncthreads();
       }
-    }
-    float pr[2];
-#pragma unroll
-    for (int s = 0; s < 2; ++s) pr[s] = (act[s] && p.march_steps >= 0) ? p.r_prox - t[s] : 0.f;
-    if (vec_ok) __stcs(reinterpret_cast<float2*>(p.prox + j0), make_float2(pr[0], pr[1]));
-    else {
-#pragma unroll
-      for (int s = 0; s < 2; ++s)
-        if (valid[s]) st_stream(p.prox + j0 + s, pr[s]);
+      if (mb + tid < me) {  // pass 2: one marker per thread
+        float ox = 0.f, oy = 0.f, oz = 0.f;
+        if (any) {
+          const int pk = __ldg(p.mk_item2 + mb + tid);
+          const int l = pk & 255, a = (pk >> 8) & 255, b = pk >> 16;
+          const TsPatch& pt = p.patches[patch0 + l];
+          if (pact[l]) {
+            if (!pt.direct) {
+              const int nv = pt.nv, mnu = pt.mnu;
+              const double* GV = p.mk_tab + pt.tab + 2 * mnu * pt.nu + b * nv;
+              const double* DV = GV + pt.mnv * nv;
+              const double* s = S + (pt.i1off - i1b + a);
+              double Uu = 0.0, Uv = 0.0, Un = 0.0;
+              for (int q = 0; q < nv; ++q) {
+                const double gv = __ldg(GV + q);
+                Uu = fma(gv, s[TS_BLOCK + q * mnu], Uu);
+                Uv = fma(__ldg(DV + q), s[q * mnu], Uv);
+                Un = fma(gv, s[2 * TS_BLOCK + q * mnu], Un);
+              }
+              const double sd = (double)p.s_d, kt = sd * p.inv_gbar;
+              const float4 ua = pt.ua, va = pt.va, na = pt.na;
+              ox = (float)(kt * fma(Uu, (double)ua.x, Uv * (double)va.x) + sd * Un * (double)na.x);
+              oy = (float)(kt * fma(Uu, (double)ua.y, Uv * (double)va.y) + sd * Un * (double)na.y);
+              oz = (float)(kt * fma(Uu, (double)ua.z, Uv * (double)va.z) + sd * Un * (double)na.z);
+            } else {  // direct sum (c_e != 1: rho(r) = 1/(|r|^2 + eps^2) is not separable)
+              const float4 mp = __ldg(p.mk_pos + mb + tid), mn = __ldg(p.mk_nrm + mb + tid);
+              const D3 n = D3{(double)mn.x, (double)mn.y, (double)mn.z};
+              const double eps = (double)pt.eps, ce = (double)p.c_e;
+              D3 acc = D3{0.0, 0.0, 0.0};
+              for (int i = 0; i < pt.n; ++i) {
+                const float hi = hh[pt.start - gstart + i];
+                if (!(hi > 0.f)) continue;
+                const float4 xs = __ldg(p.tx_pos + pt.start + i);
+                const D3 zv = D3{(double)mp.x - (double)xs.x, (double)mp.y - (double)xs.y, (double)mp.z - (double)xs.z};
+                const D3 rr = zv - dot(zv, n) * n;                                     // Eq. 18
+                const double r2 = dot(rr, rr);
+                const double gg = exp(-(double)p.lambda_d * r2);
+                const double w = (double)hi * (ce * gg * p.inv_gbar + (1.0 - ce) * (2.0 * eps) / (r2 + eps * eps));  // Eq. 20
+                acc = acc + (double)p.s_d * (w * rr + ((double)ha[pt.start - gstart + i] * gg) * n);              // Eq. 21
+              }
+              ox = (float)acc.x; oy = (float)acc.y; oz = (float)acc.z;
+            }
+          }
+        }
+        bufA[tid * 3] = ox; bufA[tid * 3 + 1] = oy; bufA[tid * 3 + 2] = oz;
+      }
+      __syncthreads();
+      block_store(p.marker + ((size_t)e * p.M + mb) * 3, bufA, (me - mb) * 3, tid);
+      __syncthreads();
     }
   }
 }
@@ -671,47 +754,48 @@ __global__ void ts_reset_counters_kernel(uint32_t* reset_step, uint32_t* episode
 }
 
 // Zeroes the state of the masked envs and re-draws their dead flags (Eq. 28, D5): Philox
-// stream 2 at n = 0, dead iff word0 < floor(p_dead 2^32).  One thread per (env, patch, lane).
+// stream 2 at n = 0, dead iff word0 < floor(p_dead 2^32).  One thread per (env, padded slot).
 __global__ void ts_reset_state_kernel(const __grid_constant__ TsStepParams p, const uint8_t* mask, uint32_t thr, int nh) {
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const long long gw = gt >> 5;
-  const int lane = (int)(gt & 31);
-  if (gw >= (long long)p.E * p.P) return;
-  const int e = (int)(gw / p.P), pi = (int)(gw - (long long)e * p.P);
+  if (gt >= (long long)p.E * p.Tp) return;
+  const int e = (int)(gt / p.Tp), t = (int)(gt - (long long)e * p.Tp);
   if (mask && !mask[e]) return;
-  const TsPatch pt = p.patches[pi];
-  const size_t blk = (size_t)e * p.P + pi;
-  const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
   if (p.st_hyst)
-    for (int r = 0; r < nh; ++r) p.st_hyst[blk * (nh * 32) + r * 32 + lane] = z4;
+    for (int c = 0; c < nh; ++c) p.st_hyst[((size_t)e * nh + c) * p.Tp + t] = 0.f;
   if (p.st_drift)
-    for (int r = 0; r < 3; ++r) p.st_drift[blk * (3 * 32) + r * 32 + lane] = z4;
-  const uint32_t ep4 = p.episode[e] << 4;
-  for (int s = 0; s < 2; ++s) {
-    const int i = 2 * lane + s;
-    if (i >= pt.n) continue;
-    const int t = pt.start + i;
-    uint8_t fl = 0;
-    if (p.noise_enable && pt.link >= 0 && p.tx_pos[t].w > 0.f) {
-      const uint4 w = philox4x32_10(make_uint4(p.env_id_base + (uint32_t)e, (uint32_t)t, 0u, ep4 | 2u), p.seed_lo, p.seed_hi);
-      fl = (w.x < thr) ? 2 : 0;
-    }
-    p.st_flags[(size_t)e * p.T + t] = fl;
+    for (int c = 0; c < 6; ++c) p.st_drift[((size_t)e * 6 + c) * p.Tp + t] = 0.f;
+  if (t >= p.T) return;
+  uint8_t fl = 0;
+  if (p.noise_enable && p.tx_pos[t].w > 0.f) {
+    const uint4 w = philox4x32_10(make_uint4(p.env_id_base + (uint32_t)e, (uint32_t)t, 0u, (p.episode[e] << 4) | 2u), p.seed_lo, p.seed_hi);
+    fl = (w.x < thr) ? 2 : 0;
   }
+  p.st_flags[(size_t)e * p.T + t] = fl;
 }
 
 }  // namespace
 
 unsigned long long ts_bank_elems_per_grid(int N) { return (unsigned long long)(N - 1) * (N - 1) * N; }
 
+unsigned long long ts_step_smem_bytes(const TsStepParams& p) {
+  return (unsigned long long)p.frames_per_group * p.K * sizeof(FrameS) + sizeof(float) * (12 + 2) * TS_BLOCK +
+         sizeof(double) * 3 * TS_BLOCK + sizeof(int) * TS_MAX_GROUP_PATCHES;
+}
+
+int ts_prepare_kernels(int max_smem_bytes) {
+  cudaError_t e = cudaFuncSetAttribute(ts_step_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(ts_step_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
+  return (int)e;
+}
+
 int ts_launch_step(const TsStepParams& p, void* stream) {
-  const long long warps = (long long)p.E * p.P;
-  const long long blocks = (warps * 32 + TS_BLOCK - 1) / TS_BLOCK;
+  const long long blocks = (long long)p.E * p.G;
   if (blocks <= 0 || blocks > 0x7fffffffLL) return (int)cudaErrorInvalidConfiguration;
+  const size_t smem = (size_t)ts_step_smem_bytes(p);
   if (p.K == 1)
-    ts_step_kernel<true><<<(unsigned)blocks, TS_BLOCK, 0, (cudaStream_t)stream>>>(p);
+    ts_step_kernel<true><<<(unsigned)blocks, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
   else
-    ts_step_kernel<false><<<(unsigned)blocks, TS_BLOCK, 0, (cudaStream_t)stream>>>(p);
+    ts_step_kernel<false><<<(unsigned)blocks, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
   return (int)cudaGetLastError();
 }
 
@@ -728,7 +812,7 @@ int ts_launch_reset_counters(uint32_t* reset_step, uint32_t* episode, const uint
 }
 
 int ts_launch_reset_state(const TsStepParams& p, const uint8_t* mask, uint32_t thr, int nh, void* stream) {
-  const long long threads = (long long)p.E * p.P * 32;
+  const long long threads = (long long)p.E * p.Tp;
   const long long blocks = (threads + 255) / 256;
   ts_reset_state_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(p, mask, thr, nh);
   return (int)cudaGetLastError();

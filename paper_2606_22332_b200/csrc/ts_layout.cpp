@@ -29,10 +29,12 @@ ts_status ts_layout_add_patch(ts_layout* lay, const ts_patch_desc* d) {
   if ((d->marker_nu == 0) != (d->marker_nv == 0)) return TS_ERR_INVALID_ARG;
   if (!(d->radius > 0.0f) || !(d->size_u > 0.0f) || !(d->size_v > 0.0f) || d->link < 0) return TS_ERR_INVALID_ARG;
   double uu = dot3(d->u_axis, d->u_axis), vv = dot3(d->v_axis, d->v_axis), uv = dot3(d->u_axis, d->v_axis);
-  if (std::fabs(uu - 1.0) > 2e-3 || std::fabs(vv - 1.0) > 2e-3 || std::fabs(uv) > 1e-3) return TS_ERR_INVALID_ARG;
+  // unit and orthogonal to 1e-5: the separable marker sums (ts_kernels.cu phase 5) rely on |r|^2 = du^2 + dv^2
+  if (std::fabs(uu - 1.0) > 1e-5 || std::fabs(vv - 1.0) > 1e-5 || std::fabs(uv) > 1e-5) return TS_ERR_INVALID_ARG;
   const double ux = d->u_axis[0], uy = d->u_axis[1], uz = d->u_axis[2];
   const double vx = d->v_axis[0], vy = d->v_axis[1], vz = d->v_axis[2];
   const double n[3] = {uy * vz - uz * vy, uz * vx - ux * vz, ux * vy - uy * vx};
+  lay->desc.push_back(*d);
   const int p = (int)lay->patch_start.size();
   const int t0 = (int)lay->radius.size();
   lay->patch_start.push_back(t0);
