@@ -189,7 +189,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     q.va = make_float4(d.v_axis[0], d.v_axis[1], d.v_axis[2], 0.f);
     q.na = q.mnu > 0 ? make_float4(lay->marker_nrm[3 * q.mstart], lay->marker_nrm[3 * q.mstart + 1], lay->marker_nrm[3 * q.mstart + 2], 0.f)
                      : make_float4(0.f, 0.f, 1.f, 0.f);
-    q.direct = (cfg->c_e != 1.0f || q.mnu * q.nv > TS_BLOCK) ? 1 : 0;
+    q.direct = (cfg->c_e != 1.0f || q.mnu * q.nv > TS_CHUNK) ? 1 : 0;
     q.tab = (int32_t)tab.size();
     q.i1off = (int32_t)item1.size();
     if (q.mnu > 0 && !q.direct) {
@@ -250,7 +250,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
       while (l < g.npatch) {
         const TsPatch& q = pts[g.patch0 + l];
         const int n1 = (q.mnu > 0 && !q.direct) ? q.mnu * q.nv : 0, nm = q.mnu * q.mnv;
-        if (l > ck.lp_begin && ((ck.i1_end - ck.i1_begin) + n1 > TS_BLOCK || (ck.m_end - ck.m_begin) + nm > TS_BLOCK)) break;
+        if (l > ck.lp_begin && ((ck.i1_end - ck.i1_begin) + n1 > TS_CHUNK || (ck.m_end - ck.m_begin) + nm > TS_CHUNK)) break;
         ck.i1_end += n1; ck.m_end += nm; ++l;
       }
       ck.lp_end = l;

@@ -354,24 +354,29 @@ __device__ __forceinline__ void box_muller(uint32_t wa, uint32_t wb, float& z0, 
   z1 = r * (sg * sn);
 }
 
-// coalesced copy of n floats from shared memory to a contiguous global range (streaming stores)
+// coalesced copy of n <= 6*TS_BLOCK floats from shared memory to a contiguous global range (streaming stores)
 __device__ __forceinline__ void block_store(float* dst, const float* src, int n, int tid) {
-  if ((reinterpret_cast<uintptr_t>(dst) & 15) == 0) {
+  if (((reinterpret_cast<uintptr_t>(dst) & 15) | (n & 3)) == 0) {
     const int n4 = n >> 2;
-    for (int i = tid; i < n4; i += TS_BLOCK) __stcs(reinterpret_cast<float4*>(dst) + i, reinterpret_cast<const float4*>(src)[i]);
-    for (int i = (n4 << 2) + tid; i < n; i += TS_BLOCK) __stcs(dst + i, src[i]);
+    float4* d4 = reinterpret_cast<float4*>(dst);
+    const float4* s4 = reinterpret_cast<const float4*>(src);
+    if (tid < n4) __stcs(d4 + tid, s4[tid]);
+    if (tid + TS_BLOCK < n4) __stcs(d4 + tid + TS_BLOCK, s4[tid + TS_BLOCK]);
   } else {
     for (int i = tid; i < n; i += TS_BLOCK) __stcs(dst + i, src[i]);
   }
 }
 
 #define TS_FULL 0xffffffffu
+#ifndef TS_MIN_BLOCKS
+#define TS_MIN_BLOCKS 3
+#endif
 
 // ---------------------------------------------------------------------------------------
 // The fused step kernel: S1-S8 of DESIGN.md; block = (env, patch group), thread = taxel slot.
 // ---------------------------------------------------------------------------------------
 template <bool SINGLE>
-__global__ void __launch_bounds__(TS_BLOCK, 2) ts_step_kernel(const __grid_constant__ TsStepParams p) {
+__global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const __grid_constant__ TsStepParams p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int nfr = p.frames_per_group * p.K;
   FrameS* frames = reinterpret_cast<FrameS*>(smem_raw);
@@ -379,12 +384,12 @@ __global__ void __launch_bounds__(TS_BLOCK, 2) ts_step_kernel(const __grid_const
   float* bufB = bufA + 6 * TS_BLOCK;                      // [6][TS_BLOCK] crosstalk exchange
   float* hh = bufB + 6 * TS_BLOCK;                        // [TS_BLOCK] penetration h_i (Eq. 19)
   float* ha = hh + TS_BLOCK;                              // [TS_BLOCK] h_i^alpha_e
-  double* S = reinterpret_cast<double*>(ha + TS_BLOCK);   // [3][TS_BLOCK] marker pass-1 sums
-  int* pact = reinterpret_cast<int*>(S + 3 * TS_BLOCK);   // [TS_MAX_GROUP_PATCHES] patch has penetration
+  double* S = reinterpret_cast<double*>(ha + TS_BLOCK);   // [3][TS_CHUNK] marker pass-1 sums
+  int* pact = reinterpret_cast<int*>(S + 3 * TS_CHUNK);   // [TS_MAX_GROUP_PATCHES] patch has penetration
 
   const int tid = threadIdx.x;
-  const int e = blockIdx.x / p.G;
-  const int gi = blockIdx.x - e * p.G;
+  const int e = blockIdx.x;
+  const int gi = blockIdx.y;
   const int4 g0 = __ldg(reinterpret_cast<const int4*>(p.groups + gi));
   const int4 g1 = __ldg(reinterpret_cast<const int4*>(p.groups + gi) + 1);
   const int gstart = g0.x, gcount = g0.y, patch0 = g0.z, npatch = g0.w, chunk0 = g1.x, nchunk = g1.y, gmcount = g1.w;
@@ -439,6 +444,27 @@ __global__ void __launch_bounds__(TS_BLOCK, 2) ts_step_kernel(const __grid_const
     hh[tid] = h;
     ha[tid] = h > 0.f ? __powf(h, p.alpha_e) : 0.f;
     if (h > 0.f) pact[lp] = 1;
+  }
+
+  // ---- state prefetch: the 12 (18) per-taxel state words of the noise chain are requested now so
+  // that their HBM latency is covered by the march and the force/torque phases.
+  float sY[6], sX[6], sD[6];
+  const size_t Tp = (size_t)p.Tp;
+  float* const st_h = p.st_hyst + (size_t)e * (p.hyst_mode == TS_HYST_MAXWELL ? 12 : 6) * Tp + j;
+  float* const st_d = p.st_drift + (size_t)e * 6 * Tp + j;
+#pragma unroll
+  for (int c = 0; c < 6; ++c) { sY[c] = 0.f; sX[c] = 0.f; sD[c] = 0.f; }
+  if (p.noise_enable && valid) {
+    if (p.hyst_mode != TS_HYST_OFF) {
+#pragma unroll
+      for (int c = 0; c < 6; ++c) sY[c] = __ldcs(st_h + c * Tp);
+    }
+    if (p.hyst_mode == TS_HYST_MAXWELL) {
+#pragma unroll
+      for (int c = 0; c < 6; ++c) sX[c] = __ldcs(st_h + (6 + c) * Tp);
+    }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) sD[c] = __ldcs(st_d + c * Tp);
   }
 
   // ---- phase 2 (S7): proximity march, t <- min(t + max(phi(q + t a), 0), r_prox), K_m evaluations.
@@ -561,29 +587,24 @@ __global__ void __launch_bounds__(TS_BLOCK, 2) ts_step_kernel(const __grid_const
   }
 
   // ---- phase 4 (S8): noise chain on the six channels (O8): hysteresis -> crosstalk -> drift -> dead
-  float outv[6];
   if (p.noise_enable) {
     float h[6];
-    const size_t Tp = (size_t)p.Tp;
     if (p.hyst_mode == TS_HYST_ASYM) {  // D3, Q14
-      float* st = p.st_hyst + (size_t)e * 6 * Tp + j;
 #pragma unroll
       for (int c = 0; c < 6; ++c) {
-        const float yp = valid ? __ldcs(st + c * Tp) : 0.f;
+        const float yp = sY[c];
         const float al = (fabsf(ft[c]) > fabsf(yp)) ? p.alpha_load : p.alpha_unload;
         h[c] = act ? fmaf(al, ft[c] - yp, yp) : 0.f;
-        if (valid) __stcs(st + c * Tp, h[c]);
+        if (valid) __stcs(st_h + c * Tp, h[c]);
       }
     } else if (p.hyst_mode == TS_HYST_MAXWELL) {  // Eq. 29-30
-      float* st = p.st_hyst + (size_t)e * 12 * Tp + j;
 #pragma unroll
       for (int c = 0; c < 6; ++c) {
-        const float xi = valid ? __ldcs(st + c * Tp) : 0.f, xp = valid ? __ldcs(st + (6 + c) * Tp) : 0.f;
-        const float z = act ? fmaf(p.decay, xi, ft[c] - xp) : 0.f;
+        const float z = act ? fmaf(p.decay, sY[c], ft[c] - sX[c]) : 0.f;
         h[c] = fmaf(p.beta, z, ft[c]);
         if (valid) {
-          __stcs(st + c * Tp, z);
-          __stcs(st + (6 + c) * Tp, act ? ft[c] : 0.f);
+          __stcs(st_h + c * Tp, z);
+          __stcs(st_h + (6 + c) * Tp, act ? ft[c] : 0.f);
         }
       }
     } else {
@@ -596,13 +617,6 @@ __global__ void __launch_bounds__(TS_BLOCK, 2) ts_step_kernel(const __grid_const
   __syncthreads();
   if (p.ft) block_store(p.ft + ((size_t)e * p.T + gstart) * 6, bufA, gcount * 6, tid);
   if (p.noise_enable) {
-    // S8c crosstalk (D4): c_j = h_j + chi/4 sum_{k in N4(j)} (h_k - h_j), neighbours from shared memory
-    const int4 nb = __ldg(p.tx_nbr + j);
-    const float q4 = 0.25f * p.chi;
-    float D[6];
-    float* sd = p.st_drift + (size_t)e * 6 * (size_t)p.Tp + j;
-#pragma unroll
-    for (int c = 0; c < 6; ++c) D[c] = valid ? __ldcs(sd + (size_t)c * p.Tp) : 0.f;
     // S8d drift draws (Eq. 25): Philox streams 0 / 1 -> six normals
     float z[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     if (act) {
@@ -615,18 +629,21 @@ __global__ void __launch_bounds__(TS_BLOCK, 2) ts_step_kernel(const __grid_const
       box_muller(w0.z, w0.w, z[2], z[3]);
       box_muller(w1.x, w1.y, z[4], z[5]);
     }
+    // S8c crosstalk (D4): c_j = h_j + chi/4 sum_{k in N4(j)} (h_k - h_j); a missing neighbour is
+    // replaced by the taxel itself (h_j - h_j = 0), so the sum needs no predicates.
+    const int4 nb = __ldg(p.tx_nbr + j);
+    const int n0 = nb.x >= 0 ? nb.x - gstart : tid, n1 = nb.y >= 0 ? nb.y - gstart : tid;
+    const int n2 = nb.z >= 0 ? nb.z - gstart : tid, n3 = nb.w >= 0 ? nb.w - gstart : tid;
+    const float q4 = 0.25f * p.chi;
+    float outv[6];
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
       const float* hb = bufB + c * TS_BLOCK;
       const float hc = hb[tid];
-      float acc = 0.f;
-      if (nb.x >= 0) acc += hb[nb.x - gstart] - hc;
-      if (nb.y >= 0) acc += hb[nb.y - gstart] - hc;
-      if (nb.z >= 0) acc += hb[nb.z - gstart] - hc;
-      if (nb.w >= 0) acc += hb[nb.w - gstart] - hc;
+      const float acc = ((hb[n0] - hc) + (hb[n1] - hc)) + ((hb[n2] - hc) + (hb[n3] - hc));
       const float cx = fmaf(q4, acc, hc);
-      const float Dn = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], D[c]) : 0.f;
-      if (valid) __stcs(sd + (size_t)c * p.Tp, Dn);
+      const float Dn = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], sD[c]) : 0.f;
+      if (valid) __stcs(st_d + c * Tp, Dn);
       outv[c] = (act && !deadb) ? cx + Dn : 0.f;  // S8a dead (Eq. 28) last
     }
     if (p.ft_noisy) {
@@ -652,73 +669,74 @@ __global__ void __launch_bounds__(TS_BLOCK, 2) ts_step_kernel(const __grid_const
       const int i1b = c0.x, i1e = c0.y, mb = c0.z, me = c0.w, lpb = c1.x, lpe = c1.y;
       bool any = false;
       for (int l = lpb; l < lpe; ++l) any = any || (pact[l] != 0);
-      if (any) {
-        if (i1b + tid < i1e) {  // pass 1
-          const int pk = __ldg(p.mk_item1 + i1b + tid);
-          const int l = pk & 255, a = (pk >> 8) & 255, q = pk >> 16;
-          const TsPatch& pt = p.patches[patch0 + l];
-          double s0 = 0.0, s1 = 0.0, t0 = 0.0;
-          if (pact[l] && !pt.direct) {
-            const int nu = pt.nu;
-            const double* GU = p.mk_tab + pt.tab + a * nu;
-            const double* DU = GU + pt.mnu * nu;
-            const int base = pt.start - gstart + q * nu;
-            for (int ip = 0; ip < nu; ++ip) {
-              const double h = (double)hh[base + ip], hal = (double)ha[base + ip], gu = __ldg(GU + ip);
-              s0 = fma(gu, h, s0);
-              s1 = fma(__ldg(DU + ip), h, s1);
-              t0 = fma(gu, hal, t0);
-            }
-          }
-          S[tid] = s0; S[TS_BLOCK + tid] = s1; S[2 * TS_BLOCK + tid] = t0;
-        }
-        __syncthreads();
+      if (!any) {  // no penetration anywhere in the chunk: the markers are exactly 0
+        float* o = p.marker + ((size_t)e * p.M + mb) * 3;
+        for (int i = tid; i < (me - mb) * 3; i += TS_BLOCK) __stcs(o + i, 0.f);
+        continue;
       }
-      if (mb + tid < me) {  // pass 2: one marker per thread
-        float ox = 0.f, oy = 0.f, oz = 0.f;
-        if (any) {
-          const int pk = __ldg(p.mk_item2 + mb + tid);
-          const int l = pk & 255, a = (pk >> 8) & 255, b = pk >> 16;
-          const TsPatch& pt = p.patches[patch0 + l];
-          if (pact[l]) {
-            if (!pt.direct) {
-              const int nv = pt.nv, mnu = pt.mnu;
-              const double* GV = p.mk_tab + pt.tab + 2 * mnu * pt.nu + b * nv;
-              const double* DV = GV + pt.mnv * nv;
-              const double* s = S + (pt.i1off - i1b + a);
-              double Uu = 0.0, Uv = 0.0, Un = 0.0;
-              for (int q = 0; q < nv; ++q) {
-                const double gv = __ldg(GV + q);
-                Uu = fma(gv, s[TS_BLOCK + q * mnu], Uu);
-                Uv = fma(__ldg(DV + q), s[q * mnu], Uv);
-                Un = fma(gv, s[2 * TS_BLOCK + q * mnu], Un);
-              }
-              const double sd = (double)p.s_d, kt = sd * p.inv_gbar;
-              const float4 ua = pt.ua, va = pt.va, na = pt.na;
-              ox = (float)(kt * fma(Uu, (double)ua.x, Uv * (double)va.x) + sd * Un * (double)na.x);
-              oy = (float)(kt * fma(Uu, (double)ua.y, Uv * (double)va.y) + sd * Un * (double)na.y);
-              oz = (float)(kt * fma(Uu, (double)ua.z, Uv * (double)va.z) + sd * Un * (double)na.z);
-            } else {  // direct sum (c_e != 1: rho(r) = 1/(|r|^2 + eps^2) is not separable)
-              const float4 mp = __ldg(p.mk_pos + mb + tid), mn = __ldg(p.mk_nrm + mb + tid);
-              const D3 n = D3{(double)mn.x, (double)mn.y, (double)mn.z};
-              const double eps = (double)pt.eps, ce = (double)p.c_e;
-              D3 acc = D3{0.0, 0.0, 0.0};
-              for (int i = 0; i < pt.n; ++i) {
-                const float hi = hh[pt.start - gstart + i];
-                if (!(hi > 0.f)) continue;
-                const float4 xs = __ldg(p.tx_pos + pt.start + i);
-                const D3 zv = D3{(double)mp.x - (double)xs.x, (double)mp.y - (double)xs.y, (double)mp.z - (double)xs.z};
-                const D3 rr = zv - dot(zv, n) * n;                                     // Eq. 18
-                const double r2 = dot(rr, rr);
-                const double gg = exp(-(double)p.lambda_d * r2);
-                const double w = (double)hi * (ce * gg * p.inv_gbar + (1.0 - ce) * (2.0 * eps) / (r2 + eps * eps));  // Eq. 20
-                acc = acc + (double)p.s_d * (w * rr + ((double)ha[pt.start - gstart + i] * gg) * n);              // Eq. 21
-              }
-              ox = (float)acc.x; oy = (float)acc.y; oz = (float)acc.z;
-            }
+      for (int it = tid; it < i1e - i1b; it += TS_BLOCK) {  // pass 1
+        const int pk = __ldg(p.mk_item1 + i1b + it);
+        const int l = pk & 255, a = (pk >> 8) & 255, q = pk >> 16;
+        const TsPatch& pt = p.patches[patch0 + l];
+        double s0 = 0.0, s1 = 0.0, t0 = 0.0;
+        if (pact[l]) {
+          const int nu = __ldg(&pt.nu);
+          const double* GU = p.mk_tab + __ldg(&pt.tab) + a * nu;
+          const double* DU = GU + __ldg(&pt.mnu) * nu;
+          const int base = __ldg(&pt.start) - gstart + q * nu;
+          for (int ip = 0; ip < nu; ++ip) {
+            const double h = (double)hh[base + ip], hal = (double)ha[base + ip], gu = __ldg(GU + ip);
+            s0 = fma(gu, h, s0);
+            s1 = fma(__ldg(DU + ip), h, s1);
+            t0 = fma(gu, hal, t0);
           }
         }
-        bufA[tid * 3] = ox; bufA[tid * 3 + 1] = oy; bufA[tid * 3 + 2] = oz;
+        S[it] = s0; S[TS_CHUNK + it] = s1; S[2 * TS_CHUNK + it] = t0;
+      }
+      __syncthreads();
+      for (int im = tid; im < me - mb; im += TS_BLOCK) {  // pass 2: one marker per item
+        float ox = 0.f, oy = 0.f, oz = 0.f;
+        const int pk = __ldg(p.mk_item2 + mb + im);
+        const int l = pk & 255, a = (pk >> 8) & 255, b = pk >> 16;
+        const TsPatch& pt = p.patches[patch0 + l];
+        if (pact[l]) {
+          if (!__ldg(&pt.direct)) {
+            const int nv = __ldg(&pt.nv), mnu = __ldg(&pt.mnu);
+            const double* GV = p.mk_tab + __ldg(&pt.tab) + 2 * mnu * __ldg(&pt.nu) + b * nv;
+            const double* DV = GV + __ldg(&pt.mnv) * nv;
+            const double* s = S + (__ldg(&pt.i1off) - i1b + a);
+            double Uu = 0.0, Uv = 0.0, Un = 0.0;
+            for (int q = 0; q < nv; ++q) {
+              const double gv = __ldg(GV + q);
+              Uu = fma(gv, s[TS_CHUNK + q * mnu], Uu);
+              Uv = fma(__ldg(DV + q), s[q * mnu], Uv);
+              Un = fma(gv, s[2 * TS_CHUNK + q * mnu], Un);
+            }
+            const double sd = (double)p.s_d, kt = sd * p.inv_gbar;
+            const float4 ua = __ldg(&pt.ua), va = __ldg(&pt.va), na = __ldg(&pt.na);
+            ox = (float)(kt * fma(Uu, (double)ua.x, Uv * (double)va.x) + sd * Un * (double)na.x);
+            oy = (float)(kt * fma(Uu, (double)ua.y, Uv * (double)va.y) + sd * Un * (double)na.y);
+            oz = (float)(kt * fma(Uu, (double)ua.z, Uv * (double)va.z) + sd * Un * (double)na.z);
+          } else {  // direct sum (c_e != 1: rho(r) = 1/(|r|^2 + eps^2) is not separable)
+            const float4 mp = __ldg(p.mk_pos + mb + im), mn = __ldg(p.mk_nrm + mb + im);
+            const D3 n = D3{(double)mn.x, (double)mn.y, (double)mn.z};
+            const double eps = (double)pt.eps, ce = (double)p.c_e;
+            D3 acc = D3{0.0, 0.0, 0.0};
+            for (int i = 0; i < pt.n; ++i) {
+              const float hi = hh[pt.start - gstart + i];
+              if (!(hi > 0.f)) continue;
+              const float4 xs = __ldg(p.tx_pos + pt.start + i);
+              const D3 zv = D3{(double)mp.x - (double)xs.x, (double)mp.y - (double)xs.y, (double)mp.z - (double)xs.z};
+              const D3 rr = zv - dot(zv, n) * n;                                     // Eq. 18
+              const double r2 = dot(rr, rr);
+              const double gg = exp(-(double)p.lambda_d * r2);
+              const double w = (double)hi * (ce * gg * p.inv_gbar + (1.0 - ce) * (2.0 * eps) / (r2 + eps * eps));  // Eq. 20
+              acc = acc + (double)p.s_d * (w * rr + ((double)ha[pt.start - gstart + i] * gg) * n);              // Eq. 21
+            }
+            ox = (float)acc.x; oy = (float)acc.y; oz = (float)acc.z;
+          }
+        }
+        bufA[im * 3] = ox; bufA[im * 3 + 1] = oy; bufA[im * 3 + 2] = oz;
       }
       __syncthreads();
       block_store(p.marker + ((size_t)e * p.M + mb) * 3, bufA, (me - mb) * 3, tid);
@@ -779,7 +797,7 @@ unsigned long long ts_bank_elems_per_grid(int N) { return (unsigned long long)(N
 
 unsigned long long ts_step_smem_bytes(const TsStepParams& p) {
   return (unsigned long long)p.frames_per_group * p.K * sizeof(FrameS) + sizeof(float) * (12 + 2) * TS_BLOCK +
-         sizeof(double) * 3 * TS_BLOCK + sizeof(int) * TS_MAX_GROUP_PATCHES;
+         sizeof(double) * 3 * TS_CHUNK + sizeof(int) * TS_MAX_GROUP_PATCHES;
 }
 
 int ts_prepare_kernels(int max_smem_bytes) {
@@ -789,13 +807,13 @@ int ts_prepare_kernels(int max_smem_bytes) {
 }
 
 int ts_launch_step(const TsStepParams& p, void* stream) {
-  const long long blocks = (long long)p.E * p.G;
-  if (blocks <= 0 || blocks > 0x7fffffffLL) return (int)cudaErrorInvalidConfiguration;
+  if (p.E <= 0 || p.G <= 0 || p.G > 65535) return (int)cudaErrorInvalidConfiguration;
   const size_t smem = (size_t)ts_step_smem_bytes(p);
+  const dim3 grid((unsigned)p.E, (unsigned)p.G);
   if (p.K == 1)
-    ts_step_kernel<true><<<(unsigned)blocks, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
+    ts_step_kernel<true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
   else
-    ts_step_kernel<false><<<(unsigned)blocks, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
+    ts_step_kernel<false><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
   return (int)cudaGetLastError();
 }
 
