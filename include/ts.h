@@ -224,6 +224,10 @@ int32_t ts_launches_per_step(const ts_ctx* ctx);
  * stream) and returns the mean duration in ms of the steps since the last call (after
  * synchronising those events).  enable = 0 switches recording off.  *n_steps gets the count. */
 ts_status ts_kernel_time_ms(ts_ctx* ctx, int32_t enable, float* mean_ms, int32_t* n_steps);
+/* Mean duration in ms of the FIRST kernel of a step (the geometry / fused kernel) over the steps the
+ * last ts_kernel_time_ms call averaged; the remainder of mean_ms is the separate noise kernel
+ * (0 when the step is one fused launch). */
+float ts_first_kernel_time_ms(const ts_ctx* ctx);
 
 const char* ts_version(void);
 

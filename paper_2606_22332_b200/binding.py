@@ -22,7 +22,7 @@ OUT_BITS = {"contact": 1, "depth": 2, "ft": 4, "marker": 8, "prox": 16, "ft_nois
 SYMBOLS = ["ts_layout_create", "ts_layout_add_patch", "ts_layout_filter_links", "ts_layout_finalize", "ts_layout_get",
            "ts_layout_destroy", "ts_config_default", "ts_create", "ts_set_geometry", "ts_step", "ts_step_host",
            "ts_reset", "ts_destroy", "ts_last_error", "ts_n_taxels", "ts_n_markers", "ts_launches_per_step",
-           "ts_kernel_time_ms", "ts_version"]
+           "ts_kernel_time_ms", "ts_first_kernel_time_ms", "ts_version"]
 
 
 class TsError(RuntimeError):
@@ -108,6 +108,8 @@ def lib():
         L.ts_n_markers.argtypes = [vp]
         L.ts_launches_per_step.argtypes = [vp]
         L.ts_kernel_time_ms.argtypes = [vp, i32, C.POINTER(C.c_float), C.POINTER(i32)]
+        L.ts_first_kernel_time_ms.argtypes = [vp]
+        L.ts_first_kernel_time_ms.restype = C.c_float
         L.ts_version.restype = C.c_char_p
         _lib = L
     return _lib
@@ -289,6 +291,9 @@ class TactileSim:
         ms, n = C.c_float(), C.c_int32()
         _check(lib().ts_kernel_time_ms(self.h, int(enable), C.byref(ms), C.byref(n)), self.h, "ts_kernel_time_ms")
         return ms.value, n.value
+
+    def first_kernel_time_ms(self):
+        return float(lib().ts_first_kernel_time_ms(self.h))
 
     def launches_per_step(self):
         return lib().ts_launches_per_step(self.h)

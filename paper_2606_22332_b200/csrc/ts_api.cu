@@ -3,12 +3,17 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
 #include <vector>
 
 #include "ts_internal.h"
+
+#ifndef TS_DEFAULT_SPLIT
+#define TS_DEFAULT_SPLIT 0
+#endif
 
 struct ts_ctx {
   int device = 0;
@@ -39,7 +44,10 @@ struct ts_ctx {
   void* stage_out[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   // timing of the main kernel
   bool timing = false;
-  std::vector<cudaEvent_t> ev;  // pairs
+  std::vector<cudaEvent_t> ev;  // triples: before the step kernel, after it, after the noise kernel
+  float last_first_kernel_ms = 0.f;
+  bool fused = true;            // one fused launch (default) or geometry + noise kernels (TS_SPLIT=1)
+  float* ft_scratch = nullptr;  // clean ft for the noise kernel when the caller does not ask for ft
   size_t ev_used = 0;
   std::string err;
 };
@@ -70,7 +78,7 @@ void free_all(ts_ctx* c) {
   cudaFree(c->tx_pos); cudaFree(c->tx_nrm); cudaFree(c->mk_pos); cudaFree(c->mk_nrm); cudaFree(c->patches);
   cudaFree(c->tx_nbr); cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab);
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->bank); cudaFree(c->st_flags); cudaFree(c->st_hyst);
-  cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode);
+  cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch);
   for (float* q : c->stage_in) cudaFree(q);
   for (void* q : c->stage_out) cudaFree(q);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
@@ -126,7 +134,7 @@ void ts_config_default(ts_config* c) {
 const char* ts_last_error(const ts_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 int32_t ts_n_taxels(const ts_ctx* ctx) { return ctx ? ctx->T : 0; }
 int32_t ts_n_markers(const ts_ctx* ctx) { return ctx ? ctx->M : 0; }
-int32_t ts_launches_per_step(const ts_ctx* ctx) { return ctx ? 1 : 0; }
+int32_t ts_launches_per_step(const ts_ctx* ctx) { return !ctx ? 0 : ((ctx->cfg.noise_enable && !ctx->fused) ? 2 : 1); }
 
 ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   if (!cfg || !out) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: NULL argument");
@@ -311,6 +319,11 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   TS_ALLOC(c->st_flags, E * T);
   TS_ALLOC(c->reset_step, sizeof(uint32_t) * E);
   TS_ALLOC(c->episode, sizeof(uint32_t) * E);
+  {
+    const char* sp = std::getenv("TS_SPLIT");
+    c->fused = !(sp ? (sp[0] == '1') : TS_DEFAULT_SPLIT);
+  }
+  if (cfg->noise_enable && !c->fused && !(cfg->output_mask & TS_OUT_FT)) TS_ALLOC(c->ft_scratch, sizeof(float) * E * T * 6);
   if (cfg->noise_enable) {
     if (c->nh) TS_ALLOC(c->st_hyst, sizeof(float) * E * c->nh * c->Tp);
     TS_ALLOC(c->st_drift, sizeof(float) * E * 6 * c->Tp);
@@ -409,21 +422,30 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
   p.contact = out->contact; p.depth = out->depth; p.ft = out->ft; p.marker = out->marker; p.prox = out->prox;
   p.ft_noisy = out->ft_noisy; p.dead = out->dead;
   cudaStream_t st = (cudaStream_t)stream;
-  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  const bool split = c->cfg.noise_enable && !c->fused;
+  if (split && !p.ft) {
+    if (!c->ft_scratch) return fail(c, TS_ERR_INVALID_ARG, "ts_step: ft is NULL although TS_OUT_FT is set in output_mask");
+    p.ft = c->ft_scratch;
+  }
+  cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
   if (c->timing) {
-    if (c->ev_used + 2 > c->ev.size()) {
-      cudaEvent_t a, b;
+    while (c->ev_used + 3 > c->ev.size()) {
+      cudaEvent_t a;
       TS_CUDA(c, cudaEventCreate(&a));
-      TS_CUDA(c, cudaEventCreate(&b));
-      c->ev.push_back(a); c->ev.push_back(b);
+      c->ev.push_back(a);
     }
-    e0 = c->ev[c->ev_used]; e1 = c->ev[c->ev_used + 1];
-    c->ev_used += 2;
+    e0 = c->ev[c->ev_used]; e1 = c->ev[c->ev_used + 1]; e2 = c->ev[c->ev_used + 2];
+    c->ev_used += 3;
     TS_CUDA(c, cudaEventRecord(e0, st));
   }
-  const cudaError_t e = (cudaError_t)ts_launch_step(p, st);
+  cudaError_t e = (cudaError_t)ts_launch_step(p, c->fused ? 1 : 0, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: launch");
   if (c->timing) TS_CUDA(c, cudaEventRecord(e1, st));
+  if (split) {
+    e = (cudaError_t)ts_launch_noise(p, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: noise launch");
+  }
+  if (c->timing) TS_CUDA(c, cudaEventRecord(e2, st));
   c->gstep += 1;
   return TS_OK;
 }
@@ -473,21 +495,25 @@ ts_status ts_reset(ts_ctx* c, const uint8_t* env_mask_dev, void* stream) {
 ts_status ts_kernel_time_ms(ts_ctx* c, int32_t enable, float* mean_ms, int32_t* n_steps) {
   if (!c) return TS_ERR_INVALID_ARG;
   DeviceGuard guard(c->device);
-  double sum = 0.0;
+  double sum = 0.0, sum1 = 0.0;
   int n = 0;
-  for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
-    TS_CUDA(c, cudaEventSynchronize(c->ev[i + 1]));
-    float ms = 0.f;
-    TS_CUDA(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
-    sum += ms;
+  for (size_t i = 0; i + 2 < c->ev_used; i += 3) {
+    TS_CUDA(c, cudaEventSynchronize(c->ev[i + 2]));
+    float ms = 0.f, ms1 = 0.f;
+    TS_CUDA(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 2]));
+    TS_CUDA(c, cudaEventElapsedTime(&ms1, c->ev[i], c->ev[i + 1]));
+    sum += ms; sum1 += ms1;
     ++n;
   }
+  c->last_first_kernel_ms = n ? (float)(sum1 / n) : 0.f;
   c->ev_used = 0;
   c->timing = enable != 0;
   if (mean_ms) *mean_ms = n ? (float)(sum / n) : 0.f;
   if (n_steps) *n_steps = n;
   return TS_OK;
 }
+
+float ts_first_kernel_time_ms(const ts_ctx* c) { return c ? c->last_first_kernel_ms : 0.f; }
 
 ts_status ts_destroy(ts_ctx* c) {
   if (!c) return TS_OK;

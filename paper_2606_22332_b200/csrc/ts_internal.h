@@ -115,7 +115,8 @@ struct TsStepParams {
 };
 
 // launchers (ts_kernels.cu)
-int ts_launch_step(const TsStepParams& p, void* stream);
+int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream);
+int ts_launch_noise(const TsStepParams& p, void* stream);
 int ts_launch_retile(const float* src_linear, float4* dst, int n_grids, int N, void* stream);
 int ts_launch_reset_counters(uint32_t* reset_step, uint32_t* episode, const uint8_t* mask, int E, uint32_t gstep,
                              void* stream);

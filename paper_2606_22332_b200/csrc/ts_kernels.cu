@@ -104,34 +104,52 @@ struct FrameS {
   int pad[3];
 };
 
-__device__ void build_frame(const TsStepParams& p, int e, int link, int k, FrameS& F) {
+// One frame is built by FOUR threads (part 0..2: row r of M and c[r]; part 3: the velocity terms),
+// which cuts the dependent double-precision chain the rest of the block waits for by ~4x.
+__device__ void build_frame_part(const TsStepParams& p, int e, int link, int k, int part, FrameS& F) {
   const size_t ek = (size_t)e * p.K + k;
-  F.type = (link >= 0) ? __ldg(p.g_type + ek) : TS_GEOM_NONE;
-  const float4 prm = __ldg(p.g_params + ek);
-  F.prm[0] = prm.x; F.prm[1] = prm.y; F.prm[2] = prm.z; F.prm[3] = prm.w;
+  if (part == 3) {
+    F.type = (link >= 0) ? __ldg(p.g_type + ek) : TS_GEOM_NONE;
+    const float4 prm = __ldg(p.g_params + ek);
+    F.prm[0] = prm.x; F.prm[1] = prm.y; F.prm[2] = prm.z; F.prm[3] = prm.w;
+  }
   if (link < 0) return;
   const size_t el = (size_t)e * p.L + link;
-  double RL[9], RO[9];
+  double RL[9];
   quat_Rd(p.link_quat + el * 4, RL);
-  quat_Rd(p.obj_quat + ek * 4, RO);
   const D3 d = ld3d(p.link_pos + el * 3) - ld3d(p.obj_pos + ek * 3);
-#pragma unroll
-  for (int r = 0; r < 3; ++r)
+  if (part < 3) {
+    const int r = part;
+    // column r of R_O, with (i, j, k) = (r, r+1, r+2) mod 3: R[i][i] = 1 - 2(q_j^2 + q_k^2),
+    // R[j][i] = 2(q_i q_j + w q_k), R[k][i] = 2(q_i q_k - w q_j)
+    const float4 q = __ldg(reinterpret_cast<const float4*>(p.obj_quat + ek * 4));
+    const double w = q.x;
+    const double qi = r == 0 ? q.y : (r == 1 ? q.z : q.w);
+    const double qj = r == 0 ? q.z : (r == 1 ? q.w : q.y);
+    const double qk = r == 0 ? q.w : (r == 1 ? q.y : q.z);
+    const double ci = 1.0 - 2.0 * (qj * qj + qk * qk), cj = 2.0 * (qi * qj + w * qk), ck = 2.0 * (qi * qk - w * qj);
+    // rows of R_O's column r in canonical order (row 0, 1, 2)
+    const double o0 = r == 0 ? ci : (r == 1 ? ck : cj);
+    const double o1 = r == 0 ? cj : (r == 1 ? ci : ck);
+    const double o2 = r == 0 ? ck : (r == 1 ? cj : ci);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      const double m = fma(RO[r], RL[c], fma(RO[3 + r], RL[3 + c], RO[6 + r] * RL[6 + c]));
+      const double m = fma(o0, RL[c], fma(o1, RL[3 + c], o2 * RL[6 + c]));
       F.M[r * 3 + c] = m;
       F.Mf[r * 3 + c] = (float)m;
     }
-  const D3 c = mulRT(RO, d), cb = mulRT(RL, d);
-  F.c[0] = c.x; F.c[1] = c.y; F.c[2] = c.z;
-  F.cf[0] = (float)c.x; F.cf[1] = (float)c.y; F.cf[2] = (float)c.z;
-  F.cbar[0] = cb.x; F.cbar[1] = cb.y; F.cbar[2] = cb.z;
-  const D3 wO = mulRT(RL, ld3d(p.obj_angvel + ek * 3)), wL = mulRT(RL, ld3d(p.link_angvel + el * 3));
-  const D3 vb = mulRT(RL, ld3d(p.obj_linvel + ek * 3) - ld3d(p.link_linvel + el * 3));
-  F.wO[0] = wO.x; F.wO[1] = wO.y; F.wO[2] = wO.z;
-  F.wL[0] = wL.x; F.wL[1] = wL.y; F.wL[2] = wL.z;
-  F.vbar[0] = vb.x; F.vbar[1] = vb.y; F.vbar[2] = vb.z;
+    const double cr = fma(o0, d.x, fma(o1, d.y, o2 * d.z));
+    F.c[r] = cr;
+    F.cf[r] = (float)cr;
+  } else {
+    const D3 cb = mulRT(RL, d);
+    F.cbar[0] = cb.x; F.cbar[1] = cb.y; F.cbar[2] = cb.z;
+    const D3 wO = mulRT(RL, ld3d(p.obj_angvel + ek * 3)), wL = mulRT(RL, ld3d(p.link_angvel + el * 3));
+    const D3 vb = mulRT(RL, ld3d(p.obj_linvel + ek * 3) - ld3d(p.link_linvel + el * 3));
+    F.wO[0] = wO.x; F.wO[1] = wO.y; F.wO[2] = wO.z;
+    F.wL[0] = wL.x; F.wL[1] = wL.y; F.wL[2] = wL.z;
+    F.vbar[0] = vb.x; F.vbar[1] = vb.y; F.vbar[2] = vb.z;
+  }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -367,107 +385,145 @@ __device__ __forceinline__ void block_store(float* dst, const float* src, int n,
   }
 }
 
+// six channels of one taxel ([E,T,6] row, 24 bytes, 8-byte aligned): three streaming 8-byte stores
+__device__ __forceinline__ void store6(float* dst, const float* v) {
+  float2* d2 = reinterpret_cast<float2*>(dst);
+  __stcs(d2, make_float2(v[0], v[1]));
+  __stcs(d2 + 1, make_float2(v[2], v[3]));
+  __stcs(d2 + 2, make_float2(v[4], v[5]));
+}
+
 #define TS_FULL 0xffffffffu
+#ifndef TS_MARCH_LAST
+#define TS_MARCH_LAST 0
+#endif
 #ifndef TS_MIN_BLOCKS
-#define TS_MIN_BLOCKS 3
+#define TS_MIN_BLOCKS 4
 #endif
 
 // ---------------------------------------------------------------------------------------
 // The fused step kernel: S1-S8 of DESIGN.md; block = (env, patch group), thread = taxel slot.
 // ---------------------------------------------------------------------------------------
-template <bool SINGLE>
-__global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const __grid_constant__ TsStepParams p) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int nfr = p.frames_per_group * p.K;
-  FrameS* frames = reinterpret_cast<FrameS*>(smem_raw);
-  float* bufA = reinterpret_cast<float*>(frames + nfr);   // [TS_BLOCK*6] output staging
-  float* bufB = bufA + 6 * TS_BLOCK;                      // [6][TS_BLOCK] crosstalk exchange
-  float* hh = bufB + 6 * TS_BLOCK;                        // [TS_BLOCK] penetration h_i (Eq. 19)
-  float* ha = hh + TS_BLOCK;                              // [TS_BLOCK] h_i^alpha_e
-  double* S = reinterpret_cast<double*>(ha + TS_BLOCK);   // [3][TS_CHUNK] marker pass-1 sums
-  int* pact = reinterpret_cast<int*>(S + 3 * TS_CHUNK);   // [TS_MAX_GROUP_PATCHES] patch has penetration
+// ---------------------------------------------------------------------------------------
+// S8: noise chain of one taxel (O8): hysteresis -> crosstalk -> drift -> dead.  Shared by the fused
+// step kernel and the stand-alone noise kernel.
+// ---------------------------------------------------------------------------------------
+struct NoiseState {
+  float sY[6], sX[6], sD[6];  // hysteresis y (asym) or xi (maxwell), maxwell x_prev, drift D
+};
 
-  const int tid = threadIdx.x;
-  const int e = blockIdx.x;
-  const int gi = blockIdx.y;
-  const int4 g0 = __ldg(reinterpret_cast<const int4*>(p.groups + gi));
-  const int4 g1 = __ldg(reinterpret_cast<const int4*>(p.groups + gi) + 1);
-  const int gstart = g0.x, gcount = g0.y, patch0 = g0.z, npatch = g0.w, chunk0 = g1.x, nchunk = g1.y, gmcount = g1.w;
-
-  // ---- phase 0: relative poses (double) -> shared memory ---------------------------------
-  if (tid < TS_MAX_GROUP_PATCHES) pact[tid] = 0;
-  for (int it = tid; it < npatch * p.K; it += TS_BLOCK) {
-    const int lp = it / p.K, k = it - lp * p.K;
-    build_frame(p, e, __ldg(&p.patches[patch0 + lp].link), k, frames[it]);
-  }
-  const bool valid = tid < gcount;
-  const int j = gstart + (valid ? tid : 0);
-  const size_t ej = (size_t)e * p.T + j;
-  const float4 P4 = __ldg(p.tx_pos + j), N4 = __ldg(p.tx_nrm + j);
-  const int lp = __float_as_int(N4.w);
-  const float Rj = valid ? P4.w : 0.f;  // R_j = 0: inactive slot (P:182)
-  const bool act = Rj > 0.f;
-  uint8_t flag = valid ? p.st_flags[ej] : (uint8_t)0;
-  __syncthreads();
-
-  // ---- phase 1 (S1-S4): x_o = c + M x_j, phi = min_k phi_k, depth (Eq. 2), contact (Eq. 3) ----
-  double phid = __longlong_as_double(0x7ff0000000000000LL);
-  D3 xd = D3{0.0, 0.0, 0.0};
-  int kst = 0;
-  if (act) {
-    const D3 xj = D3{(double)P4.x, (double)P4.y, (double)P4.z};
-    for (int k = 0; k < (SINGLE ? 1 : p.K); ++k) {
-      const FrameS& F = frames[lp * (SINGLE ? 1 : p.K) + k];
-      const D3 x = ldv(F.c) + mulR(F.M, xj);
-      const double ph = phi_d(p, F.type, F.prm, x);
-      if (ph < phid) {  // strict: ties -> lowest k (Q3)
-        phid = ph; kst = k; xd = x;
-      }
-    }
-  }
-  const float phif = (float)phid;
-  float d = 0.f;
-  if (act) {
-    const double dd = (double)Rj - phid;
-    d = dd > 0.0 ? (float)dd : 0.f;
-  }
-  const bool yb = act && ((d > p.eta_on) || ((flag & 1) && d > p.eta_off));
-  const bool deadb = p.noise_enable && act && ((flag >> 1) & 1);
-  if (valid) {
-    p.st_flags[ej] = (uint8_t)((flag & 2) | (yb ? 1 : 0));  // Schmitt state from the un-masked bit (O4)
-    if (p.contact) p.contact[ej] = (yb && !deadb) ? 1 : 0;
-    if (p.dead) p.dead[ej] = deadb ? 1 : 0;
-    if (p.depth) __stcs(p.depth + ej, d);
-  }
-  if (p.marker) {  // Eq. 19: h_i = max(0, -phi), no R_j
-    const float h = (act && phid < 0.0) ? (float)(-phid) : 0.f;
-    hh[tid] = h;
-    ha[tid] = h > 0.f ? __powf(h, p.alpha_e) : 0.f;
-    if (h > 0.f) pact[lp] = 1;
-  }
-
-  // ---- state prefetch: the 12 (18) per-taxel state words of the noise chain are requested now so
-  // that their HBM latency is covered by the march and the force/torque phases.
-  float sY[6], sX[6], sD[6];
+__device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, bool valid, NoiseState& ns) {
   const size_t Tp = (size_t)p.Tp;
-  float* const st_h = p.st_hyst + (size_t)e * (p.hyst_mode == TS_HYST_MAXWELL ? 12 : 6) * Tp + j;
-  float* const st_d = p.st_drift + (size_t)e * 6 * Tp + j;
+  const float* st_h = p.st_hyst + (size_t)e * (p.hyst_mode == TS_HYST_MAXWELL ? 12 : 6) * Tp + j;
+  const float* st_d = p.st_drift + (size_t)e * 6 * Tp + j;
 #pragma unroll
-  for (int c = 0; c < 6; ++c) { sY[c] = 0.f; sX[c] = 0.f; sD[c] = 0.f; }
-  if (p.noise_enable && valid) {
+  for (int c = 0; c < 6; ++c) { ns.sY[c] = 0.f; ns.sX[c] = 0.f; ns.sD[c] = 0.f; }
+  if (valid) {
     if (p.hyst_mode != TS_HYST_OFF) {
 #pragma unroll
-      for (int c = 0; c < 6; ++c) sY[c] = __ldcs(st_h + c * Tp);
+      for (int c = 0; c < 6; ++c) ns.sY[c] = __ldcs(st_h + c * Tp);
     }
     if (p.hyst_mode == TS_HYST_MAXWELL) {
 #pragma unroll
-      for (int c = 0; c < 6; ++c) sX[c] = __ldcs(st_h + (6 + c) * Tp);
+      for (int c = 0; c < 6; ++c) ns.sX[c] = __ldcs(st_h + (6 + c) * Tp);
     }
 #pragma unroll
-    for (int c = 0; c < 6; ++c) sD[c] = __ldcs(st_d + c * Tp);
+    for (int c = 0; c < 6; ++c) ns.sD[c] = __ldcs(st_d + c * Tp);
   }
+}
 
-  // ---- phase 2 (S7): proximity march, t <- min(t + max(phi(q + t a), 0), r_prox), K_m evaluations.
+// Every thread of the block must call this (it contains one __syncthreads).
+__device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, size_t ej, int tid, int gstart, bool valid,
+                                            bool act, bool deadb, const float* ft, const NoiseState& ns, float* bufB) {
+  const size_t Tp = (size_t)p.Tp;
+  float* const st_h = p.st_hyst + (size_t)e * (p.hyst_mode == TS_HYST_MAXWELL ? 12 : 6) * Tp + j;
+  float* const st_d = p.st_drift + (size_t)e * 6 * Tp + j;
+  float h[6];
+  if (p.hyst_mode == TS_HYST_ASYM) {  // D3, Q14
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+      const float yp = ns.sY[c];
+      const float al = (fabsf(ft[c]) > fabsf(yp)) ? p.alpha_load : p.alpha_unload;
+      h[c] = act ? fmaf(al, ft[c] - yp, yp) : 0.f;
+      if (valid) __stcs(st_h + c * Tp, h[c]);
+    }
+  } else if (p.hyst_mode == TS_HYST_MAXWELL) {  // Eq. 29-30
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+      const float z = act ? fmaf(p.decay, ns.sY[c], ft[c] - ns.sX[c]) : 0.f;
+      h[c] = fmaf(p.beta, z, ft[c]);
+      if (valid) {
+        __stcs(st_h + c * Tp, z);
+        __stcs(st_h + (6 + c) * Tp, act ? ft[c] : 0.f);
+      }
+    }
+  } else {
+#pragma unroll
+    for (int c = 0; c < 6; ++c) h[c] = ft[c];
+  }
+#pragma unroll
+  for (int c = 0; c < 6; ++c) bufB[c * TS_BLOCK + tid] = h[c];
+  // S8d drift draws (Eq. 25): Philox streams 0 / 1 -> six normals (before the barrier: independent work)
+  float z[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (act) {
+    const uint32_t nstep = p.gstep - __ldg(p.reset_step + e);
+    const uint32_t ep4 = __ldg(p.episode + e) << 4;
+    const uint32_t env = p.env_id_base + (uint32_t)e;
+    const uint4 w0 = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 0u), p.seed_lo, p.seed_hi);
+    const uint4 w1 = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 1u), p.seed_lo, p.seed_hi);
+    box_muller(w0.x, w0.y, z[0], z[1]);
+    box_muller(w0.z, w0.w, z[2], z[3]);
+    box_muller(w1.x, w1.y, z[4], z[5]);
+  }
+  __syncthreads();
+  // S8c crosstalk (D4): c_j = h_j + chi/4 sum_{k in N4(j)} (h_k - h_j); a missing neighbour is
+  // replaced by the taxel itself (h_j - h_j = 0), so the sum needs no predicates.
+  const int4 nb = __ldg(p.tx_nbr + j);
+  const int n0 = nb.x >= 0 ? nb.x - gstart : tid, n1 = nb.y >= 0 ? nb.y - gstart : tid;
+  const int n2 = nb.z >= 0 ? nb.z - gstart : tid, n3 = nb.w >= 0 ? nb.w - gstart : tid;
+  const float q4 = 0.25f * p.chi;
+  float outv[6];
+#pragma unroll
+  for (int c = 0; c < 6; ++c) {
+    const float* hb = bufB + c * TS_BLOCK;
+    const float hc = h[c];
+    const float acc = ((hb[n0] - hc) + (hb[n1] - hc)) + ((hb[n2] - hc) + (hb[n3] - hc));
+    const float cx = fmaf(q4, acc, hc);
+    const float Dn = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], ns.sD[c]) : 0.f;
+    if (valid) __stcs(st_d + c * Tp, Dn);
+    outv[c] = (act && !deadb) ? cx + Dn : 0.f;  // S8a dead (Eq. 28) last
+  }
+  if (p.ft_noisy && valid) store6(p.ft_noisy + ej * 6, outv);
+}
+
+// Stand-alone noise kernel (split variant): reads the clean ft the geometry kernel wrote.
+__global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_constant__ TsStepParams p) {
+  __shared__ float bufB[6 * TS_BLOCK];
+  const int tid = threadIdx.x;
+  const int e = blockIdx.x;
+  const int4 g0 = __ldg(reinterpret_cast<const int4*>(p.groups + blockIdx.y));
+  const int gstart = g0.x, gcount = g0.y;
+  const bool valid = tid < gcount;
+  const int j = gstart + (valid ? tid : 0);
+  const size_t ej = (size_t)e * p.T + j;
+  NoiseState ns;
+  noise_load(p, e, j, valid, ns);
+  float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  bool act = false, deadb = false;
+  if (valid) {
+    const float2* f2 = reinterpret_cast<const float2*>(p.ft + ej * 6);
+    const float2 a = __ldcs(f2), b = __ldcs(f2 + 1), c = __ldcs(f2 + 2);
+    ft[0] = a.x; ft[1] = a.y; ft[2] = b.x; ft[3] = b.y; ft[4] = c.x; ft[5] = c.y;
+    act = __ldg(&p.tx_pos[j].w) > 0.f;
+    deadb = act && ((p.st_flags[ej] >> 1) & 1);
+  }
+  noise_chain(p, e, j, ej, tid, gstart, valid, act, deadb, ft, ns, bufB);
+}
+
+template <bool SINGLE>
+__device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS* frames, int e, int lp, bool valid, bool act,
+                                            size_t ej, float phif, F3 xo, float4 P4, float4 N4) {
+// ---- phase 2 (S7): proximity march, t <- min(t + max(phi(q + t a), 0), r_prox), K_m evaluations.
   // Exact shortcuts (O7): evaluation 0 is the query above; t = r_prox is absorbing; an evaluation
   // that leaves t unchanged repeats forever.
   if (p.prox) {
@@ -481,7 +537,6 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     if (SINGLE) {
       const FrameS& F = frames[lp];
       const int gtype = __ldg(p.g_type + e);  // block-uniform (one object per env)
-      const F3 xo = mk3((float)xd.x, (float)xd.y, (float)xd.z);
       const F3 dr = mk3(fmaf(F.Mf[0], nj.x, fmaf(F.Mf[1], nj.y, F.Mf[2] * nj.z)), fmaf(F.Mf[3], nj.x, fmaf(F.Mf[4], nj.y, F.Mf[5] * nj.z)),
                         fmaf(F.Mf[6], nj.x, fmaf(F.Mf[7], nj.y, F.Mf[8] * nj.z)));
       if (gtype == TS_GEOM_SDF) {
@@ -548,10 +603,91 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     }
     if (valid) __stcs(p.prox + ej, act ? p.r_prox - t : 0.f);
   }
+}
+
+template <bool SINGLE, bool NOISE>
+__global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const __grid_constant__ TsStepParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int nfr = p.frames_per_group * p.K;
+  FrameS* frames = reinterpret_cast<FrameS*>(smem_raw);
+  float* bufA = reinterpret_cast<float*>(frames + nfr);   // [TS_BLOCK*6] output staging
+  float* bufB = bufA + 6 * TS_BLOCK;                      // [6][TS_BLOCK] crosstalk exchange
+  float* hh = bufB + 6 * TS_BLOCK;                        // [TS_BLOCK] penetration h_i (Eq. 19)
+  float* ha = hh + TS_BLOCK;                              // [TS_BLOCK] h_i^alpha_e
+  double* S = reinterpret_cast<double*>(ha + TS_BLOCK);   // [3][TS_CHUNK] marker pass-1 sums
+  int* pact = reinterpret_cast<int*>(S + 3 * TS_CHUNK);   // [TS_MAX_GROUP_PATCHES] patch has penetration
+
+  const int tid = threadIdx.x;
+  const int e = blockIdx.x;
+  const int gi = blockIdx.y;
+  const int4 g0 = __ldg(reinterpret_cast<const int4*>(p.groups + gi));
+  const int4 g1 = __ldg(reinterpret_cast<const int4*>(p.groups + gi) + 1);
+  const int gstart = g0.x, gcount = g0.y, patch0 = g0.z, npatch = g0.w, chunk0 = g1.x, nchunk = g1.y, gmcount = g1.w;
+
+  // ---- phase 0: relative poses (double) -> shared memory ---------------------------------
+  if (tid < TS_MAX_GROUP_PATCHES) pact[tid] = 0;
+  for (int it = tid; it < 4 * npatch * p.K; it += TS_BLOCK) {
+    const int f = it >> 2, lpf = f / p.K, k = f - lpf * p.K;
+    build_frame_part(p, e, __ldg(&p.patches[patch0 + lpf].link), k, it & 3, frames[f]);
+  }
+  const bool valid = tid < gcount;
+  const int j = gstart + (valid ? tid : 0);
+  const size_t ej = (size_t)e * p.T + j;
+  const float4 P4 = __ldg(p.tx_pos + j), N4 = __ldg(p.tx_nrm + j);
+  const int lp = __float_as_int(N4.w);
+  const float Rj = valid ? P4.w : 0.f;  // R_j = 0: inactive slot (P:182)
+  const bool act = Rj > 0.f;
+  uint8_t flag = valid ? p.st_flags[ej] : (uint8_t)0;
+  __syncthreads();
+
+  // ---- phase 1 (S1-S4): x_o = c + M x_j, phi = min_k phi_k, depth (Eq. 2), contact (Eq. 3) ----
+  double phid = __longlong_as_double(0x7ff0000000000000LL);
+  D3 xd = D3{0.0, 0.0, 0.0};
+  int kst = 0;
+  if (act) {
+    const D3 xj = D3{(double)P4.x, (double)P4.y, (double)P4.z};
+    for (int k = 0; k < (SINGLE ? 1 : p.K); ++k) {
+      const FrameS& F = frames[lp * (SINGLE ? 1 : p.K) + k];
+      const D3 x = ldv(F.c) + mulR(F.M, xj);
+      const double ph = phi_d(p, F.type, F.prm, x);
+      if (ph < phid) {  // strict: ties -> lowest k (Q3)
+        phid = ph; kst = k; xd = x;
+      }
+    }
+  }
+  const float phif = (float)phid;
+  float d = 0.f;
+  if (act) {
+    const double dd = (double)Rj - phid;
+    d = dd > 0.0 ? (float)dd : 0.f;
+  }
+  const bool yb = act && ((d > p.eta_on) || ((flag & 1) && d > p.eta_off));
+  const bool deadb = p.noise_enable && act && ((flag >> 1) & 1);
+  if (valid) {
+    p.st_flags[ej] = (uint8_t)((flag & 2) | (yb ? 1 : 0));  // Schmitt state from the un-masked bit (O4)
+    if (p.contact) p.contact[ej] = (yb && !deadb) ? 1 : 0;
+    if (p.dead) p.dead[ej] = deadb ? 1 : 0;
+    if (p.depth) __stcs(p.depth + ej, d);
+  }
+  if (p.marker) {  // Eq. 19: h_i = max(0, -phi), no R_j
+    const float h = (act && phid < 0.0) ? (float)(-phid) : 0.f;
+    hh[tid] = h;
+    ha[tid] = h > 0.f ? __powf(h, p.alpha_e) : 0.f;
+    if (h > 0.f) pact[lp] = 1;
+  }
+  const F3 xo = mk3((float)xd.x, (float)xd.y, (float)xd.z);  // kept for the march (last phase)
+
+  // state prefetch: the 12 (18) per-taxel state words of the noise chain are requested now so that their
+  // HBM latency is covered by the march and the force/torque phases.
+  NoiseState ns;
+  if (NOISE) noise_load(p, e, j, valid, ns);
+#if !TS_MARCH_LAST
+  march_phase<SINGLE>(p, frames, e, lp, valid, act, ej, phif, xo, P4, N4);
+#endif
 
   // ---- phase 3 (S5): kinematic force / torque (Eq. 4-9, D2) in double, link frame ---------------
   float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  if ((p.ft != nullptr || p.noise_enable) && __any_sync(TS_FULL, d > 0.f)) {
+  if ((p.ft != nullptr || NOISE) && __any_sync(TS_FULL, d > 0.f)) {
     if (d > 0.f) {  // Q5: every term gated on d > 0
       const FrameS& F = frames[lp * (SINGLE ? 1 : p.K) + kst];
       const D3 g = grad_d(p, F.type, F.prm, xd);
@@ -581,79 +717,11 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
       ft[3] = (float)tau.x; ft[4] = (float)tau.y; ft[5] = (float)tau.z;
     }
   }
-  if (p.ft) {
-#pragma unroll
-    for (int c = 0; c < 6; ++c) bufA[tid * 6 + c] = ft[c];
-  }
+  if (p.ft && valid) store6(p.ft + ej * 6, ft);
 
-  // ---- phase 4 (S8): noise chain on the six channels (O8): hysteresis -> crosstalk -> drift -> dead
-  if (p.noise_enable) {
-    float h[6];
-    if (p.hyst_mode == TS_HYST_ASYM) {  // D3, Q14
-#pragma unroll
-      for (int c = 0; c < 6; ++c) {
-        const float yp = sY[c];
-        const float al = (fabsf(ft[c]) > fabsf(yp)) ? p.alpha_load : p.alpha_unload;
-        h[c] = act ? fmaf(al, ft[c] - yp, yp) : 0.f;
-        if (valid) __stcs(st_h + c * Tp, h[c]);
-      }
-    } else if (p.hyst_mode == TS_HYST_MAXWELL) {  // Eq. 29-30
-#pragma unroll
-      for (int c = 0; c < 6; ++c) {
-        const float z = act ? fmaf(p.decay, sY[c], ft[c] - sX[c]) : 0.f;
-        h[c] = fmaf(p.beta, z, ft[c]);
-        if (valid) {
-          __stcs(st_h + c * Tp, z);
-          __stcs(st_h + (6 + c) * Tp, act ? ft[c] : 0.f);
-        }
-      }
-    } else {
-#pragma unroll
-      for (int c = 0; c < 6; ++c) h[c] = ft[c];
-    }
-#pragma unroll
-    for (int c = 0; c < 6; ++c) bufB[c * TS_BLOCK + tid] = h[c];
-  }
-  __syncthreads();
-  if (p.ft) block_store(p.ft + ((size_t)e * p.T + gstart) * 6, bufA, gcount * 6, tid);
-  if (p.noise_enable) {
-    // S8d drift draws (Eq. 25): Philox streams 0 / 1 -> six normals
-    float z[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    if (act) {
-      const uint32_t nstep = p.gstep - __ldg(p.reset_step + e);
-      const uint32_t ep4 = __ldg(p.episode + e) << 4;
-      const uint32_t env = p.env_id_base + (uint32_t)e;
-      const uint4 w0 = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 0u), p.seed_lo, p.seed_hi);
-      const uint4 w1 = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 1u), p.seed_lo, p.seed_hi);
-      box_muller(w0.x, w0.y, z[0], z[1]);
-      box_muller(w0.z, w0.w, z[2], z[3]);
-      box_muller(w1.x, w1.y, z[4], z[5]);
-    }
-    // S8c crosstalk (D4): c_j = h_j + chi/4 sum_{k in N4(j)} (h_k - h_j); a missing neighbour is
-    // replaced by the taxel itself (h_j - h_j = 0), so the sum needs no predicates.
-    const int4 nb = __ldg(p.tx_nbr + j);
-    const int n0 = nb.x >= 0 ? nb.x - gstart : tid, n1 = nb.y >= 0 ? nb.y - gstart : tid;
-    const int n2 = nb.z >= 0 ? nb.z - gstart : tid, n3 = nb.w >= 0 ? nb.w - gstart : tid;
-    const float q4 = 0.25f * p.chi;
-    float outv[6];
-#pragma unroll
-    for (int c = 0; c < 6; ++c) {
-      const float* hb = bufB + c * TS_BLOCK;
-      const float hc = hb[tid];
-      const float acc = ((hb[n0] - hc) + (hb[n1] - hc)) + ((hb[n2] - hc) + (hb[n3] - hc));
-      const float cx = fmaf(q4, acc, hc);
-      const float Dn = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], sD[c]) : 0.f;
-      if (valid) __stcs(st_d + c * Tp, Dn);
-      outv[c] = (act && !deadb) ? cx + Dn : 0.f;  // S8a dead (Eq. 28) last
-    }
-    if (p.ft_noisy) {
-      __syncthreads();  // bufA drained by the ft store
-#pragma unroll
-      for (int c = 0; c < 6; ++c) bufA[tid * 6 + c] = outv[c];
-      __syncthreads();
-      block_store(p.ft_noisy + ((size_t)e * p.T + gstart) * 6, bufA, gcount * 6, tid);
-    }
-  }
+  // ---- phase 4 (S8): noise chain (fused variant); contains the barrier that also publishes hh / ha / pact
+  if (NOISE) noise_chain(p, e, j, ej, tid, gstart, valid, act, deadb, ft, ns, bufB);
+  else __syncthreads();
 
   // ---- phase 5 (S6): elastomer marker dilation (Eq. 18-21, 23 first sum) ----------------------
   // With c = 1 and planar regular grids, g(r_ij) = exp(-lambda |r|^2) = gu(a,p) gv(b,q) and
@@ -662,7 +730,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   //   pass 2 over (a,b): Uu = sum_q gv S1, Uv = sum_q dv gv S0, Un = sum_q gv T0.
   // Sources with h_i = 0 contribute exactly 0; patches without penetration are skipped.
   if (p.marker && gmcount > 0) {
-    __syncthreads();  // hh / ha / pact complete, bufA free
+    // hh / ha / pact were completed by the barrier above
     for (int ch = 0; ch < nchunk; ++ch) {
       const int4 c0 = __ldg(reinterpret_cast<const int4*>(p.chunks + chunk0 + ch));
       const int4 c1 = __ldg(reinterpret_cast<const int4*>(p.chunks + chunk0 + ch) + 1);
@@ -740,9 +808,13 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
       }
       __syncthreads();
       block_store(p.marker + ((size_t)e * p.M + mb) * 3, bufA, (me - mb) * 3, tid);
-      __syncthreads();
+      if (ch + 1 < nchunk) __syncthreads();  // S and bufA are reused by the next chunk
     }
   }
+
+#if TS_MARCH_LAST
+  march_phase<SINGLE>(p, frames, e, lp, valid, act, ej, phif, xo, P4, N4);
+#endif
 }
 
 // ---------------------------------------------------------------------------------------
@@ -801,19 +873,33 @@ unsigned long long ts_step_smem_bytes(const TsStepParams& p) {
 }
 
 int ts_prepare_kernels(int max_smem_bytes) {
-  cudaError_t e = cudaFuncSetAttribute(ts_step_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(ts_step_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
+  cudaError_t e = cudaFuncSetAttribute(ts_step_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(ts_step_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(ts_step_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(ts_step_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
   return (int)e;
 }
 
-int ts_launch_step(const TsStepParams& p, void* stream) {
+// fused_noise != 0: one launch does everything; otherwise the geometry kernel, and (noise on) ts_launch_noise.
+int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
   if (p.E <= 0 || p.G <= 0 || p.G > 65535) return (int)cudaErrorInvalidConfiguration;
   const size_t smem = (size_t)ts_step_smem_bytes(p);
   const dim3 grid((unsigned)p.E, (unsigned)p.G);
-  if (p.K == 1)
-    ts_step_kernel<true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
-  else
-    ts_step_kernel<false><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
+  cudaStream_t st = (cudaStream_t)stream;
+  const bool nz = p.noise_enable && fused_noise;
+  if (p.K == 1) {
+    if (nz) ts_step_kernel<true, true><<<grid, TS_BLOCK, smem, st>>>(p);
+    else ts_step_kernel<true, false><<<grid, TS_BLOCK, smem, st>>>(p);
+  } else {
+    if (nz) ts_step_kernel<false, true><<<grid, TS_BLOCK, smem, st>>>(p);
+    else ts_step_kernel<false, false><<<grid, TS_BLOCK, smem, st>>>(p);
+  }
+  return (int)cudaGetLastError();
+}
+
+int ts_launch_noise(const TsStepParams& p, void* stream) {
+  const dim3 grid((unsigned)p.E, (unsigned)p.G);
+  ts_noise_kernel<<<grid, TS_BLOCK, 0, (cudaStream_t)stream>>>(p);
   return (int)cudaGetLastError();
 }
 
