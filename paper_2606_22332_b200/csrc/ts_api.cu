@@ -28,7 +28,7 @@ struct ts_ctx {
   TsPatch* patches = nullptr;
   TsGroup* groups = nullptr;
   TsChunk* chunks = nullptr;
-  int32_t *mk_item1 = nullptr, *mk_item2 = nullptr;
+  int32_t *mk_item1 = nullptr, *mk_item2 = nullptr, *grp_link = nullptr;
   double* mk_tab = nullptr;
   int32_t* g_type = nullptr;
   float4* g_params = nullptr;
@@ -76,7 +76,7 @@ struct DeviceGuard {
 
 void free_all(ts_ctx* c) {
   cudaFree(c->tx_pos); cudaFree(c->tx_nrm); cudaFree(c->mk_pos); cudaFree(c->mk_nrm); cudaFree(c->patches);
-  cudaFree(c->tx_nbr); cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab);
+  cudaFree(c->tx_nbr); cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->grp_link);
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->bank); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch);
   for (float* q : c->stage_in) cudaFree(q);
@@ -90,7 +90,7 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.E = g.n_envs; p.L = g.n_links; p.K = g.objs_per_env; p.T = c->T; p.P = c->P; p.M = c->M;
   p.G = c->G; p.Tp = c->Tp; p.frames_per_group = c->frames_per_group;
   p.tx_nbr = c->tx_nbr; p.groups = c->groups; p.chunks = c->chunks; p.mk_item1 = c->mk_item1; p.mk_item2 = c->mk_item2;
-  p.mk_tab = c->mk_tab;
+  p.mk_tab = c->mk_tab; p.grp_link = c->grp_link;
   p.env_id_base = (uint32_t)g.env_id_base;
   p.tx_pos = c->tx_pos; p.tx_nrm = c->tx_nrm; p.patches = c->patches; p.mk_pos = c->mk_pos; p.mk_nrm = c->mk_nrm;
   p.g_type = c->g_type; p.g_params = c->g_params; p.bank = c->bank;
@@ -276,6 +276,9 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     }
     groups.push_back(g);
   }
+  std::vector<int32_t> glink(groups.size() * TS_MAX_GROUP_PATCHES, -1);
+  for (size_t gi = 0; gi < groups.size(); ++gi)
+    for (int l = 0; l < groups[gi].npatch; ++l) glink[gi * TS_MAX_GROUP_PATCHES + l] = pts[groups[gi].patch0 + l].link;
   if (item1.empty()) item1.push_back(0);
   if (tab.empty()) tab.push_back(0.0);
   if (chunks.empty()) chunks.push_back(TsChunk{});
@@ -311,6 +314,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   TS_ALLOC(c->patches, sizeof(TsPatch) * pts.size());
   TS_ALLOC(c->groups, sizeof(TsGroup) * groups.size());
   TS_ALLOC(c->chunks, sizeof(TsChunk) * chunks.size());
+  TS_ALLOC(c->grp_link, sizeof(int32_t) * glink.size());
   TS_ALLOC(c->mk_item1, sizeof(int32_t) * item1.size());
   TS_ALLOC(c->mk_item2, sizeof(int32_t) * item2.size());
   TS_ALLOC(c->mk_tab, sizeof(double) * tab.size());
@@ -339,6 +343,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   cp(c->patches, pts.data(), sizeof(TsPatch) * pts.size());
   cp(c->groups, groups.data(), sizeof(TsGroup) * groups.size());
   cp(c->chunks, chunks.data(), sizeof(TsChunk) * chunks.size());
+  cp(c->grp_link, glink.data(), sizeof(int32_t) * glink.size());
   cp(c->mk_item1, item1.data(), sizeof(int32_t) * item1.size());
   cp(c->mk_item2, item2.data(), sizeof(int32_t) * item2.size());
   cp(c->mk_tab, tab.data(), sizeof(double) * tab.size());

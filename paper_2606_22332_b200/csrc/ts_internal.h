@@ -70,6 +70,7 @@ struct TsStepParams {
   const TsPatch* patches; // [P]
   const TsGroup* groups;  // [G]
   const TsChunk* chunks;
+  const int32_t* grp_link;  // [G][TS_MAX_GROUP_PATCHES] sensor link of each patch of a group (-1 = filler)
   const int32_t* mk_item1;  // packed lp | a << 8 | q << 16
   const int32_t* mk_item2;  // [M] packed lp | a << 8 | b << 16
   const double* mk_tab;     // per patch: GU[mnu][nu], DU[mnu][nu], GV[mnv][nv], DV[mnv][nv]

@@ -104,11 +104,42 @@ struct FrameS {
   int pad[3];
 };
 
-// One frame is built by FOUR threads (part 0..2: row r of M and c[r]; part 3: the velocity terms),
-// which cuts the dependent double-precision chain the rest of the block waits for by ~4x.
-__device__ void build_frame_part(const TsStepParams& p, int e, int link, int k, int part, FrameS& F) {
+// One frame is built by SEVEN threads so that the dependent double-precision chain the whole block
+// waits for stays short (~60 instructions): "row" items r = 0..2 (row r of M and c[r]) run in the lower
+// half of the block, "vector" items s = 0..3 (wO, wL, vbar, cbar) in the upper half, so a warp never
+// executes both code paths.
+__device__ __forceinline__ void build_frame_row(const TsStepParams& p, int e, int link, int k, int r, FrameS& F) {
+  if (link < 0) return;
+  const size_t ek = (size_t)e * p.K + k, el = (size_t)e * p.L + link;
+  double RL[9];
+  quat_Rd(p.link_quat + el * 4, RL);
+  const D3 d = ld3d(p.link_pos + el * 3) - ld3d(p.obj_pos + ek * 3);
+  // column r of R_O, with (i, j, k) = (r, r+1, r+2) mod 3: R[i][i] = 1 - 2(q_j^2 + q_k^2),
+  // R[j][i] = 2(q_i q_j + w q_k), R[k][i] = 2(q_i q_k - w q_j)
+  const float4 q = __ldg(reinterpret_cast<const float4*>(p.obj_quat + ek * 4));
+  const double w = q.x;
+  const double qi = r == 0 ? q.y : (r == 1 ? q.z : q.w);
+  const double qj = r == 0 ? q.z : (r == 1 ? q.w : q.y);
+  const double qk = r == 0 ? q.w : (r == 1 ? q.y : q.z);
+  const double ci = 1.0 - 2.0 * (qj * qj + qk * qk), cj = 2.0 * (qi * qj + w * qk), ck = 2.0 * (qi * qk - w * qj);
+  // rows of R_O's column r in canonical order (row 0, 1, 2)
+  const double o0 = r == 0 ? ci : (r == 1 ? ck : cj);
+  const double o1 = r == 0 ? cj : (r == 1 ? ci : ck);
+  const double o2 = r == 0 ? ck : (r == 1 ? cj : ci);
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const double m = fma(o0, RL[c], fma(o1, RL[3 + c], o2 * RL[6 + c]));
+    F.M[r * 3 + c] = m;
+    F.Mf[r * 3 + c] = (float)m;
+  }
+  const double cr = fma(o0, d.x, fma(o1, d.y, o2 * d.z));
+  F.c[r] = cr;
+  F.cf[r] = (float)cr;
+}
+
+__device__ __forceinline__ void build_frame_vec(const TsStepParams& p, int e, int link, int k, int sub, FrameS& F) {
   const size_t ek = (size_t)e * p.K + k;
-  if (part == 3) {
+  if (sub == 3) {
     F.type = (link >= 0) ? __ldg(p.g_type + ek) : TS_GEOM_NONE;
     const float4 prm = __ldg(p.g_params + ek);
     F.prm[0] = prm.x; F.prm[1] = prm.y; F.prm[2] = prm.z; F.prm[3] = prm.w;
@@ -117,39 +148,14 @@ __device__ void build_frame_part(const TsStepParams& p, int e, int link, int k, 
   const size_t el = (size_t)e * p.L + link;
   double RL[9];
   quat_Rd(p.link_quat + el * 4, RL);
-  const D3 d = ld3d(p.link_pos + el * 3) - ld3d(p.obj_pos + ek * 3);
-  if (part < 3) {
-    const int r = part;
-    // column r of R_O, with (i, j, k) = (r, r+1, r+2) mod 3: R[i][i] = 1 - 2(q_j^2 + q_k^2),
-    // R[j][i] = 2(q_i q_j + w q_k), R[k][i] = 2(q_i q_k - w q_j)
-    const float4 q = __ldg(reinterpret_cast<const float4*>(p.obj_quat + ek * 4));
-    const double w = q.x;
-    const double qi = r == 0 ? q.y : (r == 1 ? q.z : q.w);
-    const double qj = r == 0 ? q.z : (r == 1 ? q.w : q.y);
-    const double qk = r == 0 ? q.w : (r == 1 ? q.y : q.z);
-    const double ci = 1.0 - 2.0 * (qj * qj + qk * qk), cj = 2.0 * (qi * qj + w * qk), ck = 2.0 * (qi * qk - w * qj);
-    // rows of R_O's column r in canonical order (row 0, 1, 2)
-    const double o0 = r == 0 ? ci : (r == 1 ? ck : cj);
-    const double o1 = r == 0 ? cj : (r == 1 ? ci : ck);
-    const double o2 = r == 0 ? ck : (r == 1 ? cj : ci);
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-      const double m = fma(o0, RL[c], fma(o1, RL[3 + c], o2 * RL[6 + c]));
-      F.M[r * 3 + c] = m;
-      F.Mf[r * 3 + c] = (float)m;
-    }
-    const double cr = fma(o0, d.x, fma(o1, d.y, o2 * d.z));
-    F.c[r] = cr;
-    F.cf[r] = (float)cr;
-  } else {
-    const D3 cb = mulRT(RL, d);
-    F.cbar[0] = cb.x; F.cbar[1] = cb.y; F.cbar[2] = cb.z;
-    const D3 wO = mulRT(RL, ld3d(p.obj_angvel + ek * 3)), wL = mulRT(RL, ld3d(p.link_angvel + el * 3));
-    const D3 vb = mulRT(RL, ld3d(p.obj_linvel + ek * 3) - ld3d(p.link_linvel + el * 3));
-    F.wO[0] = wO.x; F.wO[1] = wO.y; F.wO[2] = wO.z;
-    F.wL[0] = wL.x; F.wL[1] = wL.y; F.wL[2] = wL.z;
-    F.vbar[0] = vb.x; F.vbar[1] = vb.y; F.vbar[2] = vb.z;
-  }
+  // sub 0: w_O, 1: w_L, 2: v_O - v_L, 3: p_L - p_O; all rotated into the link frame by R_L^T
+  const float* a = sub == 0 ? p.obj_angvel + ek * 3 : (sub == 1 ? p.link_angvel + el * 3 : (sub == 2 ? p.obj_linvel + ek * 3 : p.link_pos + el * 3));
+  const float* b = sub == 2 ? p.link_linvel + el * 3 : p.obj_pos + ek * 3;
+  D3 v = ld3d(a);
+  if (sub >= 2) v = v - ld3d(b);
+  const D3 o = mulRT(RL, v);
+  double* dst = F.wO + 3 * sub;  // wO, wL, vbar, cbar are consecutive
+  dst[0] = o.x; dst[1] = o.y; dst[2] = o.z;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -622,13 +628,22 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const int gi = blockIdx.y;
   const int4 g0 = __ldg(reinterpret_cast<const int4*>(p.groups + gi));
   const int4 g1 = __ldg(reinterpret_cast<const int4*>(p.groups + gi) + 1);
-  const int gstart = g0.x, gcount = g0.y, patch0 = g0.z, npatch = g0.w, chunk0 = g1.x, nchunk = g1.y, gmcount = g1.w;
+  const int gstart = g0.x, gcount = g0.y, patch0 = g0.z, chunk0 = g1.x, nchunk = g1.y, gmcount = g1.w;
 
   // ---- phase 0: relative poses (double) -> shared memory ---------------------------------
   if (tid < TS_MAX_GROUP_PATCHES) pact[tid] = 0;
-  for (int it = tid; it < 4 * npatch * p.K; it += TS_BLOCK) {
-    const int f = it >> 2, lpf = f / p.K, k = f - lpf * p.K;
-    build_frame_part(p, e, __ldg(&p.patches[patch0 + lpf].link), k, it & 3, frames[f]);
+  // The whole block waits for this, so its load chain is short: link ids come from a per-group table
+  // indexed by blockIdx alone, and unused frame slots carry link -1 (no dependence on the group record).
+  if (tid < TS_BLOCK / 2) {
+    for (int it = tid; it < 3 * nfr; it += TS_BLOCK / 2) {
+      const int f = it / 3, lpf = f / p.K, k = f - lpf * p.K;
+      build_frame_row(p, e, __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), k, it - 3 * f, frames[f]);
+    }
+  } else {
+    for (int it = tid - TS_BLOCK / 2; it < 4 * nfr; it += TS_BLOCK / 2) {
+      const int f = it >> 2, lpf = f / p.K, k = f - lpf * p.K;
+      build_frame_vec(p, e, __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), k, it & 3, frames[f]);
+    }
   }
   const bool valid = tid < gcount;
   const int j = gstart + (valid ? tid : 0);
