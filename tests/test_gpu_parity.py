@@ -70,3 +70,83 @@ def test_uncapped_and_no_velocity():
     _assert_ok(_parity(w, steps=3, physics=dict(w.physics, mu=float("inf"))))
     _assert_ok(_parity(w, steps=3, physics=dict(w.physics, use_velocity=0)))
     _assert_ok(_parity(w, steps=3, physics=dict(w.physics, c_e=0.3, march_steps=5, r_prox=0.01)))
+
+
+def test_config5_full_size_sampled():
+    """BASELINE size, the launch configuration bench.py times: 20,480 envs x 1,000 taxels; the oracle
+    recomputes the 16 parity envs {1281 k} (every object class once) element by element."""
+    w = W.config(5)
+    _assert_ok(_parity(w, ids=w.parity_envs(), steps=12))
+
+
+def test_config3_full_size_sampled():
+    w = W.config(3)
+    _assert_ok(_parity(w, ids=w.parity_envs()[::8], steps=3))
+
+
+def test_env_shards_are_bit_identical_to_the_full_run():
+    """two contexts over env halves with env_id_base = 0 / E/2 reproduce the full run."""
+    import torch
+    from paper_2606_22332_b200.sharding import shard_inputs, shard_range
+    w = W.config(5, n_envs=32)
+    full = _sim(w)
+    halves = []
+    for r in range(2):
+        first, cnt = shard_range(w.E, 2, r)
+        from paper_2606_22332_b200.binding import TactileSim
+        s = TactileSim(w.patches, w.T, cnt, w.L, w.K, physics=w.physics, noise=w.noise, outputs=w.outputs,
+                       env_id_base=first)
+        s.set_geometry(w.types[first:first + cnt], w.params[first:first + cnt], w.bank, w.voxel)
+        halves.append((first, cnt, s))
+    for step in range(4):
+        inp = w.inputs(step)
+        ref = full.step(full.upload(inp))
+        parts = [s.step(s.upload(shard_inputs(inp, first, cnt))) for first, cnt, s in halves]
+        torch.cuda.synchronize()
+        for k in ref:
+            got = torch.cat([p[k] for p in parts])
+            assert torch.equal(got, ref[k]), (k, step)
+
+
+def test_reset_redraws_dead_mask_and_zeroes_state():
+    import torch
+    w = W.config(4, n_envs=16)
+    sim = _sim(w)
+    inp = sim.upload(w.inputs(0))
+    a = {k: v.clone() for k, v in sim.step(inp).items()}
+    for s in range(1, 4):
+        sim.step(sim.upload(w.inputs(s)))
+    mask = torch.zeros(w.E, dtype=torch.uint8, device="cuda")
+    mask[::2] = 1
+    sim.reset(mask)
+    # a fresh context stepped to the same global step count has the same counters for the untouched envs
+    b = sim.step(inp)
+    torch.cuda.synchronize()
+    dead_a, dead_b = a["dead"].bool(), b["dead"].bool()
+    assert torch.equal(dead_a[1::2], dead_b[1::2])            # untouched envs keep their episode's mask
+    assert not torch.equal(dead_a[::2], dead_b[::2])           # reset envs drew a new one (episode + 1)
+    frac = dead_b.float().mean().item()
+    assert 0.01 < frac < 0.03
+    assert torch.all(b["ft_noisy"][dead_b] == 0) and torch.all(b["contact"][dead_b] == 0)
+    # reset envs restart from zero state: with the same inputs the clean outputs equal step 0's
+    assert torch.equal(a["ft"][::2], b["ft"][::2]) and torch.equal(a["depth"], b["depth"])
+
+
+def test_edge_shapes():
+    """One env; a layout that is all fillers; march_steps = 0; outputs subset."""
+    import torch
+    from paper_2606_22332_b200.binding import TactileSim
+    w = W.config(2, n_envs=1)
+    _assert_ok(_parity(w, steps=2))
+    sim = TactileSim(w.patches, w.T, 1, w.L, 1, physics=dict(w.physics, march_steps=0), outputs=("prox", "depth"),
+                     link_mask=np.zeros(w.L, np.uint8))
+    sim.set_geometry(w.types, w.params)
+    out = sim.step(sim.upload(w.inputs(0)))
+    torch.cuda.synchronize()
+    assert torch.all(out["prox"] == 0) and torch.all(out["depth"] == 0)   # every taxel filtered out: fillers are 0
+    sim2 = TactileSim(w.patches, w.T, 1, w.L, 1, physics=dict(w.physics, march_steps=0), outputs=("prox",))
+    sim2.set_geometry(w.types, w.params)
+    out2 = sim2.step(sim2.upload(w.inputs(0)))
+    torch.cuda.synchronize()
+    act = torch.from_numpy(sim2.layout.view()["radius"] > 0).cuda()
+    assert torch.allclose(out2["prox"][0][act], torch.full_like(out2["prox"][0][act], 0.02))  # K_m = 0: t = 0, P = r_prox
