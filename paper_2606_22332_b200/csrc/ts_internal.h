@@ -11,7 +11,9 @@
 #include "../../include/ts.h"
 
 #define TS_MAX_PATCH_TAXELS 64   // taxels (and markers) per patch
+#ifndef TS_BLOCK
 #define TS_BLOCK 256             // threads per block = taxel slots per patch group
+#endif
 #define TS_MAX_GROUP_PATCHES 32  // patches per group
 #define TS_CHUNK (2 * TS_BLOCK)   // marker pass-1 items / markers per chunk
 

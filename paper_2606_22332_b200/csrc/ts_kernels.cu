@@ -378,19 +378,6 @@ __device__ __forceinline__ void box_muller(uint32_t wa, uint32_t wb, float& z0, 
   z1 = r * (sg * sn);
 }
 
-// coalesced copy of n <= 6*TS_BLOCK floats from shared memory to a contiguous global range (streaming stores)
-__device__ __forceinline__ void block_store(float* dst, const float* src, int n, int tid) {
-  if (((reinterpret_cast<uintptr_t>(dst) & 15) | (n & 3)) == 0) {
-    const int n4 = n >> 2;
-    float4* d4 = reinterpret_cast<float4*>(dst);
-    const float4* s4 = reinterpret_cast<const float4*>(src);
-    if (tid < n4) __stcs(d4 + tid, s4[tid]);
-    if (tid + TS_BLOCK < n4) __stcs(d4 + tid + TS_BLOCK, s4[tid + TS_BLOCK]);
-  } else {
-    for (int i = tid; i < n; i += TS_BLOCK) __stcs(dst + i, src[i]);
-  }
-}
-
 // six channels of one taxel ([E,T,6] row, 24 bytes, 8-byte aligned): three streaming 8-byte stores
 __device__ __forceinline__ void store6(float* dst, const float* v) {
   float2* d2 = reinterpret_cast<float2*>(dst);
@@ -616,12 +603,13 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int nfr = p.frames_per_group * p.K;
   FrameS* frames = reinterpret_cast<FrameS*>(smem_raw);
-  float* bufA = reinterpret_cast<float*>(frames + nfr);   // [TS_BLOCK*6] output staging
-  float* bufB = bufA + 6 * TS_BLOCK;                      // [6][TS_BLOCK] crosstalk exchange
-  float* hh = bufB + 6 * TS_BLOCK;                        // [TS_BLOCK] penetration h_i (Eq. 19)
+  // Shared memory is kept small on purpose: it is carved out of the same 256 KB as L1, and the SDF gathers
+  // of the march live on L1 hits.  S (marker phase) aliases bufB (noise phase); a barrier separates them.
+  double* S = reinterpret_cast<double*>(frames + nfr);    // [3][TS_CHUNK] marker pass-1 sums
+  float* bufB = reinterpret_cast<float*>(S);              // [6][TS_BLOCK] crosstalk exchange (first half of S)
+  float* hh = reinterpret_cast<float*>(S + 3 * TS_CHUNK); // [TS_BLOCK] penetration h_i (Eq. 19)
   float* ha = hh + TS_BLOCK;                              // [TS_BLOCK] h_i^alpha_e
-  double* S = reinterpret_cast<double*>(ha + TS_BLOCK);   // [3][TS_CHUNK] marker pass-1 sums
-  int* pact = reinterpret_cast<int*>(S + 3 * TS_CHUNK);   // [TS_MAX_GROUP_PATCHES] patch has penetration
+  int* pact = reinterpret_cast<int*>(ha + TS_BLOCK);      // [TS_MAX_GROUP_PATCHES] patch has penetration
 
   const int tid = threadIdx.x;
   const int e = blockIdx.x;
@@ -745,7 +733,8 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   //   pass 2 over (a,b): Uu = sum_q gv S1, Uv = sum_q dv gv S0, Un = sum_q gv T0.
   // Sources with h_i = 0 contribute exactly 0; patches without penetration are skipped.
   if (p.marker && gmcount > 0) {
-    // hh / ha / pact were completed by the barrier above
+    // hh / ha / pact were completed by the barrier above; this one retires the crosstalk reads of bufB (= S)
+    if (NOISE) __syncthreads();
     for (int ch = 0; ch < nchunk; ++ch) {
       const int4 c0 = __ldg(reinterpret_cast<const int4*>(p.chunks + chunk0 + ch));
       const int4 c1 = __ldg(reinterpret_cast<const int4*>(p.chunks + chunk0 + ch) + 1);
@@ -819,11 +808,10 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
             ox = (float)acc.x; oy = (float)acc.y; oz = (float)acc.z;
           }
         }
-        bufA[im * 3] = ox; bufA[im * 3 + 1] = oy; bufA[im * 3 + 2] = oz;
+        float* o = p.marker + ((size_t)e * p.M + mb + im) * 3;
+        __stcs(o, ox); __stcs(o + 1, oy); __stcs(o + 2, oz);
       }
-      __syncthreads();
-      block_store(p.marker + ((size_t)e * p.M + mb) * 3, bufA, (me - mb) * 3, tid);
-      if (ch + 1 < nchunk) __syncthreads();  // S and bufA are reused by the next chunk
+      if (ch + 1 < nchunk) __syncthreads();  // S is reused by the next chunk
     }
   }
 
@@ -883,7 +871,7 @@ __global__ void ts_reset_state_kernel(const __grid_constant__ TsStepParams p, co
 unsigned long long ts_bank_elems_per_grid(int N) { return (unsigned long long)(N - 1) * (N - 1) * N; }
 
 unsigned long long ts_step_smem_bytes(const TsStepParams& p) {
-  return (unsigned long long)p.frames_per_group * p.K * sizeof(FrameS) + sizeof(float) * (12 + 2) * TS_BLOCK +
+  return (unsigned long long)p.frames_per_group * p.K * sizeof(FrameS) + sizeof(float) * 2 * TS_BLOCK +
          sizeof(double) * 3 * TS_CHUNK + sizeof(int) * TS_MAX_GROUP_PATCHES;
 }
 
