@@ -15,7 +15,9 @@
 #define TS_BLOCK 256             // threads per block = taxel slots per patch group
 #endif
 #define TS_MAX_GROUP_PATCHES 32  // patches per group
-#define TS_CHUNK (2 * TS_BLOCK)   // marker pass-1 items / markers per chunk
+#ifndef TS_CHUNK
+#define TS_CHUNK (3 * TS_BLOCK / 2)  // marker pass-1 items / markers per chunk
+#endif
 
 struct ts_layout {
   bool finalized = false;
