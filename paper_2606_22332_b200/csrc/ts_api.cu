@@ -382,6 +382,8 @@ ts_status ts_set_geometry(ts_ctx* c, const ts_geometry* geo, void* stream) {
   TS_CUDA(c, cudaMemcpyAsync(c->g_params, geo->params, sizeof(float4) * EK, cudaMemcpyHostToDevice, st));
   if (geo->n_grids > 0) {
     const int N = geo->grid_n;
+    if (ts_bank_elems_per_grid(N) * (unsigned long long)geo->n_grids >= (1ULL << 31))
+      return fail(c, TS_ERR_UNSUPPORTED, "ts_set_geometry: bank larger than 2^31 cells (32-bit cell indices)");
     const size_t need = sizeof(float4) * ts_bank_elems_per_grid(N) * geo->n_grids;
     if (need > c->bank_bytes) {
       TS_CUDA(c, cudaStreamSynchronize(st));
