@@ -156,7 +156,8 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   }
   for (size_t t = 0; t < lay->link.size(); ++t)
     if (lay->link[t] >= cfg->n_links) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: layout link index >= n_links");
-  if ((long long)cfg->n_envs * lay->n_taxels > (1LL << 40)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: too large");
+  if ((long long)cfg->n_envs * 12LL * ((lay->n_taxels + 31) / 32 * 32) >= (1LL << 32))
+    return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: n_envs * n_taxels too large (state uses 32-bit element indices)");
 
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev)

@@ -416,31 +416,37 @@ struct NoiseState {
 };
 
 __device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, bool valid, NoiseState& ns) {
-  const size_t Tp = (size_t)p.Tp;
-  const float* st_h = p.st_hyst + (size_t)e * (p.hyst_mode == TS_HYST_MAXWELL ? 12 : 6) * Tp + j;
-  const float* st_d = p.st_drift + (size_t)e * 6 * Tp + j;
+  // 32-bit element indices (ts_create guarantees E * 12 * Tp < 2^32): one IMAD + LEA pair per access
+  // instead of 64-bit address arithmetic that the register allocator keeps rematerialising.
+  const unsigned Tp = (unsigned)p.Tp;
+  const unsigned ih = (unsigned)e * (p.hyst_mode == TS_HYST_MAXWELL ? 12u : 6u) * Tp + (unsigned)j;
+  const unsigned id = (unsigned)e * 6u * Tp + (unsigned)j;
+  const float* st_h = p.st_hyst;
+  const float* st_d = p.st_drift;
 #pragma unroll
   for (int c = 0; c < 6; ++c) { ns.sY[c] = 0.f; ns.sX[c] = 0.f; ns.sD[c] = 0.f; }
   if (valid) {
     if (p.hyst_mode != TS_HYST_OFF) {
 #pragma unroll
-      for (int c = 0; c < 6; ++c) ns.sY[c] = __ldcs(st_h + c * Tp);
+      for (int c = 0; c < 6; ++c) ns.sY[c] = __ldcs(st_h + (ih + c * Tp));
     }
     if (p.hyst_mode == TS_HYST_MAXWELL) {
 #pragma unroll
-      for (int c = 0; c < 6; ++c) ns.sX[c] = __ldcs(st_h + (6 + c) * Tp);
+      for (int c = 0; c < 6; ++c) ns.sX[c] = __ldcs(st_h + (ih + (6 + c) * Tp));
     }
 #pragma unroll
-    for (int c = 0; c < 6; ++c) ns.sD[c] = __ldcs(st_d + c * Tp);
+    for (int c = 0; c < 6; ++c) ns.sD[c] = __ldcs(st_d + (id + c * Tp));
   }
 }
 
 // Every thread of the block must call this (it contains one __syncthreads).
 __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, size_t ej, int tid, int gstart, bool valid,
                                             bool act, bool deadb, const float* ft, const NoiseState& ns, float* bufB) {
-  const size_t Tp = (size_t)p.Tp;
-  float* const st_h = p.st_hyst + (size_t)e * (p.hyst_mode == TS_HYST_MAXWELL ? 12 : 6) * Tp + j;
-  float* const st_d = p.st_drift + (size_t)e * 6 * Tp + j;
+  const unsigned Tp = (unsigned)p.Tp;
+  const unsigned ih = (unsigned)e * (p.hyst_mode == TS_HYST_MAXWELL ? 12u : 6u) * Tp + (unsigned)j;
+  const unsigned id = (unsigned)e * 6u * Tp + (unsigned)j;
+  float* const st_h = p.st_hyst;
+  float* const st_d = p.st_drift;
   float h[6];
   if (p.hyst_mode == TS_HYST_ASYM) {  // D3, Q14
 #pragma unroll
@@ -448,7 +454,7 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
       const float yp = ns.sY[c];
       const float al = (fabsf(ft[c]) > fabsf(yp)) ? p.alpha_load : p.alpha_unload;
       h[c] = act ? fmaf(al, ft[c] - yp, yp) : 0.f;
-      if (valid) __stcs(st_h + c * Tp, h[c]);
+      if (valid) __stcs(st_h + (ih + c * Tp), h[c]);
     }
   } else if (p.hyst_mode == TS_HYST_MAXWELL) {  // Eq. 29-30
 #pragma unroll
@@ -456,8 +462,8 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
       const float z = act ? fmaf(p.decay, ns.sY[c], ft[c] - ns.sX[c]) : 0.f;
       h[c] = fmaf(p.beta, z, ft[c]);
       if (valid) {
-        __stcs(st_h + c * Tp, z);
-        __stcs(st_h + (6 + c) * Tp, act ? ft[c] : 0.f);
+        __stcs(st_h + (ih + c * Tp), z);
+        __stcs(st_h + (ih + (6 + c) * Tp), act ? ft[c] : 0.f);
       }
     }
   } else {
@@ -493,7 +499,7 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
     const float acc = ((hb[n0] - hc) + (hb[n1] - hc)) + ((hb[n2] - hc) + (hb[n3] - hc));
     const float cx = fmaf(q4, acc, hc);
     const float Dn = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], ns.sD[c]) : 0.f;
-    if (valid) __stcs(st_d + c * Tp, Dn);
+    if (valid) __stcs(st_d + (id + c * Tp), Dn);
     outv[c] = (act && !deadb) ? cx + Dn : 0.f;  // S8a dead (Eq. 28) last
   }
   if (p.ft_noisy && valid) store6(p.ft_noisy + ej * 6, outv);
@@ -620,7 +626,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   float* bufB = reinterpret_cast<float*>(S);              // [6][TS_BLOCK] crosstalk exchange (first half of S)
   float* hh = reinterpret_cast<float*>(S + 3 * TS_CHUNK); // [TS_BLOCK] penetration h_i (Eq. 19)
   float* ha = hh + TS_BLOCK;                              // [TS_BLOCK] h_i^alpha_e
-  int* pact = reinterpret_cast<int*>(ha + TS_BLOCK);      // [TS_MAX_GROUP_PATCHES] patch has penetration
+  unsigned* pmask = reinterpret_cast<unsigned*>(ha + TS_BLOCK);  // bit l: group-local patch l has penetration
 
   const int tid = threadIdx.x;
   const int e = blockIdx.x;
@@ -630,7 +636,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const int gstart = g0.x, gcount = g0.y, patch0 = g0.z, chunk0 = g1.x, nchunk = g1.y, gmcount = g1.w;
 
   // ---- phase 0: relative poses (double) -> shared memory ---------------------------------
-  if (tid < TS_MAX_GROUP_PATCHES) pact[tid] = 0;
+  if (tid == 0) *pmask = 0u;
   // The whole block waits for this, so its load chain is short: link ids come from a per-group table
   // indexed by blockIdx alone, and unused frame slots carry link -1 (no dependence on the group record).
   if (tid < TS_BLOCK / 2) {
@@ -687,7 +693,8 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     const float h = (act && phid < 0.0) ? (float)(-phid) : 0.f;
     hh[tid] = h;
     ha[tid] = h > 0.f ? __powf(h, p.alpha_e) : 0.f;
-    if (h > 0.f) pact[lp] = 1;
+    const unsigned wb = __reduce_or_sync(TS_FULL, h > 0.f ? (1u << lp) : 0u);  // one shared atomic per warp
+    if ((tid & 31) == 0 && wb) atomicOr(pmask, wb);
   }
   const F3 xo = mk3((float)xd.x, (float)xd.y, (float)xd.z);  // kept for the march (last phase)
 
@@ -750,8 +757,8 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
       const int4 c0 = __ldg(reinterpret_cast<const int4*>(p.chunks + chunk0 + ch));
       const int4 c1 = __ldg(reinterpret_cast<const int4*>(p.chunks + chunk0 + ch) + 1);
       const int i1b = c0.x, i1e = c0.y, mb = c0.z, me = c0.w, lpb = c1.x, lpe = c1.y;
-      bool any = false;
-      for (int l = lpb; l < lpe; ++l) any = any || (pact[l] != 0);
+      const unsigned pm = *pmask;
+      const bool any = (pm & ((lpe >= 32 ? 0u : (1u << lpe)) - (1u << lpb))) != 0u;  // bits lpb .. lpe-1
       if (!any) {  // no penetration anywhere in the chunk: the markers are exactly 0
         float* o = p.marker + ((size_t)e * p.M + mb) * 3;
         for (int i = tid; i < (me - mb) * 3; i += TS_BLOCK) __stcs(o + i, 0.f);
@@ -762,7 +769,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
         const int l = pk & 255, a = (pk >> 8) & 255, q = pk >> 16;
         const TsPatch& pt = p.patches[patch0 + l];
         double s0 = 0.0, s1 = 0.0, t0 = 0.0;
-        if (pact[l]) {
+        if ((pm >> l) & 1u) {
           const int nu = __ldg(&pt.nu);
           const double* GU = p.mk_tab + __ldg(&pt.tab) + a * nu;
           const double* DU = GU + __ldg(&pt.mnu) * nu;
@@ -782,7 +789,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
         const int pk = __ldg(p.mk_item2 + mb + im);
         const int l = pk & 255, a = (pk >> 8) & 255, b = pk >> 16;
         const TsPatch& pt = p.patches[patch0 + l];
-        if (pact[l]) {
+        if ((pm >> l) & 1u) {
           if (!__ldg(&pt.direct)) {
             const int nv = __ldg(&pt.nv), mnu = __ldg(&pt.mnu);
             const double* GV = p.mk_tab + __ldg(&pt.tab) + 2 * mnu * __ldg(&pt.nu) + b * nv;
