@@ -415,22 +415,23 @@ struct NoiseState {
   float sY[6], sX[6], sD[6];  // hysteresis y (asym) or xi (maxwell), maxwell x_prev, drift D
 };
 
+template <int HM>  // hysteresis mode (TS_HYST_*), a compile-time constant so the unused state rows cost nothing
 __device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, bool valid, NoiseState& ns) {
   // 32-bit element indices (ts_create guarantees E * 12 * Tp < 2^32): one IMAD + LEA pair per access
   // instead of 64-bit address arithmetic that the register allocator keeps rematerialising.
   const unsigned Tp = (unsigned)p.Tp;
-  const unsigned ih = (unsigned)e * (p.hyst_mode == TS_HYST_MAXWELL ? 12u : 6u) * Tp + (unsigned)j;
+  const unsigned ih = (unsigned)e * (HM == TS_HYST_MAXWELL ? 12u : 6u) * Tp + (unsigned)j;
   const unsigned id = (unsigned)e * 6u * Tp + (unsigned)j;
   const float* st_h = p.st_hyst;
   const float* st_d = p.st_drift;
 #pragma unroll
   for (int c = 0; c < 6; ++c) { ns.sY[c] = 0.f; ns.sX[c] = 0.f; ns.sD[c] = 0.f; }
   if (valid) {
-    if (p.hyst_mode != TS_HYST_OFF) {
+    if (HM != TS_HYST_OFF) {
 #pragma unroll
       for (int c = 0; c < 6; ++c) ns.sY[c] = __ldcs(st_h + (ih + c * Tp));
     }
-    if (p.hyst_mode == TS_HYST_MAXWELL) {
+    if (HM == TS_HYST_MAXWELL) {
 #pragma unroll
       for (int c = 0; c < 6; ++c) ns.sX[c] = __ldcs(st_h + (ih + (6 + c) * Tp));
     }
@@ -440,15 +441,16 @@ __device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, 
 }
 
 // Every thread of the block must call this (it contains one __syncthreads).
+template <int HM>
 __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, size_t ej, int tid, int gstart, bool valid,
                                             bool act, bool deadb, const float* ft, const NoiseState& ns, float* bufB) {
   const unsigned Tp = (unsigned)p.Tp;
-  const unsigned ih = (unsigned)e * (p.hyst_mode == TS_HYST_MAXWELL ? 12u : 6u) * Tp + (unsigned)j;
+  const unsigned ih = (unsigned)e * (HM == TS_HYST_MAXWELL ? 12u : 6u) * Tp + (unsigned)j;
   const unsigned id = (unsigned)e * 6u * Tp + (unsigned)j;
   float* const st_h = p.st_hyst;
   float* const st_d = p.st_drift;
   float h[6];
-  if (p.hyst_mode == TS_HYST_ASYM) {  // D3, Q14
+  if (HM == TS_HYST_ASYM) {  // D3, Q14
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
       const float yp = ns.sY[c];
@@ -456,7 +458,7 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
       h[c] = act ? fmaf(al, ft[c] - yp, yp) : 0.f;
       if (valid) __stcs(st_h + (ih + c * Tp), h[c]);
     }
-  } else if (p.hyst_mode == TS_HYST_MAXWELL) {  // Eq. 29-30
+  } else if (HM == TS_HYST_MAXWELL) {  // Eq. 29-30
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
       const float z = act ? fmaf(p.decay, ns.sY[c], ft[c] - ns.sX[c]) : 0.f;
@@ -496,7 +498,7 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
   for (int c = 0; c < 6; ++c) {
     const float* hb = bufB + c * TS_BLOCK;
     const float hc = h[c];
-    const float acc = ((hb[n0] - hc) + (hb[n1] - hc)) + ((hb[n2] - hc) + (hb[n3] - hc));
+    const float acc = fmaf(-4.f, hc, (hb[n0] + hb[n1]) + (hb[n2] + hb[n3]));  // sum_k (h_k - h_j)
     const float cx = fmaf(q4, acc, hc);
     const float Dn = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], ns.sD[c]) : 0.f;
     if (valid) __stcs(st_d + (id + c * Tp), Dn);
@@ -506,6 +508,7 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
 }
 
 // Stand-alone noise kernel (split variant): reads the clean ft the geometry kernel wrote.
+template <int HM>
 __global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_constant__ TsStepParams p) {
   __shared__ float bufB[6 * TS_BLOCK];
   const int tid = threadIdx.x;
@@ -516,7 +519,7 @@ __global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_cons
   const int j = gstart + (valid ? tid : 0);
   const size_t ej = (size_t)e * p.T + j;
   NoiseState ns;
-  noise_load(p, e, j, valid, ns);
+  noise_load<HM>(p, e, j, valid, ns);
   float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   bool act = false, deadb = false;
   if (valid) {
@@ -526,7 +529,7 @@ __global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_cons
     act = __ldg(&p.tx_pos[j].w) > 0.f;
     deadb = act && ((p.st_flags[ej] >> 1) & 1);
   }
-  noise_chain(p, e, j, ej, tid, gstart, valid, act, deadb, ft, ns, bufB);
+  noise_chain<HM>(p, e, j, ej, tid, gstart, valid, act, deadb, ft, ns, bufB);
 }
 
 template <bool SINGLE>
@@ -615,8 +618,9 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
   }
 }
 
-template <bool SINGLE, bool NOISE>
+template <bool SINGLE, int HM>  // HM = TS_HYST_* of the fused noise chain, -1 = no noise chain in this kernel
 __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const __grid_constant__ TsStepParams p) {
+  constexpr bool NOISE = HM >= 0;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int nfr = p.frames_per_group * p.K;
   FrameS* frames = reinterpret_cast<FrameS*>(smem_raw);
@@ -641,12 +645,12 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   // indexed by blockIdx alone, and unused frame slots carry link -1 (no dependence on the group record).
   if (tid < TS_BLOCK / 2) {
     for (int it = tid; it < 3 * nfr; it += TS_BLOCK / 2) {
-      const int f = it / 3, lpf = f / p.K, k = f - lpf * p.K;
+      const int f = it / 3, lpf = SINGLE ? f : f / p.K, k = f - lpf * p.K;
       build_frame_row(p, e, __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), k, it - 3 * f, frames[f]);
     }
   } else {
     for (int it = tid - TS_BLOCK / 2; it < 4 * nfr; it += TS_BLOCK / 2) {
-      const int f = it >> 2, lpf = f / p.K, k = f - lpf * p.K;
+      const int f = it >> 2, lpf = SINGLE ? f : f / p.K, k = f - lpf * p.K;
       build_frame_vec(p, e, __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), k, it & 3, frames[f]);
     }
   }
@@ -701,7 +705,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   // state prefetch: the 12 (18) per-taxel state words of the noise chain are requested now so that their
   // HBM latency is covered by the march and the force/torque phases.
   NoiseState ns;
-  if (NOISE) noise_load(p, e, j, valid, ns);
+  if (NOISE) noise_load<HM>(p, e, j, valid, ns);
 #if !TS_MARCH_LAST
   march_phase<SINGLE>(p, frames, e, lp, valid, act, ej, phif, xo, P4, N4);
 #endif
@@ -741,7 +745,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   if (p.ft && valid) store6(p.ft + ej * 6, ft);
 
   // ---- phase 4 (S8): noise chain (fused variant); contains the barrier that also publishes hh / ha / pact
-  if (NOISE) noise_chain(p, e, j, ej, tid, gstart, valid, act, deadb, ft, ns, bufB);
+  if (NOISE) noise_chain<HM>(p, e, j, ej, tid, gstart, valid, act, deadb, ft, ns, bufB);
   else __syncthreads();
 
   // ---- phase 5 (S6): elastomer marker dilation (Eq. 18-21, 23 first sum) ----------------------
@@ -893,11 +897,31 @@ unsigned long long ts_step_smem_bytes(const TsStepParams& p) {
          sizeof(double) * 3 * TS_CHUNK + sizeof(int) * TS_MAX_GROUP_PATCHES;
 }
 
+namespace {
+template <bool SINGLE, int HM>
+cudaError_t prep_one(int smem) {
+  return cudaFuncSetAttribute(ts_step_kernel<SINGLE, HM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+}
+template <bool SINGLE>
+void launch_one(const TsStepParams& p, int hm, dim3 grid, size_t smem, cudaStream_t st) {
+  switch (hm) {
+    case TS_HYST_OFF: ts_step_kernel<SINGLE, TS_HYST_OFF><<<grid, TS_BLOCK, smem, st>>>(p); break;
+    case TS_HYST_MAXWELL: ts_step_kernel<SINGLE, TS_HYST_MAXWELL><<<grid, TS_BLOCK, smem, st>>>(p); break;
+    case TS_HYST_ASYM: ts_step_kernel<SINGLE, TS_HYST_ASYM><<<grid, TS_BLOCK, smem, st>>>(p); break;
+    default: ts_step_kernel<SINGLE, -1><<<grid, TS_BLOCK, smem, st>>>(p); break;
+  }
+}
+}  // namespace
+
 int ts_prepare_kernels(int max_smem_bytes) {
-  cudaError_t e = cudaFuncSetAttribute(ts_step_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(ts_step_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(ts_step_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(ts_step_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_bytes);
+  cudaError_t e = prep_one<true, -1>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, TS_HYST_OFF>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, TS_HYST_MAXWELL>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, TS_HYST_ASYM>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<false, -1>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<false, TS_HYST_OFF>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<false, TS_HYST_MAXWELL>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<false, TS_HYST_ASYM>(max_smem_bytes);
   return (int)e;
 }
 
@@ -906,21 +930,18 @@ int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
   if (p.E <= 0 || p.G <= 0 || p.G > 65535) return (int)cudaErrorInvalidConfiguration;
   const size_t smem = (size_t)ts_step_smem_bytes(p);
   const dim3 grid((unsigned)p.E, (unsigned)p.G);
-  cudaStream_t st = (cudaStream_t)stream;
-  const bool nz = p.noise_enable && fused_noise;
-  if (p.K == 1) {
-    if (nz) ts_step_kernel<true, true><<<grid, TS_BLOCK, smem, st>>>(p);
-    else ts_step_kernel<true, false><<<grid, TS_BLOCK, smem, st>>>(p);
-  } else {
-    if (nz) ts_step_kernel<false, true><<<grid, TS_BLOCK, smem, st>>>(p);
-    else ts_step_kernel<false, false><<<grid, TS_BLOCK, smem, st>>>(p);
-  }
+  const int hm = (p.noise_enable && fused_noise) ? p.hyst_mode : -1;
+  if (p.K == 1) launch_one<true>(p, hm, grid, smem, (cudaStream_t)stream);
+  else launch_one<false>(p, hm, grid, smem, (cudaStream_t)stream);
   return (int)cudaGetLastError();
 }
 
 int ts_launch_noise(const TsStepParams& p, void* stream) {
   const dim3 grid((unsigned)p.E, (unsigned)p.G);
-  ts_noise_kernel<<<grid, TS_BLOCK, 0, (cudaStream_t)stream>>>(p);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (p.hyst_mode == TS_HYST_MAXWELL) ts_noise_kernel<TS_HYST_MAXWELL><<<grid, TS_BLOCK, 0, st>>>(p);
+  else if (p.hyst_mode == TS_HYST_ASYM) ts_noise_kernel<TS_HYST_ASYM><<<grid, TS_BLOCK, 0, st>>>(p);
+  else ts_noise_kernel<TS_HYST_OFF><<<grid, TS_BLOCK, 0, st>>>(p);
   return (int)cudaGetLastError();
 }
 
