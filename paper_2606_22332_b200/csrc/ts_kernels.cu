@@ -442,7 +442,7 @@ __device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, 
 
 // Every thread of the block must call this (it contains one __syncthreads).
 template <int HM>
-__device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, size_t ej, int tid, int gstart, bool valid,
+__device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, unsigned ej, int tid, int gstart, bool valid,
                                             bool act, bool deadb, const float* ft, const NoiseState& ns, float* bufB) {
   const unsigned Tp = (unsigned)p.Tp;
   const unsigned ih = (unsigned)e * (HM == TS_HYST_MAXWELL ? 12u : 6u) * Tp + (unsigned)j;
@@ -504,7 +504,7 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
     if (valid) __stcs(st_d + (id + c * Tp), Dn);
     outv[c] = (act && !deadb) ? cx + Dn : 0.f;  // S8a dead (Eq. 28) last
   }
-  if (p.ft_noisy && valid) store6(p.ft_noisy + ej * 6, outv);
+  if (p.ft_noisy && valid) store6(p.ft_noisy + ej * 6u, outv);
 }
 
 // Stand-alone noise kernel (split variant): reads the clean ft the geometry kernel wrote.
@@ -517,13 +517,13 @@ __global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_cons
   const int gstart = g0.x, gcount = g0.y;
   const bool valid = tid < gcount;
   const int j = gstart + (valid ? tid : 0);
-  const size_t ej = (size_t)e * p.T + j;
+  const unsigned ej = (unsigned)e * (unsigned)p.T + (unsigned)j;  // < 2^32 / 12 (checked by ts_create)
   NoiseState ns;
   noise_load<HM>(p, e, j, valid, ns);
   float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   bool act = false, deadb = false;
   if (valid) {
-    const float2* f2 = reinterpret_cast<const float2*>(p.ft + ej * 6);
+    const float2* f2 = reinterpret_cast<const float2*>(p.ft + ej * 6u);
     const float2 a = __ldcs(f2), b = __ldcs(f2 + 1), c = __ldcs(f2 + 2);
     ft[0] = a.x; ft[1] = a.y; ft[2] = b.x; ft[3] = b.y; ft[4] = c.x; ft[5] = c.y;
     act = __ldg(&p.tx_pos[j].w) > 0.f;
@@ -534,7 +534,7 @@ __global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_cons
 
 template <bool SINGLE>
 __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS* frames, int e, int lp, bool valid, bool act,
-                                            size_t ej, float phif, F3 xo, float4 P4, float4 N4) {
+                                            unsigned ej, float phif, F3 xo, float4 P4, float4 N4) {
 // ---- phase 2 (S7): proximity march, t <- min(t + max(phi(q + t a), 0), r_prox), K_m evaluations.
   // Exact shortcuts (O7): evaluation 0 is the query above; t = r_prox is absorbing; an evaluation
   // that leaves t unchanged repeats forever.
@@ -585,15 +585,20 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
           }
         }
       } else {
-        for (int it = 1; it < p.march_steps; ++it) {
-          if (!__any_sync(TS_FULL, go)) break;
-          if (go) {
-            const float sv = prim_value_f(gtype, F.prm, xo + t * dr);
-            const float tn = fminf(t + fmaxf(sv, 0.f), p.r_prox);
-            go = (tn != t) && (tn < p.r_prox);
-            t = tn;
-          }
-        }
+#define TS_PRIM_LOOP(TYPE)                                                         \
+  for (int it = 1; it < p.march_steps; ++it) {                                     \
+    if (!__any_sync(TS_FULL, go)) break;                                           \
+    if (go) {                                                                      \
+      const float sv = prim_value_f(TYPE, F.prm, xo + t * dr);                     \
+      const float tn = fminf(t + fmaxf(sv, 0.f), p.r_prox);                        \
+      go = (tn != t) && (tn < p.r_prox);                                           \
+      t = tn;                                                                      \
+    }                                                                              \
+  }
+        if (gtype == TS_GEOM_SPHERE) { TS_PRIM_LOOP(TS_GEOM_SPHERE) }
+        else if (gtype == TS_GEOM_BOX) { TS_PRIM_LOOP(TS_GEOM_BOX) }
+        else if (gtype == TS_GEOM_CAPSULE) { TS_PRIM_LOOP(TS_GEOM_CAPSULE) }
+#undef TS_PRIM_LOOP
       }
     } else {
       const F3 xj = mk3(P4.x, P4.y, P4.z);
@@ -656,7 +661,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   }
   const bool valid = tid < gcount;
   const int j = gstart + (valid ? tid : 0);
-  const size_t ej = (size_t)e * p.T + j;
+  const unsigned ej = (unsigned)e * (unsigned)p.T + (unsigned)j;  // < 2^32 / 12 (checked by ts_create)
   const float4 P4 = __ldg(p.tx_pos + j), N4 = __ldg(p.tx_nrm + j);
   const int lp = __float_as_int(N4.w);
   const float Rj = valid ? P4.w : 0.f;  // R_j = 0: inactive slot
@@ -742,7 +747,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
       ft[3] = (float)tau.x; ft[4] = (float)tau.y; ft[5] = (float)tau.z;
     }
   }
-  if (p.ft && valid) store6(p.ft + ej * 6, ft);
+  if (p.ft && valid) store6(p.ft + ej * 6u, ft);
 
   // ---- phase 4 (S8): noise chain (fused variant); contains the barrier that also publishes hh / ha / pact
   if (NOISE) noise_chain<HM>(p, e, j, ej, tid, gstart, valid, act, deadb, ft, ns, bufB);
