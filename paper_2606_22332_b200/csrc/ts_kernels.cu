@@ -367,8 +367,8 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1
 // z0 = sqrt(-2 ln u_a) cos(2 pi u_b), z1 = ... sin(...).
 //  * -2 ln u_a: MUFU.LG2 has an ABSOLUTE error of ~2^-22 near u = 1, so for 1 - u < 1/64 the
 //    series of -ln(1 - v) (v = 1 - u is exact) is used instead; relative error of L <= ~1e-5.
-//  * the angle is reduced EXACTLY in integers to [-pi/4, pi/4] (k_b is a 24-bit integer), then
-//    MUFU.SIN/COS (abs error ~4e-7) and a quadrant swap.
+//  * the angle is reduced EXACTLY in integers to [-pi, pi) (k_b is a 24-bit integer), then MUFU.SIN/COS
+//    (abs error ~4e-7 there).
 // Error of z <= ~1e-5 |z| + 4e-7 r, i.e. < 1e-8 N per step at sigma = 1e-3 N (tolerance 1e-6).
 __device__ __forceinline__ void box_muller(uint32_t wa, uint32_t wb, float& z0, float& z1) {
   const float ua = (float)(2u * (wa >> 9) + 1u) * 5.9604644775390625e-8f;
@@ -377,15 +377,12 @@ __device__ __forceinline__ void box_muller(uint32_t wa, uint32_t wb, float& z0, 
   const float Ll = -1.3862943611198906f * __log2f(ua);                                  // -2 ln 2 * log2 u
   const float L = (v < 0.015625f) ? Ls : Ll;
   const float r = L * rsqrtf(L);
-  const uint32_t kb = 2u * (wb >> 9) + 1u;             // angle = 2 pi kb / 2^24
-  const uint32_t q = (kb + 0x200000u) >> 22;           // nearest quadrant
-  const int rem = (int)kb - (int)(q << 22);            // in [-2^21, 2^21)
-  const float th = (float)rem * 3.7450703e-7f;         // 2 pi / 2^24
-  const float s = __sinf(th), c = __cosf(th);
-  const float cs = (q & 1u) ? -s : c, sn = (q & 1u) ? c : s;
-  const float sg = (q & 2u) ? -1.f : 1.f;
-  z0 = r * (sg * cs);
-  z1 = r * (sg * sn);
+  // angle 2 pi k_b / 2^24 mapped to [-pi, pi) by sign-extending the 24-bit integer (same sin / cos);
+  // MUFU.SIN / MUFU.COS have an absolute error of ~4e-7 on that range
+  const int kb = ((int)((2u * (wb >> 9) + 1u) << 8)) >> 8;
+  const float th = (float)kb * 3.7450703e-7f;  // 2 pi / 2^24
+  z0 = r * __cosf(th);
+  z1 = r * __sinf(th);
 }
 
 // six channels of one taxel ([E,T,6] row, 24 bytes, 8-byte aligned): three streaming 8-byte stores
