@@ -561,10 +561,23 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
         if (__all_sync(TS_FULL, inside || !go)) {  // whole segment inside the grid for every marching lane
           const unsigned cbase = (unsigned)(int)F.prm[0] * (unsigned)p.grid_stride -
                                  0x4B400000u * (unsigned)((N - 1) * N + N + 1);
+          // A converging ray takes sub-voxel steps, so consecutive evaluations mostly fall into the same cell:
+          // its 8 corners stay in registers and are reloaded only when the cell index changes.
+          unsigned pidx = 0xffffffffu;
+          float4 A = make_float4(0.f, 0.f, 0.f, 0.f), B = A;
           for (int it = 1; it < p.march_steps; ++it) {
             if (!__any_sync(TS_FULL, go)) break;
             if (go) {
-              const float sv = grid_value_fast(p.bank, cbase, (unsigned)N, u0 + t * du);
+              const F3 u = u0 + t * du;
+              const float MAGIC = 12582912.f;  // 1.5 * 2^23, see grid_value_fast
+              const float tx = __fadd_rd(u.x, MAGIC), ty = __fadd_rd(u.y, MAGIC), tz = __fadd_rd(u.z, MAGIC);
+              const unsigned idx = ((__float_as_uint(ty) * (unsigned)(N - 1) + __float_as_uint(tx)) * (unsigned)N + __float_as_uint(tz)) + cbase;
+              if (idx != pidx) {
+                A = __ldg(p.bank + idx);
+                B = __ldg(p.bank + idx + 1);
+                pidx = idx;
+              }
+              const float sv = trilerp(A, B, u.x - (tx - MAGIC), u.y - (ty - MAGIC), u.z - (tz - MAGIC));
               const float tn = fminf(t + fmaxf(sv, 0.f), p.r_prox);
               go = (tn != t) && (tn < p.r_prox);
               t = tn;
