@@ -29,6 +29,8 @@ struct ts_ctx {
   TsGroup* groups = nullptr;
   TsChunk* chunks = nullptr;
   int32_t *mk_item1 = nullptr, *mk_item2 = nullptr, *grp_link = nullptr;
+  std::vector<TsGroup> h_groups;   // host copies for the inline parameter tables
+  std::vector<int32_t> h_glink;
   double* mk_tab = nullptr;
   int32_t* g_type = nullptr;
   float4* g_params = nullptr;
@@ -91,6 +93,14 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.G = c->G; p.Tp = c->Tp; p.frames_per_group = c->frames_per_group;
   p.tx_nbr = c->tx_nbr; p.groups = c->groups; p.chunks = c->chunks; p.mk_item1 = c->mk_item1; p.mk_item2 = c->mk_item2;
   p.mk_tab = c->mk_tab; p.grp_link = c->grp_link;
+  p.inl = 0; p.inl_stride = c->frames_per_group;
+  if (c->G <= TS_INL_GROUPS && c->G * c->frames_per_group <= TS_INL_LINKS && (int)c->h_groups.size() == c->G) {
+    p.inl = 1;
+    for (int g = 0; g < c->G; ++g) {
+      p.inl_grp[g] = c->h_groups[g];
+      for (int l = 0; l < c->frames_per_group; ++l) p.inl_link[g * c->frames_per_group + l] = c->h_glink[(size_t)g * TS_MAX_GROUP_PATCHES + l];
+    }
+  }
   p.env_id_base = (uint32_t)g.env_id_base;
   p.tx_pos = c->tx_pos; p.tx_nrm = c->tx_nrm; p.patches = c->patches; p.mk_pos = c->mk_pos; p.mk_nrm = c->mk_nrm;
   p.g_type = c->g_type; p.g_params = c->g_params; p.bank = c->bank;
@@ -280,6 +290,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   std::vector<int32_t> glink(groups.size() * TS_MAX_GROUP_PATCHES, -1);
   for (size_t gi = 0; gi < groups.size(); ++gi)
     for (int l = 0; l < groups[gi].npatch; ++l) glink[gi * TS_MAX_GROUP_PATCHES + l] = pts[groups[gi].patch0 + l].link;
+  c->h_groups = groups; c->h_glink = glink;
   if (item1.empty()) item1.push_back(0);
   if (tab.empty()) tab.push_back(0.0);
   if (chunks.empty()) chunks.push_back(TsChunk{});

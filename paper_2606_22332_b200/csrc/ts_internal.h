@@ -15,6 +15,8 @@
 #define TS_BLOCK 256             // threads per block = taxel slots per patch group
 #endif
 #define TS_MAX_GROUP_PATCHES 32  // patches per group
+#define TS_INL_GROUPS 16         // group records / link ids carried inside the kernel parameters
+#define TS_INL_LINKS 192
 #ifndef TS_CHUNK
 #define TS_CHUNK (3 * TS_BLOCK / 2)  // marker pass-1 items / markers per chunk
 #endif
@@ -117,6 +119,12 @@ struct TsStepParams {
   int32_t noise_enable, hyst_mode;
   uint32_t seed_lo, seed_hi;
   float sigma_f, sigma_t, beta, decay, alpha_load, alpha_unload, chi;
+  // Small layouts carry their group records and per-group link ids in the parameter space itself (constant
+  // bank: a few cycles) so that a block's first dependent global load is already the pose row.
+  int32_t inl;                             // 1 = the two tables below are valid
+  int32_t inl_stride;                      // link ids per group in inl_link (= frames_per_group)
+  TsGroup inl_grp[TS_INL_GROUPS];
+  int32_t inl_link[TS_INL_LINKS];
 };
 
 // launchers (ts_kernels.cu)

@@ -650,9 +650,15 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const int tid = threadIdx.x;
   const int e = blockIdx.x;
   const int gi = blockIdx.y;
-  const int4 g0 = __ldg(reinterpret_cast<const int4*>(p.groups + gi));
-  const int4 g1 = __ldg(reinterpret_cast<const int4*>(p.groups + gi) + 1);
-  const int gstart = g0.x, gcount = g0.y, patch0 = g0.z, chunk0 = g1.x, nchunk = g1.y, gmcount = g1.w;
+  int gstart, gcount, patch0, chunk0, nchunk, gmcount;
+  if (p.inl) {  // group record from the parameter space (constant bank)
+    const TsGroup& g = p.inl_grp[gi];
+    gstart = g.start; gcount = g.count; patch0 = g.patch0; chunk0 = g.chunk0; nchunk = g.nchunk; gmcount = g.mcount;
+  } else {
+    const int4 g0 = __ldg(reinterpret_cast<const int4*>(p.groups + gi));
+    const int4 g1 = __ldg(reinterpret_cast<const int4*>(p.groups + gi) + 1);
+    gstart = g0.x; gcount = g0.y; patch0 = g0.z; chunk0 = g1.x; nchunk = g1.y; gmcount = g1.w;
+  }
 
   // ---- phase 0: relative poses (double) -> shared memory ---------------------------------
   if (tid == 0) *pmask = 0u;
@@ -661,12 +667,12 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   if (tid < TS_BLOCK / 2) {
     for (int it = tid; it < 3 * nfr; it += TS_BLOCK / 2) {
       const int f = it / 3, lpf = SINGLE ? f : f / p.K, k = f - lpf * p.K;
-      build_frame_row(p, e, __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), k, it - 3 * f, frames[f]);
+      build_frame_row(p, e, p.inl ? p.inl_link[gi * p.inl_stride + lpf] : __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), k, it - 3 * f, frames[f]);
     }
   } else {
     for (int it = tid - TS_BLOCK / 2; it < 4 * nfr; it += TS_BLOCK / 2) {
       const int f = it >> 2, lpf = SINGLE ? f : f / p.K, k = f - lpf * p.K;
-      build_frame_vec(p, e, __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), k, it & 3, frames[f]);
+      build_frame_vec(p, e, p.inl ? p.inl_link[gi * p.inl_stride + lpf] : __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), k, it & 3, frames[f]);
     }
   }
   const bool valid = tid < gcount;
