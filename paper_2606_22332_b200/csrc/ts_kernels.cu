@@ -4,15 +4,16 @@
 // Mapping: ONE THREAD PER (environment, taxel slot); a block owns one "patch group" of one
 // environment: up to TS_BLOCK consecutive taxel slots made of whole patches (packed on the
 // host, ts_api.cu).  Per block:
-//   phase 0  threads < npatch*K build the relative pose of every (patch link, object) pair in
-//            DOUBLE and park it in shared memory (frames);
+//   phase 0  seven threads per (patch link, object) pair build the relative pose in DOUBLE and park
+//            it in shared memory (frames);
 //   phase 1  per taxel: x_o = c + M x_j (double), phi (double), depth, Schmitt contact bit;
 //   phase 2  proximity march along a_j (fp32; evaluation 0 is the phase-1 query);
 //   phase 3  kinematic force/torque in double for warps that touch anything, rounded once;
 //   phase 4  noise chain: hysteresis -> crosstalk (neighbours through shared memory) ->
 //            Philox/Box-Muller random-walk drift -> dead taxels;
 //   phase 5  elastomer marker dilation as two separable passes over shared memory (double).
-// [E,T,6] and [E,M,3] outputs are staged in shared memory and written as coalesced float4.
+// Outputs go straight from registers to global memory with streaming stores; shared memory is kept
+// at 13 KB per block because it comes out of the L1 that serves the SDF gathers.
 //
 // Why double in phases 0/1/3/5: outputs are compared element by
 // element at rtol 1e-4 / atol 1e-6.  d = R - phi feeds f ~ d^1.2, the marker sum multiplies
@@ -40,7 +41,6 @@ struct D3 {
 };
 __device__ __forceinline__ F3 mk3(float x, float y, float z) { return F3{x, y, z}; }
 __device__ __forceinline__ F3 operator+(F3 a, F3 b) { return F3{a.x + b.x, a.y + b.y, a.z + b.z}; }
-__device__ __forceinline__ F3 operator-(F3 a, F3 b) { return F3{a.x - b.x, a.y - b.y, a.z - b.z}; }
 __device__ __forceinline__ F3 operator*(float s, F3 a) { return F3{s * a.x, s * a.y, s * a.z}; }
 __device__ __forceinline__ float dot(F3 a, F3 b) { return fmaf(a.x, b.x, fmaf(a.y, b.y, a.z * b.z)); }
 
@@ -300,19 +300,6 @@ __device__ __forceinline__ float grid_value_f(const TsStepParams& p, const float
   return phi;
 }
 
-// interior point, u in [0.75, N-1.75]: floor by a round-down add of 1.5*2^23 (ulp 1 there, so the sum is
-// floor(u) + 1.5*2^23 exactly; FADDs on the FMA pipe instead of F2I/I2F on the quarter-rate conversion
-// pipe).  The three 0x4B400000 biases of the integer images and the grid offset are folded into `cbase`
-// (32-bit wrap-around arithmetic), so the cell index costs two IMADs and one add.
-__device__ __forceinline__ float grid_value_fast(const float4* bank, unsigned cbase, unsigned N, F3 u) {
-  const float MAGIC = 12582912.f;  // 1.5 * 2^23
-  const float tx = __fadd_rd(u.x, MAGIC), ty = __fadd_rd(u.y, MAGIC), tz = __fadd_rd(u.z, MAGIC);
-  const unsigned idx = ((__float_as_uint(ty) * (N - 1u) + __float_as_uint(tx)) * N + __float_as_uint(tz)) + cbase;
-  const float fx = u.x - (tx - MAGIC), fy = u.y - (ty - MAGIC), fz = u.z - (tz - MAGIC);
-  const float4* q = bank + idx;
-  return trilerp(__ldg(q), __ldg(q + 1), fx, fy, fz);
-}
-
 // MUFU.SQRT (relative error <= 2^-22): |x| <= 0.1 m gives <= 3e-8 m per march evaluation, <= 5e-7 m over
 // 16 evaluations in the worst case against the 1e-6 m prox tolerance; the IEEE sqrtf costs 8 instructions.
 __device__ __forceinline__ float sqrt_approx(float x) {
@@ -394,9 +381,6 @@ __device__ __forceinline__ void store6(float* dst, const float* v) {
 }
 
 #define TS_FULL 0xffffffffu
-#ifndef TS_MARCH_LAST
-#define TS_MARCH_LAST 0
-#endif
 #ifndef TS_MIN_BLOCKS
 #define TS_MIN_BLOCKS 4
 #endif
@@ -561,6 +545,10 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
         if (__all_sync(TS_FULL, inside || !go)) {  // whole segment inside the grid for every marching lane
           const unsigned cbase = (unsigned)(int)F.prm[0] * (unsigned)p.grid_stride -
                                  0x4B400000u * (unsigned)((N - 1) * N + N + 1);
+          // Interior points (u in [0.75, N-1.75]): floor by a round-down add of 1.5*2^23 (ulp 1 there, so the
+          // sum is floor(u) + 1.5*2^23 exactly; FADDs on the FMA pipe instead of F2I/I2F on the quarter-rate
+          // conversion pipe).  The three 0x4B400000 biases of the integer images and the grid offset are
+          // folded into `cbase` (32-bit wrap-around arithmetic): two IMADs and one add per cell index.
           // A converging ray takes sub-voxel steps, so consecutive evaluations mostly fall into the same cell:
           // its 8 corners stay in registers and are reloaded only when the cell index changes.
           unsigned pidx = 0xffffffffu;
@@ -569,7 +557,7 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
             if (!__any_sync(TS_FULL, go)) break;
             if (go) {
               const F3 u = u0 + t * du;
-              const float MAGIC = 12582912.f;  // 1.5 * 2^23, see grid_value_fast
+              const float MAGIC = 12582912.f;  // 1.5 * 2^23
               const float tx = __fadd_rd(u.x, MAGIC), ty = __fadd_rd(u.y, MAGIC), tz = __fadd_rd(u.z, MAGIC);
               const unsigned idx = ((__float_as_uint(ty) * (unsigned)(N - 1) + __float_as_uint(tx)) * (unsigned)N + __float_as_uint(tz)) + cbase;
               if (idx != pidx) {
@@ -721,15 +709,13 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     const unsigned wb = __reduce_or_sync(TS_FULL, h > 0.f ? (1u << lp) : 0u);  // one shared atomic per warp
     if ((tid & 31) == 0 && wb) atomicOr(pmask, wb);
   }
-  const F3 xo = mk3((float)xd.x, (float)xd.y, (float)xd.z);  // kept for the march (last phase)
+  const F3 xo = mk3((float)xd.x, (float)xd.y, (float)xd.z);  // fp32 object-frame position for the march
 
   // state prefetch: the 12 (18) per-taxel state words of the noise chain are requested now so that their
   // HBM latency is covered by the march and the force/torque phases.
   NoiseState ns;
   if (NOISE) noise_load<HM>(p, e, j, valid, ns);
-#if !TS_MARCH_LAST
   march_phase<SINGLE>(p, frames, e, lp, valid, act, ej, phif, xo, P4, N4);
-#endif
 
   // ---- phase 3 (S5): kinematic force / torque (Eq. 4-9, D2) in double, link frame ---------------
   float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -858,9 +844,6 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     }
   }
 
-#if TS_MARCH_LAST
-  march_phase<SINGLE>(p, frames, e, lp, valid, act, ej, phif, xo, P4, N4);
-#endif
 }
 
 // ---------------------------------------------------------------------------------------
