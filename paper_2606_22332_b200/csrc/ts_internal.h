@@ -103,8 +103,8 @@ struct TsStepParams {
   uint8_t* dead;
   // state
   uint8_t* st_flags;          // [E,T] bit0 Schmitt, bit1 dead
-  float* st_hyst;             // [E,nh,Tp], nh = 6 (asym: y) / 12 (maxwell: xi then x_prev)
-  float* st_drift;            // [E,6,Tp]
+  float* st_hyst;             // [E,nh/2,Tp] float2 channel pairs, nh = 6 (asym: y) / 12 (maxwell: xi then x_prev)
+  float* st_drift;            // [E,3,Tp] float2 channel pairs
   const uint32_t* reset_step; // [E]
   const uint32_t* episode;    // [E]
   uint32_t gstep;

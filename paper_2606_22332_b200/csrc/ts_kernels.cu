@@ -400,24 +400,26 @@ template <int HM>  // hysteresis mode (TS_HYST_*), a compile-time constant so th
 __device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, bool valid, NoiseState& ns) {
   // 32-bit element indices (ts_create guarantees E * 12 * Tp < 2^32): one IMAD + LEA pair per access
   // instead of 64-bit address arithmetic that the register allocator keeps rematerialising.
+  // State rows hold channel PAIRS (float2): [E][nh/2][Tp] and [E][3][Tp], so a warp moves 256 contiguous
+  // bytes per access and a taxel needs 3 + 3 loads instead of 6 + 6.
   const unsigned Tp = (unsigned)p.Tp;
-  const unsigned ih = (unsigned)e * (HM == TS_HYST_MAXWELL ? 12u : 6u) * Tp + (unsigned)j;
-  const unsigned id = (unsigned)e * 6u * Tp + (unsigned)j;
-  const float* st_h = p.st_hyst;
-  const float* st_d = p.st_drift;
+  const unsigned ih = (unsigned)e * (HM == TS_HYST_MAXWELL ? 6u : 3u) * Tp + (unsigned)j;
+  const unsigned id = (unsigned)e * 3u * Tp + (unsigned)j;
+  const float2* st_h = reinterpret_cast<const float2*>(p.st_hyst);
+  const float2* st_d = reinterpret_cast<const float2*>(p.st_drift);
 #pragma unroll
   for (int c = 0; c < 6; ++c) { ns.sY[c] = 0.f; ns.sX[c] = 0.f; ns.sD[c] = 0.f; }
   if (valid) {
     if (HM != TS_HYST_OFF) {
 #pragma unroll
-      for (int c = 0; c < 6; ++c) ns.sY[c] = __ldcs(st_h + (ih + c * Tp));
+      for (int c = 0; c < 3; ++c) { const float2 v = __ldcs(st_h + (ih + c * Tp)); ns.sY[2 * c] = v.x; ns.sY[2 * c + 1] = v.y; }
     }
     if (HM == TS_HYST_MAXWELL) {
 #pragma unroll
-      for (int c = 0; c < 6; ++c) ns.sX[c] = __ldcs(st_h + (ih + (6 + c) * Tp));
+      for (int c = 0; c < 3; ++c) { const float2 v = __ldcs(st_h + (ih + (3 + c) * Tp)); ns.sX[2 * c] = v.x; ns.sX[2 * c + 1] = v.y; }
     }
 #pragma unroll
-    for (int c = 0; c < 6; ++c) ns.sD[c] = __ldcs(st_d + (id + c * Tp));
+    for (int c = 0; c < 3; ++c) { const float2 v = __ldcs(st_d + (id + c * Tp)); ns.sD[2 * c] = v.x; ns.sD[2 * c + 1] = v.y; }
   }
 }
 
@@ -426,10 +428,10 @@ template <int HM>
 __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, unsigned ej, int tid, int gstart, bool valid,
                                             bool act, bool deadb, const float* ft, const NoiseState& ns, float* bufB) {
   const unsigned Tp = (unsigned)p.Tp;
-  const unsigned ih = (unsigned)e * (HM == TS_HYST_MAXWELL ? 12u : 6u) * Tp + (unsigned)j;
-  const unsigned id = (unsigned)e * 6u * Tp + (unsigned)j;
-  float* const st_h = p.st_hyst;
-  float* const st_d = p.st_drift;
+  const unsigned ih = (unsigned)e * (HM == TS_HYST_MAXWELL ? 6u : 3u) * Tp + (unsigned)j;
+  const unsigned id = (unsigned)e * 3u * Tp + (unsigned)j;
+  float2* const st_h = reinterpret_cast<float2*>(p.st_hyst);
+  float2* const st_d = reinterpret_cast<float2*>(p.st_drift);
   float h[6];
   if (HM == TS_HYST_ASYM) {  // D3, Q14
 #pragma unroll
@@ -437,16 +439,24 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
       const float yp = ns.sY[c];
       const float al = (fabsf(ft[c]) > fabsf(yp)) ? p.alpha_load : p.alpha_unload;
       h[c] = act ? fmaf(al, ft[c] - yp, yp) : 0.f;
-      if (valid) __stcs(st_h + (ih + c * Tp), h[c]);
+    }
+    if (valid) {
+#pragma unroll
+      for (int c = 0; c < 3; ++c) __stcs(st_h + (ih + c * Tp), make_float2(h[2 * c], h[2 * c + 1]));
     }
   } else if (HM == TS_HYST_MAXWELL) {  // Eq. 29-30
 #pragma unroll
+    float zx[6];
+#pragma unroll
     for (int c = 0; c < 6; ++c) {
-      const float z = act ? fmaf(p.decay, ns.sY[c], ft[c] - ns.sX[c]) : 0.f;
-      h[c] = fmaf(p.beta, z, ft[c]);
-      if (valid) {
-        __stcs(st_h + (ih + c * Tp), z);
-        __stcs(st_h + (ih + (6 + c) * Tp), act ? ft[c] : 0.f);
+      zx[c] = act ? fmaf(p.decay, ns.sY[c], ft[c] - ns.sX[c]) : 0.f;
+      h[c] = fmaf(p.beta, zx[c], ft[c]);
+    }
+    if (valid) {
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        __stcs(st_h + (ih + c * Tp), make_float2(zx[2 * c], zx[2 * c + 1]));
+        __stcs(st_h + (ih + (3 + c) * Tp), act ? make_float2(ft[2 * c], ft[2 * c + 1]) : make_float2(0.f, 0.f));
       }
     }
   } else {
@@ -474,16 +484,19 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
   const int n0 = nb.x >= 0 ? nb.x - gstart : tid, n1 = nb.y >= 0 ? nb.y - gstart : tid;
   const int n2 = nb.z >= 0 ? nb.z - gstart : tid, n3 = nb.w >= 0 ? nb.w - gstart : tid;
   const float q4 = 0.25f * p.chi;
-  float outv[6];
+  float outv[6], Dn[6];
 #pragma unroll
   for (int c = 0; c < 6; ++c) {
     const float* hb = bufB + c * TS_BLOCK;
     const float hc = h[c];
     const float acc = fmaf(-4.f, hc, (hb[n0] + hb[n1]) + (hb[n2] + hb[n3]));  // sum_k (h_k - h_j)
     const float cx = fmaf(q4, acc, hc);
-    const float Dn = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], ns.sD[c]) : 0.f;
-    if (valid) __stcs(st_d + (id + c * Tp), Dn);
-    outv[c] = (act && !deadb) ? cx + Dn : 0.f;  // S8a dead (Eq. 28) last
+    Dn[c] = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], ns.sD[c]) : 0.f;
+    outv[c] = (act && !deadb) ? cx + Dn[c] : 0.f;  // S8a dead (Eq. 28) last
+  }
+  if (valid) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) __stcs(st_d + (id + c * Tp), make_float2(Dn[2 * c], Dn[2 * c + 1]));
   }
   if (p.ft_noisy && valid) store6(p.ft_noisy + ej * 6u, outv);
 }
