@@ -463,8 +463,9 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
 #pragma unroll
     for (int c = 0; c < 6; ++c) h[c] = ft[c];
   }
+  float2* const b2 = reinterpret_cast<float2*>(bufB);  // [3][TS_BLOCK] channel pairs
 #pragma unroll
-  for (int c = 0; c < 6; ++c) bufB[c * TS_BLOCK + tid] = h[c];
+  for (int c = 0; c < 3; ++c) b2[c * TS_BLOCK + tid] = make_float2(h[2 * c], h[2 * c + 1]);
   // S8d drift draws (Eq. 25): Philox streams 0 / 1 -> six normals (before the barrier: independent work)
   float z[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   if (act) {
@@ -484,12 +485,18 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
   const int n0 = nb.x >= 0 ? nb.x - gstart : tid, n1 = nb.y >= 0 ? nb.y - gstart : tid;
   const int n2 = nb.z >= 0 ? nb.z - gstart : tid, n3 = nb.w >= 0 ? nb.w - gstart : tid;
   const float q4 = 0.25f * p.chi;
-  float outv[6], Dn[6];
+  float outv[6], Dn[6], nsum[6];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const float2* hb = b2 + c * TS_BLOCK;
+    const float2 a0 = hb[n0], a1 = hb[n1], a2 = hb[n2], a3 = hb[n3];
+    nsum[2 * c] = (a0.x + a1.x) + (a2.x + a3.x);
+    nsum[2 * c + 1] = (a0.y + a1.y) + (a2.y + a3.y);
+  }
 #pragma unroll
   for (int c = 0; c < 6; ++c) {
-    const float* hb = bufB + c * TS_BLOCK;
     const float hc = h[c];
-    const float acc = fmaf(-4.f, hc, (hb[n0] + hb[n1]) + (hb[n2] + hb[n3]));  // sum_k (h_k - h_j)
+    const float acc = fmaf(-4.f, hc, nsum[c]);  // sum_k (h_k - h_j)
     const float cx = fmaf(q4, acc, hc);
     Dn[c] = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], ns.sD[c]) : 0.f;
     outv[c] = (act && !deadb) ? cx + Dn[c] : 0.f;  // S8a dead (Eq. 28) last
