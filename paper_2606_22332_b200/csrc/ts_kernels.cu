@@ -382,7 +382,7 @@ __device__ __forceinline__ void store6(float* dst, const float* v) {
 
 #define TS_FULL 0xffffffffu
 #ifndef TS_MIN_BLOCKS
-#define TS_MIN_BLOCKS 4
+#define TS_MIN_BLOCKS 5
 #endif
 
 // ---------------------------------------------------------------------------------------
@@ -924,7 +924,13 @@ unsigned long long ts_step_smem_bytes(const TsStepParams& p) {
 namespace {
 template <bool SINGLE, int HM>
 cudaError_t prep_one(int smem) {
-  return cudaFuncSetAttribute(ts_step_kernel<SINGLE, HM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  cudaError_t e = cudaFuncSetAttribute(ts_step_kernel<SINGLE, HM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  // Ask for no more shared memory than TS_MIN_BLOCKS resident blocks need (+1 KB reserved per block): the
+  // rest of the 228 KB stays L1, which serves the SDF gathers (measured: 1.51 -> 1.48 ms on config 5).
+  const int carve = (int)((TS_MIN_BLOCKS * (smem + 1024LL) * 100 + 228 * 1024 - 1) / (228 * 1024)) + 2;
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(ts_step_kernel<SINGLE, HM>, cudaFuncAttributePreferredSharedMemoryCarveout, carve > 100 ? 100 : carve);
+  return e;
 }
 template <bool SINGLE>
 void launch_one(const TsStepParams& p, int hm, dim3 grid, size_t smem, cudaStream_t st) {
