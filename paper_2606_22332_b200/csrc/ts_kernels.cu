@@ -392,6 +392,14 @@ __device__ __forceinline__ void store6(float* dst, const float* v) {
 // S8: noise chain of one taxel (O8): hysteresis -> crosstalk -> drift -> dead.  Shared by the fused
 // step kernel and the stand-alone noise kernel.
 // ---------------------------------------------------------------------------------------
+// Streaming float2 load that does not allocate in L1 (the state is read exactly once; L1 is kept for the
+// SDF gathers and the layout tables).
+__device__ __forceinline__ float2 ld_stream2(const float2* p) {
+  float2 v;
+  asm volatile("ld.global.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+  return v;
+}
+
 struct NoiseState {
   float sY[6], sX[6], sD[6];  // hysteresis y (asym) or xi (maxwell), maxwell x_prev, drift D
 };
@@ -412,14 +420,14 @@ __device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, 
   if (valid) {
     if (HM != TS_HYST_OFF) {
 #pragma unroll
-      for (int c = 0; c < 3; ++c) { const float2 v = __ldcs(st_h + (ih + c * Tp)); ns.sY[2 * c] = v.x; ns.sY[2 * c + 1] = v.y; }
+      for (int c = 0; c < 3; ++c) { const float2 v = ld_stream2(st_h + (ih + c * Tp)); ns.sY[2 * c] = v.x; ns.sY[2 * c + 1] = v.y; }
     }
     if (HM == TS_HYST_MAXWELL) {
 #pragma unroll
-      for (int c = 0; c < 3; ++c) { const float2 v = __ldcs(st_h + (ih + (3 + c) * Tp)); ns.sX[2 * c] = v.x; ns.sX[2 * c + 1] = v.y; }
+      for (int c = 0; c < 3; ++c) { const float2 v = ld_stream2(st_h + (ih + (3 + c) * Tp)); ns.sX[2 * c] = v.x; ns.sX[2 * c + 1] = v.y; }
     }
 #pragma unroll
-    for (int c = 0; c < 3; ++c) { const float2 v = __ldcs(st_d + (id + c * Tp)); ns.sD[2 * c] = v.x; ns.sD[2 * c + 1] = v.y; }
+    for (int c = 0; c < 3; ++c) { const float2 v = ld_stream2(st_d + (id + c * Tp)); ns.sD[2 * c] = v.x; ns.sD[2 * c + 1] = v.y; }
   }
 }
 
