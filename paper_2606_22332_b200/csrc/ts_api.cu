@@ -23,8 +23,8 @@ struct ts_ctx {
   uint32_t gstep = 0;
   uint32_t dead_thr = 0;
   // device buffers
-  float4 *tx_pos = nullptr, *tx_nrm = nullptr, *mk_pos = nullptr, *mk_nrm = nullptr;
-  int4* tx_nbr = nullptr;
+  float4 *tx_pos = nullptr, *mk_pos = nullptr, *mk_nrm = nullptr;
+  int32_t* tx_meta = nullptr;
   TsPatch* patches = nullptr;
   TsGroup* groups = nullptr;
   TsChunk* chunks = nullptr;
@@ -77,8 +77,8 @@ struct DeviceGuard {
 };
 
 void free_all(ts_ctx* c) {
-  cudaFree(c->tx_pos); cudaFree(c->tx_nrm); cudaFree(c->mk_pos); cudaFree(c->mk_nrm); cudaFree(c->patches);
-  cudaFree(c->tx_nbr); cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->grp_link);
+  cudaFree(c->tx_pos); cudaFree(c->tx_meta); cudaFree(c->mk_pos); cudaFree(c->mk_nrm); cudaFree(c->patches);
+  cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->grp_link);
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->bank); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch);
   for (float* q : c->stage_in) cudaFree(q);
@@ -91,7 +91,7 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   std::memset(&p, 0, sizeof(p));
   p.E = g.n_envs; p.L = g.n_links; p.K = g.objs_per_env; p.T = c->T; p.P = c->P; p.M = c->M;
   p.G = c->G; p.Tp = c->Tp; p.frames_per_group = c->frames_per_group;
-  p.tx_nbr = c->tx_nbr; p.groups = c->groups; p.chunks = c->chunks; p.mk_item1 = c->mk_item1; p.mk_item2 = c->mk_item2;
+  p.groups = c->groups; p.chunks = c->chunks; p.mk_item1 = c->mk_item1; p.mk_item2 = c->mk_item2;
   p.mk_tab = c->mk_tab; p.grp_link = c->grp_link;
   p.inl = 0; p.inl_stride = c->frames_per_group;
   if (c->G <= TS_INL_GROUPS && c->G * c->frames_per_group <= TS_INL_LINKS && (int)c->h_groups.size() == c->G) {
@@ -102,7 +102,7 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
     }
   }
   p.env_id_base = (uint32_t)g.env_id_base;
-  p.tx_pos = c->tx_pos; p.tx_nrm = c->tx_nrm; p.patches = c->patches; p.mk_pos = c->mk_pos; p.mk_nrm = c->mk_nrm;
+  p.tx_pos = c->tx_pos; p.tx_meta = c->tx_meta; p.patches = c->patches; p.mk_pos = c->mk_pos; p.mk_nrm = c->mk_nrm;
   p.g_type = c->g_type; p.g_params = c->g_params; p.bank = c->bank;
   p.grid_n = c->grid_n; p.voxel = c->voxel; p.inv_voxel = 1.0f / c->voxel; p.inv_voxel_d = 1.0 / (double)c->voxel;
   p.grid_stride = ts_bank_elems_per_grid(c->grid_n);
@@ -185,13 +185,10 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
 
   // ---- layout -> device records; trailing filler slots are covered by filler patches ----
   const int T = lay->n_taxels;
-  std::vector<float4> pos(T), nrm(T);
-  std::vector<int4> nbr(T);
-  for (int t = 0; t < T; ++t) {
+  std::vector<float4> pos(T);
+  std::vector<int32_t> meta(T, 0);
+  for (int t = 0; t < T; ++t)
     pos[t] = make_float4(lay->pos[3 * t], lay->pos[3 * t + 1], lay->pos[3 * t + 2], lay->radius[t]);
-    nrm[t] = make_float4(lay->nrm[3 * t], lay->nrm[3 * t + 1], lay->nrm[3 * t + 2], 0.f);
-    nbr[t] = make_int4(lay->nbr[4 * t], lay->nbr[4 * t + 1], lay->nbr[4 * t + 2], lay->nbr[4 * t + 3]);
-  }
   const int M = (int)lay->marker_patch.size();
   std::vector<TsPatch> pts;
   std::vector<double> tab;
@@ -206,8 +203,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     const double u[3] = {d.u_axis[0], d.u_axis[1], d.u_axis[2]}, v[3] = {d.v_axis[0], d.v_axis[1], d.v_axis[2]};
     q.ua = make_float4(d.u_axis[0], d.u_axis[1], d.u_axis[2], 0.f);
     q.va = make_float4(d.v_axis[0], d.v_axis[1], d.v_axis[2], 0.f);
-    q.na = q.mnu > 0 ? make_float4(lay->marker_nrm[3 * q.mstart], lay->marker_nrm[3 * q.mstart + 1], lay->marker_nrm[3 * q.mstart + 2], 0.f)
-                     : make_float4(0.f, 0.f, 1.f, 0.f);
+    q.na = make_float4(lay->nrm[3 * q.start], lay->nrm[3 * q.start + 1], lay->nrm[3 * q.start + 2], 0.f);  // = marker normal
     q.direct = (cfg->c_e != 1.0f || q.mnu * q.nv > TS_CHUNK) ? 1 : 0;
     q.tab = (int32_t)tab.size();
     q.i1off = (int32_t)item1.size();
@@ -278,7 +274,12 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     g.nchunk = (int32_t)chunks.size() - g.chunk0;
     for (int l = 0; l < g.npatch; ++l) {  // group-local patch index: per taxel (in nrm.w) and per marker item
       const TsPatch& q = pts[g.patch0 + l];
-      for (int t = q.start; t < q.start + q.n; ++t) std::memcpy(&nrm[t].w, &l, sizeof(int));
+      for (int t = q.start; t < q.start + q.n; ++t) {  // per-taxel word: patch index, grid width, neighbour bits
+        int m = l | ((q.nu & 255) << 8);
+        for (int a = 0; a < 4; ++a)
+          if (lay->nbr[4 * t + a] >= 0) m |= 1 << (16 + a);
+        meta[t] = m;
+      }
       if (q.mnu > 0 && !q.direct)
         for (int iq = 0; iq < q.nv; ++iq)
           for (int a = 0; a < q.mnu; ++a) item1[q.i1off + iq * q.mnu + a] = l | (a << 8) | (iq << 16);
@@ -319,8 +320,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     if (e_ != cudaSuccess) { ts_status s_ = cuda_fail(nullptr, e_, "cudaMalloc " #ptr); free_all(c); delete c; return s_; } \
   } while (0)
   TS_ALLOC(c->tx_pos, sizeof(float4) * T);
-  TS_ALLOC(c->tx_nrm, sizeof(float4) * T);
-  TS_ALLOC(c->tx_nbr, sizeof(int4) * T);
+  TS_ALLOC(c->tx_meta, sizeof(int32_t) * T);
   TS_ALLOC(c->mk_pos, sizeof(float4) * mpos.size());
   TS_ALLOC(c->mk_nrm, sizeof(float4) * mnrm.size());
   TS_ALLOC(c->patches, sizeof(TsPatch) * pts.size());
@@ -348,8 +348,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   cudaError_t e = cudaSuccess;
   auto cp = [&](void* d, const void* h, size_t b) { if (e == cudaSuccess) e = cudaMemcpy(d, h, b, cudaMemcpyHostToDevice); };
   cp(c->tx_pos, pos.data(), sizeof(float4) * T);
-  cp(c->tx_nrm, nrm.data(), sizeof(float4) * T);
-  cp(c->tx_nbr, nbr.data(), sizeof(int4) * T);
+  cp(c->tx_meta, meta.data(), sizeof(int32_t) * T);
   cp(c->mk_pos, mpos.data(), sizeof(float4) * mpos.size());
   cp(c->mk_nrm, mnrm.data(), sizeof(float4) * mnrm.size());
   cp(c->patches, pts.data(), sizeof(TsPatch) * pts.size());

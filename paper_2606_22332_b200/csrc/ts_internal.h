@@ -71,8 +71,7 @@ struct TsStepParams {
   uint32_t env_id_base;
   // layout
   const float4* tx_pos;   // [T] (x, y, z, R_j); R_j = 0 for every inactive slot
-  const float4* tx_nrm;   // [T] (nx, ny, nz, bits: group-local patch index)
-  const int4* tx_nbr;     // [T] neighbour slots (-u,+u,-v,+v), -1 = none
+  const int32_t* tx_meta; // [T] bits 0-7 group-local patch index, 8-15 patch nu, 16-19 has -u/+u/-v/+v neighbour
   const TsPatch* patches; // [P]
   const TsGroup* groups;  // [G]
   const TsChunk* chunks;

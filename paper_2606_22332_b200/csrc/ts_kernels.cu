@@ -101,15 +101,16 @@ struct FrameS {
   float cf[3];
   float prm[4];
   int type;
-  int pad[3];
+  float dirf[3];   // M n: march direction of the patch normal in the object frame (fp32)
 };
 
 // One frame is built by SEVEN threads so that the dependent double-precision chain the whole block
 // waits for stays short (~60 instructions): "row" items r = 0..2 (row r of M and c[r]) run in the lower
 // half of the block, "vector" items s = 0..3 (wO, wL, vbar, cbar) in the upper half, so a warp never
 // executes both code paths.
-__device__ __forceinline__ void build_frame_row(const TsStepParams& p, int e, int link, int k, int r, FrameS& F) {
+__device__ __forceinline__ void build_frame_row(const TsStepParams& p, int e, int link, int pidx, int k, int r, FrameS& F) {
   if (link < 0) return;
+  const float4 na = __ldg(&p.patches[pidx].na);
   const size_t ek = (size_t)e * p.K + k, el = (size_t)e * p.L + link;
   double RL[9];
   quat_Rd(p.link_quat + el * 4, RL);
@@ -135,6 +136,7 @@ __device__ __forceinline__ void build_frame_row(const TsStepParams& p, int e, in
   const double cr = fma(o0, d.x, fma(o1, d.y, o2 * d.z));
   F.c[r] = cr;
   F.cf[r] = (float)cr;
+  F.dirf[r] = (float)fma(F.M[r * 3], (double)na.x, fma(F.M[r * 3 + 1], (double)na.y, F.M[r * 3 + 2] * (double)na.z));
 }
 
 __device__ __forceinline__ void build_frame_vec(const TsStepParams& p, int e, int link, int k, int sub, FrameS& F) {
@@ -434,7 +436,8 @@ __device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, 
 // Every thread of the block must call this (it contains one __syncthreads).
 template <int HM>
 __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, unsigned ej, int tid, int gstart, bool valid,
-                                            bool act, bool deadb, const float* ft, const NoiseState& ns, float* bufB) {
+                                            bool act, bool deadb, int meta, const float* ft, const NoiseState& ns,
+                                            float* bufB) {
   const unsigned Tp = (unsigned)p.Tp;
   const unsigned ih = (unsigned)e * (HM == TS_HYST_MAXWELL ? 6u : 3u) * Tp + (unsigned)j;
   const unsigned id = (unsigned)e * 3u * Tp + (unsigned)j;
@@ -489,9 +492,9 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
   __syncthreads();
   // S8c crosstalk (D4): c_j = h_j + chi/4 sum_{k in N4(j)} (h_k - h_j); a missing neighbour is
   // replaced by the taxel itself (h_j - h_j = 0), so the sum needs no predicates.
-  const int4 nb = __ldg(p.tx_nbr + j);
-  const int n0 = nb.x >= 0 ? nb.x - gstart : tid, n1 = nb.y >= 0 ? nb.y - gstart : tid;
-  const int n2 = nb.z >= 0 ? nb.z - gstart : tid, n3 = nb.w >= 0 ? nb.w - gstart : tid;
+  const int nu = (meta >> 8) & 255;  // slots of a patch are consecutive: -u/+u = tid -/+ 1, -v/+v = tid -/+ nu
+  const int n0 = (meta & (1 << 16)) ? tid - 1 : tid, n1 = (meta & (1 << 17)) ? tid + 1 : tid;
+  const int n2 = (meta & (1 << 18)) ? tid - nu : tid, n3 = (meta & (1 << 19)) ? tid + nu : tid;
   const float q4 = 0.25f * p.chi;
   float outv[6], Dn[6], nsum[6];
 #pragma unroll
@@ -538,12 +541,12 @@ __global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_cons
     act = __ldg(&p.tx_pos[j].w) > 0.f;
     deadb = act && ((p.st_flags[ej] >> 1) & 1);
   }
-  noise_chain<HM>(p, e, j, ej, tid, gstart, valid, act, deadb, ft, ns, bufB);
+  noise_chain<HM>(p, e, j, ej, tid, gstart, valid, act, deadb, valid ? __ldg(p.tx_meta + j) : 0, ft, ns, bufB);
 }
 
 template <bool SINGLE>
 __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS* frames, int e, int lp, bool valid, bool act,
-                                            unsigned ej, float phif, F3 xo, float4 P4, float4 N4) {
+                                            unsigned ej, float phif, F3 xo, float4 P4, int pidx) {
 // ---- phase 2 (S7): proximity march, t <- min(t + max(phi(q + t a), 0), r_prox), K_m evaluations.
   // Exact shortcuts (O7): evaluation 0 is the query above; t = r_prox is absorbing; an evaluation
   // that leaves t unchanged repeats forever.
@@ -554,12 +557,10 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
       t = fminf(fmaxf(phif, 0.f), p.r_prox);
       go = (t > 0.f) && (t < p.r_prox);
     }
-    const F3 nj = mk3(N4.x, N4.y, N4.z);
     if (SINGLE) {
       const FrameS& F = frames[lp];
       const int gtype = __ldg(p.g_type + e);  // block-uniform (one object per env)
-      const F3 dr = mk3(fmaf(F.Mf[0], nj.x, fmaf(F.Mf[1], nj.y, F.Mf[2] * nj.z)), fmaf(F.Mf[3], nj.x, fmaf(F.Mf[4], nj.y, F.Mf[5] * nj.z)),
-                        fmaf(F.Mf[6], nj.x, fmaf(F.Mf[7], nj.y, F.Mf[8] * nj.z)));
+      const F3 dr = mk3(F.dirf[0], F.dirf[1], F.dirf[2]);  // M n of the patch normal, built with the frame
       if (gtype == TS_GEOM_SDF) {
         const int N = p.grid_n;
         const float4* bank_g = p.bank + (size_t)(int)F.prm[0] * p.grid_stride;
@@ -628,6 +629,8 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
       }
     } else {
       const F3 xj = mk3(P4.x, P4.y, P4.z);
+      const float4 na = __ldg(&p.patches[pidx].na);
+      const F3 nj = mk3(na.x, na.y, na.z);
       for (int it = 1; it < p.march_steps; ++it) {
         if (!__any_sync(TS_FULL, go)) break;
         if (go) {
@@ -683,7 +686,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   if (tid < TS_BLOCK / 2) {
     for (int it = tid; it < 3 * nfr; it += TS_BLOCK / 2) {
       const int f = it / 3, lpf = SINGLE ? f : f / p.K, k = f - lpf * p.K;
-      build_frame_row(p, e, p.inl ? p.inl_link[gi * p.inl_stride + lpf] : __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), k, it - 3 * f, frames[f]);
+      build_frame_row(p, e, p.inl ? p.inl_link[gi * p.inl_stride + lpf] : __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), patch0 + lpf, k, it - 3 * f, frames[f]);
     }
   } else {
     for (int it = tid - TS_BLOCK / 2; it < 4 * nfr; it += TS_BLOCK / 2) {
@@ -694,8 +697,9 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const bool valid = tid < gcount;
   const int j = gstart + (valid ? tid : 0);
   const unsigned ej = (unsigned)e * (unsigned)p.T + (unsigned)j;  // < 2^32 / 12 (checked by ts_create)
-  const float4 P4 = __ldg(p.tx_pos + j), N4 = __ldg(p.tx_nrm + j);
-  const int lp = __float_as_int(N4.w);
+  const float4 P4 = __ldg(p.tx_pos + j);
+  const int meta = valid ? __ldg(p.tx_meta + j) : 0;  // idle threads: no neighbours, patch 0
+  const int lp = meta & 255;
   const float Rj = valid ? P4.w : 0.f;  // R_j = 0: inactive slot
   const bool act = Rj > 0.f;
   uint8_t flag = valid ? p.st_flags[ej] : (uint8_t)0;
@@ -743,7 +747,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   // HBM latency is covered by the march and the force/torque phases.
   NoiseState ns;
   if (NOISE) noise_load<HM>(p, e, j, valid, ns);
-  march_phase<SINGLE>(p, frames, e, lp, valid, act, ej, phif, xo, P4, N4);
+  march_phase<SINGLE>(p, frames, e, lp, valid, act, ej, phif, xo, P4, patch0 + lp);
 
   // ---- phase 3 (S5): kinematic force / torque (Eq. 4-9, D2) in double, link frame ---------------
   float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -753,7 +757,10 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
       const D3 g = grad_d(p, F.type, F.prm, xd);
       const double g2 = dot(g, g);
       D3 mbar;  // contact normal in the link frame, m_bar = R_L^T m = M^T g / |g|
-      if (g2 < 1e-24) mbar = D3{-(double)N4.x, -(double)N4.y, -(double)N4.z};  // Q2
+      if (g2 < 1e-24) {  // Q2: m = -a_j, i.e. minus the patch normal in the link frame
+        const float4 na = __ldg(&p.patches[patch0 + lp].na);
+        mbar = D3{-(double)na.x, -(double)na.y, -(double)na.z};
+      }
       else mbar = drsqrt_n(g2) * mulRT(F.M, g);
       const double sj = (double)__powf(d, p.alpha);  // s_j = d^alpha
       const D3 x = D3{(double)P4.x, (double)P4.y, (double)P4.z};
@@ -780,7 +787,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   if (p.ft && valid) store6(p.ft + ej * 6u, ft);
 
   // ---- phase 4 (S8): noise chain (fused variant); contains the barrier that also publishes hh / ha / pact
-  if (NOISE) noise_chain<HM>(p, e, j, ej, tid, gstart, valid, act, deadb, ft, ns, bufB);
+  if (NOISE) noise_chain<HM>(p, e, j, ej, tid, gstart, valid, act, deadb, meta, ft, ns, bufB);
   else __syncthreads();
 
   // ---- phase 5 (S6): elastomer marker dilation (Eq. 18-21, 23 first sum) ----------------------
