@@ -19,6 +19,8 @@
 //   marker                   single-source closed form at r* (P11)
 //   march                    plane closed form t_k = D/cos(th) (1-(1-cos th)^k) (P12)
 //   noise                    Maxwell / asym closed forms, crosstalk patch-sum, drift moments, dead (P13-P16)
+//   remaining A.8 knobs      bias / white-noise moments, quantisation levels and hand values, per-episode gain,
+//                            stuck readout range and constancy (P19-P22; readings R1-R4 in DESIGN.md)
 //   whole path               rigid-frame invariance, filler slots, no-contact zeros (P8, P17)
 // parity unpinned: none of the functions; the *joint* output on star grids with all
 // stages on (configs 4-5) is pinned only through the per-stage pins above (P18).
@@ -247,6 +249,12 @@ typedef struct orc_params {
   int32_t hyst_mode;  // 0 off, 1 Maxwell (Eq. 29-30), 2 asymmetric first-order (D3)
   float beta, tau, alpha_load, alpha_unload;
   float p_dead, chi;
+  // remaining knobs of App. A.8 (readings R1-R4)
+  float sigma_white_force, sigma_white_torque;  // Eq. 25 n_t ~ N(0, sigma^2), channels 0-2 / 3-5
+  float bias_force, bias_torque;                // Eq. 25 constant bias b
+  float quant_force, quant_torque;              // Eq. 25 quantisation step q (0 = off)
+  float gain_min, gain_max;                     // Eq. 27 per-reset gain gamma_bj ~ U[min, max] (1, 1 = off)
+  float stuck_min_force, stuck_max_force, stuck_min_torque, stuck_max_torque;  // Eq. 28 stuck readout z_bj ~ U[l, u]
 } orc_params;
 }
 
@@ -269,6 +277,7 @@ struct Oracle {
   // state
   std::vector<uint8_t> ybit;                // Schmitt state [E,T]
   std::vector<double> hyst_a, hyst_b, drift;  // [E,T,6]: (xi, x_prev) or (y, -)
+  double* aux_quant = nullptr;                // [E,T,6] comparator aid, see orc_set_aux_quant
   std::vector<uint32_t> n_step, episode;      // [E]
 };
 
@@ -587,8 +596,16 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
       double decay = std::exp(-(double)pr.dt / (double)pr.tau);
       for (int j = 0; j < T; ++j) {
         size_t ej = (size_t)e * T + j;
+        // Eq. 27 (R2): per-unit calibration gain, drawn once per (env, taxel, episode): stream 3, n = 0, word 0
+        double gain = 1.0;
+        if (o.radius[j] > 0.0 && (pr.gain_min != 1.0f || pr.gain_max != 1.0f)) {
+          uint32_t key[2] = {pr.seed_lo, pr.seed_hi}, w[4];
+          uint32_t cg[4] = {(uint32_t)o.env_id[e], (uint32_t)j, 0u, (o.episode[e] << 4) | 3u};
+          philox4x32_10(cg, key, w);
+          gain = (double)pr.gain_min + ((double)pr.gain_max - (double)pr.gain_min) * word_to_uniform(w[0]);
+        }
         for (int c = 0; c < 6; ++c) {
-          double x = ftc[(size_t)j * 6 + c], hval = x;
+          double x = gain * ftc[(size_t)j * 6 + c], hval = x;
           if (aux_asym) aux_asym[ej * 6 + c] = INFINITY;
           if (o.radius[j] > 0.0) {
             if (pr.hyst_mode == 1) {                                      // Eq. 29-30
@@ -622,8 +639,36 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
           box_muller(w0[2], w0[3], &z[2], &z[3]);
           box_muller(w1[0], w1[1], &z[4], &z[5]);
         }
+        // Eq. 25 white noise n_t (R3): streams 6 / 7 of the same counter, laid out like the drift draws
+        double zw[6] = {0, 0, 0, 0, 0, 0};
+        if (active && (pr.sigma_white_force != 0.0f || pr.sigma_white_torque != 0.0f)) {
+          uint32_t key[2] = {pr.seed_lo, pr.seed_hi}, w0[4], w1[4];
+          uint32_t c0[4] = {(uint32_t)o.env_id[e], (uint32_t)j, n, (o.episode[e] << 4) | 6u};
+          uint32_t c1[4] = {(uint32_t)o.env_id[e], (uint32_t)j, n, (o.episode[e] << 4) | 7u};
+          philox4x32_10(c0, key, w0);
+          philox4x32_10(c1, key, w1);
+          box_muller(w0[0], w0[1], &zw[0], &zw[1]);
+          box_muller(w0[2], w0[3], &zw[2], &zw[3]);
+          box_muller(w1[0], w1[1], &zw[4], &zw[5]);
+        }
+        // Eq. 28 stuck readout z_bj (R4): streams 4 / 5, n = 0; only dead taxels use it
+        double stuck[6] = {0, 0, 0, 0, 0, 0};
+        if (active && deadv[j]) {
+          uint32_t key[2] = {pr.seed_lo, pr.seed_hi}, w0[4], w1[4];
+          uint32_t c0[4] = {(uint32_t)o.env_id[e], (uint32_t)j, 0u, (o.episode[e] << 4) | 4u};
+          uint32_t c1[4] = {(uint32_t)o.env_id[e], (uint32_t)j, 0u, (o.episode[e] << 4) | 5u};
+          philox4x32_10(c0, key, w0);
+          philox4x32_10(c1, key, w1);
+          const uint32_t ww[6] = {w0[0], w0[1], w0[2], w0[3], w1[0], w1[1]};
+          for (int c = 0; c < 6; ++c) {
+            double lo = c < 3 ? (double)pr.stuck_min_force : (double)pr.stuck_min_torque;
+            double hi = c < 3 ? (double)pr.stuck_max_force : (double)pr.stuck_max_torque;
+            stuck[c] = lo + (hi - lo) * word_to_uniform(ww[c]);
+          }
+        }
         for (int c = 0; c < 6; ++c) {
           double out = 0.0;
+          if (o.aux_quant) o.aux_quant[ej * 6 + c] = INFINITY;
           if (active) {
             double hj = hcl[(size_t)j * 6 + c];
             double acc = 0.0;                                             // D4, Q11
@@ -635,7 +680,20 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
             double sig = (c < 3) ? (double)pr.sigma_rw_force : (double)pr.sigma_rw_torque;
             double D = o.drift[ej * 6 + c] + sig * z[c];                  // Eq. 25 drift
             o.drift[ej * 6 + c] = D;
-            out = deadv[j] ? 0.0 : cj + D;                                // Eq. 28, D5
+            double sw = (c < 3) ? (double)pr.sigma_white_force : (double)pr.sigma_white_torque;
+            double bias = (c < 3) ? (double)pr.bias_force : (double)pr.bias_torque;
+            double y = cj + bias + sw * zw[c] + D;                        // Eq. 25 before quantisation (R1)
+            float q = (c < 3) ? pr.quant_force : pr.quant_torque;
+            if (q > 0.0f) {
+              // Eq. 25 quantize(., q): the integer decision is taken in fp32 (the precision of the readout):
+              // k = rint(y / q) on the fp32 image of y, round half to even; result k q in fp32.
+              float yf = (float)y;
+              float r = yf / q;
+              float k = std::nearbyintf(r);
+              if (o.aux_quant) o.aux_quant[ej * 6 + c] = (0.5 - std::fabs((double)r - (double)k)) * (double)q;
+              y = (double)(k * q);
+            }
+            out = deadv[j] ? stuck[c] : y;                                // Eq. 28 (D5 when l = u = 0)
           }
           if (ft_noisy) ft_noisy[ej * 6 + c] = out;
         }
@@ -644,6 +702,11 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
     o.n_step[e] += 1;
   }
 }
+
+// Comparator aid: aux_quant[E,T,6] receives, on every following step, the distance (in units of the
+// readout) of the pre-quantisation value from the nearest rounding boundary of Eq. 25's quantize(),
+// +inf where quantisation is off.  NULL switches it off.
+void orc_set_aux_quant(void* h, double* aux_quant) { ((Oracle*)h)->aux_quant = aux_quant; }
 
 // Stand-alone pieces for the pins -------------------------------------------------
 

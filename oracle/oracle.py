@@ -39,7 +39,13 @@ class OrcParams(C.Structure):
                 ("noise_enable", C.c_int32), ("seed_lo", C.c_uint32), ("seed_hi", C.c_uint32),
                 ("sigma_rw_force", C.c_float), ("sigma_rw_torque", C.c_float), ("hyst_mode", C.c_int32),
                 ("beta", C.c_float), ("tau", C.c_float), ("alpha_load", C.c_float), ("alpha_unload", C.c_float),
-                ("p_dead", C.c_float), ("chi", C.c_float)]
+                ("p_dead", C.c_float), ("chi", C.c_float),
+                ("sigma_white_force", C.c_float), ("sigma_white_torque", C.c_float),
+                ("bias_force", C.c_float), ("bias_torque", C.c_float),
+                ("quant_force", C.c_float), ("quant_torque", C.c_float),
+                ("gain_min", C.c_float), ("gain_max", C.c_float),
+                ("stuck_min_force", C.c_float), ("stuck_max_force", C.c_float),
+                ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float)]
 
 
 HYST = {"off": 0, "maxwell": 1, "asym": 2}
@@ -71,6 +77,7 @@ def lib():
         L.orc_march.restype = C.c_double
         L.orc_march.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p, C.c_void_p,
                                 C.c_double, C.c_int]
+        L.orc_set_aux_quant.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_max_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -93,7 +100,10 @@ def make_params(physics=None, noise=None):
     d = dict(k_n=500.0, c_n=1.0, alpha=1.2, k_t=2.0, k_omega=2.0, mu=1.0, eta_on=5e-4, eta_off=5e-4, use_velocity=1,
              s_d=100.0, lambda_d=8000.0, alpha_e=1.2, c_e=1.0, r_prox=0.020, march_steps=16, dt=0.005,
              noise_enable=0, seed=0, sigma_rw_force=0.0, sigma_rw_torque=0.0, hyst_mode=0, beta=0.0, tau=0.05,
-             alpha_load=1.0, alpha_unload=1.0, p_dead=0.0, chi=0.0)
+             alpha_load=1.0, alpha_unload=1.0, p_dead=0.0, chi=0.0,
+             sigma_white_force=0.0, sigma_white_torque=0.0, bias_force=0.0, bias_torque=0.0, quant_force=0.0,
+             quant_torque=0.0, gain_min=1.0, gain_max=1.0, stuck_min_force=0.0, stuck_max_force=0.0,
+             stuck_min_torque=0.0, stuck_max_torque=0.0)
     for src in (physics, noise):
         if src:
             for k, v in src.items():
@@ -200,7 +210,10 @@ class Oracle:
             out["aux_boxgap"] = np.zeros((E, T))
             if self.params.noise_enable:
                 out["aux_asym"] = np.zeros((E, T, 6))
+                if self.params.quant_force > 0 or self.params.quant_torque > 0:
+                    out["aux_quant"] = np.zeros((E, T, 6))
         g = out.get
+        self.L.orc_set_aux_quant(self.h, _p(g("aux_quant")))
         self.L.orc_step(self.h, _p(a["link_pos"]), _p(a["link_quat"]), _p(a["link_linvel"]), _p(a["link_angvel"]),
                         _p(a["obj_pos"]), _p(a["obj_quat"]), _p(a["obj_linvel"]), _p(a["obj_angvel"]),
                         _p(g("contact")), _p(g("depth")), _p(g("ft")), _p(g("marker")), _p(g("prox")),

@@ -555,6 +555,104 @@ def test_dead_taxels():
     assert (m3[np.arange(32) != 3] == keep[np.arange(32) != 3]).all() and (m3[3] != keep[3]).any()
 
 
+# ------------------------------------------------------------------ P19-P22 remaining knobs of Eq. 25-28
+def _contact_scene(noise, E=64, nu=8, nv=8):
+    """One 8x8 patch pressed 1 mm into the r = 30 mm sphere (centre taxels touch), clean ft != 0."""
+    o = scene([one_patch(nu, nv, 0.02, 0.02)], nu * nv, E=E, noise=dict(dict(noise_enable=1, seed=99, hyst_mode="off"), **noise))
+    o.threads = 4
+    return o, inputs(E=E, link_pos=(0, 0, -0.031), link_quat=(1, 0, 0, 0))
+
+
+def test_bias_and_white_noise_eq25():
+    # Eq. 25 with drift off: ft_noisy = ft + b + n_t, n_t ~ N(0, sigma^2), fresh every step
+    o, x = _contact_scene(dict(bias_force=0.25, bias_torque=-0.003, sigma_white_force=2e-3, sigma_white_torque=1e-5))
+    a, b = o.step(x), o.step(x)
+    clean = a["ft"]
+    assert np.abs(clean).max() > 0.01                                        # the scene really touches
+    ra, rb = a["ft_noisy"] - clean, b["ft_noisy"] - clean
+    assert abs(ra[..., :3].mean() - 0.25) < 4 * 2e-3 / math.sqrt(ra[..., :3].size)
+    assert abs(ra[..., 3:].mean() + 0.003) < 4 * 1e-5 / math.sqrt(ra[..., 3:].size)
+    assert abs(ra[..., :3].std() / 2e-3 - 1) < 0.03 and abs(ra[..., 3:].std() / 1e-5 - 1) < 0.03
+    assert abs(np.corrcoef(ra[..., 0].ravel(), rb[..., 0].ravel())[0, 1]) < 0.05    # white: no memory
+    # with sigma = 0 the shift is exactly the bias
+    o2, _ = _contact_scene(dict(bias_force=0.25, bias_torque=-0.003))
+    r2 = o2.step(x)
+    np.testing.assert_allclose(r2["ft_noisy"][..., :3] - r2["ft"][..., :3], 0.25, rtol=0, atol=1e-7)
+    np.testing.assert_allclose(r2["ft_noisy"][..., 3:] - r2["ft"][..., 3:], -0.003, rtol=0, atol=1e-9)
+    # white noise and drift use different Philox streams: with both on, the step-1 residual has variance s_w^2 + s_rw^2
+    o3, _ = _contact_scene(dict(sigma_white_force=2e-3, sigma_rw_force=1e-3, sigma_white_torque=0.0, sigma_rw_torque=0.0))
+    r3 = o3.step(x)
+    res = (r3["ft_noisy"] - r3["ft"])[..., :3]
+    assert abs(res.var() / (4e-6 + 1e-6) - 1) < 0.05
+
+
+def test_quantisation_eq25():
+    # quantize(y, q) = q rint(y / q): every readout is a multiple of q, within q/2 of the unquantised one
+    q_f, q_t = 0.01, 1e-4
+    o, x = _contact_scene(dict(quant_force=q_f, quant_torque=q_t))
+    ref, _ = _contact_scene(dict())
+    yq, y = o.step(x), ref.step(x)["ft_noisy"]
+    out = yq["ft_noisy"]
+    kf, kt = out[..., :3] / np.float32(q_f), out[..., 3:] / np.float32(q_t)
+    assert np.abs(kf - np.rint(kf)).max() < 1e-4 and np.abs(kt - np.rint(kt)).max() < 1e-4
+    assert np.abs(out[..., :3] - y[..., :3]).max() <= 0.5 * q_f * (1 + 1e-5)
+    assert np.abs(out[..., 3:] - y[..., 3:]).max() <= 0.5 * q_t * (1 + 1e-5)
+    assert len(np.unique(np.rint(kf))) > 3                                   # several levels are hit
+    # hand values, round half to even: 0.025 -> 0.02, 0.035 -> 0.04 (in fp32: 0.025f/0.01f = 2.5 exactly?  use bias to place y)
+    for b, want in ((0.0249, 0.02), (0.0251, 0.03), (-0.0151, -0.02)):
+        o2 = scene([one_patch()], 1, noise=dict(noise_enable=1, seed=1, hyst_mode="off", bias_force=b, quant_force=0.01))
+        r = o2.step(inputs(link_pos=(0, 0, -0.5)))["ft_noisy"][0, 0, 0]
+        assert r == pytest.approx(want, abs=1e-7)
+    # the comparator aid reports the distance to the nearest rounding boundary
+    assert "aux_quant" in yq and np.isfinite(yq["aux_quant"]).all() and (yq["aux_quant"] >= 0).all()
+    assert yq["aux_quant"][..., :3].max() <= 0.5 * q_f * (1 + 1e-5)
+
+
+def test_gain_eq27():
+    # gamma_bj ~ U[0.8, 1.2] once per episode: ft_noisy = gamma ft exactly, the same every step, new after reset
+    o, x = _contact_scene(dict(gain_min=0.8, gain_max=1.2))
+    a, b = o.step(x), o.step(x)
+    touch = np.abs(a["ft"][..., 2]) > 1e-3
+    g1 = a["ft_noisy"][..., 2][touch] / a["ft"][..., 2][touch]
+    g2 = b["ft_noisy"][..., 2][touch] / b["ft"][..., 2][touch]
+    assert g1.min() >= 0.8 and g1.max() <= 1.2 and g1.max() - g1.min() > 0.3
+    np.testing.assert_allclose(g1, g2, rtol=1e-12)
+    assert abs(g1.mean() - 1.0) < 4 * (0.4 / math.sqrt(12)) / math.sqrt(g1.size)
+    assert abs(g1.std() / (0.4 / math.sqrt(12)) - 1) < 0.1                   # uniform, not Gaussian: sd = width / sqrt(12)
+    # all six channels of a taxel share the gain
+    gx = a["ft_noisy"][..., 4][touch] / a["ft"][..., 4][touch]
+    np.testing.assert_allclose(gx, g1, rtol=1e-9)
+    o.reset()
+    g3 = o.step(x)
+    g3 = g3["ft_noisy"][..., 2][touch] / g3["ft"][..., 2][touch]
+    assert np.abs(g3 - g1).max() > 0.1
+    # gain enters BEFORE the hysteresis (R1): with ASYM loading from rest, y_1 = alpha_load * gamma * x
+    o2, _ = _contact_scene(dict(gain_min=0.8, gain_max=1.2, hyst_mode="asym", alpha_load=0.8, alpha_unload=0.5))
+    r = o2.step(x)
+    np.testing.assert_allclose(r["ft_noisy"][..., 2][touch] / r["ft"][..., 2][touch], float(np.float32(0.8)) * g1, rtol=1e-6)
+
+
+def test_stuck_value_eq28():
+    # dead taxels read z_bj ~ U[l, u] for the whole episode; l = u = 0 is D5
+    nz = dict(p_dead=0.2, stuck_min_force=0.5, stuck_max_force=1.5, stuck_min_torque=-0.02, stuck_max_torque=-0.01,
+              sigma_rw_force=1e-3, sigma_rw_torque=1e-5)
+    o, x = _contact_scene(nz)
+    a, b = o.step(x), o.step(x)
+    dead = a["dead"].astype(bool)
+    assert 0.15 < dead.mean() < 0.25
+    za = a["ft_noisy"][dead]
+    assert za[:, :3].min() >= 0.5 and za[:, :3].max() <= 1.5 and za[:, 3:].min() >= -0.02 and za[:, 3:].max() <= -0.01
+    np.testing.assert_array_equal(za, b["ft_noisy"][dead])                   # stuck: identical every step
+    assert abs(za[:, :3].mean() - 1.0) < 0.05 and za[:, 0].std() > 0.2       # spread over the interval
+    assert np.abs(np.corrcoef(za[:, 0], za[:, 1])[0, 1]) < 0.1               # channels drawn independently
+    assert (a["ft_noisy"][~dead] != b["ft_noisy"][~dead]).any()              # live taxels keep drifting
+    o.reset()
+    c = o.step(x)
+    d2 = c["dead"].astype(bool)
+    both = dead & d2
+    assert both.any() and (c["ft_noisy"][both] != a["ft_noisy"][both]).any()  # re-drawn at reset
+
+
 # ------------------------------------------------------------------ P8, P17 whole path
 def test_no_contact_and_fillers():
     w = W.config(2, n_envs=4)
