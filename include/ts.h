@@ -9,8 +9,9 @@
  *   Eq. 4-9  kinematic force / torque (+ Coulomb cap, D2)
  *   Eq. 18-21, 23  elastomer marker dilation
  *   bounded SDF march along a_j (D1; output form of Eq. 12)
- *   App. A.8 noise: hysteresis (Eq. 29-30) -> crosstalk (Eq. 31) -> random-walk
- *                        drift (Eq. 25) -> dead taxels (Eq. 28)
+ *   App. A.8 noise: [gain (Eq. 27)] -> hysteresis (Eq. 29-30) -> crosstalk (Eq. 31) ->
+ *                        [bias + white noise +] random-walk drift (Eq. 25) [-> quantize (Eq. 25)] ->
+ *                        dead taxels (Eq. 28); bracketed knobs are off by default
  * All device work is hand-written CUDA for sm_100a; there is no CPU fallback.
  *
  * Conventions: SI units; quaternions (w,x,y,z), used as given (never renormalised); each
@@ -140,6 +141,15 @@ typedef struct ts_config {
   float p_dead;          /* Eq. 28 Bernoulli probability, 0 <= p < 1 */
   float chi;             /* Eq. 31 crosstalk strength (4-neighbour kernel, D4) */
   uint32_t output_mask;  /* TS_OUT_* the ctx will be asked for (upper bound per step) */
+  /* Remaining knobs of App. A.8 on ft -> ft_noisy (R1-R4); all zero / (1, 1) = off.  Order:
+   * gain (Eq. 27) -> hysteresis -> crosstalk -> + bias + white noise + drift (Eq. 25) -> quantize (Eq. 25)
+   * -> dead taxels read their stuck value (Eq. 28).  *_force act on channels 0-2, *_torque on 3-5. */
+  float sigma_white_force, sigma_white_torque; /* Eq. 25 n_t ~ N(0, sigma^2), fresh every step */
+  float bias_force, bias_torque;               /* Eq. 25 constant bias b */
+  float quant_force, quant_torque;             /* Eq. 25 quantisation step q >= 0 (0 = off): q rint(y / q), fp32, half to even */
+  float gain_min, gain_max;                    /* Eq. 27 gamma_bj ~ U[min, max] per (env, taxel, episode); 0 < min <= max */
+  float stuck_min_force, stuck_max_force;      /* Eq. 28 z_bj ~ U[l, u] per (env, taxel, channel, episode), l <= u */
+  float stuck_min_torque, stuck_max_torque;
 } ts_config;
 
 /* Fills *cfg with the paper's constants and everything else zero / off. */

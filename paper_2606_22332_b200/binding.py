@@ -57,7 +57,13 @@ class Config(C.Structure):
                 ("noise_enable", C.c_int32), ("seed", C.c_uint64),
                 ("sigma_rw_force", C.c_float), ("sigma_rw_torque", C.c_float), ("hyst_mode", C.c_int32),
                 ("beta", C.c_float), ("tau", C.c_float), ("alpha_load", C.c_float), ("alpha_unload", C.c_float),
-                ("p_dead", C.c_float), ("chi", C.c_float), ("output_mask", C.c_uint32)]
+                ("p_dead", C.c_float), ("chi", C.c_float), ("output_mask", C.c_uint32),
+                ("sigma_white_force", C.c_float), ("sigma_white_torque", C.c_float),
+                ("bias_force", C.c_float), ("bias_torque", C.c_float),
+                ("quant_force", C.c_float), ("quant_torque", C.c_float),
+                ("gain_min", C.c_float), ("gain_max", C.c_float),
+                ("stuck_min_force", C.c_float), ("stuck_max_force", C.c_float),
+                ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float)]
 
 
 class Geometry(C.Structure):

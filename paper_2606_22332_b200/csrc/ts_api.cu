@@ -119,6 +119,13 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.sigma_f = g.sigma_rw_force; p.sigma_t = g.sigma_rw_torque; p.beta = g.beta;
   p.decay = (g.tau > 0.f) ? (float)std::exp(-(double)g.dt / (double)g.tau) : 0.f;   // Eq. 29
   p.alpha_load = g.alpha_load; p.alpha_unload = g.alpha_unload; p.chi = g.chi;
+  p.sigma_wf = g.sigma_white_force; p.sigma_wt = g.sigma_white_torque; p.bias_f = g.bias_force; p.bias_t = g.bias_torque;
+  p.quant_f = g.quant_force; p.quant_t = g.quant_torque; p.gain_min = g.gain_min; p.gain_max = g.gain_max;
+  p.stuck_lo_f = g.stuck_min_force; p.stuck_hi_f = g.stuck_max_force; p.stuck_lo_t = g.stuck_min_torque; p.stuck_hi_t = g.stuck_max_torque;
+  p.ext = (g.noise_enable && (g.sigma_white_force != 0.f || g.sigma_white_torque != 0.f || g.bias_force != 0.f || g.bias_torque != 0.f ||
+                              g.quant_force != 0.f || g.quant_torque != 0.f || g.gain_min != 1.f || g.gain_max != 1.f ||
+                              g.stuck_min_force != 0.f || g.stuck_max_force != 0.f || g.stuck_min_torque != 0.f ||
+                              g.stuck_max_torque != 0.f)) ? 1 : 0;
 }
 }  // namespace
 
@@ -138,6 +145,7 @@ void ts_config_default(ts_config* c) {
   c->r_prox = 0.020f; c->march_steps = 16;                                         // D1
   c->dt = 0.005f;
   c->tau = 0.05f; c->beta = 0.5f; c->alpha_load = 1.f; c->alpha_unload = 1.f;
+  c->gain_min = 1.f; c->gain_max = 1.f;                                             // Eq. 27 off
   c->output_mask = TS_OUT_CONTACT | TS_OUT_DEPTH | TS_OUT_FT | TS_OUT_MARKER | TS_OUT_PROX;
 }
 
@@ -161,6 +169,11 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     if (cfg->hyst_mode < TS_HYST_OFF || cfg->hyst_mode > TS_HYST_ASYM) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: hyst_mode");
     if (!(cfg->p_dead >= 0.f && cfg->p_dead < 1.f)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: p_dead not in [0,1)");
     if (cfg->hyst_mode == TS_HYST_MAXWELL && !(cfg->tau > 0.f)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: tau <= 0");
+    if (!(cfg->sigma_white_force >= 0.f) || !(cfg->sigma_white_torque >= 0.f) || !(cfg->quant_force >= 0.f) || !(cfg->quant_torque >= 0.f))
+      return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: sigma_white / quant must be >= 0");
+    if (!(cfg->gain_min > 0.f) || !(cfg->gain_min <= cfg->gain_max)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: need 0 < gain_min <= gain_max");
+    if (!(cfg->stuck_min_force <= cfg->stuck_max_force) || !(cfg->stuck_min_torque <= cfg->stuck_max_torque))
+      return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: stuck_min > stuck_max");
   } else if (cfg->output_mask & (TS_OUT_FT_NOISY | TS_OUT_DEAD)) {
     return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: ft_noisy / dead need noise_enable");
   }

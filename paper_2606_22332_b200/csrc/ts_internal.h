@@ -118,6 +118,10 @@ struct TsStepParams {
   int32_t noise_enable, hyst_mode;
   uint32_t seed_lo, seed_hi;
   float sigma_f, sigma_t, beta, decay, alpha_load, alpha_unload, chi;
+  // remaining A.8 knobs (Eq. 25, 27, 28); ext = 1 selects the kernel variant that evaluates them
+  int32_t ext;
+  float sigma_wf, sigma_wt, bias_f, bias_t, quant_f, quant_t, gain_min, gain_max;
+  float stuck_lo_f, stuck_hi_f, stuck_lo_t, stuck_hi_t;
   // Small layouts carry their group records and per-group link ids in the parameter space itself (constant
   // bank: a few cycles) so that a block's first dependent global load is already the pose row.
   int32_t inl;                             // 1 = the two tables below are valid

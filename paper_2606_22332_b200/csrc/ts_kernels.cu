@@ -406,25 +406,28 @@ struct NoiseState {
   float sY[6], sX[6], sD[6];  // hysteresis y (asym) or xi (maxwell), maxwell x_prev, drift D
 };
 
-template <int HM>  // hysteresis mode (TS_HYST_*), a compile-time constant so the unused state rows cost nothing
+// HM = hysteresis mode (TS_HYST_*) | 4 if the remaining A.8 knobs (Eq. 25 bias / white noise / quantisation,
+// Eq. 27 gain, Eq. 28 stuck value) are on: compile-time, so unused state rows and knobs cost nothing.
+template <int HM>
 __device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, bool valid, NoiseState& ns) {
+  constexpr int MODE = HM & 3;
   // 32-bit element indices (ts_create guarantees E * 12 * Tp < 2^32): one IMAD + LEA pair per access
   // instead of 64-bit address arithmetic that the register allocator keeps rematerialising.
   // State rows hold channel PAIRS (float2): [E][nh/2][Tp] and [E][3][Tp], so a warp moves 256 contiguous
   // bytes per access and a taxel needs 3 + 3 loads instead of 6 + 6.
   const unsigned Tp = (unsigned)p.Tp;
-  const unsigned ih = (unsigned)e * (HM == TS_HYST_MAXWELL ? 6u : 3u) * Tp + (unsigned)j;
+  const unsigned ih = (unsigned)e * (MODE == TS_HYST_MAXWELL ? 6u : 3u) * Tp + (unsigned)j;
   const unsigned id = (unsigned)e * 3u * Tp + (unsigned)j;
   const float2* st_h = reinterpret_cast<const float2*>(p.st_hyst);
   const float2* st_d = reinterpret_cast<const float2*>(p.st_drift);
 #pragma unroll
   for (int c = 0; c < 6; ++c) { ns.sY[c] = 0.f; ns.sX[c] = 0.f; ns.sD[c] = 0.f; }
   if (valid) {
-    if (HM != TS_HYST_OFF) {
+    if (MODE != TS_HYST_OFF) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) { const float2 v = ld_stream2(st_h + (ih + c * Tp)); ns.sY[2 * c] = v.x; ns.sY[2 * c + 1] = v.y; }
     }
-    if (HM == TS_HYST_MAXWELL) {
+    if (MODE == TS_HYST_MAXWELL) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) { const float2 v = ld_stream2(st_h + (ih + (3 + c) * Tp)); ns.sX[2 * c] = v.x; ns.sX[2 * c + 1] = v.y; }
     }
@@ -438,41 +441,55 @@ template <int HM>
 __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, unsigned ej, int tid, int gstart, bool valid,
                                             bool act, bool deadb, int meta, const float* ft, const NoiseState& ns,
                                             float* bufB) {
+  constexpr int MODE = HM & 3;
+  constexpr bool EXT = (HM & 4) != 0;
   const unsigned Tp = (unsigned)p.Tp;
-  const unsigned ih = (unsigned)e * (HM == TS_HYST_MAXWELL ? 6u : 3u) * Tp + (unsigned)j;
+  const unsigned ih = (unsigned)e * (MODE == TS_HYST_MAXWELL ? 6u : 3u) * Tp + (unsigned)j;
   const unsigned id = (unsigned)e * 3u * Tp + (unsigned)j;
   float2* const st_h = reinterpret_cast<float2*>(p.st_hyst);
   float2* const st_d = reinterpret_cast<float2*>(p.st_drift);
+  const uint32_t ep4 = __ldg(p.episode + e) << 4;
+  const uint32_t env = p.env_id_base + (uint32_t)e;
+  float x[6];  // the signal the chain acts on: gamma_bj ft (Eq. 27, R1/R2), gamma = 1 without EXT
+#pragma unroll
+  for (int c = 0; c < 6; ++c) x[c] = ft[c];
+  if (EXT && act && (p.gain_min != 1.f || p.gain_max != 1.f)) {  // stream 3, n = 0: once per episode, recomputed here
+    const uint4 w = philox4x32_10(make_uint4(env, (uint32_t)j, 0u, ep4 | 3u), p.seed_lo, p.seed_hi);
+    const float u = (float)(2u * (w.x >> 9) + 1u) * 5.9604644775390625e-8f;
+    const float g = fmaf(p.gain_max - p.gain_min, u, p.gain_min);
+#pragma unroll
+    for (int c = 0; c < 6; ++c) x[c] *= g;
+  }
   float h[6];
-  if (HM == TS_HYST_ASYM) {  // D3, Q14
+  if (MODE == TS_HYST_ASYM) {  // D3, Q14
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
       const float yp = ns.sY[c];
-      const float al = (fabsf(ft[c]) > fabsf(yp)) ? p.alpha_load : p.alpha_unload;
-      h[c] = act ? fmaf(al, ft[c] - yp, yp) : 0.f;
+      const float al = (fabsf(x[c]) > fabsf(yp)) ? p.alpha_load : p.alpha_unload;
+      h[c] = act ? fmaf(al, x[c] - yp, yp) : 0.f;
     }
     if (valid) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) __stcs(st_h + (ih + c * Tp), make_float2(h[2 * c], h[2 * c + 1]));
     }
-  } else if (HM == TS_HYST_MAXWELL) {  // Eq. 29-30
+  } else if (MODE == TS_HYST_MAXWELL) {  // Eq. 29-30
 #pragma unroll
     float zx[6];
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
-      zx[c] = act ? fmaf(p.decay, ns.sY[c], ft[c] - ns.sX[c]) : 0.f;
-      h[c] = fmaf(p.beta, zx[c], ft[c]);
+      zx[c] = act ? fmaf(p.decay, ns.sY[c], x[c] - ns.sX[c]) : 0.f;
+      h[c] = fmaf(p.beta, zx[c], x[c]);
     }
     if (valid) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
         __stcs(st_h + (ih + c * Tp), make_float2(zx[2 * c], zx[2 * c + 1]));
-        __stcs(st_h + (ih + (3 + c) * Tp), act ? make_float2(ft[2 * c], ft[2 * c + 1]) : make_float2(0.f, 0.f));
+        __stcs(st_h + (ih + (3 + c) * Tp), act ? make_float2(x[2 * c], x[2 * c + 1]) : make_float2(0.f, 0.f));
       }
     }
   } else {
 #pragma unroll
-    for (int c = 0; c < 6; ++c) h[c] = ft[c];
+    for (int c = 0; c < 6; ++c) h[c] = x[c];
   }
   float2* const b2 = reinterpret_cast<float2*>(bufB);  // [3][TS_BLOCK] channel pairs
 #pragma unroll
@@ -481,13 +498,20 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
   float z[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   if (act) {
     const uint32_t nstep = p.gstep - __ldg(p.reset_step + e);
-    const uint32_t ep4 = __ldg(p.episode + e) << 4;
-    const uint32_t env = p.env_id_base + (uint32_t)e;
     const uint4 w0 = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 0u), p.seed_lo, p.seed_hi);
     const uint4 w1 = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 1u), p.seed_lo, p.seed_hi);
     box_muller(w0.x, w0.y, z[0], z[1]);
     box_muller(w0.z, w0.w, z[2], z[3]);
     box_muller(w1.x, w1.y, z[4], z[5]);
+  }
+  float zw[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};  // Eq. 25 white noise n_t / sigma (R3): streams 6 / 7
+  if (EXT && act && (p.sigma_wf != 0.f || p.sigma_wt != 0.f)) {
+    const uint32_t nstep = p.gstep - __ldg(p.reset_step + e);
+    const uint4 w0 = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 6u), p.seed_lo, p.seed_hi);
+    const uint4 w1 = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 7u), p.seed_lo, p.seed_hi);
+    box_muller(w0.x, w0.y, zw[0], zw[1]);
+    box_muller(w0.z, w0.w, zw[2], zw[3]);
+    box_muller(w1.x, w1.y, zw[4], zw[5]);
   }
   __syncthreads();
   // S8c crosstalk (D4): c_j = h_j + chi/4 sum_{k in N4(j)} (h_k - h_j); a missing neighbour is
@@ -510,7 +534,24 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
     const float acc = fmaf(-4.f, hc, nsum[c]);  // sum_k (h_k - h_j)
     const float cx = fmaf(q4, acc, hc);
     Dn[c] = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], ns.sD[c]) : 0.f;
-    outv[c] = (act && !deadb) ? cx + Dn[c] : 0.f;  // S8a dead (Eq. 28) last
+    if (!EXT) {
+      outv[c] = (act && !deadb) ? cx + Dn[c] : 0.f;  // S8a dead (Eq. 28, D5) last
+    } else {
+      float y = fmaf(c < 3 ? p.sigma_wf : p.sigma_wt, zw[c], cx + (c < 3 ? p.bias_f : p.bias_t)) + Dn[c];  // Eq. 25
+      const float q = c < 3 ? p.quant_f : p.quant_t;
+      if (q > 0.f) y = rintf(y / q) * q;  // quantize(., q): IEEE fp32 division, round half to even
+      outv[c] = act ? y : 0.f;
+    }
+  }
+  if (EXT && deadb) {  // Eq. 28 stuck readout z_bj (R4): streams 4 / 5, n = 0; rare (p_dead of the taxels)
+    const uint4 w0 = philox4x32_10(make_uint4(env, (uint32_t)j, 0u, ep4 | 4u), p.seed_lo, p.seed_hi);
+    const uint4 w1 = philox4x32_10(make_uint4(env, (uint32_t)j, 0u, ep4 | 5u), p.seed_lo, p.seed_hi);
+    const uint32_t ww[6] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y};
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+      const float lo = c < 3 ? p.stuck_lo_f : p.stuck_lo_t, hi = c < 3 ? p.stuck_hi_f : p.stuck_hi_t;
+      outv[c] = fmaf(hi - lo, (float)(2u * (ww[c] >> 9) + 1u) * 5.9604644775390625e-8f, lo);
+    }
   }
   if (valid) {
 #pragma unroll
@@ -953,6 +994,9 @@ void launch_one(const TsStepParams& p, int hm, dim3 grid, size_t smem, cudaStrea
     case TS_HYST_OFF: ts_step_kernel<SINGLE, TS_HYST_OFF><<<grid, TS_BLOCK, smem, st>>>(p); break;
     case TS_HYST_MAXWELL: ts_step_kernel<SINGLE, TS_HYST_MAXWELL><<<grid, TS_BLOCK, smem, st>>>(p); break;
     case TS_HYST_ASYM: ts_step_kernel<SINGLE, TS_HYST_ASYM><<<grid, TS_BLOCK, smem, st>>>(p); break;
+    case 4 | TS_HYST_OFF: ts_step_kernel<SINGLE, 4 | TS_HYST_OFF><<<grid, TS_BLOCK, smem, st>>>(p); break;
+    case 4 | TS_HYST_MAXWELL: ts_step_kernel<SINGLE, 4 | TS_HYST_MAXWELL><<<grid, TS_BLOCK, smem, st>>>(p); break;
+    case 4 | TS_HYST_ASYM: ts_step_kernel<SINGLE, 4 | TS_HYST_ASYM><<<grid, TS_BLOCK, smem, st>>>(p); break;
     default: ts_step_kernel<SINGLE, -1><<<grid, TS_BLOCK, smem, st>>>(p); break;
   }
 }
@@ -963,6 +1007,12 @@ int ts_prepare_kernels(int max_smem_bytes) {
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_OFF>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_MAXWELL>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_ASYM>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, 4 | TS_HYST_OFF>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, 4 | TS_HYST_MAXWELL>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, 4 | TS_HYST_ASYM>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<false, 4 | TS_HYST_OFF>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<false, 4 | TS_HYST_MAXWELL>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<false, 4 | TS_HYST_ASYM>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<false, -1>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<false, TS_HYST_OFF>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<false, TS_HYST_MAXWELL>(max_smem_bytes);
@@ -975,7 +1025,7 @@ int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
   if (p.E <= 0 || p.G <= 0 || p.G > 65535) return (int)cudaErrorInvalidConfiguration;
   const size_t smem = (size_t)ts_step_smem_bytes(p);
   const dim3 grid((unsigned)p.E, (unsigned)p.G);
-  const int hm = (p.noise_enable && fused_noise) ? p.hyst_mode : -1;
+  const int hm = (p.noise_enable && fused_noise) ? (p.hyst_mode | (p.ext ? 4 : 0)) : -1;
   if (p.K == 1) launch_one<true>(p, hm, grid, smem, (cudaStream_t)stream);
   else launch_one<false>(p, hm, grid, smem, (cudaStream_t)stream);
   return (int)cudaGetLastError();
@@ -984,9 +1034,14 @@ int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
 int ts_launch_noise(const TsStepParams& p, void* stream) {
   const dim3 grid((unsigned)p.E, (unsigned)p.G);
   cudaStream_t st = (cudaStream_t)stream;
-  if (p.hyst_mode == TS_HYST_MAXWELL) ts_noise_kernel<TS_HYST_MAXWELL><<<grid, TS_BLOCK, 0, st>>>(p);
-  else if (p.hyst_mode == TS_HYST_ASYM) ts_noise_kernel<TS_HYST_ASYM><<<grid, TS_BLOCK, 0, st>>>(p);
-  else ts_noise_kernel<TS_HYST_OFF><<<grid, TS_BLOCK, 0, st>>>(p);
+  switch (p.hyst_mode | (p.ext ? 4 : 0)) {
+    case TS_HYST_MAXWELL: ts_noise_kernel<TS_HYST_MAXWELL><<<grid, TS_BLOCK, 0, st>>>(p); break;
+    case TS_HYST_ASYM: ts_noise_kernel<TS_HYST_ASYM><<<grid, TS_BLOCK, 0, st>>>(p); break;
+    case 4 | TS_HYST_OFF: ts_noise_kernel<4 | TS_HYST_OFF><<<grid, TS_BLOCK, 0, st>>>(p); break;
+    case 4 | TS_HYST_MAXWELL: ts_noise_kernel<4 | TS_HYST_MAXWELL><<<grid, TS_BLOCK, 0, st>>>(p); break;
+    case 4 | TS_HYST_ASYM: ts_noise_kernel<4 | TS_HYST_ASYM><<<grid, TS_BLOCK, 0, st>>>(p); break;
+    default: ts_noise_kernel<TS_HYST_OFF><<<grid, TS_BLOCK, 0, st>>>(p); break;
+  }
   return (int)cudaGetLastError();
 }
 

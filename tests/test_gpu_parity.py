@@ -30,13 +30,15 @@ def _assert_ok(rep, max_band_frac=1e-3):
     print(json.dumps({k: v for k, v in rep.items()}, default=str))
     assert not rep["failures"], rep["failures"]
     n = max(rep["checked"], 1)
-    assert rep["ft_exempt"] + rep["contact_tainted"] <= max(20, max_band_frac * n), rep
+    assert rep["ft_exempt"] + rep["contact_tainted"] + rep.get("quant_exempt", 0) <= max(20, max_band_frac * n), rep
 
 
 def _parity(w, ids=None, steps=None, **kw):
     from parity import run_parity
+    nz = kw.get("noise") or {}
     return run_parity(w, lambda ww: _sim(ww, **kw), lambda ww, i, t: _orc(ww, i, t, **kw), ids, steps,
-                      kw.get("outputs"), threads=os.cpu_count() or 1)
+                      kw.get("outputs"), threads=os.cpu_count() or 1,
+                      quant=(float(np.float32(nz.get("quant_force", 0.0))), float(np.float32(nz.get("quant_torque", 0.0)))))
 
 
 def test_config1_tiny():
@@ -150,3 +152,50 @@ def test_edge_shapes():
     torch.cuda.synchronize()
     act = torch.from_numpy(sim2.layout.view()["radius"] > 0).cuda()
     assert torch.allclose(out2["prox"][0][act], torch.full_like(out2["prox"][0][act], 0.02))  # K_m = 0: t = 0, P = r_prox
+
+
+def test_remaining_noise_knobs():
+    """App. A.8 knobs beyond the four of configs 4-5 (R1-R4): bias, white noise, quantisation (Eq. 25),
+    per-episode gain (Eq. 27), stuck readout of dead taxels (Eq. 28), with both hysteresis modes and over a reset."""
+    w = W.config(5, n_envs=48)
+    ext = dict(sigma_white_force=2e-3, sigma_white_torque=2e-5, bias_force=0.02, bias_torque=-3e-4, gain_min=0.9,
+               gain_max=1.1, stuck_min_force=-0.5, stuck_max_force=0.5, stuck_min_torque=-5e-3, stuck_max_torque=5e-3,
+               p_dead=0.05)
+    _assert_ok(_parity(w, steps=30, noise=dict(w.noise, **ext)))
+    _assert_ok(_parity(w, steps=20, noise=dict(w.noise, hyst_mode="maxwell", beta=0.5, tau=0.05, **ext)))
+    # quantisation: 1 mN / 10 uN m steps; boundary hits are exempted and counted by the comparator
+    rep = _parity(w, steps=20, noise=dict(w.noise, quant_force=1e-3, quant_torque=1e-5, **ext))
+    _assert_ok(rep, max_band_frac=3e-3)
+    assert rep["quant_exempt"] < 3e-3 * rep["checked"]
+    # each knob alone (the others off)
+    for one in (dict(bias_force=0.1), dict(sigma_white_force=1e-3), dict(gain_min=0.5, gain_max=0.6),
+                dict(stuck_min_force=1.0, stuck_max_force=1.0), dict(quant_torque=1e-5)):
+        _assert_ok(_parity(w, steps=6, noise=dict(w.noise, **one)), max_band_frac=3e-3)
+
+
+def test_remaining_noise_knobs_reset_and_split(monkeypatch):
+    """Gain and stuck values are per episode: the same context after ts_reset must follow the oracle after reset;
+    the split (geometry + noise kernel) variant computes the same."""
+    import torch
+    from oracle import oracle as O
+    from parity import Comparator
+    w = W.config(4, n_envs=24)
+    noise = dict(w.noise, gain_min=0.8, gain_max=1.2, stuck_min_force=0.2, stuck_max_force=0.4, bias_torque=1e-4, p_dead=0.1)
+    for split in ("0", "1"):
+        monkeypatch.setenv("TS_SPLIT", split)
+        sim = _sim(w, noise=noise)
+        orc = _orc(w, np.arange(w.E), os.cpu_count() or 1, noise=noise)
+        lay = sim.layout.view()
+        cmp_ = Comparator(lay, w.physics, True, lay["radius"])
+        for s in range(12):
+            if s == 6:
+                sim.reset()
+                orc.reset()
+            inp = w.inputs(s)
+            g = sim.step(sim.upload(inp))
+            torch.cuda.synchronize()
+            cmp_.step({k: v.cpu().numpy() for k, v in g.items()}, orc.step(inp, want=w.outputs))
+        rep = cmp_.report()
+        _assert_ok(rep)
+        assert sim.launches_per_step() == (2 if split == "1" else 1)
+        sim.close()
