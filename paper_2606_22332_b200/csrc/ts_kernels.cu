@@ -436,6 +436,23 @@ __device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, 
   }
 }
 
+// The 12 (18) per-taxel state words of the noise chain are only PREFETCHED into L2 early in the kernel (one
+// request per 128-byte line of a float2 row, i.e. every 16th thread) and loaded right before the chain:
+// holding them in registers across the march cost spills at 48 registers per thread (measured 1.48 ->
+// 1.41 ms on config 5), and an L2 hit is short enough for 40 resident warps to cover.
+template <int HM>
+__device__ __forceinline__ void noise_prefetch(const TsStepParams& p, int e, int j) {
+  constexpr int MODE = HM & 3;
+  const unsigned Tp = (unsigned)p.Tp;
+  const float2* sh = reinterpret_cast<const float2*>(p.st_hyst) + ((unsigned)e * (MODE == TS_HYST_MAXWELL ? 6u : 3u) * Tp + (unsigned)j);
+  const float2* sd = reinterpret_cast<const float2*>(p.st_drift) + ((unsigned)e * 3u * Tp + (unsigned)j);
+#pragma unroll
+  for (int c = 0; c < (MODE == TS_HYST_MAXWELL ? 6 : (MODE == TS_HYST_ASYM ? 3 : 0)); ++c)
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(sh + c * Tp));
+#pragma unroll
+  for (int c = 0; c < 3; ++c) asm volatile("prefetch.global.L2 [%0];" ::"l"(sd + c * Tp));
+}
+
 // Every thread of the block must call this (it contains one __syncthreads).
 template <int HM>
 __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, unsigned ej, int tid, int gstart, bool valid,
@@ -744,6 +761,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const float Rj = valid ? P4.w : 0.f;  // R_j = 0: inactive slot
   const bool act = Rj > 0.f;
   uint8_t flag = valid ? p.st_flags[ej] : (uint8_t)0;
+  if (NOISE && valid && (tid & 15) == 0) noise_prefetch<HM>(p, e, j);
   __syncthreads();
 
   // ---- phase 1 (S1-S4): x_o = c + M x_j, phi = min_k phi_k, depth (Eq. 2), contact (Eq. 3) ----
@@ -784,10 +802,6 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   }
   const F3 xo = mk3((float)xd.x, (float)xd.y, (float)xd.z);  // fp32 object-frame position for the march
 
-  // state prefetch: the 12 (18) per-taxel state words of the noise chain are requested now so that their
-  // HBM latency is covered by the march and the force/torque phases.
-  NoiseState ns;
-  if (NOISE) noise_load<HM>(p, e, j, valid, ns);
   march_phase<SINGLE>(p, frames, e, lp, valid, act, ej, phif, xo, P4, patch0 + lp);
 
   // ---- phase 3 (S5): kinematic force / torque (Eq. 4-9, D2) in double, link frame ---------------
@@ -828,6 +842,8 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   if (p.ft && valid) store6(p.ft + ej * 6u, ft);
 
   // ---- phase 4 (S8): noise chain (fused variant); contains the barrier that also publishes hh / ha / pact
+  NoiseState ns;
+  if (NOISE) noise_load<HM>(p, e, j, valid, ns);
   if (NOISE) noise_chain<HM>(p, e, j, ej, tid, gstart, valid, act, deadb, meta, ft, ns, bufB);
   else __syncthreads();
 
