@@ -38,7 +38,8 @@ def test_struct_sizes_match_header(B):
     assert (cfg.k_n, cfg.c_n, cfg.k_t, cfg.k_omega) == (500.0, 1.0, 2.0, 2.0)          # Eq. 10
     assert cfg.alpha == pytest.approx(1.2) and cfg.eta_on == pytest.approx(5e-4)
     assert (cfg.s_d, cfg.lambda_d) == (100.0, 8000.0) and cfg.march_steps == 16
-    assert cfg.chi == 0.0 and cfg.output_mask == 31                                      # last field lands right
+    assert cfg.chi == 0.0 and cfg.output_mask == 31
+    assert (cfg.gain_min, cfg.gain_max) == (1.0, 1.0) and cfg.stuck_max_torque == 0.0    # last field lands right
 
 
 @pytest.mark.parametrize("cid", [1, 2, 3, 4])
@@ -80,7 +81,10 @@ def test_create_rejects_bad_config_before_touching_cuda(B):
     lay = B.Layout(W.config(1).patches, 200)
     h = C.c_void_p()
     for bad in (dict(physics=dict(eta_off=6e-4)), dict(physics=dict(march_steps=65)), dict(n_links=3),
-                dict(noise=dict(noise_enable=1, p_dead=1.0)), dict(outputs=["ft_noisy"])):
+                dict(noise=dict(noise_enable=1, p_dead=1.0)), dict(outputs=["ft_noisy"]),
+                dict(noise=dict(noise_enable=1, gain_min=0.0)), dict(noise=dict(noise_enable=1, gain_min=1.2, gain_max=1.1)),
+                dict(noise=dict(noise_enable=1, quant_force=-1e-3)), dict(noise=dict(noise_enable=1, sigma_white_torque=-1.0)),
+                dict(noise=dict(noise_enable=1, stuck_min_force=1.0, stuck_max_force=0.5))):
         kw = dict(n_envs=4, n_links=16, objs_per_env=1, layout=lay)
         kw.update(bad)
         cfg = B.make_config(**kw)
