@@ -255,6 +255,7 @@ typedef struct orc_params {
   float quant_force, quant_torque;              // Eq. 25 quantisation step q (0 = off)
   float gain_min, gain_max;                     // Eq. 27 per-reset gain gamma_bj ~ U[min, max] (1, 1 = off)
   float stuck_min_force, stuck_max_force, stuck_min_torque, stuck_max_torque;  // Eq. 28 stuck readout z_bj ~ U[l, u]
+  float xtalk_sigma;  // Eq. 11 / 31: 0 = 4-neighbour stencil (D4); > 0 = Gaussian G_sigma, sigma in taxel pitches (R7)
 } orc_params;
 }
 
@@ -671,12 +672,36 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
           if (o.aux_quant) o.aux_quant[ej * 6 + c] = INFINITY;
           if (active) {
             double hj = hcl[(size_t)j * 6 + c];
-            double acc = 0.0;                                             // D4, Q11
-            for (int a = 0; a < 4; ++a) {
-              int k = o.nbr[(size_t)j * 4 + a];
-              if (k >= 0 && o.radius[k] > 0.0) acc += hcl[(size_t)k * 6 + c] - hj;
+            double cj;
+            if (pr.xtalk_sigma > 0.0f) {
+              // Eq. 11 / 31 (R7): z~ = (1 - chi) z + chi (G_sigma * z) on the patch grid.  G_sigma[du, dv] =
+              // g[du] g[dv], g[d] = exp(-d^2 / (2 sigma^2)) for |d| <= r = ceil(3 sigma), L1-normalised over
+              // its full support; plain convolution, zero outside the patch (inactive sources count as 0).
+              const double sg = (double)pr.xtalk_sigma;
+              const int r = (int)std::ceil(3.0 * sg);
+              double norm = 0.0;
+              for (int d = -r; d <= r; ++d) norm += std::exp(-(double)(d * d) / (2.0 * sg * sg));
+              const int pj = o.patch[j], nu = o.p_nu[pj], nv = o.p_nv[pj], u0 = o.iu[j], v0 = o.iv[j];
+              double conv = 0.0;
+              for (int dv = -r; dv <= r; ++dv)
+                for (int du = -r; du <= r; ++du) {
+                  const int u = u0 + du, v = v0 + dv;
+                  if (u < 0 || u >= nu || v < 0 || v >= nv) continue;
+                  const int k = o.p_start[pj] + v * nu + u;
+                  if (!(o.radius[k] > 0.0)) continue;
+                  const double w = std::exp(-(double)(du * du) / (2.0 * sg * sg)) / norm *
+                                   (std::exp(-(double)(dv * dv) / (2.0 * sg * sg)) / norm);
+                  conv += w * hcl[(size_t)k * 6 + c];
+                }
+              cj = (1.0 - (double)pr.chi) * hj + (double)pr.chi * conv;
+            } else {
+              double acc = 0.0;                                           // D4, Q11
+              for (int a = 0; a < 4; ++a) {
+                int k = o.nbr[(size_t)j * 4 + a];
+                if (k >= 0 && o.radius[k] > 0.0) acc += hcl[(size_t)k * 6 + c] - hj;
+              }
+              cj = hj + ((double)pr.chi / 4.0) * acc;
             }
-            double cj = hj + ((double)pr.chi / 4.0) * acc;
             double sig = (c < 3) ? (double)pr.sigma_rw_force : (double)pr.sigma_rw_torque;
             double D = o.drift[ej * 6 + c] + sig * z[c];                  // Eq. 25 drift
             o.drift[ej * 6 + c] = D;

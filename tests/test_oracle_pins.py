@@ -653,6 +653,42 @@ def test_stuck_value_eq28():
     assert both.any() and (c["ft_noisy"][both] != a["ft_noisy"][both]).any()  # re-drawn at reset
 
 
+def test_gaussian_crosstalk_eq11_vs_scipy():
+    # Eq. 11 / 31 (R7): z~ = (1 - chi) z + chi (G_sigma * z); pinned against scipy's zero-padded 2-D convolution of the
+    # oracle's own clean ft field with an L1-normalised separable Gaussian (a library routine, not the oracle's loop)
+    from scipy.signal import convolve2d
+    for nu, nv, sigma, chi in ((8, 8, 0.8, 0.3), (6, 8, 1.2, 0.05), (5, 8, 0.5, 1.0)):
+        o, x = _contact_scene(dict(chi=chi, xtalk_sigma=sigma), E=2, nu=nu, nv=nv)
+        out = o.step(x)
+        ft, got = out["ft"], out["ft_noisy"]
+        assert (np.abs(ft[..., 2]) > 1e-3).sum() > 4 and (ft[..., 2] == 0).sum() > 4      # a real, non-constant field
+        r = int(math.ceil(3 * np.float32(sigma)))
+        g = np.exp(-np.arange(-r, r + 1) ** 2 / (2.0 * float(np.float32(sigma)) ** 2))
+        g /= g.sum()
+        G = np.outer(g, g)
+        assert abs(G.sum() - 1) < 1e-12
+        for e in range(2):
+            for c in range(6):
+                z = ft[e, :, c].reshape(nv, nu)                                        # u fastest
+                want = (1 - float(np.float32(chi))) * z + float(np.float32(chi)) * convolve2d(z, G, mode="same", boundary="fill")
+                np.testing.assert_allclose(got[e, :, c].reshape(nv, nu), want, rtol=2e-6, atol=1e-9)
+    # sigma -> 0: the kernel collapses to the identity (r = 1, g[+-1] = exp(-50))
+    o, x = _contact_scene(dict(chi=0.5, xtalk_sigma=0.1), E=1)
+    out = o.step(x)
+    np.testing.assert_allclose(out["ft_noisy"], out["ft"], rtol=1e-6, atol=1e-12)
+    # interior impulse: a single loaded taxel spreads as chi * G around it and keeps (1 - chi) + chi G[0,0] itself
+    o = scene([one_patch(8, 8, 0.0008, 0.0008, radius=1e-4)], 64, noise=dict(noise_enable=1, seed=3, hyst_mode="off", chi=0.4, xtalk_sigma=0.7))
+    # tiny patch (0.1 mm pitch) under a box face: uniform depth -> constant field; interior taxels stay fixed
+    o.set_geometry(np.full((1, 1), O.GEOM["box"], np.int32), np.array([[[0.05, 0.05, 0.05, 0]]], np.float32))
+    out = o.step(inputs(link_pos=(0, 0, -0.05005)))
+    f = out["ft"][0, :, 2].reshape(8, 8)
+    assert np.ptp(f) < 1e-9 * abs(f).max() and abs(f).max() > 0
+    n = out["ft_noisy"][0, :, 2].reshape(8, 8)
+    rr = int(math.ceil(3 * 0.7))
+    np.testing.assert_allclose(n[rr:-rr, rr:-rr], f[rr:-rr, rr:-rr], rtol=1e-6)     # constants are a fixed point away from the border
+    assert abs(n[0, 0]) < abs(f[0, 0])                                             # zero padding loses mass at the border
+
+
 # ------------------------------------------------------------------ P8, P17 whole path
 def test_no_contact_and_fillers():
     w = W.config(2, n_envs=4)
