@@ -150,6 +150,10 @@ typedef struct ts_config {
   float gain_min, gain_max;                    /* Eq. 27 gamma_bj ~ U[min, max] per (env, taxel, episode); 0 < min <= max */
   float stuck_min_force, stuck_max_force;      /* Eq. 28 z_bj ~ U[l, u] per (env, taxel, channel, episode), l <= u */
   float stuck_min_torque, stuck_max_torque;
+  /* Eq. 11 / 31 crosstalk kernel: 0 = the 4-neighbour stencil (D4); > 0 = Gaussian G_sigma with sigma in
+   * taxel pitches: separable, g[d] = exp(-d^2 / (2 sigma^2)) for |d| <= ceil(3 sigma), L1-normalised, plain
+   * convolution with zeros outside the patch (R7).  sigma <= 4/3 (radius <= 4). */
+  float xtalk_sigma;
 } ts_config;
 
 /* Fills *cfg with the paper's constants and everything else zero / off. */

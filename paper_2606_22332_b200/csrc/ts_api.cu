@@ -122,7 +122,17 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.sigma_wf = g.sigma_white_force; p.sigma_wt = g.sigma_white_torque; p.bias_f = g.bias_force; p.bias_t = g.bias_torque;
   p.quant_f = g.quant_force; p.quant_t = g.quant_torque; p.gain_min = g.gain_min; p.gain_max = g.gain_max;
   p.stuck_lo_f = g.stuck_min_force; p.stuck_hi_f = g.stuck_max_force; p.stuck_lo_t = g.stuck_min_torque; p.stuck_hi_t = g.stuck_max_torque;
-  p.ext = (g.noise_enable && (g.sigma_white_force != 0.f || g.sigma_white_torque != 0.f || g.bias_force != 0.f || g.bias_torque != 0.f ||
+  p.xt_r = 0;
+  for (int d = 0; d < 5; ++d) p.xt_w[d] = 0.f;
+  if (g.noise_enable && g.xtalk_sigma > 0.f) {  // Eq. 11 / 31, R7: separable L1-normalised Gaussian taps
+    const double sg = (double)g.xtalk_sigma;
+    const int r = (int)std::ceil(3.0 * sg);
+    double norm = 0.0;
+    for (int d = -r; d <= r; ++d) norm += std::exp(-(double)(d * d) / (2.0 * sg * sg));
+    p.xt_r = r;
+    for (int d = 0; d <= r && d < 5; ++d) p.xt_w[d] = (float)(std::exp(-(double)(d * d) / (2.0 * sg * sg)) / norm);
+  }
+  p.ext = (g.noise_enable && (g.xtalk_sigma != 0.f || g.sigma_white_force != 0.f || g.sigma_white_torque != 0.f || g.bias_force != 0.f || g.bias_torque != 0.f ||
                               g.quant_force != 0.f || g.quant_torque != 0.f || g.gain_min != 1.f || g.gain_max != 1.f ||
                               g.stuck_min_force != 0.f || g.stuck_max_force != 0.f || g.stuck_min_torque != 0.f ||
                               g.stuck_max_torque != 0.f)) ? 1 : 0;
@@ -171,6 +181,8 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     if (cfg->hyst_mode == TS_HYST_MAXWELL && !(cfg->tau > 0.f)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: tau <= 0");
     if (!(cfg->sigma_white_force >= 0.f) || !(cfg->sigma_white_torque >= 0.f) || !(cfg->quant_force >= 0.f) || !(cfg->quant_torque >= 0.f))
       return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: sigma_white / quant must be >= 0");
+    if (!(cfg->xtalk_sigma >= 0.f) || std::ceil(3.0 * (double)cfg->xtalk_sigma) > 4.0)
+      return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: xtalk_sigma not in [0, 4/3]");
     if (!(cfg->gain_min > 0.f) || !(cfg->gain_min <= cfg->gain_max)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: need 0 < gain_min <= gain_max");
     if (!(cfg->stuck_min_force <= cfg->stuck_max_force) || !(cfg->stuck_min_torque <= cfg->stuck_max_torque))
       return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: stuck_min > stuck_max");

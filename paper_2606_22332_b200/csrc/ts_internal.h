@@ -122,6 +122,8 @@ struct TsStepParams {
   int32_t ext;
   float sigma_wf, sigma_wt, bias_f, bias_t, quant_f, quant_t, gain_min, gain_max;
   float stuck_lo_f, stuck_hi_f, stuck_lo_t, stuck_hi_t;
+  int32_t xt_r;     // Gaussian crosstalk radius ceil(3 sigma) <= 4; 0 = 4-neighbour stencil
+  float xt_w[5];    // L1-normalised 1-D weights g[|d|], d = 0..xt_r
   // Small layouts carry their group records and per-group link ids in the parameter space itself (constant
   // bank: a few cycles) so that a block's first dependent global load is already the pose row.
   int32_t inl;                             // 1 = the two tables below are valid

@@ -455,7 +455,7 @@ __device__ __forceinline__ void noise_prefetch(const TsStepParams& p, int e, int
 
 // Every thread of the block must call this (it contains one __syncthreads).
 template <int HM>
-__device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, unsigned ej, int tid, int gstart, bool valid,
+__device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, unsigned ej, int tid, int patch0, bool valid,
                                             bool act, bool deadb, int meta, const float* ft, const NoiseState& ns,
                                             float* bufB) {
   constexpr int MODE = HM & 3;
@@ -545,11 +545,34 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
     nsum[2 * c] = (a0.x + a1.x) + (a2.x + a3.x);
     nsum[2 * c + 1] = (a0.y + a1.y) + (a2.y + a3.y);
   }
+  // Eq. 11 / 31 with the Gaussian kernel (R7): conv = sum_{du,dv} g[|du|] g[|dv|] h(iu+du, iv+dv), zero outside the
+  // patch; slots of a patch are consecutive (u fastest), inactive sources hold h = 0.
+  float conv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  const bool gauss = EXT && p.xt_r > 0;
+  if (gauss && act) {
+    const TsPatch& pt = p.patches[patch0 + (meta & 255)];
+    const int nv = __ldg(&pt.nv), il = j - __ldg(&pt.start), iv = il / nu, iu = il - iv * nu, r = p.xt_r;
+    for (int dv = -r; dv <= r; ++dv) {
+      if (iv + dv < 0 || iv + dv >= nv) continue;
+      const float wv = p.xt_w[dv < 0 ? -dv : dv];
+      for (int du = -r; du <= r; ++du) {
+        if (iu + du < 0 || iu + du >= nu) continue;
+        const float w = wv * p.xt_w[du < 0 ? -du : du];
+        const int k = tid + dv * nu + du;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const float2 a = b2[c * TS_BLOCK + k];
+          conv[2 * c] = fmaf(w, a.x, conv[2 * c]);
+          conv[2 * c + 1] = fmaf(w, a.y, conv[2 * c + 1]);
+        }
+      }
+    }
+  }
 #pragma unroll
   for (int c = 0; c < 6; ++c) {
     const float hc = h[c];
     const float acc = fmaf(-4.f, hc, nsum[c]);  // sum_k (h_k - h_j)
-    const float cx = fmaf(q4, acc, hc);
+    const float cx = gauss ? fmaf(p.chi, conv[c], (1.f - p.chi) * hc) : fmaf(q4, acc, hc);
     Dn[c] = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], ns.sD[c]) : 0.f;
     if (!EXT) {
       outv[c] = (act && !deadb) ? cx + Dn[c] : 0.f;  // S8a dead (Eq. 28, D5) last
@@ -599,7 +622,7 @@ __global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_cons
     act = __ldg(&p.tx_pos[j].w) > 0.f;
     deadb = act && ((p.st_flags[ej] >> 1) & 1);
   }
-  noise_chain<HM>(p, e, j, ej, tid, gstart, valid, act, deadb, valid ? __ldg(p.tx_meta + j) : 0, ft, ns, bufB);
+  noise_chain<HM>(p, e, j, ej, tid, g0.z, valid, act, deadb, valid ? __ldg(p.tx_meta + j) : 0, ft, ns, bufB);
 }
 
 template <bool SINGLE>
@@ -844,7 +867,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   // ---- phase 4 (S8): noise chain (fused variant); contains the barrier that also publishes hh / ha / pact
   NoiseState ns;
   if (NOISE) noise_load<HM>(p, e, j, valid, ns);
-  if (NOISE) noise_chain<HM>(p, e, j, ej, tid, gstart, valid, act, deadb, meta, ft, ns, bufB);
+  if (NOISE) noise_chain<HM>(p, e, j, ej, tid, patch0, valid, act, deadb, meta, ft, ns, bufB);
   else __syncthreads();
 
   // ---- phase 5 (S6): elastomer marker dilation (Eq. 18-21, 23 first sum) ----------------------

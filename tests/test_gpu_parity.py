@@ -199,3 +199,14 @@ def test_remaining_noise_knobs_reset_and_split(monkeypatch):
         _assert_ok(rep)
         assert sim.launches_per_step() == (2 if split == "1" else 1)
         sim.close()
+
+
+def test_gaussian_crosstalk(monkeypatch):
+    """Eq. 11 / 31 with the paper's Gaussian kernel G_sigma (R7) instead of the 4-neighbour stencil, on the
+    8x8 / 6x8 / 5x8 patches of config 5 (borders matter), alone and with the other knobs, fused and split."""
+    w = W.config(5, n_envs=48)
+    _assert_ok(_parity(w, steps=20, noise=dict(w.noise, chi=0.3, xtalk_sigma=0.8)))
+    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=1.0, xtalk_sigma=1.3, hyst_mode="maxwell", beta=0.5, tau=0.05)))
+    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=0.05, xtalk_sigma=0.3, bias_force=0.01, gain_min=0.9, gain_max=1.1)))
+    monkeypatch.setenv("TS_SPLIT", "1")
+    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=0.3, xtalk_sigma=0.8)))
