@@ -210,3 +210,49 @@ def test_gaussian_crosstalk(monkeypatch):
     _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=0.05, xtalk_sigma=0.3, bias_force=0.01, gain_min=0.9, gain_max=1.1)))
     monkeypatch.setenv("TS_SPLIT", "1")
     _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=0.3, xtalk_sigma=0.8)))
+
+
+def test_two_objects_per_env():
+    """K = 2 (Eq. 2's max over geometries, Q3): every env holds its config-2 primitive plus a second object (a sphere
+    or an SDF star grid) a few centimetres away, so some links touch one, some the other; exercises the K > 1 kernels
+    (frames per (patch, object), winner selection, march over min_k phi_k) against the oracle."""
+    import torch
+    from paper_2606_22332_b200.binding import TactileSim
+    from oracle import oracle as O
+    from parity import Comparator
+    w = W.config(2, n_envs=96)
+    w3 = W.config(3, n_envs=1)                                  # its 64^3 star grid serves as the bank
+    E, K = w.E, 2
+    rng = np.random.default_rng(5)
+    types = np.zeros((E, K), np.int32); params = np.zeros((E, K, 4), np.float32)
+    types[:, 0] = w.types[:, 0]; params[:, 0] = w.params[:, 0]
+    types[:, 1] = np.where(np.arange(E) % 2 == 0, 1, 4)         # sphere / grid 0
+    params[np.arange(E) % 2 == 0, 1, 0] = 0.025
+    noise = dict(noise_enable=1, seed=11, sigma_rw_force=1e-3, sigma_rw_torque=1e-5, hyst_mode="asym", alpha_load=0.8,
+                 alpha_unload=0.5, p_dead=0.02, chi=0.05)
+    outs = ("contact", "depth", "ft", "marker", "prox", "ft_noisy", "dead")
+    sim = TactileSim(w.patches, w.T, E, w.L, K, physics=w.physics, noise=noise, outputs=outs)
+    sim.set_geometry(types, params, w3.bank, w3.voxel)
+    orc = O.Oracle(w.patches, w.T, w.L, K, np.arange(E), physics=w.physics, noise=noise, threads=os.cpu_count() or 1)
+    orc.set_geometry(types, params, w3.bank, w3.voxel)
+    lay = sim.layout.view()
+    cmp_ = Comparator(lay, w.physics, True, lay["radius"])
+    off = rng.uniform(-0.03, 0.03, (E, 1, 3)).astype(np.float32)
+    win = np.zeros(2, np.int64)
+    for s in range(6):
+        base = w.inputs(s)
+        inp = dict(base)
+        for k in ("obj_pos", "obj_quat", "obj_linvel", "obj_angvel"):
+            second = base[k].copy()
+            if k == "obj_pos":
+                second = second + off                          # the second object sits a few cm from the first
+            if k == "obj_linvel":
+                second = -second
+            inp[k] = np.ascontiguousarray(np.concatenate([base[k], second], axis=1))
+        g = sim.step(sim.upload(inp))
+        torch.cuda.synchronize()
+        ref = orc.step(inp, want=outs)
+        cmp_.step({k: v.cpu().numpy() for k, v in g.items()}, ref)
+    rep = cmp_.report()
+    _assert_ok(rep, max_band_frac=2e-3)
+    assert rep["max_ratio"]["prox"] <= 1.0 and rep["checked"] > 1e6
