@@ -583,7 +583,12 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
       outv[c] = act ? y : 0.f;
     }
   }
-  if (EXT && deadb) {  // Eq. 28 stuck readout z_bj (R4): streams 4 / 5, n = 0; rare (p_dead of the taxels)
+  const bool stuck_on = p.stuck_lo_f != 0.f || p.stuck_hi_f != 0.f || p.stuck_lo_t != 0.f || p.stuck_hi_t != 0.f;
+  if (EXT && deadb && !stuck_on) {
+#pragma unroll
+    for (int c = 0; c < 6; ++c) outv[c] = 0.f;  // D5: stuck at zero
+  }
+  if (EXT && deadb && stuck_on) {  // Eq. 28 stuck readout z_bj (R4): streams 4 / 5, n = 0; rare (p_dead of the taxels)
     const uint4 w0 = philox4x32_10(make_uint4(env, (uint32_t)j, 0u, ep4 | 4u), p.seed_lo, p.seed_hi);
     const uint4 w1 = philox4x32_10(make_uint4(env, (uint32_t)j, 0u, ep4 | 5u), p.seed_lo, p.seed_hi);
     const uint32_t ww[6] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y};
