@@ -21,6 +21,8 @@
 //   noise                    Maxwell / asym closed forms, crosstalk patch-sum, drift moments, dead (P13-P16)
 //   remaining A.8 knobs      bias / white-noise moments, quantisation levels and hand values, per-episode gain,
 //                            stuck readout range and constancy (P19-P22; readings R1-R4 in DESIGN.md)
+//   radius noise (Eq. 26)    eps = d~ - d read back from |f| = k_n d^alpha: range, moments, the Philox word,
+//                            reach limits, constancy per episode, the max(0, .) clamp (P24; reading R8)
 //   whole path               rigid-frame invariance, filler slots, no-contact zeros (P8, P17)
 // parity unpinned: none of the functions; the *joint* output on star grids with all
 // stages on (configs 4-5) is pinned only through the per-stage pins above (P18).
@@ -256,6 +258,7 @@ typedef struct orc_params {
   float gain_min, gain_max;                     // Eq. 27 per-reset gain gamma_bj ~ U[min, max] (1, 1 = off)
   float stuck_min_force, stuck_max_force, stuck_min_torque, stuck_max_torque;  // Eq. 28 stuck readout z_bj ~ U[l, u]
   float xtalk_sigma;  // Eq. 11 / 31: 0 = 4-neighbour stencil (D4); > 0 = Gaussian G_sigma, sigma in taxel pitches (R7)
+  float radius_noise; // Eq. 26: rho (metres), R~_j = max(0, R_j + eps_j), eps_j ~ U[-rho, rho] (R8); 0 = off
 } orc_params;
 }
 
@@ -279,6 +282,7 @@ struct Oracle {
   std::vector<uint8_t> ybit;                // Schmitt state [E,T]
   std::vector<double> hyst_a, hyst_b, drift;  // [E,T,6]: (xi, x_prev) or (y, -)
   double* aux_quant = nullptr;                // [E,T,6] comparator aid, see orc_set_aux_quant
+  double* aux_rgate = nullptr;                // [E,T] comparator aid, see orc_set_aux_rgate
   std::vector<uint32_t> n_step, episode;      // [E]
 };
 
@@ -497,7 +501,7 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
 #pragma omp parallel for schedule(dynamic, 1) num_threads(n_threads > 0 ? n_threads : 1)
 #endif
   for (int e = 0; e < o.E; ++e) {
-    std::vector<double> phi_min(T), dep(T), ftc((size_t)T * 6), hcl((size_t)T * 6);
+    std::vector<double> phi_min(T), dep(T), ftc((size_t)T * 6), ftn((size_t)T * 6), hcl((size_t)T * 6);
     std::vector<uint8_t> deadv(T, 0);
     for (int j = 0; j < T; ++j) {
       size_t ej = (size_t)e * T + j;
@@ -544,6 +548,32 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
                      ld3(obj_angvel + ((size_t)e * K + kstar) * 3), f6);
       }
       for (int c = 0; c < 6; ++c) { ftc[(size_t)j * 6 + c] = f6[c]; if (ft) ft[ej * 6 + c] = f6[c]; }
+      // Eq. 26 (R8): the NOISY readout senses with the perturbed radius R~_j = max(0, R_j + eps_j),
+      // eps_j ~ U[-rho, rho] drawn once per (env, taxel, episode): stream 8, n = 0, word 0.  The clean
+      // outputs above keep R_j; the noise chain below starts from the Eq. 4-9 readout at depth
+      // d~ = [R~_j - phi]_+ (same winner, same contact normal).
+      double g6[6] = {f6[0], f6[1], f6[2], f6[3], f6[4], f6[5]};
+      if (o.aux_rgate) o.aux_rgate[ej] = INFINITY;
+      if (pr.noise_enable && pr.radius_noise != 0.0f && active) {
+        uint32_t key[2] = {pr.seed_lo, pr.seed_hi}, w[4];
+        uint32_t cr[4] = {(uint32_t)o.env_id[e], (uint32_t)j, 0u, (o.episode[e] << 4) | 8u};
+        philox4x32_10(cr, key, w);
+        double rho = (double)pr.radius_noise;
+        double eps = -rho + 2.0 * rho * word_to_uniform(w[0]);
+        double Rt = std::fmax(0.0, o.radius[j] + eps);
+        double dt_ = (kstar >= 0) ? std::fmax(0.0, Rt - best_phi) : 0.0;
+        if (o.aux_rgate) o.aux_rgate[ej] = std::fabs(Rt - best_phi);
+        for (int c = 0; c < 6; ++c) g6[c] = 0.0;
+        if (dt_ > 0.0) {
+          double gn = norm(qstar.g);
+          V3 m = (gn < 1e-12) ? (-1.0) * a : (1.0 / gn) * mul(RO_star, qstar.g);   // Q2
+          V3 pO = ld3(obj_pos + ((size_t)e * K + kstar) * 3);
+          kinematic_ft(pr, dt_, m, q, o.pos[j], RL, pL, ld3(link_linvel + ((size_t)e * L + l) * 3),
+                       ld3(link_angvel + ((size_t)e * L + l) * 3), pO, ld3(obj_linvel + ((size_t)e * K + kstar) * 3),
+                       ld3(obj_angvel + ((size_t)e * K + kstar) * 3), g6);
+        }
+      }
+      for (int c = 0; c < 6; ++c) ftn[(size_t)j * 6 + c] = g6[c];
       // O7
       if (prox) {
         double P = 0.0;
@@ -606,7 +636,7 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
           gain = (double)pr.gain_min + ((double)pr.gain_max - (double)pr.gain_min) * word_to_uniform(w[0]);
         }
         for (int c = 0; c < 6; ++c) {
-          double x = gain * ftc[(size_t)j * 6 + c], hval = x;
+          double x = gain * ftn[(size_t)j * 6 + c], hval = x;
           if (aux_asym) aux_asym[ej * 6 + c] = INFINITY;
           if (o.radius[j] > 0.0) {
             if (pr.hyst_mode == 1) {                                      // Eq. 29-30
@@ -732,6 +762,10 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
 // readout) of the pre-quantisation value from the nearest rounding boundary of Eq. 25's quantize(),
 // +inf where quantisation is off.  NULL switches it off.
 void orc_set_aux_quant(void* h, double* aux_quant) { ((Oracle*)h)->aux_quant = aux_quant; }
+
+// Comparator aid: aux_rgate[E,T] receives |R~_j - phi| (the distance of the perturbed d~ > 0 gate of Eq. 26,
+// R8), +inf where radius noise is off or the slot is inactive.  NULL switches it off.
+void orc_set_aux_rgate(void* h, double* aux_rgate) { ((Oracle*)h)->aux_rgate = aux_rgate; }
 
 // Stand-alone pieces for the pins -------------------------------------------------
 

@@ -45,7 +45,8 @@ class OrcParams(C.Structure):
                 ("quant_force", C.c_float), ("quant_torque", C.c_float),
                 ("gain_min", C.c_float), ("gain_max", C.c_float),
                 ("stuck_min_force", C.c_float), ("stuck_max_force", C.c_float),
-                ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float), ("xtalk_sigma", C.c_float)]
+                ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float), ("xtalk_sigma", C.c_float),
+                ("radius_noise", C.c_float)]
 
 
 HYST = {"off": 0, "maxwell": 1, "asym": 2}
@@ -78,6 +79,7 @@ def lib():
         L.orc_march.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p, C.c_void_p,
                                 C.c_double, C.c_int]
         L.orc_set_aux_quant.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_set_aux_rgate.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_max_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -103,7 +105,7 @@ def make_params(physics=None, noise=None):
              alpha_load=1.0, alpha_unload=1.0, p_dead=0.0, chi=0.0,
              sigma_white_force=0.0, sigma_white_torque=0.0, bias_force=0.0, bias_torque=0.0, quant_force=0.0,
              quant_torque=0.0, gain_min=1.0, gain_max=1.0, stuck_min_force=0.0, stuck_max_force=0.0,
-             stuck_min_torque=0.0, stuck_max_torque=0.0, xtalk_sigma=0.0)
+             stuck_min_torque=0.0, stuck_max_torque=0.0, xtalk_sigma=0.0, radius_noise=0.0)
     for src in (physics, noise):
         if src:
             for k, v in src.items():
@@ -212,8 +214,11 @@ class Oracle:
                 out["aux_asym"] = np.zeros((E, T, 6))
                 if self.params.quant_force > 0 or self.params.quant_torque > 0:
                     out["aux_quant"] = np.zeros((E, T, 6))
+                if self.params.radius_noise != 0:
+                    out["aux_rgate"] = np.zeros((E, T))
         g = out.get
         self.L.orc_set_aux_quant(self.h, _p(g("aux_quant")))
+        self.L.orc_set_aux_rgate(self.h, _p(g("aux_rgate")))
         self.L.orc_step(self.h, _p(a["link_pos"]), _p(a["link_quat"]), _p(a["link_linvel"]), _p(a["link_angvel"]),
                         _p(a["obj_pos"]), _p(a["obj_quat"]), _p(a["obj_linvel"]), _p(a["obj_angvel"]),
                         _p(g("contact")), _p(g("depth")), _p(g("ft")), _p(g("marker")), _p(g("prox")),

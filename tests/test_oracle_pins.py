@@ -653,6 +653,54 @@ def test_stuck_value_eq28():
     assert both.any() and (c["ft_noisy"][both] != a["ft_noisy"][both]).any()  # re-drawn at reset
 
 
+def test_radius_noise_eq26():
+    # P24, Eq. 26 (R8): the noisy readout senses with R~_j = max(0, R_j + eps_j), eps_j ~ U[-rho, rho] per
+    # (env, taxel, episode); with zero velocities Eq. 10 gives |f| = k_n d^alpha, so d~ can be read back.
+    rho, k_n, alpha = float(np.float32(5e-4)), 500.0, float(np.float32(1.2))   # the fp32 images the oracle holds
+    o, x = _contact_scene(dict(radius_noise=rho), E=256)
+    ref, _ = _contact_scene(dict(), E=256)
+    a, b, c0 = o.step(x), o.step(x), ref.step(x)
+    for k in ("depth", "ft", "contact", "prox"):                               # clean outputs keep R_j
+        np.testing.assert_array_equal(a[k], c0[k])
+    phi, d = a["aux_phi"], a["depth"]
+    fn = np.linalg.norm(a["ft_noisy"][..., :3], axis=-1)
+    dt = (fn / k_n) ** (1.0 / alpha)
+    sure = (R_TAX - rho - phi) > 1e-9                                          # touching under every eps
+    assert sure.sum() > 2000
+    eps = dt[sure] - d[sure]
+    assert eps.min() >= -rho * (1 + 1e-6) and eps.max() <= rho * (1 + 1e-6)
+    assert abs(eps.mean()) < 4 * rho / math.sqrt(3 * eps.size)                 # U[-rho, rho]: mean 0, var rho^2/3
+    assert abs(eps.var() / (rho * rho / 3) - 1) < 0.08
+    assert eps.min() < -0.95 * rho and eps.max() > 0.95 * rho
+    never = (R_TAX + rho - phi) < -1e-9                                        # out of reach under every eps
+    assert never.any() and (a["ft_noisy"][never] == 0).all()
+    maybe = ~sure & ~never                                                     # contact only appears / vanishes here
+    gained, lost = (fn > 0) & (d == 0), (fn == 0) & (d > 0)
+    assert gained.any() and lost.any() and not (gained & ~maybe).any() and not (lost & ~maybe).any()
+    # same contact normal: f~ is parallel to f, torque = x_j x f~ keeps the same lever arm
+    both = sure & (d > 0)
+    f, g = a["ft"][both], a["ft_noisy"][both]
+    assert np.abs(np.cross(f[:, :3], g[:, :3])).max() < 1e-9 * np.abs(f[:, :3]).max() * np.abs(g[:, :3]).max() + 1e-15
+    np.testing.assert_allclose(g[:, 3:] * np.linalg.norm(f[:, :3], axis=-1)[:, None],
+                               f[:, 3:] * np.linalg.norm(g[:, :3], axis=-1)[:, None], rtol=1e-9, atol=1e-15)
+    np.testing.assert_array_equal(a["ft_noisy"], b["ft_noisy"])                # fixed for the episode
+    # the draw itself: stream 8, n = 0, word 0 of the (env, taxel, episode) counter
+    e, j = np.argwhere(sure)[7]
+    u = O.uniform(int(O.philox((e, j, 0, (0 << 4) | 8), (99, 0))[0]))
+    assert abs((dt[e, j] - d[e, j]) - (-rho + 2 * rho * u)) < 1e-12
+    np.testing.assert_allclose(a["aux_rgate"][e, j], abs(float(np.float32(R_TAX)) - rho + 2 * rho * u - phi[e, j]), rtol=0, atol=1e-12)
+    o.reset()
+    c = o.step(x)
+    assert (c["ft_noisy"][sure][:, 2] != a["ft_noisy"][sure][:, 2]).mean() > 0.99          # re-drawn at reset
+    # the clamp: rho = 10 R leaves R~ = 0 for ~45 % of the taxels; those read [0 - phi]_+
+    big, xb = _contact_scene(dict(radius_noise=10 * R_TAX), E=64)
+    r = big.step(xb)
+    fz = np.linalg.norm(r["ft_noisy"][..., :3], axis=-1)
+    zero = fz == 0
+    assert 0.35 < zero.mean() < 0.6 and (r["aux_phi"] > 0).all()               # nothing penetrates: clamped ones read 0
+    assert ((fz / k_n) ** (1 / alpha) <= 11 * R_TAX).all()
+
+
 def test_gaussian_crosstalk_eq11_vs_scipy():
     # Eq. 11 / 31 (R7): z~ = (1 - chi) z + chi (G_sigma * z); pinned against scipy's zero-padded 2-D convolution of the
     # oracle's own clean ft field with an L1-normalised separable Gaussian (a library routine, not the oracle's loop)
