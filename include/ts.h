@@ -154,6 +154,10 @@ typedef struct ts_config {
    * taxel pitches: separable, g[d] = exp(-d^2 / (2 sigma^2)) for |d| <= ceil(3 sigma), L1-normalised, plain
    * convolution with zeros outside the patch (R7).  sigma <= 4/3 (radius <= 4). */
   float xtalk_sigma;
+  /* Eq. 26 radius noise rho >= 0 [m] (0 = off): the noisy readout senses with R~_j = max(0, R_j + eps_j),
+   * eps_j ~ U[-rho, rho] per (env, taxel, episode); ft_noisy then starts from Eq. 4-9 at d~ = [R~_j - phi]_+.
+   * contact, depth, ft, marker and prox keep R_j (R8). */
+  float radius_noise;
 } ts_config;
 
 /* Fills *cfg with the paper's constants and everything else zero / off. */

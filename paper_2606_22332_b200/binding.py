@@ -63,7 +63,8 @@ class Config(C.Structure):
                 ("quant_force", C.c_float), ("quant_torque", C.c_float),
                 ("gain_min", C.c_float), ("gain_max", C.c_float),
                 ("stuck_min_force", C.c_float), ("stuck_max_force", C.c_float),
-                ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float), ("xtalk_sigma", C.c_float)]
+                ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float), ("xtalk_sigma", C.c_float),
+                ("radius_noise", C.c_float)]
 
 
 class Geometry(C.Structure):

@@ -124,6 +124,8 @@ struct TsStepParams {
   float stuck_lo_f, stuck_hi_f, stuck_lo_t, stuck_hi_t;
   int32_t xt_r;     // Gaussian crosstalk radius ceil(3 sigma) <= 4; 0 = 4-neighbour stencil
   float xt_w[5];    // L1-normalised 1-D weights g[|d|], d = 0..xt_r
+  float rho;        // Eq. 26 radius noise (0 = off or noise off)
+  float* ft_pert;   // two-kernel variant with rho != 0: [E,T,6] Eq. 4-9 at the perturbed depth, else NULL
   // Small layouts carry their group records and per-group link ids in the parameter space itself (constant
   // bank: a few cycles) so that a block's first dependent global load is already the pose row.
   int32_t inl;                             // 1 = the two tables below are valid

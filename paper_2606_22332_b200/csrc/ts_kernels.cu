@@ -621,7 +621,7 @@ __global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_cons
   float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   bool act = false, deadb = false;
   if (valid) {
-    const float2* f2 = reinterpret_cast<const float2*>(p.ft + ej * 6u);
+    const float2* f2 = reinterpret_cast<const float2*>((p.ft_pert ? p.ft_pert : p.ft) + ej * 6u);  // ft_pert: Eq. 26 readout
     const float2 a = __ldcs(f2), b = __ldcs(f2 + 1), c = __ldcs(f2 + 2);
     ft[0] = a.x; ft[1] = a.y; ft[2] = b.x; ft[3] = b.y; ft[4] = c.x; ft[5] = c.y;
     act = __ldg(&p.tx_pos[j].w) > 0.f;
@@ -833,9 +833,25 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   march_phase<SINGLE>(p, frames, e, lp, valid, act, ej, phif, xo, P4, patch0 + lp);
 
   // ---- phase 3 (S5): kinematic force / torque (Eq. 4-9, D2) in double, link frame ---------------
+  // Eq. 26 (R8): the noisy readout senses with R~_j = max(0, R_j + eps_j), eps_j ~ U[-rho, rho] drawn once per
+  // (env, taxel, episode) from stream 8, n = 0, word 0; dn = [R~_j - phi]_+ is the depth the noise chain starts
+  // from.  Only the variants that carry the remaining A.8 knobs (and the two-kernel variant) evaluate it.
+  constexpr bool RN = HM < 0 || (HM & 4) != 0;
+  const bool rn_on = RN && p.rho != 0.f;  // block-uniform
+  float dn = d;
+  if (rn_on && act) {
+    const uint4 w = philox4x32_10(make_uint4(p.env_id_base + (uint32_t)e, (uint32_t)j, 0u, (__ldg(p.episode + e) << 4) | 8u),
+                                  p.seed_lo, p.seed_hi);
+    const double u = (double)(2u * (w.x >> 9) + 1u) * 5.9604644775390625e-8;
+    const double Rt = fmax(0.0, (double)Rj + fma(2.0 * (double)p.rho, u, -(double)p.rho));
+    const double dd = Rt - phid;
+    dn = dd > 0.0 ? (float)dd : 0.f;
+  }
   float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  if ((p.ft != nullptr || NOISE) && __any_sync(TS_FULL, d > 0.f)) {
-    if (d > 0.f) {  // Q5: every term gated on d > 0
+  float fn6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};  // Eq. 4-9 at depth dn (dead code unless rn_on)
+  const bool touch = d > 0.f || (rn_on && dn > 0.f);
+  if ((p.ft != nullptr || NOISE || rn_on) && __any_sync(TS_FULL, touch)) {
+    if (touch) {  // Q5: every term gated on d > 0
       const FrameS& F = frames[lp * (SINGLE ? 1 : p.K) + kst];
       const D3 g = grad_d(p, F.type, F.prm, xd);
       const double g2 = dot(g, g);
@@ -845,29 +861,68 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
         mbar = D3{-(double)na.x, -(double)na.y, -(double)na.z};
       }
       else mbar = drsqrt_n(g2) * mulRT(F.M, g);
-      const double sj = (double)__powf(d, p.alpha);  // s_j = d^alpha
       const D3 x = D3{(double)P4.x, (double)P4.y, (double)P4.z};
-      D3 f, tau;
-      if (p.use_velocity) {
+      // Everything but the depth is shared by the clean readout (depth d) and the Eq. 26 one (depth dn).
+      if (!RN) {
+        // Variants without Eq. 26 (compile-time): one readout, written straight through.  The shared form below
+        // costs this variant 0.6 % of the step on config 5 (different register allocation), measured.
+        const double sj = (double)__powf(d, p.alpha);  // s_j = d^alpha
+        D3 f, tau;
+        if (p.use_velocity) {
+          const D3 wO = ldv(F.wO), wL = ldv(F.wL);
+          const D3 vrel = ldv(F.vbar) + cross(wO, ldv(F.cbar) + x) - cross(wL, x);     // Eq. 4-6
+          const double vns = dot(vrel, mbar);
+          const D3 vt = vrel - vns * mbar;                                             // Eq. 7
+          const double fnm = sj * fma((double)p.c_n, vns, (double)p.k_n);
+          D3 ftan = (-(double)p.k_t) * vt;                                             // Eq. 8 tangential
+          const double lim = (double)p.mu * fabs(fnm), nft2 = dot(ftan, ftan);
+          if (nft2 > lim * lim) ftan = (lim * drsqrt_n(nft2)) * ftan;                  // D2 Coulomb cap
+          f = fnm * mbar + ftan;
+          tau = cross(x, f) - ((double)p.k_omega * dot(wO - wL, mbar)) * mbar;         // Eq. 9
+        } else {
+          f = ((double)p.k_n * sj) * mbar;
+          tau = cross(x, f);
+        }
+        ft[0] = (float)f.x; ft[1] = (float)f.y; ft[2] = (float)f.z;
+        ft[3] = (float)tau.x; ft[4] = (float)tau.y; ft[5] = (float)tau.z;
+      } else if (p.use_velocity) {
         const D3 wO = ldv(F.wO), wL = ldv(F.wL);
         const D3 vrel = ldv(F.vbar) + cross(wO, ldv(F.cbar) + x) - cross(wL, x);       // Eq. 4-6
         const double vns = dot(vrel, mbar);
         const D3 vt = vrel - vns * mbar;                                               // Eq. 7
-        const double fnm = sj * fma((double)p.c_n, vns, (double)p.k_n);
-        D3 ftan = (-(double)p.k_t) * vt;                                               // Eq. 8 tangential
-        const double lim = (double)p.mu * fabs(fnm), nft2 = dot(ftan, ftan);
-        if (nft2 > lim * lim) ftan = (lim * drsqrt_n(nft2)) * ftan;                    // D2 Coulomb cap
-        f = fnm * mbar + ftan;
-        tau = cross(x, f) - ((double)p.k_omega * dot(wO - wL, mbar)) * mbar;           // Eq. 9
+        const D3 ftan0 = (-(double)p.k_t) * vt;                                        // Eq. 8 tangential
+        const double nft2 = dot(ftan0, ftan0);
+        const double spin = (double)p.k_omega * dot(wO - wL, mbar);
+        auto readout = [&](float dep, float* o) {
+          const double fnm = (double)__powf(dep, p.alpha) * fma((double)p.c_n, vns, (double)p.k_n);  // s_j = d^alpha
+          D3 ftan = ftan0;
+          const double lim = (double)p.mu * fabs(fnm);
+          if (nft2 > lim * lim) ftan = (lim * drsqrt_n(nft2)) * ftan;                  // D2 Coulomb cap
+          const D3 f = fnm * mbar + ftan;
+          const D3 tau = cross(x, f) - spin * mbar;                                    // Eq. 9
+          o[0] = (float)f.x; o[1] = (float)f.y; o[2] = (float)f.z;
+          o[3] = (float)tau.x; o[4] = (float)tau.y; o[5] = (float)tau.z;
+        };
+        if (d > 0.f) readout(d, ft);
+        if (rn_on && dn > 0.f) readout(dn, fn6);
       } else {
-        f = ((double)p.k_n * sj) * mbar;
-        tau = cross(x, f);
+        auto readout = [&](float dep, float* o) {
+          const D3 f = ((double)p.k_n * (double)__powf(dep, p.alpha)) * mbar;
+          const D3 tau = cross(x, f);
+          o[0] = (float)f.x; o[1] = (float)f.y; o[2] = (float)f.z;
+          o[3] = (float)tau.x; o[4] = (float)tau.y; o[5] = (float)tau.z;
+        };
+        if (d > 0.f) readout(d, ft);
+        if (rn_on && dn > 0.f) readout(dn, fn6);
       }
-      ft[0] = (float)f.x; ft[1] = (float)f.y; ft[2] = (float)f.z;
-      ft[3] = (float)tau.x; ft[4] = (float)tau.y; ft[5] = (float)tau.z;
     }
   }
   if (p.ft && valid) store6(p.ft + ej * 6u, ft);
+  if (rn_on) {  // from here on only the Eq. 26 readout is needed
+#pragma unroll
+    for (int c = 0; c < 6; ++c) ft[c] = fn6[c];
+    if (HM < 0 && p.ft_pert && valid) store6(p.ft_pert + ej * 6u, ft);  // two-kernel variant: input of ts_noise_kernel
+  }
 
   // ---- phase 4 (S8): noise chain (fused variant); contains the barrier that also publishes hh / ha / pact
   NoiseState ns;

@@ -71,6 +71,8 @@ class Comparator:
             if "aux_asym" in ref:
                 asym = (np.abs(ref["aux_asym"]) < BAND).any(-1)
             src = ex | asym
+            if "aux_rgate" in ref:                 # Eq. 26: the noisy readout's own d~ > 0 gate sits at R~_j, not R_j
+                src = src | ((ref["aux_rgate"] < BAND) & active)
             self.noisy_taint = np.maximum(self.noisy_taint - 1, 0)
             self.noisy_taint[src] = NOISY_TAINT_STEPS
             t = self.noisy_taint > 0

@@ -201,6 +201,38 @@ def test_remaining_noise_knobs_reset_and_split(monkeypatch):
         sim.close()
 
 
+def test_radius_noise(monkeypatch):
+    """Eq. 26 (R8): ft_noisy starts from the readout at the perturbed radius; the clean outputs keep R_j.
+    rho = 0.5 mm of R = 2 mm, and rho = 3 mm (exercises the max(0, .) clamp); alone, with the other knobs, over a
+    reset, and in the two-kernel variant."""
+    import torch
+    from parity import Comparator
+    w = W.config(5, n_envs=48)
+    _assert_ok(_parity(w, steps=20, noise=dict(w.noise, radius_noise=5e-4)))
+    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, radius_noise=3e-3, hyst_mode="maxwell", beta=0.5, tau=0.05)))
+    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, radius_noise=5e-4, gain_min=0.9, gain_max=1.1, bias_force=0.01,
+                                               xtalk_sigma=0.8, chi=0.3)))
+    _assert_ok(_parity(W.config(2, n_envs=96), steps=8, noise=dict(noise_enable=1, seed=5, radius_noise=1e-3)))
+    for split in ("0", "1"):
+        monkeypatch.setenv("TS_SPLIT", split)
+        for outputs in (w.outputs, [o for o in w.outputs if o != "ft"]):
+            noise = dict(w.noise, radius_noise=5e-4)
+            sim = _sim(w, noise=noise, outputs=outputs)
+            orc = _orc(w, np.arange(w.E), os.cpu_count() or 1, noise=noise)
+            lay = sim.layout.view()
+            cmp_ = Comparator(lay, w.physics, True, lay["radius"])
+            for s in range(8):
+                if s == 4:
+                    sim.reset()
+                    orc.reset()
+                inp = w.inputs(s)
+                g = sim.step(sim.upload(inp))
+                torch.cuda.synchronize()
+                cmp_.step({k: v.cpu().numpy() for k, v in g.items() if k in outputs}, orc.step(inp, want=outputs))
+            _assert_ok(cmp_.report())
+            sim.close()
+
+
 def test_gaussian_crosstalk(monkeypatch):
     """Eq. 11 / 31 with the paper's Gaussian kernel G_sigma (R7) instead of the 4-neighbour stencil, on the
     8x8 / 6x8 / 5x8 patches of config 5 (borders matter), alone and with the other knobs, fused and split."""
