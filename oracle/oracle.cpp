@@ -23,6 +23,9 @@
 //                            stuck readout range and constancy (P19-P22; readings R1-R4 in DESIGN.md)
 //   radius noise (Eq. 26)    eps = d~ - d read back from |f| = k_n d^alpha: range, moments, the Philox word,
 //                            reach limits, constancy per episode, the max(0, .) clamp (P24; reading R8)
+//   read delay (Eq. 25)      delayed run = undelayed run shifted by Delta steps, zeros while the pipe fills and
+//                            after a reset; additive terms not delayed; jitter value unique per (env, step), all
+//                            values reached, one draw reproduced from the Philox word (P25; reading R9)
 //   whole path               rigid-frame invariance, filler slots, no-contact zeros (P8, P17)
 // parity unpinned: none of the functions; the *joint* output on star grids with all
 // stages on (configs 4-5) is pinned only through the per-stage pins above (P18).
@@ -32,6 +35,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <deque>
 #include <limits>
 #include <vector>
 #ifdef _OPENMP
@@ -259,6 +263,7 @@ typedef struct orc_params {
   float stuck_min_force, stuck_max_force, stuck_min_torque, stuck_max_torque;  // Eq. 28 stuck readout z_bj ~ U[l, u]
   float xtalk_sigma;  // Eq. 11 / 31: 0 = 4-neighbour stencil (D4); > 0 = Gaussian G_sigma, sigma in taxel pitches (R7)
   float radius_noise; // Eq. 26: rho (metres), R~_j = max(0, R_j + eps_j), eps_j ~ U[-rho, rho] (R8); 0 = off
+  int32_t read_delay, read_jitter;  // Eq. 25 Delta_read in steps and its uniform jitter +-J steps (R9); 0, 0 = off
 } orc_params;
 }
 
@@ -283,6 +288,7 @@ struct Oracle {
   std::vector<double> hyst_a, hyst_b, drift;  // [E,T,6]: (xi, x_prev) or (y, -)
   double* aux_quant = nullptr;                // [E,T,6] comparator aid, see orc_set_aux_quant
   double* aux_rgate = nullptr;                // [E,T] comparator aid, see orc_set_aux_rgate
+  std::vector<std::deque<std::vector<double>>> hist;  // [E] the last Delta + J post-crosstalk fields [T,6] of the episode
   std::vector<uint32_t> n_step, episode;      // [E]
 };
 
@@ -410,6 +416,7 @@ void* orc_create(const orc_params* prm, const orc_patch* patches, int n_patches,
   o->ybit.assign(ET, 0);
   o->hyst_a.assign(ET * 6, 0.0); o->hyst_b.assign(ET * 6, 0.0); o->drift.assign(ET * 6, 0.0);   // Q12
   o->n_step.assign(o->E, 0); o->episode.assign(o->E, 0);
+  o->hist.assign(o->E, {});
   Geom none; none.type = G_NONE; none.grid = nullptr; none.N = 0; none.hv = 0; for (double& v : none.p) v = 0;
   o->geom.assign((size_t)o->E * o->K, none);
   return o;
@@ -471,6 +478,7 @@ void orc_reset(void* h, const uint8_t* env_mask) {
     }
     o.n_step[e] = 0;
     o.episode[e] += 1;
+    o.hist[e].clear();
   }
 }
 
@@ -625,6 +633,24 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
     if (pr.noise_enable) {
       uint32_t n = o.n_step[e];
       double decay = std::exp(-(double)pr.dt / (double)pr.tau);
+      // Eq. 25 read delay (R9): the readout at step n shows the post-crosstalk signal of step n - Delta_n,
+      // Delta_n = max(0, Delta + k_n), k_n uniform on {-J..J}, one draw per (env, step) shared by all taxels:
+      // stream 9, taxel counter 0xffffffff, k_n = (((word0 >> 9) * (2J + 1)) >> 23) - J.  Steps before the
+      // episode began read 0 (Q12).
+      const bool delay_on = pr.read_delay > 0 || pr.read_jitter > 0;
+      int delta_n = 0;
+      std::vector<double> cfield;
+      if (delay_on) {
+        int k_n = 0;
+        if (pr.read_jitter > 0) {
+          uint32_t key[2] = {pr.seed_lo, pr.seed_hi}, w[4];
+          uint32_t cj[4] = {(uint32_t)o.env_id[e], 0xffffffffu, n, (o.episode[e] << 4) | 9u};
+          philox4x32_10(cj, key, w);
+          k_n = (int)(((uint64_t)(w[0] >> 9) * (uint64_t)(2 * pr.read_jitter + 1)) >> 23) - pr.read_jitter;
+        }
+        delta_n = std::max(0, pr.read_delay + k_n);
+        cfield.assign((size_t)T * 6, 0.0);
+      }
       for (int j = 0; j < T; ++j) {
         size_t ej = (size_t)e * T + j;
         // Eq. 27 (R2): per-unit calibration gain, drawn once per (env, taxel, episode): stream 3, n = 0, word 0
@@ -732,6 +758,11 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
               }
               cj = hj + ((double)pr.chi / 4.0) * acc;
             }
+            if (delay_on) {                                               // Eq. 25 y_{t - Delta_read} (R9)
+              cfield[(size_t)j * 6 + c] = cj;
+              const int have = (int)o.hist[e].size();                     // earlier steps of this episode still held
+              if (delta_n > 0) cj = (delta_n <= have) ? o.hist[e][have - delta_n][(size_t)j * 6 + c] : 0.0;
+            }
             double sig = (c < 3) ? (double)pr.sigma_rw_force : (double)pr.sigma_rw_torque;
             double D = o.drift[ej * 6 + c] + sig * z[c];                  // Eq. 25 drift
             o.drift[ej * 6 + c] = D;
@@ -752,6 +783,10 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
           }
           if (ft_noisy) ft_noisy[ej * 6 + c] = out;
         }
+      }
+      if (delay_on) {  // keep the last Delta + J fields of the episode
+        o.hist[e].push_back(cfield);
+        while ((int)o.hist[e].size() > pr.read_delay + pr.read_jitter) o.hist[e].pop_front();
       }
     }
     o.n_step[e] += 1;

@@ -46,7 +46,7 @@ class OrcParams(C.Structure):
                 ("gain_min", C.c_float), ("gain_max", C.c_float),
                 ("stuck_min_force", C.c_float), ("stuck_max_force", C.c_float),
                 ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float), ("xtalk_sigma", C.c_float),
-                ("radius_noise", C.c_float)]
+                ("radius_noise", C.c_float), ("read_delay", C.c_int32), ("read_jitter", C.c_int32)]
 
 
 HYST = {"off": 0, "maxwell": 1, "asym": 2}
@@ -105,7 +105,7 @@ def make_params(physics=None, noise=None):
              alpha_load=1.0, alpha_unload=1.0, p_dead=0.0, chi=0.0,
              sigma_white_force=0.0, sigma_white_torque=0.0, bias_force=0.0, bias_torque=0.0, quant_force=0.0,
              quant_torque=0.0, gain_min=1.0, gain_max=1.0, stuck_min_force=0.0, stuck_max_force=0.0,
-             stuck_min_torque=0.0, stuck_max_torque=0.0, xtalk_sigma=0.0, radius_noise=0.0)
+             stuck_min_torque=0.0, stuck_max_torque=0.0, xtalk_sigma=0.0, radius_noise=0.0, read_delay=0, read_jitter=0)
     for src in (physics, noise):
         if src:
             for k, v in src.items():

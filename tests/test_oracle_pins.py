@@ -701,6 +701,77 @@ def test_radius_noise_eq26():
     assert ((fz / k_n) ** (1 / alpha) <= 11 * R_TAX).all()
 
 
+def _moving_inputs(E, steps):
+    """The patch of _contact_scene pressed by a depth that changes every step (and differs per env)."""
+    out = []
+    for t in range(steps):
+        z = -0.0305 - 0.0004 * np.sin(0.9 * t + 0.3 * np.arange(E))
+        d = inputs(E=E, link_quat=(1, 0, 0, 0))
+        d["link_pos"][:, 0, 2] = z
+        out.append(d)
+    return out
+
+
+def test_read_delay_eq25():
+    # P25, Eq. 25 (R9): quantize(y_{t - Delta} + b + n_t + d_t, q): the delayed term is the post-crosstalk signal, the
+    # additive terms are of the current step.  Pinned by shifting an undelayed run of the same scene.
+    E, S, D = 8, 14, 3
+    xs = _moving_inputs(E, S)
+    base = dict(hyst_mode="asym", alpha_load=0.8, alpha_unload=0.5, chi=0.2)
+    ref, _ = _contact_scene(base, E=E)
+    c = [ref.step(x)["ft_noisy"] for x in xs]                                 # no additive terms: y_t = c_t
+    assert max(np.abs(c[t + 1] - c[t]).max() for t in range(S - 1)) > 1e-3    # the signal really moves
+    dly, _ = _contact_scene(dict(base, read_delay=D), E=E)
+    for t, x in enumerate(xs):
+        y = dly.step(x)["ft_noisy"]
+        np.testing.assert_array_equal(y, c[t - D] if t >= D else np.zeros_like(y))
+        if t == 8:                                                             # a reset empties the pipe
+            dly.reset()
+            ref2, _ = _contact_scene(base, E=E)
+            c2 = [ref2.step(x2)["ft_noisy"] for x2 in xs[9:]]
+            for u, x2 in enumerate(xs[9:]):
+                y2 = dly.step(x2)["ft_noisy"]
+                np.testing.assert_array_equal(y2, c2[u - D] if u >= D else np.zeros_like(y2))
+            break
+    # drift, bias and white noise are NOT delayed: y_delay[t] - y_nodelay[t] = c[t - D] - c[t] with the same seed
+    add = dict(base, sigma_rw_force=1e-3, sigma_rw_torque=1e-5, bias_force=0.05, sigma_white_force=1e-3)
+    a0, _ = _contact_scene(add, E=E)
+    a1, _ = _contact_scene(dict(add, read_delay=D), E=E)
+    for t, x in enumerate(xs):
+        y0, y1 = a0.step(x)["ft_noisy"], a1.step(x)["ft_noisy"]
+        want = (c[t - D] if t >= D else 0.0) - c[t]
+        np.testing.assert_allclose(y1 - y0, want, rtol=0, atol=1e-12)
+    # jitter: one Delta_n in [D - J, D + J] per (env, step), shared by all taxels, every value reached, about uniform
+    J, E2, S2 = 2, 64, 40
+    xs2 = _moving_inputs(E2, S2)
+    r2, _ = _contact_scene(base, E=E2)
+    c2 = [r2.step(x)["ft_noisy"] for x in xs2]
+    jit, _ = _contact_scene(dict(base, read_delay=D, read_jitter=J), E=E2)
+    counts = np.zeros(2 * J + 1, int)
+    for t, x in enumerate(xs2):
+        y = jit.step(x)["ft_noisy"]
+        if t < D + J:
+            continue
+        for e in range(E2):
+            hits = [k for k in range(-J, J + 1) if np.array_equal(y[e], c2[t - D - k][e])]
+            assert len(hits) == 1, (t, e, hits)
+            counts[hits[0] + J] += 1
+    assert counts.min() > 0.7 * counts.sum() / (2 * J + 1), counts
+    # the draw itself: stream 9, taxel counter 0xffffffff, step n; k = (((w >> 9) * (2J + 1)) >> 23) - J
+    w0 = int(O.philox((5, 0xffffffff, 20, (0 << 4) | 9), (99, 0))[0])
+    k = (((w0 >> 9) * (2 * J + 1)) >> 23) - J
+    jit2, _ = _contact_scene(dict(base, read_delay=D, read_jitter=J), E=E2)
+    for t in range(21):
+        y = jit2.step(xs2[t])["ft_noisy"]
+    np.testing.assert_array_equal(y[5], c2[20 - D - k][5])
+    # jitter larger than the delay clamps at zero delay
+    z, _ = _contact_scene(dict(base, read_delay=0, read_jitter=1), E=E2)
+    for t, x in enumerate(xs2[:12]):
+        y = z.step(x)["ft_noisy"]
+        for e in range(E2):
+            assert np.array_equal(y[e], c2[t][e]) or (np.array_equal(y[e], c2[t - 1][e]) if t >= 1 else not y[e].any())
+
+
 def test_gaussian_crosstalk_eq11_vs_scipy():
     # Eq. 11 / 31 (R7): z~ = (1 - chi) z + chi (G_sigma * z); pinned against scipy's zero-padded 2-D convolution of the
     # oracle's own clean ft field with an L1-normalised separable Gaussian (a library routine, not the oracle's loop)
