@@ -158,6 +158,12 @@ typedef struct ts_config {
    * eps_j ~ U[-rho, rho] per (env, taxel, episode); ft_noisy then starts from Eq. 4-9 at d~ = [R~_j - phi]_+.
    * contact, depth, ft, marker and prox keep R_j (R8). */
   float radius_noise;
+  /* Eq. 25 read delay Delta_read in STEPS (0 = off) and its uniform jitter +-J steps: the readout of step n shows the
+   * post-crosstalk signal of step n - max(0, Delta + k_n), k_n uniform on {-J..J}, one draw per (env, step); steps
+   * before the episode began read 0; bias, white noise and drift are those of step n (R9).
+   * 0 <= read_delay, read_jitter and read_delay + read_jitter <= 64; the ctx holds that many past fields
+   * (24 B x n_envs x n_taxels each). */
+  int32_t read_delay, read_jitter;
 } ts_config;
 
 /* Fills *cfg with the paper's constants and everything else zero / off. */

@@ -64,7 +64,7 @@ class Config(C.Structure):
                 ("gain_min", C.c_float), ("gain_max", C.c_float),
                 ("stuck_min_force", C.c_float), ("stuck_max_force", C.c_float),
                 ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float), ("xtalk_sigma", C.c_float),
-                ("radius_noise", C.c_float)]
+                ("radius_noise", C.c_float), ("read_delay", C.c_int32), ("read_jitter", C.c_int32)]
 
 
 class Geometry(C.Structure):

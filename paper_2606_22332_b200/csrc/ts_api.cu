@@ -50,6 +50,7 @@ struct ts_ctx {
   float last_first_kernel_ms = 0.f;
   bool fused = true;            // one fused launch (default) or geometry + noise kernels (TS_SPLIT=1)
   float* ft_scratch = nullptr;  // clean ft for the noise kernel when the caller does not ask for ft
+  float* st_ring = nullptr;       // Eq. 25 read delay: the last read_delay + read_jitter post-crosstalk fields
   float* ft_scratch_r = nullptr;  // two-kernel variant with radius noise: Eq. 4-9 at the perturbed depth (Eq. 26)
   size_t ev_used = 0;
   std::string err;
@@ -81,7 +82,7 @@ void free_all(ts_ctx* c) {
   cudaFree(c->tx_pos); cudaFree(c->tx_meta); cudaFree(c->mk_pos); cudaFree(c->mk_nrm); cudaFree(c->patches);
   cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->grp_link);
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->bank); cudaFree(c->st_flags); cudaFree(c->st_hyst);
-  cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch); cudaFree(c->ft_scratch_r);
+  cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch); cudaFree(c->ft_scratch_r); cudaFree(c->st_ring);
   for (float* q : c->stage_in) cudaFree(q);
   for (void* q : c->stage_out) cudaFree(q);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
@@ -133,9 +134,11 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
     p.xt_r = r;
     for (int d = 0; d <= r && d < 5; ++d) p.xt_w[d] = (float)(std::exp(-(double)(d * d) / (2.0 * sg * sg)) / norm);
   }
+  p.rd_delay = g.noise_enable ? g.read_delay : 0; p.rd_jitter = g.noise_enable ? g.read_jitter : 0;
+  p.rd_S = p.rd_delay + p.rd_jitter; p.st_ring = c->st_ring;
   p.rho = g.noise_enable ? g.radius_noise : 0.f;
   p.ft_pert = (p.rho != 0.f && !c->fused) ? c->ft_scratch_r : nullptr;
-  p.ext = (g.noise_enable && (g.radius_noise != 0.f || g.xtalk_sigma != 0.f || g.sigma_white_force != 0.f || g.sigma_white_torque != 0.f || g.bias_force != 0.f || g.bias_torque != 0.f ||
+  p.ext = (g.noise_enable && (g.read_delay != 0 || g.read_jitter != 0 || g.radius_noise != 0.f || g.xtalk_sigma != 0.f || g.sigma_white_force != 0.f || g.sigma_white_torque != 0.f || g.bias_force != 0.f || g.bias_torque != 0.f ||
                               g.quant_force != 0.f || g.quant_torque != 0.f || g.gain_min != 1.f || g.gain_max != 1.f ||
                               g.stuck_min_force != 0.f || g.stuck_max_force != 0.f || g.stuck_min_torque != 0.f ||
                               g.stuck_max_torque != 0.f)) ? 1 : 0;
@@ -187,6 +190,10 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     if (!(cfg->xtalk_sigma >= 0.f) || std::ceil(3.0 * (double)cfg->xtalk_sigma) > 4.0)
       return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: xtalk_sigma not in [0, 4/3]");
     if (!(cfg->radius_noise >= 0.f) || !(cfg->radius_noise < INFINITY)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: radius_noise must be finite and >= 0");
+    if (cfg->read_delay < 0 || cfg->read_jitter < 0 || cfg->read_delay + cfg->read_jitter > 64)
+      return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: need 0 <= read_delay, read_jitter and read_delay + read_jitter <= 64");
+    if ((long long)cfg->n_envs * 3LL * (cfg->read_delay + cfg->read_jitter) * ((lay->n_taxels + 31) / 32 * 32) >= (1LL << 32))
+      return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: n_envs * n_taxels * (read_delay + read_jitter) too large (32-bit element indices)");
     if (!(cfg->gain_min > 0.f) || !(cfg->gain_min <= cfg->gain_max)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: need 0 < gain_min <= gain_max");
     if (!(cfg->stuck_min_force <= cfg->stuck_max_force) || !(cfg->stuck_min_torque <= cfg->stuck_max_torque))
       return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: stuck_min > stuck_max");
@@ -373,6 +380,8 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   if (cfg->noise_enable) {
     if (c->nh) TS_ALLOC(c->st_hyst, sizeof(float) * E * c->nh * c->Tp);
     TS_ALLOC(c->st_drift, sizeof(float) * E * 6 * c->Tp);
+    // never read before written: a slot is read only for a step of the current episode (ts_kernels.cu, noise_chain)
+    if (cfg->read_delay + cfg->read_jitter > 0) TS_ALLOC(c->st_ring, sizeof(float) * E * 6 * c->Tp * (size_t)(cfg->read_delay + cfg->read_jitter));
   }
 #undef TS_ALLOC
   cudaError_t e = cudaSuccess;

@@ -126,6 +126,8 @@ struct TsStepParams {
   float xt_w[5];    // L1-normalised 1-D weights g[|d|], d = 0..xt_r
   float rho;        // Eq. 26 radius noise (0 = off or noise off)
   float* ft_pert;   // two-kernel variant with rho != 0: [E,T,6] Eq. 4-9 at the perturbed depth, else NULL
+  int32_t rd_delay, rd_jitter, rd_S;  // Eq. 25 read delay (steps), jitter, ring slots S = delay + jitter (0 = off)
+  float* st_ring;   // [E,S,3,Tp] float2 channel pairs: post-crosstalk fields of the last S steps
   // Small layouts carry their group records and per-group link ids in the parameter space itself (constant
   // bank: a few cycles) so that a block's first dependent global load is already the pose row.
   int32_t inl;                             // 1 = the two tables below are valid

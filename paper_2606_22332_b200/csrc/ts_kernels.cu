@@ -568,11 +568,45 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
       }
     }
   }
+  float cxv[6];
 #pragma unroll
   for (int c = 0; c < 6; ++c) {
     const float hc = h[c];
     const float acc = fmaf(-4.f, hc, nsum[c]);  // sum_k (h_k - h_j)
-    const float cx = gauss ? fmaf(p.chi, conv[c], (1.f - p.chi) * hc) : fmaf(q4, acc, hc);
+    cxv[c] = gauss ? fmaf(p.chi, conv[c], (1.f - p.chi) * hc) : fmaf(q4, acc, hc);
+  }
+  // Eq. 25 read delay (R9): the readout of step n shows the post-crosstalk signal of step n - Delta_n,
+  // Delta_n = max(0, Delta + k_n), k_n uniform on {-J..J}, one draw per (env, step): stream 9, taxel counter
+  // 0xffffffff.  The ring holds the fields of the last S = Delta + J steps; step n lives in slot n mod S, which is
+  // also the slot of step n - S, so the read comes first.  A slot is only read for a step >= 0 of the current
+  // episode (earlier ones read 0, Q12), hence no clearing at reset.
+  if (EXT && p.rd_S > 0 && valid) {
+    const uint32_t nstep = p.gstep - __ldg(p.reset_step + e);
+    int delta = p.rd_delay;
+    if (p.rd_jitter > 0) {
+      const uint4 w = philox4x32_10(make_uint4(env, 0xffffffffu, nstep, ep4 | 9u), p.seed_lo, p.seed_hi);
+      const int k = (int)(((unsigned long long)(w.x >> 9) * (unsigned long long)(2 * p.rd_jitter + 1)) >> 23) - p.rd_jitter;
+      delta = max(0, p.rd_delay + k);
+    }
+    float2* const ring = reinterpret_cast<float2*>(p.st_ring);
+    const unsigned S = (unsigned)p.rd_S;
+    float2 dl[3] = {make_float2(cxv[0], cxv[1]), make_float2(cxv[2], cxv[3]), make_float2(cxv[4], cxv[5])};
+    if (delta > 0) {
+      const bool have = (uint32_t)delta <= nstep;
+      const unsigned ir = (((unsigned)e * S + (nstep - (uint32_t)delta) % S) * 3u) * Tp + (unsigned)j;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) dl[c] = have ? ld_stream2(ring + (ir + c * Tp)) : make_float2(0.f, 0.f);
+    }
+    const unsigned iw = (((unsigned)e * S + nstep % S) * 3u) * Tp + (unsigned)j;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      __stcs(ring + (iw + c * Tp), make_float2(cxv[2 * c], cxv[2 * c + 1]));
+      cxv[2 * c] = dl[c].x; cxv[2 * c + 1] = dl[c].y;
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 6; ++c) {
+    const float cx = cxv[c];
     Dn[c] = act ? fmaf(c < 3 ? p.sigma_f : p.sigma_t, z[c], ns.sD[c]) : 0.f;
     if (!EXT) {
       outv[c] = (act && !deadb) ? cx + Dn[c] : 0.f;  // S8a dead (Eq. 28, D5) last

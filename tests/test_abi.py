@@ -40,7 +40,7 @@ def test_struct_sizes_match_header(B):
     assert (cfg.s_d, cfg.lambda_d) == (100.0, 8000.0) and cfg.march_steps == 16
     assert cfg.chi == 0.0 and cfg.output_mask == 31
     assert (cfg.gain_min, cfg.gain_max) == (1.0, 1.0) and cfg.stuck_max_torque == 0.0
-    assert cfg.xtalk_sigma == 0.0 and cfg.radius_noise == 0.0 and C.sizeof(B.Config) % 8 == 0                         # last field lands right
+    assert cfg.xtalk_sigma == 0.0 and cfg.radius_noise == 0.0 and (cfg.read_delay, cfg.read_jitter) == (0, 0) and C.sizeof(B.Config) % 8 == 0                         # last field lands right
 
 
 @pytest.mark.parametrize("cid", [1, 2, 3, 4])
@@ -87,7 +87,8 @@ def test_create_rejects_bad_config_before_touching_cuda(B):
                 dict(noise=dict(noise_enable=1, quant_force=-1e-3)), dict(noise=dict(noise_enable=1, sigma_white_torque=-1.0)),
                 dict(noise=dict(noise_enable=1, stuck_min_force=1.0, stuck_max_force=0.5)),
                 dict(noise=dict(noise_enable=1, xtalk_sigma=1.5)), dict(noise=dict(noise_enable=1, xtalk_sigma=-0.1)),
-                dict(noise=dict(noise_enable=1, radius_noise=-1e-4)), dict(noise=dict(noise_enable=1, radius_noise=float("inf")))):
+                dict(noise=dict(noise_enable=1, radius_noise=-1e-4)), dict(noise=dict(noise_enable=1, read_delay=-1)),
+                dict(noise=dict(noise_enable=1, read_delay=60, read_jitter=5)), dict(noise=dict(noise_enable=1, radius_noise=float("inf")))):
         kw = dict(n_envs=4, n_links=16, objs_per_env=1, layout=lay)
         kw.update(bad)
         cfg = B.make_config(**kw)

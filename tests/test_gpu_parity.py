@@ -233,6 +233,39 @@ def test_radius_noise(monkeypatch):
             sim.close()
 
 
+def test_read_delay(monkeypatch):
+    """Eq. 25 read delay with jitter (R9): ring of past post-crosstalk fields, per-env step counters
+    (a partial reset puts the envs at different ring positions), both hysteresis modes, fused and two-kernel."""
+    import torch
+    from parity import Comparator
+    w = W.config(5, n_envs=48)
+    _assert_ok(_parity(w, steps=16, noise=dict(w.noise, read_delay=3)))
+    _assert_ok(_parity(w, steps=24, noise=dict(w.noise, read_delay=2, read_jitter=2, hyst_mode="maxwell", beta=0.5, tau=0.05,
+                                               bias_force=0.01, radius_noise=3e-4)))
+    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, read_delay=0, read_jitter=1)))
+    mask = (np.arange(w.E) % 3 == 0).astype(np.uint8)
+    for split in ("0", "1"):
+        monkeypatch.setenv("TS_SPLIT", split)
+        noise = dict(w.noise, read_delay=2, read_jitter=1)
+        sim = _sim(w, noise=noise)
+        orc = _orc(w, np.arange(w.E), os.cpu_count() or 1, noise=noise)
+        lay = sim.layout.view()
+        cmp_ = Comparator(lay, w.physics, True, lay["radius"])
+        for s in range(14):
+            if s == 5:
+                sim.reset(torch.from_numpy(mask).cuda())
+                orc.reset(mask)
+            if s == 9:
+                sim.reset()
+                orc.reset()
+            inp = w.inputs(s)
+            g = sim.step(sim.upload(inp))
+            torch.cuda.synchronize()
+            cmp_.step({k: v.cpu().numpy() for k, v in g.items()}, orc.step(inp, want=w.outputs))
+        _assert_ok(cmp_.report())
+        sim.close()
+
+
 def test_gaussian_crosstalk(monkeypatch):
     """Eq. 11 / 31 with the paper's Gaussian kernel G_sigma (R7) instead of the 4-neighbour stencil, on the
     8x8 / 6x8 / 5x8 patches of config 5 (borders matter), alone and with the other knobs, fused and split."""
