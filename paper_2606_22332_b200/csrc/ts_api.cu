@@ -88,6 +88,14 @@ void free_all(ts_ctx* c) {
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
 }
 
+// 1 = a knob beyond the four of configs 4-5 is set: selects the kernel variants that carry them (HM | 4).
+int cfg_ext(const ts_config& g) {
+  return (g.noise_enable && (g.read_delay != 0 || g.read_jitter != 0 || g.radius_noise != 0.f || g.xtalk_sigma != 0.f || g.sigma_white_force != 0.f || g.sigma_white_torque != 0.f || g.bias_force != 0.f || g.bias_torque != 0.f ||
+                              g.quant_force != 0.f || g.quant_torque != 0.f || g.gain_min != 1.f || g.gain_max != 1.f ||
+                              g.stuck_min_force != 0.f || g.stuck_max_force != 0.f || g.stuck_min_torque != 0.f ||
+                              g.stuck_max_torque != 0.f)) ? 1 : 0;
+}
+
 void fill_params(const ts_ctx* c, TsStepParams& p) {
   const ts_config& g = c->cfg;
   std::memset(&p, 0, sizeof(p));
@@ -138,10 +146,7 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.rd_S = p.rd_delay + p.rd_jitter; p.st_ring = c->st_ring;
   p.rho = g.noise_enable ? g.radius_noise : 0.f;
   p.ft_pert = (p.rho != 0.f && !c->fused) ? c->ft_scratch_r : nullptr;
-  p.ext = (g.noise_enable && (g.read_delay != 0 || g.read_jitter != 0 || g.radius_noise != 0.f || g.xtalk_sigma != 0.f || g.sigma_white_force != 0.f || g.sigma_white_torque != 0.f || g.bias_force != 0.f || g.bias_torque != 0.f ||
-                              g.quant_force != 0.f || g.quant_torque != 0.f || g.gain_min != 1.f || g.gain_max != 1.f ||
-                              g.stuck_min_force != 0.f || g.stuck_max_force != 0.f || g.stuck_min_torque != 0.f ||
-                              g.stuck_max_torque != 0.f)) ? 1 : 0;
+  p.ext = cfg_ext(g);
 }
 }  // namespace
 
@@ -373,7 +378,11 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   TS_ALLOC(c->episode, sizeof(uint32_t) * E);
   {
     const char* sp = std::getenv("TS_SPLIT");
-    c->fused = !(sp ? (sp[0] == '1') : TS_DEFAULT_SPLIT);
+    // Default: one fused launch, except when optional A.8 knobs are on: the fused variant that carries them executes
+    // 46.7 KB of SASS per block (41.9 KB without them), past the instruction-cache knee (ncu: no_instruction stall
+    // 0.27 -> 2.97 cycles per issue), and the two-kernel form is 0.1-0.2 ms faster on config 5 (measured, DESIGN.md
+    // section 6).  TS_SPLIT=0 / 1 forces either form.
+    c->fused = sp ? (sp[0] != '1') : !(TS_DEFAULT_SPLIT || cfg_ext(*cfg));
   }
   if (cfg->noise_enable && !c->fused && !(cfg->output_mask & TS_OUT_FT)) TS_ALLOC(c->ft_scratch, sizeof(float) * E * T * 6);
   if (cfg->noise_enable && !c->fused && cfg->radius_noise != 0.f) TS_ALLOC(c->ft_scratch_r, sizeof(float) * E * T * 6);

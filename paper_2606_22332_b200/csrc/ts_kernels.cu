@@ -578,9 +578,14 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
   // Eq. 25 read delay (R9): the readout of step n shows the post-crosstalk signal of step n - Delta_n,
   // Delta_n = max(0, Delta + k_n), k_n uniform on {-J..J}, one draw per (env, step): stream 9, taxel counter
   // 0xffffffff.  The ring holds the fields of the last S = Delta + J steps; step n lives in slot n mod S, which is
-  // also the slot of step n - S, so the read comes first.  A slot is only read for a step >= 0 of the current
-  // episode (earlier ones read 0, Q12), hence no clearing at reset.
-  if (EXT && p.rd_S > 0 && valid) {
+  // also the slot of step n - S, so the read comes first; the write is issued at the very end of the chain, after
+  // the loaded values have been consumed: a store to a line whose read miss is still outstanding cost 0.9 ms per
+  // step on config 5 (2.65 -> 1.9 ms, measured).  A slot is only read for a step >= 0 of the current episode
+  // (earlier ones read 0, Q12), hence no clearing at reset.
+  const bool ring_on = EXT && p.rd_S > 0 && valid;
+  float2 ringw[3];
+  unsigned iw = 0u;
+  if (ring_on) {
     const uint32_t nstep = p.gstep - __ldg(p.reset_step + e);
     int delta = p.rd_delay;
     if (p.rd_jitter > 0) {
@@ -597,10 +602,10 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
 #pragma unroll
       for (int c = 0; c < 3; ++c) dl[c] = have ? ld_stream2(ring + (ir + c * Tp)) : make_float2(0.f, 0.f);
     }
-    const unsigned iw = (((unsigned)e * S + nstep % S) * 3u) * Tp + (unsigned)j;
+    iw = (((unsigned)e * S + nstep % S) * 3u) * Tp + (unsigned)j;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      __stcs(ring + (iw + c * Tp), make_float2(cxv[2 * c], cxv[2 * c + 1]));
+      ringw[c] = make_float2(cxv[2 * c], cxv[2 * c + 1]);
       cxv[2 * c] = dl[c].x; cxv[2 * c + 1] = dl[c].y;
     }
   }
@@ -637,6 +642,10 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
     for (int c = 0; c < 3; ++c) __stcs(st_d + (id + c * Tp), make_float2(Dn[2 * c], Dn[2 * c + 1]));
   }
   if (p.ft_noisy && valid) store6(p.ft_noisy + ej * 6u, outv);
+  if (ring_on) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) __stcs(reinterpret_cast<float2*>(p.st_ring) + (iw + c * Tp), ringw[c]);
+  }
 }
 
 // Stand-alone noise kernel (split variant): reads the clean ft the geometry kernel wrote.
@@ -874,8 +883,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const bool rn_on = RN && p.rho != 0.f;  // block-uniform
   float dn = d;
   if (rn_on && act) {
-    const uint4 w = philox4x32_10(make_uint4(p.env_id_base + (uint32_t)e, (uint32_t)j, 0u, (__ldg(p.episode + e) << 4) | 8u),
-                                  p.seed_lo, p.seed_hi);
+    const uint4 w = philox4x32_10(make_uint4(p.env_id_base + (uint32_t)e, (uint32_t)j, 0u, (__ldg(p.episode + e) << 4) | 8u), p.seed_lo, p.seed_hi);
     const double u = (double)(2u * (w.x >> 9) + 1u) * 5.9604644775390625e-8;
     const double Rt = fmax(0.0, (double)Rj + fma(2.0 * (double)p.rho, u, -(double)p.rho));
     const double dd = Rt - phid;

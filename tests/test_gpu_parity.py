@@ -154,10 +154,12 @@ def test_edge_shapes():
     assert torch.allclose(out2["prox"][0][act], torch.full_like(out2["prox"][0][act], 0.02))  # K_m = 0: t = 0, P = r_prox
 
 
-def test_remaining_noise_knobs():
+def test_remaining_noise_knobs(monkeypatch):
     """App. A.8 knobs beyond the four of configs 4-5 (R1-R4): bias, white noise, quantisation (Eq. 25),
-    per-episode gain (Eq. 27), stuck readout of dead taxels (Eq. 28), with both hysteresis modes and over a reset."""
+    per-episode gain (Eq. 27), stuck readout of dead taxels (Eq. 28), with both hysteresis modes and over a reset.
+    With such a knob set the ctx defaults to the two-kernel form; TS_SPLIT=0 forces the fused variant (tested first)."""
     w = W.config(5, n_envs=48)
+    monkeypatch.setenv("TS_SPLIT", "0")
     ext = dict(sigma_white_force=2e-3, sigma_white_torque=2e-5, bias_force=0.02, bias_torque=-3e-4, gain_min=0.9,
                gain_max=1.1, stuck_min_force=-0.5, stuck_max_force=0.5, stuck_min_torque=-5e-3, stuck_max_torque=5e-3,
                p_dead=0.05)
@@ -167,7 +169,8 @@ def test_remaining_noise_knobs():
     rep = _parity(w, steps=20, noise=dict(w.noise, quant_force=1e-3, quant_torque=1e-5, **ext))
     _assert_ok(rep, max_band_frac=3e-3)
     assert rep["quant_exempt"] < 3e-3 * rep["checked"]
-    # each knob alone (the others off)
+    # each knob alone (the others off), in the default (two-kernel) form
+    monkeypatch.delenv("TS_SPLIT")
     for one in (dict(bias_force=0.1), dict(sigma_white_force=1e-3), dict(gain_min=0.5, gain_max=0.6),
                 dict(stuck_min_force=1.0, stuck_max_force=1.0), dict(quant_torque=1e-5)):
         _assert_ok(_parity(w, steps=6, noise=dict(w.noise, **one)), max_band_frac=3e-3)
@@ -266,10 +269,22 @@ def test_read_delay(monkeypatch):
         sim.close()
 
 
+def test_table12_force_row():
+    """The paper's "noisy condition" for force / force_torque probes (Table 12): sigma = 5e-3 N white noise,
+    p_dead = 0.05, gain in [0.85, 1.15], Maxwell hysteresis (0.5, 0.05 s); plus the table's probe-radius noise of the
+    depth row (3e-4 m) and the Schmitt release threshold 2e-4 m of the bool row."""
+    w = W.config(4, n_envs=48)
+    noise = dict(noise_enable=1, seed=2606, hyst_mode="maxwell", beta=0.5, tau=0.05, p_dead=0.05, gain_min=0.85, gain_max=1.15,
+                 sigma_white_force=5e-3, sigma_white_torque=5e-5, radius_noise=3e-4)
+    assert abs(w.physics["eta_off"] - 2e-4) < 1e-12
+    _assert_ok(_parity(w, steps=40, noise=noise))
+
+
 def test_gaussian_crosstalk(monkeypatch):
     """Eq. 11 / 31 with the paper's Gaussian kernel G_sigma (R7) instead of the 4-neighbour stencil, on the
     8x8 / 6x8 / 5x8 patches of config 5 (borders matter), alone and with the other knobs, fused and split."""
     w = W.config(5, n_envs=48)
+    monkeypatch.setenv("TS_SPLIT", "0")
     _assert_ok(_parity(w, steps=20, noise=dict(w.noise, chi=0.3, xtalk_sigma=0.8)))
     _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=1.0, xtalk_sigma=1.3, hyst_mode="maxwell", beta=0.5, tau=0.05)))
     _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=0.05, xtalk_sigma=0.3, bias_force=0.01, gain_min=0.9, gain_max=1.1)))
