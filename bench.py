@@ -149,6 +149,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="budget of the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--noise-knobs", default="", help="profiling aid, not the headline workload: extra App. A.8 knobs "
+                    "as k=v,k=v (e.g. bias_force=0.02,read_delay=2); named in config.workload")
     a = ap.parse_args()
     K, Wm = a.steps, max(a.warmup, 0)
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -186,6 +188,11 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     w = W.config(a.config, n_envs=a.envs or None, seed=rank)
+    if a.noise_knobs:
+        assert w.noise, "--noise-knobs needs a config with the noise model on (4 or 5)"
+        extra = {k: (int(v) if k.startswith("read_") else (v if k == "hyst_mode" else float(v)))
+                 for k, v in (kv.split("=") for kv in a.noise_knobs.split(","))}
+        w.noise = dict(w.noise, **extra)
     sim = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=w.physics, noise=w.noise, outputs=w.outputs,
                      env_id_base=rank * w.E, device=local)
     sim.set_geometry(w.types, w.params, w.bank, w.voxel)
@@ -263,7 +270,8 @@ def main():
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": "config%d %s: %d envs x %d taxels per GPU, %d links, %d markers, outputs=%s, noise=%s"
                                    % (a.config, w.name, E, T, w.L, M, "+".join(w.outputs),
-                                      (w.noise or {}).get("hyst_mode", "off") if w.noise else "off"),
+                                      ((w.noise or {}).get("hyst_mode", "off") if w.noise else "off")
+                                      + ("+" + a.noise_knobs if a.noise_knobs else "")),
                        "n_envs_per_gpu": E, "n_taxels": T, "parallelism": "env-shard x%d, no collective" % world,
                        "l2": "per-step working set %.2f GB >> 126 MB L2 (state + outputs stream through); no explicit flush"
                              % (bpt * E * T / 1e9),
