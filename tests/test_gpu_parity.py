@@ -81,6 +81,31 @@ def test_config5_full_size_sampled():
     _assert_ok(_parity(w, ids=w.parity_envs(), steps=12))
 
 
+def test_config5_full_size_optional_knobs_sampled(monkeypatch):
+    """BASELINE size with the optional App. A.8 knobs (Table 12 force row + radius noise + a 2 +- 1 step read delay +
+    quantisation): the default two-kernel form against the oracle on the 16 parity envs, then fused against two-kernel
+    bit for bit on every env (both forms run the same chain code on the same fp32 force/torque values)."""
+    import torch
+    w = W.config(5)
+    noise = dict(w.noise, hyst_mode="maxwell", beta=0.5, tau=0.05, p_dead=0.05, gain_min=0.85, gain_max=1.15,
+                 sigma_white_force=5e-3, sigma_white_torque=5e-5, radius_noise=3e-4, read_delay=2, read_jitter=1,
+                 quant_force=1e-3, quant_torque=1e-5)
+    rep = _parity(w, ids=w.parity_envs(), steps=8, noise=noise)
+    _assert_ok(rep, max_band_frac=3e-3)
+    outs = {}
+    for split in ("0", "1"):
+        monkeypatch.setenv("TS_SPLIT", split)
+        sim = _sim(w, noise=noise)
+        assert sim.launches_per_step() == (2 if split == "1" else 1)
+        for s in range(5):
+            g = sim.step(sim.upload(w.inputs(s)))
+        torch.cuda.synchronize()
+        outs[split] = {k: v.clone() for k, v in g.items()}
+        sim.close()
+    for k in outs["0"]:
+        assert torch.equal(outs["0"][k], outs["1"][k]), k
+
+
 def test_config3_full_size_sampled():
     w = W.config(3)
     _assert_ok(_parity(w, ids=w.parity_envs()[::8], steps=3))
