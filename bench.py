@@ -232,6 +232,11 @@ def main():
     kern_ms, kern_n = sim.kernel_time_ms(False)
     first_ms = sim.first_kernel_time_ms()
     launches = K * sim.launches_per_step()
+    # how much contact / march work the scene carries (last timed step, this rank): belongs next to the timing
+    act_n = max(int((sim.layout.view()["radius"] > 0).sum()) * E, 1)
+    scene = {k2: round(float(fn(out[k1]).sum().item()) / act_n, 4) for k1, k2, fn in
+             (("depth", "frac_depth_gt0", lambda x: x > 0), ("contact", "frac_contact", lambda x: x > 0),
+              ("prox", "frac_prox_gt0", lambda x: x > 0), ("dead", "frac_dead", lambda x: x > 0)) if k1 in out}
 
     # ---- e2e: ts_step_host on pinned host buffers (H2D + kernel + D2H inside the timed region)
     Ke = max(1, min(a.e2e_steps, K))
@@ -272,7 +277,7 @@ def main():
                                    % (a.config, w.name, E, T, w.L, M, "+".join(w.outputs),
                                       ((w.noise or {}).get("hyst_mode", "off") if w.noise else "off")
                                       + ("+" + a.noise_knobs if a.noise_knobs else "")),
-                       "n_envs_per_gpu": E, "n_taxels": T, "parallelism": "env-shard x%d, no collective" % world,
+                       "n_envs_per_gpu": E, "n_taxels": T, "scene": scene, "parallelism": "env-shard x%d, no collective" % world,
                        "l2": "per-step working set %.2f GB >> 126 MB L2 (state + outputs stream through); no explicit flush"
                              % (bpt * E * T / 1e9),
                        "precision": "fp32 I/O and state; relative pose, first query, force/torque and marker sums in fp64 (DESIGN.md section 5)"},
