@@ -288,6 +288,7 @@ struct Oracle {
   std::vector<double> hyst_a, hyst_b, drift;  // [E,T,6]: (xi, x_prev) or (y, -)
   double* aux_quant = nullptr;                // [E,T,6] comparator aid, see orc_set_aux_quant
   double* aux_rgate = nullptr;                // [E,T] comparator aid, see orc_set_aux_rgate
+  double* aux_wingap = nullptr;               // [E,T] comparator aid, see orc_set_aux_wingap
   std::vector<std::deque<std::vector<double>>> hist;  // [E] the last Delta + J post-crosstalk fields [T,6] of the episode
   std::vector<uint32_t> n_step, episode;      // [E]
 };
@@ -522,6 +523,7 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
       V3 a = mul(RL, o.nrm[j]);
       // O2/O3: query all K objects, winner = max_k [R - phi_k]_+, ties -> lowest k
       double best_phi = INFINITY; int kstar = -1; Query qstar{}; M3 RO_star{};
+      double second_phi = INFINITY;                          // comparator aid only (winner ties when K > 1)
       for (int k = 0; k < K; ++k) {
         const Geom& g = o.geom[(size_t)e * K + k];
         if (g.type == G_NONE) continue;
@@ -529,9 +531,11 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
         M3 RO = quat_to_R(obj_quat + ((size_t)e * K + k) * 4);
         V3 xo = mulT(RO, q - pO);
         Query r = sdf_eval(g, xo);
-        if (r.phi < best_phi) { best_phi = r.phi; kstar = k; qstar = r; RO_star = RO; }
+        if (r.phi < best_phi) { second_phi = best_phi; best_phi = r.phi; kstar = k; qstar = r; RO_star = RO; }
+        else if (r.phi < second_phi) second_phi = r.phi;
       }
       phi_min[j] = best_phi;
+      if (o.aux_wingap) o.aux_wingap[ej] = second_phi - best_phi;   // +inf with fewer than two objects
       double d = (active && kstar >= 0) ? std::fmax(0.0, o.radius[j] - best_phi) : 0.0;   // Eq. 2
       dep[j] = d;
       if (aux_phi) aux_phi[ej] = best_phi;
@@ -801,6 +805,10 @@ void orc_set_aux_quant(void* h, double* aux_quant) { ((Oracle*)h)->aux_quant = a
 // Comparator aid: aux_rgate[E,T] receives |R~_j - phi| (the distance of the perturbed d~ > 0 gate of Eq. 26,
 // R8), +inf where radius noise is off or the slot is inactive.  NULL switches it off.
 void orc_set_aux_rgate(void* h, double* aux_rgate) { ((Oracle*)h)->aux_rgate = aux_rgate; }
+
+// Comparator aid: aux_wingap[E,T] receives phi_second - phi_best over the K objects of the env (the margin by
+// which Eq. 2's winner g* won), +inf with fewer than two objects.  NULL switches it off.
+void orc_set_aux_wingap(void* h, double* aux_wingap) { ((Oracle*)h)->aux_wingap = aux_wingap; }
 
 // Stand-alone pieces for the pins -------------------------------------------------
 

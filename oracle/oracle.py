@@ -80,6 +80,7 @@ def lib():
                                 C.c_double, C.c_int]
         L.orc_set_aux_quant.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_set_aux_rgate.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_set_aux_wingap.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_max_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -210,6 +211,8 @@ class Oracle:
             out["aux_phi"] = np.zeros((E, T))
             out["aux_face"] = np.zeros((E, T))
             out["aux_boxgap"] = np.zeros((E, T))
+            if self.K > 1:
+                out["aux_wingap"] = np.zeros((E, T))
             if self.params.noise_enable:
                 out["aux_asym"] = np.zeros((E, T, 6))
                 if self.params.quant_force > 0 or self.params.quant_torque > 0:
@@ -219,6 +222,7 @@ class Oracle:
         g = out.get
         self.L.orc_set_aux_quant(self.h, _p(g("aux_quant")))
         self.L.orc_set_aux_rgate(self.h, _p(g("aux_rgate")))
+        self.L.orc_set_aux_wingap(self.h, _p(g("aux_wingap")))
         self.L.orc_step(self.h, _p(a["link_pos"]), _p(a["link_quat"]), _p(a["link_linvel"]), _p(a["link_angvel"]),
                         _p(a["obj_pos"]), _p(a["obj_quat"]), _p(a["obj_linvel"]), _p(a["obj_angvel"]),
                         _p(g("contact")), _p(g("depth")), _p(g("ft")), _p(g("marker")), _p(g("prox")),

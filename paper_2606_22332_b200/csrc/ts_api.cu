@@ -1,6 +1,7 @@
 // C ABI of include/ts.h: context, validation, uploads, launches.  No compute happens here.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -34,8 +35,12 @@ struct ts_ctx {
   double* mk_tab = nullptr;
   int32_t* g_type = nullptr;
   float4* g_params = nullptr;
+  int32_t* env_perm = nullptr;  // block -> env order of the step kernel (sorted by geometry; set by ts_set_geometry)
   float4* bank = nullptr;
   size_t bank_bytes = 0;
+  float* bank_stage = nullptr;  // linear copy of the bank the re-tiling kernel reads (kept between ts_set_geometry calls)
+  size_t bank_stage_bytes = 0;
+  std::vector<int32_t> h_perm;  // host copy of env_perm (source of the asynchronous upload)
   int grid_n = 2, n_grids = 0;
   float voxel = 1.f;
   uint8_t* st_flags = nullptr;
@@ -81,7 +86,7 @@ struct DeviceGuard {
 void free_all(ts_ctx* c) {
   cudaFree(c->tx_pos); cudaFree(c->tx_meta); cudaFree(c->mk_pos); cudaFree(c->mk_nrm); cudaFree(c->patches);
   cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->grp_link);
-  cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->bank); cudaFree(c->st_flags); cudaFree(c->st_hyst);
+  cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->env_perm); cudaFree(c->bank); cudaFree(c->bank_stage); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch); cudaFree(c->ft_scratch_r); cudaFree(c->st_ring);
   for (float* q : c->stage_in) cudaFree(q);
   for (void* q : c->stage_out) cudaFree(q);
@@ -113,7 +118,7 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   }
   p.env_id_base = (uint32_t)g.env_id_base;
   p.tx_pos = c->tx_pos; p.tx_meta = c->tx_meta; p.patches = c->patches; p.mk_pos = c->mk_pos; p.mk_nrm = c->mk_nrm;
-  p.g_type = c->g_type; p.g_params = c->g_params; p.bank = c->bank;
+  p.g_type = c->g_type; p.g_params = c->g_params; p.bank = c->bank; p.env_perm = c->env_perm;
   p.grid_n = c->grid_n; p.voxel = c->voxel; p.inv_voxel = 1.0f / c->voxel; p.inv_voxel_d = 1.0 / (double)c->voxel;
   p.grid_stride = ts_bank_elems_per_grid(c->grid_n);
   p.st_flags = c->st_flags; p.st_hyst = c->st_hyst; p.st_drift = c->st_drift;
@@ -373,6 +378,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   TS_ALLOC(c->mk_tab, sizeof(double) * tab.size());
   TS_ALLOC(c->g_type, sizeof(int32_t) * EK);
   TS_ALLOC(c->g_params, sizeof(float4) * EK);
+  TS_ALLOC(c->env_perm, sizeof(int32_t) * E);
   TS_ALLOC(c->st_flags, E * T);
   TS_ALLOC(c->reset_step, sizeof(uint32_t) * E);
   TS_ALLOC(c->episode, sizeof(uint32_t) * E);
@@ -424,7 +430,8 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
 ts_status ts_set_geometry(ts_ctx* c, const ts_geometry* geo, void* stream) {
   if (!c) return TS_ERR_INVALID_ARG;
   if (!geo || !geo->type || !geo->params) return fail(c, TS_ERR_INVALID_ARG, "ts_set_geometry: NULL argument");
-  const size_t EK = (size_t)c->cfg.n_envs * c->cfg.objs_per_env;
+  const int E = c->cfg.n_envs, K = c->cfg.objs_per_env;
+  const size_t EK = (size_t)E * K;
   if (geo->n_grids < 0 || (geo->n_grids > 0 && (!geo->grids || geo->grid_n < 2 || geo->grid_n > 512 || !(geo->voxel > 0.f))))
     return fail(c, TS_ERR_INVALID_ARG, "ts_set_geometry: bad grid bank");
   for (size_t i = 0; i < EK; ++i) {
@@ -435,34 +442,51 @@ ts_status ts_set_geometry(ts_ctx* c, const ts_geometry* geo, void* stream) {
       if (!(id >= 0.f) || id >= (float)geo->n_grids || id != std::floor(id)) return fail(c, TS_ERR_INVALID_ARG, "ts_set_geometry: grid id out of range");
     }
   }
+  const int N = geo->grid_n;
+  if (geo->n_grids > 0 && ts_bank_elems_per_grid(N) * (unsigned long long)geo->n_grids >= (1ULL << 31))
+    return fail(c, TS_ERR_UNSUPPORTED, "ts_set_geometry: bank larger than 2^31 cells (32-bit cell indices)");
   DeviceGuard guard(c->device);
   cudaStream_t st = (cudaStream_t)stream;
-  TS_CUDA(c, cudaMemcpyAsync(c->g_type, geo->type, sizeof(int32_t) * EK, cudaMemcpyHostToDevice, st));
-  TS_CUDA(c, cudaMemcpyAsync(c->g_params, geo->params, sizeof(float4) * EK, cudaMemcpyHostToDevice, st));
+  // From here on the old geometry is gone: every failure path leaves the ctx WITHOUT geometry (ts_step refuses), never
+  // with new descriptors next to an old or missing bank.  Allocation first, uploads last.
+  c->have_geometry = false;
+  c->n_grids = 0;
+  size_t lin = 0;
   if (geo->n_grids > 0) {
-    const int N = geo->grid_n;
-    if (ts_bank_elems_per_grid(N) * (unsigned long long)geo->n_grids >= (1ULL << 31))
-      return fail(c, TS_ERR_UNSUPPORTED, "ts_set_geometry: bank larger than 2^31 cells (32-bit cell indices)");
     const size_t need = sizeof(float4) * ts_bank_elems_per_grid(N) * geo->n_grids;
+    lin = sizeof(float) * (size_t)N * N * N * geo->n_grids;
+    if (need > c->bank_bytes || lin > c->bank_stage_bytes) TS_CUDA(c, cudaStreamSynchronize(st));  // steps in flight still read them
     if (need > c->bank_bytes) {
-      TS_CUDA(c, cudaStreamSynchronize(st));
       cudaFree(c->bank); c->bank = nullptr; c->bank_bytes = 0;
       TS_CUDA(c, cudaMalloc((void**)&c->bank, need));
       c->bank_bytes = need;
     }
-    float* staging = nullptr;
-    const size_t lin = sizeof(float) * (size_t)N * N * N * geo->n_grids;
-    TS_CUDA(c, cudaMalloc((void**)&staging, lin));
-    cudaError_t e = cudaMemcpyAsync(staging, geo->grids, lin, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = (cudaError_t)ts_launch_retile(staging, c->bank, geo->n_grids, N, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(staging);
-    if (e != cudaSuccess) return cuda_fail(c, e, "ts_set_geometry: bank upload");
-    c->grid_n = N; c->voxel = geo->voxel; c->n_grids = geo->n_grids;
-  } else {
-    c->n_grids = 0;
+    if (lin > c->bank_stage_bytes) {  // linear staging copy of the bank, kept for the next call
+      cudaFree(c->bank_stage); c->bank_stage = nullptr; c->bank_stage_bytes = 0;
+      TS_CUDA(c, cudaMalloc((void**)&c->bank_stage, lin));
+      c->bank_stage_bytes = lin;
+    }
   }
-  TS_CUDA(c, cudaStreamSynchronize(st));
+  // Block -> env order of the step kernel: envs sorted (stably) by the geometry of their first object -- type, then
+  // grid id -- so that the ~740 blocks resident at any time gather from one grid of the bank (it stays in L2: 8 x 96^3
+  // quad-layout grids are 113 MB, one is 14 MB) and run the same march loop.  Scheduling only: results do not depend on it.
+  c->h_perm.resize(E);
+  for (int e = 0; e < E; ++e) c->h_perm[e] = e;
+  auto key = [&](int e) {
+    const int t = geo->type[(size_t)e * K];
+    return t * 4096 + (t == TS_GEOM_SDF ? (int)geo->params[4 * (size_t)e * K] % 4096 : 0);
+  };
+  std::stable_sort(c->h_perm.begin(), c->h_perm.end(), [&](int a, int b) { return key(a) < key(b); });
+  TS_CUDA(c, cudaMemcpyAsync(c->env_perm, c->h_perm.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaMemcpyAsync(c->g_type, geo->type, sizeof(int32_t) * EK, cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaMemcpyAsync(c->g_params, geo->params, sizeof(float4) * EK, cudaMemcpyHostToDevice, st));
+  if (geo->n_grids > 0) {
+    TS_CUDA(c, cudaMemcpyAsync(c->bank_stage, geo->grids, lin, cudaMemcpyHostToDevice, st));
+    const cudaError_t e = (cudaError_t)ts_launch_retile(c->bank_stage, c->bank, geo->n_grids, N, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "ts_set_geometry: retile launch");
+  }
+  TS_CUDA(c, cudaStreamSynchronize(st));  // the caller may free or reuse its arrays once this returns
+  if (geo->n_grids > 0) { c->grid_n = N; c->voxel = geo->voxel; c->n_grids = geo->n_grids; }
   c->have_geometry = true;
   return TS_OK;
 }

@@ -84,6 +84,8 @@ struct TsStepParams {
   // geometry
   const int32_t* g_type;   // [E,K]
   const float4* g_params;  // [E,K]
+  const int32_t* env_perm; // [E] block -> env: envs ordered by (geometry type, grid id) so that the blocks resident at any
+                           // time gather from ONE grid of the bank (L2-resident) and run one march loop; NULL = identity
   const float4* bank;      // re-tiled SDF bank (see ts_kernels.cu, "bank layout")
   int32_t grid_n;
   float voxel, inv_voxel;

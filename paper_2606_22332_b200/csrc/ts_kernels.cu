@@ -796,7 +796,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   unsigned* pmask = reinterpret_cast<unsigned*>(ha + TS_BLOCK);  // bit l: group-local patch l has penetration
 
   const int tid = threadIdx.x;
-  const int e = blockIdx.x;
+  const int e = p.env_perm ? __ldg(p.env_perm + blockIdx.x) : (int)blockIdx.x;
   const int gi = blockIdx.y;
   int gstart, gcount, patch0, chunk0, nchunk, gmcount;
   if (p.inl) {  // group record from the parameter space (constant bank)

@@ -6,14 +6,39 @@ counted and reported); tolerances are never loosened.
 """
 import numpy as np
 
+import math
+
 ATOL, RTOL, BAND = 1e-6, 1e-4, 1e-6
 FACE_BAND = 1e-4        # voxels: trilinear gradient jumps across cell faces
-NOISY_TAINT_STEPS = 100  # hysteresis memory of an exempted ft value (0.905^100 < 1e-4)
+NOISY_TAINT_STEPS = 100  # default hysteresis memory of an exempted ft value (Maxwell, tau = 0.05 s: 0.905^100 < 1e-4)
+
+
+def taint_steps(noise):
+    """Steps until an exempted ft value has left the hysteresis state (its weight has decayed below RTOL):
+    Maxwell xi decays by exp(-dt / tau) per step (Eq. 29), ASYM y by (1 - min(alpha_load, alpha_unload)) (D3);
+    without hysteresis the chain has no memory of past ft values (drift and white noise do not depend on ft).
+    A read delay of Delta + J steps (R9) shows the value that much later."""
+    if not noise:
+        return NOISY_TAINT_STEPS
+    hm = noise.get("hyst_mode", "off")
+    delay = int(noise.get("read_delay", 0)) + int(noise.get("read_jitter", 0))
+    if hm in ("maxwell", 1):
+        r = math.exp(-float(noise.get("dt", 0.005)) / float(noise.get("tau", 0.05)))
+    elif hm in ("asym", 2):
+        r = 1.0 - min(float(noise.get("alpha_load", 1.0)), float(noise.get("alpha_unload", 1.0)))
+    else:
+        return 1 + delay
+    if r <= 0.0:
+        return 1 + delay
+    return min(NOISY_TAINT_STEPS, 1 + int(math.ceil(math.log(RTOL) / math.log(r)))) + delay
 
 
 class Comparator:
-    def __init__(self, layout, physics, noise_on, radius):
+    def __init__(self, layout, physics, noise_on, radius, noise=None):
         self.nbr = np.asarray(layout["nbr"])
+        self.taint_steps = taint_steps(noise)
+        sg = float((noise or {}).get("xtalk_sigma", 0.0))
+        self.xt_radius = int(math.ceil(3.0 * sg)) if sg > 0 else 0   # R7: Gaussian support, else the 4-neighbour stencil
         self.eta_on = float(np.float32(physics.get("eta_on", 5e-4)))
         self.eta_off = float(np.float32(physics.get("eta_off", 5e-4)))
         self.radius = np.asarray(radius, np.float64)
@@ -22,7 +47,7 @@ class Comparator:
         self.contact_taint = None
         self.noisy_taint = None
         self.stats = dict(steps=0, contact_band=0, contact_tainted=0, ft_exempt=0, noisy_exempt=0, quant_exempt=0,
-                          checked=0, max_ratio={})
+                          win_tie=0, checked=0, taxel_steps=0, noisy_taxel_steps=0, max_ratio={})
         self.failures = []
 
     def _tol_ratio(self, g, r):
@@ -63,7 +88,12 @@ class Comparator:
         face = (ref["aux_face"] < FACE_BAND) & (d > 0)
         box = (ref["aux_boxgap"] < BAND) & (d > 0)
         ex = (gate | face | box) & active
+        if "aux_wingap" in ref:                    # K > 1: two objects within 1e-6 of the winning phi: g* (and the normal) may differ
+            tie = (ref["aux_wingap"] < BAND) & (d > 0) & active
+            st["win_tie"] += int(tie.sum())
+            ex = ex | tie
         st["ft_exempt"] += int(ex.sum())
+        st["taxel_steps"] += int(active.sum()) * E
         if "ft" in gpu:
             self._check("ft", gpu["ft"], ref["ft"], ex)
         if "ft_noisy" in gpu:
@@ -74,14 +104,11 @@ class Comparator:
             if "aux_rgate" in ref:                 # Eq. 26: the noisy readout's own d~ > 0 gate sits at R~_j, not R_j
                 src = src | ((ref["aux_rgate"] < BAND) & active)
             self.noisy_taint = np.maximum(self.noisy_taint - 1, 0)
-            self.noisy_taint[src] = NOISY_TAINT_STEPS
+            self.noisy_taint[src] = self.taint_steps
             t = self.noisy_taint > 0
-            spread = t.copy()                      # crosstalk carries a tainted value to its 4 neighbours
-            for a in range(4):
-                nb = self.nbr[:, a]
-                ok = nb >= 0
-                spread[:, ok] |= t[:, nb[ok]]
+            spread = self._spread(t)               # crosstalk carries a tainted value over its support
             st["noisy_exempt"] += int(spread.sum())
+            st["noisy_taxel_steps"] += int(active.sum()) * E
             ex6 = np.broadcast_to(spread[..., None], ref["ft_noisy"].shape)
             if "aux_quant" in ref:
                 # Eq. 25 quantize(): a readout whose pre-quantisation value lies within the float tolerance of a
@@ -96,6 +123,25 @@ class Comparator:
                 st["quant_exempt"] += int((qflip & ~ex6).sum())
                 ex6 = ex6 | qflip
             self._check("ft_noisy", gpu["ft_noisy"], ref["ft_noisy"], ex6)
+
+    def _spread(self, t):
+        """Taxels whose crosstalk support (Eq. 31) contains a tainted taxel: the 4 neighbours (D4), or the
+        (2r+1) x (2r+1) square of the Gaussian kernel (R7), within the patch."""
+        def dilate(m, cols):
+            out = m.copy()
+            for a in cols:
+                nb = self.nbr[:, a]
+                ok = nb >= 0
+                out[:, ok] |= m[:, nb[ok]]
+            return out
+        if self.xt_radius == 0:
+            return dilate(t, (0, 1, 2, 3))
+        s = t
+        for _ in range(self.xt_radius):
+            s = dilate(s, (0, 1))                  # along u
+        for _ in range(self.xt_radius):
+            s = dilate(s, (2, 3))                  # along v
+        return s
 
     def _check(self, name, g, r, exempt):
         ratio = self._tol_ratio(g, r)
@@ -116,10 +162,14 @@ class Comparator:
     def report(self):
         s = dict(self.stats)
         s["failures"] = self.failures[:10]
+        s["ft_exempt_frac"] = s["ft_exempt"] / max(s["taxel_steps"], 1)
+        s["noisy_exempt_frac"] = s["noisy_exempt"] / max(s["noisy_taxel_steps"], 1)
+        s["taint_steps"] = self.taint_steps
         return s
 
 
-def run_parity(workload, sim_factory, oracle_factory, env_ids=None, steps=None, outputs=None, threads=8, quant=(0.0, 0.0)):
+def run_parity(workload, sim_factory, oracle_factory, env_ids=None, steps=None, outputs=None, threads=8, quant=(0.0, 0.0),
+               noise="workload"):
     """Steps the CUDA path over ALL envs of `workload` and the oracle over `env_ids`, comparing each step."""
     import torch
     w = workload
@@ -127,7 +177,8 @@ def run_parity(workload, sim_factory, oracle_factory, env_ids=None, steps=None, 
     sim = sim_factory(w)
     orc = oracle_factory(w, ids, threads)
     lay = sim.layout.view()
-    cmp_ = Comparator(lay, w.physics, w.noise is not None, lay["radius"])
+    nz = w.noise if noise == "workload" else noise
+    cmp_ = Comparator(lay, w.physics, nz is not None, lay["radius"], noise=nz)
     cmp_.quant = quant
     outs = outputs or w.outputs
     for s in range(steps or w.steps):

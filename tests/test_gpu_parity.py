@@ -26,11 +26,16 @@ def _orc(w, ids, threads, **kw):
     return o
 
 
-def _assert_ok(rep, max_band_frac=1e-3):
+def _assert_ok(rep, max_band_frac=1e-3, max_noisy_frac=0.03):
+    """No element outside the tolerance, and the exemptions (bands) stay a small, stated share:
+    ft / contact / quantisation bands <= max_band_frac of the checked elements; ft_noisy taxel-steps exempted through
+    hysteresis memory and crosstalk spread <= max_noisy_frac of the ft_noisy taxel-steps (printed either way)."""
     print(json.dumps({k: v for k, v in rep.items()}, default=str))
     assert not rep["failures"], rep["failures"]
     n = max(rep["checked"], 1)
     assert rep["ft_exempt"] + rep["contact_tainted"] + rep.get("quant_exempt", 0) <= max(20, max_band_frac * n), rep
+    assert rep["noisy_exempt"] <= max(50, max_noisy_frac * rep["noisy_taxel_steps"]), \
+        ("noisy_exempt_frac", rep["noisy_exempt_frac"], rep)
 
 
 def _parity(w, ids=None, steps=None, **kw):
@@ -38,7 +43,8 @@ def _parity(w, ids=None, steps=None, **kw):
     nz = kw.get("noise") or {}
     return run_parity(w, lambda ww: _sim(ww, **kw), lambda ww, i, t: _orc(ww, i, t, **kw), ids, steps,
                       kw.get("outputs"), threads=os.cpu_count() or 1,
-                      quant=(float(np.float32(nz.get("quant_force", 0.0))), float(np.float32(nz.get("quant_torque", 0.0)))))
+                      quant=(float(np.float32(nz.get("quant_force", 0.0))), float(np.float32(nz.get("quant_torque", 0.0)))),
+                      noise=kw.get("noise", w.noise))
 
 
 def test_config1_tiny():
@@ -47,6 +53,11 @@ def test_config1_tiny():
 
 def test_config2_primitives_small():
     _assert_ok(_parity(W.config(2, n_envs=192)))          # every primitive class, ragged last block
+
+
+def test_config2_full_size_all_envs():
+    """SURVEY 8(d) parity set of config 2: all 4,096 envs x 10 steps, element by element."""
+    _assert_ok(_parity(W.config(2)))
 
 
 def test_config3_sdf_small():
@@ -75,10 +86,23 @@ def test_uncapped_and_no_velocity():
 
 
 def test_config5_full_size_sampled():
-    """BASELINE size, the launch configuration bench.py times: 20,480 envs x 1,000 taxels; the oracle
-    recomputes the 16 parity envs {1281 k} (every object class once) element by element."""
+    """SURVEY 8(d) parity set of config 5 -- BASELINE size, the launch configuration bench.py times: 20,480 envs x
+    1,000 taxels x 200 steps (state carries over: drift grows, hysteresis and Schmitt state evolve over five
+    trajectory periods); the oracle recomputes the 16 parity envs {1281 k} (every object class once) element by element."""
     w = W.config(5)
-    _assert_ok(_parity(w, ids=w.parity_envs(), steps=12))
+    rep = _parity(w, ids=w.parity_envs(), steps=200)
+    _assert_ok(rep)
+    assert rep["steps"] == 200 and rep["checked"] > 5e7
+
+
+def test_config4_full_size_sampled():
+    """SURVEY 8(d) parity set of config 4: 16,384 envs x 1,000 taxels x 100 steps, 128 envs (stride 128) recomputed by the
+    oracle; ASYM hysteresis as timed, then a second pass with the paper's Maxwell loop (Eq. 29-30, Table 12 values)."""
+    w = W.config(4)
+    ids = w.parity_envs()
+    assert len(ids) == 128
+    _assert_ok(_parity(w, ids=ids, steps=100))
+    _assert_ok(_parity(w, ids=ids, steps=100, noise=dict(w.noise, hyst_mode="maxwell", beta=0.5, tau=0.05)), max_noisy_frac=0.15)
 
 
 def test_config5_full_size_optional_knobs_sampled(monkeypatch):
@@ -107,8 +131,10 @@ def test_config5_full_size_optional_knobs_sampled(monkeypatch):
 
 
 def test_config3_full_size_sampled():
+    """SURVEY 8(d) parity set of config 3: 8,192 envs x 500 taxels x 10 steps, 512 envs (stride 16) recomputed."""
     w = W.config(3)
-    _assert_ok(_parity(w, ids=w.parity_envs()[::8], steps=3))
+    assert len(w.parity_envs()) == 512
+    _assert_ok(_parity(w, ids=w.parity_envs(), steps=10))
 
 
 def test_env_shards_are_bit_identical_to_the_full_run():
@@ -214,7 +240,7 @@ def test_remaining_noise_knobs_reset_and_split(monkeypatch):
         sim = _sim(w, noise=noise)
         orc = _orc(w, np.arange(w.E), os.cpu_count() or 1, noise=noise)
         lay = sim.layout.view()
-        cmp_ = Comparator(lay, w.physics, True, lay["radius"])
+        cmp_ = Comparator(lay, w.physics, True, lay["radius"], noise=noise)
         for s in range(12):
             if s == 6:
                 sim.reset()
@@ -238,8 +264,9 @@ def test_radius_noise(monkeypatch):
     w = W.config(5, n_envs=48)
     _assert_ok(_parity(w, steps=20, noise=dict(w.noise, radius_noise=5e-4)))
     _assert_ok(_parity(w, steps=10, noise=dict(w.noise, radius_noise=3e-3, hyst_mode="maxwell", beta=0.5, tau=0.05)))
+    # Gaussian crosstalk spreads an exempted taxel over its 7 x 7 support instead of 5 taxels: larger exempt share
     _assert_ok(_parity(w, steps=10, noise=dict(w.noise, radius_noise=5e-4, gain_min=0.9, gain_max=1.1, bias_force=0.01,
-                                               xtalk_sigma=0.8, chi=0.3)))
+                                               xtalk_sigma=0.8, chi=0.3)), max_noisy_frac=0.10)
     _assert_ok(_parity(W.config(2, n_envs=96), steps=8, noise=dict(noise_enable=1, seed=5, radius_noise=1e-3)))
     for split in ("0", "1"):
         monkeypatch.setenv("TS_SPLIT", split)
@@ -248,7 +275,7 @@ def test_radius_noise(monkeypatch):
             sim = _sim(w, noise=noise, outputs=outputs)
             orc = _orc(w, np.arange(w.E), os.cpu_count() or 1, noise=noise)
             lay = sim.layout.view()
-            cmp_ = Comparator(lay, w.physics, True, lay["radius"])
+            cmp_ = Comparator(lay, w.physics, True, lay["radius"], noise=noise)
             for s in range(8):
                 if s == 4:
                     sim.reset()
@@ -278,7 +305,7 @@ def test_read_delay(monkeypatch):
         sim = _sim(w, noise=noise)
         orc = _orc(w, np.arange(w.E), os.cpu_count() or 1, noise=noise)
         lay = sim.layout.view()
-        cmp_ = Comparator(lay, w.physics, True, lay["radius"])
+        cmp_ = Comparator(lay, w.physics, True, lay["radius"], noise=noise)
         for s in range(14):
             if s == 5:
                 sim.reset(torch.from_numpy(mask).cuda())
@@ -310,11 +337,14 @@ def test_gaussian_crosstalk(monkeypatch):
     8x8 / 6x8 / 5x8 patches of config 5 (borders matter), alone and with the other knobs, fused and split."""
     w = W.config(5, n_envs=48)
     monkeypatch.setenv("TS_SPLIT", "0")
-    _assert_ok(_parity(w, steps=20, noise=dict(w.noise, chi=0.3, xtalk_sigma=0.8)))
-    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=1.0, xtalk_sigma=1.3, hyst_mode="maxwell", beta=0.5, tau=0.05)))
-    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=0.05, xtalk_sigma=0.3, bias_force=0.01, gain_min=0.9, gain_max=1.1)))
+    # the taint of an exempted taxel covers the kernel's (2r+1)^2 support (r = ceil(3 sigma)): larger exempt share
+    _assert_ok(_parity(w, steps=20, noise=dict(w.noise, chi=0.3, xtalk_sigma=0.8)), max_noisy_frac=0.10)
+    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=1.0, xtalk_sigma=1.3, hyst_mode="maxwell", beta=0.5, tau=0.05)),
+               max_noisy_frac=0.20)
+    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=0.05, xtalk_sigma=0.3, bias_force=0.01, gain_min=0.9, gain_max=1.1)),
+               max_noisy_frac=0.05)
     monkeypatch.setenv("TS_SPLIT", "1")
-    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=0.3, xtalk_sigma=0.8)))
+    _assert_ok(_parity(w, steps=10, noise=dict(w.noise, chi=0.3, xtalk_sigma=0.8)), max_noisy_frac=0.10)
 
 
 def test_two_objects_per_env():
@@ -341,7 +371,7 @@ def test_two_objects_per_env():
     orc = O.Oracle(w.patches, w.T, w.L, K, np.arange(E), physics=w.physics, noise=noise, threads=os.cpu_count() or 1)
     orc.set_geometry(types, params, w3.bank, w3.voxel)
     lay = sim.layout.view()
-    cmp_ = Comparator(lay, w.physics, True, lay["radius"])
+    cmp_ = Comparator(lay, w.physics, True, lay["radius"], noise=noise)
     off = rng.uniform(-0.03, 0.03, (E, 1, 3)).astype(np.float32)
     win = np.zeros(2, np.int64)
     for s in range(6):
@@ -359,5 +389,5 @@ def test_two_objects_per_env():
         ref = orc.step(inp, want=outs)
         cmp_.step({k: v.cpu().numpy() for k, v in g.items()}, ref)
     rep = cmp_.report()
-    _assert_ok(rep, max_band_frac=2e-3)
+    _assert_ok(rep)                                             # winner ties (|phi_k - phi_k'| < 1e-6) are a counted band
     assert rep["max_ratio"]["prox"] <= 1.0 and rep["checked"] > 1e6
