@@ -33,6 +33,8 @@ struct ts_ctx {
   std::vector<TsGroup> h_groups;   // host copies for the inline parameter tables
   std::vector<int32_t> h_glink;
   double* mk_tab = nullptr;
+  double* mk_tab8 = nullptr;   // zero-padded 8 x 8 separable tables (DMMA marker path)
+  bool mk_mma = false;
   int32_t* g_type = nullptr;
   float4* g_params = nullptr;
   int32_t* env_perm = nullptr;  // block -> env order of the step kernel (sorted by geometry; set by ts_set_geometry)
@@ -85,7 +87,7 @@ struct DeviceGuard {
 
 void free_all(ts_ctx* c) {
   cudaFree(c->tx_pos); cudaFree(c->tx_meta); cudaFree(c->mk_pos); cudaFree(c->mk_nrm); cudaFree(c->patches);
-  cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->grp_link);
+  cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->mk_tab8); cudaFree(c->grp_link);
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->env_perm); cudaFree(c->bank); cudaFree(c->bank_stage); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch); cudaFree(c->ft_scratch_r); cudaFree(c->st_ring);
   for (float* q : c->stage_in) cudaFree(q);
@@ -108,6 +110,8 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.G = c->G; p.Tp = c->Tp; p.frames_per_group = c->frames_per_group;
   p.groups = c->groups; p.chunks = c->chunks; p.mk_item1 = c->mk_item1; p.mk_item2 = c->mk_item2;
   p.mk_tab = c->mk_tab; p.grp_link = c->grp_link;
+  p.mk_tab8 = c->mk_tab8; p.mk_mma = c->mk_mma ? 1 : 0;
+  p.s_bytes = c->mk_mma ? (int32_t)(sizeof(float) * 6 * TS_BLOCK) : (int32_t)(sizeof(double) * 3 * TS_CHUNK);
   p.inl = 0; p.inl_stride = c->frames_per_group;
   if (c->G <= TS_INL_GROUPS && c->G * c->frames_per_group <= TS_INL_LINKS && (int)c->h_groups.size() == c->G) {
     p.inl = 1;
@@ -238,6 +242,8 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   const int M = (int)lay->marker_patch.size();
   std::vector<TsPatch> pts;
   std::vector<double> tab;
+  std::vector<double> tab8;   // [patch][4][8][8], zero-padded copies of the separable tables
+  bool all_mma = true;        // every patch with markers fits the 8 x 8 DMMA tiles
   std::vector<int32_t> item1, item2(M > 0 ? M : 1, 0);
   int used = 0;
   for (size_t pi = 0; pi < lay->patch_start.size(); ++pi) {
@@ -280,9 +286,20 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
       tab.insert(tab.end(), DU.begin(), DU.end());
       tab.insert(tab.end(), GV.begin(), GV.end());
       tab.insert(tab.end(), DV.begin(), DV.end());
+      if (q.nu <= 8 && q.nv <= 8 && q.mnu <= 8 && q.mnv <= 8) {
+        tab8.resize((pts.size() + 1) * 256, 0.0);
+        double* t8 = tab8.data() + pts.size() * 256;
+        for (int a = 0; a < q.mnu; ++a)
+          for (int ip = 0; ip < q.nu; ++ip) { t8[a * 8 + ip] = GU[a * q.nu + ip]; t8[64 + a * 8 + ip] = DU[a * q.nu + ip]; }
+        for (int b = 0; b < q.mnv; ++b)
+          for (int iq = 0; iq < q.nv; ++iq) { t8[128 + b * 8 + iq] = GV[b * q.nv + iq]; t8[192 + b * 8 + iq] = DV[b * q.nv + iq]; }
+      } else {
+        all_mma = false;
+      }
       for (int iq = 0; iq < q.nv; ++iq)
         for (int a = 0; a < q.mnu; ++a) item1.push_back(0);  // packed below, once the group-local index is known
     }
+    if (q.mnu > 0 && q.direct) all_mma = false;
     pts.push_back(q);
     used = q.start + q.n;
   }
@@ -340,6 +357,8 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   c->h_groups = groups; c->h_glink = glink;
   if (item1.empty()) item1.push_back(0);
   if (tab.empty()) tab.push_back(0.0);
+  tab8.resize(pts.size() * 256, 0.0);
+  c->mk_mma = all_mma && M > 0;
   if (chunks.empty()) chunks.push_back(TsChunk{});
   std::vector<float4> mpos(M > 0 ? M : 1), mnrm(M > 0 ? M : 1);
   for (int j = 0; j < M; ++j) {
@@ -376,6 +395,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   TS_ALLOC(c->mk_item1, sizeof(int32_t) * item1.size());
   TS_ALLOC(c->mk_item2, sizeof(int32_t) * item2.size());
   TS_ALLOC(c->mk_tab, sizeof(double) * tab.size());
+  TS_ALLOC(c->mk_tab8, sizeof(double) * tab8.size());
   TS_ALLOC(c->g_type, sizeof(int32_t) * EK);
   TS_ALLOC(c->g_params, sizeof(float4) * EK);
   TS_ALLOC(c->env_perm, sizeof(int32_t) * E);
@@ -412,6 +432,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   cp(c->mk_item1, item1.data(), sizeof(int32_t) * item1.size());
   cp(c->mk_item2, item2.data(), sizeof(int32_t) * item2.size());
   cp(c->mk_tab, tab.data(), sizeof(double) * tab.size());
+  cp(c->mk_tab8, tab8.data(), sizeof(double) * tab8.size());
   if (e == cudaSuccess) e = cudaMemset(c->g_type, 0, sizeof(int32_t) * EK);
   if (e == cudaSuccess) e = cudaMemset(c->g_params, 0, sizeof(float4) * EK);
   if (e == cudaSuccess) e = cudaMemset(c->reset_step, 0, sizeof(uint32_t) * E);

@@ -79,6 +79,9 @@ struct TsStepParams {
   const int32_t* mk_item1;  // packed lp | a << 8 | q << 16
   const int32_t* mk_item2;  // [M] packed lp | a << 8 | b << 16
   const double* mk_tab;     // per patch: GU[mnu][nu], DU[mnu][nu], GV[mnv][nv], DV[mnv][nv]
+  const double* mk_tab8;    // per patch [4][8][8], zero-padded: GU[a][p], DU[a][p], GV[b][q], DV[b][q] (DMMA marker path)
+  int32_t mk_mma;           // 1 = every patch with markers has nu, nv, mnu, mnv <= 8 and a separable sum: DMMA path
+  int32_t s_bytes;          // bytes of the shared-memory region S / bufB (9 KB with the generic marker path, 6 KB with DMMA)
   const float4* mk_pos;   // [M]
   const float4* mk_nrm;   // [M]
   // geometry

@@ -382,6 +382,11 @@ __device__ __forceinline__ void store6(float* dst, const float* v) {
   __stcs(d2 + 2, make_float2(v[4], v[5]));
 }
 
+// D (8 x 8) += A (8 x 4, row) B (4 x 8, col) on the FP64 tensor cores: lane = 4 g + m holds A[g][m], B[m][g], D[g][2m], D[g][2m+1].
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
 #define TS_FULL 0xffffffffu
 #ifndef TS_MIN_BLOCKS
 #define TS_MIN_BLOCKS 5
@@ -789,23 +794,23 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   FrameS* frames = reinterpret_cast<FrameS*>(smem_raw);
   // Shared memory is kept small on purpose: it is carved out of the same 256 KB as L1, and the SDF gathers
   // of the march live on L1 hits.  S (marker phase) aliases bufB (noise phase); a barrier separates them.
-  double* S = reinterpret_cast<double*>(frames + nfr);    // [3][TS_CHUNK] marker pass-1 sums
-  float* bufB = reinterpret_cast<float*>(S);              // [6][TS_BLOCK] crosstalk exchange (first half of S)
-  float* hh = reinterpret_cast<float*>(S + 3 * TS_CHUNK); // [TS_BLOCK] penetration h_i (Eq. 19)
+  double* S = reinterpret_cast<double*>(frames + nfr);    // [3][TS_CHUNK] marker pass-1 sums (generic marker path only)
+  float* bufB = reinterpret_cast<float*>(S);              // [6][TS_BLOCK] crosstalk exchange (first 6 KB of S)
+  float* hh = reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(S) + p.s_bytes);  // [TS_BLOCK] penetration h_i (Eq. 19)
   float* ha = hh + TS_BLOCK;                              // [TS_BLOCK] h_i^alpha_e
   unsigned* pmask = reinterpret_cast<unsigned*>(ha + TS_BLOCK);  // bit l: group-local patch l has penetration
 
   const int tid = threadIdx.x;
   const int e = p.env_perm ? __ldg(p.env_perm + blockIdx.x) : (int)blockIdx.x;
   const int gi = blockIdx.y;
-  int gstart, gcount, patch0, chunk0, nchunk, gmcount;
+  int gstart, gcount, patch0, npatch, chunk0, nchunk, gmcount;
   if (p.inl) {  // group record from the parameter space (constant bank)
     const TsGroup& g = p.inl_grp[gi];
-    gstart = g.start; gcount = g.count; patch0 = g.patch0; chunk0 = g.chunk0; nchunk = g.nchunk; gmcount = g.mcount;
+    gstart = g.start; gcount = g.count; patch0 = g.patch0; npatch = g.npatch; chunk0 = g.chunk0; nchunk = g.nchunk; gmcount = g.mcount;
   } else {
     const int4 g0 = __ldg(reinterpret_cast<const int4*>(p.groups + gi));
     const int4 g1 = __ldg(reinterpret_cast<const int4*>(p.groups + gi) + 1);
-    gstart = g0.x; gcount = g0.y; patch0 = g0.z; chunk0 = g1.x; nchunk = g1.y; gmcount = g1.w;
+    gstart = g0.x; gcount = g0.y; patch0 = g0.z; npatch = g0.w; chunk0 = g1.x; nchunk = g1.y; gmcount = g1.w;
   }
 
   // ---- phase 0: relative poses (double) -> shared memory ---------------------------------
@@ -978,7 +983,61 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   //   pass 1 over (a,q): S0 = sum_p gu h, S1 = sum_p du gu h, T0 = sum_p gu h^alpha_e
   //   pass 2 over (a,b): Uu = sum_q gv S1, Uv = sum_q dv gv S0, Un = sum_q gv T0.
   // Sources with h_i = 0 contribute exactly 0; patches without penetration are skipped.
-  if (p.marker && gmcount > 0) {
+  if (p.marker && gmcount > 0 && p.mk_mma) {
+    // DMMA path (every patch fits 8 x 8 tiles): ONE WARP PER PATCH evaluates both passes as FP64 tensor-core products
+    // (mma.m8n8k4, SASS DMMA.8x8x4) on zero-padded 8 x 8 tables; lane = 4 g + m holds A[row g][k m], B[k m][col g]
+    // and C[row g][cols 2m, 2m+1].
+    //   pass 1 (k = p):  S0 = GU H^T, S1 = DU H^T, T0 = GU Ha^T        with H[q][p] = h_i, C = S[a = g][q = 2m, 2m+1]
+    //   pass 2 (k = q):  Uu = S1 GV^T, Uv = S0 DV^T, Un = T0 GV^T       contraction order q = 2m + kk, so that the A
+    //                    operand of k-step kk is exactly the C element kk this lane already holds (no exchange).
+    // hh / ha / pmask were published by the barrier above; no shared-memory scratch and no further barrier.
+    const int lane = tid & 31, g = lane >> 2, m = lane & 3;
+    const unsigned pm = *pmask;
+    for (int l = tid >> 5; l < npatch; l += TS_BLOCK / 32) {
+      const TsPatch& pt = p.patches[patch0 + l];
+      const int mnu = __ldg(&pt.mnu), mnv = __ldg(&pt.mnv);
+      if (mnu == 0) continue;
+      float* o = p.marker + ((size_t)e * p.M + __ldg(&pt.mstart)) * 3;
+      if (!((pm >> l) & 1u)) {  // no penetration anywhere in the patch: its markers are exactly 0
+        for (int i = lane; i < mnu * mnv * 3; i += 32) __stcs(o + i, 0.f);
+        continue;
+      }
+      const int nu = __ldg(&pt.nu), nv = __ldg(&pt.nv), base = __ldg(&pt.start) - gstart;
+      const double* tab = p.mk_tab8 + (size_t)(patch0 + l) * 256;
+      double s0a = 0.0, s0b = 0.0, s1a = 0.0, s1b = 0.0, t0a = 0.0, t0b = 0.0;
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk) {
+        const int ip = kk * 4 + m;                    // B[k = p][n = q = g] = h[q][p]
+        const bool ok = g < nv && ip < nu;
+        const double h = ok ? (double)hh[base + g * nu + ip] : 0.0, hal = ok ? (double)ha[base + g * nu + ip] : 0.0;
+        const double gu = __ldg(tab + g * 8 + ip), du = __ldg(tab + 64 + g * 8 + ip);   // A[a = g][k = p]
+        dmma884(s0a, s0b, gu, h);
+        dmma884(s1a, s1b, du, h);
+        dmma884(t0a, t0b, gu, hal);
+      }
+      double uua = 0.0, uub = 0.0, uva = 0.0, uvb = 0.0, una = 0.0, unb = 0.0;
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk) {
+        const double gv = __ldg(tab + 128 + g * 8 + 2 * m + kk), dv = __ldg(tab + 192 + g * 8 + 2 * m + kk);  // B[k = q][n = b = g]
+        dmma884(uua, uub, kk ? s1b : s1a, gv);
+        dmma884(uva, uvb, kk ? s0b : s0a, dv);
+        dmma884(una, unb, kk ? t0b : t0a, gv);
+      }
+      const double sd = (double)p.s_d, kt = sd * p.inv_gbar;
+      const float4 ua = __ldg(&pt.ua), va = __ldg(&pt.va), na = __ldg(&pt.na);
+#pragma unroll
+      for (int h2 = 0; h2 < 2; ++h2) {               // markers (a = g, b = 2m) and (a = g, b = 2m + 1)
+        const int b = 2 * m + h2;
+        if (g < mnu && b < mnv) {
+          const double Uu = kt * (h2 ? uub : uua), Uv = kt * (h2 ? uvb : uva), Un = sd * (h2 ? unb : una);
+          float* om = o + (b * mnu + g) * 3;
+          __stcs(om, (float)fma(Uu, (double)ua.x, fma(Uv, (double)va.x, Un * (double)na.x)));
+          __stcs(om + 1, (float)fma(Uu, (double)ua.y, fma(Uv, (double)va.y, Un * (double)na.y)));
+          __stcs(om + 2, (float)fma(Uu, (double)ua.z, fma(Uv, (double)va.z, Un * (double)na.z)));
+        }
+      }
+    }
+  } else if (p.marker && gmcount > 0) {
     // hh / ha / pact were completed by the barrier above; this one retires the crosstalk reads of bufB (= S)
     if (NOISE) __syncthreads();
     for (int ch = 0; ch < nchunk; ++ch) {
@@ -1059,7 +1118,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
       }
       if (ch + 1 < nchunk) __syncthreads();  // S is reused by the next chunk
     }
-  }
+    }
 
 }
 
@@ -1115,7 +1174,7 @@ unsigned long long ts_bank_elems_per_grid(int N) { return (unsigned long long)(N
 
 unsigned long long ts_step_smem_bytes(const TsStepParams& p) {
   return (unsigned long long)p.frames_per_group * p.K * sizeof(FrameS) + sizeof(float) * 2 * TS_BLOCK +
-         sizeof(double) * 3 * TS_CHUNK + sizeof(int) * TS_MAX_GROUP_PATCHES;
+         (unsigned long long)p.s_bytes + sizeof(int) * TS_MAX_GROUP_PATCHES;
 }
 
 namespace {
