@@ -359,13 +359,23 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1
 //  * the angle is reduced EXACTLY in integers to [-pi, pi) (k_b is a 24-bit integer), then MUFU.SIN/COS
 //    (abs error ~4e-7 there).
 // Error of z <= ~1e-5 |z| + 4e-7 r, i.e. < 1e-8 N per step at sigma = 1e-3 N (tolerance 1e-6).
+__device__ __forceinline__ float lg2_ftz(float x) {  // MUFU.LG2 without the denormal fix-up of __log2f (x >= 2^-24 here)
+  float r;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float rsqrt_ftz(float x) {  // MUFU.RSQ without the denormal fix-up of rsqrtf (x >= 1e-7 here)
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
 __device__ __forceinline__ void box_muller(uint32_t wa, uint32_t wb, float& z0, float& z1) {
   const float ua = (float)(2u * (wa >> 9) + 1u) * 5.9604644775390625e-8f;
   const float v = 1.f - ua;  // exact
   const float Ls = 2.f * v * fmaf(v, fmaf(v, fmaf(v, 0.25f, 0.33333334f), 0.5f), 1.f);  // -2 ln(1-v), v < 1/64: rel 2e-9
-  const float Ll = -1.3862943611198906f * __log2f(ua);                                  // -2 ln 2 * log2 u
-  const float L = (v < 0.015625f) ? Ls : Ll;
-  const float r = L * rsqrtf(L);
+  const float Ll = -1.3862943611198906f * lg2_ftz(ua);                                  // -2 ln 2 * log2 u
+  const float L = (v < 0.015625f) ? Ls : Ll;                                           // L >= -2 ln(1 - 2^-24) = 1.2e-7
+  const float r = L * rsqrt_ftz(L);
   // angle 2 pi k_b / 2^24 mapped to [-pi, pi) by sign-extending the 24-bit integer (same sin / cos);
   // MUFU.SIN / MUFU.COS have an absolute error of ~4e-7 on that range
   const int kb = ((int)((2u * (wb >> 9) + 1u) << 8)) >> 8;
@@ -389,7 +399,7 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 
 #define TS_FULL 0xffffffffu
 #ifndef TS_MIN_BLOCKS
-#define TS_MIN_BLOCKS 5
+#define TS_MIN_BLOCKS 6
 #endif
 
 // ---------------------------------------------------------------------------------------
