@@ -37,6 +37,8 @@ struct ts_ctx {
   bool mk_mma = false;
   int32_t* g_type = nullptr;
   float4* g_params = nullptr;
+  void* frames_g = nullptr;       // [E][P*K] relative-pose frames of the current step (ts_frames_kernel -> ts_step_kernel)
+  int32_t* patch_link = nullptr;  // [P]
   int32_t* env_perm = nullptr;  // block -> env order of the step kernel (sorted by geometry; set by ts_set_geometry)
   float4* bank = nullptr;
   size_t bank_bytes = 0;
@@ -88,7 +90,7 @@ struct DeviceGuard {
 void free_all(ts_ctx* c) {
   cudaFree(c->tx_pos); cudaFree(c->tx_meta); cudaFree(c->mk_pos); cudaFree(c->mk_nrm); cudaFree(c->patches);
   cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->mk_tab8); cudaFree(c->grp_link);
-  cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->env_perm); cudaFree(c->bank); cudaFree(c->bank_stage); cudaFree(c->st_flags); cudaFree(c->st_hyst);
+  cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->env_perm); cudaFree(c->frames_g); cudaFree(c->patch_link); cudaFree(c->bank); cudaFree(c->bank_stage); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch); cudaFree(c->ft_scratch_r); cudaFree(c->st_ring);
   for (float* q : c->stage_in) cudaFree(q);
   for (void* q : c->stage_out) cudaFree(q);
@@ -122,7 +124,7 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   }
   p.env_id_base = (uint32_t)g.env_id_base;
   p.tx_pos = c->tx_pos; p.tx_meta = c->tx_meta; p.patches = c->patches; p.mk_pos = c->mk_pos; p.mk_nrm = c->mk_nrm;
-  p.g_type = c->g_type; p.g_params = c->g_params; p.bank = c->bank; p.env_perm = c->env_perm;
+  p.g_type = c->g_type; p.g_params = c->g_params; p.bank = c->bank; p.env_perm = c->env_perm; p.frames_g = c->frames_g; p.patch_link = c->patch_link;
   p.grid_n = c->grid_n; p.voxel = c->voxel; p.inv_voxel = 1.0f / c->voxel; p.inv_voxel_d = 1.0 / (double)c->voxel;
   p.grid_stride = ts_bank_elems_per_grid(c->grid_n);
   p.st_flags = c->st_flags; p.st_hyst = c->st_hyst; p.st_drift = c->st_drift;
@@ -182,7 +184,7 @@ void ts_config_default(ts_config* c) {
 const char* ts_last_error(const ts_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 int32_t ts_n_taxels(const ts_ctx* ctx) { return ctx ? ctx->T : 0; }
 int32_t ts_n_markers(const ts_ctx* ctx) { return ctx ? ctx->M : 0; }
-int32_t ts_launches_per_step(const ts_ctx* ctx) { return !ctx ? 0 : ((ctx->cfg.noise_enable && !ctx->fused) ? 2 : 1); }
+int32_t ts_launches_per_step(const ts_ctx* ctx) { return !ctx ? 0 : ((ctx->cfg.noise_enable && !ctx->fused) ? 3 : 2); }
 
 ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   if (!cfg || !out) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: NULL argument");
@@ -399,6 +401,8 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   TS_ALLOC(c->g_type, sizeof(int32_t) * EK);
   TS_ALLOC(c->g_params, sizeof(float4) * EK);
   TS_ALLOC(c->env_perm, sizeof(int32_t) * E);
+  TS_ALLOC(c->frames_g, (size_t)ts_frame_bytes() * E * pts.size() * cfg->objs_per_env);
+  TS_ALLOC(c->patch_link, sizeof(int32_t) * pts.size());
   TS_ALLOC(c->st_flags, E * T);
   TS_ALLOC(c->reset_step, sizeof(uint32_t) * E);
   TS_ALLOC(c->episode, sizeof(uint32_t) * E);
@@ -429,6 +433,11 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   cp(c->groups, groups.data(), sizeof(TsGroup) * groups.size());
   cp(c->chunks, chunks.data(), sizeof(TsChunk) * chunks.size());
   cp(c->grp_link, glink.data(), sizeof(int32_t) * glink.size());
+  {
+    std::vector<int32_t> plink(pts.size());
+    for (size_t pi = 0; pi < pts.size(); ++pi) plink[pi] = pts[pi].link;
+    cp(c->patch_link, plink.data(), sizeof(int32_t) * plink.size());
+  }
   cp(c->mk_item1, item1.data(), sizeof(int32_t) * item1.size());
   cp(c->mk_item2, item2.data(), sizeof(int32_t) * item2.size());
   cp(c->mk_tab, tab.data(), sizeof(double) * tab.size());
@@ -549,7 +558,8 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
     c->ev_used += 3;
     TS_CUDA(c, cudaEventRecord(e0, st));
   }
-  cudaError_t e = (cudaError_t)ts_launch_step(p, c->fused ? 1 : 0, st);
+  cudaError_t e = (cudaError_t)ts_launch_frames(p, st);
+  if (e == cudaSuccess) e = (cudaError_t)ts_launch_step(p, c->fused ? 1 : 0, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: launch");
   if (c->timing) TS_CUDA(c, cudaEventRecord(e1, st));
   if (split) {

@@ -87,6 +87,9 @@ struct TsStepParams {
   // geometry
   const int32_t* g_type;   // [E,K]
   const float4* g_params;  // [E,K]
+  void* frames_g;          // [E][P*K] FrameS (ts_kernels.cu): relative poses of every (env, patch, object), written by
+                           // ts_frames_kernel at the start of the step, bulk-copied (TMA) into shared memory by each block
+  const int32_t* patch_link;  // [P] sensor link of each patch (-1 = filler)
   const int32_t* env_perm; // [E] block -> env: envs ordered by (geometry type, grid id) so that the blocks resident at any
                            // time gather from ONE grid of the bank (L2-resident) and run one march loop; NULL = identity
   const float4* bank;      // re-tiled SDF bank (see ts_kernels.cu, "bank layout")
@@ -144,6 +147,8 @@ struct TsStepParams {
 // launchers (ts_kernels.cu)
 int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream);
 int ts_launch_noise(const TsStepParams& p, void* stream);
+int ts_launch_frames(const TsStepParams& p, void* stream);
+unsigned long long ts_frame_bytes();
 int ts_launch_retile(const float* src_linear, float4* dst, int n_grids, int N, void* stream);
 int ts_launch_reset_counters(uint32_t* reset_step, uint32_t* episode, const uint8_t* mask, int E, uint32_t gstep,
                              void* stream);

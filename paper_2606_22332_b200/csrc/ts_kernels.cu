@@ -160,6 +160,31 @@ __device__ __forceinline__ void build_frame_vec(const TsStepParams& p, int e, in
   dst[0] = o.x; dst[1] = o.y; dst[2] = o.z;
 }
 
+// Phase 0 as its own launch: one thread per (env, patch, object) builds the whole frame in registers and writes it to
+// frames_g[e][patch * K + k].  Inside the step kernel the same arithmetic sat in front of a block barrier and took
+// ~19 % of every block's lifetime (a ~250-instruction dependent double-precision chain behind a DRAM round trip, with
+// 6 of 8 warps waiting); here it is 410 k independent threads, and the step kernel's blocks receive their frames with
+// one TMA bulk copy.  Same functions, same operation order: bit-identical frames.
+__global__ void __launch_bounds__(128) ts_frames_kernel(const __grid_constant__ TsStepParams p) {
+  const int PK = p.P * p.K;
+  const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gt >= (long long)p.E * PK) return;
+  const int e = (int)(gt / PK), f = (int)(gt - (long long)e * PK);
+  const int pidx = f / p.K, k = f - pidx * p.K;
+  const int link = __ldg(p.patch_link + pidx);
+  FrameS F;
+#pragma unroll
+  for (int i = 0; i < (int)(sizeof(FrameS) / 4); ++i) reinterpret_cast<uint32_t*>(&F)[i] = 0u;
+#pragma unroll
+  for (int r = 0; r < 3; ++r) build_frame_row(p, e, link, pidx, k, r, F);
+#pragma unroll
+  for (int sub = 0; sub < 4; ++sub) build_frame_vec(p, e, link, k, sub, F);
+  uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<FrameS*>(p.frames_g) + gt);
+  const uint4* src = reinterpret_cast<const uint4*>(&F);
+#pragma unroll
+  for (int i = 0; i < (int)(sizeof(FrameS) / 16); ++i) dst[i] = src[i];
+}
+
 // ---------------------------------------------------------------------------------------
 // O2 in double: signed distance and (unnormalised, object-frame) gradient of one geometry at
 // the object-frame point x.  Used once per taxel (the first query).
@@ -395,6 +420,29 @@ __device__ __forceinline__ void store6(float* dst, const float* v) {
 // D (8 x 8) += A (8 x 4, row) B (4 x 8, col) on the FP64 tensor cores: lane = 4 g + m holds A[g][m], B[m][g], D[g][2m], D[g][2m+1].
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+// ---- TMA bulk copy global -> shared memory, completion on an mbarrier (cp.async.bulk, SASS UBLKCP) -------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@!p bra WAIT_%=;\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
 
 #define TS_FULL 0xffffffffu
@@ -823,20 +871,14 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     gstart = g0.x; gcount = g0.y; patch0 = g0.z; npatch = g0.w; chunk0 = g1.x; nchunk = g1.y; gmcount = g1.w;
   }
 
-  // ---- phase 0: relative poses (double) -> shared memory ---------------------------------
-  if (tid == 0) *pmask = 0u;
-  // The whole block waits for this, so its load chain is short: link ids come from a per-group table
-  // indexed by blockIdx alone, and unused frame slots carry link -1 (no dependence on the group record).
-  if (tid < TS_BLOCK / 2) {
-    for (int it = tid; it < 3 * nfr; it += TS_BLOCK / 2) {
-      const int f = it / 3, lpf = SINGLE ? f : f / p.K, k = f - lpf * p.K;
-      build_frame_row(p, e, p.inl ? p.inl_link[gi * p.inl_stride + lpf] : __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), patch0 + lpf, k, it - 3 * f, frames[f]);
-    }
-  } else {
-    for (int it = tid - TS_BLOCK / 2; it < 4 * nfr; it += TS_BLOCK / 2) {
-      const int f = it >> 2, lpf = SINGLE ? f : f / p.K, k = f - lpf * p.K;
-      build_frame_vec(p, e, p.inl ? p.inl_link[gi * p.inl_stride + lpf] : __ldg(p.grp_link + gi * TS_MAX_GROUP_PATCHES + lpf), k, it & 3, frames[f]);
-    }
+  // ---- phase 0: this block's relative poses arrive from frames_g (ts_frames_kernel) by ONE bulk copy (TMA) ------
+  __shared__ __align__(8) uint64_t fbar;
+  if (tid == 0) {
+    *pmask = 0u;
+    mbar_init(&fbar, 1);
+    const unsigned bytes = (unsigned)(npatch * p.K) * (unsigned)sizeof(FrameS);
+    mbar_expect_tx(&fbar, bytes);
+    bulk_g2s(frames, reinterpret_cast<const FrameS*>(p.frames_g) + ((size_t)e * p.P + patch0) * p.K, bytes, &fbar);
   }
   const bool valid = tid < gcount;
   const int j = gstart + (valid ? tid : 0);
@@ -848,7 +890,8 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const bool act = Rj > 0.f;
   uint8_t flag = valid ? p.st_flags[ej] : (uint8_t)0;
   if (NOISE && valid && (tid & 15) == 0) noise_prefetch<HM>(p, e, j);
-  __syncthreads();
+  __syncthreads();        // publishes the mbarrier (and pmask); every warp arrives within a few cycles of block start
+  mbar_wait(&fbar, 0u);   // frames landed in shared memory (async-proxy writes are visible after the wait)
 
   // ---- phase 1 (S1-S4): x_o = c + M x_j, phi = min_k phi_k, depth (Eq. 2), contact (Eq. 3) ----
   double phid = __longlong_as_double(0x7ff0000000000000LL);
@@ -1238,6 +1281,14 @@ int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
   const int hm = (p.noise_enable && fused_noise) ? (p.hyst_mode | (p.ext ? 4 : 0)) : -1;
   if (p.K == 1) launch_one<true>(p, hm, grid, smem, (cudaStream_t)stream);
   else launch_one<false>(p, hm, grid, smem, (cudaStream_t)stream);
+  return (int)cudaGetLastError();
+}
+
+unsigned long long ts_frame_bytes() { return sizeof(FrameS); }
+
+int ts_launch_frames(const TsStepParams& p, void* stream) {
+  const long long n = (long long)p.E * p.P * p.K;
+  ts_frames_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(p);
   return (int)cudaGetLastError();
 }
 

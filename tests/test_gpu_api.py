@@ -48,7 +48,7 @@ def test_kernel_time_introspection():
     assert n == 5 and 0.0 < ms < 50.0
     assert 0.0 < sim.first_kernel_time_ms() <= ms * 1.001
     # TS_SPLIT=1 selects the two-kernel variant (readout, then the stand-alone noise kernel)
-    assert sim.launches_per_step() == (2 if os.environ.get("TS_SPLIT") == "1" else 1)
+    assert sim.launches_per_step() == (3 if os.environ.get("TS_SPLIT") == "1" else 2)
     sim.step(inp, out)                         # recording is off again
     assert sim.kernel_time_ms(False) == (0.0, 0)
 

@@ -120,7 +120,7 @@ def test_config5_full_size_optional_knobs_sampled(monkeypatch):
     for split in ("0", "1"):
         monkeypatch.setenv("TS_SPLIT", split)
         sim = _sim(w, noise=noise)
-        assert sim.launches_per_step() == (2 if split == "1" else 1)
+        assert sim.launches_per_step() == (3 if split == "1" else 2)   # frames kernel + step kernel (+ noise kernel)
         for s in range(5):
             g = sim.step(sim.upload(w.inputs(s)))
         torch.cuda.synchronize()
@@ -251,7 +251,7 @@ def test_remaining_noise_knobs_reset_and_split(monkeypatch):
             cmp_.step({k: v.cpu().numpy() for k, v in g.items()}, orc.step(inp, want=w.outputs))
         rep = cmp_.report()
         _assert_ok(rep)
-        assert sim.launches_per_step() == (2 if split == "1" else 1)
+        assert sim.launches_per_step() == (3 if split == "1" else 2)   # frames kernel + step kernel (+ noise kernel)
         sim.close()
 
 
