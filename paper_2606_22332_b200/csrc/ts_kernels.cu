@@ -177,7 +177,10 @@ __global__ void __launch_bounds__(128) ts_frames_kernel(const __grid_constant__ 
 #pragma unroll
   for (int i = 0; i < (int)(sizeof(FrameS) / 4); ++i) reinterpret_cast<uint32_t*>(&F)[i] = 0u;
   if (gt < total) {
-    const int e = (int)(gt / PK), f = (int)(gt - (long long)e * PK);
+    // frames are stored in BLOCK order of the step kernel (row bx = frames of env env_perm[bx]), so that a block's bulk
+    // copy needs no env lookup in front of it and the rows of the blocks scheduled next sit at a fixed distance ahead
+    const int bx = (int)(gt / PK), f = (int)(gt - (long long)bx * PK);
+    const int e = p.env_perm ? __ldg(p.env_perm + bx) : bx;
     const int pidx = f / p.K, k = f - pidx * p.K;
     const int link = __ldg(p.patch_link + pidx);
 #pragma unroll
@@ -472,6 +475,12 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
 }
 
 #define TS_FULL 0xffffffffu
+#ifndef TS_HYST_STORE_LATE
+#define TS_HYST_STORE_LATE 1
+#endif
+#ifndef TS_PF_AHEAD
+#define TS_PF_AHEAD 1184  // blocks: ~1.3 waves of 6 resident blocks x 148 SMs
+#endif
 #ifndef TS_MIN_BLOCKS
 #define TS_MIN_BLOCKS 6
 #endif
@@ -530,16 +539,18 @@ __device__ __forceinline__ void noise_load(const TsStepParams& p, int e, int j, 
 // holding them in registers across the march cost spills at 48 registers per thread (measured 1.48 ->
 // 1.41 ms on config 5), and an L2 hit is short enough for 40 resident warps to cover.
 template <int HM>
-__device__ __forceinline__ void noise_prefetch(const TsStepParams& p, int e, int j) {
+__device__ __forceinline__ void noise_prefetch(const TsStepParams& p, int e, int j0, int jend, int lane) {
+  // One request per 128-byte line of the warp's state rows: lane = 2 * row + half (a warp's 32 slots are 256 bytes of a
+  // float2 row); every lane forms ONE address (the earlier form had every 16th lane walk all rows: 18 issue slots).
   constexpr int MODE = HM & 3;
-  const unsigned Tp = (unsigned)p.Tp;
-  const float2* sh = reinterpret_cast<const float2*>(p.st_hyst) + ((unsigned)e * (MODE == TS_HYST_MAXWELL ? 6u : 3u) * Tp + (unsigned)j);
-  const float2* sd = reinterpret_cast<const float2*>(p.st_drift) + ((unsigned)e * 3u * Tp + (unsigned)j);
-#pragma unroll
-  for (int c = 0; c < (MODE == TS_HYST_MAXWELL ? 6 : (MODE == TS_HYST_ASYM ? 3 : 0)); ++c)
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(sh + c * Tp));
-#pragma unroll
-  for (int c = 0; c < 3; ++c) asm volatile("prefetch.global.L2 [%0];" ::"l"(sd + c * Tp));
+  constexpr int NH = MODE == TS_HYST_MAXWELL ? 6 : (MODE == TS_HYST_ASYM ? 3 : 0);
+  const int r = lane >> 1, jj = j0 + (lane & 1) * 16;
+  if (r < NH + 3 && jj < jend) {
+    const unsigned Tp = (unsigned)p.Tp;
+    const float2* row = r < NH ? reinterpret_cast<const float2*>(p.st_hyst) + ((unsigned)e * (unsigned)NH + (unsigned)r) * Tp
+                               : reinterpret_cast<const float2*>(p.st_drift) + ((unsigned)e * 3u + (unsigned)(r - NH)) * Tp;
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(row + jj));
+  }
 }
 
 // Every thread of the block must call this (it contains one __syncthreads).
@@ -574,7 +585,8 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
       const float al = (fabsf(x[c]) > fabsf(yp)) ? p.alpha_load : p.alpha_unload;
       h[c] = act ? fmaf(al, x[c] - yp, yp) : 0.f;
     }
-    if (valid) {
+    // the new state (= h) is written back AFTER the exchange barrier below (TS_HYST_STORE_LATE)
+    if (!TS_HYST_STORE_LATE && valid) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) __stcs(st_h + (ih + c * Tp), make_float2(h[2 * c], h[2 * c + 1]));
     }
@@ -620,6 +632,10 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
     box_muller(w1.x, w1.y, zw[4], zw[5]);
   }
   __syncthreads();
+  if (TS_HYST_STORE_LATE && MODE == TS_HYST_ASYM && valid) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) __stcs(st_h + (ih + c * Tp), make_float2(h[2 * c], h[2 * c + 1]));
+  }
   // S8c crosstalk (D4): c_j = h_j + chi/4 sum_{k in N4(j)} (h_k - h_j); a missing neighbour is
   // replaced by the taxel itself (h_j - h_j = 0), so the sum needs no predicates.
   const int nu = (meta >> 8) & 255;  // slots of a patch are consecutive: -u/+u = tid -/+ 1, -v/+v = tid -/+ nu
@@ -909,7 +925,12 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     mbar_init(&fbar, 1);
     const unsigned bytes = (unsigned)(npatch * p.K) * (unsigned)sizeof(FrameS);
     mbar_expect_tx(&fbar, bytes);
-    bulk_g2s(frames, reinterpret_cast<const FrameS*>(p.frames_g) + ((size_t)e * p.P + patch0) * p.K, bytes, &fbar);
+    const FrameS* src = reinterpret_cast<const FrameS*>(p.frames_g) + ((size_t)blockIdx.x * p.P + patch0) * p.K;
+    bulk_g2s(frames, src, bytes, &fbar);
+    // L2 prefetch of the same rows for the block TS_PF_AHEAD positions later in launch order (blockIdx.x runs fastest):
+    // by the time that block starts, its bulk copy is an L2 hit instead of a DRAM round trip in front of phase 1.
+    if (TS_PF_AHEAD > 0 && blockIdx.x + TS_PF_AHEAD < gridDim.x)
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src + (size_t)TS_PF_AHEAD * p.P * p.K), "r"(bytes) : "memory");
   }
   const bool valid = tid < gcount;
   const int j = gstart + (valid ? tid : 0);
@@ -920,7 +941,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const float Rj = valid ? P4.w : 0.f;  // R_j = 0: inactive slot
   const bool act = Rj > 0.f;
   uint8_t flag = valid ? p.st_flags[ej] : (uint8_t)0;
-  if (NOISE && valid && (tid & 15) == 0) noise_prefetch<HM>(p, e, j);
+  if (NOISE) noise_prefetch<HM>(p, e, gstart + (tid & ~31), gstart + gcount, tid & 31);
   __syncthreads();        // publishes the mbarrier (and pmask); every warp arrives within a few cycles of block start
   mbar_wait(&fbar, 0u);   // frames landed in shared memory (async-proxy writes are visible after the wait)
 
