@@ -482,7 +482,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
 #define TS_PF_AHEAD 1184  // blocks: ~1.3 waves of 6 resident blocks x 148 SMs
 #endif
 #ifndef TS_MIN_BLOCKS
-#define TS_MIN_BLOCKS 6
+#define TS_MIN_BLOCKS 5
 #endif
 
 // ---------------------------------------------------------------------------------------
