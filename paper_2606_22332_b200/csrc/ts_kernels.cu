@@ -481,6 +481,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
 #ifndef TS_PF_AHEAD
 #define TS_PF_AHEAD 1184  // blocks: ~1.3 waves of 6 resident blocks x 148 SMs
 #endif
+#ifndef TS_GRID_GFAST
+#define TS_GRID_GFAST 1  // launch order: the patch groups of one env are adjacent (its frames, state and output rows are touched together)
+#endif
 #ifndef TS_MIN_BLOCKS
 #define TS_MIN_BLOCKS 5
 #endif
@@ -906,8 +909,14 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   unsigned* pmask = reinterpret_cast<unsigned*>(ha + TS_BLOCK);  // bit l: group-local patch l has penetration
 
   const int tid = threadIdx.x;
-  const int e = p.env_perm ? __ldg(p.env_perm + blockIdx.x) : (int)blockIdx.x;
+#if TS_GRID_GFAST
+  const unsigned bxi = blockIdx.x / (unsigned)p.G;
+  const int gi = (int)(blockIdx.x - bxi * (unsigned)p.G);
+#else
+  const unsigned bxi = blockIdx.x;
   const int gi = blockIdx.y;
+#endif
+  const int e = p.env_perm ? __ldg(p.env_perm + bxi) : (int)bxi;
   int gstart, gcount, patch0, npatch, chunk0, nchunk, gmcount;
   if (p.inl) {  // group record from the parameter space (constant bank)
     const TsGroup& g = p.inl_grp[gi];
@@ -925,12 +934,13 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     mbar_init(&fbar, 1);
     const unsigned bytes = (unsigned)(npatch * p.K) * (unsigned)sizeof(FrameS);
     mbar_expect_tx(&fbar, bytes);
-    const FrameS* src = reinterpret_cast<const FrameS*>(p.frames_g) + ((size_t)blockIdx.x * p.P + patch0) * p.K;
+    const FrameS* src = reinterpret_cast<const FrameS*>(p.frames_g) + ((size_t)bxi * p.P + patch0) * p.K;
     bulk_g2s(frames, src, bytes, &fbar);
     // L2 prefetch of the same rows for the block TS_PF_AHEAD positions later in launch order (blockIdx.x runs fastest):
     // by the time that block starts, its bulk copy is an L2 hit instead of a DRAM round trip in front of phase 1.
-    if (TS_PF_AHEAD > 0 && blockIdx.x + TS_PF_AHEAD < gridDim.x)
-      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src + (size_t)TS_PF_AHEAD * p.P * p.K), "r"(bytes) : "memory");
+    constexpr unsigned AH = TS_GRID_GFAST ? TS_PF_AHEAD / 4 : TS_PF_AHEAD;
+    if (TS_PF_AHEAD > 0 && bxi + AH < (unsigned)p.E)
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src + (size_t)AH * p.P * p.K), "r"(bytes) : "memory");
   }
   const bool valid = tid < gcount;
   const int j = gstart + (valid ? tid : 0);
@@ -1329,7 +1339,11 @@ int ts_prepare_kernels(int max_smem_bytes) {
 int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
   if (p.E <= 0 || p.G <= 0 || p.G > 65535) return (int)cudaErrorInvalidConfiguration;
   const size_t smem = (size_t)ts_step_smem_bytes(p);
+#if TS_GRID_GFAST
+  const dim3 grid((unsigned)p.E * (unsigned)p.G, 1u);
+#else
   const dim3 grid((unsigned)p.E, (unsigned)p.G);
+#endif
   const int hm = (p.noise_enable && fused_noise) ? (p.hyst_mode | (p.ext ? 4 : 0)) : -1;
   if (p.K == 1) launch_one<true>(p, hm, grid, smem, (cudaStream_t)stream);
   else launch_one<false>(p, hm, grid, smem, (cudaStream_t)stream);
