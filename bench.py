@@ -15,9 +15,11 @@ environments are independent); rank r uses env_id_base = r*E so Philo
              CUDA events on the launch stream, barrier + synchronize on both sides, max over ranks.
 `e2e`        the same metric through ts_step_host(): pinned HOST inputs and outputs, H2D + kernel +
              D2H of every requested output inside the timed region.
-`roofline`   dominant (only) kernel ts_step_kernel: algorithmic bytes (DESIGN.md, 167 B per
-             env-taxel with ASYM hysteresis) / mean kernel duration from CUDA events recorded
-             around the launch inside ts_step (ts_kernel_time_ms), vs MEASURED_PEAKS.json hbm_gbs.
+`roofline`   the step's kernels (ts_frames_kernel + ts_step_kernel): algorithmic bytes (DESIGN.md, 169 B per
+             env-taxel with ASYM hysteresis) / mean duration of ALL kernels of a step from CUDA events recorded
+             around every launch inside ts_step (a second pass over the same steps with recording on), vs
+             MEASURED_PEAKS.json hbm_gbs; per-step median / p10 / p90, per-kernel means and the kernels' own
+             %globaltimer span (first block start to last block end) are reported beside it.
 `cpu_baseline` the oracle (oracle/, as it stands) on this box's host cores over the 16-env parity
              subset of the same workload; a reported baseline, not the target.
 --impl reference: the oracle arm (this tier has no reference implementation): each step is the
@@ -40,8 +42,9 @@ if ROOT not in sys.path:
 METRIC = "env_taxel_updates_per_sec"
 UNIT = "env*taxel/s"
 # SURVEY 8d / DESIGN.md "algorithmic bytes": per (env, taxel) per step, everything on.
-# ncu --set full capture of ts_step_kernel at this workload (profiles/): dram bytes per launch.
-TRAFFIC_FILE = os.path.join(ROOT, "profiles", "traffic_config5.txt")
+# ncu --set full capture of ts_step_kernel at this workload: DRAM bytes per launch and L2 hit rate, copied from the
+# committed capture summary named in the file (a profile run, never measured inside this benchmark).
+NCU_FILE = os.path.join(ROOT, "profiles", "ncu_config%d.txt")
 
 
 def algorithmic_bytes_per_taxel(w, T, L, K, M):
@@ -66,16 +69,20 @@ def hbm_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def recorded_traffic():
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture."""
+def recorded_ncu(config):
+    """{traffic_bytes_per_launch, lts_hit_rate_pct, l1_hit_rate_pct, source} from the committed ncu --set full capture
+    of this config's step kernel (profiles/ncu_config<N>.txt), or {} if none is committed."""
+    out = {}
     try:
-        with open(TRAFFIC_FILE) as f:
+        with open(NCU_FILE % config) as f:
             for line in f:
-                if line.startswith("traffic_bytes_per_launch"):
-                    return float(line.split()[1])
+                if line.startswith("#") or not line.strip():
+                    continue
+                k, v = line.split(None, 1)
+                out[k] = v.strip()
     except OSError:
         pass
-    return None
+    return out
 
 
 class ClockSampler:
@@ -219,7 +226,6 @@ def main():
         for s in range(8):
             sim.step(dev_in[s % n_distinct], out)
         torch.cuda.synchronize(dev)
-    sim.kernel_time_ms(True)                               # start recording per-launch events inside ts_step
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record(stream)
@@ -228,8 +234,20 @@ def main():
     ev1.record(stream)
     barrier()
     total_ms = ev0.elapsed_time(ev1)
+    # second pass over the same K steps with per-launch recording on (CUDA events around every kernel inside ts_step,
+    # on the step's stream, plus the kernels' own %globaltimer stamps): the per-kernel numbers behind `roofline`
+    sim.kernel_time_ms(1)                                  # one pair of events around the kernels of each step
+    for s in range(Wm, Wm + K):
+        sim.step(dev_in[s % n_distinct], out)
+    barrier()
     clk = clocks.stop()
-    kern_ms, kern_n = sim.kernel_time_ms(False)
+    whole = sim.kernel_times_ms()                          # [K, 4]: column 1 = all kernels of the step, 3 = device-side clock
+    kern_ms, kern_n = sim.kernel_time_ms(2)                # third pass: events between the kernels too (per-kernel split)
+    for s in range(Wm, Wm + K):
+        sim.step(dev_in[s % n_distinct], out)
+    barrier()
+    per_step = sim.kernel_times_ms()                       # [K, 4]: frames, step, noise kernel; device-side clock span
+    sim.kernel_time_ms(False)
     first_ms = sim.first_kernel_time_ms()
     launches = K * sim.launches_per_step()
     # how much contact / march work the scene carries (last timed step, this rank): belongs next to the timing
@@ -265,9 +283,24 @@ def main():
     bpt = algorithmic_bytes_per_taxel(w, T, w.L, w.K, M)
     peak, peak_src = hbm_peak()
     achieved = bpt * E * T / (kern_ms * 1e-3) / 1e9 if kern_ms > 0 else 0.0
-    roof = {"bound": "hbm", "kernel": "ts_step_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak, "traffic": recorded_traffic(), "algorithmic_bytes_per_launch": bpt * E * T,
-            "bytes_per_env_taxel": bpt, "kernel_ms": kern_ms, "first_kernel_ms": first_ms, "kernel_launches_timed": kern_n, "peak_source": peak_src,
+    ncu = recorded_ncu(a.config) if not a.noise_knobs and not a.envs else {}
+    tot = whole[:, 1] if len(whole) else np.zeros(1)
+    pct = lambda v: {"median": float(np.median(v)), "p10": float(np.percentile(v, 10)), "p90": float(np.percentile(v, 90))}
+    # `achieved` divides the step's algorithmic bytes by the duration of ALL kernels of the step (frames kernel + step
+    # kernel [+ noise kernel]): the frames kernel's intermediate bytes count as time, not as useful bytes.
+    roof = {"bound": "hbm", "kernel": "ts_frames_kernel + ts_step_kernel" + (" + ts_noise_kernel" if sim.launches_per_step() == 3 else ""),
+            "achieved": achieved, "peak": peak, "unit": "GB/s",
+            "frac": achieved / peak,
+            "traffic": float(ncu["traffic_bytes_per_launch"]) if "traffic_bytes_per_launch" in ncu else None,
+            "traffic_source": ncu.get("source"),
+            "l2_hit_rate_pct": float(ncu["lts_hit_rate_pct"]) if "lts_hit_rate_pct" in ncu else None,
+            "algorithmic_bytes_per_launch": bpt * E * T,
+            "bytes_per_env_taxel": bpt, "kernel_ms": kern_ms, "kernel_ms_stats": pct(tot),
+            "kernels_ms_mean": {"ts_frames_kernel": float(per_step[:, 0].mean()) if len(per_step) else None,
+                                "ts_step_kernel": float(per_step[:, 1].mean()) if len(per_step) else None,
+                                "ts_noise_kernel": float(per_step[:, 2].mean()) if len(per_step) else None},
+            "device_clock_ms_stats": pct(whole[:, 3]) if len(whole) else None,
+            "kernel_launches_timed": kern_n, "peak_source": peak_src,
             "frac_of_nominal_8TBs": achieved / 8000.0}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
@@ -292,10 +325,13 @@ def main():
         v1, ms1 = oracle_arm(w, ids, 1, 1, threads)
         n = int(max(2, min(200, a.cpu_seconds * 1e3 / max(ms1, 1e-3))))
         v, ms = oracle_arm(w, ids, n, 1, threads)
+        n1 = int(max(1, min(50, 0.25 * a.cpu_seconds * 1e3 / max(ms1 * threads, 1e-3))))
+        v_st, ms_st = oracle_arm(w, ids, n1, 1, 1)             # the same oracle on ONE thread (SURVEY 8d asks for both)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
                                 "sample": "%d envs %s x %d taxels, %d steps, OpenMP over envs; %.1f ms per 16-env step "
                                           "(x%d envs/16 = %.0f ms per full step, linear extrapolation)"
-                                          % (len(ids), ids.tolist(), T, n, ms, E, ms * E / len(ids))}
+                                          % (len(ids), ids.tolist(), T, n, ms, E, ms * E / len(ids)),
+                                "single_thread": {"value": v_st, "unit": UNIT, "cores": 1, "steps": n1, "ms_per_16env_step": ms_st}}
     if rank == 0:
         print(json.dumps(line))
     sim.close()

@@ -21,7 +21,10 @@
  * Threading: calls on one ctx are not thread-safe.  Streams: every device operation of
  * ts_set_geometry / ts_step / ts_reset is enqueued on the caller's stream (a cudaStream_t
  * passed as void*; NULL = the legacy default stream); none of them synchronises except where
- * stated.  Errors: every call returns a ts_status; nothing throws, aborts or prints.
+ * stated.  The ctx keeps state between calls (Schmitt bits, hysteresis, drift, counters, the
+ * frames of the step in flight), so successive calls on one ctx must be ordered: use ONE stream,
+ * or order the streams yourself with events; the library does not check this.
+ * Errors: every call returns a ts_status; nothing throws, aborts or prints.
  */
 #ifndef TS_H_
 #define TS_H_
@@ -105,7 +108,14 @@ ts_status ts_layout_destroy(ts_layout* lay); /* NULL is a no-op */
  * ------------------------------------------------------------------------------------- */
 enum { TS_HYST_OFF = 0, TS_HYST_MAXWELL = 1 /* Eq. 29-30 */, TS_HYST_ASYM = 2 /* DESIGN.md D3 */ };
 
-enum {                      /* output_mask bits; a bit set with a NULL pointer is an error */
+/* How ts_step runs the noise chain (App. A.8): inside the step kernel (one launch after the frames kernel) or as a
+ * separate kernel behind it.  AUTO = fused for the four knobs of drift / hysteresis / dead taxels / 4-neighbour
+ * crosstalk, split when any further A.8 knob is set (the fused variant with every knob exceeds the instruction
+ * cache).  Both forms compute bit-identical results. */
+enum { TS_FORM_AUTO = 0, TS_FORM_FUSED = 1, TS_FORM_SPLIT = 2 };
+
+enum {                      /* output_mask bits.  ts_step contract: every output whose bit is set must be given (non-NULL)
+                               and every output whose bit is clear must be NULL; anything else is TS_ERR_INVALID_ARG */
   TS_OUT_CONTACT = 1 << 0,  /* Eq. 3   uint8 [E,T] */
   TS_OUT_DEPTH = 1 << 1,    /* Eq. 2   f32   [E,T] */
   TS_OUT_FT = 1 << 2,       /* Eq. 8-9 f32   [E,T,6] (f_x,f_y,f_z,tau_x,tau_y,tau_z), link frame */
@@ -119,7 +129,8 @@ typedef struct ts_config {
   int32_t n_envs;        /* E >= 1 */
   int32_t n_links;       /* L >= 1 */
   int32_t objs_per_env;  /* K >= 1 */
-  int64_t env_id_base;   /* global id of env 0 (Philox counters use env_id_base + e; multi-GPU sharding) */
+  int64_t env_id_base;   /* global id of env 0 (Philox counters use env_id_base + e; multi-GPU sharding);
+                            0 <= env_id_base and env_id_base + n_envs <= 2^32 (the counter word is 32 bits) */
   const ts_layout* layout; /* finalised; copied to the device, may be destroyed afterwards */
   /* KinematicTaxel, Eq. 10: k_n=500 c_n=1 alpha=1.2 k_t=2 k_omega=2; mu = Coulomb cap
    * (INFINITY reproduces Eq. 8 exactly); use_velocity = 0 drops the velocity terms. */
@@ -164,6 +175,7 @@ typedef struct ts_config {
    * 0 <= read_delay, read_jitter and read_delay + read_jitter <= 64; the ctx holds that many past fields
    * (24 B x n_envs x n_taxels each). */
   int32_t read_delay, read_jitter;
+  int32_t kernel_form;   /* TS_FORM_* (0 = AUTO) */
 } ts_config;
 
 /* Fills *cfg with the paper's constants and everything else zero / off. */
@@ -181,7 +193,9 @@ typedef struct ts_geometry {
                            (axis = local z) | SDF: grid id in params[0] */
   int32_t n_grids;      /* G >= 0 */
   int32_t grid_n;       /* N: nodes per axis, 2 <= N <= 512 (all grids alike) */
-  float voxel;          /* h_v [m]; node i sits at (i - (N-1)/2) h_v on each axis */
+  float voxel;          /* h_v [m]; node i sits at (i - (N-1)/2) h_v on each axis: every grid is centred on its object's
+                           frame origin (there is no per-grid origin[3]: an offset grid is expressed by the object pose
+                           the caller passes each step, which the path applies anyway, Q26) */
   const float* grids;   /* [G,N,N,N] fp32 signed distance, x fastest: index (k*N + j)*N + i */
 } ts_geometry;
 
@@ -244,13 +258,22 @@ int32_t ts_n_taxels(const ts_ctx* ctx);
 int32_t ts_n_markers(const ts_ctx* ctx);
 /* Number of kernel launches one ts_step enqueues with the ctx's current configuration. */
 int32_t ts_launches_per_step(const ts_ctx* ctx);
-/* Records CUDA events around the main kernel of every subsequent ts_step (on the step's own
- * stream) and returns the mean duration in ms of the steps since the last call (after
- * synchronising those events).  enable = 0 switches recording off.  *n_steps gets the count. */
+/* Kernel timing.  With recording on, ts_step brackets its launches with CUDA events on the step's own stream (a fixed
+ * pool of TS_TIMING_MAX_STEPS slots created when recording is switched on; further steps are not recorded, nothing is
+ * ever allocated inside ts_step).  ts_kernel_time_ms synchronises the recorded events, returns the MEAN duration in ms
+ * of all kernels of a step over the steps recorded since the last call, and sets recording to `enable`: 0 = off,
+ * 1 = one pair of events around the kernels of a step (the whole step lands in the step-kernel column below),
+ * 2 = events between the kernels as well (per-kernel durations; the extra records cost a few microseconds per step).
+ * ts_kernel_times_ms (call it BEFORE ts_kernel_time_ms, which clears the record) copies the per-step durations:
+ * out_ms[4 * i + 0] = frames kernel, + 1 = step kernel, + 2 = separate noise kernel (0 when fused), from the CUDA
+ * events, and + 3 = the step's span on the DEVICE-SIDE clock: %globaltimer at the start of the first block of the
+ * frames kernel to %globaltimer at the end of the last block of the step's last kernel (written by the kernels
+ * themselves while recording is on), for i < min(recorded, capacity); *n_steps gets the number recorded. */
+enum { TS_TIMING_MAX_STEPS = 4096 };
 ts_status ts_kernel_time_ms(ts_ctx* ctx, int32_t enable, float* mean_ms, int32_t* n_steps);
-/* Mean duration in ms of the FIRST kernel of a step (the geometry / fused kernel) over the steps the
- * last ts_kernel_time_ms call averaged; the remainder of mean_ms is the separate noise kernel
- * (0 when the step is one fused launch). */
+ts_status ts_kernel_times_ms(ts_ctx* ctx, float* out_ms, int32_t capacity, int32_t* n_steps);
+/* Mean duration in ms of the frames kernel + the step kernel over the steps the last ts_kernel_time_ms call averaged;
+ * the remainder of its mean_ms is the separate noise kernel (0 when the noise chain is fused). */
 float ts_first_kernel_time_ms(const ts_ctx* ctx);
 
 const char* ts_version(void);

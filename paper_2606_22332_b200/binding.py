@@ -15,6 +15,7 @@ TS_OK = 0
 STATUS = {0: "TS_OK", 1: "TS_ERR_INVALID_ARG", 2: "TS_ERR_CUDA", 3: "TS_ERR_OOM", 4: "TS_ERR_STATE",
           5: "TS_ERR_UNSUPPORTED"}
 HYST = {"off": 0, "maxwell": 1, "asym": 2}
+FORM = {"auto": 0, "fused": 1, "split": 2}
 GEOM = {"none": 0, "sphere": 1, "box": 2, "capsule": 3, "sdf": 4, "grid": 4}
 OUT_BITS = {"contact": 1, "depth": 2, "ft": 4, "marker": 8, "prox": 16, "ft_noisy": 32, "dead": 64}
 
@@ -22,7 +23,7 @@ OUT_BITS = {"contact": 1, "depth": 2, "ft": 4, "marker": 8, "prox": 16, "ft_nois
 SYMBOLS = ["ts_layout_create", "ts_layout_add_patch", "ts_layout_filter_links", "ts_layout_finalize", "ts_layout_get",
            "ts_layout_destroy", "ts_config_default", "ts_create", "ts_set_geometry", "ts_step", "ts_step_host",
            "ts_reset", "ts_destroy", "ts_last_error", "ts_n_taxels", "ts_n_markers", "ts_launches_per_step",
-           "ts_kernel_time_ms", "ts_first_kernel_time_ms", "ts_version"]
+           "ts_kernel_time_ms", "ts_kernel_times_ms", "ts_first_kernel_time_ms", "ts_version"]
 
 
 class TsError(RuntimeError):
@@ -64,7 +65,8 @@ class Config(C.Structure):
                 ("gain_min", C.c_float), ("gain_max", C.c_float),
                 ("stuck_min_force", C.c_float), ("stuck_max_force", C.c_float),
                 ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float), ("xtalk_sigma", C.c_float),
-                ("radius_noise", C.c_float), ("read_delay", C.c_int32), ("read_jitter", C.c_int32)]
+                ("radius_noise", C.c_float), ("read_delay", C.c_int32), ("read_jitter", C.c_int32),
+                ("kernel_form", C.c_int32)]
 
 
 class Geometry(C.Structure):
@@ -115,6 +117,7 @@ def lib():
         L.ts_n_markers.argtypes = [vp]
         L.ts_launches_per_step.argtypes = [vp]
         L.ts_kernel_time_ms.argtypes = [vp, i32, C.POINTER(C.c_float), C.POINTER(i32)]
+        L.ts_kernel_times_ms.argtypes = [vp, vp, i32, C.POINTER(i32)]
         L.ts_first_kernel_time_ms.argtypes = [vp]
         L.ts_first_kernel_time_ms.restype = C.c_float
         L.ts_version.restype = C.c_char_p
@@ -192,7 +195,13 @@ def make_config(n_envs, n_links, objs_per_env, layout, physics=None, noise=None,
                 raise KeyError(k)
             if k == "hyst_mode" and isinstance(v, str):
                 v = HYST[v]
+            if k == "kernel_form" and isinstance(v, str):
+                v = FORM[v]
             setattr(cfg, k, v)
+    # test override only: TS_SPLIT=0 / 1 in the environment forces the fused / two-kernel form when the caller left
+    # kernel_form on AUTO (the C library itself reads no environment variable)
+    if cfg.kernel_form == 0 and os.environ.get("TS_SPLIT") in ("0", "1"):
+        cfg.kernel_form = FORM["split"] if os.environ["TS_SPLIT"] == "1" else FORM["fused"]
     if outputs is not None:
         cfg.output_mask = sum(OUT_BITS[o] for o in outputs)
     return cfg
@@ -295,9 +304,19 @@ class TactileSim:
         _check(lib().ts_reset(self.h, ptr, self._stream()), self.h, "ts_reset")
 
     def kernel_time_ms(self, enable=True):
+        """enable: False / 0 = off, True / 1 = events around the whole step, 2 = events between its kernels too."""
         ms, n = C.c_float(), C.c_int32()
         _check(lib().ts_kernel_time_ms(self.h, int(enable), C.byref(ms), C.byref(n)), self.h, "ts_kernel_time_ms")
         return ms.value, n.value
+
+    def kernel_times_ms(self):
+        """Per-step durations [n, 4] recorded since recording was switched on: frames, step, noise kernel (CUDA events)
+        and the step's span on the device-side clock (%globaltimer, first block start to last block end), in ms."""
+        n = C.c_int32()
+        _check(lib().ts_kernel_times_ms(self.h, None, 0, C.byref(n)), self.h, "ts_kernel_times_ms")
+        out = np.zeros((max(n.value, 1), 4), np.float32)
+        _check(lib().ts_kernel_times_ms(self.h, out.ctypes.data_as(C.c_void_p), n.value, C.byref(n)), self.h, "ts_kernel_times_ms")
+        return out[:n.value]
 
     def first_kernel_time_ms(self):
         return float(lib().ts_first_kernel_time_ms(self.h))

@@ -55,13 +55,16 @@ struct ts_ctx {
   void* stage_out[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   // timing of the main kernel
   bool timing = false;
-  std::vector<cudaEvent_t> ev;  // triples: before the step kernel, after it, after the noise kernel
+  bool timing_detail = false;   // events between the kernels of a step too (enable = 2)
+  std::vector<cudaEvent_t> ev;  // 4 per step: before the frames kernel, after it, after the step kernel, after the noise kernel;
+                                // fixed pool of 4 * TS_TIMING_MAX_STEPS created when recording is switched on
   float last_first_kernel_ms = 0.f;
   bool fused = true;            // one fused launch (default) or geometry + noise kernels (TS_SPLIT=1)
   float* ft_scratch = nullptr;  // clean ft for the noise kernel when the caller does not ask for ft
   float* st_ring = nullptr;       // Eq. 25 read delay: the last read_delay + read_jitter post-crosstalk fields
   float* ft_scratch_r = nullptr;  // two-kernel variant with radius noise: Eq. 4-9 at the perturbed depth (Eq. 26)
   size_t ev_used = 0;
+  unsigned long long* clock_buf = nullptr;  // [TS_TIMING_MAX_STEPS][2] device-side clock stamps (allocated with the event pool)
   std::string err;
 };
 
@@ -95,6 +98,7 @@ void free_all(ts_ctx* c) {
   for (float* q : c->stage_in) cudaFree(q);
   for (void* q : c->stage_out) cudaFree(q);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  cudaFree(c->clock_buf);
 }
 
 // 1 = a knob beyond the four of configs 4-5 is set: selects the kernel variants that carry them (HM | 4).
@@ -194,6 +198,9 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   if (cfg->n_envs < 1 || cfg->n_links < 1 || cfg->objs_per_env < 1)
     return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: n_envs, n_links, objs_per_env must be >= 1");
   if (!(cfg->eta_off <= cfg->eta_on)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: eta_off > eta_on");
+  if (cfg->kernel_form < TS_FORM_AUTO || cfg->kernel_form > TS_FORM_SPLIT) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: kernel_form");
+  if (cfg->env_id_base < 0 || cfg->env_id_base + (int64_t)cfg->n_envs > (1LL << 32))
+    return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: need 0 <= env_id_base and env_id_base + n_envs <= 2^32 (32-bit Philox counter word)");
   if (cfg->march_steps < 0 || cfg->march_steps > 64) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: march_steps not in 0..64");
   if (!(cfg->alpha > 0.f) || !(cfg->r_prox >= 0.f) || !(cfg->lambda_d > 0.f) || !(cfg->c_e >= 0.f && cfg->c_e <= 1.f))
     return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: physics parameter out of range");
@@ -376,7 +383,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     fill_params(c, sp);
     const unsigned long long smem = ts_step_smem_bytes(sp);
     if (smem > 200 * 1024) { delete c; return fail(nullptr, TS_ERR_UNSUPPORTED, "ts_create: objs_per_env too large for the shared-memory frames"); }
-    const cudaError_t ea = (cudaError_t)ts_prepare_kernels((int)smem);
+    const cudaError_t ea = (cudaError_t)ts_prepare_kernels(cuda_device, (int)smem);
     if (ea != cudaSuccess) { ts_status s_ = cuda_fail(nullptr, ea, "cudaFuncSetAttribute"); delete c; return s_; }
   }
 
@@ -406,14 +413,9 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   TS_ALLOC(c->st_flags, E * T);
   TS_ALLOC(c->reset_step, sizeof(uint32_t) * E);
   TS_ALLOC(c->episode, sizeof(uint32_t) * E);
-  {
-    const char* sp = std::getenv("TS_SPLIT");
-    // Default: one fused launch, except when optional A.8 knobs are on: the fused variant that carries them executes
-    // 46.7 KB of SASS per block (41.9 KB without them), past the instruction-cache knee (ncu: no_instruction stall
-    // 0.27 -> 2.97 cycles per issue), and the two-kernel form is 0.1-0.2 ms faster on config 5 (measured, DESIGN.md
-    // section 6).  TS_SPLIT=0 / 1 forces either form.
-    c->fused = sp ? (sp[0] != '1') : !(TS_DEFAULT_SPLIT || cfg_ext(*cfg));
-  }
+  // Default (TS_FORM_AUTO): one fused launch, except when optional A.8 knobs are on: the fused variant that carries them
+  // runs past the instruction-cache knee and the two-kernel form is faster.
+  c->fused = cfg->kernel_form == TS_FORM_FUSED ? true : (cfg->kernel_form == TS_FORM_SPLIT ? false : !(TS_DEFAULT_SPLIT || cfg_ext(*cfg)));
   if (cfg->noise_enable && !c->fused && !(cfg->output_mask & TS_OUT_FT)) TS_ALLOC(c->ft_scratch, sizeof(float) * E * T * 6);
   if (cfg->noise_enable && !c->fused && cfg->radius_noise != 0.f) TS_ALLOC(c->ft_scratch_r, sizeof(float) * E * T * 6);
   if (cfg->noise_enable) {
@@ -528,6 +530,14 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
   if (!in->link_pos || !in->link_quat || !in->link_linvel || !in->link_angvel || !in->obj_pos || !in->obj_quat ||
       !in->obj_linvel || !in->obj_angvel)
     return fail(c, TS_ERR_INVALID_ARG, "ts_step: NULL input pointer");
+  {  // output_mask contract (ts.h): bit set <=> pointer given
+    const void* ptr[7] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead};
+    for (int b = 0; b < 7; ++b) {
+      const bool want = (c->cfg.output_mask >> b) & 1u;
+      if (want && !ptr[b]) return fail(c, TS_ERR_INVALID_ARG, "ts_step: an output declared in output_mask is NULL");
+      if (!want && ptr[b]) return fail(c, TS_ERR_INVALID_ARG, "ts_step: an output not declared in output_mask is non-NULL");
+    }
+  }
   if ((out->ft_noisy || out->dead) && !c->cfg.noise_enable) return fail(c, TS_ERR_INVALID_ARG, "ts_step: ft_noisy / dead need noise_enable");
   if (out->marker && c->M == 0) return fail(c, TS_ERR_INVALID_ARG, "ts_step: marker requested but the layout has no markers");
   const uintptr_t al = (uintptr_t)out->contact | (uintptr_t)out->depth | (uintptr_t)out->ft | (uintptr_t)out->marker |
@@ -547,26 +557,20 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
     if (!c->ft_scratch) return fail(c, TS_ERR_INVALID_ARG, "ts_step: ft is NULL although TS_OUT_FT is set in output_mask");
     p.ft = c->ft_scratch;
   }
-  cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
-  if (c->timing) {
-    while (c->ev_used + 3 > c->ev.size()) {
-      cudaEvent_t a;
-      TS_CUDA(c, cudaEventCreate(&a));
-      c->ev.push_back(a);
-    }
-    e0 = c->ev[c->ev_used]; e1 = c->ev[c->ev_used + 1]; e2 = c->ev[c->ev_used + 2];
-    c->ev_used += 3;
-    TS_CUDA(c, cudaEventRecord(e0, st));
-  }
+  const bool rec = c->timing && c->ev_used + 4 <= c->ev.size();   // pool exhausted: later steps are not recorded
+  cudaEvent_t* ev = rec ? &c->ev[c->ev_used] : nullptr;
+  if (rec) { p.clock = c->clock_buf + 2 * (c->ev_used / 4); c->ev_used += 4; TS_CUDA(c, cudaEventRecord(ev[0], st)); }
   cudaError_t e = (cudaError_t)ts_launch_frames(p, st);
-  if (e == cudaSuccess) e = (cudaError_t)ts_launch_step(p, c->fused ? 1 : 0, st);
+  if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: frames launch");
+  if (rec && c->timing_detail) TS_CUDA(c, cudaEventRecord(ev[1], st));
+  e = (cudaError_t)ts_launch_step(p, c->fused ? 1 : 0, st);
   if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: launch");
-  if (c->timing) TS_CUDA(c, cudaEventRecord(e1, st));
+  if (rec && c->timing_detail) TS_CUDA(c, cudaEventRecord(ev[2], st));
   if (split) {
     e = (cudaError_t)ts_launch_noise(p, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: noise launch");
   }
-  if (c->timing) TS_CUDA(c, cudaEventRecord(e2, st));
+  if (rec) TS_CUDA(c, cudaEventRecord(ev[3], st));
   c->gstep += 1;
   return TS_OK;
 }
@@ -613,22 +617,59 @@ ts_status ts_reset(ts_ctx* c, const uint8_t* env_mask_dev, void* stream) {
   return TS_OK;
 }
 
+ts_status ts_kernel_times_ms(ts_ctx* c, float* out_ms, int32_t capacity, int32_t* n_steps) {
+  if (!c) return TS_ERR_INVALID_ARG;
+  DeviceGuard guard(c->device);
+  const int n = (int)(c->ev_used / 4);
+  for (int i = 0; i < n && i < capacity && out_ms; ++i) {
+    cudaEvent_t* ev = &c->ev[(size_t)4 * i];
+    TS_CUDA(c, cudaEventSynchronize(ev[3]));
+    if (c->timing_detail) {
+      for (int k = 0; k < 3; ++k) TS_CUDA(c, cudaEventElapsedTime(out_ms + 4 * i + k, ev[k], ev[k + 1]));
+    } else {  // enable = 1: one pair of events around the whole step (reported in the step-kernel column)
+      out_ms[4 * i] = 0.f; out_ms[4 * i + 2] = 0.f;
+      TS_CUDA(c, cudaEventElapsedTime(out_ms + 4 * i + 1, ev[0], ev[3]));
+    }
+    unsigned long long ck[2] = {0, 0};
+    TS_CUDA(c, cudaMemcpy(ck, c->clock_buf + 2 * i, sizeof(ck), cudaMemcpyDeviceToHost));
+    out_ms[4 * i + 3] = ck[1] > ck[0] ? (float)((double)(ck[1] - ck[0]) * 1e-6) : 0.f;
+  }
+  if (n_steps) *n_steps = n;
+  return TS_OK;
+}
+
 ts_status ts_kernel_time_ms(ts_ctx* c, int32_t enable, float* mean_ms, int32_t* n_steps) {
   if (!c) return TS_ERR_INVALID_ARG;
   DeviceGuard guard(c->device);
   double sum = 0.0, sum1 = 0.0;
-  int n = 0;
-  for (size_t i = 0; i + 2 < c->ev_used; i += 3) {
-    TS_CUDA(c, cudaEventSynchronize(c->ev[i + 2]));
+  const int n = (int)(c->ev_used / 4);
+  for (int i = 0; i < n; ++i) {
+    cudaEvent_t* ev = &c->ev[(size_t)4 * i];
+    TS_CUDA(c, cudaEventSynchronize(ev[3]));
     float ms = 0.f, ms1 = 0.f;
-    TS_CUDA(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 2]));
-    TS_CUDA(c, cudaEventElapsedTime(&ms1, c->ev[i], c->ev[i + 1]));
+    TS_CUDA(c, cudaEventElapsedTime(&ms, ev[0], ev[3]));
+    if (c->timing_detail) TS_CUDA(c, cudaEventElapsedTime(&ms1, ev[0], ev[2]));
+    else ms1 = ms;
     sum += ms; sum1 += ms1;
-    ++n;
   }
   c->last_first_kernel_ms = n ? (float)(sum1 / n) : 0.f;
   c->ev_used = 0;
+  if (enable) {                    // device-side clock slots: {first block start (min), last block end (max)}
+    if (!c->clock_buf) TS_CUDA(c, cudaMalloc((void**)&c->clock_buf, sizeof(unsigned long long) * 2 * TS_TIMING_MAX_STEPS));
+    std::vector<unsigned long long> init((size_t)2 * TS_TIMING_MAX_STEPS);
+    for (int i = 0; i < TS_TIMING_MAX_STEPS; ++i) { init[2 * i] = ~0ULL; init[2 * i + 1] = 0ULL; }
+    TS_CUDA(c, cudaMemcpy(c->clock_buf, init.data(), sizeof(unsigned long long) * init.size(), cudaMemcpyHostToDevice));
+  }
+  if (enable && c->ev.empty()) {   // the pool is created here, never inside ts_step
+    c->ev.reserve((size_t)4 * TS_TIMING_MAX_STEPS);
+    for (int i = 0; i < 4 * TS_TIMING_MAX_STEPS; ++i) {
+      cudaEvent_t a;
+      TS_CUDA(c, cudaEventCreate(&a));
+      c->ev.push_back(a);
+    }
+  }
   c->timing = enable != 0;
+  c->timing_detail = enable == 2;
   if (mean_ms) *mean_ms = n ? (float)(sum / n) : 0.f;
   if (n_steps) *n_steps = n;
   return TS_OK;

@@ -87,6 +87,7 @@ struct TsStepParams {
   // geometry
   const int32_t* g_type;   // [E,K]
   const float4* g_params;  // [E,K]
+  unsigned long long* clock;  // NULL, or this step's {first block start, last block end} %globaltimer stamps [ns]
   void* frames_g;          // [E][P*K] FrameS (ts_kernels.cu): relative poses of every (env, patch, object), written by
                            // ts_frames_kernel at the start of the step, bulk-copied (TMA) into shared memory by each block
   const int32_t* patch_link;  // [P] sensor link of each patch (-1 = filler)
@@ -155,6 +156,6 @@ int ts_launch_reset_counters(uint32_t* reset_step, uint32_t* episode, const uint
 int ts_launch_reset_state(const TsStepParams& p, const uint8_t* mask, uint32_t dead_threshold, int nh, void* stream);
 unsigned long long ts_bank_elems_per_grid(int N);
 unsigned long long ts_step_smem_bytes(const TsStepParams& p);
-int ts_prepare_kernels(int max_smem_bytes);
+int ts_prepare_kernels(int device, int smem_bytes);
 
 #endif  // TS_INTERNAL_H_

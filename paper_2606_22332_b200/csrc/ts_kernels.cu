@@ -28,10 +28,17 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <mutex>
 
 #include "ts_internal.h"
 
 namespace {
+
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
 
 struct F3 {
   float x, y, z;
@@ -170,6 +177,7 @@ __global__ void __launch_bounds__(128) ts_frames_kernel(const __grid_constant__ 
   // fully coalesced run: per-thread 272-byte rows straight to global memory cost 32 sectors per store request
   // (ncu: lg_throttle 4.2 per issue, 47 us); staged 17 x 512-byte requests per warp.
   __shared__ __align__(16) unsigned char stage[128 * sizeof(FrameS)];
+  if (p.clock && threadIdx.x == 0) atomicMin(p.clock, globaltimer_ns());   // device-side clock: first block start
   const int PK = p.P * p.K;
   const long long total = (long long)p.E * PK;
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -499,7 +507,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
 // SDF gathers and the layout tables).
 __device__ __forceinline__ float2 ld_stream2(const float2* p) {
   float2 v;
-  asm volatile("ld.global.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+  asm volatile("ld.global.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p) : "memory");
   return v;
 }
 
@@ -785,6 +793,7 @@ __global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_cons
     deadb = act && ((p.st_flags[ej] >> 1) & 1);
   }
   noise_chain<HM>(p, e, j, ej, tid, g0.z, valid, act, deadb, valid ? __ldg(p.tx_meta + j) : 0, ft, ns, bufB);
+  if (p.clock && tid == 0) atomicMax(p.clock + 1, globaltimer_ns());   // device-side clock: the split form ends the step here
 }
 
 template <bool SINGLE>
@@ -1233,8 +1242,9 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
       }
       if (ch + 1 < nchunk) __syncthreads();  // S is reused by the next chunk
     }
-    }
-
+  }
+  // device-side clock: last block end (thread 0 of every block; the fused form ends the step here)
+  if (p.clock && tid == 0 && (NOISE || !p.noise_enable)) atomicMax(p.clock + 1, globaltimer_ns());
 }
 
 // ---------------------------------------------------------------------------------------
@@ -1317,7 +1327,16 @@ void launch_one(const TsStepParams& p, int hm, dim3 grid, size_t smem, cudaStrea
 }
 }  // namespace
 
-int ts_prepare_kernels(int max_smem_bytes) {
+// cudaFuncAttributeMaxDynamicSharedMemorySize and the carveout are per DEVICE, not per ctx: contexts with different
+// shared-memory needs (K = 1 next to K = 8, say) share them, so the attribute is only ever RAISED to the running
+// maximum of what any ctx on the device asked for (a later, smaller ctx must not shrink it under an earlier one).
+int ts_prepare_kernels(int device, int smem_bytes) {
+  static std::mutex mu;
+  static int max_smem[64] = {0};
+  std::lock_guard<std::mutex> lock(mu);
+  const int d = device >= 0 && device < 64 ? device : 0;
+  if (smem_bytes <= max_smem[d]) return 0;
+  const int max_smem_bytes = smem_bytes;
   cudaError_t e = prep_one<true, -1>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_OFF>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_MAXWELL>(max_smem_bytes);
@@ -1332,6 +1351,7 @@ int ts_prepare_kernels(int max_smem_bytes) {
   if (e == cudaSuccess) e = prep_one<false, TS_HYST_OFF>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<false, TS_HYST_MAXWELL>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<false, TS_HYST_ASYM>(max_smem_bytes);
+  if (e == cudaSuccess) max_smem[d] = max_smem_bytes;
   return (int)e;
 }
 

@@ -117,3 +117,80 @@ def test_outputs_subset_and_replaced_geometry():
     assert touched.any()
     assert torch.allclose(r2["depth"][touched], r1["depth"][touched] - 1e-3, atol=2e-6)
     assert torch.equal(r2["depth"][~grid_env], r1["depth"][~grid_env])               # primitives are untouched
+
+
+def test_output_mask_contract_and_config_ranges():
+    """ts.h: every output declared in output_mask must be given and no other; env_id_base must fit the 32-bit Philox
+    counter word; kernel_form must be a TS_FORM_* value."""
+    from paper_2606_22332_b200 import binding as B
+    w = W.config(2, n_envs=8)
+    sim = _sim(w, outputs=("depth", "prox"))
+    inp = sim.upload(w.inputs(0))
+    out = sim.alloc_outputs()
+    L = B.lib()
+    si, so = sim._structs(inp, out, host=False)
+    so.prox = None                                                          # declared, but not given
+    assert L.ts_step(sim.h, C.byref(si), C.byref(so), sim._stream()) == 1 and b"declared in output_mask is NULL" in L.ts_last_error(sim.h)
+    si, so = sim._structs(inp, out, host=False)
+    so.contact = out["depth"].data_ptr()                                    # given, but not declared
+    assert L.ts_step(sim.h, C.byref(si), C.byref(so), sim._stream()) == 1 and b"not declared" in L.ts_last_error(sim.h)
+    si, so = sim._structs(inp, out, host=False)
+    assert L.ts_step(sim.h, C.byref(si), C.byref(so), sim._stream()) == 0
+    for bad in (dict(env_id_base=-1), dict(env_id_base=2 ** 32 - 4), dict(physics=dict(w.physics, kernel_form=3))):
+        with pytest.raises(B.TsError, match="TS_ERR_INVALID_ARG"):
+            B.TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=bad.get("physics", w.physics), env_id_base=bad.get("env_id_base", 0))
+    ok = B.TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=w.physics, env_id_base=2 ** 32 - 8)   # the last admissible base
+    ok.close()
+
+
+def test_two_contexts_with_different_shared_memory_needs():
+    """the dynamic shared-memory attribute is per device, not per ctx.  A K = 2 ctx (twice the frames per
+    block) created FIRST and a K = 1 ctx created after it must both keep stepping, in either order."""
+    import torch
+    from paper_2606_22332_b200.binding import TactileSim
+    w = W.config(2, n_envs=32)
+    w3 = W.config(3, n_envs=1)
+    E = w.E
+    types2 = np.zeros((E, 2), np.int32); params2 = np.zeros((E, 2, 4), np.float32)
+    types2[:, 0] = w.types[:, 0]; params2[:, 0] = w.params[:, 0]
+    types2[:, 1] = 1; params2[:, 1, 0] = 0.02
+    big = TactileSim(w.patches, w.T, E, w.L, 2, physics=w.physics, outputs=w.outputs)
+    big.set_geometry(types2, params2, w3.bank, w3.voxel)
+    small = _sim(w)
+    ref = _sim(w)
+    for s in range(3):
+        inp = w.inputs(s)
+        two = {k: (np.ascontiguousarray(np.concatenate([v, v + (0.2 if k == "obj_pos" else 0.0)], axis=1)) if k.startswith("obj_") else v)
+               for k, v in inp.items()}
+        a = big.step(big.upload(two))          # the second object sits 20 cm away: it never wins
+        b = small.step(small.upload(inp))
+        c = ref.step(ref.upload(inp))
+        torch.cuda.synchronize()
+        for k in b:
+            assert torch.equal(b[k], c[k]), k
+        assert torch.allclose(a["depth"], b["depth"], atol=1e-6)
+
+
+def test_per_step_kernel_times_and_kernel_form():
+    import torch
+    from paper_2606_22332_b200.binding import TactileSim
+    w = W.config(4, n_envs=64)
+    outs = {}
+    for form, launches in (("fused", 2), ("split", 3)):
+        sim = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=dict(w.physics, kernel_form=form), noise=w.noise, outputs=w.outputs)
+        sim.set_geometry(w.types, w.params, w.bank, w.voxel)
+        assert sim.launches_per_step() == launches
+        sim.kernel_time_ms(2)
+        for s in range(4):
+            g = sim.step(sim.upload(w.inputs(s)))
+        torch.cuda.synchronize()
+        t = sim.kernel_times_ms()
+        assert t.shape == (4, 4) and (t[:, :2] > 0).all() and ((t[:, 2] > 0).all() if form == "split" else (t[:, 2] < 0.02).all())
+        ev = t[:, :3].sum(1)
+        assert (t[:, 3] > 0).all() and (np.abs(t[:, 3] - ev) < 0.05 + 0.3 * ev).all()     # device-side clock agrees with the events
+        ms, n = sim.kernel_time_ms(False)
+        assert n == 4 and abs(ms - ev.mean()) < 0.05
+        outs[form] = {k: v.clone() for k, v in g.items()}
+        sim.close()
+    for k in outs["fused"]:
+        assert torch.equal(outs["fused"][k], outs["split"][k]), k      # both forms are bit-identical
