@@ -421,8 +421,13 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   if (cfg->noise_enable) {
     if (c->nh) TS_ALLOC(c->st_hyst, sizeof(float) * E * c->nh * c->Tp);
     TS_ALLOC(c->st_drift, sizeof(float) * E * 6 * c->Tp);
-    // never read before written: a slot is read only for a step of the current episode (ts_kernels.cu, noise_chain)
-    if (cfg->read_delay + cfg->read_jitter > 0) TS_ALLOC(c->st_ring, sizeof(float) * E * 6 * c->Tp * (size_t)(cfg->read_delay + cfg->read_jitter));
+    // A slot is only read for a step of the current episode (ts_kernels.cu, noise_chain), i.e. after it was written;
+    // the ring is zeroed once anyway so that no read can ever see uninitialised memory.
+    if (cfg->read_delay + cfg->read_jitter > 0) {
+      const size_t rb = sizeof(float) * E * 6 * c->Tp * (size_t)(cfg->read_delay + cfg->read_jitter);
+      TS_ALLOC(c->st_ring, rb);
+      if (cudaMemset(c->st_ring, 0, rb) != cudaSuccess) { free_all(c); delete c; return fail(nullptr, TS_ERR_CUDA, "ts_create: cudaMemset ring"); }
+    }
   }
 #undef TS_ALLOC
   cudaError_t e = cudaSuccess;

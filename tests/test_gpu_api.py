@@ -194,3 +194,37 @@ def test_per_step_kernel_times_and_kernel_form():
         sim.close()
     for k in outs["fused"]:
         assert torch.equal(outs["fused"][k], outs["split"][k]), k      # both forms are bit-identical
+
+
+def test_outputs_stay_inside_their_buffers():
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizer.md), so the bounds are checked here: every
+    output tensor is a window into a larger allocation whose margins hold a canary pattern; after stepping configs with
+    ragged groups (240 / 248 slots), fillers, K = 1 and every noise knob, the margins must be untouched and the windows
+    fully written (no canary left inside)."""
+    import torch
+    from paper_2606_22332_b200.binding import TactileSim
+    for cid, n_envs, extra in ((5, 33, dict(read_delay=2, read_jitter=1, radius_noise=3e-4)), (2, 17, None), (1, 4, None)):
+        w = W.config(cid, n_envs=n_envs)
+        noise = dict(w.noise, **extra) if (w.noise and extra) else w.noise
+        for form in (("fused", "split") if noise else ("auto",)):
+            sim = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=dict(w.physics, kernel_form=form), noise=noise, outputs=w.outputs)
+            sim.set_geometry(w.types, w.params, w.bank, w.voxel)
+            sh = sim.out_shapes()
+            pad = 4096
+            big, out = {}, {}
+            for k in sim.outputs:
+                shape, dt = sh[k]
+                n = int(np.prod(shape))
+                canary = 0xA5 if dt == torch.uint8 else float("nan")
+                big[k] = torch.full((n + 2 * pad,), canary, dtype=dt, device="cuda")
+                out[k] = big[k][pad:pad + n].view(shape)
+            for s in range(3):
+                sim.step(sim.upload(w.inputs(s)), out)
+            torch.cuda.synchronize()
+            for k in sim.outputs:
+                lo, hi, mid = big[k][:pad], big[k][-pad:], big[k][pad:-pad]
+                if big[k].dtype == torch.uint8:
+                    assert (lo == 0xA5).all() and (hi == 0xA5).all() and (mid <= 1).all(), (cid, form, k)
+                else:
+                    assert torch.isnan(lo).all() and torch.isnan(hi).all() and torch.isfinite(mid).all(), (cid, form, k)
+            sim.close()
