@@ -264,6 +264,10 @@ typedef struct orc_params {
   float xtalk_sigma;  // Eq. 11 / 31: 0 = 4-neighbour stencil (D4); > 0 = Gaussian G_sigma, sigma in taxel pitches (R7)
   float radius_noise; // Eq. 26: rho (metres), R~_j = max(0, R_j + eps_j), eps_j ~ U[-rho, rho] (R8); 0 = off
   int32_t read_delay, read_jitter;  // Eq. 25 Delta_read in steps and its uniform jitter +-J steps (R9); 0, 0 = off
+  // Noisy readouts of the scalar sensors (Table 3: ContactDepth, Proximity, Elastomer take every knob but
+  // crosstalk; values Table 12; reading R10): per class {depth, prox, marker}
+  // white sigma, random-walk sigma, bias, quantisation step, stuck range [l, u]
+  float sn_sigma_white[3], sn_sigma_rw[3], sn_bias[3], sn_quant[3], sn_stuck_min[3], sn_stuck_max[3];
 } orc_params;
 }
 
@@ -289,6 +293,11 @@ struct Oracle {
   double* aux_quant = nullptr;                // [E,T,6] comparator aid, see orc_set_aux_quant
   double* aux_rgate = nullptr;                // [E,T] comparator aid, see orc_set_aux_rgate
   double* aux_wingap = nullptr;               // [E,T] comparator aid, see orc_set_aux_wingap
+  // noisy scalar readouts (R10): outputs and comparator aids handed in by orc_set_scalar_noisy; state
+  double *depth_noisy = nullptr, *prox_noisy = nullptr, *marker_noisy = nullptr;   // [E,T], [E,T], [E,M,3]
+  double *aux_sq_depth = nullptr, *aux_sq_prox = nullptr, *aux_sq_marker = nullptr, *aux_sasym_marker = nullptr;
+  std::vector<double> sn_ha, sn_hb, sn_dr;    // [E,T,2] depth, prox: hysteresis (xi | y), x_prev, drift
+  std::vector<double> sm_ha, sm_hb, sm_dr;    // [E,M,3] marker channels
   std::vector<std::deque<std::vector<double>>> hist;  // [E] the last Delta + J post-crosstalk fields [T,6] of the episode
   std::vector<uint32_t> n_step, episode;      // [E]
 };
@@ -418,6 +427,8 @@ void* orc_create(const orc_params* prm, const orc_patch* patches, int n_patches,
   o->hyst_a.assign(ET * 6, 0.0); o->hyst_b.assign(ET * 6, 0.0); o->drift.assign(ET * 6, 0.0);   // Q12
   o->n_step.assign(o->E, 0); o->episode.assign(o->E, 0);
   o->hist.assign(o->E, {});
+  o->sn_ha.assign(ET * 2, 0.0); o->sn_hb.assign(ET * 2, 0.0); o->sn_dr.assign(ET * 2, 0.0);
+  { size_t EM = (size_t)o->E * o->M * 3; o->sm_ha.assign(EM, 0.0); o->sm_hb.assign(EM, 0.0); o->sm_dr.assign(EM, 0.0); }
   Geom none; none.type = G_NONE; none.grid = nullptr; none.N = 0; none.hv = 0; for (double& v : none.p) v = 0;
   o->geom.assign((size_t)o->E * o->K, none);
   return o;
@@ -480,6 +491,8 @@ void orc_reset(void* h, const uint8_t* env_mask) {
     o.n_step[e] = 0;
     o.episode[e] += 1;
     o.hist[e].clear();
+    for (size_t i = (size_t)e * o.T * 2; i < (size_t)(e + 1) * o.T * 2; ++i) { o.sn_ha[i] = 0; o.sn_hb[i] = 0; o.sn_dr[i] = 0; }
+    for (size_t i = (size_t)e * o.M * 3; i < (size_t)(e + 1) * o.M * 3; ++i) { o.sm_ha[i] = 0; o.sm_hb[i] = 0; o.sm_dr[i] = 0; }
   }
 }
 
@@ -492,6 +505,40 @@ static bool is_dead(const Oracle& o, int e, int t) {
   uint32_t w[4];
   philox4x32_10(ctr, key, w);
   return w[0] < thr;
+}
+
+// R10: one channel of a noisy scalar readout (Eq. 25, 27-30; no crosstalk, Table 3):
+//   x = gamma * clean -> hysteresis (Eq. 29-30 or ASYM) -> y = h + b + sigma_w z_w + D, D <- D + sigma_rw z_rw
+//   -> quantize(y, q) -> a dead probe reads its stuck value.  Returns the readout; aq / aa receive the comparator aids
+// (distance to the nearest rounding boundary; |x| - |y_prev| where the signs differ), +inf where not applicable.
+static double scalar_chain(const orc_params& pr, int cls, double clean, double gain, bool is_dead, double stuck_u,
+                           double z_rw, double z_w, double& ha, double& hb, double& drift, double decay,
+                           double* aq, double* aa) {
+  double x = gain * clean, hval = x;
+  if (aa) *aa = INFINITY;
+  if (pr.hyst_mode == 1) {                                        // Eq. 29-30
+    double xi = decay * ha + (x - hb);
+    ha = xi; hb = x;
+    hval = x + (double)pr.beta * xi;
+  } else if (pr.hyst_mode == 2) {                                 // D3, Q14
+    double yp = ha;
+    if (aa && x * yp < 0.0) *aa = std::fabs(x) - std::fabs(yp);
+    double al = (std::fabs(x) > std::fabs(yp)) ? (double)pr.alpha_load : (double)pr.alpha_unload;
+    double y = yp + al * (x - yp);
+    ha = y;
+    hval = y;
+  }
+  drift += (double)pr.sn_sigma_rw[cls] * z_rw;                    // Eq. 25 d_t = d_{t-1} + w_t
+  double y = hval + (double)pr.sn_bias[cls] + (double)pr.sn_sigma_white[cls] * z_w + drift;
+  if (aq) *aq = INFINITY;
+  float q = pr.sn_quant[cls];
+  if (q > 0.0f) {                                                 // quantize(., q) as R5: decision in fp32
+    float yf = (float)y, r = yf / q, k = std::nearbyintf(r);
+    if (aq) *aq = (0.5 - std::fabs((double)r - (double)k)) * (double)q;
+    y = (double)(k * q);
+  }
+  if (is_dead) y = (double)pr.sn_stuck_min[cls] + ((double)pr.sn_stuck_max[cls] - (double)pr.sn_stuck_min[cls]) * stuck_u;
+  return y;
 }
 
 // One step of the whole path.  Inputs fp32 [E,L,*] / [E,K,*]; outputs double (NULL = skip).
@@ -511,6 +558,7 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
 #endif
   for (int e = 0; e < o.E; ++e) {
     std::vector<double> phi_min(T), dep(T), ftc((size_t)T * 6), ftn((size_t)T * 6), hcl((size_t)T * 6);
+    std::vector<double> dep_t(T, 0.0), prox_c(T, 0.0), marker_c((size_t)M * 3, 0.0);   // inputs of the noisy scalar readouts (R10)
     std::vector<uint8_t> deadv(T, 0);
     for (int j = 0; j < T; ++j) {
       size_t ej = (size_t)e * T + j;
@@ -538,6 +586,7 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
       if (o.aux_wingap) o.aux_wingap[ej] = second_phi - best_phi;   // +inf with fewer than two objects
       double d = (active && kstar >= 0) ? std::fmax(0.0, o.radius[j] - best_phi) : 0.0;   // Eq. 2
       dep[j] = d;
+      dep_t[j] = d;
       if (aux_phi) aux_phi[ej] = best_phi;
       if (aux_face) aux_face[ej] = kstar >= 0 ? qstar.face : INFINITY;
       if (aux_boxgap) aux_boxgap[ej] = kstar >= 0 ? qstar.boxgap : INFINITY;
@@ -575,6 +624,7 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
         double Rt = std::fmax(0.0, o.radius[j] + eps);
         double dt_ = (kstar >= 0) ? std::fmax(0.0, Rt - best_phi) : 0.0;
         if (o.aux_rgate) o.aux_rgate[ej] = std::fabs(Rt - best_phi);
+        dep_t[j] = dt_;                                          // the noisy depth readout senses with R~_j too
         for (int c = 0; c < 6; ++c) g6[c] = 0.0;
         if (dt_ > 0.0) {
           double gn = norm(qstar.g);
@@ -605,6 +655,7 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
           P = march(phi_at, (double)pr.r_prox, pr.march_steps);
         }
         prox[ej] = P;
+        prox_c[j] = P;
       }
     }
     // O6 (Eq. 18-21, 23 first sum; Q15-Q17): dilation of each patch's markers by its active taxels
@@ -631,6 +682,7 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
         }
         size_t o3 = ((size_t)e * M + jm) * 3;
         marker[o3] = u.x; marker[o3 + 1] = u.y; marker[o3 + 2] = u.z;
+        marker_c[(size_t)jm * 3] = u.x; marker_c[(size_t)jm * 3 + 1] = u.y; marker_c[(size_t)jm * 3 + 2] = u.z;
       }
     }
     // O8: hysteresis -> crosstalk -> drift -> dead
@@ -793,6 +845,75 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
         while ((int)o.hist[e].size() > pr.read_delay + pr.read_jitter) o.hist[e].pop_front();
       }
     }
+    // R10: noisy readouts of the scalar sensors (ContactDepth, Proximity, Elastomer markers): Table 3 gives them every
+    // knob of App. A.8 except crosstalk.  Probe-level draws (gain stream 3, dead stream 2) are those of the taxel;
+    // markers are probes of their own, numbered 0x80000000 + m in the taxel word of the counter.
+    if (pr.noise_enable && (o.depth_noisy || o.prox_noisy || o.marker_noisy)) {
+      const uint32_t n = o.n_step[e], ep4 = o.episode[e] << 4, env = (uint32_t)o.env_id[e];
+      const uint32_t key[2] = {pr.seed_lo, pr.seed_hi};
+      const uint32_t thr = (uint32_t)std::floor((double)pr.p_dead * 4294967296.0);
+      const double decay = std::exp(-(double)pr.dt / (double)pr.tau);
+      const bool gain_on = pr.gain_min != 1.0f || pr.gain_max != 1.0f;
+      auto draw = [&](uint32_t probe, uint32_t step, uint32_t stream, uint32_t w[4]) {
+        uint32_t c[4] = {env, probe, step, ep4 | stream};
+        philox4x32_10(c, key, w);
+      };
+      for (int j = 0; j < T; ++j) {
+        size_t ej = (size_t)e * T + j;
+        double od = 0.0, op = 0.0;
+        if (o.aux_sq_depth) o.aux_sq_depth[ej] = INFINITY;
+        if (o.aux_sq_prox) o.aux_sq_prox[ej] = INFINITY;
+        if (o.radius[j] > 0.0) {
+          uint32_t w[4], ws[4], wg[4];
+          draw((uint32_t)j, n, 10u, w);                          // stream 10: (0,1) -> depth (rw, white), (2,3) -> prox
+          double zd[2], zp[2];
+          box_muller(w[0], w[1], &zd[0], &zd[1]);
+          box_muller(w[2], w[3], &zp[0], &zp[1]);
+          draw((uint32_t)j, 0u, 11u, ws);                        // stream 11, n = 0: stuck values (word 0 depth, 1 prox)
+          double gain = 1.0;
+          if (gain_on) { draw((uint32_t)j, 0u, 3u, wg); gain = (double)pr.gain_min + ((double)pr.gain_max - (double)pr.gain_min) * word_to_uniform(wg[0]); }
+          od = scalar_chain(pr, 0, dep_t[j], gain, deadv[j], word_to_uniform(ws[0]), zd[0], zd[1], o.sn_ha[ej * 2], o.sn_hb[ej * 2],
+                            o.sn_dr[ej * 2], decay, o.aux_sq_depth ? &o.aux_sq_depth[ej] : nullptr, nullptr);
+          op = scalar_chain(pr, 1, prox_c[j], gain, deadv[j], word_to_uniform(ws[1]), zp[0], zp[1], o.sn_ha[ej * 2 + 1],
+                            o.sn_hb[ej * 2 + 1], o.sn_dr[ej * 2 + 1], decay, o.aux_sq_prox ? &o.aux_sq_prox[ej] : nullptr, nullptr);
+        }
+        if (o.depth_noisy) o.depth_noisy[ej] = od;
+        if (o.prox_noisy) o.prox_noisy[ej] = op;
+      }
+      if (o.marker_noisy) {
+        for (int jm = 0; jm < M; ++jm) {
+          const int pm = o.mpatch[jm];
+          const bool mact = o.radius[o.p_start[pm]] > 0.0;       // markers of a filtered-out link are fillers too
+          const uint32_t probe = 0x80000000u + (uint32_t)jm;
+          uint32_t w0[4], w1[4], wd[4], wg[4], ws[4];
+          double zr[4] = {0, 0, 0, 0}, zw[2] = {0, 0};
+          bool mdead = false;
+          double gain = 1.0;
+          if (mact) {
+            draw(probe, n, 0u, w0);                              // stream 0: (0,1) -> rw ch 0,1; (2,3) -> rw ch 2, white ch 0
+            draw(probe, n, 1u, w1);                              // stream 1: (0,1) -> white ch 1, 2
+            box_muller(w0[0], w0[1], &zr[0], &zr[1]);
+            box_muller(w0[2], w0[3], &zr[2], &zr[3]);
+            box_muller(w1[0], w1[1], &zw[0], &zw[1]);
+            draw(probe, 0u, 2u, wd);
+            mdead = wd[0] < thr;
+            if (gain_on) { draw(probe, 0u, 3u, wg); gain = (double)pr.gain_min + ((double)pr.gain_max - (double)pr.gain_min) * word_to_uniform(wg[0]); }
+            draw(probe, 0u, 4u, ws);                             // stream 4, n = 0: stuck values, words 0-2
+          }
+          for (int c = 0; c < 3; ++c) {
+            size_t i3 = ((size_t)e * M + jm) * 3 + c;
+            double out = 0.0;
+            if (o.aux_sq_marker) o.aux_sq_marker[i3] = INFINITY;
+            if (o.aux_sasym_marker) o.aux_sasym_marker[i3] = INFINITY;
+            if (mact)
+              out = scalar_chain(pr, 2, marker_c[(size_t)jm * 3 + c], gain, mdead, word_to_uniform(ws[c]), zr[c],
+                                 c == 0 ? zr[3] : zw[c - 1], o.sm_ha[i3], o.sm_hb[i3], o.sm_dr[i3], decay,
+                                 o.aux_sq_marker ? &o.aux_sq_marker[i3] : nullptr, o.aux_sasym_marker ? &o.aux_sasym_marker[i3] : nullptr);
+            o.marker_noisy[i3] = out;
+          }
+        }
+      }
+    }
     o.n_step[e] += 1;
   }
 }
@@ -809,6 +930,15 @@ void orc_set_aux_rgate(void* h, double* aux_rgate) { ((Oracle*)h)->aux_rgate = a
 // Comparator aid: aux_wingap[E,T] receives phi_second - phi_best over the K objects of the env (the margin by
 // which Eq. 2's winner g* won), +inf with fewer than two objects.  NULL switches it off.
 void orc_set_aux_wingap(void* h, double* aux_wingap) { ((Oracle*)h)->aux_wingap = aux_wingap; }
+
+// R10: hands in the buffers the following orc_step calls fill with the noisy scalar readouts (NULL = not produced) and
+// their comparator aids (distance to the quantisation boundary per element; marker ASYM sign-flip margin).
+void orc_set_scalar_noisy(void* h, double* depth_noisy, double* prox_noisy, double* marker_noisy, double* aux_sq_depth,
+                          double* aux_sq_prox, double* aux_sq_marker, double* aux_sasym_marker) {
+  Oracle& o = *(Oracle*)h;
+  o.depth_noisy = depth_noisy; o.prox_noisy = prox_noisy; o.marker_noisy = marker_noisy;
+  o.aux_sq_depth = aux_sq_depth; o.aux_sq_prox = aux_sq_prox; o.aux_sq_marker = aux_sq_marker; o.aux_sasym_marker = aux_sasym_marker;
+}
 
 // Stand-alone pieces for the pins -------------------------------------------------
 

@@ -46,7 +46,12 @@ class OrcParams(C.Structure):
                 ("gain_min", C.c_float), ("gain_max", C.c_float),
                 ("stuck_min_force", C.c_float), ("stuck_max_force", C.c_float),
                 ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float), ("xtalk_sigma", C.c_float),
-                ("radius_noise", C.c_float), ("read_delay", C.c_int32), ("read_jitter", C.c_int32)]
+                ("radius_noise", C.c_float), ("read_delay", C.c_int32), ("read_jitter", C.c_int32),
+                ("sn_sigma_white", C.c_float * 3), ("sn_sigma_rw", C.c_float * 3), ("sn_bias", C.c_float * 3),
+                ("sn_quant", C.c_float * 3), ("sn_stuck_min", C.c_float * 3), ("sn_stuck_max", C.c_float * 3)]
+
+SN_CLASS = {"depth": 0, "prox": 1, "marker": 2}          # noisy scalar readouts (R10)
+SN_KNOBS = ("sigma_white", "sigma_rw", "bias", "quant", "stuck_min", "stuck_max")
 
 
 HYST = {"off": 0, "maxwell": 1, "asym": 2}
@@ -81,6 +86,7 @@ def lib():
         L.orc_set_aux_quant.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_set_aux_rgate.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_set_aux_wingap.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_set_scalar_noisy.argtypes = [C.c_void_p] + [C.c_void_p] * 7
         L.orc_max_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -107,9 +113,14 @@ def make_params(physics=None, noise=None):
              sigma_white_force=0.0, sigma_white_torque=0.0, bias_force=0.0, bias_torque=0.0, quant_force=0.0,
              quant_torque=0.0, gain_min=1.0, gain_max=1.0, stuck_min_force=0.0, stuck_max_force=0.0,
              stuck_min_torque=0.0, stuck_max_torque=0.0, xtalk_sigma=0.0, radius_noise=0.0, read_delay=0, read_jitter=0)
+    sn = {}
     for src in (physics, noise):
         if src:
             for k, v in src.items():
+                knob, _, cls = k.rpartition("_")
+                if knob in SN_KNOBS and cls in SN_CLASS:     # e.g. sigma_white_depth, quant_marker
+                    sn[(knob, cls)] = float(v)
+                    continue
                 if k not in d:
                     raise KeyError(k)
                 d[k] = v
@@ -121,6 +132,8 @@ def make_params(physics=None, noise=None):
         setattr(p, k, v)
     p.seed_lo = seed & 0xFFFFFFFF
     p.seed_hi = (seed >> 32) & 0xFFFFFFFF
+    for (knob, cls), v in sn.items():
+        getattr(p, "sn_" + knob)[SN_CLASS[cls]] = v
     return p
 
 
@@ -207,6 +220,12 @@ class Oracle:
         if self.params.noise_enable:
             if "ft_noisy" in want: out["ft_noisy"] = np.zeros((E, T, 6))
             if "dead" in want: out["dead"] = np.zeros((E, T), np.uint8)
+            # noisy scalar readouts (R10); each needs its clean input computed too
+            if "depth_noisy" in want: out["depth_noisy"] = np.zeros((E, T))
+            if "prox_noisy" in want:
+                out["prox_noisy"] = np.zeros((E, T)); out.setdefault("prox", np.zeros((E, T)))
+            if "marker_noisy" in want and M > 0:
+                out["marker_noisy"] = np.zeros((E, M, 3)); out.setdefault("marker", np.zeros((E, M, 3)))
         if aux:
             out["aux_phi"] = np.zeros((E, T))
             out["aux_face"] = np.zeros((E, T))
@@ -219,10 +238,16 @@ class Oracle:
                     out["aux_quant"] = np.zeros((E, T, 6))
                 if self.params.radius_noise != 0:
                     out["aux_rgate"] = np.zeros((E, T))
+                if "depth_noisy" in out: out["aux_sq_depth"] = np.zeros((E, T))
+                if "prox_noisy" in out: out["aux_sq_prox"] = np.zeros((E, T))
+                if "marker_noisy" in out:
+                    out["aux_sq_marker"] = np.zeros((E, M, 3)); out["aux_sasym_marker"] = np.zeros((E, M, 3))
         g = out.get
         self.L.orc_set_aux_quant(self.h, _p(g("aux_quant")))
         self.L.orc_set_aux_rgate(self.h, _p(g("aux_rgate")))
         self.L.orc_set_aux_wingap(self.h, _p(g("aux_wingap")))
+        self.L.orc_set_scalar_noisy(self.h, _p(g("depth_noisy")), _p(g("prox_noisy")), _p(g("marker_noisy")), _p(g("aux_sq_depth")),
+                                    _p(g("aux_sq_prox")), _p(g("aux_sq_marker")), _p(g("aux_sasym_marker")))
         self.L.orc_step(self.h, _p(a["link_pos"]), _p(a["link_quat"]), _p(a["link_linvel"]), _p(a["link_angvel"]),
                         _p(a["obj_pos"]), _p(a["obj_quat"]), _p(a["obj_linvel"]), _p(a["obj_angvel"]),
                         _p(g("contact")), _p(g("depth")), _p(g("ft")), _p(g("marker")), _p(g("prox")),
