@@ -122,7 +122,12 @@ enum {                      /* output_mask bits.  ts_step contract: every output
   TS_OUT_MARKER = 1 << 3,   /* Eq. 21  f32   [E,M,3] link frame */
   TS_OUT_PROX = 1 << 4,     /* march   f32   [E,T]  P_j = r_prox - t */
   TS_OUT_FT_NOISY = 1 << 5, /* A.8     f32   [E,T,6]; needs noise_enable */
-  TS_OUT_DEAD = 1 << 6      /* Eq. 28  uint8 [E,T];   needs noise_enable */
+  TS_OUT_DEAD = 1 << 6,     /* Eq. 28  uint8 [E,T];   needs noise_enable */
+  /* noisy readouts of the scalar sensors (Table 3: every knob of App. A.8 except crosstalk; R10);
+     need noise_enable */
+  TS_OUT_DEPTH_NOISY = 1 << 7,  /* f32 [E,T]   ContactDepth readout; senses with the Eq. 26 radius when radius_noise > 0 */
+  TS_OUT_PROX_NOISY = 1 << 8,   /* f32 [E,T]   Proximity readout */
+  TS_OUT_MARKER_NOISY = 1 << 9  /* f32 [E,M,3] Elastomer marker readout (every marker is a probe of its own) */
 };
 
 typedef struct ts_config {
@@ -176,6 +181,12 @@ typedef struct ts_config {
    * (24 B x n_envs x n_taxels each). */
   int32_t read_delay, read_jitter;
   int32_t kernel_form;   /* TS_FORM_* (0 = AUTO) */
+  /* Noisy scalar readouts (TS_OUT_DEPTH_NOISY / PROX_NOISY / MARKER_NOISY), index 0 = depth, 1 = prox, 2 = marker:
+   * x = gamma * clean -> hysteresis (hyst_mode, beta, tau, alpha_*) -> y = h + bias + white + drift (Eq. 25) ->
+   * quantize -> a dead probe reads its stuck value U[min, max] (Eq. 28).  gain_*, p_dead and the hysteresis are the
+   * ones above; depth / prox share their taxel's gain and dead draw, a marker draws its own.  Table 12 P:523-535:
+   * depth sigma 2e-4 m; proximity sigma 1e-2, rw 1e-3, quant 1e-2; elastomer sigma 1e-4 m, rw 1e-5 m, quant 1e-4 m. */
+  float sn_sigma_white[3], sn_sigma_rw[3], sn_bias[3], sn_quant[3], sn_stuck_min[3], sn_stuck_max[3];
 } ts_config;
 
 /* Fills *cfg with the paper's constants and everything else zero / off. */
@@ -222,6 +233,9 @@ typedef struct ts_step_out {
   float* prox;      /* [E,T]   */
   float* ft_noisy;  /* [E,T,6] */
   uint8_t* dead;    /* [E,T]   */
+  float* depth_noisy;  /* [E,T]   */
+  float* prox_noisy;   /* [E,T]   */
+  float* marker_noisy; /* [E,M,3] */
 } ts_step_out;
 
 /* Creates a context on `cuda_device` (must be sm_100).  Allocates every device buffer the

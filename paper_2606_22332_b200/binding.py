@@ -17,7 +17,10 @@ STATUS = {0: "TS_OK", 1: "TS_ERR_INVALID_ARG", 2: "TS_ERR_CUDA", 3: "TS_ERR_OOM"
 HYST = {"off": 0, "maxwell": 1, "asym": 2}
 FORM = {"auto": 0, "fused": 1, "split": 2}
 GEOM = {"none": 0, "sphere": 1, "box": 2, "capsule": 3, "sdf": 4, "grid": 4}
-OUT_BITS = {"contact": 1, "depth": 2, "ft": 4, "marker": 8, "prox": 16, "ft_noisy": 32, "dead": 64}
+OUT_BITS = {"contact": 1, "depth": 2, "ft": 4, "marker": 8, "prox": 16, "ft_noisy": 32, "dead": 64,
+            "depth_noisy": 128, "prox_noisy": 256, "marker_noisy": 512}
+SN_CLASS = {"depth": 0, "prox": 1, "marker": 2}          # noisy scalar readouts (ts_config.sn_*[3])
+SN_KNOBS = ("sigma_white", "sigma_rw", "bias", "quant", "stuck_min", "stuck_max")
 
 # every symbol include/ts.h declares (tests check that the library exports them all)
 SYMBOLS = ["ts_layout_create", "ts_layout_add_patch", "ts_layout_filter_links", "ts_layout_finalize", "ts_layout_get",
@@ -66,7 +69,9 @@ class Config(C.Structure):
                 ("stuck_min_force", C.c_float), ("stuck_max_force", C.c_float),
                 ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float), ("xtalk_sigma", C.c_float),
                 ("radius_noise", C.c_float), ("read_delay", C.c_int32), ("read_jitter", C.c_int32),
-                ("kernel_form", C.c_int32)]
+                ("kernel_form", C.c_int32),
+                ("sn_sigma_white", C.c_float * 3), ("sn_sigma_rw", C.c_float * 3), ("sn_bias", C.c_float * 3),
+                ("sn_quant", C.c_float * 3), ("sn_stuck_min", C.c_float * 3), ("sn_stuck_max", C.c_float * 3)]
 
 
 class Geometry(C.Structure):
@@ -80,7 +85,8 @@ class StepIn(C.Structure):
 
 
 class StepOut(C.Structure):
-    _fields_ = [(k, C.c_void_p) for k in ("contact", "depth", "ft", "marker", "prox", "ft_noisy", "dead")]
+    _fields_ = [(k, C.c_void_p) for k in ("contact", "depth", "ft", "marker", "prox", "ft_noisy", "dead", "depth_noisy",
+                                          "prox_noisy", "marker_noisy")]
 
 
 IN_KEYS = [k for k, _ in StepIn._fields_]
@@ -191,6 +197,10 @@ def make_config(n_envs, n_links, objs_per_env, layout, physics=None, noise=None,
     names = {f for f, _ in Config._fields_}
     for src in (physics, noise):
         for k, v in (src or {}).items():
+            knob, _, cls = k.rpartition("_")
+            if knob in SN_KNOBS and cls in SN_CLASS:         # e.g. sigma_white_depth, quant_marker -> sn_*[class]
+                getattr(cfg, "sn_" + knob)[SN_CLASS[cls]] = float(v)
+                continue
             if k not in names:
                 raise KeyError(k)
             if k == "hyst_mode" and isinstance(v, str):
@@ -237,7 +247,8 @@ class TactileSim:
         t = self.torch
         return dict(contact=((E, T), t.uint8), depth=((E, T), t.float32), ft=((E, T, 6), t.float32),
                     marker=((E, M, 3), t.float32), prox=((E, T), t.float32), ft_noisy=((E, T, 6), t.float32),
-                    dead=((E, T), t.uint8))
+                    dead=((E, T), t.uint8), depth_noisy=((E, T), t.float32), prox_noisy=((E, T), t.float32),
+                    marker_noisy=((E, M, 3), t.float32))
 
     def in_shapes(self):
         E, L, K = self.E, self.L, self.K

@@ -52,7 +52,10 @@ struct ts_ctx {
   uint32_t *reset_step = nullptr, *episode = nullptr;
   // device staging of ts_step_host
   float* stage_in[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-  void* stage_out[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  void* stage_out[10] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  // noisy scalar readouts (R10): state, the perturbed depth (Eq. 26), scratch copies of clean inputs the caller did not ask for
+  float4* sn_h = nullptr; float2* sn_d = nullptr; float *sm_h = nullptr, *sm_d = nullptr;
+  float *depth_pert = nullptr, *sc_depth = nullptr, *sc_prox = nullptr, *sc_marker = nullptr;
   // timing of the main kernel
   bool timing = false;
   bool timing_detail = false;   // events between the kernels of a step too (enable = 2)
@@ -95,6 +98,8 @@ void free_all(ts_ctx* c) {
   cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->mk_tab8); cudaFree(c->grp_link);
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->env_perm); cudaFree(c->frames_g); cudaFree(c->patch_link); cudaFree(c->bank); cudaFree(c->bank_stage); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch); cudaFree(c->ft_scratch_r); cudaFree(c->st_ring);
+  cudaFree(c->sn_h); cudaFree(c->sn_d); cudaFree(c->sm_h); cudaFree(c->sm_d); cudaFree(c->depth_pert); cudaFree(c->sc_depth);
+  cudaFree(c->sc_prox); cudaFree(c->sc_marker);
   for (float* q : c->stage_in) cudaFree(q);
   for (void* q : c->stage_out) cudaFree(q);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
@@ -162,6 +167,12 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.rho = g.noise_enable ? g.radius_noise : 0.f;
   p.ft_pert = (p.rho != 0.f && !c->fused) ? c->ft_scratch_r : nullptr;
   p.ext = cfg_ext(g);
+  p.sn_h = c->sn_h; p.sn_d = c->sn_d; p.sm_h = c->sm_h; p.sm_d = c->sm_d; p.depth_pert = c->depth_pert;
+  for (int k = 0; k < 3; ++k) {
+    p.sn_sigma_white[k] = g.sn_sigma_white[k]; p.sn_sigma_rw[k] = g.sn_sigma_rw[k]; p.sn_bias[k] = g.sn_bias[k];
+    p.sn_quant[k] = g.sn_quant[k]; p.sn_stuck_min[k] = g.sn_stuck_min[k]; p.sn_stuck_max[k] = g.sn_stuck_max[k];
+  }
+  p.dead_thr = c->dead_thr;
 }
 }  // namespace
 
@@ -188,7 +199,11 @@ void ts_config_default(ts_config* c) {
 const char* ts_last_error(const ts_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 int32_t ts_n_taxels(const ts_ctx* ctx) { return ctx ? ctx->T : 0; }
 int32_t ts_n_markers(const ts_ctx* ctx) { return ctx ? ctx->M : 0; }
-int32_t ts_launches_per_step(const ts_ctx* ctx) { return !ctx ? 0 : ((ctx->cfg.noise_enable && !ctx->fused) ? 3 : 2); }
+int32_t ts_launches_per_step(const ts_ctx* ctx) {
+  if (!ctx) return 0;
+  return ((ctx->cfg.noise_enable && !ctx->fused) ? 3 : 2) +
+         ((ctx->cfg.output_mask & (TS_OUT_DEPTH_NOISY | TS_OUT_PROX_NOISY | TS_OUT_MARKER_NOISY)) ? 1 : 0);
+}
 
 ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   if (!cfg || !out) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: NULL argument");
@@ -220,8 +235,13 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     if (!(cfg->gain_min > 0.f) || !(cfg->gain_min <= cfg->gain_max)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: need 0 < gain_min <= gain_max");
     if (!(cfg->stuck_min_force <= cfg->stuck_max_force) || !(cfg->stuck_min_torque <= cfg->stuck_max_torque))
       return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: stuck_min > stuck_max");
-  } else if (cfg->output_mask & (TS_OUT_FT_NOISY | TS_OUT_DEAD)) {
-    return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: ft_noisy / dead need noise_enable");
+    for (int k = 0; k < 3; ++k)
+      if (!(cfg->sn_sigma_white[k] >= 0.f) || !(cfg->sn_sigma_rw[k] >= 0.f) || !(cfg->sn_quant[k] >= 0.f) || !(cfg->sn_stuck_min[k] <= cfg->sn_stuck_max[k]))
+        return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: sn_* knobs: sigma, quant >= 0 and stuck_min <= stuck_max");
+    if ((cfg->output_mask & TS_OUT_MARKER_NOISY) && lay->marker_patch.empty())
+      return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: marker_noisy requested but the layout has no markers");
+  } else if (cfg->output_mask & (TS_OUT_FT_NOISY | TS_OUT_DEAD | TS_OUT_DEPTH_NOISY | TS_OUT_PROX_NOISY | TS_OUT_MARKER_NOISY)) {
+    return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: noisy outputs and dead need noise_enable");
   }
   for (size_t t = 0; t < lay->link.size(); ++t)
     if (lay->link[t] >= cfg->n_links) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_create: layout link index >= n_links");
@@ -371,7 +391,9 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   if (chunks.empty()) chunks.push_back(TsChunk{});
   std::vector<float4> mpos(M > 0 ? M : 1), mnrm(M > 0 ? M : 1);
   for (int j = 0; j < M; ++j) {
-    mpos[j] = make_float4(lay->marker_pos[3 * j], lay->marker_pos[3 * j + 1], lay->marker_pos[3 * j + 2], 0.f);
+    // w = 1: the marker's patch is active (not removed by the link filter); read by the noisy marker readout (R10)
+    mpos[j] = make_float4(lay->marker_pos[3 * j], lay->marker_pos[3 * j + 1], lay->marker_pos[3 * j + 2],
+                          lay->radius[lay->patch_start[lay->marker_patch[j]]] > 0.f ? 1.f : 0.f);
     mnrm[j] = make_float4(lay->marker_nrm[3 * j], lay->marker_nrm[3 * j + 1], lay->marker_nrm[3 * j + 2], 0.f);
   }
   c->T = T; c->P = (int)pts.size(); c->M = M; c->G = (int)groups.size(); c->Tp = (T + 31) / 32 * 32;
@@ -418,6 +440,18 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   c->fused = cfg->kernel_form == TS_FORM_FUSED ? true : (cfg->kernel_form == TS_FORM_SPLIT ? false : !(TS_DEFAULT_SPLIT || cfg_ext(*cfg)));
   if (cfg->noise_enable && !c->fused && !(cfg->output_mask & TS_OUT_FT)) TS_ALLOC(c->ft_scratch, sizeof(float) * E * T * 6);
   if (cfg->noise_enable && !c->fused && cfg->radius_noise != 0.f) TS_ALLOC(c->ft_scratch_r, sizeof(float) * E * T * 6);
+  if (cfg->output_mask & (TS_OUT_DEPTH_NOISY | TS_OUT_PROX_NOISY)) {
+    TS_ALLOC(c->sn_h, sizeof(float4) * E * T);
+    TS_ALLOC(c->sn_d, sizeof(float2) * E * T);
+    if ((cfg->output_mask & TS_OUT_DEPTH_NOISY) && cfg->radius_noise != 0.f) TS_ALLOC(c->depth_pert, sizeof(float) * E * T);
+    if ((cfg->output_mask & TS_OUT_DEPTH_NOISY) && !(cfg->output_mask & TS_OUT_DEPTH)) TS_ALLOC(c->sc_depth, sizeof(float) * E * T);
+    if ((cfg->output_mask & TS_OUT_PROX_NOISY) && !(cfg->output_mask & TS_OUT_PROX)) TS_ALLOC(c->sc_prox, sizeof(float) * E * T);
+  }
+  if (cfg->output_mask & TS_OUT_MARKER_NOISY) {
+    TS_ALLOC(c->sm_h, sizeof(float) * E * M * 6);
+    TS_ALLOC(c->sm_d, sizeof(float) * E * M * 3);
+    if (!(cfg->output_mask & TS_OUT_MARKER)) TS_ALLOC(c->sc_marker, sizeof(float) * E * M * 3);
+  }
   if (cfg->noise_enable) {
     if (c->nh) TS_ALLOC(c->st_hyst, sizeof(float) * E * c->nh * c->Tp);
     TS_ALLOC(c->st_drift, sizeof(float) * E * 6 * c->Tp);
@@ -457,6 +491,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     TsStepParams p;
     fill_params(c, p);
     e = (cudaError_t)ts_launch_reset_state(p, nullptr, c->dead_thr, c->nh, nullptr);
+    if (e == cudaSuccess && (c->sn_d || c->sm_d)) e = (cudaError_t)ts_launch_reset_scalar(p, nullptr, nullptr);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
   }
   if (e != cudaSuccess) { ts_status s = cuda_fail(nullptr, e, "ts_create: upload"); free_all(c); delete c; return s; }
@@ -536,8 +571,9 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
       !in->obj_linvel || !in->obj_angvel)
     return fail(c, TS_ERR_INVALID_ARG, "ts_step: NULL input pointer");
   {  // output_mask contract (ts.h): bit set <=> pointer given
-    const void* ptr[7] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead};
-    for (int b = 0; b < 7; ++b) {
+    const void* ptr[10] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead,
+                           out->depth_noisy, out->prox_noisy, out->marker_noisy};
+    for (int b = 0; b < 10; ++b) {
       const bool want = (c->cfg.output_mask >> b) & 1u;
       if (want && !ptr[b]) return fail(c, TS_ERR_INVALID_ARG, "ts_step: an output declared in output_mask is NULL");
       if (!want && ptr[b]) return fail(c, TS_ERR_INVALID_ARG, "ts_step: an output not declared in output_mask is non-NULL");
@@ -556,6 +592,12 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
   p.obj_pos = in->obj_pos; p.obj_quat = in->obj_quat; p.obj_linvel = in->obj_linvel; p.obj_angvel = in->obj_angvel;
   p.contact = out->contact; p.depth = out->depth; p.ft = out->ft; p.marker = out->marker; p.prox = out->prox;
   p.ft_noisy = out->ft_noisy; p.dead = out->dead;
+  p.depth_noisy = out->depth_noisy; p.prox_noisy = out->prox_noisy; p.marker_noisy = out->marker_noisy;
+  const bool scalar_noisy = p.depth_noisy || p.prox_noisy || p.marker_noisy;
+  if (p.depth_noisy && !p.depth) p.depth = c->sc_depth;      // clean inputs of the noisy readouts the caller did not ask for
+  if (p.prox_noisy && !p.prox) p.prox = c->sc_prox;
+  if (p.marker_noisy && !p.marker) p.marker = c->sc_marker;
+  if (!p.depth_noisy) p.depth_pert = nullptr;
   cudaStream_t st = (cudaStream_t)stream;
   const bool split = c->cfg.noise_enable && !c->fused;
   if (split && !p.ft) {
@@ -575,6 +617,10 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
     e = (cudaError_t)ts_launch_noise(p, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: noise launch");
   }
+  if (scalar_noisy) {
+    e = (cudaError_t)ts_launch_scalar_noise(p, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: scalar noise launch");
+  }
   if (rec) TS_CUDA(c, cudaEventRecord(ev[3], st));
   c->gstep += 1;
   return TS_OK;
@@ -589,24 +635,27 @@ ts_status ts_step_host(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, 
   const float* hin[8] = {in->link_pos, in->link_quat, in->link_linvel, in->link_angvel,
                          in->obj_pos, in->obj_quat, in->obj_linvel, in->obj_angvel};
   const size_t in_bytes[8] = {E * L * 12, E * L * 16, E * L * 12, E * L * 12, E * K * 12, E * K * 16, E * K * 12, E * K * 12};
-  void* hout[7] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead};
-  const size_t out_bytes[7] = {E * T, E * T * 4, E * T * 24, E * (size_t)c->M * 12, E * T * 4, E * T * 24, E * T};
+  void* hout[10] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead,
+                    out->depth_noisy, out->prox_noisy, out->marker_noisy};
+  const size_t out_bytes[10] = {E * T, E * T * 4, E * T * 24, E * (size_t)c->M * 12, E * T * 4, E * T * 24, E * T,
+                                E * T * 4, E * T * 4, E * (size_t)c->M * 12};
   for (int i = 0; i < 8; ++i) {
     if (!hin[i]) return fail(c, TS_ERR_INVALID_ARG, "ts_step_host: NULL input pointer");
     if (!c->stage_in[i]) TS_CUDA(c, cudaMalloc((void**)&c->stage_in[i], in_bytes[i]));
     TS_CUDA(c, cudaMemcpyAsync(c->stage_in[i], hin[i], in_bytes[i], cudaMemcpyHostToDevice, st));
   }
-  for (int i = 0; i < 7; ++i)
+  for (int i = 0; i < 10; ++i)
     if (hout[i] && !c->stage_out[i]) TS_CUDA(c, cudaMalloc(&c->stage_out[i], out_bytes[i] ? out_bytes[i] : 16));
   ts_step_in din = {c->stage_in[0], c->stage_in[1], c->stage_in[2], c->stage_in[3],
                     c->stage_in[4], c->stage_in[5], c->stage_in[6], c->stage_in[7]};
   ts_step_out dout = {hout[0] ? (uint8_t*)c->stage_out[0] : nullptr, hout[1] ? (float*)c->stage_out[1] : nullptr,
                       hout[2] ? (float*)c->stage_out[2] : nullptr,   hout[3] ? (float*)c->stage_out[3] : nullptr,
                       hout[4] ? (float*)c->stage_out[4] : nullptr,   hout[5] ? (float*)c->stage_out[5] : nullptr,
-                      hout[6] ? (uint8_t*)c->stage_out[6] : nullptr};
+                      hout[6] ? (uint8_t*)c->stage_out[6] : nullptr, hout[7] ? (float*)c->stage_out[7] : nullptr,
+                      hout[8] ? (float*)c->stage_out[8] : nullptr,   hout[9] ? (float*)c->stage_out[9] : nullptr};
   const ts_status s = ts_step(c, &din, &dout, stream);
   if (s != TS_OK) return s;
-  for (int i = 0; i < 7; ++i)
+  for (int i = 0; i < 10; ++i)
     if (hout[i]) TS_CUDA(c, cudaMemcpyAsync(hout[i], c->stage_out[i], out_bytes[i], cudaMemcpyDeviceToHost, st));
   return TS_OK;
 }
@@ -618,6 +667,7 @@ ts_status ts_reset(ts_ctx* c, const uint8_t* env_mask_dev, void* stream) {
   fill_params(c, p);
   cudaError_t e = (cudaError_t)ts_launch_reset_counters(c->reset_step, c->episode, env_mask_dev, c->cfg.n_envs, c->gstep, stream);
   if (e == cudaSuccess) e = (cudaError_t)ts_launch_reset_state(p, env_mask_dev, c->dead_thr, c->nh, stream);
+  if (e == cudaSuccess && (c->sn_d || c->sm_d)) e = (cudaError_t)ts_launch_reset_scalar(p, env_mask_dev, stream);
   if (e != cudaSuccess) return cuda_fail(c, e, "ts_reset: launch");
   return TS_OK;
 }

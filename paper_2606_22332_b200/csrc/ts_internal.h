@@ -109,6 +109,17 @@ struct TsStepParams {
   float* prox;
   float* ft_noisy;
   uint8_t* dead;
+  // noisy scalar readouts (R10): outputs, the perturbed depth the step kernel leaves for them (Eq. 26), their state
+  float* depth_noisy;
+  float* prox_noisy;
+  float* marker_noisy;
+  float* depth_pert;          // [E,T] d~ = [R~_j - phi]_+ (written by the step kernel when radius noise is on), else NULL
+  float4* sn_h;               // [E,T] hysteresis of (depth, prox): Maxwell (xi_d, xprev_d, xi_p, xprev_p), ASYM (y_d, y_p, -, -)
+  float2* sn_d;               // [E,T] drift of (depth, prox)
+  float* sm_h;                // [E,M,6] marker hysteresis: 3 x (xi | y), 3 x x_prev
+  float* sm_d;                // [E,M,3] marker drift
+  float sn_sigma_white[3], sn_sigma_rw[3], sn_bias[3], sn_quant[3], sn_stuck_min[3], sn_stuck_max[3];
+  uint32_t dead_thr;          // floor(p_dead 2^32)
   // state
   uint8_t* st_flags;          // [E,T] bit0 Schmitt, bit1 dead
   float* st_hyst;             // [E,nh/2,Tp] float2 channel pairs, nh = 6 (asym: y) / 12 (maxwell: xi then x_prev)
@@ -149,6 +160,8 @@ struct TsStepParams {
 int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream);
 int ts_launch_noise(const TsStepParams& p, void* stream);
 int ts_launch_frames(const TsStepParams& p, void* stream);
+int ts_launch_scalar_noise(const TsStepParams& p, void* stream);
+int ts_launch_reset_scalar(const TsStepParams& p, const uint8_t* mask, void* stream);
 unsigned long long ts_frame_bytes();
 int ts_launch_retile(const float* src_linear, float4* dst, int n_grids, int N, void* stream);
 int ts_launch_reset_counters(uint32_t* reset_step, uint32_t* episode, const uint8_t* mask, int E, uint32_t gstep,

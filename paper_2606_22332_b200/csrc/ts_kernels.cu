@@ -1018,6 +1018,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     const double dd = Rt - phid;
     dn = dd > 0.0 ? (float)dd : 0.f;
   }
+  if (RN && p.depth_pert && valid) __stcs(p.depth_pert + ej, dn);   // input of the noisy depth readout (R10)
   float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   float fn6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};  // Eq. 4-9 at depth dn (dead code unless rn_on)
   const bool touch = d > 0.f || (rn_on && dn > 0.f);
@@ -1293,6 +1294,134 @@ __global__ void ts_reset_state_kernel(const __grid_constant__ TsStepParams p, co
   p.st_flags[(size_t)e * p.T + t] = fl;
 }
 
+// ---------------------------------------------------------------------------------------
+// R10: noisy readouts of the scalar sensors (Table 3: every knob of App. A.8 but crosstalk).
+// One channel: x = gamma clean -> hysteresis -> y = h + b + sigma_w z_w + D (Eq. 25) -> quantize -> dead: stuck value.
+// ---------------------------------------------------------------------------------------
+template <int MODE>
+__device__ __forceinline__ float scalar_chain(const TsStepParams& p, int cls, float clean, float gain, bool dead, float stuck_u,
+                                              float z_rw, float z_w, float& ha, float& hb, float& drift) {
+  const float x = gain * clean;
+  float h = x;
+  if (MODE == TS_HYST_MAXWELL) {            // Eq. 29-30
+    const float xi = fmaf(p.decay, ha, x - hb);
+    ha = xi; hb = x;
+    h = fmaf(p.beta, xi, x);
+  } else if (MODE == TS_HYST_ASYM) {        // D3, Q14
+    const float al = (fabsf(x) > fabsf(ha)) ? p.alpha_load : p.alpha_unload;
+    h = fmaf(al, x - ha, ha);
+    ha = h;
+  }
+  drift = fmaf(p.sn_sigma_rw[cls], z_rw, drift);
+  float y = fmaf(p.sn_sigma_white[cls], z_w, h + p.sn_bias[cls]) + drift;
+  const float q = p.sn_quant[cls];
+  if (q > 0.f) y = rintf(y / q) * q;        // quantize(., q): IEEE fp32 division, round half to even (R5)
+  if (dead) y = fmaf(p.sn_stuck_max[cls] - p.sn_stuck_min[cls], stuck_u, p.sn_stuck_min[cls]);
+  return y;
+}
+
+__device__ __forceinline__ float u24(uint32_t w) { return (float)(2u * (w >> 9) + 1u) * 5.9604644775390625e-8f; }
+
+// Threads [0, E T): depth + prox of one taxel (probe draws of the taxel: gain stream 3, dead flag from the state;
+// stream 10 -> (z_rw, z_w) of depth and of prox, stream 11 -> stuck values).  Threads [E T, E T + E M): the three
+// channels of one marker (probe 0x80000000 + m: streams 0 / 1 -> z_rw, z_w; 2 dead; 3 gain; 4 stuck).
+template <int MODE>
+__global__ void __launch_bounds__(256) ts_scalar_noise_kernel(const __grid_constant__ TsStepParams p) {
+  const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long ET = (long long)p.E * p.T, EM = (long long)p.E * p.M;
+  const bool gain_on = p.gain_min != 1.f || p.gain_max != 1.f;
+  if (gt < ET) {
+    if (!p.depth_noisy && !p.prox_noisy) return;
+    const int e = (int)(gt / p.T), j = (int)(gt - (long long)e * p.T);
+    const bool act = __ldg(&p.tx_pos[j].w) > 0.f;
+    float od = 0.f, op = 0.f;
+    if (act) {
+      const uint32_t ep4 = __ldg(p.episode + e) << 4, env = p.env_id_base + (uint32_t)e;
+      const uint32_t nstep = p.gstep - __ldg(p.reset_step + e);
+      const uint4 w = philox4x32_10(make_uint4(env, (uint32_t)j, nstep, ep4 | 10u), p.seed_lo, p.seed_hi);
+      float zd0, zd1, zp0, zp1;
+      box_muller(w.x, w.y, zd0, zd1);
+      box_muller(w.z, w.w, zp0, zp1);
+      const bool dead = (p.st_flags[gt] >> 1) & 1;
+      float gain = 1.f, su_d = 0.f, su_p = 0.f;
+      if (gain_on) gain = fmaf(p.gain_max - p.gain_min, u24(philox4x32_10(make_uint4(env, (uint32_t)j, 0u, ep4 | 3u), p.seed_lo, p.seed_hi).x), p.gain_min);
+      if (dead) {
+        const uint4 ws = philox4x32_10(make_uint4(env, (uint32_t)j, 0u, ep4 | 11u), p.seed_lo, p.seed_hi);
+        su_d = u24(ws.x); su_p = u24(ws.y);
+      }
+      float4 hs = MODE != TS_HYST_OFF ? p.sn_h[gt] : make_float4(0.f, 0.f, 0.f, 0.f);
+      float2 dr = p.sn_d[gt];
+      const float cd = p.depth_pert ? __ldcs(p.depth_pert + gt) : (p.depth ? p.depth[gt] : 0.f);
+      const float cp = p.prox ? p.prox[gt] : 0.f;
+      if (MODE == TS_HYST_MAXWELL) {
+        od = scalar_chain<MODE>(p, 0, cd, gain, dead, su_d, zd0, zd1, hs.x, hs.y, dr.x);
+        op = scalar_chain<MODE>(p, 1, cp, gain, dead, su_p, zp0, zp1, hs.z, hs.w, dr.y);
+      } else {
+        float dummy = 0.f;
+        od = scalar_chain<MODE>(p, 0, cd, gain, dead, su_d, zd0, zd1, hs.x, dummy, dr.x);
+        op = scalar_chain<MODE>(p, 1, cp, gain, dead, su_p, zp0, zp1, hs.y, dummy, dr.y);
+      }
+      if (MODE != TS_HYST_OFF) p.sn_h[gt] = hs;
+      p.sn_d[gt] = dr;
+    }
+    if (p.depth_noisy) __stcs(p.depth_noisy + gt, od);
+    if (p.prox_noisy) __stcs(p.prox_noisy + gt, op);
+  } else if (gt < ET + EM) {
+    if (!p.marker_noisy) return;
+    const long long gm = gt - ET;
+    const int e = (int)(gm / p.M), m = (int)(gm - (long long)e * p.M);
+    // a marker is active iff its patch is (link filter): marker normals of filtered patches stay, radii go to 0
+    const bool act = __ldg(&p.mk_pos[m].w) > 0.f;  // w = 1 for markers of active patches (set by ts_create)
+    float out[3] = {0.f, 0.f, 0.f};
+    if (act) {
+      const uint32_t ep4 = __ldg(p.episode + e) << 4, env = p.env_id_base + (uint32_t)e, probe = 0x80000000u + (uint32_t)m;
+      const uint32_t nstep = p.gstep - __ldg(p.reset_step + e);
+      const uint4 w0 = philox4x32_10(make_uint4(env, probe, nstep, ep4 | 0u), p.seed_lo, p.seed_hi);
+      const uint4 w1 = philox4x32_10(make_uint4(env, probe, nstep, ep4 | 1u), p.seed_lo, p.seed_hi);
+      float zr[4], zw[2];
+      box_muller(w0.x, w0.y, zr[0], zr[1]);
+      box_muller(w0.z, w0.w, zr[2], zr[3]);
+      box_muller(w1.x, w1.y, zw[0], zw[1]);
+      const bool dead = philox4x32_10(make_uint4(env, probe, 0u, ep4 | 2u), p.seed_lo, p.seed_hi).x < p.dead_thr;
+      float gain = 1.f;
+      if (gain_on) gain = fmaf(p.gain_max - p.gain_min, u24(philox4x32_10(make_uint4(env, probe, 0u, ep4 | 3u), p.seed_lo, p.seed_hi).x), p.gain_min);
+      uint4 ws = make_uint4(0u, 0u, 0u, 0u);
+      if (dead) ws = philox4x32_10(make_uint4(env, probe, 0u, ep4 | 4u), p.seed_lo, p.seed_hi);
+      const uint32_t wsv[3] = {ws.x, ws.y, ws.z};
+      float* hp = p.sm_h + gm * 6;
+      float* dp = p.sm_d + gm * 3;
+      const float* cm = p.marker + gm * 3;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        float ha = MODE != TS_HYST_OFF ? hp[c] : 0.f, hb = MODE == TS_HYST_MAXWELL ? hp[3 + c] : 0.f, dr = dp[c];
+        out[c] = scalar_chain<MODE>(p, 2, cm[c], gain, dead, u24(wsv[c]), zr[c], c == 0 ? zr[3] : zw[c - 1], ha, hb, dr);
+        if (MODE != TS_HYST_OFF) hp[c] = ha;
+        if (MODE == TS_HYST_MAXWELL) hp[3 + c] = hb;
+        dp[c] = dr;
+      }
+    }
+    float* o = p.marker_noisy + gm * 3;
+    __stcs(o, out[0]); __stcs(o + 1, out[1]); __stcs(o + 2, out[2]);
+  }
+}
+
+// zeroes the state of the noisy scalar readouts for the masked envs
+__global__ void ts_reset_scalar_kernel(const __grid_constant__ TsStepParams p, const uint8_t* mask) {
+  const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int per = p.T > p.M ? p.T : p.M;
+  if (gt >= (long long)p.E * per) return;
+  const int e = (int)(gt / per), i = (int)(gt - (long long)e * per);
+  if (mask && !mask[e]) return;
+  if (i < p.T && p.sn_d) {
+    p.sn_h[(size_t)e * p.T + i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    p.sn_d[(size_t)e * p.T + i] = make_float2(0.f, 0.f);
+  }
+  if (i < p.M && p.sm_d) {
+    for (int c = 0; c < 6; ++c) p.sm_h[((size_t)e * p.M + i) * 6 + c] = 0.f;
+    for (int c = 0; c < 3; ++c) p.sm_d[((size_t)e * p.M + i) * 3 + c] = 0.f;
+  }
+}
+
 }  // namespace
 
 unsigned long long ts_bank_elems_per_grid(int N) { return (unsigned long long)(N - 1) * (N - 1) * N; }
@@ -1375,6 +1504,24 @@ unsigned long long ts_frame_bytes() { return sizeof(FrameS); }
 int ts_launch_frames(const TsStepParams& p, void* stream) {
   const long long n = (long long)p.E * p.P * p.K;
   ts_frames_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(p);
+  return (int)cudaGetLastError();
+}
+
+int ts_launch_scalar_noise(const TsStepParams& p, void* stream) {
+  const long long n = (long long)p.E * p.T + (long long)p.E * p.M;
+  const unsigned blocks = (unsigned)((n + 255) / 256);
+  cudaStream_t st = (cudaStream_t)stream;
+  switch (p.hyst_mode) {
+    case TS_HYST_MAXWELL: ts_scalar_noise_kernel<TS_HYST_MAXWELL><<<blocks, 256, 0, st>>>(p); break;
+    case TS_HYST_ASYM: ts_scalar_noise_kernel<TS_HYST_ASYM><<<blocks, 256, 0, st>>>(p); break;
+    default: ts_scalar_noise_kernel<TS_HYST_OFF><<<blocks, 256, 0, st>>>(p); break;
+  }
+  return (int)cudaGetLastError();
+}
+
+int ts_launch_reset_scalar(const TsStepParams& p, const uint8_t* mask, void* stream) {
+  const long long n = (long long)p.E * (p.T > p.M ? p.T : p.M);
+  ts_reset_scalar_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(p, mask);
   return (int)cudaGetLastError();
 }
 

@@ -44,6 +44,8 @@ class Comparator:
         self.radius = np.asarray(radius, np.float64)
         self.noise_on = noise_on
         self.quant = (0.0, 0.0)   # Eq. 25 steps (force, torque); set by the caller when quantisation is on
+        self.sn_quant = tuple(float(np.float32((noise or {}).get("quant_" + c, 0.0))) for c in ("depth", "prox", "marker"))
+        self.sn_taint = {}
         self.contact_taint = None
         self.noisy_taint = None
         self.stats = dict(steps=0, contact_band=0, contact_tainted=0, ft_exempt=0, noisy_exempt=0, quant_exempt=0,
@@ -81,6 +83,29 @@ class Comparator:
                 self._check(k, gpu[k], ref[k], None)
         if "marker" in gpu:
             self._check("marker", gpu["marker"], ref["marker"], None)
+        # ---- noisy scalar readouts (R10): continuous in their inputs; only a quantisation flip (one step q while the
+        # pre-quantisation value sits within the tolerance of a rounding boundary) or, for the signed marker channels, an
+        # ASYM load/unload tie can legitimately differ; such elements are exempted, counted, and taint the hysteresis state
+        for k, cls in (("depth_noisy", 0), ("prox_noisy", 1), ("marker_noisy", 2)):
+            if k not in gpu:
+                continue
+            r = ref[k]
+            ex = np.zeros(r.shape, bool)
+            tol = ATOL + RTOL * np.abs(r)
+            q = self.sn_quant[cls]
+            if q > 0:
+                diff = np.abs(gpu[k].astype(np.float64) - r)
+                aq = ref["aux_sq_" + k.split("_")[0]]
+                ex |= (np.abs(diff - q) <= 1e-6 * np.maximum(np.abs(r), q)) & (aq < tol)
+            if k == "marker_noisy" and "aux_sasym_marker" in ref:
+                ex |= np.abs(ref["aux_sasym_marker"]) < BAND
+            t = self.sn_taint.setdefault(k, np.zeros(r.shape, np.int32))
+            t[:] = np.maximum(t - 1, 0)
+            t[ex] = self.taint_steps
+            exn = t > 0
+            st["sn_exempt"] = st.get("sn_exempt", 0) + int(exn.sum())
+            st["sn_checked"] = st.get("sn_checked", 0) + exn.size
+            self._check(k, gpu[k], r, exn)
         # ---- ft: exempt discontinuities of the normal / the d > 0 gate
         phi = ref["aux_phi"]
         active = self.radius[None, :] > 0

@@ -391,3 +391,48 @@ def test_two_objects_per_env():
     rep = cmp_.report()
     _assert_ok(rep)                                             # winner ties (|phi_k - phi_k'| < 1e-6) are a counted band
     assert rep["max_ratio"]["prox"] <= 1.0 and rep["checked"] > 1e6
+
+
+def test_noisy_scalar_readouts():
+    """SURVEY 8(f-1) / DESIGN.md R10: noisy depth, prox and marker readouts (Table 3 P:346-359 gives them every knob of
+    App. A.8 except crosstalk) with the Table 12 values and beyond: white noise, drift, bias, quantisation,
+    gain, dead probes with stuck values, both hysteresis modes, the Eq. 26 radius for the depth readout, over a reset,
+    with and without the clean outputs requested next to them."""
+    import torch
+    from oracle import oracle as O
+    from parity import Comparator
+    from paper_2606_22332_b200.binding import TactileSim
+    w = W.config(5, n_envs=48)
+    t12 = dict(sigma_white_depth=2e-4, sigma_white_prox=1e-2, sigma_rw_prox=1e-3, quant_prox=1e-2, sigma_white_marker=1e-4,
+               sigma_rw_marker=1e-5, quant_marker=1e-4, p_dead=0.05, gain_min=0.85, gain_max=1.15, radius_noise=3e-4)
+    more = dict(sigma_rw_depth=1e-5, bias_depth=1e-4, bias_prox=-1e-3, bias_marker=2e-3, quant_depth=5e-5, stuck_min_depth=1e-3,
+                stuck_max_depth=2e-3, stuck_min_prox=0.0, stuck_max_prox=0.02, stuck_min_marker=-0.1, stuck_max_marker=0.1)
+    full = w.outputs + ("depth_noisy", "prox_noisy", "marker_noisy")
+    only = ("contact", "ft", "ft_noisy", "dead", "depth_noisy", "prox_noisy", "marker_noisy")   # clean inputs from scratch buffers
+    cases = ((dict(w.noise, hyst_mode="maxwell", beta=0.5, tau=0.05, **t12), full),
+             (dict(w.noise, **t12, **more), full),
+             (dict(w.noise, hyst_mode="off", **more), only))
+    for noise, outs in cases:
+        sim = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=w.physics, noise=noise, outputs=outs)
+        sim.set_geometry(w.types, w.params, w.bank, w.voxel)
+        assert sim.launches_per_step() in (3, 4)
+        orc = O.Oracle(w.patches, w.T, w.L, w.K, np.arange(w.E), physics=w.physics, noise=noise, threads=os.cpu_count() or 1)
+        orc.set_geometry(w.types, w.params, w.bank, w.voxel)
+        lay = sim.layout.view()
+        cmp_ = Comparator(lay, w.physics, True, lay["radius"], noise=noise)
+        cmp_.quant = (float(np.float32(noise.get("quant_force", 0.0))), float(np.float32(noise.get("quant_torque", 0.0))))
+        for s in range(24):
+            if s == 12:
+                mask = (np.arange(w.E) % 3 == 0).astype(np.uint8)
+                sim.reset(torch.from_numpy(mask).cuda())
+                orc.reset(mask)
+            inp = w.inputs(s)
+            g = sim.step(sim.upload(inp))
+            torch.cuda.synchronize()
+            cmp_.step({k: v.cpu().numpy() for k, v in g.items()}, orc.step(inp, want=tuple(outs) + ("depth",)))   # the bands need depth
+        rep = cmp_.report()
+        _assert_ok(rep, max_band_frac=3e-3, max_noisy_frac=0.05)
+        assert rep["sn_checked"] > 1e6 and rep["sn_exempt"] <= 5e-3 * rep["sn_checked"], rep
+        for k in ("depth_noisy", "prox_noisy", "marker_noisy"):
+            assert rep["max_ratio"][k] <= 1.0
+        sim.close()
