@@ -268,6 +268,9 @@ typedef struct orc_params {
   // crosstalk; values Table 12; reading R10): per class {depth, prox, marker}
   // white sigma, random-walk sigma, bias, quantisation step, stuck range [l, u]
   float sn_sigma_white[3], sn_sigma_rw[3], sn_bias[3], sn_quant[3], sn_stuck_min[3], sn_stuck_max[3];
+  // Point-cloud ProximityTaxel (App. A.6, Eq. 12-17): sensing radius R_j, k, k_s, density scalar
+  // (0.01 m, 300, 10, 100)
+  float pc_radius, pc_k, pc_ks, pc_density;
 } orc_params;
 }
 
@@ -298,6 +301,11 @@ struct Oracle {
   double *aux_sq_depth = nullptr, *aux_sq_prox = nullptr, *aux_sq_marker = nullptr, *aux_sasym_marker = nullptr;
   std::vector<double> sn_ha, sn_hb, sn_dr;    // [E,T,2] depth, prox: hysteresis (xi | y), x_prev, drift
   std::vector<double> sm_ha, sm_hb, sm_dr;    // [E,M,3] marker channels
+  // point-cloud ProximityTaxel (A.6): bank of surface point clouds in the object frame, cloud id per (env, object)
+  std::vector<float> pc_pts;                  // [G,N,3]
+  int pc_G = 0, pc_N = 0;
+  std::vector<int32_t> pc_id;                 // [E,K], -1 = the object is not tracked
+  double* proxpc = nullptr;                   // [E,T,6] output handed in by orc_set_proxpc
   std::vector<std::deque<std::vector<double>>> hist;  // [E] the last Delta + J post-crosstalk fields [T,6] of the episode
   std::vector<uint32_t> n_step, episode;      // [E]
 };
@@ -657,6 +665,46 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
         prox[ej] = P;
         prox_c[j] = P;
       }
+      // A.6 point-cloud ProximityTaxel.  Tracked points p_i = p_O + R_O p_i^o of every tracked object;
+      // P_j = {i : |p_i - q_j| < R_j} (Eq. 12 set), P_ij = R_j - |p_i - q_j| (Eq. 12), point / taxel velocities with
+      // r_i = p_O, r_L = p_L (Eq. 13, Q4), tangential part (Eq. 14), density scale rho_b = density / max(N_active_b, 1)
+      // with N_active_b = tracked points of env b (Eq. 15, reading Q27), world force / torque (Eq. 16-17), reported
+      // as R_L^T f^w, R_L^T tau^w.
+      if (o.proxpc) {
+        double out6[6] = {0, 0, 0, 0, 0, 0};
+        if (active && o.pc_N > 0) {
+          long n_active = 0;
+          for (int k = 0; k < K; ++k) if (o.pc_id[(size_t)e * K + k] >= 0) n_active += o.pc_N;
+          const double rho = (double)pr.pc_density / (double)std::max(n_active, 1L);
+          const double Rj = (double)pr.pc_radius;
+          V3 vL = ld3(link_linvel + ((size_t)e * L + l) * 3), wL = ld3(link_angvel + ((size_t)e * L + l) * 3);
+          V3 vtax = vL + cross(wL, q - pL);                                  // Eq. 13
+          V3 fw = {0, 0, 0}, tw = {0, 0, 0};
+          for (int k = 0; k < K; ++k) {
+            const int id = o.pc_id[(size_t)e * K + k];
+            if (id < 0) continue;
+            V3 pO = ld3(obj_pos + ((size_t)e * K + k) * 3);
+            M3 RO = quat_to_R(obj_quat + ((size_t)e * K + k) * 4);
+            V3 vO = ld3(obj_linvel + ((size_t)e * K + k) * 3), wO = ld3(obj_angvel + ((size_t)e * K + k) * 3);
+            const float* pts = o.pc_pts.data() + (size_t)id * o.pc_N * 3;
+            for (int i = 0; i < o.pc_N; ++i) {
+              V3 pi = pO + mul(RO, ld3(pts + 3 * i));
+              V3 dv = pi - q;
+              double dist = norm(dv);
+              if (!(dist < Rj)) continue;                                    // P_j
+              double P = Rj - dist;                                          // Eq. 12
+              V3 vp = vO + cross(wO, pi - pO);                               // Eq. 13
+              V3 vr = vp - vtax;
+              V3 vt = vr - dot(vr, a) * a;                                   // Eq. 14
+              fw = fw + ((double)pr.pc_k * rho * P) * a + ((double)pr.pc_ks * rho * P) * vt;   // Eq. 16
+              tw = tw + ((double)pr.pc_k * rho * P) * cross(dv, a);          // Eq. 17
+            }
+          }
+          V3 fl = mulT(RL, fw), tl = mulT(RL, tw);
+          out6[0] = fl.x; out6[1] = fl.y; out6[2] = fl.z; out6[3] = tl.x; out6[4] = tl.y; out6[5] = tl.z;
+        }
+        for (int c = 0; c < 6; ++c) o.proxpc[ej * 6 + c] = out6[c];
+      }
     }
     // O6 (Eq. 18-21, 23 first sum; Q15-Q17): dilation of each patch's markers by its active taxels
     if (marker) {
@@ -930,6 +978,18 @@ void orc_set_aux_rgate(void* h, double* aux_rgate) { ((Oracle*)h)->aux_rgate = a
 // Comparator aid: aux_wingap[E,T] receives phi_second - phi_best over the K objects of the env (the margin by
 // which Eq. 2's winner g* won), +inf with fewer than two objects.  NULL switches it off.
 void orc_set_aux_wingap(void* h, double* aux_wingap) { ((Oracle*)h)->aux_wingap = aux_wingap; }
+
+// A.6: bank of tracked surface point clouds [n_clouds, n_points, 3] (object frame, fp32, copied) and the cloud of each
+// (env, object) (-1 = not tracked); orc_set_proxpc hands in the [E,T,6] output the following orc_step calls fill.
+int orc_set_pointclouds(void* h, int n_clouds, int n_points, const float* pts, const int32_t* cloud_id) {
+  Oracle& o = *(Oracle*)h;
+  o.pc_G = n_clouds; o.pc_N = n_points;
+  o.pc_pts.assign(pts, pts + (size_t)n_clouds * n_points * 3);
+  o.pc_id.assign(cloud_id, cloud_id + (size_t)o.E * o.K);
+  for (int32_t id : o.pc_id) if (id >= n_clouds) return 1;
+  return 0;
+}
+void orc_set_proxpc(void* h, double* proxpc) { ((Oracle*)h)->proxpc = proxpc; }
 
 // R10: hands in the buffers the following orc_step calls fill with the noisy scalar readouts (NULL = not produced) and
 // their comparator aids (distance to the quantisation boundary per element; marker ASYM sign-flip margin).

@@ -48,7 +48,8 @@ class OrcParams(C.Structure):
                 ("stuck_min_torque", C.c_float), ("stuck_max_torque", C.c_float), ("xtalk_sigma", C.c_float),
                 ("radius_noise", C.c_float), ("read_delay", C.c_int32), ("read_jitter", C.c_int32),
                 ("sn_sigma_white", C.c_float * 3), ("sn_sigma_rw", C.c_float * 3), ("sn_bias", C.c_float * 3),
-                ("sn_quant", C.c_float * 3), ("sn_stuck_min", C.c_float * 3), ("sn_stuck_max", C.c_float * 3)]
+                ("sn_quant", C.c_float * 3), ("sn_stuck_min", C.c_float * 3), ("sn_stuck_max", C.c_float * 3),
+                ("pc_radius", C.c_float), ("pc_k", C.c_float), ("pc_ks", C.c_float), ("pc_density", C.c_float)]
 
 SN_CLASS = {"depth": 0, "prox": 1, "marker": 2}          # noisy scalar readouts (R10)
 SN_KNOBS = ("sigma_white", "sigma_rw", "bias", "quant", "stuck_min", "stuck_max")
@@ -87,6 +88,8 @@ def lib():
         L.orc_set_aux_rgate.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_set_aux_wingap.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_set_scalar_noisy.argtypes = [C.c_void_p] + [C.c_void_p] * 7
+        L.orc_set_pointclouds.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.orc_set_proxpc.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_max_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -112,7 +115,8 @@ def make_params(physics=None, noise=None):
              alpha_load=1.0, alpha_unload=1.0, p_dead=0.0, chi=0.0,
              sigma_white_force=0.0, sigma_white_torque=0.0, bias_force=0.0, bias_torque=0.0, quant_force=0.0,
              quant_torque=0.0, gain_min=1.0, gain_max=1.0, stuck_min_force=0.0, stuck_max_force=0.0,
-             stuck_min_torque=0.0, stuck_max_torque=0.0, xtalk_sigma=0.0, radius_noise=0.0, read_delay=0, read_jitter=0)
+             stuck_min_torque=0.0, stuck_max_torque=0.0, xtalk_sigma=0.0, radius_noise=0.0, read_delay=0, read_jitter=0,
+             pc_radius=0.01, pc_k=300.0, pc_ks=10.0, pc_density=100.0)          # A.6 constants
     sn = {}
     for src in (physics, noise):
         if src:
@@ -201,6 +205,14 @@ class Oracle:
         if rc:
             raise ValueError("orc_set_geometry: grid id out of range")
 
+    def set_pointclouds(self, points, cloud_id):
+        """A.6: points [G, N, 3] fp32 (object frame); cloud_id [E, K] int32 (-1 = object not tracked)."""
+        pts = _f32(points)
+        cid = np.ascontiguousarray(cloud_id, dtype=np.int32).reshape(self.E, self.K)
+        self._pc = True
+        if self.L.orc_set_pointclouds(self.h, pts.shape[0], pts.shape[1], _p(pts), _p(cid)):
+            raise ValueError("orc_set_pointclouds: cloud id out of range")
+
     def reset(self, env_mask=None):
         m = None if env_mask is None else np.ascontiguousarray(env_mask, dtype=np.uint8)
         self.L.orc_reset(self.h, _p(m))
@@ -217,6 +229,7 @@ class Oracle:
         if "ft" in want: out["ft"] = np.zeros((E, T, 6))
         if "marker" in want and M > 0: out["marker"] = np.zeros((E, M, 3))
         if "prox" in want: out["prox"] = np.zeros((E, T))
+        if "proxpc" in want: out["proxpc"] = np.zeros((E, T, 6))
         if self.params.noise_enable:
             if "ft_noisy" in want: out["ft_noisy"] = np.zeros((E, T, 6))
             if "dead" in want: out["dead"] = np.zeros((E, T), np.uint8)
@@ -246,6 +259,7 @@ class Oracle:
         self.L.orc_set_aux_quant(self.h, _p(g("aux_quant")))
         self.L.orc_set_aux_rgate(self.h, _p(g("aux_rgate")))
         self.L.orc_set_aux_wingap(self.h, _p(g("aux_wingap")))
+        self.L.orc_set_proxpc(self.h, _p(g("proxpc")))
         self.L.orc_set_scalar_noisy(self.h, _p(g("depth_noisy")), _p(g("prox_noisy")), _p(g("marker_noisy")), _p(g("aux_sq_depth")),
                                     _p(g("aux_sq_prox")), _p(g("aux_sq_marker")), _p(g("aux_sasym_marker")))
         self.L.orc_step(self.h, _p(a["link_pos"]), _p(a["link_quat"]), _p(a["link_linvel"]), _p(a["link_angvel"]),
