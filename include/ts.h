@@ -127,7 +127,9 @@ enum {                      /* output_mask bits.  ts_step contract: every output
      need noise_enable */
   TS_OUT_DEPTH_NOISY = 1 << 7,  /* f32 [E,T]   ContactDepth readout; senses with the Eq. 26 radius when radius_noise > 0 */
   TS_OUT_PROX_NOISY = 1 << 8,   /* f32 [E,T]   Proximity readout */
-  TS_OUT_MARKER_NOISY = 1 << 9  /* f32 [E,M,3] Elastomer marker readout (every marker is a probe of its own) */
+  TS_OUT_MARKER_NOISY = 1 << 9, /* f32 [E,M,3] Elastomer marker readout (every marker is a probe of its own) */
+  TS_OUT_PROXPC = 1 << 10       /* f32 [E,T,6] point-cloud ProximityTaxel (App. A.6, Eq. 12-17), link frame; needs
+                                   ts_set_pointclouds */
 };
 
 typedef struct ts_config {
@@ -187,6 +189,9 @@ typedef struct ts_config {
    * ones above; depth / prox share their taxel's gain and dead draw, a marker draws its own.  Table 12 P:523-535:
    * depth sigma 2e-4 m; proximity sigma 1e-2, rw 1e-3, quant 1e-2; elastomer sigma 1e-4 m, rw 1e-5 m, quant 1e-4 m. */
   float sn_sigma_white[3], sn_sigma_rw[3], sn_bias[3], sn_quant[3], sn_stuck_min[3], sn_stuck_max[3];
+  /* Point-cloud ProximityTaxel (App. A.6): sensing radius R_j [m], k, k_s, density scalar (0.01, 300,
+   * 10, 100; ts_config_default sets these).  rho_b = density / max(N_b, 1), N_b = tracked points of env b (Q27). */
+  float pc_radius, pc_k, pc_ks, pc_density;
 } ts_config;
 
 /* Fills *cfg with the paper's constants and everything else zero / off. */
@@ -236,6 +241,7 @@ typedef struct ts_step_out {
   float* depth_noisy;  /* [E,T]   */
   float* prox_noisy;   /* [E,T]   */
   float* marker_noisy; /* [E,M,3] */
+  float* proxpc;       /* [E,T,6] */
 } ts_step_out;
 
 /* Creates a context on `cuda_device` (must be sm_100).  Allocates every device buffer the
@@ -247,6 +253,18 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out);
  * kernel on `stream`).  May be called again to replace the geometry.  Synchronises `stream`
  * once before returning, so host arrays may be freed immediately. */
 ts_status ts_set_geometry(ts_ctx* ctx, const ts_geometry* geo, void* stream);
+
+/* App. A.6: "tracked links are sampled into a surface point cloud at scene reset and organized in a static BVH".
+ * Here: a bank of n_clouds clouds of n_points points each, in the OBJECT frame (host fp32 [G,N,3]), and the cloud of every
+ * (env, object) (host int32 [E,K], -1 = not tracked).  The ctx sorts each cloud into a uniform grid of cell size
+ * pc_radius (the static spatial index; a taxel's sensing sphere meets at most 27 cells) and keeps it on the device.
+ * Needed before a ts_step that asks for TS_OUT_PROXPC.  Synchronises `stream` once; may be called again. */
+typedef struct ts_pointclouds {
+  int32_t n_clouds, n_points;
+  const float* points;
+  const int32_t* cloud_id;
+} ts_pointclouds;
+ts_status ts_set_pointclouds(ts_ctx* ctx, const ts_pointclouds* pc, void* stream);
 
 /* One pass of the whole hot path over all envs.  Asynchronous; never allocates. */
 ts_status ts_step(ts_ctx* ctx, const ts_step_in* in, const ts_step_out* out, void* stream);

@@ -18,13 +18,13 @@ HYST = {"off": 0, "maxwell": 1, "asym": 2}
 FORM = {"auto": 0, "fused": 1, "split": 2}
 GEOM = {"none": 0, "sphere": 1, "box": 2, "capsule": 3, "sdf": 4, "grid": 4}
 OUT_BITS = {"contact": 1, "depth": 2, "ft": 4, "marker": 8, "prox": 16, "ft_noisy": 32, "dead": 64,
-            "depth_noisy": 128, "prox_noisy": 256, "marker_noisy": 512}
+            "depth_noisy": 128, "prox_noisy": 256, "marker_noisy": 512, "proxpc": 1024}
 SN_CLASS = {"depth": 0, "prox": 1, "marker": 2}          # noisy scalar readouts (ts_config.sn_*[3])
 SN_KNOBS = ("sigma_white", "sigma_rw", "bias", "quant", "stuck_min", "stuck_max")
 
 # every symbol include/ts.h declares (tests check that the library exports them all)
 SYMBOLS = ["ts_layout_create", "ts_layout_add_patch", "ts_layout_filter_links", "ts_layout_finalize", "ts_layout_get",
-           "ts_layout_destroy", "ts_config_default", "ts_create", "ts_set_geometry", "ts_step", "ts_step_host",
+           "ts_layout_destroy", "ts_config_default", "ts_create", "ts_set_geometry", "ts_set_pointclouds", "ts_step", "ts_step_host",
            "ts_reset", "ts_destroy", "ts_last_error", "ts_n_taxels", "ts_n_markers", "ts_launches_per_step",
            "ts_kernel_time_ms", "ts_kernel_times_ms", "ts_first_kernel_time_ms", "ts_version"]
 
@@ -71,7 +71,12 @@ class Config(C.Structure):
                 ("radius_noise", C.c_float), ("read_delay", C.c_int32), ("read_jitter", C.c_int32),
                 ("kernel_form", C.c_int32),
                 ("sn_sigma_white", C.c_float * 3), ("sn_sigma_rw", C.c_float * 3), ("sn_bias", C.c_float * 3),
-                ("sn_quant", C.c_float * 3), ("sn_stuck_min", C.c_float * 3), ("sn_stuck_max", C.c_float * 3)]
+                ("sn_quant", C.c_float * 3), ("sn_stuck_min", C.c_float * 3), ("sn_stuck_max", C.c_float * 3),
+                ("pc_radius", C.c_float), ("pc_k", C.c_float), ("pc_ks", C.c_float), ("pc_density", C.c_float)]
+
+
+class PointClouds(C.Structure):
+    _fields_ = [("n_clouds", C.c_int32), ("n_points", C.c_int32), ("points", C.c_void_p), ("cloud_id", C.c_void_p)]
 
 
 class Geometry(C.Structure):
@@ -86,7 +91,7 @@ class StepIn(C.Structure):
 
 class StepOut(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in ("contact", "depth", "ft", "marker", "prox", "ft_noisy", "dead", "depth_noisy",
-                                          "prox_noisy", "marker_noisy")]
+                                          "prox_noisy", "marker_noisy", "proxpc")]
 
 
 IN_KEYS = [k for k, _ in StepIn._fields_]
@@ -113,6 +118,7 @@ def lib():
         L.ts_config_default.restype = None
         L.ts_create.argtypes = [C.POINTER(Config), C.c_int, C.POINTER(vp)]
         L.ts_set_geometry.argtypes = [vp, C.POINTER(Geometry), vp]
+        L.ts_set_pointclouds.argtypes = [vp, C.POINTER(PointClouds), vp]
         L.ts_step.argtypes = [vp, C.POINTER(StepIn), C.POINTER(StepOut), vp]
         L.ts_step_host.argtypes = [vp, C.POINTER(StepIn), C.POINTER(StepOut), vp]
         L.ts_reset.argtypes = [vp, vp, vp]
@@ -248,7 +254,7 @@ class TactileSim:
         return dict(contact=((E, T), t.uint8), depth=((E, T), t.float32), ft=((E, T, 6), t.float32),
                     marker=((E, M, 3), t.float32), prox=((E, T), t.float32), ft_noisy=((E, T, 6), t.float32),
                     dead=((E, T), t.uint8), depth_noisy=((E, T), t.float32), prox_noisy=((E, T), t.float32),
-                    marker_noisy=((E, M, 3), t.float32))
+                    marker_noisy=((E, M, 3), t.float32), proxpc=((E, T, 6), t.float32))
 
     def in_shapes(self):
         E, L, K = self.E, self.L, self.K
@@ -278,6 +284,14 @@ class TactileSim:
             g.grids = bank.ctypes.data_as(C.c_void_p)
         with self.torch.cuda.device(self.device):
             _check(lib().ts_set_geometry(self.h, C.byref(g), self._stream()), self.h, "ts_set_geometry")
+
+    def set_pointclouds(self, points, cloud_id):
+        """App. A.6: points [G, N, 3] fp32 in the object frame; cloud_id [E, K] int32 (-1 = object not tracked)."""
+        pts = np.ascontiguousarray(points, dtype=np.float32)
+        cid = np.ascontiguousarray(cloud_id, dtype=np.int32).reshape(self.E, self.K)
+        pc = PointClouds(pts.shape[0], pts.shape[1], pts.ctypes.data_as(C.c_void_p), cid.ctypes.data_as(C.c_void_p))
+        with self.torch.cuda.device(self.device):
+            _check(lib().ts_set_pointclouds(self.h, C.byref(pc), self._stream()), self.h, "ts_set_pointclouds")
 
     def _structs(self, inp, out, host):
         si, so = StepIn(), StepOut()

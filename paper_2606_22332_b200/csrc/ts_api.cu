@@ -52,7 +52,11 @@ struct ts_ctx {
   uint32_t *reset_step = nullptr, *episode = nullptr;
   // device staging of ts_step_host
   float* stage_in[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-  void* stage_out[10] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  void* stage_out[11] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  // point-cloud ProximityTaxel (A.6): clouds sorted by grid cell, cell starts, grid records, cloud of each (env, object)
+  float4* pc_pts = nullptr; int32_t* pc_cell = nullptr; TsPcGrid* pc_grid = nullptr; int32_t* pc_id = nullptr;
+  int32_t* tx_patch = nullptr;
+  int pc_n = 0; bool have_pc = false;
   // noisy scalar readouts (R10): state, the perturbed depth (Eq. 26), scratch copies of clean inputs the caller did not ask for
   float4* sn_h = nullptr; float2* sn_d = nullptr; float *sm_h = nullptr, *sm_d = nullptr;
   float *depth_pert = nullptr, *sc_depth = nullptr, *sc_prox = nullptr, *sc_marker = nullptr;
@@ -98,6 +102,7 @@ void free_all(ts_ctx* c) {
   cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->mk_tab8); cudaFree(c->grp_link);
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->env_perm); cudaFree(c->frames_g); cudaFree(c->patch_link); cudaFree(c->bank); cudaFree(c->bank_stage); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch); cudaFree(c->ft_scratch_r); cudaFree(c->st_ring);
+  cudaFree(c->pc_pts); cudaFree(c->pc_cell); cudaFree(c->pc_grid); cudaFree(c->pc_id); cudaFree(c->tx_patch);
   cudaFree(c->sn_h); cudaFree(c->sn_d); cudaFree(c->sm_h); cudaFree(c->sm_d); cudaFree(c->depth_pert); cudaFree(c->sc_depth);
   cudaFree(c->sc_prox); cudaFree(c->sc_marker);
   for (float* q : c->stage_in) cudaFree(q);
@@ -173,6 +178,8 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
     p.sn_quant[k] = g.sn_quant[k]; p.sn_stuck_min[k] = g.sn_stuck_min[k]; p.sn_stuck_max[k] = g.sn_stuck_max[k];
   }
   p.dead_thr = c->dead_thr;
+  p.pc_pts = c->pc_pts; p.pc_cell = c->pc_cell; p.pc_grid = c->pc_grid; p.pc_id = c->pc_id; p.pc_n = c->pc_n; p.tx_patch = c->tx_patch;
+  p.pc_radius = g.pc_radius; p.pc_k = g.pc_k; p.pc_ks = g.pc_ks; p.pc_density = g.pc_density;
 }
 }  // namespace
 
@@ -193,6 +200,7 @@ void ts_config_default(ts_config* c) {
   c->dt = 0.005f;
   c->tau = 0.05f; c->beta = 0.5f; c->alpha_load = 1.f; c->alpha_unload = 1.f;
   c->gain_min = 1.f; c->gain_max = 1.f;                                             // Eq. 27 off
+  c->pc_radius = 0.01f; c->pc_k = 300.f; c->pc_ks = 10.f; c->pc_density = 100.f;    // A.6 P:267
   c->output_mask = TS_OUT_CONTACT | TS_OUT_DEPTH | TS_OUT_FT | TS_OUT_MARKER | TS_OUT_PROX;
 }
 
@@ -202,7 +210,8 @@ int32_t ts_n_markers(const ts_ctx* ctx) { return ctx ? ctx->M : 0; }
 int32_t ts_launches_per_step(const ts_ctx* ctx) {
   if (!ctx) return 0;
   return ((ctx->cfg.noise_enable && !ctx->fused) ? 3 : 2) +
-         ((ctx->cfg.output_mask & (TS_OUT_DEPTH_NOISY | TS_OUT_PROX_NOISY | TS_OUT_MARKER_NOISY)) ? 1 : 0);
+         ((ctx->cfg.output_mask & (TS_OUT_DEPTH_NOISY | TS_OUT_PROX_NOISY | TS_OUT_MARKER_NOISY)) ? 1 : 0) +
+         ((ctx->cfg.output_mask & TS_OUT_PROXPC) ? 1 : 0);
 }
 
 ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
@@ -417,6 +426,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   } while (0)
   TS_ALLOC(c->tx_pos, sizeof(float4) * T);
   TS_ALLOC(c->tx_meta, sizeof(int32_t) * T);
+  TS_ALLOC(c->tx_patch, sizeof(int32_t) * T);
   TS_ALLOC(c->mk_pos, sizeof(float4) * mpos.size());
   TS_ALLOC(c->mk_nrm, sizeof(float4) * mnrm.size());
   TS_ALLOC(c->patches, sizeof(TsPatch) * pts.size());
@@ -468,6 +478,12 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   auto cp = [&](void* d, const void* h, size_t b) { if (e == cudaSuccess) e = cudaMemcpy(d, h, b, cudaMemcpyHostToDevice); };
   cp(c->tx_pos, pos.data(), sizeof(float4) * T);
   cp(c->tx_meta, meta.data(), sizeof(int32_t) * T);
+  {
+    std::vector<int32_t> tpatch(T, 0);
+    for (size_t pi = 0; pi < pts.size(); ++pi)
+      for (int t = pts[pi].start; t < pts[pi].start + pts[pi].n && t < T; ++t) tpatch[t] = (int32_t)pi;
+    cp(c->tx_patch, tpatch.data(), sizeof(int32_t) * T);
+  }
   cp(c->mk_pos, mpos.data(), sizeof(float4) * mpos.size());
   cp(c->mk_nrm, mnrm.data(), sizeof(float4) * mnrm.size());
   cp(c->patches, pts.data(), sizeof(TsPatch) * pts.size());
@@ -563,6 +579,71 @@ ts_status ts_set_geometry(ts_ctx* c, const ts_geometry* geo, void* stream) {
   return TS_OK;
 }
 
+ts_status ts_set_pointclouds(ts_ctx* c, const ts_pointclouds* pc, void* stream) {
+  if (!c) return TS_ERR_INVALID_ARG;
+  if (!pc || !pc->points || !pc->cloud_id || pc->n_clouds < 1 || pc->n_points < 1)
+    return fail(c, TS_ERR_INVALID_ARG, "ts_set_pointclouds: NULL argument or empty bank");
+  if (!(c->cfg.pc_radius > 0.f)) return fail(c, TS_ERR_INVALID_ARG, "ts_set_pointclouds: pc_radius must be > 0");
+  const int G = pc->n_clouds, N = pc->n_points;
+  const size_t EK = (size_t)c->cfg.n_envs * c->cfg.objs_per_env;
+  for (size_t i = 0; i < EK; ++i)
+    if (pc->cloud_id[i] >= G) return fail(c, TS_ERR_INVALID_ARG, "ts_set_pointclouds: cloud id out of range");
+  if ((long long)G * N >= (1LL << 31)) return fail(c, TS_ERR_UNSUPPORTED, "ts_set_pointclouds: bank larger than 2^31 points");
+  // static spatial index ("organized in a static BVH"): per cloud a uniform grid with cell = sensing radius,
+  // points counting-sorted by linear cell index (x fastest), cell_start[ncell + 1]
+  const float cell = c->cfg.pc_radius;
+  std::vector<TsPcGrid> grids(G);
+  std::vector<int32_t> cells;
+  std::vector<float4> sorted((size_t)G * N);
+  for (int g = 0; g < G; ++g) {
+    const float* P = pc->points + (size_t)g * N * 3;
+    float lo[3] = {P[0], P[1], P[2]}, hi[3] = {P[0], P[1], P[2]};
+    for (int i = 0; i < N; ++i)
+      for (int a = 0; a < 3; ++a) {
+        if (!std::isfinite(P[3 * i + a])) return fail(c, TS_ERR_INVALID_ARG, "ts_set_pointclouds: non-finite point");
+        lo[a] = std::fmin(lo[a], P[3 * i + a]); hi[a] = std::fmax(hi[a], P[3 * i + a]);
+      }
+    TsPcGrid& gr = grids[g];
+    gr.ox = lo[0]; gr.oy = lo[1]; gr.oz = lo[2]; gr.inv_cell = 1.0f / cell;
+    gr.nx = (int)std::floor((hi[0] - lo[0]) * gr.inv_cell) + 1; gr.ny = (int)std::floor((hi[1] - lo[1]) * gr.inv_cell) + 1;
+    gr.nz = (int)std::floor((hi[2] - lo[2]) * gr.inv_cell) + 1;
+    const long long ncell = (long long)gr.nx * gr.ny * gr.nz;
+    if (ncell > (1LL << 26)) return fail(c, TS_ERR_UNSUPPORTED, "ts_set_pointclouds: cloud extent / pc_radius too large for the grid");
+    gr.cell0 = (int32_t)cells.size(); gr.pt0 = g * N;
+    std::vector<int32_t> cidx(N), start((size_t)ncell + 1, 0);
+    for (int i = 0; i < N; ++i) {
+      // the same fp32 expression the kernel uses for the taxel's cell
+      int ci = (int)std::floor((P[3 * i] - gr.ox) * gr.inv_cell), cj = (int)std::floor((P[3 * i + 1] - gr.oy) * gr.inv_cell),
+          ck = (int)std::floor((P[3 * i + 2] - gr.oz) * gr.inv_cell);
+      ci = std::min(std::max(ci, 0), gr.nx - 1); cj = std::min(std::max(cj, 0), gr.ny - 1); ck = std::min(std::max(ck, 0), gr.nz - 1);
+      cidx[i] = (ck * gr.ny + cj) * gr.nx + ci;
+      start[(size_t)cidx[i] + 1] += 1;
+    }
+    for (long long k = 0; k < ncell; ++k) start[k + 1] += start[k];
+    std::vector<int32_t> fill(start.begin(), start.end() - 1);
+    for (int i = 0; i < N; ++i) sorted[(size_t)g * N + fill[cidx[i]]++] = make_float4(P[3 * i], P[3 * i + 1], P[3 * i + 2], 0.f);
+    cells.insert(cells.end(), start.begin(), start.end());
+  }
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  c->have_pc = false;
+  TS_CUDA(c, cudaStreamSynchronize(st));   // steps in flight may still read the old index
+  cudaFree(c->pc_pts); cudaFree(c->pc_cell); cudaFree(c->pc_grid); cudaFree(c->pc_id);
+  c->pc_pts = nullptr; c->pc_cell = nullptr; c->pc_grid = nullptr; c->pc_id = nullptr;
+  TS_CUDA(c, cudaMalloc((void**)&c->pc_pts, sizeof(float4) * sorted.size()));
+  TS_CUDA(c, cudaMalloc((void**)&c->pc_cell, sizeof(int32_t) * cells.size()));
+  TS_CUDA(c, cudaMalloc((void**)&c->pc_grid, sizeof(TsPcGrid) * G));
+  TS_CUDA(c, cudaMalloc((void**)&c->pc_id, sizeof(int32_t) * EK));
+  TS_CUDA(c, cudaMemcpyAsync(c->pc_pts, sorted.data(), sizeof(float4) * sorted.size(), cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaMemcpyAsync(c->pc_cell, cells.data(), sizeof(int32_t) * cells.size(), cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaMemcpyAsync(c->pc_grid, grids.data(), sizeof(TsPcGrid) * G, cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaMemcpyAsync(c->pc_id, pc->cloud_id, sizeof(int32_t) * EK, cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaStreamSynchronize(st));
+  c->pc_n = N;
+  c->have_pc = true;
+  return TS_OK;
+}
+
 ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void* stream) {
   if (!c) return TS_ERR_INVALID_ARG;
   if (!in || !out) return fail(c, TS_ERR_INVALID_ARG, "ts_step: NULL argument");
@@ -571,9 +652,9 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
       !in->obj_linvel || !in->obj_angvel)
     return fail(c, TS_ERR_INVALID_ARG, "ts_step: NULL input pointer");
   {  // output_mask contract (ts.h): bit set <=> pointer given
-    const void* ptr[10] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead,
-                           out->depth_noisy, out->prox_noisy, out->marker_noisy};
-    for (int b = 0; b < 10; ++b) {
+    const void* ptr[11] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead,
+                           out->depth_noisy, out->prox_noisy, out->marker_noisy, out->proxpc};
+    for (int b = 0; b < 11; ++b) {
       const bool want = (c->cfg.output_mask >> b) & 1u;
       if (want && !ptr[b]) return fail(c, TS_ERR_INVALID_ARG, "ts_step: an output declared in output_mask is NULL");
       if (!want && ptr[b]) return fail(c, TS_ERR_INVALID_ARG, "ts_step: an output not declared in output_mask is non-NULL");
@@ -593,6 +674,8 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
   p.contact = out->contact; p.depth = out->depth; p.ft = out->ft; p.marker = out->marker; p.prox = out->prox;
   p.ft_noisy = out->ft_noisy; p.dead = out->dead;
   p.depth_noisy = out->depth_noisy; p.prox_noisy = out->prox_noisy; p.marker_noisy = out->marker_noisy;
+  p.proxpc = out->proxpc;
+  if (p.proxpc && !c->have_pc) return fail(c, TS_ERR_STATE, "ts_step: proxpc requested before ts_set_pointclouds");
   const bool scalar_noisy = p.depth_noisy || p.prox_noisy || p.marker_noisy;
   if (p.depth_noisy && !p.depth) p.depth = c->sc_depth;      // clean inputs of the noisy readouts the caller did not ask for
   if (p.prox_noisy && !p.prox) p.prox = c->sc_prox;
@@ -617,6 +700,10 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
     e = (cudaError_t)ts_launch_noise(p, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: noise launch");
   }
+  if (p.proxpc) {
+    e = (cudaError_t)ts_launch_proxpc(p, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: proxpc launch");
+  }
   if (scalar_noisy) {
     e = (cudaError_t)ts_launch_scalar_noise(p, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: scalar noise launch");
@@ -635,16 +722,16 @@ ts_status ts_step_host(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, 
   const float* hin[8] = {in->link_pos, in->link_quat, in->link_linvel, in->link_angvel,
                          in->obj_pos, in->obj_quat, in->obj_linvel, in->obj_angvel};
   const size_t in_bytes[8] = {E * L * 12, E * L * 16, E * L * 12, E * L * 12, E * K * 12, E * K * 16, E * K * 12, E * K * 12};
-  void* hout[10] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead,
-                    out->depth_noisy, out->prox_noisy, out->marker_noisy};
-  const size_t out_bytes[10] = {E * T, E * T * 4, E * T * 24, E * (size_t)c->M * 12, E * T * 4, E * T * 24, E * T,
-                                E * T * 4, E * T * 4, E * (size_t)c->M * 12};
+  void* hout[11] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead,
+                    out->depth_noisy, out->prox_noisy, out->marker_noisy, out->proxpc};
+  const size_t out_bytes[11] = {E * T, E * T * 4, E * T * 24, E * (size_t)c->M * 12, E * T * 4, E * T * 24, E * T,
+                                E * T * 4, E * T * 4, E * (size_t)c->M * 12, E * T * 24};
   for (int i = 0; i < 8; ++i) {
     if (!hin[i]) return fail(c, TS_ERR_INVALID_ARG, "ts_step_host: NULL input pointer");
     if (!c->stage_in[i]) TS_CUDA(c, cudaMalloc((void**)&c->stage_in[i], in_bytes[i]));
     TS_CUDA(c, cudaMemcpyAsync(c->stage_in[i], hin[i], in_bytes[i], cudaMemcpyHostToDevice, st));
   }
-  for (int i = 0; i < 10; ++i)
+  for (int i = 0; i < 11; ++i)
     if (hout[i] && !c->stage_out[i]) TS_CUDA(c, cudaMalloc(&c->stage_out[i], out_bytes[i] ? out_bytes[i] : 16));
   ts_step_in din = {c->stage_in[0], c->stage_in[1], c->stage_in[2], c->stage_in[3],
                     c->stage_in[4], c->stage_in[5], c->stage_in[6], c->stage_in[7]};
@@ -652,10 +739,11 @@ ts_status ts_step_host(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, 
                       hout[2] ? (float*)c->stage_out[2] : nullptr,   hout[3] ? (float*)c->stage_out[3] : nullptr,
                       hout[4] ? (float*)c->stage_out[4] : nullptr,   hout[5] ? (float*)c->stage_out[5] : nullptr,
                       hout[6] ? (uint8_t*)c->stage_out[6] : nullptr, hout[7] ? (float*)c->stage_out[7] : nullptr,
-                      hout[8] ? (float*)c->stage_out[8] : nullptr,   hout[9] ? (float*)c->stage_out[9] : nullptr};
+                      hout[8] ? (float*)c->stage_out[8] : nullptr,   hout[9] ? (float*)c->stage_out[9] : nullptr,
+                      hout[10] ? (float*)c->stage_out[10] : nullptr};
   const ts_status s = ts_step(c, &din, &dout, stream);
   if (s != TS_OK) return s;
-  for (int i = 0; i < 10; ++i)
+  for (int i = 0; i < 11; ++i)
     if (hout[i]) TS_CUDA(c, cudaMemcpyAsync(hout[i], c->stage_out[i], out_bytes[i], cudaMemcpyDeviceToHost, st));
   return TS_OK;
 }

@@ -64,6 +64,15 @@ struct TsChunk {
   int32_t pad0, pad1;
 };
 
+// Uniform grid over one tracked point cloud (object frame), cell size = the sensing radius.
+struct TsPcGrid {
+  float ox, oy, oz, inv_cell;  // cell (i, j, k) covers origin + (i..i+1, j..j+1, k..k+1) * cell
+  int32_t nx, ny, nz;
+  int32_t cell0;               // offset of this cloud's cell_start array in pc_cell
+  int32_t pt0;                 // offset of this cloud's points in pc_pts
+  int32_t pad[3];
+};
+
 // Kernel parameters of one step (passed by value).
 struct TsStepParams {
   int32_t E, L, K, T, P, M, G, Tp;
@@ -71,6 +80,7 @@ struct TsStepParams {
   uint32_t env_id_base;
   // layout
   const float4* tx_pos;   // [T] (x, y, z, R_j); R_j = 0 for every inactive slot
+  const int32_t* tx_patch; // [T] global patch index of each slot (fillers: their filler patch)
   const int32_t* tx_meta; // [T] bits 0-7 group-local patch index, 8-15 patch nu, 16-19 has -u/+u/-v/+v neighbour
   const TsPatch* patches; // [P]
   const TsGroup* groups;  // [G]
@@ -120,6 +130,14 @@ struct TsStepParams {
   float* sm_d;                // [E,M,3] marker drift
   float sn_sigma_white[3], sn_sigma_rw[3], sn_bias[3], sn_quant[3], sn_stuck_min[3], sn_stuck_max[3];
   uint32_t dead_thr;          // floor(p_dead 2^32)
+  // point-cloud ProximityTaxel (A.6)
+  float* proxpc;              // [E,T,6] output
+  const float4* pc_pts;       // clouds sorted by grid cell: (x, y, z, -) in the object frame
+  const int32_t* pc_cell;     // per cloud: cell_start[ncell + 1] (indices into pc_pts), concatenated
+  const struct TsPcGrid* pc_grid;  // [G]
+  const int32_t* pc_id;       // [E,K] cloud of each object, -1 = none
+  int32_t pc_n;               // points per cloud
+  float pc_radius, pc_k, pc_ks, pc_density;
   // state
   uint8_t* st_flags;          // [E,T] bit0 Schmitt, bit1 dead
   float* st_hyst;             // [E,nh/2,Tp] float2 channel pairs, nh = 6 (asym: y) / 12 (maxwell: xi then x_prev)
@@ -161,6 +179,7 @@ int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream);
 int ts_launch_noise(const TsStepParams& p, void* stream);
 int ts_launch_frames(const TsStepParams& p, void* stream);
 int ts_launch_scalar_noise(const TsStepParams& p, void* stream);
+int ts_launch_proxpc(const TsStepParams& p, void* stream);
 int ts_launch_reset_scalar(const TsStepParams& p, const uint8_t* mask, void* stream);
 unsigned long long ts_frame_bytes();
 int ts_launch_retile(const float* src_linear, float4* dst, int n_grids, int N, void* stream);

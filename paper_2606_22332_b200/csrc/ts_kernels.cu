@@ -1422,6 +1422,91 @@ __global__ void ts_reset_scalar_kernel(const __grid_constant__ TsStepParams p, c
   }
 }
 
+// ---------------------------------------------------------------------------------------
+// App. A.6 point-cloud ProximityTaxel (Eq. 12-17).  One thread per (env, taxel).
+// The tracked points are static in their object's frame, so each cloud was sorted once into a uniform grid of cell
+// size R_j (ts_set_pointclouds): the taxel centre is taken into the object frame (double), the 27 cells around it are
+// scanned, and of the points inside the sensing sphere only two sums are kept,
+//     S0 = sum_i P_ij,   S1 = sum_i P_ij (p_i - q_j)          (P_ij = R_j - |p_i - q_j|, Eq. 12)
+// because Eq. 13-17 are linear in p_i:  v_p,i - v_tax = A + w_O x (p_i - q_j),  A = v_O + w_O x (q_j - p_O) - v_tax, so
+//     sum_i P_ij v_t,ij = Pi_a (S0 A + w_O x S1),   f^w = k rho S0 a + k_s rho Pi_a(...),   tau^w = k rho S1 x a.
+// Same result as the per-point sums of the paper up to rounding order.  Distances in fp32 on fp32 differences of
+// nearby points, the sums in double.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) ts_proxpc_kernel(const __grid_constant__ TsStepParams p) {
+  const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gt >= (long long)p.E * p.T) return;
+  const int e = (int)(gt / p.T), j = (int)(gt - (long long)e * p.T);
+  const float4 P4 = __ldg(p.tx_pos + j);
+  float out[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  if (P4.w > 0.f) {
+    const int pidx = __ldg(p.tx_patch + j);
+    const TsPatch& pt = p.patches[pidx];
+    const int link = __ldg(&pt.link);
+    const float4 na = __ldg(&pt.na);
+    const size_t el = (size_t)e * p.L + link;
+    double RL[9];
+    quat_Rd(p.link_quat + el * 4, RL);
+    const D3 pL = ld3d(p.link_pos + el * 3);
+    const D3 q = pL + mulR(RL, D3{(double)P4.x, (double)P4.y, (double)P4.z});       // Eq. 1
+    const D3 a = mulR(RL, D3{(double)na.x, (double)na.y, (double)na.z});
+    const D3 vtax = ld3d(p.link_linvel + el * 3) + cross(ld3d(p.link_angvel + el * 3), q - pL);   // Eq. 13
+    long long n_track = 0;
+    for (int k = 0; k < p.K; ++k) n_track += __ldg(p.pc_id + (size_t)e * p.K + k) >= 0 ? p.pc_n : 0;
+    const double rho = (double)p.pc_density / (double)(n_track > 0 ? n_track : 1);          // Eq. 15 (Q27)
+    const float R = p.pc_radius, R2 = R * R;
+    D3 fw = D3{0.0, 0.0, 0.0}, tw = D3{0.0, 0.0, 0.0};
+    for (int k = 0; k < p.K; ++k) {
+      const int id = __ldg(p.pc_id + (size_t)e * p.K + k);
+      if (id < 0) continue;
+      const size_t ek = (size_t)e * p.K + k;
+      double RO[9];
+      quat_Rd(p.obj_quat + ek * 4, RO);
+      const D3 pO = ld3d(p.obj_pos + ek * 3);
+      const D3 xd = mulRT(RO, q - pO);                                                       // taxel centre, object frame
+      const float xf = (float)xd.x, yf = (float)xd.y, zf = (float)xd.z;
+      const TsPcGrid g = p.pc_grid[id];
+      const int ci = (int)floorf((xf - g.ox) * g.inv_cell), cj = (int)floorf((yf - g.oy) * g.inv_cell), ck = (int)floorf((zf - g.oz) * g.inv_cell);
+      double S0 = 0.0, S1x = 0.0, S1y = 0.0, S1z = 0.0;
+      for (int dk = -1; dk <= 1; ++dk) {
+        const int kk = ck + dk;
+        if (kk < 0 || kk >= g.nz) continue;
+        for (int dj = -1; dj <= 1; ++dj) {
+          const int jj = cj + dj;
+          if (jj < 0 || jj >= g.ny) continue;
+          // the three x-neighbours of a row are consecutive cells: one contiguous run of points
+          const int i0 = max(ci - 1, 0), i1 = min(ci + 1, g.nx - 1);
+          if (i0 > i1) continue;
+          const int row = g.cell0 + (kk * g.ny + jj) * g.nx;
+          const int b = __ldg(p.pc_cell + row + i0), en = __ldg(p.pc_cell + row + i1 + 1);
+          for (int i = b; i < en; ++i) {
+            const float4 pp = __ldg(p.pc_pts + g.pt0 + i);
+            const float dx = pp.x - xf, dy = pp.y - yf, dz = pp.z - zf;
+            const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+            if (d2 < R2) {
+              const float P = R - sqrtf(d2);                                                 // Eq. 12
+              S0 += (double)P;
+              S1x = fma((double)P, (double)dx, S1x); S1y = fma((double)P, (double)dy, S1y); S1z = fma((double)P, (double)dz, S1z);
+            }
+          }
+        }
+      }
+      if (S0 > 0.0) {
+        const D3 S1w = mulR(RO, D3{S1x, S1y, S1z});                                          // sum P (p_i - q_j), world axes
+        const D3 wO = ld3d(p.obj_angvel + ek * 3);
+        const D3 A = ld3d(p.obj_linvel + ek * 3) + cross(wO, q - pO) - vtax;                 // Eq. 13 at p_i = q_j
+        const D3 sv = S0 * A + cross(wO, S1w);                                               // sum P (v_p - v_tax)
+        const D3 st = sv - dot(sv, a) * a;                                                   // Eq. 14 (linear)
+        fw = fw + ((double)p.pc_k * rho * S0) * a + ((double)p.pc_ks * rho) * st;            // Eq. 16
+        tw = tw + ((double)p.pc_k * rho) * cross(S1w, a);                                    // Eq. 17
+      }
+    }
+    const D3 fl = mulRT(RL, fw), tl = mulRT(RL, tw);                                         // reported in the link frame
+    out[0] = (float)fl.x; out[1] = (float)fl.y; out[2] = (float)fl.z; out[3] = (float)tl.x; out[4] = (float)tl.y; out[5] = (float)tl.z;
+  }
+  store6(p.proxpc + gt * 6, out);
+}
+
 }  // namespace
 
 unsigned long long ts_bank_elems_per_grid(int N) { return (unsigned long long)(N - 1) * (N - 1) * N; }
@@ -1504,6 +1589,12 @@ unsigned long long ts_frame_bytes() { return sizeof(FrameS); }
 int ts_launch_frames(const TsStepParams& p, void* stream) {
   const long long n = (long long)p.E * p.P * p.K;
   ts_frames_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(p);
+  return (int)cudaGetLastError();
+}
+
+int ts_launch_proxpc(const TsStepParams& p, void* stream) {
+  const long long n = (long long)p.E * p.T;
+  ts_proxpc_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(p);
   return (int)cudaGetLastError();
 }
 

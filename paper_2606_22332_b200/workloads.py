@@ -298,5 +298,22 @@ class Workload:
         return {k: a[ids] for k, a in inp.items()}
 
 
+def star_point_cloud(n_points, scale=1.0, rot=None, seed=0):
+    """n_points surface samples of the star r(u) = 40 mm (1 + 0.2 Y_3^2(u)) (scaled / rotated like star_grid), object
+    frame, fp32: uniform random directions times the closed-form radius (the paper samples tracked links into surface
+    point clouds at reset; N_pc = 5,000 P:267)."""
+    rng = np.random.default_rng([seed, 4242, n_points])
+    u = _rand_dir(rng, (n_points,))
+    return (star_radius(u, scale, rot)[:, None] * u).astype(np.float32)
+
+
+def point_cloud_bank(w, n_points=5000):
+    """Tracked point clouds for a grid-object workload (configs 3-5): cloud k samples star k of the SDF bank; envs whose
+    object is a primitive get cloud_id -1 (not tracked).  Returns (points [G, N, 3], cloud_id [E, 1])."""
+    pts = np.stack([star_point_cloud(n_points, s["scale"], s["rot"], seed=k) for k, s in enumerate(w.stars)])
+    cid = np.where(w.types[:, 0] == GEOM_GRID, w.params[:, 0, 0].astype(np.int32), -1).astype(np.int32)
+    return pts, cid.reshape(-1, 1)
+
+
 def config(cid, n_envs=None, seed=0):
     return Workload(cid, n_envs=n_envs, seed=seed)

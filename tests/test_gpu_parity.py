@@ -436,3 +436,34 @@ def test_noisy_scalar_readouts():
         for k in ("depth_noisy", "prox_noisy", "marker_noisy"):
             assert rep["max_ratio"][k] <= 1.0
         sim.close()
+
+
+def test_point_cloud_proximity_taxel():
+    """the paper's ProximityTaxel (App. A.6, Eq. 12-17) on tracked surface point clouds (N_pc = 5,000 per
+    object, R_j = 10 mm, k = 300, k_s = 10, density 100): uniform-grid neighbour query on the GPU against the
+    oracle's brute-force sum over every point.  Config-5 scene: star objects are tracked, primitives are not (zeros)."""
+    import torch
+    from oracle import oracle as O
+    from paper_2606_22332_b200.binding import TactileSim
+    from parity import ATOL, RTOL
+    w = W.config(5, n_envs=32)
+    pts, cid = W.point_cloud_bank(w, 5000)
+    outs = ("depth", "proxpc")
+    sim = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=w.physics, outputs=outs)
+    sim.set_geometry(w.types, w.params, w.bank, w.voxel)
+    sim.set_pointclouds(pts, cid)
+    orc = O.Oracle(w.patches, w.T, w.L, w.K, np.arange(w.E), physics=w.physics, threads=os.cpu_count() or 1)
+    orc.set_geometry(w.types, w.params, w.bank, w.voxel)
+    orc.set_pointclouds(pts, cid)
+    worst, nz = 0.0, 0
+    for s in (0, 7, 19):
+        inp = w.inputs(s)
+        g = sim.step(sim.upload(inp))["proxpc"].cpu().numpy().astype(np.float64)
+        r = orc.step(inp, want=outs, aux=False)["proxpc"]
+        ratio = np.abs(g - r) / (ATOL + RTOL * np.abs(r))
+        worst = max(worst, float(ratio.max()))
+        nz += int((np.abs(r[..., 2]) > 1e-3).sum())
+        assert not g[cid[:, 0] < 0].any()                                    # untracked objects: exactly zero
+    print(json.dumps({"proxpc_max_ratio": worst, "taxels_with_force": nz}))
+    assert worst <= 1.0 and nz > 20000
+    sim.close()
