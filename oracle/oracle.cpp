@@ -32,6 +32,7 @@
 //
 // Build: g++ -O2 -std=c++17 -fPIC -shared -fopenmp oracle.cpp -o liboracle.so
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -271,6 +272,10 @@ typedef struct orc_params {
   // Point-cloud ProximityTaxel (App. A.6, Eq. 12-17): sensing radius R_j, k, k_s, density scalar
   // (0.01 m, 300, 10, 100)
   float pc_radius, pc_k, pc_ks, pc_density;
+  // Elastomer shear history (App. A.7, Eq. 22-23; constants P:304: s_s = 100, lambda_s = 2000,
+  // eta_enter = 1e-5 m, eta_exit = 1e-4 m); shear_enable adds sum_p u^s_pj to the marker output (reading R11)
+  int32_t shear_enable;
+  float s_s, lambda_s, eta_enter, eta_exit;
 } orc_params;
 }
 
@@ -306,6 +311,11 @@ struct Oracle {
   int pc_G = 0, pc_N = 0;
   std::vector<int32_t> pc_id;                 // [E,K], -1 = the object is not tracked
   double* proxpc = nullptr;                   // [E,T,6] output handed in by orc_set_proxpc
+  // elastomer shear history (Eq. 22): anchor per (env, patch, object, tracked point), link frame
+  std::vector<uint8_t> sh_on;                 // [E,P,K,N] anchored?
+  std::vector<V3> sh_e;                       // [E,P,K,N] anchor e_p
+  std::vector<V3> p_center, p_ua, p_va;       // [P] pad centre and unit axes (fp32 values), link frame
+  std::vector<double> p_su, p_sv;             // [P] pad extents
   std::vector<std::deque<std::vector<double>>> hist;  // [E] the last Delta + J post-crosstalk fields [T,6] of the episode
   std::vector<uint32_t> n_step, episode;      // [E]
 };
@@ -319,6 +329,7 @@ void build_layout(Oracle& o, const orc_patch* patches, int P, int T, const uint8
   o.link.assign(T, 0); o.patch.assign(T, -1); o.iu.assign(T, 0); o.iv.assign(T, 0);
   o.nbr.assign((size_t)T * 4, -1);
   o.mpos.clear(); o.mnrm.clear(); o.mpatch.clear();
+  o.p_center.clear(); o.p_ua.clear(); o.p_va.clear(); o.p_su.clear(); o.p_sv.clear();
   o.p_start.clear(); o.p_nu.clear(); o.p_nv.clear(); o.p_link.clear(); o.p_mstart.clear(); o.p_mcount.clear(); o.p_eps.clear();
   int t = 0;
   for (int p = 0; p < P; ++p) {
@@ -328,6 +339,8 @@ void build_layout(Oracle& o, const orc_patch* patches, int P, int T, const uint8
     bool keep = (link_mask == nullptr) || link_mask[d.link];
     o.p_start.push_back(t); o.p_nu.push_back(d.nu); o.p_nv.push_back(d.nv); o.p_link.push_back(d.link);
     o.p_eps.push_back(f32((double)d.size_u / d.nu));
+    o.p_center.push_back(org); o.p_ua.push_back(ua); o.p_va.push_back(va);
+    o.p_su.push_back((double)d.size_u); o.p_sv.push_back((double)d.size_v);
     for (int v = 0; v < d.nv; ++v)
       for (int u = 0; u < d.nu; ++u, ++t) {
         double su = ((u + 0.5) / d.nu - 0.5) * (double)d.size_u;
@@ -499,6 +512,10 @@ void orc_reset(void* h, const uint8_t* env_mask) {
     o.n_step[e] = 0;
     o.episode[e] += 1;
     o.hist[e].clear();
+    if (!o.sh_on.empty()) {
+      size_t per = (size_t)o.P * o.K * o.pc_N;
+      std::fill(o.sh_on.begin() + (size_t)e * per, o.sh_on.begin() + (size_t)(e + 1) * per, (uint8_t)0);
+    }
     for (size_t i = (size_t)e * o.T * 2; i < (size_t)(e + 1) * o.T * 2; ++i) { o.sn_ha[i] = 0; o.sn_hb[i] = 0; o.sn_dr[i] = 0; }
     for (size_t i = (size_t)e * o.M * 3; i < (size_t)(e + 1) * o.M * 3; ++i) { o.sm_ha[i] = 0; o.sm_hb[i] = 0; o.sm_dr[i] = 0; }
   }
@@ -731,6 +748,51 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
         size_t o3 = ((size_t)e * M + jm) * 3;
         marker[o3] = u.x; marker[o3 + 1] = u.y; marker[o3 + 2] = u.z;
         marker_c[(size_t)jm * 3] = u.x; marker_c[(size_t)jm * 3 + 1] = u.y; marker_c[(size_t)jm * 3 + 2] = u.z;
+      }
+      // Eq. 22-23 (R11): anchored shear history of the tracked surface points.  For every patch (elastomer pad) and
+      // tracked point p: z_p = R_L^T (p_O + R_O p^o - p_L) (sensor-link frame); elastomer SDF of a flat pad
+      // phi_el = n . (z_p - x_c) over the pad (|u| <= size_u / 2, |v| <= size_v / 2), +inf beside it; the anchor
+      // e_p = z_p is set when phi_el < -eta_enter and cleared when phi_el > +eta_exit; h_p = max(0, -phi_el);
+      // u^s_pj = s_s Pi_n(z_p - e_p) h_p exp(-lambda_s |Pi_n(x_j - z_p)|^2) is added to every marker j of the patch.
+      if (pr.shear_enable && o.pc_N > 0) {
+        const int P = o.P, N = o.pc_N;
+        for (int pi = 0; pi < P; ++pi) {
+          if (o.p_mcount[pi] == 0 || !(o.radius[o.p_start[pi]] > 0.0)) continue;     // no markers / filtered-out link
+          const int l = o.p_link[pi];
+          M3 RL = quat_to_R(link_quat + ((size_t)e * L + l) * 4);
+          V3 pL = ld3(link_pos + ((size_t)e * L + l) * 3);
+          V3 n = o.mnrm[o.p_mstart[pi]];
+          for (int k = 0; k < K; ++k) {
+            const int id = o.pc_id[(size_t)e * K + k];
+            if (id < 0) continue;
+            V3 pO = ld3(obj_pos + ((size_t)e * K + k) * 3);
+            M3 RO = quat_to_R(obj_quat + ((size_t)e * K + k) * 4);
+            const float* pts = o.pc_pts.data() + (size_t)id * N * 3;
+            for (int i = 0; i < N; ++i) {
+              size_t si = (((size_t)e * P + pi) * K + k) * N + i;
+              V3 z = mulT(RL, pO + mul(RO, ld3(pts + 3 * i)) - pL);
+              V3 rel = z - o.p_center[pi];
+              double phi_el = INFINITY;
+              if (std::fabs(dot(rel, o.p_ua[pi])) <= 0.5 * o.p_su[pi] && std::fabs(dot(rel, o.p_va[pi])) <= 0.5 * o.p_sv[pi])
+                phi_el = dot(rel, n);
+              if (!o.sh_on[si] && phi_el < -(double)pr.eta_enter) { o.sh_on[si] = 1; o.sh_e[si] = z; }
+              else if (o.sh_on[si] && phi_el > (double)pr.eta_exit) o.sh_on[si] = 0;
+              if (!o.sh_on[si]) continue;
+              double hp = std::fmax(0.0, -phi_el);
+              if (!(hp > 0.0)) continue;
+              V3 dz = z - o.sh_e[si];
+              V3 dzt = dz - dot(dz, n) * n;                                           // Pi_n(z_p - e_p)
+              for (int jm = o.p_mstart[pi]; jm < o.p_mstart[pi] + o.p_mcount[pi]; ++jm) {
+                V3 r = o.mpos[jm] - z;
+                V3 rt = r - dot(r, n) * n;                                            // Pi_n(x_j - z_p)
+                double wgt = (double)pr.s_s * hp * std::exp(-(double)pr.lambda_s * dot(rt, rt));   // Eq. 22
+                size_t o3 = ((size_t)e * M + jm) * 3;
+                marker[o3] += wgt * dzt.x; marker[o3 + 1] += wgt * dzt.y; marker[o3 + 2] += wgt * dzt.z;   // Eq. 23
+                marker_c[(size_t)jm * 3] += wgt * dzt.x; marker_c[(size_t)jm * 3 + 1] += wgt * dzt.y; marker_c[(size_t)jm * 3 + 2] += wgt * dzt.z;
+              }
+            }
+          }
+        }
       }
     }
     // O8: hysteresis -> crosstalk -> drift -> dead
@@ -987,6 +1049,8 @@ int orc_set_pointclouds(void* h, int n_clouds, int n_points, const float* pts, c
   o.pc_pts.assign(pts, pts + (size_t)n_clouds * n_points * 3);
   o.pc_id.assign(cloud_id, cloud_id + (size_t)o.E * o.K);
   for (int32_t id : o.pc_id) if (id >= n_clouds) return 1;
+  size_t ns = (size_t)o.E * o.P * o.K * n_points;
+  o.sh_on.assign(ns, 0); o.sh_e.assign(ns, V3{0, 0, 0});
   return 0;
 }
 void orc_set_proxpc(void* h, double* proxpc) { ((Oracle*)h)->proxpc = proxpc; }

@@ -49,7 +49,9 @@ class OrcParams(C.Structure):
                 ("radius_noise", C.c_float), ("read_delay", C.c_int32), ("read_jitter", C.c_int32),
                 ("sn_sigma_white", C.c_float * 3), ("sn_sigma_rw", C.c_float * 3), ("sn_bias", C.c_float * 3),
                 ("sn_quant", C.c_float * 3), ("sn_stuck_min", C.c_float * 3), ("sn_stuck_max", C.c_float * 3),
-                ("pc_radius", C.c_float), ("pc_k", C.c_float), ("pc_ks", C.c_float), ("pc_density", C.c_float)]
+                ("pc_radius", C.c_float), ("pc_k", C.c_float), ("pc_ks", C.c_float), ("pc_density", C.c_float),
+                ("shear_enable", C.c_int32), ("s_s", C.c_float), ("lambda_s", C.c_float), ("eta_enter", C.c_float),
+                ("eta_exit", C.c_float)]
 
 SN_CLASS = {"depth": 0, "prox": 1, "marker": 2}          # noisy scalar readouts (R10)
 SN_KNOBS = ("sigma_white", "sigma_rw", "bias", "quant", "stuck_min", "stuck_max")
@@ -116,7 +118,8 @@ def make_params(physics=None, noise=None):
              sigma_white_force=0.0, sigma_white_torque=0.0, bias_force=0.0, bias_torque=0.0, quant_force=0.0,
              quant_torque=0.0, gain_min=1.0, gain_max=1.0, stuck_min_force=0.0, stuck_max_force=0.0,
              stuck_min_torque=0.0, stuck_max_torque=0.0, xtalk_sigma=0.0, radius_noise=0.0, read_delay=0, read_jitter=0,
-             pc_radius=0.01, pc_k=300.0, pc_ks=10.0, pc_density=100.0)          # A.6 constants
+             pc_radius=0.01, pc_k=300.0, pc_ks=10.0, pc_density=100.0,          # A.6 constants
+             shear_enable=0, s_s=100.0, lambda_s=2000.0, eta_enter=1e-5, eta_exit=1e-4)   # A.7 shear constants
     sn = {}
     for src in (physics, noise):
         if src:
