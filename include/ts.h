@@ -192,6 +192,13 @@ typedef struct ts_config {
   /* Point-cloud ProximityTaxel (App. A.6): sensing radius R_j [m], k, k_s, density scalar (0.01, 300,
    * 10, 100; ts_config_default sets these).  rho_b = density / max(N_b, 1), N_b = tracked points of env b (Q27). */
   float pc_radius, pc_k, pc_ks, pc_density;
+  /* Elastomer shear history (App. A.7, Eq. 22-23; R11): with shear_enable the marker output is
+   * sum_i u^d_ij + sum_p u^s_pj; the tracked points p are those of ts_set_pointclouds.  A point anchors (e_p = its
+   * link-frame position) when the pad's SDF at it drops below -eta_enter and un-anchors above +eta_exit;
+   * u^s_pj = s_s Pi_n(z_p - e_p) h_p exp(-lambda_s |Pi_n(x_j - z_p)|^2).  P:304: s_s = 100, lambda_s = 2000,
+   * eta_enter = 1e-5 m, eta_exit = 1e-4 m (ts_config_default sets these; shear_enable = 0). */
+  int32_t shear_enable;
+  float s_s, lambda_s, eta_enter, eta_exit;
 } ts_config;
 
 /* Fills *cfg with the paper's constants and everything else zero / off. */

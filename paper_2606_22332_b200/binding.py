@@ -72,7 +72,9 @@ class Config(C.Structure):
                 ("kernel_form", C.c_int32),
                 ("sn_sigma_white", C.c_float * 3), ("sn_sigma_rw", C.c_float * 3), ("sn_bias", C.c_float * 3),
                 ("sn_quant", C.c_float * 3), ("sn_stuck_min", C.c_float * 3), ("sn_stuck_max", C.c_float * 3),
-                ("pc_radius", C.c_float), ("pc_k", C.c_float), ("pc_ks", C.c_float), ("pc_density", C.c_float)]
+                ("pc_radius", C.c_float), ("pc_k", C.c_float), ("pc_ks", C.c_float), ("pc_density", C.c_float),
+                ("shear_enable", C.c_int32), ("s_s", C.c_float), ("lambda_s", C.c_float), ("eta_enter", C.c_float),
+                ("eta_exit", C.c_float)]
 
 
 class PointClouds(C.Structure):

@@ -57,6 +57,7 @@ struct ts_ctx {
   float4* pc_pts = nullptr; int32_t* pc_cell = nullptr; TsPcGrid* pc_grid = nullptr; int32_t* pc_id = nullptr;
   int32_t* tx_patch = nullptr;
   int pc_n = 0; bool have_pc = false;
+  uint8_t* sh_on = nullptr; float4* sh_e = nullptr; float4* pc_raw = nullptr;   // elastomer shear history (Eq. 22)
   // noisy scalar readouts (R10): state, the perturbed depth (Eq. 26), scratch copies of clean inputs the caller did not ask for
   float4* sn_h = nullptr; float2* sn_d = nullptr; float *sm_h = nullptr, *sm_d = nullptr;
   float *depth_pert = nullptr, *sc_depth = nullptr, *sc_prox = nullptr, *sc_marker = nullptr;
@@ -102,6 +103,7 @@ void free_all(ts_ctx* c) {
   cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->mk_tab8); cudaFree(c->grp_link);
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->env_perm); cudaFree(c->frames_g); cudaFree(c->patch_link); cudaFree(c->bank); cudaFree(c->bank_stage); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch); cudaFree(c->ft_scratch_r); cudaFree(c->st_ring);
+  cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw);
   cudaFree(c->pc_pts); cudaFree(c->pc_cell); cudaFree(c->pc_grid); cudaFree(c->pc_id); cudaFree(c->tx_patch);
   cudaFree(c->sn_h); cudaFree(c->sn_d); cudaFree(c->sm_h); cudaFree(c->sm_d); cudaFree(c->depth_pert); cudaFree(c->sc_depth);
   cudaFree(c->sc_prox); cudaFree(c->sc_marker);
@@ -180,6 +182,8 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.dead_thr = c->dead_thr;
   p.pc_pts = c->pc_pts; p.pc_cell = c->pc_cell; p.pc_grid = c->pc_grid; p.pc_id = c->pc_id; p.pc_n = c->pc_n; p.tx_patch = c->tx_patch;
   p.pc_radius = g.pc_radius; p.pc_k = g.pc_k; p.pc_ks = g.pc_ks; p.pc_density = g.pc_density;
+  p.sh_on = c->sh_on; p.sh_e = c->sh_e; p.pc_raw = c->pc_raw;
+  p.shear_enable = (g.shear_enable && c->sh_on) ? 1 : 0; p.s_s = g.s_s; p.lambda_s = g.lambda_s; p.eta_enter = g.eta_enter; p.eta_exit = g.eta_exit;
 }
 }  // namespace
 
@@ -201,6 +205,7 @@ void ts_config_default(ts_config* c) {
   c->tau = 0.05f; c->beta = 0.5f; c->alpha_load = 1.f; c->alpha_unload = 1.f;
   c->gain_min = 1.f; c->gain_max = 1.f;                                             // Eq. 27 off
   c->pc_radius = 0.01f; c->pc_k = 300.f; c->pc_ks = 10.f; c->pc_density = 100.f;    // A.6 P:267
+  c->s_s = 100.f; c->lambda_s = 2000.f; c->eta_enter = 1e-5f; c->eta_exit = 1e-4f;  // A.7 P:304
   c->output_mask = TS_OUT_CONTACT | TS_OUT_DEPTH | TS_OUT_FT | TS_OUT_MARKER | TS_OUT_PROX;
 }
 
@@ -211,7 +216,8 @@ int32_t ts_launches_per_step(const ts_ctx* ctx) {
   if (!ctx) return 0;
   return ((ctx->cfg.noise_enable && !ctx->fused) ? 3 : 2) +
          ((ctx->cfg.output_mask & (TS_OUT_DEPTH_NOISY | TS_OUT_PROX_NOISY | TS_OUT_MARKER_NOISY)) ? 1 : 0) +
-         ((ctx->cfg.output_mask & TS_OUT_PROXPC) ? 1 : 0);
+         ((ctx->cfg.output_mask & TS_OUT_PROXPC) ? 1 : 0) +
+         ((ctx->cfg.shear_enable && (ctx->cfg.output_mask & (TS_OUT_MARKER | TS_OUT_MARKER_NOISY))) ? 1 : 0);
 }
 
 ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
@@ -291,8 +297,9 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     q.link = d.link; q.mstart = lay->marker_start[pi]; q.mnu = d.marker_nu; q.mnv = d.marker_nv;
     q.eps = lay->patch_eps[pi];
     const double u[3] = {d.u_axis[0], d.u_axis[1], d.u_axis[2]}, v[3] = {d.v_axis[0], d.v_axis[1], d.v_axis[2]};
-    q.ua = make_float4(d.u_axis[0], d.u_axis[1], d.u_axis[2], 0.f);
-    q.va = make_float4(d.v_axis[0], d.v_axis[1], d.v_axis[2], 0.f);
+    q.ua = make_float4(d.u_axis[0], d.u_axis[1], d.u_axis[2], d.size_u);
+    q.va = make_float4(d.v_axis[0], d.v_axis[1], d.v_axis[2], d.size_v);
+    q.ctr = make_float4(d.origin[0], d.origin[1], d.origin[2], 0.f);
     q.na = make_float4(lay->nrm[3 * q.start], lay->nrm[3 * q.start + 1], lay->nrm[3 * q.start + 2], 0.f);  // = marker normal
     q.direct = (cfg->c_e != 1.0f || q.mnu * q.nv > TS_CHUNK) ? 1 : 0;
     q.tab = (int32_t)tab.size();
@@ -345,7 +352,7 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     TsPatch q{};
     q.start = t; q.n = (T - t < TS_BLOCK) ? T - t : TS_BLOCK; q.nu = q.n; q.nv = 1; q.link = -1; q.mstart = M;
     q.tab = (int32_t)tab.size(); q.i1off = (int32_t)item1.size();
-    q.ua = q.va = q.na = make_float4(0.f, 0.f, 0.f, 0.f);
+    q.ua = q.va = q.na = q.ctr = make_float4(0.f, 0.f, 0.f, 0.f);
     pts.push_back(q);
   }
   // ---- pack whole patches into groups of <= TS_BLOCK slots; markers of a group into chunks ----
@@ -628,6 +635,7 @@ ts_status ts_set_pointclouds(ts_ctx* c, const ts_pointclouds* pc, void* stream) 
   cudaStream_t st = (cudaStream_t)stream;
   c->have_pc = false;
   TS_CUDA(c, cudaStreamSynchronize(st));   // steps in flight may still read the old index
+  cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw);
   cudaFree(c->pc_pts); cudaFree(c->pc_cell); cudaFree(c->pc_grid); cudaFree(c->pc_id);
   c->pc_pts = nullptr; c->pc_cell = nullptr; c->pc_grid = nullptr; c->pc_id = nullptr;
   TS_CUDA(c, cudaMalloc((void**)&c->pc_pts, sizeof(float4) * sorted.size()));
@@ -638,6 +646,18 @@ ts_status ts_set_pointclouds(ts_ctx* c, const ts_pointclouds* pc, void* stream) 
   TS_CUDA(c, cudaMemcpyAsync(c->pc_cell, cells.data(), sizeof(int32_t) * cells.size(), cudaMemcpyHostToDevice, st));
   TS_CUDA(c, cudaMemcpyAsync(c->pc_grid, grids.data(), sizeof(TsPcGrid) * G, cudaMemcpyHostToDevice, st));
   TS_CUDA(c, cudaMemcpyAsync(c->pc_id, pc->cloud_id, sizeof(int32_t) * EK, cudaMemcpyHostToDevice, st));
+  if (c->cfg.shear_enable && c->M > 0) {   // Eq. 22 anchors: one per (env, patch, object, tracked point)
+    cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw);
+    c->sh_on = nullptr; c->sh_e = nullptr; c->pc_raw = nullptr;
+    const size_t ns = (size_t)c->cfg.n_envs * c->P * c->cfg.objs_per_env * N;
+    std::vector<float4> raw((size_t)G * N);
+    for (size_t i = 0; i < raw.size(); ++i) raw[i] = make_float4(pc->points[3 * i], pc->points[3 * i + 1], pc->points[3 * i + 2], 0.f);
+    TS_CUDA(c, cudaMalloc((void**)&c->sh_on, ns));
+    TS_CUDA(c, cudaMalloc((void**)&c->sh_e, sizeof(float4) * ns));
+    TS_CUDA(c, cudaMalloc((void**)&c->pc_raw, sizeof(float4) * raw.size()));
+    TS_CUDA(c, cudaMemsetAsync(c->sh_on, 0, ns, st));
+    TS_CUDA(c, cudaMemcpyAsync(c->pc_raw, raw.data(), sizeof(float4) * raw.size(), cudaMemcpyHostToDevice, st));
+  }
   TS_CUDA(c, cudaStreamSynchronize(st));
   c->pc_n = N;
   c->have_pc = true;
@@ -700,6 +720,11 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
     e = (cudaError_t)ts_launch_noise(p, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: noise launch");
   }
+  if (c->cfg.shear_enable && p.marker) {
+    if (!c->sh_on) return fail(c, TS_ERR_STATE, "ts_step: shear_enable needs ts_set_pointclouds before the first step");
+    e = (cudaError_t)ts_launch_shear(p, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: shear launch");
+  }
   if (p.proxpc) {
     e = (cudaError_t)ts_launch_proxpc(p, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: proxpc launch");
@@ -756,6 +781,7 @@ ts_status ts_reset(ts_ctx* c, const uint8_t* env_mask_dev, void* stream) {
   cudaError_t e = (cudaError_t)ts_launch_reset_counters(c->reset_step, c->episode, env_mask_dev, c->cfg.n_envs, c->gstep, stream);
   if (e == cudaSuccess) e = (cudaError_t)ts_launch_reset_state(p, env_mask_dev, c->dead_thr, c->nh, stream);
   if (e == cudaSuccess && (c->sn_d || c->sm_d)) e = (cudaError_t)ts_launch_reset_scalar(p, env_mask_dev, stream);
+  if (e == cudaSuccess && c->sh_on) e = (cudaError_t)ts_launch_reset_shear(p, env_mask_dev, stream);
   if (e != cudaSuccess) return cuda_fail(c, e, "ts_reset: launch");
   return TS_OK;
 }

@@ -33,7 +33,7 @@ struct ts_layout {
   std::vector<int32_t> marker_patch;
 };
 
-// Device-side patch record (96 bytes).
+// Device-side patch record (112 bytes).
 struct TsPatch {
   int32_t start;   // first taxel slot
   int32_t n;       // taxel slots in the patch
@@ -45,7 +45,8 @@ struct TsPatch {
   int32_t tab;     // offset (doubles) of this patch's separable tables in mk_tab
   int32_t i1off;   // first pass-1 item of this patch (index into mk_item1)
   int32_t direct;  // 1 = direct (non-separable) marker sum
-  float4 ua, va, na;  // u axis, v axis, normal (link frame)
+  float4 ua, va, na;  // u axis (w = pad extent size_u), v axis (w = size_v), normal (link frame)
+  float4 ctr;         // pad centre (link frame); the pad is the elastomer surface of Eq. 22's SDF
 };
 
 // A group = consecutive patches whose taxel slots fit one block.
@@ -138,6 +139,12 @@ struct TsStepParams {
   const int32_t* pc_id;       // [E,K] cloud of each object, -1 = none
   int32_t pc_n;               // points per cloud
   float pc_radius, pc_k, pc_ks, pc_density;
+  // elastomer shear history (Eq. 22): anchors per (env, patch, object, tracked point)
+  uint8_t* sh_on;             // [E,P,K,N] anchored?
+  float4* sh_e;               // [E,P,K,N] anchor relative to the pad centre (link frame); only read where sh_on is set
+  const float4* pc_raw;       // [G,N] tracked points in their original order (the grid-sorted copy serves the proximity query)
+  int32_t shear_enable;
+  float s_s, lambda_s, eta_enter, eta_exit;
   // state
   uint8_t* st_flags;          // [E,T] bit0 Schmitt, bit1 dead
   float* st_hyst;             // [E,nh/2,Tp] float2 channel pairs, nh = 6 (asym: y) / 12 (maxwell: xi then x_prev)
@@ -180,6 +187,8 @@ int ts_launch_noise(const TsStepParams& p, void* stream);
 int ts_launch_frames(const TsStepParams& p, void* stream);
 int ts_launch_scalar_noise(const TsStepParams& p, void* stream);
 int ts_launch_proxpc(const TsStepParams& p, void* stream);
+int ts_launch_shear(const TsStepParams& p, void* stream);
+int ts_launch_reset_shear(const TsStepParams& p, const uint8_t* mask, void* stream);
 int ts_launch_reset_scalar(const TsStepParams& p, const uint8_t* mask, void* stream);
 unsigned long long ts_frame_bytes();
 int ts_launch_retile(const float* src_linear, float4* dst, int n_grids, int N, void* stream);

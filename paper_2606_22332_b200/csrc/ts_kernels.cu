@@ -1507,6 +1507,106 @@ __global__ void __launch_bounds__(128) ts_proxpc_kernel(const __grid_constant__ 
   store6(p.proxpc + gt * 6, out);
 }
 
+// ---------------------------------------------------------------------------------------
+// App. A.7 elastomer shear history (Eq. 22-23; reading R11).  One block per (env, patch with markers).
+// Phase A: the relative pose link <- object in double (z_p = t + Rm p^o, sensor-link frame).
+// Phase B: every thread walks tracked points: pad SDF phi_el = n . (z_p - x_c) over the pad, anchor update
+//          (set below -eta_enter, cleared above +eta_exit; decisions in double like the oracle), and the anchored,
+//          penetrating points (a few tens per touching pad) are queued in shared memory.
+// Phase C: one thread per marker sums s_s Pi_n(z_p - e_p) h_p exp(-lambda_s |Pi_n(x_j - z_p)|^2) over the queue and adds
+//          it to the dilation value the step kernel wrote (Eq. 23).
+// ---------------------------------------------------------------------------------------
+#define TS_SHEAR_Q 512
+__global__ void __launch_bounds__(256) ts_shear_kernel(const __grid_constant__ TsStepParams p) {
+  __shared__ double Rm[9], tv[3];
+  __shared__ float4 qd[TS_SHEAR_Q];   // (tangential slide x, y, z, h_p)
+  __shared__ float4 qz[TS_SHEAR_Q];   // z_p relative to the pad centre
+  __shared__ int qn;
+  const int e = blockIdx.x / p.P, pi = blockIdx.x - e * p.P, tid = threadIdx.x;
+  const TsPatch& pt = p.patches[pi];
+  const int mcount = __ldg(&pt.mnu) * __ldg(&pt.mnv), link = __ldg(&pt.link);
+  if (mcount == 0 || link < 0) return;
+  if (!(__ldg(&p.tx_pos[__ldg(&pt.start)].w) > 0.f)) return;       // link filtered out: fillers
+  const float4 na = __ldg(&pt.na), ua = __ldg(&pt.ua), va = __ldg(&pt.va), ctr = __ldg(&pt.ctr);
+  const D3 n = D3{(double)na.x, (double)na.y, (double)na.z}, uu = D3{(double)ua.x, (double)ua.y, (double)ua.z}, vv = D3{(double)va.x, (double)va.y, (double)va.z};
+  const D3 xc = D3{(double)ctr.x, (double)ctr.y, (double)ctr.z};
+  const double hu = 0.5 * (double)ua.w, hv = 0.5 * (double)va.w;
+  const int N = p.pc_n;
+  float ax = 0.f, ay = 0.f, az = 0.f;   // this thread's marker (tid < mcount): shear sum
+  for (int k = 0; k < p.K; ++k) {
+    const int id = __ldg(p.pc_id + (size_t)e * p.K + k);   // block-uniform
+    if (id < 0) continue;
+    __syncthreads();
+    if (tid == 0) {
+      qn = 0;
+      const size_t el = (size_t)e * p.L + link, ek = (size_t)e * p.K + k;
+      double RL[9], RO[9];
+      quat_Rd(p.link_quat + el * 4, RL);
+      quat_Rd(p.obj_quat + ek * 4, RO);
+      const D3 d = ld3d(p.obj_pos + ek * 3) - ld3d(p.link_pos + el * 3);
+      const D3 t = mulRT(RL, d);
+      tv[0] = t.x; tv[1] = t.y; tv[2] = t.z;
+      for (int r = 0; r < 3; ++r)
+        for (int c2 = 0; c2 < 3; ++c2) Rm[r * 3 + c2] = fma(RL[r], RO[c2], fma(RL[3 + r], RO[3 + c2], RL[6 + r] * RO[6 + c2]));   // R_L^T R_O
+    }
+    __syncthreads();
+    const size_t sbase = (((size_t)e * p.P + pi) * p.K + k) * N;
+    for (int i = tid; i < N; i += 256) {
+      const float4 po = __ldg(p.pc_raw + (size_t)id * N + i);
+      const D3 z = D3{tv[0], tv[1], tv[2]} + mulR(Rm, D3{(double)po.x, (double)po.y, (double)po.z});
+      const D3 rel = z - xc;
+      double phi_el = __longlong_as_double(0x7ff0000000000000LL);
+      if (fabs(dot(rel, uu)) <= hu && fabs(dot(rel, vv)) <= hv) phi_el = dot(rel, n);
+      uint8_t on = p.sh_on[sbase + i];
+      float4 anc;
+      if (!on && phi_el < -(double)p.eta_enter) {
+        on = 1; anc = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
+        p.sh_on[sbase + i] = 1; p.sh_e[sbase + i] = anc;
+      } else if (on && phi_el > (double)p.eta_exit) {
+        on = 0; p.sh_on[sbase + i] = 0;
+      } else if (on) {
+        anc = p.sh_e[sbase + i];
+      }
+      if (on && phi_el < 0.0) {
+        const D3 dz = D3{rel.x - (double)anc.x, rel.y - (double)anc.y, rel.z - (double)anc.z};
+        const D3 dzt = dz - dot(dz, n) * n;                          // Pi_n(z_p - e_p)
+        const int slot = atomicAdd(&qn, 1);
+        if (slot < TS_SHEAR_Q) {
+          qd[slot] = make_float4((float)dzt.x, (float)dzt.y, (float)dzt.z, (float)(-phi_el));
+          qz[slot] = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
+        }
+      }
+    }
+    __syncthreads();
+    const int nq = min(qn, TS_SHEAR_Q);
+    if (tid < mcount && nq > 0) {
+      const float4 mp = __ldg(p.mk_pos + __ldg(&pt.mstart) + tid);
+      const float mx = mp.x - ctr.x, my = mp.y - ctr.y, mz = mp.z - ctr.z;
+      for (int s2 = 0; s2 < nq; ++s2) {
+        const float4 d4 = qd[s2], z4 = qz[s2];
+        const float rx = mx - z4.x, ry = my - z4.y, rz = mz - z4.z;
+        const float rn = fmaf(rx, na.x, fmaf(ry, na.y, rz * na.z));
+        const float tx = fmaf(-rn, na.x, rx), ty = fmaf(-rn, na.y, ry), tz = fmaf(-rn, na.z, rz);   // Pi_n(x_j - z_p)
+        const float wgt = p.s_s * d4.w * expf(-p.lambda_s * fmaf(tx, tx, fmaf(ty, ty, tz * tz)));   // Eq. 22
+        ax = fmaf(wgt, d4.x, ax); ay = fmaf(wgt, d4.y, ay); az = fmaf(wgt, d4.z, az);
+      }
+    }
+  }
+  if (tid < mcount && (ax != 0.f || ay != 0.f || az != 0.f)) {
+    float* o = p.marker + ((size_t)e * p.M + __ldg(&pt.mstart) + tid) * 3;
+    o[0] += ax; o[1] += ay; o[2] += az;                               // Eq. 23
+  }
+}
+
+__global__ void ts_reset_shear_kernel(const __grid_constant__ TsStepParams p, const uint8_t* mask) {
+  const size_t per = (size_t)p.P * p.K * p.pc_n;
+  const size_t gt = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gt >= (size_t)p.E * per) return;
+  const int e = (int)(gt / per);
+  if (mask && !mask[e]) return;
+  p.sh_on[gt] = 0;
+}
+
 }  // namespace
 
 unsigned long long ts_bank_elems_per_grid(int N) { return (unsigned long long)(N - 1) * (N - 1) * N; }
@@ -1589,6 +1689,17 @@ unsigned long long ts_frame_bytes() { return sizeof(FrameS); }
 int ts_launch_frames(const TsStepParams& p, void* stream) {
   const long long n = (long long)p.E * p.P * p.K;
   ts_frames_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(p);
+  return (int)cudaGetLastError();
+}
+
+int ts_launch_shear(const TsStepParams& p, void* stream) {
+  ts_shear_kernel<<<(unsigned)(p.E * p.P), 256, 0, (cudaStream_t)stream>>>(p);
+  return (int)cudaGetLastError();
+}
+
+int ts_launch_reset_shear(const TsStepParams& p, const uint8_t* mask, void* stream) {
+  const size_t n = (size_t)p.E * p.P * p.K * p.pc_n;
+  ts_reset_shear_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(p, mask);
   return (int)cudaGetLastError();
 }
 

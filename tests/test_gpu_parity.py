@@ -467,3 +467,44 @@ def test_point_cloud_proximity_taxel():
     print(json.dumps({"proxpc_max_ratio": worst, "taxels_with_force": nz}))
     assert worst <= 1.0 and nz > 20000
     sim.close()
+
+
+def test_elastomer_shear_history():
+    """ElastomerTaxel shear history (App. A.7 Eq. 22-23, constants P:304, N_pc = 1,000 tracked points per
+    object): anchors per (env, patch, tracked point) carried over 40 steps of the config-5 trajectories (objects slide
+    over the pads), a masked reset in the middle, shear added to the dilation markers; element-wise against the oracle."""
+    import torch
+    from oracle import oracle as O
+    from parity import Comparator
+    from paper_2606_22332_b200.binding import TactileSim
+    w = W.config(5, n_envs=32)
+    pts, cid = W.point_cloud_bank(w, 1000)
+    phys = dict(w.physics, shear_enable=1)
+    outs = ("contact", "depth", "ft", "marker", "prox")
+    sim = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=phys, outputs=outs)
+    sim.set_geometry(w.types, w.params, w.bank, w.voxel)
+    sim.set_pointclouds(pts, cid)
+    plain = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=w.physics, outputs=outs)
+    plain.set_geometry(w.types, w.params, w.bank, w.voxel)
+    orc = O.Oracle(w.patches, w.T, w.L, w.K, np.arange(w.E), physics=phys, threads=os.cpu_count() or 1)
+    orc.set_geometry(w.types, w.params, w.bank, w.voxel)
+    orc.set_pointclouds(pts, cid)
+    lay = sim.layout.view()
+    cmp_ = Comparator(lay, phys, False, lay["radius"])
+    moved = 0
+    for s in range(40):
+        if s == 20:
+            mask = (np.arange(w.E) % 2 == 0).astype(np.uint8)
+            sim.reset(torch.from_numpy(mask).cuda())
+            orc.reset(mask)
+        inp = w.inputs(s)
+        x = sim.upload(inp)
+        g = sim.step(x)
+        d = plain.step(x)
+        torch.cuda.synchronize()
+        cmp_.step({k: v.cpu().numpy() for k, v in g.items()}, orc.step(inp, want=outs))
+        moved += int(((g["marker"] - d["marker"]).abs() > 1e-4).sum().item())
+    rep = cmp_.report()
+    _assert_ok(rep)
+    assert rep["max_ratio"]["marker"] <= 1.0 and moved > 5000, (rep["max_ratio"], moved)    # the shear term really acts
+    sim.close(); plain.close()
