@@ -207,6 +207,44 @@ Query sdf_grid(V3 x, const float* data, int N, double hv) {
   return q;
 }
 
+// Closest point of triangle (a, b, c) to p: the Voronoi-region walk of Ericson, "Real-Time Collision Detection" 5.1.5,
+// restated (vertex regions, edge regions, face).
+V3 closest_point_triangle(V3 p, V3 a, V3 b, V3 c) {
+  V3 ab = b - a, ac = c - a, ap = p - a;
+  double d1 = dot(ab, ap), d2 = dot(ac, ap);
+  if (d1 <= 0.0 && d2 <= 0.0) return a;
+  V3 bp = p - b;
+  double d3 = dot(ab, bp), d4 = dot(ac, bp);
+  if (d3 >= 0.0 && d4 <= d3) return b;
+  double vc = d1 * d4 - d3 * d2;
+  if (vc <= 0.0 && d1 >= 0.0 && d3 <= 0.0) return a + (d1 / (d1 - d3)) * ab;
+  V3 cp = p - c;
+  double d5 = dot(ab, cp), d6 = dot(ac, cp);
+  if (d6 >= 0.0 && d5 <= d6) return c;
+  double vb = d5 * d2 - d1 * d6;
+  if (vb <= 0.0 && d2 >= 0.0 && d6 <= 0.0) return a + (d2 / (d2 - d6)) * ac;
+  double va = d3 * d6 - d5 * d4;
+  if (va <= 0.0 && (d4 - d3) >= 0.0 && (d5 - d6) >= 0.0) return b + ((d4 - d3) / ((d4 - d3) + (d5 - d6))) * (c - b);
+  double denom = 1.0 / (va + vb + vc);
+  return a + (vb * denom) * ab + (vc * denom) * ac;
+}
+
+// Ray (orig, unit dir) against triangle (a, b, c), both faces (Moeller-Trumbore, restated): hit distance t >= 0, or -1.
+double ray_triangle(V3 orig, V3 dir, V3 a, V3 b, V3 c) {
+  V3 e1 = b - a, e2 = c - a, pv = cross(dir, e2);
+  double det = dot(e1, pv);
+  if (std::fabs(det) < 1e-300) return -1.0;
+  double inv = 1.0 / det;
+  V3 tv = orig - a;
+  double u = dot(tv, pv) * inv;
+  if (u < 0.0 || u > 1.0) return -1.0;
+  V3 qv = cross(tv, e1);
+  double v = dot(dir, qv) * inv;
+  if (v < 0.0 || u + v > 1.0) return -1.0;
+  double t = dot(e2, qv) * inv;
+  return t >= 0.0 ? t : -1.0;
+}
+
 struct Geom {
   int type;
   double p[4];
@@ -316,6 +354,12 @@ struct Oracle {
   std::vector<V3> sh_e;                       // [E,P,K,N] anchor e_p
   std::vector<V3> p_center, p_ua, p_va;       // [P] pad centre and unit axes (fp32 values), link frame
   std::vector<double> p_su, p_sv;             // [P] pad extents
+  // raycast depth backend (App. A.1): bank of triangle meshes in the object frame, mesh of each (env, object)
+  std::vector<float> rc_verts;                // all vertices [sum V, 3]
+  std::vector<int32_t> rc_tris;               // all triangles [sum F, 3], vertex indices local to their mesh
+  std::vector<int32_t> rc_voff, rc_toff;      // [G + 1] offsets
+  std::vector<int32_t> rc_id;                 // [E,K], -1 = no mesh
+  double *rc_depth = nullptr, *rc_nrm = nullptr, *rc_gap = nullptr;   // [E,T], [E,T,3], [E,T] outputs handed in by orc_set_raycast_out
   std::vector<std::deque<std::vector<double>>> hist;  // [E] the last Delta + J post-crosstalk fields [T,6] of the episode
   std::vector<uint32_t> n_step, episode;      // [E]
 };
@@ -722,6 +766,47 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
         }
         for (int c = 0; c < 6; ++c) o.proxpc[ej * 6 + c] = out6[c];
       }
+      // A.1 raycast depth backend, brute force over every triangle of every meshed object (the BVH of the
+      // paper only prunes candidates): sphere-triangle closest-point test, penetration = R_j - dist, and ray-triangle
+      // test from q_j along -a_j, penetration = R_j - hit_distance (reading Q28: ray from the probe centre, both
+      // faces); the deepest of all wins, the normal is the winning triangle's face normal (object winding), reported in
+      // the sensor-link frame.  rc_gap = margin to the best triangle with a DIFFERENT normal (comparator aid).
+      if (o.rc_depth) {
+        double best = 0.0, second = 0.0;
+        V3 bn = {0, 0, 0};
+        if (active) {
+          const double Rj = o.radius[j];
+          for (int k = 0; k < K; ++k) {
+            const int id = o.rc_id.empty() ? -1 : o.rc_id[(size_t)e * K + k];
+            if (id < 0) continue;
+            V3 pO = ld3(obj_pos + ((size_t)e * K + k) * 3);
+            M3 RO = quat_to_R(obj_quat + ((size_t)e * K + k) * 4);
+            V3 qo = mulT(RO, q - pO), ao = mulT(RO, a);
+            const float* V = o.rc_verts.data() + (size_t)o.rc_voff[id] * 3;
+            for (int f = o.rc_toff[id]; f < o.rc_toff[id + 1]; ++f) {
+              V3 A = ld3(V + 3 * o.rc_tris[3 * f]), B = ld3(V + 3 * o.rc_tris[3 * f + 1]), C3 = ld3(V + 3 * o.rc_tris[3 * f + 2]);
+              double pen = 0.0;
+              double dist = norm(qo - closest_point_triangle(qo, A, B, C3));
+              if (dist < Rj) pen = Rj - dist;
+              double th = ray_triangle(qo, (-1.0) * ao, A, B, C3);
+              if (th >= 0.0 && th < Rj) pen = std::fmax(pen, Rj - th);
+              if (!(pen > 0.0)) continue;
+              V3 fn = cross(B - A, C3 - A);
+              double fl = norm(fn);
+              V3 nw = fl > 0.0 ? mulT(RL, mul(RO, (1.0 / fl) * fn)) : V3{0, 0, 0};   // link frame
+              if (pen > best) {
+                if (norm(nw - bn) > 1e-6) second = best;
+                best = pen; bn = nw;
+              } else if (pen > second && norm(nw - bn) > 1e-6) {
+                second = pen;
+              }
+            }
+          }
+        }
+        o.rc_depth[ej] = best;
+        if (o.rc_nrm) { o.rc_nrm[ej * 3] = bn.x; o.rc_nrm[ej * 3 + 1] = bn.y; o.rc_nrm[ej * 3 + 2] = bn.z; }
+        if (o.rc_gap) o.rc_gap[ej] = best - second;
+      }
     }
     // O6 (Eq. 18-21, 23 first sum; Q15-Q17): dilation of each patch's markers by its active taxels
     if (marker) {
@@ -1054,6 +1139,30 @@ int orc_set_pointclouds(void* h, int n_clouds, int n_points, const float* pts, c
   return 0;
 }
 void orc_set_proxpc(void* h, double* proxpc) { ((Oracle*)h)->proxpc = proxpc; }
+
+// A.1 raycast backend: bank of triangle meshes (object frame; vertex / triangle offsets [n_meshes + 1]) and the mesh of
+// each (env, object) (-1 = none); orc_set_raycast_out hands in the outputs of the following orc_step calls.
+int orc_set_meshes(void* h, int n_meshes, const int32_t* vert_off, const int32_t* tri_off, const float* verts,
+                   const int32_t* tris, const int32_t* mesh_id) {
+  Oracle& o = *(Oracle*)h;
+  o.rc_voff.assign(vert_off, vert_off + n_meshes + 1); o.rc_toff.assign(tri_off, tri_off + n_meshes + 1);
+  o.rc_verts.assign(verts, verts + (size_t)vert_off[n_meshes] * 3);
+  o.rc_tris.assign(tris, tris + (size_t)tri_off[n_meshes] * 3);
+  o.rc_id.assign(mesh_id, mesh_id + (size_t)o.E * o.K);
+  for (int32_t id : o.rc_id) if (id >= n_meshes) return 1;
+  return 0;
+}
+void orc_set_raycast_out(void* h, double* depth, double* nrm, double* gap) {
+  Oracle& o = *(Oracle*)h;
+  o.rc_depth = depth; o.rc_nrm = nrm; o.rc_gap = gap;
+}
+void orc_closest_point_triangle(const double* p, const double* a, const double* b, const double* c, double* out) {
+  V3 r = closest_point_triangle({p[0], p[1], p[2]}, {a[0], a[1], a[2]}, {b[0], b[1], b[2]}, {c[0], c[1], c[2]});
+  out[0] = r.x; out[1] = r.y; out[2] = r.z;
+}
+double orc_ray_triangle(const double* o, const double* d, const double* a, const double* b, const double* c) {
+  return ray_triangle({o[0], o[1], o[2]}, {d[0], d[1], d[2]}, {a[0], a[1], a[2]}, {b[0], b[1], b[2]}, {c[0], c[1], c[2]});
+}
 
 // R10: hands in the buffers the following orc_step calls fill with the noisy scalar readouts (NULL = not produced) and
 // their comparator aids (distance to the quantisation boundary per element; marker ASYM sign-flip margin).

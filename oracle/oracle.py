@@ -92,6 +92,11 @@ def lib():
         L.orc_set_scalar_noisy.argtypes = [C.c_void_p] + [C.c_void_p] * 7
         L.orc_set_pointclouds.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
         L.orc_set_proxpc.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_set_meshes.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 5
+        L.orc_set_raycast_out.argtypes = [C.c_void_p] + [C.c_void_p] * 3
+        L.orc_closest_point_triangle.argtypes = [C.c_void_p] * 5
+        L.orc_ray_triangle.restype = C.c_double
+        L.orc_ray_triangle.argtypes = [C.c_void_p] * 5
         L.orc_max_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -216,6 +221,17 @@ class Oracle:
         if self.L.orc_set_pointclouds(self.h, pts.shape[0], pts.shape[1], _p(pts), _p(cid)):
             raise ValueError("orc_set_pointclouds: cloud id out of range")
 
+    def set_meshes(self, meshes, mesh_id):
+        """A.1 raycast backend: meshes = list of (verts [V,3] fp32, tris [F,3] int32) in the object frame;
+        mesh_id [E, K] int32 (-1 = object has no mesh)."""
+        voff = np.cumsum([0] + [len(v) for v, _ in meshes]).astype(np.int32)
+        toff = np.cumsum([0] + [len(t) for _, t in meshes]).astype(np.int32)
+        verts = _f32(np.concatenate([v for v, _ in meshes]))
+        tris = np.ascontiguousarray(np.concatenate([t for _, t in meshes]), dtype=np.int32)
+        mid = np.ascontiguousarray(mesh_id, dtype=np.int32).reshape(self.E, self.K)
+        if self.L.orc_set_meshes(self.h, len(meshes), _p(voff), _p(toff), _p(verts), _p(tris), _p(mid)):
+            raise ValueError("orc_set_meshes: mesh id out of range")
+
     def reset(self, env_mask=None):
         m = None if env_mask is None else np.ascontiguousarray(env_mask, dtype=np.uint8)
         self.L.orc_reset(self.h, _p(m))
@@ -233,6 +249,8 @@ class Oracle:
         if "marker" in want and M > 0: out["marker"] = np.zeros((E, M, 3))
         if "prox" in want: out["prox"] = np.zeros((E, T))
         if "proxpc" in want: out["proxpc"] = np.zeros((E, T, 6))
+        if "depth_rc" in want:
+            out["depth_rc"] = np.zeros((E, T)); out["nrm_rc"] = np.zeros((E, T, 3)); out["aux_rc_gap"] = np.zeros((E, T))
         if self.params.noise_enable:
             if "ft_noisy" in want: out["ft_noisy"] = np.zeros((E, T, 6))
             if "dead" in want: out["dead"] = np.zeros((E, T), np.uint8)
@@ -263,6 +281,7 @@ class Oracle:
         self.L.orc_set_aux_rgate(self.h, _p(g("aux_rgate")))
         self.L.orc_set_aux_wingap(self.h, _p(g("aux_wingap")))
         self.L.orc_set_proxpc(self.h, _p(g("proxpc")))
+        self.L.orc_set_raycast_out(self.h, _p(g("depth_rc")), _p(g("nrm_rc")), _p(g("aux_rc_gap")))
         self.L.orc_set_scalar_noisy(self.h, _p(g("depth_noisy")), _p(g("prox_noisy")), _p(g("marker_noisy")), _p(g("aux_sq_depth")),
                                     _p(g("aux_sq_prox")), _p(g("aux_sq_marker")), _p(g("aux_sasym_marker")))
         self.L.orc_step(self.h, _p(a["link_pos"]), _p(a["link_quat"]), _p(a["link_linvel"]), _p(a["link_angvel"]),
@@ -328,6 +347,16 @@ def march(kind, params, x0, a, r_prox, steps, grid=None, voxel=0.0):
         N = gp.shape[0]
     x0, a = _f64(x0), _f64(a)
     return lib().orc_march(GEOM[kind], _p(pr), _p(gp), N, float(voxel), _p(x0), _p(a), float(r_prox), int(steps))
+
+
+def closest_point_triangle(p, a, b, c):
+    o = np.zeros(3)
+    lib().orc_closest_point_triangle(_p(_f64(p)), _p(_f64(a)), _p(_f64(b)), _p(_f64(c)), _p(o))
+    return o
+
+
+def ray_triangle(orig, d, a, b, c):
+    return lib().orc_ray_triangle(_p(_f64(orig)), _p(_f64(d)), _p(_f64(a)), _p(_f64(b)), _p(_f64(c)))
 
 
 def max_threads():

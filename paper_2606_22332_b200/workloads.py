@@ -315,5 +315,49 @@ def point_cloud_bank(w, n_points=5000):
     return pts, cid.reshape(-1, 1)
 
 
+def cube_mesh(b):
+    """12-triangle box with half-extents b (outward winding): (verts [8,3] fp32, tris [12,3] int32)."""
+    b = np.asarray(b, np.float64)
+    v = np.array([[sx, sy, sz] for sx in (-1, 1) for sy in (-1, 1) for sz in (-1, 1)], np.float64) * b
+    quads = [(0, 1, 3, 2), (4, 6, 7, 5), (0, 4, 5, 1), (2, 3, 7, 6), (0, 2, 6, 4), (1, 5, 7, 3)]   # -x, +x, -y, +y, -z, +z
+    tris = [t for a, b_, c, d in quads for t in ((a, b_, c), (a, c, d))]
+    return v.astype(np.float32), np.asarray(tris, np.int32)
+
+
+def star_mesh(level=3, scale=1.0, rot=None):
+    """Triangle mesh of the star surface r(u) = 40 mm (1 + 0.2 Y_3^2(u)): an icosahedron subdivided `level` times
+    (20 * 4^level triangles, outward winding), vertices pushed to the star radius.  Object frame, fp32."""
+    t = (1.0 + math.sqrt(5.0)) / 2.0
+    v = [(-1, t, 0), (1, t, 0), (-1, -t, 0), (1, -t, 0), (0, -1, t), (0, 1, t), (0, -1, -t), (0, 1, -t), (t, 0, -1), (t, 0, 1),
+         (-t, 0, -1), (-t, 0, 1)]
+    f = [(0, 11, 5), (0, 5, 1), (0, 1, 7), (0, 7, 10), (0, 10, 11), (1, 5, 9), (5, 11, 4), (11, 10, 2), (10, 7, 6), (7, 1, 8),
+         (3, 9, 4), (3, 4, 2), (3, 2, 6), (3, 6, 8), (3, 8, 9), (4, 9, 5), (2, 4, 11), (6, 2, 10), (8, 6, 7), (9, 8, 1)]
+    v = [np.asarray(x, np.float64) / np.linalg.norm(x) for x in v]
+    for _ in range(level):
+        cache, nf = {}, []
+
+        def mid(i, j):
+            key = (min(i, j), max(i, j))
+            if key not in cache:
+                m = v[i] + v[j]
+                v.append(m / np.linalg.norm(m))
+                cache[key] = len(v) - 1
+            return cache[key]
+        for a, b, c in f:
+            ab, bc, ca = mid(a, b), mid(b, c), mid(c, a)
+            nf += [(a, ab, ca), (b, bc, ab), (c, ca, bc), (ab, bc, ca)]
+        f = nf
+    u = np.asarray(v)
+    return (star_radius(u, scale, rot)[:, None] * u).astype(np.float32), np.asarray(f, np.int32)
+
+
+def mesh_bank(w, level=3):
+    """Triangle meshes for a grid-object workload (configs 3-5): mesh k triangulates star k of the SDF bank; envs whose
+    object is a primitive get mesh_id -1.  Returns (list of (verts, tris), mesh_id [E, 1])."""
+    meshes = [star_mesh(level, s["scale"], s["rot"]) for s in w.stars]
+    mid = np.where(w.types[:, 0] == GEOM_GRID, w.params[:, 0, 0].astype(np.int32), -1).astype(np.int32)
+    return meshes, mid.reshape(-1, 1)
+
+
 def config(cid, n_envs=None, seed=0):
     return Workload(cid, n_envs=n_envs, seed=seed)
