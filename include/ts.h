@@ -128,8 +128,11 @@ enum {                      /* output_mask bits.  ts_step contract: every output
   TS_OUT_DEPTH_NOISY = 1 << 7,  /* f32 [E,T]   ContactDepth readout; senses with the Eq. 26 radius when radius_noise > 0 */
   TS_OUT_PROX_NOISY = 1 << 8,   /* f32 [E,T]   Proximity readout */
   TS_OUT_MARKER_NOISY = 1 << 9, /* f32 [E,M,3] Elastomer marker readout (every marker is a probe of its own) */
-  TS_OUT_PROXPC = 1 << 10       /* f32 [E,T,6] point-cloud ProximityTaxel (App. A.6, Eq. 12-17), link frame; needs
+  TS_OUT_PROXPC = 1 << 10,      /* f32 [E,T,6] point-cloud ProximityTaxel (App. A.6, Eq. 12-17), link frame; needs
                                    ts_set_pointclouds */
+  /* raycast contact-depth backend (App. A.1) on triangle meshes; needs ts_set_meshes */
+  TS_OUT_DEPTH_RC = 1 << 11,    /* f32 [E,T]   deepest of sphere-triangle (R_j - dist) and ray-triangle (R_j - hit) */
+  TS_OUT_NRM_RC = 1 << 12       /* f32 [E,T,3] face normal of the deepest-penetrating triangle, link frame (0 = none) */
 };
 
 typedef struct ts_config {
@@ -249,6 +252,8 @@ typedef struct ts_step_out {
   float* prox_noisy;   /* [E,T]   */
   float* marker_noisy; /* [E,M,3] */
   float* proxpc;       /* [E,T,6] */
+  float* depth_rc;     /* [E,T]   */
+  float* nrm_rc;       /* [E,T,3] */
 } ts_step_out;
 
 /* Creates a context on `cuda_device` (must be sm_100).  Allocates every device buffer the
@@ -272,6 +277,22 @@ typedef struct ts_pointclouds {
   const int32_t* cloud_id;
 } ts_pointclouds;
 ts_status ts_set_pointclouds(ts_ctx* ctx, const ts_pointclouds* pc, void* stream);
+
+/* App. A.1 raycast backend: a bank of triangle meshes in the OBJECT frame -- host arrays: vert_off / tri_off
+ * [n_meshes + 1] offsets into verts [sum V, 3] fp32 and tris [sum F, 3] int32 (vertex indices local to their mesh,
+ * outward winding) -- and the mesh of every (env, object) (host int32 [E,K], -1 = none).  The ctx builds one bounding
+ * volume hierarchy per mesh (median split, leaves of <= 4 triangles; static, because every query is made in the object
+ * frame) and keeps it on the device.  Needed before a ts_step that asks for TS_OUT_DEPTH_RC / TS_OUT_NRM_RC.
+ * Synchronises `stream` once; may be called again. */
+typedef struct ts_meshes {
+  int32_t n_meshes;
+  const int32_t* vert_off;
+  const int32_t* tri_off;
+  const float* verts;
+  const int32_t* tris;
+  const int32_t* mesh_id;
+} ts_meshes;
+ts_status ts_set_meshes(ts_ctx* ctx, const ts_meshes* meshes, void* stream);
 
 /* One pass of the whole hot path over all envs.  Asynchronous; never allocates. */
 ts_status ts_step(ts_ctx* ctx, const ts_step_in* in, const ts_step_out* out, void* stream);

@@ -18,13 +18,13 @@ HYST = {"off": 0, "maxwell": 1, "asym": 2}
 FORM = {"auto": 0, "fused": 1, "split": 2}
 GEOM = {"none": 0, "sphere": 1, "box": 2, "capsule": 3, "sdf": 4, "grid": 4}
 OUT_BITS = {"contact": 1, "depth": 2, "ft": 4, "marker": 8, "prox": 16, "ft_noisy": 32, "dead": 64,
-            "depth_noisy": 128, "prox_noisy": 256, "marker_noisy": 512, "proxpc": 1024}
+            "depth_noisy": 128, "prox_noisy": 256, "marker_noisy": 512, "proxpc": 1024, "depth_rc": 2048, "nrm_rc": 4096}
 SN_CLASS = {"depth": 0, "prox": 1, "marker": 2}          # noisy scalar readouts (ts_config.sn_*[3])
 SN_KNOBS = ("sigma_white", "sigma_rw", "bias", "quant", "stuck_min", "stuck_max")
 
 # every symbol include/ts.h declares (tests check that the library exports them all)
 SYMBOLS = ["ts_layout_create", "ts_layout_add_patch", "ts_layout_filter_links", "ts_layout_finalize", "ts_layout_get",
-           "ts_layout_destroy", "ts_config_default", "ts_create", "ts_set_geometry", "ts_set_pointclouds", "ts_step", "ts_step_host",
+           "ts_layout_destroy", "ts_config_default", "ts_create", "ts_set_geometry", "ts_set_pointclouds", "ts_set_meshes", "ts_step", "ts_step_host",
            "ts_reset", "ts_destroy", "ts_last_error", "ts_n_taxels", "ts_n_markers", "ts_launches_per_step",
            "ts_kernel_time_ms", "ts_kernel_times_ms", "ts_first_kernel_time_ms", "ts_version"]
 
@@ -77,6 +77,11 @@ class Config(C.Structure):
                 ("eta_exit", C.c_float)]
 
 
+class Meshes(C.Structure):
+    _fields_ = [("n_meshes", C.c_int32), ("vert_off", C.c_void_p), ("tri_off", C.c_void_p), ("verts", C.c_void_p),
+                ("tris", C.c_void_p), ("mesh_id", C.c_void_p)]
+
+
 class PointClouds(C.Structure):
     _fields_ = [("n_clouds", C.c_int32), ("n_points", C.c_int32), ("points", C.c_void_p), ("cloud_id", C.c_void_p)]
 
@@ -93,7 +98,7 @@ class StepIn(C.Structure):
 
 class StepOut(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in ("contact", "depth", "ft", "marker", "prox", "ft_noisy", "dead", "depth_noisy",
-                                          "prox_noisy", "marker_noisy", "proxpc")]
+                                          "prox_noisy", "marker_noisy", "proxpc", "depth_rc", "nrm_rc")]
 
 
 IN_KEYS = [k for k, _ in StepIn._fields_]
@@ -121,6 +126,7 @@ def lib():
         L.ts_create.argtypes = [C.POINTER(Config), C.c_int, C.POINTER(vp)]
         L.ts_set_geometry.argtypes = [vp, C.POINTER(Geometry), vp]
         L.ts_set_pointclouds.argtypes = [vp, C.POINTER(PointClouds), vp]
+        L.ts_set_meshes.argtypes = [vp, C.POINTER(Meshes), vp]
         L.ts_step.argtypes = [vp, C.POINTER(StepIn), C.POINTER(StepOut), vp]
         L.ts_step_host.argtypes = [vp, C.POINTER(StepIn), C.POINTER(StepOut), vp]
         L.ts_reset.argtypes = [vp, vp, vp]
@@ -256,7 +262,8 @@ class TactileSim:
         return dict(contact=((E, T), t.uint8), depth=((E, T), t.float32), ft=((E, T, 6), t.float32),
                     marker=((E, M, 3), t.float32), prox=((E, T), t.float32), ft_noisy=((E, T, 6), t.float32),
                     dead=((E, T), t.uint8), depth_noisy=((E, T), t.float32), prox_noisy=((E, T), t.float32),
-                    marker_noisy=((E, M, 3), t.float32), proxpc=((E, T, 6), t.float32))
+                    marker_noisy=((E, M, 3), t.float32), proxpc=((E, T, 6), t.float32),
+                    depth_rc=((E, T), t.float32), nrm_rc=((E, T, 3), t.float32))
 
     def in_shapes(self):
         E, L, K = self.E, self.L, self.K
@@ -286,6 +293,19 @@ class TactileSim:
             g.grids = bank.ctypes.data_as(C.c_void_p)
         with self.torch.cuda.device(self.device):
             _check(lib().ts_set_geometry(self.h, C.byref(g), self._stream()), self.h, "ts_set_geometry")
+
+    def set_meshes(self, meshes, mesh_id):
+        """App. A.1 raycast backend: meshes = list of (verts [V,3] fp32, tris [F,3] int32) in the object frame;
+        mesh_id [E, K] int32 (-1 = object has no mesh)."""
+        voff = np.cumsum([0] + [len(v) for v, _ in meshes]).astype(np.int32)
+        toff = np.cumsum([0] + [len(t) for _, t in meshes]).astype(np.int32)
+        verts = np.ascontiguousarray(np.concatenate([v for v, _ in meshes]), dtype=np.float32)
+        tris = np.ascontiguousarray(np.concatenate([t for _, t in meshes]), dtype=np.int32)
+        mid = np.ascontiguousarray(mesh_id, dtype=np.int32).reshape(self.E, self.K)
+        vp = lambda a: a.ctypes.data_as(C.c_void_p)
+        m = Meshes(len(meshes), vp(voff), vp(toff), vp(verts), vp(tris), vp(mid))
+        with self.torch.cuda.device(self.device):
+            _check(lib().ts_set_meshes(self.h, C.byref(m), self._stream()), self.h, "ts_set_meshes")
 
     def set_pointclouds(self, points, cloud_id):
         """App. A.6: points [G, N, 3] fp32 in the object frame; cloud_id [E, K] int32 (-1 = object not tracked)."""

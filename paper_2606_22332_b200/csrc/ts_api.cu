@@ -52,7 +52,9 @@ struct ts_ctx {
   uint32_t *reset_step = nullptr, *episode = nullptr;
   // device staging of ts_step_host
   float* stage_in[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-  void* stage_out[11] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  void* stage_out[13] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  // raycast depth backend (A.1): BVH nodes, leaf-ordered triangles, root per mesh, mesh of each (env, object)
+  float4* rc_nodes = nullptr; float4* rc_tri = nullptr; int32_t* rc_root = nullptr; int32_t* rc_id = nullptr; bool have_mesh = false;
   // point-cloud ProximityTaxel (A.6): clouds sorted by grid cell, cell starts, grid records, cloud of each (env, object)
   float4* pc_pts = nullptr; int32_t* pc_cell = nullptr; TsPcGrid* pc_grid = nullptr; int32_t* pc_id = nullptr;
   int32_t* tx_patch = nullptr;
@@ -103,6 +105,7 @@ void free_all(ts_ctx* c) {
   cudaFree(c->groups); cudaFree(c->chunks); cudaFree(c->mk_item1); cudaFree(c->mk_item2); cudaFree(c->mk_tab); cudaFree(c->mk_tab8); cudaFree(c->grp_link);
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->env_perm); cudaFree(c->frames_g); cudaFree(c->patch_link); cudaFree(c->bank); cudaFree(c->bank_stage); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch); cudaFree(c->ft_scratch_r); cudaFree(c->st_ring);
+  cudaFree(c->rc_nodes); cudaFree(c->rc_tri); cudaFree(c->rc_root); cudaFree(c->rc_id);
   cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw);
   cudaFree(c->pc_pts); cudaFree(c->pc_cell); cudaFree(c->pc_grid); cudaFree(c->pc_id); cudaFree(c->tx_patch);
   cudaFree(c->sn_h); cudaFree(c->sn_d); cudaFree(c->sm_h); cudaFree(c->sm_d); cudaFree(c->depth_pert); cudaFree(c->sc_depth);
@@ -183,6 +186,7 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.pc_pts = c->pc_pts; p.pc_cell = c->pc_cell; p.pc_grid = c->pc_grid; p.pc_id = c->pc_id; p.pc_n = c->pc_n; p.tx_patch = c->tx_patch;
   p.pc_radius = g.pc_radius; p.pc_k = g.pc_k; p.pc_ks = g.pc_ks; p.pc_density = g.pc_density;
   p.sh_on = c->sh_on; p.sh_e = c->sh_e; p.pc_raw = c->pc_raw;
+  p.rc_nodes = c->rc_nodes; p.rc_tri = c->rc_tri; p.rc_root = c->rc_root; p.rc_id = c->rc_id;
   p.shear_enable = (g.shear_enable && c->sh_on) ? 1 : 0; p.s_s = g.s_s; p.lambda_s = g.lambda_s; p.eta_enter = g.eta_enter; p.eta_exit = g.eta_exit;
 }
 }  // namespace
@@ -216,7 +220,7 @@ int32_t ts_launches_per_step(const ts_ctx* ctx) {
   if (!ctx) return 0;
   return ((ctx->cfg.noise_enable && !ctx->fused) ? 3 : 2) +
          ((ctx->cfg.output_mask & (TS_OUT_DEPTH_NOISY | TS_OUT_PROX_NOISY | TS_OUT_MARKER_NOISY)) ? 1 : 0) +
-         ((ctx->cfg.output_mask & TS_OUT_PROXPC) ? 1 : 0) +
+         ((ctx->cfg.output_mask & TS_OUT_PROXPC) ? 1 : 0) + ((ctx->cfg.output_mask & (TS_OUT_DEPTH_RC | TS_OUT_NRM_RC)) ? 1 : 0) +
          ((ctx->cfg.shear_enable && (ctx->cfg.output_mask & (TS_OUT_MARKER | TS_OUT_MARKER_NOISY))) ? 1 : 0);
 }
 
@@ -586,6 +590,95 @@ ts_status ts_set_geometry(ts_ctx* c, const ts_geometry* geo, void* stream) {
   return TS_OK;
 }
 
+namespace {
+// median-split BVH over the triangles tri[lo, hi) of one mesh (indices into `order`); returns the node index
+struct BvhBuild {
+  const float* V;             // vertices of the mesh
+  const int32_t* T;           // triangles of the mesh (local vertex indices)
+  std::vector<int32_t> order; // triangle permutation (leaf order)
+  std::vector<float4>* nodes; // flattened nodes (2 float4 each), shared by all meshes
+  std::vector<float4>* tris;  // leaf-ordered triangles (3 float4 each), shared by all meshes
+  void box(int t, float lo[3], float hi[3]) const {
+    for (int a = 0; a < 3; ++a) { lo[a] = INFINITY; hi[a] = -INFINITY; }
+    for (int v = 0; v < 3; ++v)
+      for (int a = 0; a < 3; ++a) { const float x = V[3 * T[3 * t + v] + a]; lo[a] = std::fmin(lo[a], x); hi[a] = std::fmax(hi[a], x); }
+  }
+  int build(int lo_i, int hi_i) {
+    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int i = lo_i; i < hi_i; ++i) {
+      float l[3], h[3];
+      box(order[i], l, h);
+      for (int a = 0; a < 3; ++a) { lo[a] = std::fmin(lo[a], l[a]); hi[a] = std::fmax(hi[a], h[a]); }
+    }
+    const int node = (int)(nodes->size() / 2);
+    nodes->push_back(make_float4(lo[0], lo[1], lo[2], 0.f));
+    nodes->push_back(make_float4(hi[0], hi[1], hi[2], 0.f));
+    auto seti = [&](size_t idx, int v) { int32_t iv = v; std::memcpy(&(*nodes)[idx].w, &iv, 4); };
+    if (hi_i - lo_i <= 4) {   // leaf: triangles appended in leaf order
+      seti((size_t)2 * node, (int)(tris->size() / 3));
+      seti((size_t)2 * node + 1, hi_i - lo_i);
+      for (int i = lo_i; i < hi_i; ++i)
+        for (int v = 0; v < 3; ++v) { const float* p = V + 3 * T[3 * order[i] + v]; tris->push_back(make_float4(p[0], p[1], p[2], 0.f)); }
+      return node;
+    }
+    int ax = 0;
+    if (hi[1] - lo[1] > hi[ax] - lo[ax]) ax = 1;
+    if (hi[2] - lo[2] > hi[ax] - lo[ax]) ax = 2;
+    const int mid = (lo_i + hi_i) / 2;
+    std::nth_element(order.begin() + lo_i, order.begin() + mid, order.begin() + hi_i, [&](int a, int b) {
+      float la[3], ha[3], lb[3], hb[3];
+      box(a, la, ha); box(b, lb, hb);
+      return la[ax] + ha[ax] < lb[ax] + hb[ax];
+    });
+    const int left = build(lo_i, mid), right = build(mid, hi_i);
+    seti((size_t)2 * node, left);
+    seti((size_t)2 * node + 1, -right);
+    return node;
+  }
+};
+}  // namespace
+
+ts_status ts_set_meshes(ts_ctx* c, const ts_meshes* m, void* stream) {
+  if (!c) return TS_ERR_INVALID_ARG;
+  if (!m || m->n_meshes < 1 || !m->vert_off || !m->tri_off || !m->verts || !m->tris || !m->mesh_id)
+    return fail(c, TS_ERR_INVALID_ARG, "ts_set_meshes: NULL argument or empty bank");
+  const int G = m->n_meshes;
+  const size_t EK = (size_t)c->cfg.n_envs * c->cfg.objs_per_env;
+  for (size_t i = 0; i < EK; ++i)
+    if (m->mesh_id[i] >= G) return fail(c, TS_ERR_INVALID_ARG, "ts_set_meshes: mesh id out of range");
+  std::vector<float4> nodes, tris;
+  std::vector<int32_t> roots(G);
+  for (int g = 0; g < G; ++g) {
+    const int nv = m->vert_off[g + 1] - m->vert_off[g], nt = m->tri_off[g + 1] - m->tri_off[g];
+    if (nv < 3 || nt < 1) return fail(c, TS_ERR_INVALID_ARG, "ts_set_meshes: empty mesh");
+    const int32_t* T = m->tris + (size_t)m->tri_off[g] * 3;
+    for (int i = 0; i < 3 * nt; ++i)
+      if (T[i] < 0 || T[i] >= nv) return fail(c, TS_ERR_INVALID_ARG, "ts_set_meshes: vertex index out of range");
+    BvhBuild b;
+    b.V = m->verts + (size_t)m->vert_off[g] * 3; b.T = T; b.nodes = &nodes; b.tris = &tris;
+    b.order.resize(nt);
+    for (int i = 0; i < nt; ++i) b.order[i] = i;
+    roots[g] = b.build(0, nt);
+  }
+  DeviceGuard guard(c->device);
+  cudaStream_t st = (cudaStream_t)stream;
+  c->have_mesh = false;
+  TS_CUDA(c, cudaStreamSynchronize(st));
+  cudaFree(c->rc_nodes); cudaFree(c->rc_tri); cudaFree(c->rc_root); cudaFree(c->rc_id);
+  c->rc_nodes = nullptr; c->rc_tri = nullptr; c->rc_root = nullptr; c->rc_id = nullptr;
+  TS_CUDA(c, cudaMalloc((void**)&c->rc_nodes, sizeof(float4) * nodes.size()));
+  TS_CUDA(c, cudaMalloc((void**)&c->rc_tri, sizeof(float4) * tris.size()));
+  TS_CUDA(c, cudaMalloc((void**)&c->rc_root, sizeof(int32_t) * G));
+  TS_CUDA(c, cudaMalloc((void**)&c->rc_id, sizeof(int32_t) * EK));
+  TS_CUDA(c, cudaMemcpyAsync(c->rc_nodes, nodes.data(), sizeof(float4) * nodes.size(), cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaMemcpyAsync(c->rc_tri, tris.data(), sizeof(float4) * tris.size(), cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaMemcpyAsync(c->rc_root, roots.data(), sizeof(int32_t) * G, cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaMemcpyAsync(c->rc_id, m->mesh_id, sizeof(int32_t) * EK, cudaMemcpyHostToDevice, st));
+  TS_CUDA(c, cudaStreamSynchronize(st));
+  c->have_mesh = true;
+  return TS_OK;
+}
+
 ts_status ts_set_pointclouds(ts_ctx* c, const ts_pointclouds* pc, void* stream) {
   if (!c) return TS_ERR_INVALID_ARG;
   if (!pc || !pc->points || !pc->cloud_id || pc->n_clouds < 1 || pc->n_points < 1)
@@ -635,6 +728,7 @@ ts_status ts_set_pointclouds(ts_ctx* c, const ts_pointclouds* pc, void* stream) 
   cudaStream_t st = (cudaStream_t)stream;
   c->have_pc = false;
   TS_CUDA(c, cudaStreamSynchronize(st));   // steps in flight may still read the old index
+  cudaFree(c->rc_nodes); cudaFree(c->rc_tri); cudaFree(c->rc_root); cudaFree(c->rc_id);
   cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw);
   cudaFree(c->pc_pts); cudaFree(c->pc_cell); cudaFree(c->pc_grid); cudaFree(c->pc_id);
   c->pc_pts = nullptr; c->pc_cell = nullptr; c->pc_grid = nullptr; c->pc_id = nullptr;
@@ -672,9 +766,9 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
       !in->obj_linvel || !in->obj_angvel)
     return fail(c, TS_ERR_INVALID_ARG, "ts_step: NULL input pointer");
   {  // output_mask contract (ts.h): bit set <=> pointer given
-    const void* ptr[11] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead,
-                           out->depth_noisy, out->prox_noisy, out->marker_noisy, out->proxpc};
-    for (int b = 0; b < 11; ++b) {
+    const void* ptr[13] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead,
+                           out->depth_noisy, out->prox_noisy, out->marker_noisy, out->proxpc, out->depth_rc, out->nrm_rc};
+    for (int b = 0; b < 13; ++b) {
       const bool want = (c->cfg.output_mask >> b) & 1u;
       if (want && !ptr[b]) return fail(c, TS_ERR_INVALID_ARG, "ts_step: an output declared in output_mask is NULL");
       if (!want && ptr[b]) return fail(c, TS_ERR_INVALID_ARG, "ts_step: an output not declared in output_mask is non-NULL");
@@ -694,6 +788,8 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
   p.contact = out->contact; p.depth = out->depth; p.ft = out->ft; p.marker = out->marker; p.prox = out->prox;
   p.ft_noisy = out->ft_noisy; p.dead = out->dead;
   p.depth_noisy = out->depth_noisy; p.prox_noisy = out->prox_noisy; p.marker_noisy = out->marker_noisy;
+  p.depth_rc = out->depth_rc; p.nrm_rc = out->nrm_rc;
+  if ((p.depth_rc || p.nrm_rc) && !c->have_mesh) return fail(c, TS_ERR_STATE, "ts_step: raycast outputs requested before ts_set_meshes");
   p.proxpc = out->proxpc;
   if (p.proxpc && !c->have_pc) return fail(c, TS_ERR_STATE, "ts_step: proxpc requested before ts_set_pointclouds");
   const bool scalar_noisy = p.depth_noisy || p.prox_noisy || p.marker_noisy;
@@ -725,6 +821,10 @@ ts_status ts_step(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, void*
     e = (cudaError_t)ts_launch_shear(p, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: shear launch");
   }
+  if (p.depth_rc || p.nrm_rc) {
+    e = (cudaError_t)ts_launch_raycast(p, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: raycast launch");
+  }
   if (p.proxpc) {
     e = (cudaError_t)ts_launch_proxpc(p, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "ts_step: proxpc launch");
@@ -747,16 +847,16 @@ ts_status ts_step_host(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, 
   const float* hin[8] = {in->link_pos, in->link_quat, in->link_linvel, in->link_angvel,
                          in->obj_pos, in->obj_quat, in->obj_linvel, in->obj_angvel};
   const size_t in_bytes[8] = {E * L * 12, E * L * 16, E * L * 12, E * L * 12, E * K * 12, E * K * 16, E * K * 12, E * K * 12};
-  void* hout[11] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead,
-                    out->depth_noisy, out->prox_noisy, out->marker_noisy, out->proxpc};
-  const size_t out_bytes[11] = {E * T, E * T * 4, E * T * 24, E * (size_t)c->M * 12, E * T * 4, E * T * 24, E * T,
-                                E * T * 4, E * T * 4, E * (size_t)c->M * 12, E * T * 24};
+  void* hout[13] = {out->contact, out->depth, out->ft, out->marker, out->prox, out->ft_noisy, out->dead,
+                    out->depth_noisy, out->prox_noisy, out->marker_noisy, out->proxpc, out->depth_rc, out->nrm_rc};
+  const size_t out_bytes[13] = {E * T, E * T * 4, E * T * 24, E * (size_t)c->M * 12, E * T * 4, E * T * 24, E * T,
+                                E * T * 4, E * T * 4, E * (size_t)c->M * 12, E * T * 24, E * T * 4, E * T * 12};
   for (int i = 0; i < 8; ++i) {
     if (!hin[i]) return fail(c, TS_ERR_INVALID_ARG, "ts_step_host: NULL input pointer");
     if (!c->stage_in[i]) TS_CUDA(c, cudaMalloc((void**)&c->stage_in[i], in_bytes[i]));
     TS_CUDA(c, cudaMemcpyAsync(c->stage_in[i], hin[i], in_bytes[i], cudaMemcpyHostToDevice, st));
   }
-  for (int i = 0; i < 11; ++i)
+  for (int i = 0; i < 13; ++i)
     if (hout[i] && !c->stage_out[i]) TS_CUDA(c, cudaMalloc(&c->stage_out[i], out_bytes[i] ? out_bytes[i] : 16));
   ts_step_in din = {c->stage_in[0], c->stage_in[1], c->stage_in[2], c->stage_in[3],
                     c->stage_in[4], c->stage_in[5], c->stage_in[6], c->stage_in[7]};
@@ -765,10 +865,11 @@ ts_status ts_step_host(ts_ctx* c, const ts_step_in* in, const ts_step_out* out, 
                       hout[4] ? (float*)c->stage_out[4] : nullptr,   hout[5] ? (float*)c->stage_out[5] : nullptr,
                       hout[6] ? (uint8_t*)c->stage_out[6] : nullptr, hout[7] ? (float*)c->stage_out[7] : nullptr,
                       hout[8] ? (float*)c->stage_out[8] : nullptr,   hout[9] ? (float*)c->stage_out[9] : nullptr,
-                      hout[10] ? (float*)c->stage_out[10] : nullptr};
+                      hout[10] ? (float*)c->stage_out[10] : nullptr, hout[11] ? (float*)c->stage_out[11] : nullptr,
+                      hout[12] ? (float*)c->stage_out[12] : nullptr};
   const ts_status s = ts_step(c, &din, &dout, stream);
   if (s != TS_OK) return s;
-  for (int i = 0; i < 11; ++i)
+  for (int i = 0; i < 13; ++i)
     if (hout[i]) TS_CUDA(c, cudaMemcpyAsync(hout[i], c->stage_out[i], out_bytes[i], cudaMemcpyDeviceToHost, st));
   return TS_OK;
 }

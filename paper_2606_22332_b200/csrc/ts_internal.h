@@ -139,6 +139,13 @@ struct TsStepParams {
   const int32_t* pc_id;       // [E,K] cloud of each object, -1 = none
   int32_t pc_n;               // points per cloud
   float pc_radius, pc_k, pc_ks, pc_density;
+  // raycast depth backend (A.1): BVH nodes and leaf-ordered triangles of every mesh
+  float* depth_rc;            // [E,T]
+  float* nrm_rc;              // [E,T,3]
+  const float4* rc_nodes;     // 2 float4 per node: (lo.xyz, first triangle | left child), (hi.xyz, count > 0 | -right child)
+  const float4* rc_tri;       // 3 float4 per triangle (vertices a, b, c), in leaf order
+  const int32_t* rc_root;     // [G] root node of each mesh
+  const int32_t* rc_id;       // [E,K] mesh of each object, -1 = none
   // elastomer shear history (Eq. 22): anchors per (env, patch, object, tracked point)
   uint8_t* sh_on;             // [E,P,K,N] anchored?
   float4* sh_e;               // [E,P,K,N] anchor relative to the pad centre (link frame); only read where sh_on is set
@@ -188,6 +195,7 @@ int ts_launch_frames(const TsStepParams& p, void* stream);
 int ts_launch_scalar_noise(const TsStepParams& p, void* stream);
 int ts_launch_proxpc(const TsStepParams& p, void* stream);
 int ts_launch_shear(const TsStepParams& p, void* stream);
+int ts_launch_raycast(const TsStepParams& p, void* stream);
 int ts_launch_reset_shear(const TsStepParams& p, const uint8_t* mask, void* stream);
 int ts_launch_reset_scalar(const TsStepParams& p, const uint8_t* mask, void* stream);
 unsigned long long ts_frame_bytes();

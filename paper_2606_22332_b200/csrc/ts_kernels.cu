@@ -1607,6 +1607,118 @@ __global__ void ts_reset_shear_kernel(const __grid_constant__ TsStepParams p, co
   p.sh_on[gt] = 0;
 }
 
+// ---------------------------------------------------------------------------------------
+// App. A.1 raycast contact-depth backend (reading Q28).  One thread per (env, taxel): the probe centre and
+// normal go into the object frame (double), the mesh's bounding volume hierarchy is walked with a private stack
+// (a node is entered when its box meets the probe sphere; the ray segment of length R_j lies inside that sphere), and
+// every triangle of a reached leaf takes the sphere-triangle closest-point test (penetration R_j - dist) and the
+// ray-triangle test from the centre along -a_j (penetration R_j - hit distance).  The deepest wins; its face normal
+// is reported in the sensor-link frame.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ F3 sub3(F3 a, F3 b) { return mk3(a.x - b.x, a.y - b.y, a.z - b.z); }
+__device__ __forceinline__ F3 cross3(F3 a, F3 b) { return mk3(a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x); }
+
+// closest point of triangle (a, b, c) to p (Voronoi-region walk; Ericson 5.1.5 restated in fp32)
+__device__ __forceinline__ F3 closest_pt_tri(F3 p, F3 a, F3 b, F3 c) {
+  const F3 ab = sub3(b, a), ac = sub3(c, a), ap = sub3(p, a);
+  const float d1 = dot(ab, ap), d2 = dot(ac, ap);
+  if (d1 <= 0.f && d2 <= 0.f) return a;
+  const F3 bp = sub3(p, b);
+  const float d3 = dot(ab, bp), d4 = dot(ac, bp);
+  if (d3 >= 0.f && d4 <= d3) return b;
+  const float vc = d1 * d4 - d3 * d2;
+  if (vc <= 0.f && d1 >= 0.f && d3 <= 0.f) return a + (d1 / (d1 - d3)) * ab;
+  const F3 cp = sub3(p, c);
+  const float d5 = dot(ab, cp), d6 = dot(ac, cp);
+  if (d6 >= 0.f && d5 <= d6) return c;
+  const float vb = d5 * d2 - d1 * d6;
+  if (vb <= 0.f && d2 >= 0.f && d6 <= 0.f) return a + (d2 / (d2 - d6)) * ac;
+  const float va = d3 * d6 - d5 * d4;
+  if (va <= 0.f && (d4 - d3) >= 0.f && (d5 - d6) >= 0.f) return b + ((d4 - d3) / ((d4 - d3) + (d5 - d6))) * sub3(c, b);
+  const float den = 1.f / (va + vb + vc);
+  return a + (vb * den) * ab + (vc * den) * ac;
+}
+
+// ray (o, unit d) against (a, b, c), both faces (Moeller-Trumbore restated): hit distance >= 0 or -1
+__device__ __forceinline__ float ray_tri(F3 o, F3 d, F3 a, F3 b, F3 c) {
+  const F3 e1 = sub3(b, a), e2 = sub3(c, a), pv = cross3(d, e2);
+  const float det = dot(e1, pv);
+  if (fabsf(det) < 1e-30f) return -1.f;
+  const float inv = 1.f / det;
+  const F3 tv = sub3(o, a);
+  const float u = dot(tv, pv) * inv;
+  if (u < 0.f || u > 1.f) return -1.f;
+  const F3 qv = cross3(tv, e1);
+  const float v = dot(d, qv) * inv;
+  if (v < 0.f || u + v > 1.f) return -1.f;
+  const float t = dot(e2, qv) * inv;
+  return t >= 0.f ? t : -1.f;
+}
+
+__global__ void __launch_bounds__(128) ts_raycast_kernel(const __grid_constant__ TsStepParams p) {
+  const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gt >= (long long)p.E * p.T) return;
+  const int e = (int)(gt / p.T), j = (int)(gt - (long long)e * p.T);
+  const float4 P4 = __ldg(p.tx_pos + j);
+  float best = 0.f;
+  D3 bn = D3{0.0, 0.0, 0.0};
+  if (P4.w > 0.f) {
+    const TsPatch& pt = p.patches[__ldg(p.tx_patch + j)];
+    const int link = __ldg(&pt.link);
+    const float4 na = __ldg(&pt.na);
+    const size_t el = (size_t)e * p.L + link;
+    double RL[9];
+    quat_Rd(p.link_quat + el * 4, RL);
+    const D3 q = ld3d(p.link_pos + el * 3) + mulR(RL, D3{(double)P4.x, (double)P4.y, (double)P4.z});   // Eq. 1
+    const D3 a = mulR(RL, D3{(double)na.x, (double)na.y, (double)na.z});
+    const float R = P4.w, R2 = R * R;
+    for (int k = 0; k < p.K; ++k) {
+      const int id = __ldg(p.rc_id + (size_t)e * p.K + k);
+      if (id < 0) continue;
+      const size_t ek = (size_t)e * p.K + k;
+      double RO[9];
+      quat_Rd(p.obj_quat + ek * 4, RO);
+      const D3 qd = mulRT(RO, q - ld3d(p.obj_pos + ek * 3)), ad = mulRT(RO, a);
+      const F3 qo = mk3((float)qd.x, (float)qd.y, (float)qd.z), nd = mk3(-(float)ad.x, -(float)ad.y, -(float)ad.z);
+      int stack[48];
+      int sp = 0;
+      stack[sp++] = __ldg(p.rc_root + id);
+      F3 wn = mk3(0.f, 0.f, 0.f);
+      bool won = false;
+      while (sp > 0) {
+        const int node = stack[--sp];
+        const float4 n0 = __ldg(p.rc_nodes + 2 * node), n1 = __ldg(p.rc_nodes + 2 * node + 1);
+        const float dx = fmaxf(fmaxf(n0.x - qo.x, qo.x - n1.x), 0.f), dy = fmaxf(fmaxf(n0.y - qo.y, qo.y - n1.y), 0.f),
+                    dz = fmaxf(fmaxf(n0.z - qo.z, qo.z - n1.z), 0.f);
+        if (fmaf(dx, dx, fmaf(dy, dy, dz * dz)) >= R2) continue;           // the box misses the probe sphere
+        const int cnt = __float_as_int(n1.w);
+        if (cnt > 0) {
+          const int first = __float_as_int(n0.w);
+          for (int f = first; f < first + cnt; ++f) {
+            const float4 A4 = __ldg(p.rc_tri + 3 * f), B4 = __ldg(p.rc_tri + 3 * f + 1), C4 = __ldg(p.rc_tri + 3 * f + 2);
+            const F3 A = mk3(A4.x, A4.y, A4.z), B = mk3(B4.x, B4.y, B4.z), C3 = mk3(C4.x, C4.y, C4.z);
+            const F3 dcp = sub3(qo, closest_pt_tri(qo, A, B, C3));
+            const float d2 = dot(dcp, dcp);
+            float pen = d2 < R2 ? R - sqrtf(d2) : 0.f;
+            const float th = ray_tri(qo, nd, A, B, C3);
+            if (th >= 0.f && th < R) pen = fmaxf(pen, R - th);
+            if (pen > best) { best = pen; wn = cross3(sub3(B, A), sub3(C3, A)); won = true; }
+          }
+        } else if (sp + 2 <= 48) {
+          stack[sp++] = __float_as_int(n0.w);        // inner node: left child, and the right child stored negated
+          stack[sp++] = -__float_as_int(n1.w);       // (count > 0 marks a leaf; child indices are >= 1)
+        }
+      }
+      if (won) {  // face normal of the winner of THIS object, object frame -> link frame
+        const double nl = sqrt((double)wn.x * wn.x + (double)wn.y * wn.y + (double)wn.z * wn.z);
+        if (nl > 0.0) bn = mulRT(RL, mulR(RO, D3{wn.x / nl, wn.y / nl, wn.z / nl}));
+      }
+    }
+  }
+  if (p.depth_rc) __stcs(p.depth_rc + gt, best);
+  if (p.nrm_rc) { __stcs(p.nrm_rc + gt * 3, (float)bn.x); __stcs(p.nrm_rc + gt * 3 + 1, (float)bn.y); __stcs(p.nrm_rc + gt * 3 + 2, (float)bn.z); }
+}
+
 }  // namespace
 
 unsigned long long ts_bank_elems_per_grid(int N) { return (unsigned long long)(N - 1) * (N - 1) * N; }
@@ -1700,6 +1812,12 @@ int ts_launch_shear(const TsStepParams& p, void* stream) {
 int ts_launch_reset_shear(const TsStepParams& p, const uint8_t* mask, void* stream) {
   const size_t n = (size_t)p.E * p.P * p.K * p.pc_n;
   ts_reset_shear_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(p, mask);
+  return (int)cudaGetLastError();
+}
+
+int ts_launch_raycast(const TsStepParams& p, void* stream) {
+  const long long n = (long long)p.E * p.T;
+  ts_raycast_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(p);
   return (int)cudaGetLastError();
 }
 

@@ -32,7 +32,7 @@ def test_library_exports_every_declared_symbol(B):
 def test_struct_sizes_match_header(B):
     # ts_patch_desc: 1+3+3+3+2 floats/ints + 2 + 1 + 2 = 17 x 4 bytes; ts_step_in 8 ptrs; ts_step_out 7 ptrs
     assert C.sizeof(B.PatchDesc) == 17 * 4
-    assert C.sizeof(B.StepIn) == 8 * 8 and C.sizeof(B.StepOut) == 11 * 8
+    assert C.sizeof(B.StepIn) == 8 * 8 and C.sizeof(B.StepOut) == 13 * 8
     cfg = B.Config()
     B.lib().ts_config_default(C.byref(cfg))
     assert (cfg.k_n, cfg.c_n, cfg.k_t, cfg.k_omega) == (500.0, 1.0, 2.0, 2.0)          # Eq. 10

@@ -508,3 +508,47 @@ def test_elastomer_shear_history():
     _assert_ok(rep)
     assert rep["max_ratio"]["marker"] <= 1.0 and moved > 5000, (rep["max_ratio"], moved)    # the shear term really acts
     sim.close(); plain.close()
+
+
+def test_raycast_depth_backend():
+    """the raycast contact-depth backend (App. A.1) on triangle meshes: BVH walk on the GPU against
+    the oracle's brute force over every triangle.  Config-5 scene with 1,280-triangle star meshes; depth element-wise,
+    the face normal wherever the winning triangle is unique (margin to the best triangle with another normal > 1e-6 m;
+    two triangles sharing the closest edge tie exactly and either normal is valid)."""
+    import torch
+    from oracle import oracle as O
+    from paper_2606_22332_b200.binding import TactileSim
+    from parity import ATOL, RTOL
+    w = W.config(5, n_envs=32)
+    meshes, mid = W.mesh_bank(w, 3)
+    outs = ("depth", "depth_rc", "nrm_rc")
+    sim = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=w.physics, outputs=outs)
+    sim.set_geometry(w.types, w.params, w.bank, w.voxel)
+    sim.set_meshes(meshes, mid)
+    orc = O.Oracle(w.patches, w.T, w.L, w.K, np.arange(w.E), physics=w.physics, threads=os.cpu_count() or 1)
+    orc.set_geometry(w.types, w.params, w.bank, w.voxel)
+    orc.set_meshes(meshes, mid)
+    n_touch = n_nrm = 0
+    for s in (0, 11):
+        inp = w.inputs(s)
+        g = sim.step(sim.upload(inp))
+        torch.cuda.synchronize()
+        r = orc.step(inp, want=outs, aux=False)
+        gd, gn = g["depth_rc"].cpu().numpy().astype(np.float64), g["nrm_rc"].cpu().numpy().astype(np.float64)
+        ratio = np.abs(gd - r["depth_rc"]) / (ATOL + RTOL * np.abs(r["depth_rc"]))
+        assert ratio.max() <= 1.0, ratio.max()
+        unique = (r["depth_rc"] > 2e-6) & (r["aux_rc_gap"] > 2e-6)
+        assert np.abs(gn[unique] - r["nrm_rc"][unique]).max() < 2e-5
+        touch = r["depth_rc"] > 0
+        # where the normal is not unique it must still be a unit vector (some triangle's face normal)
+        assert np.abs(np.linalg.norm(gn[gd > 0], axis=-1) - 1).max() < 1e-5 and not gn[gd == 0].any()
+        assert not gd[mid[:, 0] < 0].any()
+        n_touch += int(touch.sum()); n_nrm += int(unique.sum())
+        # the two backends agree to the mesh's chord error where the probe centre is outside (P:188 "equivalent depths
+        # to leading order for smooth meshes")
+        sdf = g["depth"].cpu().numpy()
+        both = touch & (sdf > 0) & (sdf < 1.5e-3)
+        assert np.abs(gd[both] - sdf[both]).max() < 4e-4
+    print(json.dumps({"raycast_touching": n_touch, "normals_checked": n_nrm}))
+    assert n_touch > 3000 and n_nrm > 0.8 * n_touch
+    sim.close()
