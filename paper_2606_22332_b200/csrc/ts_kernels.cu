@@ -565,7 +565,7 @@ __device__ __forceinline__ void noise_prefetch(const TsStepParams& p, int e, int
 }
 
 // Every thread of the block must call this (it contains one __syncthreads).
-template <int HM>
+template <int HM, bool FAST = false>
 __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, unsigned ej, int tid, int patch0, bool valid,
                                             bool act, bool deadb, int meta, const float* ft, const NoiseState& ns,
                                             float* bufB) {
@@ -763,7 +763,7 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
 #pragma unroll
     for (int c = 0; c < 3; ++c) __stcs(st_d + (id + c * Tp), make_float2(Dn[2 * c], Dn[2 * c + 1]));
   }
-  if (p.ft_noisy && valid) store6(p.ft_noisy + ej * 6u, outv);
+  if ((FAST || p.ft_noisy) && valid) store6(p.ft_noisy + ej * 6u, outv);
   if (ring_on) {
 #pragma unroll
     for (int c = 0; c < 3; ++c) __stcs(reinterpret_cast<float2*>(p.st_ring) + (iw + c * Tp), ringw[c]);
@@ -796,13 +796,13 @@ __global__ void __launch_bounds__(TS_BLOCK, 6) ts_noise_kernel(const __grid_cons
   if (p.clock && tid == 0) atomicMax(p.clock + 1, globaltimer_ns());   // device-side clock: the split form ends the step here
 }
 
-template <bool SINGLE>
+template <bool SINGLE, bool FAST = false>
 __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS* frames, int e, int lp, bool valid, bool act,
                                             unsigned ej, float phif, F3 xo, float4 P4, int pidx) {
 // ---- phase 2 (S7): proximity march, t <- min(t + max(phi(q + t a), 0), r_prox), K_m evaluations.
   // Exact shortcuts (O7): evaluation 0 is the query above; t = r_prox is absorbing; an evaluation
   // that leaves t unchanged repeats forever.
-  if (p.prox) {
+  if (FAST || p.prox) {
     float t = 0.f;
     int go = 0;  // int, not bool: a bool that lives across the loop is packed into a byte and costs PRMTs
     if (act && p.march_steps > 0) {
@@ -903,7 +903,11 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
   }
 }
 
-template <bool SINGLE, int HM>  // HM = TS_HYST_* of the fused noise chain, -1 = no noise chain in this kernel
+// HM = TS_HYST_* of the fused noise chain, -1 = no noise chain in this kernel.  FAST = the common full configuration
+// fixed at compile time: every output pointer given, group records in the parameter space, env order table present,
+// DMMA marker path.  The generic variant tests each of these per block (a 64-bit pointer test per output, both group
+// record paths issued under predicates): ~35 issue slots per warp that FAST does not spend.
+template <bool SINGLE, int HM, bool FAST = false>
 __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const __grid_constant__ TsStepParams p) {
   constexpr bool NOISE = HM >= 0;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -925,9 +929,9 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const unsigned bxi = blockIdx.x;
   const int gi = blockIdx.y;
 #endif
-  const int e = p.env_perm ? __ldg(p.env_perm + bxi) : (int)bxi;
+  const int e = (FAST || p.env_perm) ? __ldg(p.env_perm + bxi) : (int)bxi;
   int gstart, gcount, patch0, npatch, chunk0, nchunk, gmcount;
-  if (p.inl) {  // group record from the parameter space (constant bank)
+  if (FAST || p.inl) {  // group record from the parameter space (constant bank)
     const TsGroup& g = p.inl_grp[gi];
     gstart = g.start; gcount = g.count; patch0 = g.patch0; npatch = g.npatch; chunk0 = g.chunk0; nchunk = g.nchunk; gmcount = g.mcount;
   } else {
@@ -989,11 +993,11 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const bool deadb = p.noise_enable && act && ((flag >> 1) & 1);
   if (valid) {
     p.st_flags[ej] = (uint8_t)((flag & 2) | (yb ? 1 : 0));  // Schmitt state from the un-masked bit (O4)
-    if (p.contact) p.contact[ej] = (yb && !deadb) ? 1 : 0;
-    if (p.dead) p.dead[ej] = deadb ? 1 : 0;
-    if (p.depth) __stcs(p.depth + ej, d);
+    if (FAST || p.contact) p.contact[ej] = (yb && !deadb) ? 1 : 0;
+    if (FAST || p.dead) p.dead[ej] = deadb ? 1 : 0;
+    if (FAST || p.depth) __stcs(p.depth + ej, d);
   }
-  if (p.marker) {  // Eq. 19: h_i = max(0, -phi), no R_j
+  if (FAST || p.marker) {  // Eq. 19: h_i = max(0, -phi), no R_j
     const float h = (act && phid < 0.0) ? (float)(-phid) : 0.f;
     hh[tid] = h;
     ha[tid] = h > 0.f ? __powf(h, p.alpha_e) : 0.f;
@@ -1002,7 +1006,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   }
   const F3 xo = mk3((float)xd.x, (float)xd.y, (float)xd.z);  // fp32 object-frame position for the march
 
-  march_phase<SINGLE>(p, frames, e, lp, valid, act, ej, phif, xo, P4, patch0 + lp);
+  march_phase<SINGLE, FAST>(p, frames, e, lp, valid, act, ej, phif, xo, P4, patch0 + lp);
 
   // ---- phase 3 (S5): kinematic force / torque (Eq. 4-9, D2) in double, link frame ---------------
   // Eq. 26 (R8): the noisy readout senses with R~_j = max(0, R_j + eps_j), eps_j ~ U[-rho, rho] drawn once per
@@ -1022,7 +1026,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   float ft[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   float fn6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};  // Eq. 4-9 at depth dn (dead code unless rn_on)
   const bool touch = d > 0.f || (rn_on && dn > 0.f);
-  if ((p.ft != nullptr || NOISE || rn_on) && __any_sync(TS_FULL, touch)) {
+  if ((FAST || p.ft != nullptr || NOISE || rn_on) && __any_sync(TS_FULL, touch)) {
     if (touch) {  // Q5: every term gated on d > 0
       const FrameS& F = frames[lp * (SINGLE ? 1 : p.K) + kst];
       const D3 g = grad_d(p, F.type, F.prm, xd);
@@ -1089,7 +1093,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
       }
     }
   }
-  if (p.ft && valid) store6(p.ft + ej * 6u, ft);
+  if ((FAST || p.ft) && valid) store6(p.ft + ej * 6u, ft);
   if (rn_on) {  // from here on only the Eq. 26 readout is needed
 #pragma unroll
     for (int c = 0; c < 6; ++c) ft[c] = fn6[c];
@@ -1099,7 +1103,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   // ---- phase 4 (S8): noise chain (fused variant); contains the barrier that also publishes hh / ha / pact
   NoiseState ns;
   if (NOISE) noise_load<HM>(p, e, j, valid, ns);
-  if (NOISE) noise_chain<HM>(p, e, j, ej, tid, patch0, valid, act, deadb, meta, ft, ns, bufB);
+  if (NOISE) noise_chain<HM, FAST>(p, e, j, ej, tid, patch0, valid, act, deadb, meta, ft, ns, bufB);
   else __syncthreads();
 
   // ---- phase 5 (S6): elastomer marker dilation (Eq. 18-21, 23 first sum) ----------------------
@@ -1108,7 +1112,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   //   pass 1 over (a,q): S0 = sum_p gu h, S1 = sum_p du gu h, T0 = sum_p gu h^alpha_e
   //   pass 2 over (a,b): Uu = sum_q gv S1, Uv = sum_q dv gv S0, Un = sum_q gv T0.
   // Sources with h_i = 0 contribute exactly 0; patches without penetration are skipped.
-  if (p.marker && gmcount > 0 && p.mk_mma) {
+  if ((FAST || (p.marker && p.mk_mma)) && gmcount > 0) {
     // DMMA path (every patch fits 8 x 8 tiles): ONE WARP PER PATCH evaluates both passes as FP64 tensor-core products
     // (mma.m8n8k4, SASS DMMA.8x8x4) on zero-padded 8 x 8 tables; lane = 4 g + m holds A[row g][k m], B[k m][col g]
     // and C[row g][cols 2m, 2m+1].
@@ -1162,7 +1166,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
         }
       }
     }
-  } else if (p.marker && gmcount > 0) {
+  } else if (!FAST && p.marker && gmcount > 0) {
     // hh / ha / pact were completed by the barrier above; this one retires the crosstalk reads of bufB (= S)
     if (NOISE) __syncthreads();
     for (int ch = 0; ch < nchunk; ++ch) {
@@ -1729,14 +1733,14 @@ unsigned long long ts_step_smem_bytes(const TsStepParams& p) {
 }
 
 namespace {
-template <bool SINGLE, int HM>
+template <bool SINGLE, int HM, bool FAST = false>
 cudaError_t prep_one(int smem) {
-  cudaError_t e = cudaFuncSetAttribute(ts_step_kernel<SINGLE, HM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  cudaError_t e = cudaFuncSetAttribute(ts_step_kernel<SINGLE, HM, FAST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   // Ask for no more shared memory than TS_MIN_BLOCKS resident blocks need (+1 KB reserved per block): the
   // rest of the 228 KB stays L1, which serves the SDF gathers (measured: 1.51 -> 1.48 ms on config 5).
   const int carve = (int)((TS_MIN_BLOCKS * (smem + 1024LL) * 100 + 228 * 1024 - 1) / (228 * 1024)) + 2;
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(ts_step_kernel<SINGLE, HM>, cudaFuncAttributePreferredSharedMemoryCarveout, carve > 100 ? 100 : carve);
+    e = cudaFuncSetAttribute(ts_step_kernel<SINGLE, HM, FAST>, cudaFuncAttributePreferredSharedMemoryCarveout, carve > 100 ? 100 : carve);
   return e;
 }
 template <bool SINGLE>
@@ -1764,6 +1768,8 @@ int ts_prepare_kernels(int device, int smem_bytes) {
   if (smem_bytes <= max_smem[d]) return 0;
   const int max_smem_bytes = smem_bytes;
   cudaError_t e = prep_one<true, -1>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, TS_HYST_MAXWELL, true>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, TS_HYST_ASYM, true>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_OFF>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_MAXWELL>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_ASYM>(max_smem_bytes);
@@ -1791,7 +1797,12 @@ int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
   const dim3 grid((unsigned)p.E, (unsigned)p.G);
 #endif
   const int hm = (p.noise_enable && fused_noise) ? (p.hyst_mode | (p.ext ? 4 : 0)) : -1;
-  if (p.K == 1) launch_one<true>(p, hm, grid, smem, (cudaStream_t)stream);
+  // the common full configuration has its own compile-time-specialised variants (see ts_step_kernel)
+  const bool fast = p.K == 1 && p.inl && p.env_perm && p.mk_mma && p.contact && p.depth && p.ft && p.marker && p.prox &&
+                    p.ft_noisy && p.dead && (hm == TS_HYST_ASYM || hm == TS_HYST_MAXWELL);
+  if (fast && hm == TS_HYST_ASYM) ts_step_kernel<true, TS_HYST_ASYM, true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
+  else if (fast) ts_step_kernel<true, TS_HYST_MAXWELL, true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
+  else if (p.K == 1) launch_one<true>(p, hm, grid, smem, (cudaStream_t)stream);
   else launch_one<false>(p, hm, grid, smem, (cudaStream_t)stream);
   return (int)cudaGetLastError();
 }
