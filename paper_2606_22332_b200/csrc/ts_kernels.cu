@@ -923,8 +923,10 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
 
   const int tid = threadIdx.x;
 #if TS_GRID_GFAST
-  const unsigned bxi = blockIdx.x / (unsigned)p.G;
-  const int gi = (int)(blockIdx.x - bxi * (unsigned)p.G);
+  // grid (G, min(E, 65535), ceil(E / 65535)): the group index runs fastest, and no integer division is needed
+  const unsigned bxi = blockIdx.z * 65535u + blockIdx.y;
+  const int gi = (int)blockIdx.x;
+  if (bxi >= (unsigned)p.E) return;
 #else
   const unsigned bxi = blockIdx.x;
   const int gi = blockIdx.y;
@@ -1792,7 +1794,7 @@ int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
   if (p.E <= 0 || p.G <= 0 || p.G > 65535) return (int)cudaErrorInvalidConfiguration;
   const size_t smem = (size_t)ts_step_smem_bytes(p);
 #if TS_GRID_GFAST
-  const dim3 grid((unsigned)p.E * (unsigned)p.G, 1u);
+  const dim3 grid((unsigned)p.G, (unsigned)(p.E < 65535 ? p.E : 65535), (unsigned)((p.E + 65534) / 65535));
 #else
   const dim3 grid((unsigned)p.E, (unsigned)p.G);
 #endif
