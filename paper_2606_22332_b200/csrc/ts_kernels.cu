@@ -996,7 +996,7 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   if (valid) {
     p.st_flags[ej] = (uint8_t)((flag & 2) | (yb ? 1 : 0));  // Schmitt state from the un-masked bit (O4)
     if (FAST || p.contact) p.contact[ej] = (yb && !deadb) ? 1 : 0;
-    if (FAST || p.dead) p.dead[ej] = deadb ? 1 : 0;
+    if ((FAST && NOISE) || p.dead) p.dead[ej] = deadb ? 1 : 0;
     if (FAST || p.depth) __stcs(p.depth + ej, d);
   }
   if (FAST || p.marker) {  // Eq. 19: h_i = max(0, -phi), no R_j
@@ -1770,6 +1770,7 @@ int ts_prepare_kernels(int device, int smem_bytes) {
   if (smem_bytes <= max_smem[d]) return 0;
   const int max_smem_bytes = smem_bytes;
   cudaError_t e = prep_one<true, -1>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, -1, true>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_MAXWELL, true>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_ASYM, true>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_OFF>(max_smem_bytes);
@@ -1800,9 +1801,11 @@ int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
 #endif
   const int hm = (p.noise_enable && fused_noise) ? (p.hyst_mode | (p.ext ? 4 : 0)) : -1;
   // the common full configuration has its own compile-time-specialised variants (see ts_step_kernel)
-  const bool fast = p.K == 1 && p.inl && p.env_perm && p.mk_mma && p.contact && p.depth && p.ft && p.marker && p.prox &&
-                    p.ft_noisy && p.dead && (hm == TS_HYST_ASYM || hm == TS_HYST_MAXWELL);
-  if (fast && hm == TS_HYST_ASYM) ts_step_kernel<true, TS_HYST_ASYM, true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
+  const bool clean5 = p.K == 1 && p.inl && p.env_perm && p.mk_mma && p.contact && p.depth && p.ft && p.marker && p.prox;
+  const bool fast = clean5 && p.ft_noisy && p.dead && (hm == TS_HYST_ASYM || hm == TS_HYST_MAXWELL);
+  if (clean5 && hm == -1 && !p.noise_enable && !p.dead && !p.depth_pert)
+    ts_step_kernel<true, -1, true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
+  else if (fast && hm == TS_HYST_ASYM) ts_step_kernel<true, TS_HYST_ASYM, true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
   else if (fast) ts_step_kernel<true, TS_HYST_MAXWELL, true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
   else if (p.K == 1) launch_one<true>(p, hm, grid, smem, (cudaStream_t)stream);
   else launch_one<false>(p, hm, grid, smem, (cudaStream_t)stream);
