@@ -145,6 +145,55 @@ def oracle_arm(w, ids, steps, warmup, threads):
     return len(ids) * w.T * steps / dt, 1e3 * dt / steps
 
 
+def time_extras(W, TactileSim, torch, dev, n_envs=4096, steps=20):
+    """Device time per step (CUDA events on the launch stream, mean of `steps` after 3 warm-up steps) of the SURVEY 8(f)
+    sensor kernels: a context that asks for the extra output next to `depth`, minus the same context without it.
+    Workload: config 4 (8 star objects, 1,000 taxels) at 4,096 envs; tracked clouds of 5,000 (proximity) / 1,000
+    (shear) surface points and 1,280-triangle meshes per object."""
+    w = W.config(4, n_envs=n_envs)
+    stream = torch.cuda.current_stream(dev)
+    inputs = None
+
+    def run(outs, physics=None, noise=None, setup=None):
+        nonlocal inputs
+        sim = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=physics or w.physics, noise=noise, outputs=outs)
+        sim.set_geometry(w.types, w.params, w.bank, w.voxel)
+        if setup:
+            setup(sim)
+        if inputs is None:
+            inputs = [sim.upload(w.inputs(s)) for s in range(8)]
+        out = sim.alloc_outputs()
+        for s in range(3):
+            sim.step(inputs[s % 8], out)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        e0.record(stream)
+        for s in range(steps):
+            sim.step(inputs[s % 8], out)
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        sim.close()
+        return e0.elapsed_time(e1) / steps
+
+    res = {"workload": "config4 noise: %d envs x %d taxels, %d markers" % (w.E, w.T, 980)}
+    base = run(("depth",))
+    base_m = run(("depth", "marker"))
+    pts5, cid = W.point_cloud_bank(w, 5000)
+    pts1, _ = W.point_cloud_bank(w, 1000)
+    meshes, mid = W.mesh_bank(w, 3)
+    res["base_depth_only_ms"] = base
+    res["proxpc_ms"] = run(("depth", "proxpc"), setup=lambda s: s.set_pointclouds(pts5, cid)) - base
+    res["raycast_ms"] = run(("depth", "depth_rc", "nrm_rc"), setup=lambda s: s.set_meshes(meshes, mid)) - base
+    res["shear_ms"] = run(("depth", "marker"), physics=dict(w.physics, shear_enable=1), setup=lambda s: s.set_pointclouds(pts1, cid)) - base_m
+    t12 = dict(w.noise, sigma_white_depth=2e-4, sigma_white_prox=1e-2, sigma_rw_prox=1e-3, quant_prox=1e-2, sigma_white_marker=1e-4,
+               sigma_rw_marker=1e-5, quant_marker=1e-4, gain_min=0.85, gain_max=1.15)
+    full = tuple(w.outputs)
+    res["scalar_noise_ms"] = run(full + ("depth_noisy", "prox_noisy", "marker_noisy"), noise=t12) - run(full, noise=t12)
+    n = float(w.E) * w.T
+    res["env_taxel_per_s"] = {k[:-3]: n / (v * 1e-3) for k, v in res.items() if k.endswith("_ms") and k != "base_depth_only_ms" and v > 0}
+    return res
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -156,6 +205,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="budget of the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--extras", action="store_true", help="also time the SURVEY 8(f) sensor kernels (noisy scalar readouts, "
+                    "point-cloud ProximityTaxel, shear history, raycast depth) on a 4,096-env config-4 scene; adds an "
+                    "`extras` object to the line")
     ap.add_argument("--noise-knobs", default="", help="profiling aid, not the headline workload: extra App. A.8 knobs "
                     "as k=v,k=v (e.g. bias_force=0.02,read_delay=2); named in config.workload")
     a = ap.parse_args()
@@ -332,6 +384,8 @@ def main():
                                           "(x%d envs/16 = %.0f ms per full step, linear extrapolation)"
                                           % (len(ids), ids.tolist(), T, n, ms, E, ms * E / len(ids)),
                                 "single_thread": {"value": v_st, "unit": UNIT, "cores": 1, "steps": n1, "ms_per_16env_step": ms_st}}
+    if a.extras and rank == 0 and world == 1:
+        line["extras"] = time_extras(W, TactileSim, torch, dev)
     if rank == 0:
         print(json.dumps(line))
     sim.close()
