@@ -1539,6 +1539,23 @@ __global__ void __launch_bounds__(256) ts_shear_kernel(const __grid_constant__ T
   const double hu = 0.5 * (double)ua.w, hv = 0.5 * (double)va.w;
   const int N = p.pc_n;
   float ax = 0.f, ay = 0.f, az = 0.f;   // this thread's marker (tid < mcount): shear sum
+  float mx = 0.f, my = 0.f, mz = 0.f;
+  if (tid < mcount) {
+    const float4 mp = __ldg(p.mk_pos + __ldg(&pt.mstart) + tid);
+    mx = mp.x - ctr.x; my = mp.y - ctr.y; mz = mp.z - ctr.z;
+  }
+  auto shear_drain = [&]() {             // phase C over the queued points (call between barriers)
+    const int nq = qn;
+    if (tid >= mcount) return;
+    for (int s2 = 0; s2 < nq; ++s2) {
+      const float4 d4 = qd[s2], z4 = qz[s2];
+      const float rx = mx - z4.x, ry = my - z4.y, rz = mz - z4.z;
+      const float rn = fmaf(rx, na.x, fmaf(ry, na.y, rz * na.z));
+      const float tx = fmaf(-rn, na.x, rx), ty = fmaf(-rn, na.y, ry), tz = fmaf(-rn, na.z, rz);   // Pi_n(x_j - z_p)
+      const float wgt = p.s_s * d4.w * expf(-p.lambda_s * fmaf(tx, tx, fmaf(ty, ty, tz * tz)));   // Eq. 22
+      ax = fmaf(wgt, d4.x, ax); ay = fmaf(wgt, d4.y, ay); az = fmaf(wgt, d4.z, az);
+    }
+  };
   for (int k = 0; k < p.K; ++k) {
     const int id = __ldg(p.pc_id + (size_t)e * p.K + k);   // block-uniform
     if (id < 0) continue;
@@ -1557,7 +1574,18 @@ __global__ void __launch_bounds__(256) ts_shear_kernel(const __grid_constant__ T
     }
     __syncthreads();
     const size_t sbase = (((size_t)e * p.P + pi) * p.K + k) * N;
-    for (int i = tid; i < N; i += 256) {
+    for (int i0 = 0; i0 < N; i0 += 256) {
+      if (i0) {                              // one pass queues at most 256 points: drain before the queue could overflow
+        __syncthreads();
+        if (qn > TS_SHEAR_Q - 256) {         // block-uniform
+          shear_drain();
+          __syncthreads();
+          if (tid == 0) qn = 0;
+          __syncthreads();
+        }
+      }
+      const int i = i0 + tid;
+      if (i >= N) continue;
       const float4 po = __ldg(p.pc_raw + (size_t)id * N + i);
       const D3 z = D3{tv[0], tv[1], tv[2]} + mulR(Rm, D3{(double)po.x, (double)po.y, (double)po.z});
       const D3 rel = z - xc;
@@ -1576,27 +1604,13 @@ __global__ void __launch_bounds__(256) ts_shear_kernel(const __grid_constant__ T
       if (on && phi_el < 0.0) {
         const D3 dz = D3{rel.x - (double)anc.x, rel.y - (double)anc.y, rel.z - (double)anc.z};
         const D3 dzt = dz - dot(dz, n) * n;                          // Pi_n(z_p - e_p)
-        const int slot = atomicAdd(&qn, 1);
-        if (slot < TS_SHEAR_Q) {
-          qd[slot] = make_float4((float)dzt.x, (float)dzt.y, (float)dzt.z, (float)(-phi_el));
-          qz[slot] = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
-        }
+        const int slot = atomicAdd(&qn, 1);                          // < TS_SHEAR_Q by the drain rule above
+        qd[slot] = make_float4((float)dzt.x, (float)dzt.y, (float)dzt.z, (float)(-phi_el));
+        qz[slot] = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
       }
     }
     __syncthreads();
-    const int nq = min(qn, TS_SHEAR_Q);
-    if (tid < mcount && nq > 0) {
-      const float4 mp = __ldg(p.mk_pos + __ldg(&pt.mstart) + tid);
-      const float mx = mp.x - ctr.x, my = mp.y - ctr.y, mz = mp.z - ctr.z;
-      for (int s2 = 0; s2 < nq; ++s2) {
-        const float4 d4 = qd[s2], z4 = qz[s2];
-        const float rx = mx - z4.x, ry = my - z4.y, rz = mz - z4.z;
-        const float rn = fmaf(rx, na.x, fmaf(ry, na.y, rz * na.z));
-        const float tx = fmaf(-rn, na.x, rx), ty = fmaf(-rn, na.y, ry), tz = fmaf(-rn, na.z, rz);   // Pi_n(x_j - z_p)
-        const float wgt = p.s_s * d4.w * expf(-p.lambda_s * fmaf(tx, tx, fmaf(ty, ty, tz * tz)));   // Eq. 22
-        ax = fmaf(wgt, d4.x, ax); ay = fmaf(wgt, d4.y, ay); az = fmaf(wgt, d4.z, az);
-      }
-    }
+    shear_drain();
   }
   if (tid < mcount && (ax != 0.f || ay != 0.f || az != 0.f)) {
     float* o = p.marker + ((size_t)e * p.M + __ldg(&pt.mstart) + tid) * 3;

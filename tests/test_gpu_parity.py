@@ -510,6 +510,45 @@ def test_elastomer_shear_history():
     sim.close(); plain.close()
 
 
+def test_shear_dense_contact_drains_the_queue():
+    """A flat, densely sampled face (4,000 tracked points over one 20 x 20 mm pad, all anchored and penetrating) is far more
+    than the shear kernel's 512-entry shared-memory queue holds at once: the kernel must drain it in passes and still
+    equal the oracle's plain sum over every anchored point (Eq. 22)."""
+    import torch
+    from oracle import oracle as O
+    from paper_2606_22332_b200.binding import TactileSim
+    from parity import ATOL, RTOL
+    patch = dict(link=0, origin=(0, 0, 0), u_axis=(1, 0, 0), v_axis=(0, 1, 0), size_u=0.02, size_v=0.02, nu=8, nv=8, radius=2e-3,
+                 marker_nu=7, marker_nv=7)
+    E, N = 3, 4000
+    rng = np.random.default_rng(77)
+    pts = np.zeros((1, N, 3), np.float32)
+    pts[0, :, :2] = rng.uniform(-0.012, 0.012, (N, 2))          # a flat face a little wider than the pad
+    cid = np.zeros((E, 1), np.int32)
+    phys = dict(shear_enable=1)
+    sim = TactileSim([patch], 64, E, 1, 1, physics=phys, outputs=("marker",))
+    sim.set_geometry(np.zeros((E, 1), np.int32), np.zeros((E, 1, 4), np.float32))
+    sim.set_pointclouds(pts, cid)
+    orc = O.Oracle([patch], 64, 1, 1, np.arange(E), physics=phys)
+    orc.set_geometry(np.zeros((E, 1), np.int32), np.zeros((E, 1, 4), np.float32))
+    orc.set_pointclouds(pts, cid)
+    z = lambda n: np.zeros((E, 1, n), np.float32)
+    q = z(4); q[..., 0] = 1
+    worst, peak = 0.0, 0.0
+    for s in range(4):
+        op = z(3)
+        op[:, 0, 2] = -0.001                                    # 1 mm into the pad
+        op[:, 0, 0] = 0.0003 * s * (1 + np.arange(E))           # each env slides at its own rate
+        inp = dict(link_pos=z(3), link_quat=q, link_linvel=z(3), link_angvel=z(3), obj_pos=op, obj_quat=q, obj_linvel=z(3), obj_angvel=z(3))
+        g = sim.step(sim.upload(inp))["marker"].cpu().numpy().astype(np.float64)
+        r = orc.step(inp, want=("marker",), aux=False)["marker"]
+        worst = max(worst, float((np.abs(g - r) / (ATOL + RTOL * np.abs(r))).max()))
+        peak = max(peak, float(np.abs(r).max()))
+    print(json.dumps({"shear_dense_max_ratio": worst, "peak_marker_m": peak}))
+    assert worst <= 1.0 and peak > 1e-2                         # thousands of anchored points really contribute
+    sim.close()
+
+
 def test_raycast_depth_backend():
     """the raycast contact-depth backend (App. A.1) on triangle meshes: BVH walk on the GPU against
     the oracle's brute force over every triangle.  Config-5 scene with 1,280-triangle star meshes; depth element-wise,
