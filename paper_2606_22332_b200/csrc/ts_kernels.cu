@@ -834,23 +834,28 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
           // its 8 corners stay in registers and are reloaded only when the cell index changes.
           unsigned pidx = 0xffffffffu;
           float4 A = make_float4(0.f, 0.f, 0.f, 0.f), B = A;
-          // No branch around the evaluation: finished lanes run it too and discard the result (t stays, so go stays
-          // 0); only the gathers are predicated on `go` (a finished lane's cell index may lie outside the bank).  This
-          // saves the BSSY / BRA / BSYNC bracket of every iteration (5 of 54 instructions).
-          for (int it = 1; it < p.march_steps; ++it) {
-            if (!__any_sync(TS_FULL, go)) break;
+          // No per-lane "finished" state inside the loop: every exit of O7 is a fixed point of the update (t = cap
+          // stays at cap; an evaluation that left t unchanged is repeated at the same point and leaves it unchanged
+          // again), so a finished lane simply keeps evaluating and t does not move.  Lanes that never march get their own
+          // cap = t (and never gather: their segment may leave the bank; A = B = 0 gives s = 0).  Only the loop exit
+          // looks at the lanes: one vote on "t moved and is below the cap".  Against the form with a per-lane flag this
+          // drops the FSEL / SEL / 3 ISETP of every iteration (5 of 45 instructions); same t, bit for bit.
+          const bool m0 = go != 0;
+          const float cap = m0 ? p.r_prox : t;
+          bool cont = __any_sync(TS_FULL, m0);
+          for (int it = 1; it < p.march_steps && cont; ++it) {
             const F3 u = u0 + t * du;
             const float MAGIC = 12582912.f;  // 1.5 * 2^23
             const float tx = __fadd_rd(u.x, MAGIC), ty = __fadd_rd(u.y, MAGIC), tz = __fadd_rd(u.z, MAGIC);
             const unsigned idx = ((__float_as_uint(ty) * (unsigned)(N - 1) + __float_as_uint(tx)) * (unsigned)N + __float_as_uint(tz)) + cbase;
-            if (go && idx != pidx) {
+            if (m0 && idx != pidx) {
               A = __ldg(p.bank + idx);
               B = __ldg(p.bank + idx + 1);
               pidx = idx;
             }
             const float sv = trilerp(A, B, u.x - (tx - MAGIC), u.y - (ty - MAGIC), u.z - (tz - MAGIC));
-            const float tn = go ? fminf(t + fmaxf(sv, 0.f), p.r_prox) : t;
-            go = (tn != t) && (tn < p.r_prox);
+            const float tn = fminf(t + fmaxf(sv, 0.f), cap);
+            cont = __any_sync(TS_FULL, (tn != t) && (tn < cap));
             t = tn;
           }
         } else {
@@ -865,12 +870,14 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
           }
         }
       } else {
+        // same fixed-point form as the grid loop: lanes that never march carry cap = t
+        const float cap = go ? p.r_prox : t;
+        bool cont = __any_sync(TS_FULL, go);
 #define TS_PRIM_LOOP(TYPE)                                                         \
-  for (int it = 1; it < p.march_steps; ++it) {                                     \
-    if (!__any_sync(TS_FULL, go)) break;                                           \
+  for (int it = 1; it < p.march_steps && cont; ++it) {                             \
     const float sv = prim_value_f(TYPE, F.prm, xo + t * dr);                       \
-    const float tn = go ? fminf(t + fmaxf(sv, 0.f), p.r_prox) : t;                 \
-    go = (tn != t) && (tn < p.r_prox);                                             \
+    const float tn = fminf(t + fmaxf(sv, 0.f), cap);                               \
+    cont = __any_sync(TS_FULL, (tn != t) && (tn < cap));                           \
     t = tn;                                                                        \
   }
         if (gtype == TS_GEOM_SPHERE) { TS_PRIM_LOOP(TS_GEOM_SPHERE) }
