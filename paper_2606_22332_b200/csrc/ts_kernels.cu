@@ -4,16 +4,16 @@
 // Mapping: ONE THREAD PER (environment, taxel slot); a block owns one "patch group" of one
 // environment: up to TS_BLOCK consecutive taxel slots made of whole patches (packed on the
 // host, ts_api.cu).  Per block:
-//   phase 0  seven threads per (patch link, object) pair build the relative pose in DOUBLE and park
-//            it in shared memory (frames);
+//   phase 0  (own launch, ts_frames_kernel) one thread per (env, patch link, object) builds the relative pose in
+//            DOUBLE into frames_g; the step kernel's block fetches its span with one TMA bulk copy on an mbarrier;
 //   phase 1  per taxel: x_o = c + M x_j (double), phi (double), depth, Schmitt contact bit;
 //   phase 2  proximity march along a_j (fp32; evaluation 0 is the phase-1 query);
 //   phase 3  kinematic force/torque in double for warps that touch anything, rounded once;
 //   phase 4  noise chain: hysteresis -> crosstalk (neighbours through shared memory) ->
 //            Philox/Box-Muller random-walk drift -> dead taxels;
-//   phase 5  elastomer marker dilation as two separable passes over shared memory (double).
+//   phase 5  elastomer marker dilation per patch warp as FP64 tensor-core products (DMMA.8x8x4) of the separable tables.
 // Outputs go straight from registers to global memory with streaming stores; shared memory is kept
-// at 13 KB per block because it comes out of the L1 that serves the SDF gathers.
+// at 10 KB per block because it comes out of the L1 that serves the SDF gathers.
 //
 // Why double in phases 0/1/3/5: outputs are compared element by
 // element at rtol 1e-4 / atol 1e-6.  d = R - phi feeds f ~ d^1.2, the marker sum multiplies
@@ -31,6 +31,10 @@
 #include <mutex>
 
 #include "ts_internal.h"
+
+#ifndef TS_PDL
+#define TS_PDL 1  // step kernel launched as a programmatic dependent of ts_frames_kernel (griddepcontrol)
+#endif
 
 namespace {
 
@@ -178,6 +182,9 @@ __global__ void __launch_bounds__(128) ts_frames_kernel(const __grid_constant__ 
   // (ncu: lg_throttle 4.2 per issue, 47 us); staged 17 x 512-byte requests per warp.
   __shared__ __align__(16) unsigned char stage[128 * sizeof(FrameS)];
   if (p.clock && threadIdx.x == 0) atomicMin(p.clock, globaltimer_ns());   // device-side clock: first block start
+#if TS_PDL
+  asm volatile("griddepcontrol.launch_dependents;");   // once every block of this grid is resident, the step kernel's may start
+#endif
   const int PK = p.P * p.K;
   const long long total = (long long)p.E * PK;
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -564,6 +571,28 @@ __device__ __forceinline__ void noise_prefetch(const TsStepParams& p, int e, int
   }
 }
 
+// The same prefetch for the whole block by ONE thread: a bulk L2 prefetch (cp.async.bulk.prefetch.L2, SASS UBLKPF) per
+// state row of the block's slots [gstart, gstart + gcount), issued from the uniform datapath next to the frames copy:
+// ~3 issue slots per warp on average instead of 24 in every warp.  Start and size are rounded outwards to 16 bytes
+// (rows are padded to Tp = 32 k slots, so the span stays inside the env's row).
+#ifndef TS_STATE_BULK_PF
+#define TS_STATE_BULK_PF 1
+#endif
+template <int HM>
+__device__ __forceinline__ void noise_prefetch_bulk(const TsStepParams& p, int e, int gstart, int gcount) {
+  constexpr int MODE = HM & 3;
+  constexpr int NH = MODE == TS_HYST_MAXWELL ? 6 : (MODE == TS_HYST_ASYM ? 3 : 0);
+  const unsigned Tp = (unsigned)p.Tp;
+  const unsigned j0 = (unsigned)gstart & ~1u;
+  const unsigned bytes = ((((unsigned)(gstart + gcount) + 1u) & ~1u) - j0) * 8u;
+  const float2* h = reinterpret_cast<const float2*>(p.st_hyst) + (size_t)((unsigned)e * (unsigned)NH) * Tp + j0;
+  const float2* d = reinterpret_cast<const float2*>(p.st_drift) + (size_t)((unsigned)e * 3u) * Tp + j0;
+#pragma unroll
+  for (int r = 0; r < NH; ++r) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(h + (size_t)r * Tp), "r"(bytes) : "memory");
+#pragma unroll
+  for (int r = 0; r < 3; ++r) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(d + (size_t)r * Tp), "r"(bytes) : "memory");
+}
+
 // Every thread of the block must call this (it contains one __syncthreads).
 template <int HM, bool FAST = false>
 __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j, unsigned ej, int tid, int patch0, bool valid,
@@ -843,7 +872,7 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
           const bool m0 = go != 0;
           const float cap = m0 ? p.r_prox : t;
           bool cont = __any_sync(TS_FULL, m0);
-          for (int it = 1; it < p.march_steps && cont; ++it) {
+          for (int left = p.march_steps - 1; left > 0 && cont; --left) {   // down-counter: no re-read of march_steps
             const F3 u = u0 + t * du;
             const float MAGIC = 12582912.f;  // 1.5 * 2^23
             const float tx = __fadd_rd(u.x, MAGIC), ty = __fadd_rd(u.y, MAGIC), tz = __fadd_rd(u.z, MAGIC);
@@ -874,7 +903,7 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
         const float cap = go ? p.r_prox : t;
         bool cont = __any_sync(TS_FULL, go);
 #define TS_PRIM_LOOP(TYPE)                                                         \
-  for (int it = 1; it < p.march_steps && cont; ++it) {                             \
+  for (int left = p.march_steps - 1; left > 0 && cont; --left) {                   \
     const float sv = prim_value_f(TYPE, F.prm, xo + t * dr);                       \
     const float tn = fminf(t + fmaxf(sv, 0.f), cap);                               \
     cont = __any_sync(TS_FULL, (tn != t) && (tn < cap));                           \
@@ -957,12 +986,22 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     const unsigned bytes = (unsigned)(npatch * p.K) * (unsigned)sizeof(FrameS);
     mbar_expect_tx(&fbar, bytes);
     const FrameS* src = reinterpret_cast<const FrameS*>(p.frames_g) + ((size_t)bxi * p.P + patch0) * p.K;
+#if TS_PDL
+    // Programmatic dependent launch: this grid may start while ts_frames_kernel is still draining.  frames_g is the only
+    // thing it produces, and this thread is the only one that reads it (through the bulk copy below), so it is the one
+    // that waits for the frames grid to complete and flush.  Everything else the prologue touches (layout tables, the
+    // state rows written by the PREVIOUS step kernel, which finished before the frames kernel began) is older.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
     bulk_g2s(frames, src, bytes, &fbar);
     // L2 prefetch of the same rows for the block TS_PF_AHEAD positions later in launch order (blockIdx.x runs fastest):
     // by the time that block starts, its bulk copy is an L2 hit instead of a DRAM round trip in front of phase 1.
     constexpr unsigned AH = TS_GRID_GFAST ? TS_PF_AHEAD / 4 : TS_PF_AHEAD;
     if (TS_PF_AHEAD > 0 && bxi + AH < (unsigned)p.E)
       asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src + (size_t)AH * p.P * p.K), "r"(bytes) : "memory");
+#if TS_STATE_BULK_PF == 1
+    if (NOISE) noise_prefetch_bulk<HM>(p, e, gstart, gcount);
+#endif
   }
   const bool valid = tid < gcount;
   const int j = gstart + (valid ? tid : 0);
@@ -973,7 +1012,9 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const float Rj = valid ? P4.w : 0.f;  // R_j = 0: inactive slot
   const bool act = Rj > 0.f;
   uint8_t flag = valid ? p.st_flags[ej] : (uint8_t)0;
+#if TS_STATE_BULK_PF == 0
   if (NOISE) noise_prefetch<HM>(p, e, gstart + (tid & ~31), gstart + gcount, tid & 31);
+#endif
   __syncthreads();        // publishes the mbarrier (and pmask); every warp arrives within a few cycles of block start
   mbar_wait(&fbar, 0u);   // frames landed in shared memory (async-proxy writes are visible after the wait)
 
@@ -1812,6 +1853,25 @@ int ts_prepare_kernels(int device, int smem_bytes) {
 }
 
 // fused_noise != 0: one launch does everything; otherwise the geometry kernel, and (noise on) ts_launch_noise.
+// Launch with the programmatic-stream-serialization attribute: the grid may begin once every block of the kernel in
+// front of it in the stream (ts_frames_kernel) has executed griddepcontrol.launch_dependents; its thread 0 waits for that
+// grid's completion before it touches frames_g.  A predecessor that never triggers (an event record, a memcpy, another
+// library's kernel) degrades this to a normal launch.
+template <typename KernelT>
+static int launch_dependent(KernelT kernel, dim3 grid, size_t smem, cudaStream_t stream, const TsStepParams& p) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(TS_BLOCK);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = TS_PDL ? 1 : 0;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return (int)cudaLaunchKernelEx(&cfg, kernel, p);
+}
+
 int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
   if (p.E <= 0 || p.G <= 0 || p.G > 65535) return (int)cudaErrorInvalidConfiguration;
   const size_t smem = (size_t)ts_step_smem_bytes(p);
@@ -1825,9 +1885,9 @@ int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
   const bool clean5 = p.K == 1 && p.inl && p.env_perm && p.mk_mma && p.contact && p.depth && p.ft && p.marker && p.prox;
   const bool fast = clean5 && p.ft_noisy && p.dead && (hm == TS_HYST_ASYM || hm == TS_HYST_MAXWELL);
   if (clean5 && hm == -1 && !p.noise_enable && !p.dead && !p.depth_pert)
-    ts_step_kernel<true, -1, true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
-  else if (fast && hm == TS_HYST_ASYM) ts_step_kernel<true, TS_HYST_ASYM, true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
-  else if (fast) ts_step_kernel<true, TS_HYST_MAXWELL, true><<<grid, TS_BLOCK, smem, (cudaStream_t)stream>>>(p);
+    return launch_dependent(ts_step_kernel<true, -1, true>, grid, smem, (cudaStream_t)stream, p);
+  else if (fast && hm == TS_HYST_ASYM) return launch_dependent(ts_step_kernel<true, TS_HYST_ASYM, true>, grid, smem, (cudaStream_t)stream, p);
+  else if (fast) return launch_dependent(ts_step_kernel<true, TS_HYST_MAXWELL, true>, grid, smem, (cudaStream_t)stream, p);
   else if (p.K == 1) launch_one<true>(p, hm, grid, smem, (cudaStream_t)stream);
   else launch_one<false>(p, hm, grid, smem, (cudaStream_t)stream);
   return (int)cudaGetLastError();
