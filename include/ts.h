@@ -24,6 +24,12 @@
  * stated.  The ctx keeps state between calls (Schmitt bits, hysteresis, drift, counters, the
  * frames of the step in flight), so successive calls on one ctx must be ordered: use ONE stream,
  * or order the streams yourself with events; the library does not check this.
+ * Programmatic dependent launch: within a step the readout kernel is launched as a programmatic dependent of the
+ * pose kernel, and the pose kernel of the NEXT ts_step as a dependent of this step's readout kernel, so when ts_step
+ * calls are enqueued back to back on one stream the launch latencies and block ramp-up are hidden behind the kernel in
+ * front.  The pose kernel still waits, on the device, for everything enqueued in front of it (the caller's kernels that
+ * produce the next poses included) to complete and become visible before it reads anything, and the readout kernel
+ * for the pose kernel; results do not depend on the overlap (tests/test_gpu_api.py).
  * Errors: every call returns a ts_status; nothing throws, aborts or prints.
  */
 #ifndef TS_H_

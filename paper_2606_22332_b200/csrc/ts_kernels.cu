@@ -33,7 +33,8 @@
 #include "ts_internal.h"
 
 #ifndef TS_PDL
-#define TS_PDL 1  // step kernel launched as a programmatic dependent of ts_frames_kernel (griddepcontrol)
+#define TS_PDL 2  // 1: step kernel launched as a programmatic dependent of ts_frames_kernel (griddepcontrol);
+                  // 2: also the NEXT step's frames kernel as a dependent of this step kernel (see ts_launch_frames)
 #endif
 
 namespace {
@@ -181,10 +182,17 @@ __global__ void __launch_bounds__(128) ts_frames_kernel(const __grid_constant__ 
   // fully coalesced run: per-thread 272-byte rows straight to global memory cost 32 sectors per store request
   // (ncu: lg_throttle 4.2 per issue, 47 us); staged 17 x 512-byte requests per warp.
   __shared__ __align__(16) unsigned char stage[128 * sizeof(FrameS)];
-  if (p.clock && threadIdx.x == 0) atomicMin(p.clock, globaltimer_ns());   // device-side clock: first block start
 #if TS_PDL
   asm volatile("griddepcontrol.launch_dependents;");   // once every block of this grid is resident, the step kernel's may start
 #endif
+#if TS_PDL >= 2
+  // Launched as a programmatic dependent (ts_launch_frames): the blocks may become resident while the kernel in front of
+  // this one in the stream is in its last wave; they wait here until it -- the previous step kernel, or whatever the
+  // caller enqueued to produce this step's poses -- has completed and its writes are visible.  (Reading the poses before
+  // this wait, which is legal only for inputs that are older than the previous step, measured no faster.)
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+  if (p.clock && threadIdx.x == 0) atomicMin(p.clock, globaltimer_ns());   // device-side clock: first block's start of work
   const int PK = p.P * p.K;
   const long long total = (long long)p.E * PK;
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -987,10 +995,10 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
     mbar_expect_tx(&fbar, bytes);
     const FrameS* src = reinterpret_cast<const FrameS*>(p.frames_g) + ((size_t)bxi * p.P + patch0) * p.K;
 #if TS_PDL
-    // Programmatic dependent launch: this grid may start while ts_frames_kernel is still draining.  frames_g is the only
-    // thing it produces, and this thread is the only one that reads it (through the bulk copy below), so it is the one
-    // that waits for the frames grid to complete and flush.  Everything else the prologue touches (layout tables, the
-    // state rows written by the PREVIOUS step kernel, which finished before the frames kernel began) is older.
+    // Programmatic dependent launch: this grid may start while ts_frames_kernel is still draining.  This thread reads
+    // frames_g (through the bulk copy below), so it waits for the frames grid to complete and flush.  (With TS_PDL = 1
+    // it is the only thread that has to: the previous step kernel finished before the frames kernel began.  With the
+    // chained launch of TS_PDL = 2 every thread waits again below, before it reads state.)
     asm volatile("griddepcontrol.wait;" ::: "memory");
 #endif
     bulk_g2s(frames, src, bytes, &fbar);
@@ -1011,12 +1019,23 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   const int lp = meta & 255;
   const float Rj = valid ? P4.w : 0.f;  // R_j = 0: inactive slot
   const bool act = Rj > 0.f;
+#if TS_PDL >= 2
+  // Every thread: the flag byte and the state rows read below were written by the PREVIOUS step kernel.  With the
+  // chained launch this grid's blocks can be resident before that kernel has finished; it is complete once the frames
+  // grid in front of this one is (whose blocks waited for it at their top).
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
   uint8_t flag = valid ? p.st_flags[ej] : (uint8_t)0;
 #if TS_STATE_BULK_PF == 0
   if (NOISE) noise_prefetch<HM>(p, e, gstart + (tid & ~31), gstart + gcount, tid & 31);
 #endif
   __syncthreads();        // publishes the mbarrier (and pmask); every warp arrives within a few cycles of block start
   mbar_wait(&fbar, 0u);   // frames landed in shared memory (async-proxy writes are visible after the wait)
+#if TS_PDL >= 2
+  // This block no longer needs frames_g: once every block of the grid has said so, the next step's frames kernel may
+  // start overwriting it (it then runs alongside this grid's last wave).
+  asm volatile("griddepcontrol.launch_dependents;");
+#endif
 
   // ---- phase 1 (S1-S4): x_o = c + M x_j, phi = min_k phi_k, depth (Eq. 2), contact (Eq. 3) ----
   double phid = __longlong_as_double(0x7ff0000000000000LL);
@@ -1897,8 +1916,26 @@ unsigned long long ts_frame_bytes() { return sizeof(FrameS); }
 
 int ts_launch_frames(const TsStepParams& p, void* stream) {
   const long long n = (long long)p.E * p.P * p.K;
+#if TS_PDL >= 2
+  // Chained across steps: when the kernel in front of this one in the stream is the previous ts_step_kernel, this grid's
+  // blocks may become resident once every block of it has fetched its frames; they wait at their top for it to complete
+  // (griddepcontrol.wait), so only launch latency and ramp-up overlap.  Anything else in front (the caller's own kernels
+  // writing the next poses, an event record, a copy) makes this an ordinary launch.
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)((n + 127) / 128));
+  cfg.blockDim = dim3(128);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = (cudaStream_t)stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return (int)cudaLaunchKernelEx(&cfg, ts_frames_kernel, p);
+#else
   ts_frames_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(p);
   return (int)cudaGetLastError();
+#endif
 }
 
 int ts_launch_shear(const TsStepParams& p, void* stream) {

@@ -228,3 +228,30 @@ def test_outputs_stay_inside_their_buffers():
                 else:
                     assert torch.isnan(lo).all() and torch.isnan(hi).all() and torch.isfinite(mid).all(), (cid, form, k)
             sim.close()
+
+
+def test_chained_launches_equal_serialised_steps():
+    """The frames kernel of step n+1 is launched as a programmatic dependent of step n's kernel and the step kernel as a
+    dependent of its frames kernel (include/ts.h, "Programmatic dependent launch"): with steps enqueued back to back the
+    blocks of the next grid are resident while the grid in front drains.  The result must equal, bit for bit, the same
+    steps with a device synchronise after each one (no overlap possible), at BASELINE size where every SM holds blocks of
+    both grids at the hand-over."""
+    import torch
+    w = W.config(5)
+    xs = None
+    res = []
+    for serialise in (False, True, False):
+        sim = _sim(w)
+        if xs is None:
+            xs = [sim.upload(w.inputs(s)) for s in range(6)]
+        torch.cuda.synchronize()
+        for s in range(36):
+            out = sim.step(xs[s % 6])
+            if serialise:
+                torch.cuda.synchronize()
+        torch.cuda.synchronize()
+        res.append({k: v.clone() for k, v in out.items()})
+        sim.close()
+    for r in res[1:]:
+        for k in res[0]:
+            assert torch.equal(res[0][k], r[k]), k
