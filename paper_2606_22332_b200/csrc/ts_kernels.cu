@@ -109,12 +109,11 @@ struct FrameS {
   double wL[3];    // R_L^T w_L
   double vbar[3];  // R_L^T (v_O - v_L)
   double cbar[3];  // R_L^T (p_L - p_O)
-  float Mf[9];     // fp32 copies for the march
-  float cf[3];
   float prm[4];
   int type;
   float dirf[3];   // M n: march direction of the patch normal in the object frame (fp32)
-};
+};                 // 224 bytes: a multiple of 16 (the step kernel's bulk copy moves whole records)
+static_assert(sizeof(FrameS) == 224, "FrameS layout");
 
 // One frame is built by SEVEN threads so that the dependent double-precision chain the whole block
 // waits for stays short (~60 instructions): "row" items r = 0..2 (row r of M and c[r]) run in the lower
@@ -143,11 +142,9 @@ __device__ __forceinline__ void build_frame_row(const TsStepParams& p, int e, in
   for (int c = 0; c < 3; ++c) {
     const double m = fma(o0, RL[c], fma(o1, RL[3 + c], o2 * RL[6 + c]));
     F.M[r * 3 + c] = m;
-    F.Mf[r * 3 + c] = (float)m;
   }
   const double cr = fma(o0, d.x, fma(o1, d.y, o2 * d.z));
   F.c[r] = cr;
-  F.cf[r] = (float)cr;
   F.dirf[r] = (float)fma(F.M[r * 3], (double)na.x, fma(F.M[r * 3 + 1], (double)na.y, F.M[r * 3 + 2] * (double)na.z));
 }
 
@@ -172,16 +169,18 @@ __device__ __forceinline__ void build_frame_vec(const TsStepParams& p, int e, in
   dst[0] = o.x; dst[1] = o.y; dst[2] = o.z;
 }
 
-// Phase 0 as its own launch: one thread per (env, patch, object) builds the whole frame in registers and writes it to
-// frames_g[e][patch * K + k].  Inside the step kernel the same arithmetic sat in front of a block barrier and took
+// Phase 0 as its own launch: one thread per (env, patch, object) builds the whole frame and writes it to frames_g (block
+// order of the step kernel).  Inside the step kernel the same arithmetic sat in front of a block barrier and took
 // ~19 % of every block's lifetime (a ~250-instruction dependent double-precision chain behind a DRAM round trip, with
 // 6 of 8 warps waiting); here it is 410 k independent threads, and the step kernel's blocks receive their frames with
-// one TMA bulk copy.  Same functions, same operation order: bit-identical frames.
+// one TMA bulk copy.
 __global__ void __launch_bounds__(128) ts_frames_kernel(const __grid_constant__ TsStepParams p) {
-  // Each warp stages its 32 consecutive frames (8.5 KB) in shared memory and writes them out as one contiguous,
-  // fully coalesced run: per-thread 272-byte rows straight to global memory cost 32 sectors per store request
-  // (ncu: lg_throttle 4.2 per issue, 47 us); staged 17 x 512-byte requests per warp.
-  __shared__ __align__(16) unsigned char stage[128 * sizeof(FrameS)];
+  // Each warp stages its 32 consecutive frames in shared memory and writes them out as one contiguous, fully coalesced
+  // run: per-thread rows straight to global memory cost 32 sectors per store request (ncu: lg_throttle 4.2 per issue,
+  // 47 us).  The fields go straight into the thread's staging row (no register image of the record: 96 -> ~56
+  // registers); the row stride of 232 bytes (= 58 words) spreads the 16 lanes of an 8-byte store over distinct banks.
+  constexpr int STRIDE = (int)sizeof(FrameS) + 8;
+  __shared__ __align__(16) unsigned char stage[128 * STRIDE];
 #if TS_PDL
   asm volatile("griddepcontrol.launch_dependents;");   // once every block of this grid is resident, the step kernel's may start
 #endif
@@ -196,34 +195,36 @@ __global__ void __launch_bounds__(128) ts_frames_kernel(const __grid_constant__ 
   const int PK = p.P * p.K;
   const long long total = (long long)p.E * PK;
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  FrameS F;
-#pragma unroll
-  for (int i = 0; i < (int)(sizeof(FrameS) / 4); ++i) reinterpret_cast<uint32_t*>(&F)[i] = 0u;
+  FrameS& F = *reinterpret_cast<FrameS*>(stage + (size_t)threadIdx.x * STRIDE);
+  int link = -1;
   if (gt < total) {
     // frames are stored in BLOCK order of the step kernel (row bx = frames of env env_perm[bx]), so that a block's bulk
     // copy needs no env lookup in front of it and the rows of the blocks scheduled next sit at a fixed distance ahead
     const int bx = (int)(gt / PK), f = (int)(gt - (long long)bx * PK);
     const int e = p.env_perm ? __ldg(p.env_perm + bx) : bx;
     const int pidx = f / p.K, k = f - pidx * p.K;
-    const int link = __ldg(p.patch_link + pidx);
+    link = __ldg(p.patch_link + pidx);
+    if (link < 0) {   // filtered link: everything but type / prm stays zero
+#pragma unroll
+      for (int i = 0; i < (int)(sizeof(FrameS) / 8); ++i) reinterpret_cast<uint2*>(&F)[i] = make_uint2(0u, 0u);
+    }
 #pragma unroll
     for (int r = 0; r < 3; ++r) build_frame_row(p, e, link, pidx, k, r, F);
 #pragma unroll
     for (int sub = 0; sub < 4; ++sub) build_frame_vec(p, e, link, k, sub, F);
   }
-  uint4* row = reinterpret_cast<uint4*>(stage + (size_t)threadIdx.x * sizeof(FrameS));
-  const uint4* src = reinterpret_cast<const uint4*>(&F);
-#pragma unroll
-  for (int i = 0; i < (int)(sizeof(FrameS) / 16); ++i) row[i] = src[i];
   __syncwarp();
   const int lane = threadIdx.x & 31, w0 = threadIdx.x & ~31;
   const long long g0 = (long long)blockIdx.x * blockDim.x + w0;              // first frame of this warp
-  const long long n16 = (total - g0 < 32 ? (total - g0 > 0 ? total - g0 : 0) : 32) * (long long)(sizeof(FrameS) / 16);
-  const uint4* wsrc = reinterpret_cast<const uint4*>(stage + (size_t)w0 * sizeof(FrameS));
-  uint4* wdst = reinterpret_cast<uint4*>(reinterpret_cast<FrameS*>(p.frames_g) + g0);
+  constexpr int W8 = (int)(sizeof(FrameS) / 8);                              // 8-byte words per record
+  const int n8 = (int)(total - g0 < 32 ? (total - g0 > 0 ? total - g0 : 0) : 32) * W8;
+  const unsigned char* wsrc = stage + (size_t)w0 * STRIDE;
+  uint2* wdst = reinterpret_cast<uint2*>(reinterpret_cast<FrameS*>(p.frames_g) + g0);
 #pragma unroll
-  for (int i = 0; i < (int)(sizeof(FrameS) / 16); ++i)
-    if (i * 32 + lane < n16) wdst[i * 32 + lane] = wsrc[i * 32 + lane];
+  for (int i = 0; i < W8; ++i) {
+    const int q = i * 32 + lane, fr = q / W8, part = q - fr * W8;
+    if (q < n8) wdst[q] = *reinterpret_cast<const uint2*>(wsrc + fr * STRIDE + part * 8);
+  }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -933,8 +934,11 @@ __device__ __forceinline__ void march_phase(const TsStepParams& p, const FrameS*
           float sv = __int_as_float(0x7f800000);
           for (int k = 0; k < p.K; ++k) {
             const FrameS& F = frames[lp * p.K + k];
-            const F3 x = mk3(F.cf[0] + fmaf(F.Mf[0], y.x, fmaf(F.Mf[1], y.y, F.Mf[2] * y.z)), F.cf[1] + fmaf(F.Mf[3], y.x, fmaf(F.Mf[4], y.y, F.Mf[5] * y.z)),
-                             F.cf[2] + fmaf(F.Mf[6], y.x, fmaf(F.Mf[7], y.y, F.Mf[8] * y.z)));
+            // fp32 images of M and c, rounded here (K > 1 only; the single-object path marches from xo and dirf)
+            const float m0 = (float)F.M[0], m1 = (float)F.M[1], m2 = (float)F.M[2], m3 = (float)F.M[3], m4 = (float)F.M[4],
+                        m5 = (float)F.M[5], m6 = (float)F.M[6], m7 = (float)F.M[7], m8 = (float)F.M[8];
+            const F3 x = mk3((float)F.c[0] + fmaf(m0, y.x, fmaf(m1, y.y, m2 * y.z)), (float)F.c[1] + fmaf(m3, y.x, fmaf(m4, y.y, m5 * y.z)),
+                             (float)F.c[2] + fmaf(m6, y.x, fmaf(m7, y.y, m8 * y.z)));
             sv = fminf(sv, phi_f(p, F.type, F.prm, x));
           }
           const float tn = fminf(t + fmaxf(sv, 0.f), p.r_prox);
