@@ -32,6 +32,9 @@
 
 #include "ts_internal.h"
 
+#ifndef TS_MARCH_LATE
+#define TS_MARCH_LATE 0  // 1: proximity march after the noise chain (experiment)
+#endif
 #ifndef TS_PDL
 #define TS_PDL 2  // 1: step kernel launched as a programmatic dependent of ts_frames_kernel (griddepcontrol);
                   // 2: also the NEXT step's frames kernel as a dependent of this step kernel (see ts_launch_frames)
@@ -1079,7 +1082,9 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   }
   const F3 xo = mk3((float)xd.x, (float)xd.y, (float)xd.z);  // fp32 object-frame position for the march
 
+#if !TS_MARCH_LATE
   march_phase<SINGLE, FAST>(p, frames, e, lp, valid, act, ej, phif, xo, P4, patch0 + lp);
+#endif
 
   // ---- phase 3 (S5): kinematic force / torque (Eq. 4-9, D2) in double, link frame ---------------
   // Eq. 26 (R8): the noisy readout senses with R~_j = max(0, R_j + eps_j), eps_j ~ U[-rho, rho] drawn once per
@@ -1178,6 +1183,9 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
   if (NOISE) noise_load<HM>(p, e, j, valid, ns);
   if (NOISE) noise_chain<HM, FAST>(p, e, j, ej, tid, patch0, valid, act, deadb, meta, ft, ns, bufB);
   else __syncthreads();
+#if TS_MARCH_LATE
+  march_phase<SINGLE, FAST>(p, frames, e, lp, valid, act, ej, phif, xo, P4, patch0 + lp);
+#endif
 
   // ---- phase 5 (S6): elastomer marker dilation (Eq. 18-21, 23 first sum) ----------------------
   // With c = 1 and planar regular grids, g(r_ij) = exp(-lambda |r|^2) = gu(a,p) gv(b,q) and
