@@ -1054,7 +1054,9 @@ __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const 
       const FrameS& F = frames[lp * (SINGLE ? 1 : p.K) + k];
       const D3 x = ldv(F.c) + mulR(F.M, xj);
       const double ph = phi_d(p, F.type, F.prm, x);
-      if (ph < phid) {  // strict: ties -> lowest k (Q3)
+      if (SINGLE) {  // one object: no comparison (and none of its 8 predicated register moves)
+        phid = ph; xd = x;
+      } else if (ph < phid) {  // strict: ties -> lowest k (Q3)
         phid = ph; kst = k; xd = x;
       }
     }
