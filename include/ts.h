@@ -316,6 +316,20 @@ ts_status ts_reset(ts_ctx* ctx, const uint8_t* env_mask_dev, void* stream);
 
 ts_status ts_destroy(ts_ctx* ctx); /* NULL is a no-op returning TS_OK */
 
+/* Checkpoint / resume.  Everything a ctx carries from step to step -- the Schmitt contact bits and
+ * dead flags, hysteresis and drift state, the read-delay ring, the state of the noisy scalar readouts, the shear
+ * anchors, the per-env reset step / episode counters and the global step counter -- as ONE flat blob in HOST memory
+ * (a fixed header followed by the arrays, each padded to 16 bytes).  Layout, geometry, point clouds and meshes are NOT part of it: the blob
+ * restores into a ctx created with the same layout and configuration (sizes and section set are checked; anything else
+ * returns TS_ERR_INVALID_ARG and leaves the ctx untouched), after which stepping continues bit for bit as in the ctx it
+ * was taken from.  Both calls enqueue their copies on `stream` and synchronise it once before returning.
+ * ts_state_bytes: size of the blob for this ctx (it depends on the configuration only).
+ * ts_get_state:   host_buf [capacity >= ts_state_bytes] is filled.
+ * ts_set_state:   host_buf [bytes] as written by ts_get_state. */
+ts_status ts_state_bytes(const ts_ctx* ctx, uint64_t* bytes);
+ts_status ts_get_state(ts_ctx* ctx, void* host_buf, uint64_t capacity, void* stream);
+ts_status ts_set_state(ts_ctx* ctx, const void* host_buf, uint64_t bytes, void* stream);
+
 /* Last error text of this ctx (or of the last failed ts_create when ctx is NULL).  Never NULL. */
 const char* ts_last_error(const ts_ctx* ctx);
 

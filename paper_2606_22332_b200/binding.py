@@ -26,7 +26,8 @@ SN_KNOBS = ("sigma_white", "sigma_rw", "bias", "quant", "stuck_min", "stuck_max"
 SYMBOLS = ["ts_layout_create", "ts_layout_add_patch", "ts_layout_filter_links", "ts_layout_finalize", "ts_layout_get",
            "ts_layout_destroy", "ts_config_default", "ts_create", "ts_set_geometry", "ts_set_pointclouds", "ts_set_meshes", "ts_step", "ts_step_host",
            "ts_reset", "ts_destroy", "ts_last_error", "ts_n_taxels", "ts_n_markers", "ts_launches_per_step",
-           "ts_kernel_time_ms", "ts_kernel_times_ms", "ts_first_kernel_time_ms", "ts_version"]
+           "ts_kernel_time_ms", "ts_kernel_times_ms", "ts_first_kernel_time_ms", "ts_version",
+           "ts_state_bytes", "ts_get_state", "ts_set_state"]
 
 
 class TsError(RuntimeError):
@@ -139,6 +140,9 @@ def lib():
         L.ts_kernel_time_ms.argtypes = [vp, i32, C.POINTER(C.c_float), C.POINTER(i32)]
         L.ts_kernel_times_ms.argtypes = [vp, vp, i32, C.POINTER(i32)]
         L.ts_first_kernel_time_ms.argtypes = [vp]
+        L.ts_state_bytes.argtypes = [vp, C.POINTER(C.c_uint64)]
+        L.ts_get_state.argtypes = [vp, vp, C.c_uint64, vp]
+        L.ts_set_state.argtypes = [vp, vp, C.c_uint64, vp]
         L.ts_first_kernel_time_ms.restype = C.c_float
         L.ts_version.restype = C.c_char_p
         _lib = L
@@ -364,6 +368,22 @@ class TactileSim:
         out = np.zeros((max(n.value, 1), 4), np.float32)
         _check(lib().ts_kernel_times_ms(self.h, out.ctypes.data_as(C.c_void_p), n.value, C.byref(n)), self.h, "ts_kernel_times_ms")
         return out[:n.value]
+
+    def state_bytes(self):
+        n = C.c_uint64()
+        _check(lib().ts_state_bytes(self.h, C.byref(n)), self.h, "ts_state_bytes")
+        return int(n.value)
+
+    def get_state(self):
+        """The ctx's step-to-step state as one host blob (uint8 array): checkpoint."""
+        blob = np.empty(self.state_bytes(), np.uint8)
+        _check(lib().ts_get_state(self.h, blob.ctypes.data_as(C.c_void_p), blob.nbytes, self._stream()), self.h, "ts_get_state")
+        return blob
+
+    def set_state(self, blob):
+        """Restore a blob taken by get_state() from a ctx with the same layout and configuration: resume."""
+        blob = np.ascontiguousarray(blob, np.uint8)
+        _check(lib().ts_set_state(self.h, blob.ctypes.data_as(C.c_void_p), blob.nbytes, self._stream()), self.h, "ts_set_state")
 
     def first_kernel_time_ms(self):
         return float(lib().ts_first_kernel_time_ms(self.h))

@@ -887,6 +887,101 @@ ts_status ts_reset(ts_ctx* c, const uint8_t* env_mask_dev, void* stream) {
   return TS_OK;
 }
 
+// ---- checkpoint / resume ----------------------------------------------------------------------------------------
+namespace {
+constexpr int kStateSections = 12;
+struct StateHeader {            // 160 bytes
+  uint64_t magic, total;
+  uint32_t version, n_envs, n_taxels, tp, nh, n_markers, ring_slots, pc_n, n_patches, objs, gstep, n_sections;
+  uint64_t section_bytes[kStateSections];
+};
+static_assert(sizeof(StateHeader) == 16 + 48 + 8 * kStateSections, "StateHeader layout");
+constexpr uint64_t kStateMagic = 0x3130455441545354ull;  // "TSSTATE01"
+struct StateSection { void* dev; uint64_t bytes; };
+
+// Every array a ctx carries across steps, in blob order.  Absent ones (feature off) have 0 bytes.
+void state_sections(const ts_ctx* c, StateSection s[kStateSections], uint32_t* ring_slots) {
+  const uint64_t E = (uint64_t)c->cfg.n_envs, T = (uint64_t)c->T, M = (uint64_t)c->M, Tp = (uint64_t)c->Tp;
+  const uint32_t S = c->st_ring ? (uint32_t)(c->cfg.read_delay + c->cfg.read_jitter) : 0u;
+  const uint64_t nsh = c->sh_on ? E * (uint64_t)c->P * (uint64_t)c->cfg.objs_per_env * (uint64_t)c->pc_n : 0;
+  *ring_slots = S;
+  s[0] = {c->st_flags, E * T};
+  s[1] = {c->reset_step, sizeof(uint32_t) * E};
+  s[2] = {c->episode, sizeof(uint32_t) * E};
+  s[3] = {c->st_hyst, c->st_hyst ? sizeof(float) * E * (uint64_t)c->nh * Tp : 0};
+  s[4] = {c->st_drift, c->st_drift ? sizeof(float) * E * 6 * Tp : 0};
+  s[5] = {c->st_ring, sizeof(float) * E * 6 * Tp * S};
+  s[6] = {c->sn_h, c->sn_h ? sizeof(float4) * E * T : 0};
+  s[7] = {c->sn_d, c->sn_d ? sizeof(float2) * E * T : 0};
+  s[8] = {c->sm_h, c->sm_h ? sizeof(float) * E * M * 6 : 0};
+  s[9] = {c->sm_d, c->sm_d ? sizeof(float) * E * M * 3 : 0};
+  s[10] = {c->sh_on, nsh};
+  s[11] = {c->sh_e, sizeof(float4) * nsh};
+}
+
+StateHeader state_header(const ts_ctx* c, const StateSection s[kStateSections], uint32_t ring_slots) {
+  StateHeader h = {};
+  h.magic = kStateMagic; h.version = 1;
+  h.n_envs = (uint32_t)c->cfg.n_envs; h.n_taxels = (uint32_t)c->T; h.tp = (uint32_t)c->Tp; h.nh = (uint32_t)c->nh;
+  h.n_markers = (uint32_t)c->M; h.ring_slots = ring_slots; h.pc_n = c->sh_on ? (uint32_t)c->pc_n : 0u;
+  h.n_patches = (uint32_t)c->P; h.objs = (uint32_t)c->cfg.objs_per_env; h.gstep = c->gstep; h.n_sections = kStateSections;
+  h.total = sizeof(StateHeader);
+  for (int i = 0; i < kStateSections; ++i) { h.section_bytes[i] = s[i].bytes; h.total += (s[i].bytes + 15) & ~(uint64_t)15; }
+  return h;
+}
+}  // namespace
+
+ts_status ts_state_bytes(const ts_ctx* c, uint64_t* bytes) {
+  if (!c || !bytes) return TS_ERR_INVALID_ARG;
+  StateSection s[kStateSections]; uint32_t S;
+  state_sections(c, s, &S);
+  *bytes = state_header(c, s, S).total;
+  return TS_OK;
+}
+
+ts_status ts_get_state(ts_ctx* c, void* host_buf, uint64_t capacity, void* stream) {
+  if (!c) return TS_ERR_INVALID_ARG;
+  if (!host_buf) return fail(c, TS_ERR_INVALID_ARG, "ts_get_state: null buffer");
+  DeviceGuard guard(c->device);
+  StateSection s[kStateSections]; uint32_t S;
+  state_sections(c, s, &S);
+  const StateHeader h = state_header(c, s, S);
+  if (capacity < h.total) return fail(c, TS_ERR_INVALID_ARG, "ts_get_state: buffer smaller than ts_state_bytes");
+  std::memcpy(host_buf, &h, sizeof(h));
+  uint64_t off = sizeof(h);
+  for (int i = 0; i < kStateSections; ++i) {
+    if (s[i].bytes) TS_CUDA(c, cudaMemcpyAsync((char*)host_buf + off, s[i].dev, s[i].bytes, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    off += (s[i].bytes + 15) & ~(uint64_t)15;
+  }
+  TS_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
+  return TS_OK;
+}
+
+ts_status ts_set_state(ts_ctx* c, const void* host_buf, uint64_t bytes, void* stream) {
+  if (!c) return TS_ERR_INVALID_ARG;
+  if (!host_buf || bytes < sizeof(StateHeader)) return fail(c, TS_ERR_INVALID_ARG, "ts_set_state: no header");
+  DeviceGuard guard(c->device);
+  StateSection s[kStateSections]; uint32_t S;
+  state_sections(c, s, &S);
+  const StateHeader want = state_header(c, s, S);
+  StateHeader h;
+  std::memcpy(&h, host_buf, sizeof(h));
+  if (h.magic != kStateMagic || h.version != 1) return fail(c, TS_ERR_INVALID_ARG, "ts_set_state: not a ts state blob");
+  bool same = h.total == want.total && bytes >= h.total && h.n_envs == want.n_envs && h.n_taxels == want.n_taxels && h.tp == want.tp &&
+              h.nh == want.nh && h.n_markers == want.n_markers && h.ring_slots == want.ring_slots && h.pc_n == want.pc_n &&
+              h.n_patches == want.n_patches && h.objs == want.objs && h.n_sections == want.n_sections;
+  for (int i = 0; same && i < kStateSections; ++i) same = h.section_bytes[i] == want.section_bytes[i];
+  if (!same) return fail(c, TS_ERR_INVALID_ARG, "ts_set_state: blob was taken from a ctx with another configuration");
+  uint64_t off = sizeof(h);
+  for (int i = 0; i < kStateSections; ++i) {
+    if (s[i].bytes) TS_CUDA(c, cudaMemcpyAsync(s[i].dev, (const char*)host_buf + off, s[i].bytes, cudaMemcpyHostToDevice, (cudaStream_t)stream));
+    off += (s[i].bytes + 15) & ~(uint64_t)15;
+  }
+  TS_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
+  c->gstep = h.gstep;
+  return TS_OK;
+}
+
 ts_status ts_kernel_times_ms(ts_ctx* c, float* out_ms, int32_t capacity, int32_t* n_steps) {
   if (!c) return TS_ERR_INVALID_ARG;
   DeviceGuard guard(c->device);

@@ -1608,8 +1608,8 @@ __global__ void __launch_bounds__(256) ts_shear_kernel(const __grid_constant__ T
   __shared__ double Rm[9], tv[3];
   __shared__ float4 qd[TS_SHEAR_Q];   // (tangential slide x, y, z, h_p)
   __shared__ float4 qz[TS_SHEAR_Q];   // z_p relative to the pad centre
-  __shared__ int qn;
-  const int e = blockIdx.x / p.P, pi = blockIdx.x - e * p.P, tid = threadIdx.x;
+  __shared__ int wcnt[2][8];          // anchored points per warp of the current pass (double-buffered by pass parity)
+  const int e = blockIdx.x / p.P, pi = blockIdx.x - e * p.P, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const TsPatch& pt = p.patches[pi];
   const int mcount = __ldg(&pt.mnu) * __ldg(&pt.mnv), link = __ldg(&pt.link);
   if (mcount == 0 || link < 0) return;
@@ -1625,10 +1625,10 @@ __global__ void __launch_bounds__(256) ts_shear_kernel(const __grid_constant__ T
     const float4 mp = __ldg(p.mk_pos + __ldg(&pt.mstart) + tid);
     mx = mp.x - ctr.x; my = mp.y - ctr.y; mz = mp.z - ctr.z;
   }
+  int qn = 0;                            // queue fill: the same value in every thread (block-uniform)
   auto shear_drain = [&]() {             // phase C over the queued points (call between barriers)
-    const int nq = qn;
     if (tid >= mcount) return;
-    for (int s2 = 0; s2 < nq; ++s2) {
+    for (int s2 = 0; s2 < qn; ++s2) {
       const float4 d4 = qd[s2], z4 = qz[s2];
       const float rx = mx - z4.x, ry = my - z4.y, rz = mz - z4.z;
       const float rn = fmaf(rx, na.x, fmaf(ry, na.y, rz * na.z));
@@ -1637,12 +1637,12 @@ __global__ void __launch_bounds__(256) ts_shear_kernel(const __grid_constant__ T
       ax = fmaf(wgt, d4.x, ax); ay = fmaf(wgt, d4.y, ay); az = fmaf(wgt, d4.z, az);
     }
   };
+  int pass = 0;
   for (int k = 0; k < p.K; ++k) {
     const int id = __ldg(p.pc_id + (size_t)e * p.K + k);   // block-uniform
     if (id < 0) continue;
     __syncthreads();
     if (tid == 0) {
-      qn = 0;
       const size_t el = (size_t)e * p.L + link, ek = (size_t)e * p.K + k;
       double RL[9], RO[9];
       quat_Rd(p.link_quat + el * 4, RL);
@@ -1655,43 +1655,61 @@ __global__ void __launch_bounds__(256) ts_shear_kernel(const __grid_constant__ T
     }
     __syncthreads();
     const size_t sbase = (((size_t)e * p.P + pi) * p.K + k) * N;
-    for (int i0 = 0; i0 < N; i0 += 256) {
-      if (i0) {                              // one pass queues at most 256 points: drain before the queue could overflow
+    for (int i0 = 0; i0 < N; i0 += 256, ++pass) {
+      if (qn > TS_SHEAR_Q - 256) {           // a pass queues at most 256 points: drain before the queue could overflow
         __syncthreads();
-        if (qn > TS_SHEAR_Q - 256) {         // block-uniform
-          shear_drain();
-          __syncthreads();
-          if (tid == 0) qn = 0;
-          __syncthreads();
-        }
+        shear_drain();
+        qn = 0;
+        __syncthreads();
       }
       const int i = i0 + tid;
-      if (i >= N) continue;
-      const float4 po = __ldg(p.pc_raw + (size_t)id * N + i);
-      const D3 z = D3{tv[0], tv[1], tv[2]} + mulR(Rm, D3{(double)po.x, (double)po.y, (double)po.z});
-      const D3 rel = z - xc;
-      double phi_el = __longlong_as_double(0x7ff0000000000000LL);
-      if (fabs(dot(rel, uu)) <= hu && fabs(dot(rel, vv)) <= hv) phi_el = dot(rel, n);
-      uint8_t on = p.sh_on[sbase + i];
-      float4 anc;
-      if (!on && phi_el < -(double)p.eta_enter) {
-        on = 1; anc = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
-        p.sh_on[sbase + i] = 1; p.sh_e[sbase + i] = anc;
-      } else if (on && phi_el > (double)p.eta_exit) {
-        on = 0; p.sh_on[sbase + i] = 0;
-      } else if (on) {
-        anc = p.sh_e[sbase + i];
+      bool push = false;
+      float4 vd = make_float4(0.f, 0.f, 0.f, 0.f), vz = vd;
+      if (i < N) {
+        const float4 po = __ldg(p.pc_raw + (size_t)id * N + i);
+        const D3 z = D3{tv[0], tv[1], tv[2]} + mulR(Rm, D3{(double)po.x, (double)po.y, (double)po.z});
+        const D3 rel = z - xc;
+        double phi_el = __longlong_as_double(0x7ff0000000000000LL);
+        if (fabs(dot(rel, uu)) <= hu && fabs(dot(rel, vv)) <= hv) phi_el = dot(rel, n);
+        uint8_t on = p.sh_on[sbase + i];
+        float4 anc = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (!on && phi_el < -(double)p.eta_enter) {
+          on = 1; anc = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
+          p.sh_on[sbase + i] = 1; p.sh_e[sbase + i] = anc;
+        } else if (on && phi_el > (double)p.eta_exit) {
+          on = 0; p.sh_on[sbase + i] = 0;
+        } else if (on) {
+          anc = p.sh_e[sbase + i];
+        }
+        if (on && phi_el < 0.0) {
+          const D3 dz = D3{rel.x - (double)anc.x, rel.y - (double)anc.y, rel.z - (double)anc.z};
+          const D3 dzt = dz - dot(dz, n) * n;                          // Pi_n(z_p - e_p)
+          push = true;
+          vd = make_float4((float)dzt.x, (float)dzt.y, (float)dzt.z, (float)(-phi_el));
+          vz = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
+        }
       }
-      if (on && phi_el < 0.0) {
-        const D3 dz = D3{rel.x - (double)anc.x, rel.y - (double)anc.y, rel.z - (double)anc.z};
-        const D3 dzt = dz - dot(dz, n) * n;                          // Pi_n(z_p - e_p)
-        const int slot = atomicAdd(&qn, 1);                          // < TS_SHEAR_Q by the drain rule above
-        qd[slot] = make_float4((float)dzt.x, (float)dzt.y, (float)dzt.z, (float)(-phi_el));
-        qz[slot] = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
+      // Ordered compaction: the queue holds the anchored points in index order, so the fp32 sums below are the same from
+      // run to run (a shared-memory atomic counter would enqueue in arrival order).
+      const unsigned bal = __ballot_sync(TS_FULL, push);
+      if (lane == 0) wcnt[pass & 1][warp] = __popc(bal);
+      __syncthreads();
+      int base = qn, tot = 0;
+#pragma unroll
+      for (int w2 = 0; w2 < 8; ++w2) {
+        const int c2 = wcnt[pass & 1][w2];
+        if (w2 < warp) base += c2;
+        tot += c2;
       }
+      if (push) {
+        const int slot = base + __popc(bal & ((1u << lane) - 1u));     // < TS_SHEAR_Q by the drain rule above
+        qd[slot] = vd; qz[slot] = vz;
+      }
+      qn += tot;
     }
     __syncthreads();
     shear_drain();
+    qn = 0;
   }
   if (tid < mcount && (ax != 0.f || ay != 0.f || az != 0.f)) {
     float* o = p.marker + ((size_t)e * p.M + __ldg(&pt.mstart) + tid) * 3;

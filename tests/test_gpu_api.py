@@ -255,3 +255,51 @@ def test_chained_launches_equal_serialised_steps():
     for r in res[1:]:
         for k in res[0]:
             assert torch.equal(res[0][k], r[k]), k
+
+
+def test_checkpoint_resume_is_bit_exact():
+    """ts_get_state / ts_set_state: a blob taken after 6 steps (a masked reset among them) restores into a FRESH ctx of
+    the same configuration, which then produces the same 6 further steps bit for bit: Schmitt bits, Maxwell hysteresis,
+    drift, the read-delay ring, the noisy scalar readouts' state, the shear anchors and every counter travel with it.
+    A blob from another configuration is refused and leaves the ctx untouched."""
+    import torch
+    from paper_2606_22332_b200.binding import TactileSim, TsError
+    w = W.config(5, n_envs=48)
+    pts, cid = W.point_cloud_bank(w, 500)
+    noise = dict(w.noise, hyst_mode="maxwell", beta=0.5, tau=0.05, read_delay=2, read_jitter=1, sigma_white_force=2e-3,
+                 radius_noise=3e-4, sigma_rw_depth=1e-5, sigma_white_prox=1e-3, sigma_rw_marker=1e-5, quant_marker=1e-4)
+    outs = tuple(w.outputs) + ("depth_noisy", "prox_noisy", "marker_noisy")
+
+    def make():
+        s = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=dict(w.physics, shear_enable=1), noise=noise, outputs=outs)
+        s.set_geometry(w.types, w.params, w.bank, w.voxel)
+        s.set_pointclouds(pts, cid)
+        return s
+
+    a = make()
+    for s in range(6):
+        if s == 3:
+            a.reset(torch.from_numpy((np.arange(w.E) % 3 == 0).astype(np.uint8)).cuda())
+        a.step(a.upload(w.inputs(s)))
+    blob = a.get_state()
+    assert blob.nbytes == a.state_bytes() and blob.nbytes > w.E * w.T * 50
+    want = []
+    for s in range(6, 12):
+        want.append({k: v.clone() for k, v in a.step(a.upload(w.inputs(s))).items()})
+    b = make()
+    b.step(b.upload(w.inputs(0)))                      # some other history first: the blob must overwrite all of it
+    b.set_state(blob)
+    for i, s in enumerate(range(6, 12)):
+        got = b.step(b.upload(w.inputs(s)))
+        torch.cuda.synchronize()
+        for k in got:
+            assert torch.equal(got[k], want[i][k]), (k, s)
+    # a ctx with another configuration refuses the blob
+    c = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=w.physics, noise=w.noise, outputs=w.outputs)
+    c.set_geometry(w.types, w.params, w.bank, w.voxel)
+    assert c.state_bytes() != blob.nbytes
+    with pytest.raises(TsError):
+        c.set_state(blob)
+    with pytest.raises(TsError):
+        c.set_state(blob[:64])
+    a.close(); b.close(); c.close()
