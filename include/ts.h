@@ -330,7 +330,30 @@ ts_status ts_state_bytes(const ts_ctx* ctx, uint64_t* bytes);
 ts_status ts_get_state(ts_ctx* ctx, void* host_buf, uint64_t capacity, void* stream);
 ts_status ts_set_state(ts_ctx* ctx, const void* host_buf, uint64_t bytes, void* stream);
 
-/* Last error text of this ctx (or of the last failed ts_create when ctx is NULL).  Never NULL. */
+/* Allocation-free entry point, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it).  It needs no ctx and calls no cudaMalloc, cudaFree or allocating library routine:
+ * the contact depth d = [R_j - phi(x_o)]_+ (App. A.1-A.2, Eq. 1-2) of every (env, taxel) against ONE analytic primitive
+ * per env (TS_GEOM_SPHERE / BOX / CAPSULE; any other type reads as "no object", depth 0), the same arithmetic as the
+ * depth output of the ctx path.  Its only scratch, the relative pose of every (env, link), lives in a static device array
+ * of TS_STATIC_SCRATCH_BYTES (8 MiB) inside the library, which every GPU that loads the library holds until the process
+ * exits: n_envs * n_links <= TS_STATIC_MAX_FRAMES, anything larger returns TS_ERR_INVALID_ARG with the limit in
+ * the error text (read it with a NULL ctx below).  Runs on the CURRENT device, on `stream`; two kernels are enqueued, nothing
+ * synchronises.  All calls on a device share that array: calls on one stream are ordered and each call overwrites what it
+ * reads (nothing has to be cleared between calls), but calls that overlap on the GPU (different streams without an
+ * event between them) race on it.
+ * All pointers are DEVICE pointers, caller-owned, row-major fp32 / int32:
+ *   taxel_pos [T,3] link-frame positions, taxel_radius [T] R_j (<= 0: filler, depth 0), taxel_link [T] link of each
+ *   taxel (outside [0, n_links): depth 0)  -- the pos / radius / link arrays of ts_layout_view, copied to the device;
+ *   link_pos [E,L,3], link_quat [E,L,4] (w,x,y,z), obj_pos [E,3], obj_quat [E,4];
+ *   geom_type [E] int32, geom_params [E,4] (16-byte aligned) as in ts_geometry with objs_per_env = 1;
+ *   depth [E,T] out. */
+enum { TS_STATIC_SCRATCH_BYTES = 8 << 20, TS_STATIC_MAX_FRAMES = (8 << 20) / 96 };
+ts_status ts_depth_static(int32_t n_envs, int32_t n_links, int32_t n_taxels, const float* taxel_pos, const float* taxel_radius,
+                          const int32_t* taxel_link, const float* link_pos, const float* link_quat, const float* obj_pos,
+                          const float* obj_quat, const int32_t* geom_type, const float* geom_params, float* depth, void* stream);
+
+/* Last error text of this ctx (with a NULL ctx: of the last failed ctx-free call of this thread, i.e. ts_create or
+ * ts_depth_static).  Never NULL. */
 const char* ts_last_error(const ts_ctx* ctx);
 
 /* Introspection used by the binding and the bench. */

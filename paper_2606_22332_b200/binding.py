@@ -12,6 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libts.so")
 
 TS_OK = 0
+TS_ERR_INVALID_ARG = 1
 STATUS = {0: "TS_OK", 1: "TS_ERR_INVALID_ARG", 2: "TS_ERR_CUDA", 3: "TS_ERR_OOM", 4: "TS_ERR_STATE",
           5: "TS_ERR_UNSUPPORTED"}
 HYST = {"off": 0, "maxwell": 1, "asym": 2}
@@ -27,7 +28,9 @@ SYMBOLS = ["ts_layout_create", "ts_layout_add_patch", "ts_layout_filter_links", 
            "ts_layout_destroy", "ts_config_default", "ts_create", "ts_set_geometry", "ts_set_pointclouds", "ts_set_meshes", "ts_step", "ts_step_host",
            "ts_reset", "ts_destroy", "ts_last_error", "ts_n_taxels", "ts_n_markers", "ts_launches_per_step",
            "ts_kernel_time_ms", "ts_kernel_times_ms", "ts_first_kernel_time_ms", "ts_version",
-           "ts_state_bytes", "ts_get_state", "ts_set_state"]
+           "ts_state_bytes", "ts_get_state", "ts_set_state", "ts_depth_static"]
+STATIC_SCRATCH_BYTES = 8 << 20                      # include/ts.h TS_STATIC_SCRATCH_BYTES
+STATIC_MAX_FRAMES = STATIC_SCRATCH_BYTES // 96      # TS_STATIC_MAX_FRAMES
 
 
 class TsError(RuntimeError):
@@ -143,6 +146,7 @@ def lib():
         L.ts_state_bytes.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.ts_get_state.argtypes = [vp, vp, C.c_uint64, vp]
         L.ts_set_state.argtypes = [vp, vp, C.c_uint64, vp]
+        L.ts_depth_static.argtypes = [i32, i32, i32] + [vp] * 11
         L.ts_first_kernel_time_ms.restype = C.c_float
         L.ts_version.restype = C.c_char_p
         _lib = L
@@ -233,6 +237,17 @@ def make_config(n_envs, n_links, objs_per_env, layout, physics=None, noise=None,
     if outputs is not None:
         cfg.output_mask = sum(OUT_BITS[o] for o in outputs)
     return cfg
+
+
+def depth_static(n_envs, n_links, n_taxels, taxel_pos, taxel_radius, taxel_link, link_pos, link_quat, obj_pos, obj_quat,
+                 geom_type, geom_params, depth, stream=None):
+    """ts_depth_static on device tensors (anything with data_ptr(); fp32 / int32, contiguous): the allocation-free contact
+    depth against one primitive per env, on the current device.  Marshalling only; `stream` is a raw cudaStream_t or None."""
+    ptr = lambda t: C.c_void_p(t.data_ptr() if t is not None else 0)
+    st = lib().ts_depth_static(int(n_envs), int(n_links), int(n_taxels), ptr(taxel_pos), ptr(taxel_radius), ptr(taxel_link),
+                               ptr(link_pos), ptr(link_quat), ptr(obj_pos), ptr(obj_quat), ptr(geom_type), ptr(geom_params),
+                               ptr(depth), C.c_void_p(stream or 0))
+    _check(st, None, "ts_depth_static")
 
 
 class TactileSim:

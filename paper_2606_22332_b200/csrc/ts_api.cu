@@ -887,6 +887,27 @@ ts_status ts_reset(ts_ctx* c, const uint8_t* env_mask_dev, void* stream) {
   return TS_OK;
 }
 
+// ---- allocation-free contact depth (include/ts.h) -----------------------------------------------------------------
+ts_status ts_depth_static(int32_t n_envs, int32_t n_links, int32_t n_taxels, const float* taxel_pos, const float* taxel_radius,
+                          const int32_t* taxel_link, const float* link_pos, const float* link_quat, const float* obj_pos,
+                          const float* obj_quat, const int32_t* geom_type, const float* geom_params, float* depth, void* stream) {
+  // sizes first: nothing below this block runs, and no CUDA call is made, for a request the static scratch cannot hold
+  if (n_envs <= 0 || n_links <= 0 || n_taxels <= 0) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_depth_static: sizes must be positive");
+  if ((long long)n_envs * n_links > (long long)TS_STATIC_MAX_FRAMES)
+    return fail(nullptr, TS_ERR_INVALID_ARG, "ts_depth_static: n_envs * n_links = " + std::to_string((long long)n_envs * n_links) +
+                " exceeds TS_STATIC_MAX_FRAMES = " + std::to_string((long long)TS_STATIC_MAX_FRAMES) +
+                " (the static scratch array holds " + std::to_string((long long)TS_STATIC_SCRATCH_BYTES) + " bytes)");
+  if ((long long)n_envs * n_taxels >= (1LL << 40)) return fail(nullptr, TS_ERR_INVALID_ARG, "ts_depth_static: n_envs * n_taxels too large");
+  if (!taxel_pos || !taxel_radius || !taxel_link || !link_pos || !link_quat || !obj_pos || !obj_quat || !geom_type || !geom_params || !depth)
+    return fail(nullptr, TS_ERR_INVALID_ARG, "ts_depth_static: null pointer");
+  if ((reinterpret_cast<uintptr_t>(geom_params) & 15u) || (reinterpret_cast<uintptr_t>(link_quat) & 15u) || (reinterpret_cast<uintptr_t>(obj_quat) & 15u))
+    return fail(nullptr, TS_ERR_INVALID_ARG, "ts_depth_static: link_quat, obj_quat and geom_params must be 16-byte aligned");
+  const cudaError_t e = (cudaError_t)ts_static_depth_launch(n_envs, n_links, n_taxels, taxel_pos, taxel_radius, taxel_link, link_pos, link_quat,
+                                                            obj_pos, obj_quat, geom_type, geom_params, depth, stream);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "ts_depth_static");
+  return TS_OK;
+}
+
 // ---- checkpoint / resume ----------------------------------------------------------------------------------------
 namespace {
 constexpr int kStateSections = 12;

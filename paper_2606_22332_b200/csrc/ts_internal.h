@@ -206,5 +206,10 @@ int ts_launch_reset_state(const TsStepParams& p, const uint8_t* mask, uint32_t d
 unsigned long long ts_bank_elems_per_grid(int N);
 unsigned long long ts_step_smem_bytes(const TsStepParams& p);
 int ts_prepare_kernels(int device, int smem_bytes);
+// ts_depth_static: pose kernel + depth kernel on the current device with the poses in the library's static scratch
+// array (sizes as in include/ts.h: TS_STATIC_SCRATCH_BYTES, TS_STATIC_MAX_FRAMES); returns a cudaError_t.
+int ts_static_depth_launch(int E, int L, int T, const float* taxel_pos, const float* taxel_radius, const int32_t* taxel_link,
+                           const float* link_pos, const float* link_quat, const float* obj_pos, const float* obj_quat,
+                           const int32_t* geom_type, const float* geom_params, float* depth, void* stream);
 
 #endif  // TS_INTERNAL_H_

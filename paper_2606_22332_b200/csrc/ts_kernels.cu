@@ -2043,3 +2043,119 @@ int ts_launch_reset_state(const TsStepParams& p, const uint8_t* mask, uint32_t t
   ts_reset_state_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(p, mask, thr, nh);
   return (int)cudaGetLastError();
 }
+
+// =======================================================================================
+// ts_depth_static (include/ts.h): the contact-depth readout S1-S4 for analytic primitives with NO device allocation.
+// It is the ctx-free variant of the frames-kernel -> step-kernel pair: the relative poses (the scratch that the ctx
+// path keeps in the cudaMalloc'd frames_g) live in the file-scope array below, which every GPU that loads this library
+// holds until the process exits.  Callers that cannot call cudaMalloc (graph capture, serving loops) use it.
+// All calls on a device share the array; a call's pose kernel overwrites every record its depth kernel reads, so nothing
+// in it needs to start at zero and nothing is cleared; two calls that overlap on the GPU (different streams) race on it.
+// =======================================================================================
+struct TsStaticFrame {   // 96 bytes: x_o = c + M x_j (link frame -> object frame), as FrameS::M / FrameS::c
+  double M[9];
+  double c[3];
+};
+static_assert(sizeof(TsStaticFrame) == 96 && TS_STATIC_SCRATCH_BYTES / sizeof(TsStaticFrame) == TS_STATIC_MAX_FRAMES,
+              "static scratch layout");
+
+// In host code this name is only a handle for cudaGetSymbolAddress; it is NOT a device address.
+static __device__ __align__(256) unsigned char ts_static_scratch[TS_STATIC_SCRATCH_BYTES];
+
+namespace {
+// One thread per (env, link): M = R_O^T R_L, c = R_O^T (p_L - p_O) in double (Eq. 1; p_L - p_O formed before
+// rotating, as in build_frame_row).
+__global__ void __launch_bounds__(128) ts_static_frames_kernel(TsStaticFrame* __restrict__ fr, int E, int L, const float* __restrict__ link_pos,
+                                                               const float* __restrict__ link_quat, const float* __restrict__ obj_pos,
+                                                               const float* __restrict__ obj_quat) {
+  const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+  if (gt >= E * L) return;
+  const int e = gt / L;
+  double RL[9], RO[9];
+  quat_Rd(link_quat + (size_t)gt * 4, RL);
+  quat_Rd(obj_quat + (size_t)e * 4, RO);
+  const D3 d = ld3d(link_pos + (size_t)gt * 3) - ld3d(obj_pos + (size_t)e * 3);
+  TsStaticFrame F;
+#pragma unroll
+  for (int r = 0; r < 3; ++r) {   // row r of R_O^T = column r of R_O
+    const double o0 = RO[r], o1 = RO[3 + r], o2 = RO[6 + r];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) F.M[r * 3 + c] = fma(o0, RL[c], fma(o1, RL[3 + c], o2 * RL[6 + c]));
+    F.c[r] = fma(o0, d.x, fma(o1, d.y, o2 * d.z));
+  }
+  fr[gt] = F;
+}
+
+// The primitive cases of phi_d (O2), same expressions.
+__device__ __forceinline__ double phi_prim_d(int type, float4 prm, D3 x) {
+  if (type == TS_GEOM_SPHERE) return dsqrt_n(dot(x, x)) - (double)prm.x;
+  if (type == TS_GEOM_BOX) {
+    const double wx = fabs(x.x) - (double)prm.x, wy = fabs(x.y) - (double)prm.y, wz = fabs(x.z) - (double)prm.z;
+    const double px = fmax(wx, 0.0), py = fmax(wy, 0.0), pz = fmax(wz, 0.0);
+    return dsqrt_n(fma(px, px, fma(py, py, pz * pz))) + fmin(fmax(wx, fmax(wy, wz)), 0.0);
+  }
+  if (type == TS_GEOM_CAPSULE) {
+    const double h = (double)prm.y;
+    const double zc = fmin(fmax(x.z, -h), h);
+    const D3 y = D3{x.x, x.y, x.z - zc};
+    return dsqrt_n(dot(y, y)) - (double)prm.x;
+  }
+  return __longlong_as_double(0x7ff0000000000000LL);   // no object (or a type this entry point does not serve): depth 0
+}
+
+// One thread per (env, taxel): d = [R_j - phi(c + M x_j)]_+ (Eq. 2), rounded once.
+__global__ void __launch_bounds__(256) ts_static_depth_kernel(const TsStaticFrame* __restrict__ fr, int E, int L, int T,
+                                                              const float* __restrict__ taxel_pos, const float* __restrict__ taxel_radius,
+                                                              const int32_t* __restrict__ taxel_link, const int32_t* __restrict__ geom_type,
+                                                              const float* __restrict__ geom_params, float* __restrict__ depth) {
+  const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gt >= (long long)E * T) return;
+  const int e = (int)(gt / T), j = (int)(gt - (long long)e * T);
+  const float Rj = __ldg(taxel_radius + j);
+  const int link = __ldg(taxel_link + j);
+  float d = 0.f;
+  if (Rj > 0.f && link >= 0 && link < L) {
+    const TsStaticFrame& F = fr[(size_t)e * L + link];
+    const D3 xj = ld3d(taxel_pos + (size_t)j * 3);
+    const D3 x = ldv(F.c) + mulR(F.M, xj);
+    const float4 prm = __ldg(reinterpret_cast<const float4*>(geom_params) + e);
+    const double dd = (double)Rj - phi_prim_d(__ldg(geom_type + e), prm, x);
+    d = dd > 0.0 ? (float)dd : 0.f;
+  }
+  depth[gt] = d;
+}
+
+// Device address of ts_static_scratch, looked up once per device with that device current.
+std::mutex g_static_mu;
+void* g_static_ptr[64] = {};
+}  // namespace
+
+int ts_static_depth_launch(int E, int L, int T, const float* taxel_pos, const float* taxel_radius, const int32_t* taxel_link,
+                           const float* link_pos, const float* link_quat, const float* obj_pos, const float* obj_quat,
+                           const int32_t* geom_type, const float* geom_params, float* depth, void* stream) {
+  if ((long long)E * L > (long long)TS_STATIC_MAX_FRAMES) return (int)cudaErrorInvalidValue;   // the caller checked already
+  int dev = -1;
+  cudaError_t err = cudaGetDevice(&dev);
+  if (err != cudaSuccess) return (int)err;
+  if (dev < 0 || dev >= 64) return (int)cudaErrorInvalidDevice;
+  void* ptr = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {   // set-up, once per device: the symbol's address ON THIS DEVICE (no allocation happens here)
+      void* q = nullptr;
+      err = cudaGetSymbolAddress(&q, ts_static_scratch);
+      if (err != cudaSuccess) return (int)err;
+      g_static_ptr[dev] = q;
+    }
+    ptr = g_static_ptr[dev];
+  }
+  TsStaticFrame* fr = static_cast<TsStaticFrame*>(ptr);
+  const cudaStream_t st = (cudaStream_t)stream;
+  ts_static_frames_kernel<<<(unsigned)((E * L + 127) / 128), 128, 0, st>>>(fr, E, L, link_pos, link_quat, obj_pos, obj_quat);
+  err = cudaGetLastError();
+  if (err != cudaSuccess) return (int)err;
+  const long long n = (long long)E * T;
+  ts_static_depth_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(fr, E, L, T, taxel_pos, taxel_radius, taxel_link, geom_type,
+                                                                      geom_params, depth);
+  return (int)cudaGetLastError();
+}
