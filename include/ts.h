@@ -275,7 +275,7 @@ ts_status ts_set_geometry(ts_ctx* ctx, const ts_geometry* geo, void* stream);
 /* App. A.6: "tracked links are sampled into a surface point cloud at scene reset and organized in a static BVH".
  * Here: a bank of n_clouds clouds of n_points points each, in the OBJECT frame (host fp32 [G,N,3]), and the cloud of every
  * (env, object) (host int32 [E,K], -1 = not tracked).  The ctx sorts each cloud into a uniform grid of cell size
- * pc_radius (the static spatial index; a taxel's sensing sphere meets at most 27 cells) and keeps it on the device.
+ * pc_radius / 2 (the static spatial index; a taxel's sensing sphere meets at most 125 cells) and keeps it on the device.
  * Needed before a ts_step that asks for TS_OUT_PROXPC.  Synchronises `stream` once; may be called again. */
 typedef struct ts_pointclouds {
   int32_t n_clouds, n_points;

@@ -689,9 +689,9 @@ ts_status ts_set_pointclouds(ts_ctx* c, const ts_pointclouds* pc, void* stream) 
   for (size_t i = 0; i < EK; ++i)
     if (pc->cloud_id[i] >= G) return fail(c, TS_ERR_INVALID_ARG, "ts_set_pointclouds: cloud id out of range");
   if ((long long)G * N >= (1LL << 31)) return fail(c, TS_ERR_UNSUPPORTED, "ts_set_pointclouds: bank larger than 2^31 points");
-  // static spatial index ("organized in a static BVH"): per cloud a uniform grid with cell = sensing radius,
+  // static spatial index ("organized in a static BVH"): per cloud a uniform grid with cell = sensing radius / TS_PC_REACH,
   // points counting-sorted by linear cell index (x fastest), cell_start[ncell + 1]
-  const float cell = c->cfg.pc_radius;
+  const float cell = c->cfg.pc_radius / (float)TS_PC_REACH;
   std::vector<TsPcGrid> grids(G);
   std::vector<int32_t> cells;
   std::vector<float4> sorted((size_t)G * N);

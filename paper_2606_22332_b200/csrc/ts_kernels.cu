@@ -1512,86 +1512,139 @@ __global__ void ts_reset_scalar_kernel(const __grid_constant__ TsStepParams p, c
 // ---------------------------------------------------------------------------------------
 // App. A.6 point-cloud ProximityTaxel (Eq. 12-17).  One thread per (env, taxel).
 // The tracked points are static in their object's frame, so each cloud was sorted once into a uniform grid of cell
-// size R_j (ts_set_pointclouds): the taxel centre is taken into the object frame (double), the 27 cells around it are
-// scanned, and of the points inside the sensing sphere only two sums are kept,
+// size R_j / TS_PC_REACH (ts_set_pointclouds): the taxel centre is taken into the object frame (double), the rows of
+// cells that reach into its sensing sphere are scanned, and of the points inside the sensing sphere only two sums are kept,
 //     S0 = sum_i P_ij,   S1 = sum_i P_ij (p_i - q_j)          (P_ij = R_j - |p_i - q_j|, Eq. 12)
 // because Eq. 13-17 are linear in p_i:  v_p,i - v_tax = A + w_O x (p_i - q_j),  A = v_O + w_O x (q_j - p_O) - v_tax, so
 //     sum_i P_ij v_t,ij = Pi_a (S0 A + w_O x S1),   f^w = k rho S0 a + k_s rho Pi_a(...),   tau^w = k rho S1 x a.
-// Same result as the per-point sums of the paper up to rounding order.  Distances in fp32 on fp32 differences of
-// nearby points, the sums in double.
+// Same result as the per-point sums of the paper up to rounding order.  Distances and the two sums in fp32 on fp32
+// differences of nearby points (a few hundred terms of bounded size: ~1e-6 relative), the rest in double.
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) ts_proxpc_kernel(const __grid_constant__ TsStepParams p) {
+#ifndef TS_PC_GROUP
+#define TS_PC_GROUP 4   // lanes that scan one taxel's neighbourhood together (32 / TS_PC_GROUP taxels per warp round)
+#endif
+// The scan is bound by the latency of its dependent loads (run bounds -> points), so residency matters more than
+// registers: 12 blocks of 128 threads per SM (40 registers; the double-precision pose data that lives across the scan is
+// spilled around it) runs 1.40 ms where 4 blocks (128 registers, nothing spilled) run 2.62 ms (config-4 scene, 4,096 envs).
+#ifndef TS_PC_MINB
+#define TS_PC_MINB 12
+#endif
+__global__ void __launch_bounds__(128, TS_PC_MINB) ts_proxpc_kernel(const __grid_constant__ TsStepParams p) {
+  // Thread = (env, taxel) for the pose arithmetic and the force / torque; the SCAN of a taxel's neighbourhood is shared
+  // by TS_PC_GROUP lanes: a thread-per-taxel scan runs every warp to its longest neighbourhood at ~14 of 32 lanes (ncu),
+  // the shared scan keeps the lanes busy and splits each run of points.  Every lane of the warp stays in the kernel
+  // (shuffles below): threads past the end and filler taxels carry ok = false.
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gt >= (long long)p.E * p.T) return;
-  const int e = (int)(gt / p.T), j = (int)(gt - (long long)e * p.T);
+  const bool in_range = gt < (long long)p.E * p.T;
+  const int lane = threadIdx.x & 31;
+  const int e = in_range ? (int)(gt / p.T) : 0, j = in_range ? (int)(gt - (long long)e * p.T) : 0;
   const float4 P4 = __ldg(p.tx_pos + j);
+  const bool act = in_range && P4.w > 0.f;
   float out[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  if (P4.w > 0.f) {
+  double RL[9];
+  D3 pL = D3{0.0, 0.0, 0.0}, q = pL, a = pL, vtax = pL;
+  double rho = 0.0;
+  if (act) {
     const int pidx = __ldg(p.tx_patch + j);
     const TsPatch& pt = p.patches[pidx];
     const int link = __ldg(&pt.link);
     const float4 na = __ldg(&pt.na);
     const size_t el = (size_t)e * p.L + link;
-    double RL[9];
     quat_Rd(p.link_quat + el * 4, RL);
-    const D3 pL = ld3d(p.link_pos + el * 3);
-    const D3 q = pL + mulR(RL, D3{(double)P4.x, (double)P4.y, (double)P4.z});       // Eq. 1
-    const D3 a = mulR(RL, D3{(double)na.x, (double)na.y, (double)na.z});
-    const D3 vtax = ld3d(p.link_linvel + el * 3) + cross(ld3d(p.link_angvel + el * 3), q - pL);   // Eq. 13
+    pL = ld3d(p.link_pos + el * 3);
+    q = pL + mulR(RL, D3{(double)P4.x, (double)P4.y, (double)P4.z});       // Eq. 1
+    a = mulR(RL, D3{(double)na.x, (double)na.y, (double)na.z});
+    vtax = ld3d(p.link_linvel + el * 3) + cross(ld3d(p.link_angvel + el * 3), q - pL);   // Eq. 13
     long long n_track = 0;
     for (int k = 0; k < p.K; ++k) n_track += __ldg(p.pc_id + (size_t)e * p.K + k) >= 0 ? p.pc_n : 0;
-    const double rho = (double)p.pc_density / (double)(n_track > 0 ? n_track : 1);          // Eq. 15 (Q27)
-    const float R = p.pc_radius, R2 = R * R;
-    D3 fw = D3{0.0, 0.0, 0.0}, tw = D3{0.0, 0.0, 0.0};
-    for (int k = 0; k < p.K; ++k) {
-      const int id = __ldg(p.pc_id + (size_t)e * p.K + k);
-      if (id < 0) continue;
-      const size_t ek = (size_t)e * p.K + k;
-      double RO[9];
+    rho = (double)p.pc_density / (double)(n_track > 0 ? n_track : 1);          // Eq. 15 (Q27)
+  }
+  const float R = p.pc_radius, R2 = R * R;
+  D3 fw = D3{0.0, 0.0, 0.0}, tw = D3{0.0, 0.0, 0.0};
+  for (int k = 0; k < p.K; ++k) {   // warp-uniform
+    const size_t ek = (size_t)e * p.K + k;
+    const int id = act ? __ldg(p.pc_id + ek) : -1;
+    double RO[9];
+    D3 pO = D3{0.0, 0.0, 0.0};
+    float xf = 0.f, yf = 0.f, zf = 0.f;
+    if (id >= 0) {
       quat_Rd(p.obj_quat + ek * 4, RO);
-      const D3 pO = ld3d(p.obj_pos + ek * 3);
+      pO = ld3d(p.obj_pos + ek * 3);
       const D3 xd = mulRT(RO, q - pO);                                                       // taxel centre, object frame
-      const float xf = (float)xd.x, yf = (float)xd.y, zf = (float)xd.z;
-      const TsPcGrid g = p.pc_grid[id];
-      const int ci = (int)floorf((xf - g.ox) * g.inv_cell), cj = (int)floorf((yf - g.oy) * g.inv_cell), ck = (int)floorf((zf - g.oz) * g.inv_cell);
-      double S0 = 0.0, S1x = 0.0, S1y = 0.0, S1z = 0.0;
-      for (int dk = -1; dk <= 1; ++dk) {
-        const int kk = ck + dk;
-        if (kk < 0 || kk >= g.nz) continue;
-        for (int dj = -1; dj <= 1; ++dj) {
-          const int jj = cj + dj;
-          if (jj < 0 || jj >= g.ny) continue;
-          // the three x-neighbours of a row are consecutive cells: one contiguous run of points
-          const int i0 = max(ci - 1, 0), i1 = min(ci + 1, g.nx - 1);
-          if (i0 > i1) continue;
-          const int row = g.cell0 + (kk * g.ny + jj) * g.nx;
-          const int b = __ldg(p.pc_cell + row + i0), en = __ldg(p.pc_cell + row + i1 + 1);
-          for (int i = b; i < en; ++i) {
-            const float4 pp = __ldg(p.pc_pts + g.pt0 + i);
-            const float dx = pp.x - xf, dy = pp.y - yf, dz = pp.z - zf;
-            const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-            if (d2 < R2) {
-              const float P = R - sqrtf(d2);                                                 // Eq. 12
-              S0 += (double)P;
-              S1x = fma((double)P, (double)dx, S1x); S1y = fma((double)P, (double)dy, S1y); S1z = fma((double)P, (double)dz, S1z);
+      xf = (float)xd.x; yf = (float)xd.y; zf = (float)xd.z;
+    }
+    // ---- shared scan: in round r the TS_PC_GROUP lanes of group gq serve the taxel of lane r * NG + gq
+    constexpr int NG = 32 / TS_PC_GROUP;          // groups per warp = taxels per round
+    const int gq = lane / TS_PC_GROUP, sub = lane % TS_PC_GROUP;
+    float S0f = 0.f, S1xf = 0.f, S1yf = 0.f, S1zf = 0.f;   // this lane's own taxel: filled in its round
+    if (__any_sync(TS_FULL, id >= 0)) {
+#pragma unroll 1
+      for (int r = 0; r < TS_PC_GROUP; ++r) {
+        const int owner = r * NG + gq;
+        const int oid = __shfl_sync(TS_FULL, id, owner);
+        const float ox = __shfl_sync(TS_FULL, xf, owner), oy = __shfl_sync(TS_FULL, yf, owner), oz = __shfl_sync(TS_FULL, zf, owner);
+        float s0 = 0.f, sx = 0.f, sy = 0.f, sz = 0.f;
+        if (oid >= 0) {
+          const TsPcGrid g = p.pc_grid[oid];
+          const int ci = (int)floorf((ox - g.ox) * g.inv_cell), cj = (int)floorf((oy - g.oy) * g.inv_cell), ck = (int)floorf((oz - g.oz) * g.inv_cell);
+          const float cellw = 1.0f / g.inv_cell;
+          const float ry = oy - g.oy, rz = oz - g.oz;       // position relative to the grid origin
+          const int i0 = max(ci - TS_PC_REACH, 0), i1 = min(ci + TS_PC_REACH, g.nx - 1);
+          const float4* pts = p.pc_pts + g.pt0;
+          if (i0 <= i1) {
+            for (int dk = -TS_PC_REACH; dk <= TS_PC_REACH; ++dk) {
+              const int kk = ck + dk;
+              if (kk < 0 || kk >= g.nz) continue;
+              const float gz = fmaxf(fmaxf((float)kk * cellw - rz, rz - (float)(kk + 1) * cellw), 0.f);   // gap to the slab in z
+              for (int dj = -TS_PC_REACH; dj <= TS_PC_REACH; ++dj) {
+                const int jj = cj + dj;
+                if (jj < 0 || jj >= g.ny) continue;
+                const float gy = fmaxf(fmaxf((float)jj * cellw - ry, ry - (float)(jj + 1) * cellw), 0.f);
+                // the whole row of cells lies outside the sensing sphere (1e-6 m of slack for the rounding of the cell edges)
+                if (fmaf(gy, gy, gz * gz) >= (R + 1e-6f) * (R + 1e-6f)) continue;
+                // the x-neighbours of a row are consecutive cells: one contiguous run of points, split over the group's lanes
+                const int row = g.cell0 + (kk * g.ny + jj) * g.nx;
+                const int b = __ldg(p.pc_cell + row + i0), en = __ldg(p.pc_cell + row + i1 + 1);
+                for (int i = b + sub; i < en; i += TS_PC_GROUP) {
+                  const float4 pp = __ldg(pts + i);
+                  const float dx = pp.x - ox, dy = pp.y - oy, dz = pp.z - oz;
+                  const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                  const float P = d2 < R2 ? R - sqrtf(d2) : 0.f;                             // Eq. 12 (0 outside the sphere)
+                  s0 += P;
+                  sx = fmaf(P, dx, sx); sy = fmaf(P, dy, sy); sz = fmaf(P, dz, sz);
+                }
+              }
             }
           }
         }
-      }
-      if (S0 > 0.0) {
-        const D3 S1w = mulR(RO, D3{S1x, S1y, S1z});                                          // sum P (p_i - q_j), world axes
-        const D3 wO = ld3d(p.obj_angvel + ek * 3);
-        const D3 A = ld3d(p.obj_linvel + ek * 3) + cross(wO, q - pO) - vtax;                 // Eq. 13 at p_i = q_j
-        const D3 sv = S0 * A + cross(wO, S1w);                                               // sum P (v_p - v_tax)
-        const D3 st = sv - dot(sv, a) * a;                                                   // Eq. 14 (linear)
-        fw = fw + ((double)p.pc_k * rho * S0) * a + ((double)p.pc_ks * rho) * st;            // Eq. 16
-        tw = tw + ((double)p.pc_k * rho) * cross(S1w, a);                                    // Eq. 17
+        // sum over the group's lanes (fp32: <= a few hundred terms of bounded size), then hand the totals to the owner
+#pragma unroll
+        for (int o = TS_PC_GROUP / 2; o > 0; o >>= 1) {
+          s0 += __shfl_xor_sync(TS_FULL, s0, o); sx += __shfl_xor_sync(TS_FULL, sx, o);
+          sy += __shfl_xor_sync(TS_FULL, sy, o); sz += __shfl_xor_sync(TS_FULL, sz, o);
+        }
+        const int src = (lane % NG) * TS_PC_GROUP;      // first lane of the group that served THIS lane's taxel in round lane / NG
+        const float t0 = __shfl_sync(TS_FULL, s0, src), tx = __shfl_sync(TS_FULL, sx, src), ty = __shfl_sync(TS_FULL, sy, src),
+                    tz = __shfl_sync(TS_FULL, sz, src);
+        if (lane / NG == r) { S0f = t0; S1xf = tx; S1yf = ty; S1zf = tz; }
       }
     }
+    if (id >= 0 && S0f > 0.f) {
+      const double S0 = (double)S0f;
+      const D3 S1w = mulR(RO, D3{(double)S1xf, (double)S1yf, (double)S1zf});                 // sum P (p_i - q_j), world axes
+      const D3 wO = ld3d(p.obj_angvel + ek * 3);
+      const D3 A = ld3d(p.obj_linvel + ek * 3) + cross(wO, q - pO) - vtax;                   // Eq. 13 at p_i = q_j
+      const D3 sv = S0 * A + cross(wO, S1w);                                                 // sum P (v_p - v_tax)
+      const D3 st = sv - dot(sv, a) * a;                                                     // Eq. 14 (linear)
+      fw = fw + ((double)p.pc_k * rho * S0) * a + ((double)p.pc_ks * rho) * st;              // Eq. 16
+      tw = tw + ((double)p.pc_k * rho) * cross(S1w, a);                                      // Eq. 17
+    }
+  }
+  if (act) {
     const D3 fl = mulRT(RL, fw), tl = mulRT(RL, tw);                                         // reported in the link frame
     out[0] = (float)fl.x; out[1] = (float)fl.y; out[2] = (float)fl.z; out[3] = (float)tl.x; out[4] = (float)tl.y; out[5] = (float)tl.z;
   }
-  store6(p.proxpc + gt * 6, out);
+  if (in_range) store6(p.proxpc + gt * 6, out);
 }
 
 // ---------------------------------------------------------------------------------------
