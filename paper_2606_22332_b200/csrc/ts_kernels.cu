@@ -1657,7 +1657,11 @@ __global__ void __launch_bounds__(128, TS_PC_MINB) ts_proxpc_kernel(const __grid
 //          it to the dilation value the step kernel wrote (Eq. 23).
 // ---------------------------------------------------------------------------------------
 #define TS_SHEAR_Q 512
-__global__ void __launch_bounds__(256) ts_shear_kernel(const __grid_constant__ TsStepParams p) {
+// 2 / 4 / 6 / 8 blocks per SM: 1.38 / 0.84 / 0.68 / 0.73 ms (the point loop waits on its loads).
+#ifndef TS_SH_MINB
+#define TS_SH_MINB 6
+#endif
+__global__ void __launch_bounds__(256, TS_SH_MINB) ts_shear_kernel(const __grid_constant__ TsStepParams p) {
   __shared__ double Rm[9], tv[3];
   __shared__ float4 qd[TS_SHEAR_Q];   // (tangential slide x, y, z, h_p)
   __shared__ float4 qz[TS_SHEAR_Q];   // z_p relative to the pad centre
@@ -1827,7 +1831,11 @@ __device__ __forceinline__ float ray_tri(F3 o, F3 d, F3 a, F3 b, F3 c) {
   return t >= 0.f ? t : -1.f;
 }
 
-__global__ void __launch_bounds__(128) ts_raycast_kernel(const __grid_constant__ TsStepParams p) {
+// Latency-bound tree walk: residency beats registers (4 / 8 / 12 / 16 blocks per SM: 1.35 / 0.85 / 0.80 / 0.90 ms).
+#ifndef TS_RC_MINB
+#define TS_RC_MINB 12
+#endif
+__global__ void __launch_bounds__(128, TS_RC_MINB) ts_raycast_kernel(const __grid_constant__ TsStepParams p) {
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (gt >= (long long)p.E * p.T) return;
   const int e = (int)(gt / p.T), j = (int)(gt - (long long)e * p.T);
