@@ -115,9 +115,8 @@ ts_status ts_layout_destroy(ts_layout* lay); /* NULL is a no-op */
 enum { TS_HYST_OFF = 0, TS_HYST_MAXWELL = 1 /* Eq. 29-30 */, TS_HYST_ASYM = 2 /* DESIGN.md D3 */ };
 
 /* How ts_step runs the noise chain (App. A.8): inside the step kernel (one launch after the frames kernel) or as a
- * separate kernel behind it.  AUTO = fused for the four knobs of drift / hysteresis / dead taxels / 4-neighbour
- * crosstalk, split when any further A.8 knob is set (the fused variant with every knob exceeds the instruction
- * cache).  Both forms compute bit-identical results. */
+ * separate kernel behind it.  AUTO = fused (the faster form for every knob combination measured).
+ * Both forms compute bit-identical results. */
 enum { TS_FORM_AUTO = 0, TS_FORM_FUSED = 1, TS_FORM_SPLIT = 2 };
 
 enum {                      /* output_mask bits.  ts_step contract: every output whose bit is set must be given (non-NULL)

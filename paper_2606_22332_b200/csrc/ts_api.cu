@@ -456,9 +456,10 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
   TS_ALLOC(c->st_flags, E * T);
   TS_ALLOC(c->reset_step, sizeof(uint32_t) * E);
   TS_ALLOC(c->episode, sizeof(uint32_t) * E);
-  // Default (TS_FORM_AUTO): one fused launch, except when optional A.8 knobs are on: the fused variant that carries them
-  // runs past the instruction-cache knee and the two-kernel form is faster.
-  c->fused = cfg->kernel_form == TS_FORM_FUSED ? true : (cfg->kernel_form == TS_FORM_SPLIT ? false : !(TS_DEFAULT_SPLIT || cfg_ext(*cfg)));
+  // Default (TS_FORM_AUTO): one fused launch.  (In round 1 the fused variant that carries the optional A.8 knobs ran past
+  // the instruction-cache knee and AUTO chose two kernels for it; since the frames kernel and the DMMA marker path took
+  // ~8 KB of SASS out of the step kernel the fused form wins with every knob set: DESIGN.md section 5.)
+  c->fused = cfg->kernel_form == TS_FORM_FUSED ? true : (cfg->kernel_form == TS_FORM_SPLIT ? false : !TS_DEFAULT_SPLIT);
   if (cfg->noise_enable && !c->fused && !(cfg->output_mask & TS_OUT_FT)) TS_ALLOC(c->ft_scratch, sizeof(float) * E * T * 6);
   if (cfg->noise_enable && !c->fused && cfg->radius_noise != 0.f) TS_ALLOC(c->ft_scratch_r, sizeof(float) * E * T * 6);
   if (cfg->output_mask & (TS_OUT_DEPTH_NOISY | TS_OUT_PROX_NOISY)) {
