@@ -703,22 +703,44 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
     nsum[2 * c + 1] = (a0.y + a1.y) + (a2.y + a3.y);
   }
   // Eq. 11 / 31 with the Gaussian kernel (R7): conv = sum_{du,dv} g[|du|] g[|dv|] h(iu+du, iv+dv), zero outside the
-  // patch; slots of a patch are consecutive (u fastest), inactive sources hold h = 0.
+  // patch; slots of a patch are consecutive (u fastest), inactive sources hold h = 0.  The kernel is separable, so the
+  // sum runs as two 1-D passes through the exchange buffer, (2r+1) + (2r+1) taps instead of (2r+1)^2: row sums
+  // t(iu, iv) = sum_du g[|du|] h(iu+du, iv) replace h in the buffer (two barriers; `gauss` is block-uniform), then
+  // conv = sum_dv g[|dv|] t(iu, iv+dv).  A patch is active or filtered as a whole (the link filter works per link, R_j per
+  // patch), so the row sums a column pass reads were all formed.
   float conv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   const bool gauss = EXT && p.xt_r > 0;
-  if (gauss && act) {
-    const TsPatch& pt = p.patches[patch0 + (meta & 255)];
-    const int nv = __ldg(&pt.nv), il = j - __ldg(&pt.start), iv = il / nu, iu = il - iv * nu, r = p.xt_r;
-    for (int dv = -r; dv <= r; ++dv) {
-      if (iv + dv < 0 || iv + dv >= nv) continue;
-      const float wv = p.xt_w[dv < 0 ? -dv : dv];
+  if (gauss) {
+    const int r = p.xt_r;
+    int nv = 0, iv = 0, iu = 0;
+    float t6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (act) {
+      const TsPatch& pt = p.patches[patch0 + (meta & 255)];
+      nv = __ldg(&pt.nv);
+      const int il = j - __ldg(&pt.start);
+      iv = il / nu; iu = il - iv * nu;
       for (int du = -r; du <= r; ++du) {
         if (iu + du < 0 || iu + du >= nu) continue;
-        const float w = wv * p.xt_w[du < 0 ? -du : du];
-        const int k = tid + dv * nu + du;
+        const float w = p.xt_w[du < 0 ? -du : du];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-          const float2 a = b2[c * TS_BLOCK + k];
+          const float2 a = b2[c * TS_BLOCK + tid + du];
+          t6[2 * c] = fmaf(w, a.x, t6[2 * c]);
+          t6[2 * c + 1] = fmaf(w, a.y, t6[2 * c + 1]);
+        }
+      }
+    }
+    __syncthreads();   // every row pass has read h
+#pragma unroll
+    for (int c = 0; c < 3; ++c) b2[c * TS_BLOCK + tid] = make_float2(t6[2 * c], t6[2 * c + 1]);
+    __syncthreads();
+    if (act) {
+      for (int dv = -r; dv <= r; ++dv) {
+        if (iv + dv < 0 || iv + dv >= nv) continue;
+        const float w = p.xt_w[dv < 0 ? -dv : dv];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const float2 a = b2[c * TS_BLOCK + tid + dv * nu];
           conv[2 * c] = fmaf(w, a.x, conv[2 * c]);
           conv[2 * c + 1] = fmaf(w, a.y, conv[2 * c + 1]);
         }
