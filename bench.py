@@ -191,6 +191,17 @@ def time_extras(W, TactileSim, torch, dev, n_envs=4096, steps=20):
     res["scalar_noise_ms"] = run(full + ("depth_noisy", "prox_noisy", "marker_noisy"), noise=t12) - run(full, noise=t12)
     n = float(w.E) * w.T
     res["env_taxel_per_s"] = {k[:-3]: n / (v * 1e-3) for k, v in res.items() if k.endswith("_ms") and k != "base_depth_only_ms" and v > 0}
+    # What bounds them (profiles/r02_other_configs.md): the scalar-noise kernel streams its state:
+    # per taxel clean depth + prox 8 B, flags 1 B, state 24 B read + 24 B written, outputs 8 B; per marker 12 B in, 36 B
+    # of state read + 36 B written, 12 B out.  The other three move little and wait on dependent loads.
+    b = (8 + 1 + 48 + 8) + (12 + 72 + 12) * 980.0 / w.T
+    peak, src = hbm_peak()
+    ach = b * n / (res["scalar_noise_ms"] * 1e-3) / 1e9 if res["scalar_noise_ms"] > 0 else 0.0
+    res["roofline"] = {"scalar_noise": {"bound": "hbm", "bytes_per_env_taxel": b, "achieved": ach, "peak": peak, "unit": "GB/s",
+                                        "frac": ach / peak, "peak_source": src},
+                       "proxpc": {"bound": "latency (dependent loads: run bounds -> points)", "frac": None},
+                       "raycast": {"bound": "latency (BVH node -> children / triangles)", "frac": None},
+                       "shear": {"bound": "latency (anchor flag -> anchor; one double transform per tracked point per pad)", "frac": None}}
     return res
 
 

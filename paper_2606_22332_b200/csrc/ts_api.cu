@@ -729,8 +729,8 @@ ts_status ts_set_pointclouds(ts_ctx* c, const ts_pointclouds* pc, void* stream) 
   cudaStream_t st = (cudaStream_t)stream;
   c->have_pc = false;
   TS_CUDA(c, cudaStreamSynchronize(st));   // steps in flight may still read the old index
-  cudaFree(c->rc_nodes); cudaFree(c->rc_tri); cudaFree(c->rc_root); cudaFree(c->rc_id);
   cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw);
+  c->sh_on = nullptr; c->sh_e = nullptr; c->pc_raw = nullptr;
   cudaFree(c->pc_pts); cudaFree(c->pc_cell); cudaFree(c->pc_grid); cudaFree(c->pc_id);
   c->pc_pts = nullptr; c->pc_cell = nullptr; c->pc_grid = nullptr; c->pc_id = nullptr;
   TS_CUDA(c, cudaMalloc((void**)&c->pc_pts, sizeof(float4) * sorted.size()));
@@ -742,8 +742,6 @@ ts_status ts_set_pointclouds(ts_ctx* c, const ts_pointclouds* pc, void* stream) 
   TS_CUDA(c, cudaMemcpyAsync(c->pc_grid, grids.data(), sizeof(TsPcGrid) * G, cudaMemcpyHostToDevice, st));
   TS_CUDA(c, cudaMemcpyAsync(c->pc_id, pc->cloud_id, sizeof(int32_t) * EK, cudaMemcpyHostToDevice, st));
   if (c->cfg.shear_enable && c->M > 0) {   // Eq. 22 anchors: one per (env, patch, object, tracked point)
-    cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw);
-    c->sh_on = nullptr; c->sh_e = nullptr; c->pc_raw = nullptr;
     const size_t ns = (size_t)c->cfg.n_envs * c->P * c->cfg.objs_per_env * N;
     std::vector<float4> raw((size_t)G * N);
     for (size_t i = 0; i < raw.size(); ++i) raw[i] = make_float4(pc->points[3 * i], pc->points[3 * i + 1], pc->points[3 * i + 2], 0.f);

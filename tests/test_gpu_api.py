@@ -303,3 +303,41 @@ def test_checkpoint_resume_is_bit_exact():
     with pytest.raises(TsError):
         c.set_state(blob[:64])
     a.close(); b.close(); c.close()
+
+
+def test_meshes_and_pointclouds_on_one_ctx_in_any_order_and_replaced():
+    """ts_set_meshes and ts_set_pointclouds own separate buffers: one ctx that gets both (in either order, each of them
+    twice) and asks for raycast depth, point-cloud proximity and sheared markers at once equals, bit for bit, contexts
+    that were given only what each output needs."""
+    import torch
+    from paper_2606_22332_b200.binding import TactileSim
+    w = W.config(5, n_envs=24)
+    pts, cid = W.point_cloud_bank(w, 600)
+    meshes, mid = W.mesh_bank(w, 2)
+    phys = dict(w.physics, shear_enable=1)
+    x = None
+
+    def run(outs, order, physics):
+        nonlocal x
+        sim = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=physics, outputs=outs)
+        sim.set_geometry(w.types, w.params, w.bank, w.voxel)
+        for what in order:
+            sim.set_meshes(meshes, mid) if what == "m" else sim.set_pointclouds(pts, cid)
+        if x is None:
+            x = [sim.upload(w.inputs(s)) for s in range(3)]
+        for s in range(3):
+            g = sim.step(x[s])
+        torch.cuda.synchronize()
+        res = {k: v.clone() for k, v in g.items()}
+        sim.close()
+        return res
+
+    ref_rc = run(("depth", "depth_rc", "nrm_rc"), "m", w.physics)
+    ref_pc = run(("depth", "marker", "proxpc"), "p", phys)
+    assert ref_rc["depth_rc"].abs().sum() > 0 and ref_pc["proxpc"].abs().sum() > 0
+    for order in ("mp", "pm", "mpmp", "ppmm"):
+        got = run(("depth", "marker", "proxpc", "depth_rc", "nrm_rc"), order, phys)
+        for k in ("depth_rc", "nrm_rc"):
+            assert torch.equal(got[k], ref_rc[k]), (order, k)
+        for k in ("proxpc", "marker", "depth"):
+            assert torch.equal(got[k], ref_pc[k]), (order, k)
