@@ -137,6 +137,18 @@ def test_config3_full_size_sampled():
     _assert_ok(_parity(w, ids=w.parity_envs(), steps=10))
 
 
+def test_more_than_65535_envs():
+    """Maximum-size edge: beyond 65,535 envs the step kernel's grid folds the env index over blockIdx.y / blockIdx.z (and
+    every other kernel runs a 1-D grid over more than 2^16 envs).  Config 4 (noise on) at 66,000 envs and config 2 (no
+    noise) at 70,000 envs; the oracle recomputes the envs around the fold and the last one."""
+    w = W.config(4, n_envs=66000)
+    ids = np.array([0, 1, 65534, 65535, 65536, 65537, 65999])
+    _assert_ok(_parity(w, ids=ids, steps=4))
+    w = W.config(2, n_envs=70000)
+    ids = np.array([0, 65534, 65535, 65536, 69999])
+    _assert_ok(_parity(w, ids=ids, steps=2))
+
+
 def test_env_shards_are_bit_identical_to_the_full_run():
     """two contexts over env halves with env_id_base = 0 / E/2 reproduce the full run."""
     import torch
