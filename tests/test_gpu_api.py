@@ -91,6 +91,12 @@ def test_error_paths_return_status_and_message():
     sim.step(inp, out)
     torch.cuda.synchronize()
     assert L.ts_destroy(None) == 0 and L.ts_step(None, None, None, None) == 1
+    # maximum sizes: the state rows use 32-bit element indices, n_envs * 12 * T (rounded up to 32) must stay below 2^32
+    w5 = W.config(5, n_envs=8)
+    with pytest.raises(B.TsError, match="32-bit element indices"):
+        B.TactileSim(w5.patches, w5.T, 350000, w5.L, w5.K, physics=w5.physics, noise=w5.noise, outputs=w5.outputs)
+    with pytest.raises(B.TsError, match="32-bit element indices"):          # the read-delay ring has its own bound
+        B.TactileSim(w5.patches, w5.T, 200000, w5.L, w5.K, physics=w5.physics, noise=dict(w5.noise, read_delay=8), outputs=w5.outputs)
 
 
 def test_outputs_subset_and_replaced_geometry():
