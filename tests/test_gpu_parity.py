@@ -149,6 +149,15 @@ def test_more_than_65535_envs():
     _assert_ok(_parity(w, ids=ids, steps=2))
 
 
+def test_near_the_maximum_env_count():
+    """Maximum-size edge: config 5 at 340,000 envs x 1,000 taxels, just under the 32-bit state-index limit of ts_create
+    (n_envs * 12 * 1,024 < 2^32, i.e. 349,525 envs; about 45 GB of outputs and state).  Every 32-bit offset in the kernels
+    is at its largest here; the oracle recomputes envs at the start, the middle and the very end."""
+    w = W.config(5, n_envs=340000)
+    ids = np.array([0, 1281, 169999, 170000, 339984, 339999])
+    _assert_ok(_parity(w, ids=ids, steps=3))
+
+
 def test_env_shards_are_bit_identical_to_the_full_run():
     """two contexts over env halves with env_id_base = 0 / E/2 reproduce the full run."""
     import torch
