@@ -1969,6 +1969,8 @@ int ts_prepare_kernels(int device, int smem_bytes) {
   if (e == cudaSuccess) e = prep_one<true, -1, true>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_MAXWELL, true>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_ASYM, true>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, 4 | TS_HYST_MAXWELL, true>(max_smem_bytes);
+  if (e == cudaSuccess) e = prep_one<true, 4 | TS_HYST_ASYM, true>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_OFF>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_MAXWELL>(max_smem_bytes);
   if (e == cudaSuccess) e = prep_one<true, TS_HYST_ASYM>(max_smem_bytes);
@@ -2017,11 +2019,13 @@ int ts_launch_step(const TsStepParams& p, int fused_noise, void* stream) {
   const int hm = (p.noise_enable && fused_noise) ? (p.hyst_mode | (p.ext ? 4 : 0)) : -1;
   // the common full configuration has its own compile-time-specialised variants (see ts_step_kernel)
   const bool clean5 = p.K == 1 && p.inl && p.env_perm && p.mk_mma && p.contact && p.depth && p.ft && p.marker && p.prox;
-  const bool fast = clean5 && p.ft_noisy && p.dead && (hm == TS_HYST_ASYM || hm == TS_HYST_MAXWELL);
+  const bool fast = clean5 && p.ft_noisy && p.dead && ((hm & 3) == TS_HYST_ASYM || (hm & 3) == TS_HYST_MAXWELL);
   if (clean5 && hm == -1 && !p.noise_enable && !p.dead && !p.depth_pert)
     return launch_dependent(ts_step_kernel<true, -1, true>, grid, smem, (cudaStream_t)stream, p);
   else if (fast && hm == TS_HYST_ASYM) return launch_dependent(ts_step_kernel<true, TS_HYST_ASYM, true>, grid, smem, (cudaStream_t)stream, p);
-  else if (fast) return launch_dependent(ts_step_kernel<true, TS_HYST_MAXWELL, true>, grid, smem, (cudaStream_t)stream, p);
+  else if (fast && hm == TS_HYST_MAXWELL) return launch_dependent(ts_step_kernel<true, TS_HYST_MAXWELL, true>, grid, smem, (cudaStream_t)stream, p);
+  else if (fast && hm == (4 | TS_HYST_ASYM)) return launch_dependent(ts_step_kernel<true, 4 | TS_HYST_ASYM, true>, grid, smem, (cudaStream_t)stream, p);
+  else if (fast) return launch_dependent(ts_step_kernel<true, 4 | TS_HYST_MAXWELL, true>, grid, smem, (cudaStream_t)stream, p);
   else if (p.K == 1) launch_one<true>(p, hm, grid, smem, (cudaStream_t)stream);
   else launch_one<false>(p, hm, grid, smem, (cudaStream_t)stream);
   return (int)cudaGetLastError();
