@@ -347,3 +347,38 @@ def test_meshes_and_pointclouds_on_one_ctx_in_any_order_and_replaced():
             assert torch.equal(got[k], ref_rc[k]), (order, k)
         for k in ("proxpc", "marker", "depth"):
             assert torch.equal(got[k], ref_pc[k]), (order, k)
+
+
+def test_two_contexts_on_two_streams_run_concurrently():
+    """Contexts are independent: two of them stepped from two CUDA streams at the same time (their chained launches and
+    the per-device kernel attributes are shared machinery) give, bit for bit, what each gives when stepped alone."""
+    import torch
+    wa, wb = W.config(5, n_envs=3000), W.config(4, n_envs=2500)
+    xa = xb = None
+    res = {}
+    for mode in ("alone", "together"):
+        a, b = _sim(wa), _sim(wb)
+        if xa is None:
+            xa = [a.upload(wa.inputs(s)) for s in range(5)]
+            xb = [b.upload(wb.inputs(s)) for s in range(5)]
+        oa, ob = a.alloc_outputs(), b.alloc_outputs()
+        torch.cuda.synchronize()
+        if mode == "alone":
+            for s in range(15):
+                a.step(xa[s % 5], oa)
+            torch.cuda.synchronize()
+            for s in range(15):
+                b.step(xb[s % 5], ob)
+        else:
+            sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+            for s in range(15):
+                with torch.cuda.stream(sa):
+                    a.step(xa[s % 5], oa)
+                with torch.cuda.stream(sb):
+                    b.step(xb[s % 5], ob)
+        torch.cuda.synchronize()
+        res[mode] = ({k: v.clone() for k, v in oa.items()}, {k: v.clone() for k, v in ob.items()})
+        a.close(); b.close()
+    for i in (0, 1):
+        for k in res["alone"][i]:
+            assert torch.equal(res["alone"][i][k], res["together"][i][k]), (i, k)
