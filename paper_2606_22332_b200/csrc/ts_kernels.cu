@@ -984,15 +984,18 @@ template <bool SINGLE, int HM, bool FAST = false>
 __global__ void __launch_bounds__(TS_BLOCK, TS_MIN_BLOCKS) ts_step_kernel(const __grid_constant__ TsStepParams p) {
   constexpr bool NOISE = HM >= 0;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int nfr = p.frames_per_group * p.K;
-  FrameS* frames = reinterpret_cast<FrameS*>(smem_raw);
   // Shared memory is kept small on purpose: it is carved out of the same 256 KB as L1, and the SDF gathers
   // of the march live on L1 hits.  S (marker phase) aliases bufB (noise phase); a barrier separates them.
-  double* S = reinterpret_cast<double*>(frames + nfr);    // [3][TS_CHUNK] marker pass-1 sums (generic marker path only)
-  float* bufB = reinterpret_cast<float*>(S);              // [6][TS_BLOCK] crosstalk exchange (first 6 KB of S)
-  float* hh = reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(S) + p.s_bytes);  // [TS_BLOCK] penetration h_i (Eq. 19)
+  // Fixed-size arrays first, at compile-time offsets (their addresses are re-formed at every use under the 48-register
+  // budget: an immediate instead of arithmetic on kernel parameters); the frames, whose count is the layout's, last.
+  float* hh = reinterpret_cast<float*>(smem_raw);         // [TS_BLOCK] penetration h_i (Eq. 19)
   float* ha = hh + TS_BLOCK;                              // [TS_BLOCK] h_i^alpha_e
   unsigned* pmask = reinterpret_cast<unsigned*>(ha + TS_BLOCK);  // bit l: group-local patch l has penetration
+  double* S = reinterpret_cast<double*>(smem_raw + sizeof(float) * 2 * TS_BLOCK + sizeof(int) * TS_MAX_GROUP_PATCHES);
+                                                          // [3][TS_CHUNK] marker pass-1 sums (generic marker path only)
+  float* bufB = reinterpret_cast<float*>(S);              // [6][TS_BLOCK] crosstalk exchange (first 6 KB of S)
+  FrameS* frames = reinterpret_cast<FrameS*>(reinterpret_cast<unsigned char*>(S) +
+                                             (FAST ? (int)(sizeof(float) * 6 * TS_BLOCK) : p.s_bytes));   // FAST implies the DMMA marker path
 
   const int tid = threadIdx.x;
 #if TS_GRID_GFAST
