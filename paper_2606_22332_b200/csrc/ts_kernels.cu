@@ -354,7 +354,6 @@ __device__ __forceinline__ D3 grad_d(const TsStepParams& p, int type, const floa
 // Packed fp32 pairs (Blackwell FADD2 / FFMA2: one issue slot for two lanes of arithmetic; a scalar operand is broadcast).
 __device__ __forceinline__ unsigned long long pk2(float2 a) { unsigned long long r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y)); return r; }
 __device__ __forceinline__ float2 upk2(unsigned long long a) { float2 r; asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(a)); return r; }
-__device__ __forceinline__ float2 add2(float2 a, float2 b) { unsigned long long d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk2(a)), "l"(pk2(b))); return upk2(d); }
 __device__ __forceinline__ float2 sub2(float2 a, float2 b) { unsigned long long d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk2(a)), "l"(pk2(b))); return upk2(d); }
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { unsigned long long d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pk2(a)), "l"(pk2(b)), "l"(pk2(c))); return upk2(d); }
 __device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
@@ -643,7 +642,6 @@ __device__ __forceinline__ void noise_chain(const TsStepParams& p, int e, int j,
       for (int c = 0; c < 3; ++c) __stcs(st_h + (ih + c * Tp), make_float2(h[2 * c], h[2 * c + 1]));
     }
   } else if (MODE == TS_HYST_MAXWELL) {  // Eq. 29-30
-#pragma unroll
     float zx[6];
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
