@@ -361,6 +361,7 @@ struct Oracle {
   std::vector<int32_t> rc_id;                 // [E,K], -1 = no mesh
   double *rc_depth = nullptr, *rc_nrm = nullptr, *rc_gap = nullptr;   // [E,T], [E,T,3], [E,T] outputs handed in by orc_set_raycast_out
   std::vector<std::deque<std::vector<double>>> hist;  // [E] the last Delta + J post-crosstalk fields [T,6] of the episode
+  std::vector<std::deque<std::vector<double>>> shist;  // [E] the same for the scalar readouts (R10): post-hysteresis depth [T], prox [T], markers [M,3]
   std::vector<uint32_t> n_step, episode;      // [E]
 };
 
@@ -492,6 +493,7 @@ void* orc_create(const orc_params* prm, const orc_patch* patches, int n_patches,
   o->hyst_a.assign(ET * 6, 0.0); o->hyst_b.assign(ET * 6, 0.0); o->drift.assign(ET * 6, 0.0);   // Q12
   o->n_step.assign(o->E, 0); o->episode.assign(o->E, 0);
   o->hist.assign(o->E, {});
+  o->shist.assign(o->E, {});
   o->sn_ha.assign(ET * 2, 0.0); o->sn_hb.assign(ET * 2, 0.0); o->sn_dr.assign(ET * 2, 0.0);
   { size_t EM = (size_t)o->E * o->M * 3; o->sm_ha.assign(EM, 0.0); o->sm_hb.assign(EM, 0.0); o->sm_dr.assign(EM, 0.0); }
   Geom none; none.type = G_NONE; none.grid = nullptr; none.N = 0; none.hv = 0; for (double& v : none.p) v = 0;
@@ -556,6 +558,7 @@ void orc_reset(void* h, const uint8_t* env_mask) {
     o.n_step[e] = 0;
     o.episode[e] += 1;
     o.hist[e].clear();
+    o.shist[e].clear();
     if (!o.sh_on.empty()) {
       size_t per = (size_t)o.P * o.K * o.pc_N;
       std::fill(o.sh_on.begin() + (size_t)e * per, o.sh_on.begin() + (size_t)(e + 1) * per, (uint8_t)0);
@@ -582,7 +585,7 @@ static bool is_dead(const Oracle& o, int e, int t) {
 // (distance to the nearest rounding boundary; |x| - |y_prev| where the signs differ), +inf where not applicable.
 static double scalar_chain(const orc_params& pr, int cls, double clean, double gain, bool is_dead, double stuck_u,
                            double z_rw, double z_w, double& ha, double& hb, double& drift, double decay,
-                           double* aq, double* aa) {
+                           double* aq, double* aa, const double* delayed = nullptr, double* hrec = nullptr) {
   double x = gain * clean, hval = x;
   if (aa) *aa = INFINITY;
   if (pr.hyst_mode == 1) {                                        // Eq. 29-30
@@ -597,6 +600,10 @@ static double scalar_chain(const orc_params& pr, int cls, double clean, double g
     ha = y;
     hval = y;
   }
+  // Eq. 25 read delay (R9 / R10): only the signal is delayed, y_{t - Delta_n}; bias, white noise and drift are those
+  // of step t.  hrec receives this step's signal for the history, delayed points at the one to show (NULL: Delta_n = 0).
+  if (hrec) *hrec = hval;
+  if (delayed) hval = *delayed;
   drift += (double)pr.sn_sigma_rw[cls] * z_rw;                    // Eq. 25 d_t = d_{t-1} + w_t
   double y = hval + (double)pr.sn_bias[cls] + (double)pr.sn_sigma_white[cls] * z_w + drift;
   if (aq) *aq = INFINITY;
@@ -1053,6 +1060,27 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
         uint32_t c[4] = {env, probe, step, ep4 | stream};
         philox4x32_10(c, key, w);
       };
+      // Read delay of the scalar readouts (Table 3: every sensor has it): the SAME Delta_n as the force / torque readout
+      // of this env and step (one sensor read; stream 9, R9), applied to the post-hysteresis signal of each probe.
+      const bool sdelay_on = pr.read_delay > 0 || pr.read_jitter > 0;
+      int sdelta = 0;
+      std::vector<double> scur;
+      const double szero = 0.0;
+      if (sdelay_on) {
+        int k_n = 0;
+        if (pr.read_jitter > 0) {
+          uint32_t wj[4];
+          draw(0xffffffffu, n, 9u, wj);
+          k_n = (int)(((uint64_t)(wj[0] >> 9) * (uint64_t)(2 * pr.read_jitter + 1)) >> 23) - pr.read_jitter;
+        }
+        sdelta = std::max(0, pr.read_delay + k_n);
+        scur.assign((size_t)T * 2 + (size_t)M * 3, 0.0);
+      }
+      const int shave = (int)o.shist[e].size();
+      auto delayed_of = [&](size_t idx) -> const double* {   // the signal of step n - Delta_n, 0 before the episode began (Q12)
+        if (!sdelay_on || sdelta == 0) return nullptr;
+        return sdelta <= shave ? &o.shist[e][shave - sdelta][idx] : &szero;
+      };
       for (int j = 0; j < T; ++j) {
         size_t ej = (size_t)e * T + j;
         double od = 0.0, op = 0.0;
@@ -1068,9 +1096,11 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
           double gain = 1.0;
           if (gain_on) { draw((uint32_t)j, 0u, 3u, wg); gain = (double)pr.gain_min + ((double)pr.gain_max - (double)pr.gain_min) * word_to_uniform(wg[0]); }
           od = scalar_chain(pr, 0, dep_t[j], gain, deadv[j], word_to_uniform(ws[0]), zd[0], zd[1], o.sn_ha[ej * 2], o.sn_hb[ej * 2],
-                            o.sn_dr[ej * 2], decay, o.aux_sq_depth ? &o.aux_sq_depth[ej] : nullptr, nullptr);
+                            o.sn_dr[ej * 2], decay, o.aux_sq_depth ? &o.aux_sq_depth[ej] : nullptr, nullptr, delayed_of((size_t)j * 2),
+                            sdelay_on ? &scur[(size_t)j * 2] : nullptr);
           op = scalar_chain(pr, 1, prox_c[j], gain, deadv[j], word_to_uniform(ws[1]), zp[0], zp[1], o.sn_ha[ej * 2 + 1],
-                            o.sn_hb[ej * 2 + 1], o.sn_dr[ej * 2 + 1], decay, o.aux_sq_prox ? &o.aux_sq_prox[ej] : nullptr, nullptr);
+                            o.sn_hb[ej * 2 + 1], o.sn_dr[ej * 2 + 1], decay, o.aux_sq_prox ? &o.aux_sq_prox[ej] : nullptr, nullptr,
+                            delayed_of((size_t)j * 2 + 1), sdelay_on ? &scur[(size_t)j * 2 + 1] : nullptr);
         }
         if (o.depth_noisy) o.depth_noisy[ej] = od;
         if (o.prox_noisy) o.prox_noisy[ej] = op;
@@ -1103,10 +1133,15 @@ void orc_step(void* h, const float* link_pos, const float* link_quat, const floa
             if (mact)
               out = scalar_chain(pr, 2, marker_c[(size_t)jm * 3 + c], gain, mdead, word_to_uniform(ws[c]), zr[c],
                                  c == 0 ? zr[3] : zw[c - 1], o.sm_ha[i3], o.sm_hb[i3], o.sm_dr[i3], decay,
-                                 o.aux_sq_marker ? &o.aux_sq_marker[i3] : nullptr, o.aux_sasym_marker ? &o.aux_sasym_marker[i3] : nullptr);
+                                 o.aux_sq_marker ? &o.aux_sq_marker[i3] : nullptr, o.aux_sasym_marker ? &o.aux_sasym_marker[i3] : nullptr,
+                                 delayed_of((size_t)T * 2 + (size_t)jm * 3 + c), sdelay_on ? &scur[(size_t)T * 2 + (size_t)jm * 3 + c] : nullptr);
             o.marker_noisy[i3] = out;
           }
         }
+      }
+      if (sdelay_on) {  // keep the last Delta + J signal fields of the episode
+        o.shist[e].push_back(scur);
+        while ((int)o.shist[e].size() > pr.read_delay + pr.read_jitter) o.shist[e].pop_front();
       }
     }
     o.n_step[e] += 1;

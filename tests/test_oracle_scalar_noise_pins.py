@@ -174,3 +174,41 @@ def test_depth_noisy_senses_with_the_perturbed_radius_eq26():
             want = max(0.0, max(0.0, float(np.float32(R_TAX)) + eps) - r["aux_phi"][e, j])
             np.testing.assert_allclose(r["depth_noisy"][e, j], want, rtol=0, atol=1e-15)
     assert (r["depth_noisy"] != r["depth"]).any()
+
+
+def test_read_delay_of_the_scalar_readouts():
+    """Eq. 25 / Table 3: every sensor honours the read delay.  Only the signal is delayed (y_{t - Delta_n}); the bias is
+    that of step t; steps before the episode began read 0 (Q12); Delta_n = max(0, Delta + k_n) with k_n from stream 9,
+    taxel word 0xffffffff -- the same draw as the force / torque readout of that env and step (one sensor read)."""
+    zs = [-0.0316, -0.0312, -0.0319, -0.0314, -0.0317, -0.0311, -0.0318, -0.0313]      # a different indentation every step
+    bias = float(np.float32(3e-4))
+    # fixed delay of 2 steps, no jitter
+    o = _oracle(dict(read_delay=2, bias_depth=3e-4, bias_prox=3e-4, bias_marker=3e-4), nu=4, nv=4, m=3)
+    hist = []
+    for n, z in enumerate(zs):
+        r = o.step(_inputs(z), want=WANT)
+        hist.append({k: r[k].copy() for k in ("depth", "prox", "marker")})
+        for k in ("depth", "prox", "marker"):
+            want = (hist[n - 2][k] if n >= 2 else 0.0 * hist[n][k]) + bias
+            np.testing.assert_allclose(r[k + "_noisy"], want, rtol=1e-12, atol=1e-18)
+        if n >= 2:
+            assert np.abs(hist[n]["depth"] - hist[n - 2]["depth"]).max() > 5e-5          # the delay is visible
+    # a reset starts a new episode: the history is gone
+    o.reset()
+    r = o.step(_inputs(zs[0]), want=WANT)
+    np.testing.assert_allclose(r["depth_noisy"], 0.0 * r["depth"] + bias, rtol=0, atol=1e-18)
+    # jitter: Delta_n = max(0, 1 + k_n), k_n in {-1, 0, 1}, per (env, step); shared with ft_noisy
+    J = 1
+    o = _oracle(dict(read_delay=1, read_jitter=J), nu=4, nv=4, m=3)
+    hist, seen = [], set()
+    for n, z in enumerate(zs):
+        r = o.step(_inputs(z), want=WANT + ("ft", "ft_noisy"))
+        hist.append({k: r[k].copy() for k in ("depth", "prox", "marker", "ft")})
+        for e, env in enumerate(ENVS):
+            w0 = O.philox((int(env), 0xFFFFFFFF, n, 9), KEY)[0]
+            delta = max(0, 1 + ((int(w0) >> 9) * (2 * J + 1) >> 23) - J)
+            seen.add(delta)
+            for k, kn in (("depth", "depth_noisy"), ("prox", "prox_noisy"), ("marker", "marker_noisy"), ("ft", "ft_noisy")):
+                want = hist[n - delta][k][e] if n - delta >= 0 else 0.0 * hist[n][k][e]
+                np.testing.assert_allclose(r[kn][e], want, rtol=1e-12, atol=1e-18)
+    assert seen == {0, 1, 2}
