@@ -188,7 +188,8 @@ typedef struct ts_config {
    * post-crosstalk signal of step n - max(0, Delta + k_n), k_n uniform on {-J..J}, one draw per (env, step); steps
    * before the episode began read 0; bias, white noise and drift are those of step n (R9).
    * 0 <= read_delay, read_jitter and read_delay + read_jitter <= 64; the ctx holds that many past fields
-   * (24 B x n_envs x n_taxels each). */
+   * (24 B x n_envs x n_taxels each).  The noisy scalar readouts (TS_OUT_DEPTH_NOISY / PROX_NOISY / MARKER_NOISY) are
+   * delayed by the same number of steps (their post-hysteresis signal; 8 B per taxel and 12 B per marker per slot). */
   int32_t read_delay, read_jitter;
   int32_t kernel_form;   /* TS_FORM_* (0 = AUTO) */
   /* Noisy scalar readouts (TS_OUT_DEPTH_NOISY / PROX_NOISY / MARKER_NOISY), index 0 = depth, 1 = prox, 2 = marker:

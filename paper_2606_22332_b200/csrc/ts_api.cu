@@ -63,6 +63,7 @@ struct ts_ctx {
   // noisy scalar readouts (R10): state, the perturbed depth (Eq. 26), scratch copies of clean inputs the caller did not ask for
   float4* sn_h = nullptr; float2* sn_d = nullptr; float *sm_h = nullptr, *sm_d = nullptr;
   float *depth_pert = nullptr, *sc_depth = nullptr, *sc_prox = nullptr, *sc_marker = nullptr;
+  float2* sn_ring = nullptr; float* sm_ring = nullptr;   // read-delay rings of the scalar readouts (R10)
   // timing of the main kernel
   bool timing = false;
   bool timing_detail = false;   // events between the kernels of a step too (enable = 2)
@@ -109,7 +110,7 @@ void free_all(ts_ctx* c) {
   cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw);
   cudaFree(c->pc_pts); cudaFree(c->pc_cell); cudaFree(c->pc_grid); cudaFree(c->pc_id); cudaFree(c->tx_patch);
   cudaFree(c->sn_h); cudaFree(c->sn_d); cudaFree(c->sm_h); cudaFree(c->sm_d); cudaFree(c->depth_pert); cudaFree(c->sc_depth);
-  cudaFree(c->sc_prox); cudaFree(c->sc_marker);
+  cudaFree(c->sc_prox); cudaFree(c->sc_marker); cudaFree(c->sn_ring); cudaFree(c->sm_ring);
   for (float* q : c->stage_in) cudaFree(q);
   for (void* q : c->stage_out) cudaFree(q);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
@@ -178,6 +179,7 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
   p.ft_pert = (p.rho != 0.f && !c->fused) ? c->ft_scratch_r : nullptr;
   p.ext = cfg_ext(g);
   p.sn_h = c->sn_h; p.sn_d = c->sn_d; p.sm_h = c->sm_h; p.sm_d = c->sm_d; p.depth_pert = c->depth_pert;
+  p.sn_ring = c->sn_ring; p.sm_ring = c->sm_ring;
   for (int k = 0; k < 3; ++k) {
     p.sn_sigma_white[k] = g.sn_sigma_white[k]; p.sn_sigma_rw[k] = g.sn_sigma_rw[k]; p.sn_bias[k] = g.sn_bias[k];
     p.sn_quant[k] = g.sn_quant[k]; p.sn_stuck_min[k] = g.sn_stuck_min[k]; p.sn_stuck_max[k] = g.sn_stuck_max[k];
@@ -473,6 +475,17 @@ ts_status ts_create(const ts_config* cfg, int cuda_device, ts_ctx** out) {
     TS_ALLOC(c->sm_h, sizeof(float) * E * M * 6);
     TS_ALLOC(c->sm_d, sizeof(float) * E * M * 3);
     if (!(cfg->output_mask & TS_OUT_MARKER)) TS_ALLOC(c->sc_marker, sizeof(float) * E * M * 3);
+  }
+  if (cfg->noise_enable && cfg->read_delay + cfg->read_jitter > 0) {   // Eq. 25 read delay of the scalar readouts (R10)
+    const size_t S = (size_t)(cfg->read_delay + cfg->read_jitter);
+    if (cfg->output_mask & (TS_OUT_DEPTH_NOISY | TS_OUT_PROX_NOISY)) {
+      TS_ALLOC(c->sn_ring, sizeof(float2) * E * S * T);
+      if (cudaMemset(c->sn_ring, 0, sizeof(float2) * E * S * T) != cudaSuccess) { free_all(c); delete c; return fail(nullptr, TS_ERR_CUDA, "ts_create: cudaMemset ring"); }
+    }
+    if ((cfg->output_mask & TS_OUT_MARKER_NOISY) && M > 0) {
+      TS_ALLOC(c->sm_ring, sizeof(float) * E * S * M * 3);
+      if (cudaMemset(c->sm_ring, 0, sizeof(float) * E * S * M * 3) != cudaSuccess) { free_all(c); delete c; return fail(nullptr, TS_ERR_CUDA, "ts_create: cudaMemset ring"); }
+    }
   }
   if (cfg->noise_enable) {
     if (c->nh) TS_ALLOC(c->st_hyst, sizeof(float) * E * c->nh * c->Tp);
@@ -909,7 +922,7 @@ ts_status ts_depth_static(int32_t n_envs, int32_t n_links, int32_t n_taxels, con
 
 // ---- checkpoint / resume ----------------------------------------------------------------------------------------
 namespace {
-constexpr int kStateSections = 12;
+constexpr int kStateSections = 14;
 struct StateHeader {            // 160 bytes
   uint64_t magic, total;
   uint32_t version, n_envs, n_taxels, tp, nh, n_markers, ring_slots, pc_n, n_patches, objs, gstep, n_sections;
@@ -937,6 +950,9 @@ void state_sections(const ts_ctx* c, StateSection s[kStateSections], uint32_t* r
   s[9] = {c->sm_d, c->sm_d ? sizeof(float) * E * M * 3 : 0};
   s[10] = {c->sh_on, nsh};
   s[11] = {c->sh_e, sizeof(float4) * nsh};
+  const uint64_t Sr = (uint64_t)(c->cfg.read_delay + c->cfg.read_jitter);
+  s[12] = {c->sn_ring, c->sn_ring ? sizeof(float2) * E * Sr * T : 0};
+  s[13] = {c->sm_ring, c->sm_ring ? sizeof(float) * E * Sr * M * 3 : 0};
 }
 
 StateHeader state_header(const ts_ctx* c, const StateSection s[kStateSections], uint32_t ring_slots) {

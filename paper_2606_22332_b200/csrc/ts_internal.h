@@ -158,6 +158,9 @@ struct TsStepParams {
   const float4* pc_raw;       // [G,N] tracked points in their original order (the grid-sorted copy serves the proximity query)
   int32_t shear_enable;
   float s_s, lambda_s, eta_enter, eta_exit;
+  // read delay of the noisy scalar readouts (R10): the last rd_S post-hysteresis signals
+  float2* sn_ring;            // [E, rd_S, T] (depth, prox); NULL = no delay or outputs not requested
+  float* sm_ring;             // [E, rd_S, M, 3] markers
   // state
   uint8_t* st_flags;          // [E,T] bit0 Schmitt, bit1 dead
   float* st_hyst;             // [E,nh/2,Tp] float2 channel pairs, nh = 6 (asym: y) / 12 (maxwell: xi then x_prev)

@@ -1410,7 +1410,8 @@ __global__ void ts_reset_state_kernel(const __grid_constant__ TsStepParams p, co
 // ---------------------------------------------------------------------------------------
 template <int MODE>
 __device__ __forceinline__ float scalar_chain(const TsStepParams& p, int cls, float clean, float gain, bool dead, float stuck_u,
-                                              float z_rw, float z_w, float& ha, float& hb, float& drift) {
+                                              float z_rw, float z_w, float& ha, float& hb, float& drift, bool use_delayed,
+                                              float delayed, float& hrec) {
   const float x = gain * clean;
   float h = x;
   if (MODE == TS_HYST_MAXWELL) {            // Eq. 29-30
@@ -1422,6 +1423,8 @@ __device__ __forceinline__ float scalar_chain(const TsStepParams& p, int cls, fl
     h = fmaf(al, x - ha, ha);
     ha = h;
   }
+  hrec = h;                                 // this step's signal, for the read-delay ring
+  if (use_delayed) h = delayed;             // Eq. 25: y_{t - Delta_n}; bias, white noise and drift are those of step t
   drift = fmaf(p.sn_sigma_rw[cls], z_rw, drift);
   float y = fmaf(p.sn_sigma_white[cls], z_w, h + p.sn_bias[cls]) + drift;
   const float q = p.sn_quant[cls];
@@ -1431,6 +1434,18 @@ __device__ __forceinline__ float scalar_chain(const TsStepParams& p, int cls, fl
 }
 
 __device__ __forceinline__ float u24(uint32_t w) { return (float)(2u * (w >> 9) + 1u) * 5.9604644775390625e-8f; }
+
+// Delta_n of the read delay (R9): max(0, Delta + k_n), k_n uniform on {-J..J}, ONE draw per (env, step) shared by every
+// sensor of the env: stream 9, taxel word 0xffffffff (the draw the force / torque chain makes).
+__device__ __forceinline__ int read_delay_steps(const TsStepParams& p, uint32_t env, uint32_t nstep, uint32_t ep4) {
+  int delta = p.rd_delay;
+  if (p.rd_jitter > 0) {
+    const uint4 w = philox4x32_10(make_uint4(env, 0xffffffffu, nstep, ep4 | 9u), p.seed_lo, p.seed_hi);
+    const int k = (int)(((unsigned long long)(w.x >> 9) * (unsigned long long)(2 * p.rd_jitter + 1)) >> 23) - p.rd_jitter;
+    delta = max(0, p.rd_delay + k);
+  }
+  return delta;
+}
 
 // Threads [0, E T): depth + prox of one taxel (probe draws of the taxel: gain stream 3, dead flag from the state;
 // stream 10 -> (z_rw, z_w) of depth and of prox, stream 11 -> stuck values).  Threads [E T, E T + E M): the three
@@ -1463,14 +1478,29 @@ __global__ void __launch_bounds__(256) ts_scalar_noise_kernel(const __grid_const
       float2 dr = p.sn_d[gt];
       const float cd = p.depth_pert ? __ldcs(p.depth_pert + gt) : (p.depth ? p.depth[gt] : 0.f);
       const float cp = p.prox ? p.prox[gt] : 0.f;
+      // read delay: ring slot n mod S holds the signal of step n (and of step n - S: read first, write last)
+      const bool ring_on = p.sn_ring != nullptr && p.rd_S > 0;
+      bool use_del = false;
+      float2 del = make_float2(0.f, 0.f);
+      float2* ring_w = nullptr;
+      if (ring_on) {
+        const unsigned S = (unsigned)p.rd_S;
+        float2* const ring = p.sn_ring + (size_t)e * S * p.T + j;
+        const int delta = read_delay_steps(p, env, nstep, ep4);
+        use_del = delta > 0;
+        if (use_del && nstep >= (uint32_t)delta) del = ring[(size_t)((nstep - (uint32_t)delta) % S) * p.T];   // else: before the episode (Q12)
+        ring_w = ring + (size_t)(nstep % S) * p.T;
+      }
+      float2 rec = make_float2(0.f, 0.f);
       if (MODE == TS_HYST_MAXWELL) {
-        od = scalar_chain<MODE>(p, 0, cd, gain, dead, su_d, zd0, zd1, hs.x, hs.y, dr.x);
-        op = scalar_chain<MODE>(p, 1, cp, gain, dead, su_p, zp0, zp1, hs.z, hs.w, dr.y);
+        od = scalar_chain<MODE>(p, 0, cd, gain, dead, su_d, zd0, zd1, hs.x, hs.y, dr.x, use_del, del.x, rec.x);
+        op = scalar_chain<MODE>(p, 1, cp, gain, dead, su_p, zp0, zp1, hs.z, hs.w, dr.y, use_del, del.y, rec.y);
       } else {
         float dummy = 0.f;
-        od = scalar_chain<MODE>(p, 0, cd, gain, dead, su_d, zd0, zd1, hs.x, dummy, dr.x);
-        op = scalar_chain<MODE>(p, 1, cp, gain, dead, su_p, zp0, zp1, hs.y, dummy, dr.y);
+        od = scalar_chain<MODE>(p, 0, cd, gain, dead, su_d, zd0, zd1, hs.x, dummy, dr.x, use_del, del.x, rec.x);
+        op = scalar_chain<MODE>(p, 1, cp, gain, dead, su_p, zp0, zp1, hs.y, dummy, dr.y, use_del, del.y, rec.y);
       }
+      if (ring_w) *ring_w = rec;
       if (MODE != TS_HYST_OFF) p.sn_h[gt] = hs;
       p.sn_d[gt] = dr;
     }
@@ -1501,14 +1531,32 @@ __global__ void __launch_bounds__(256) ts_scalar_noise_kernel(const __grid_const
       float* hp = p.sm_h + gm * 6;
       float* dp = p.sm_d + gm * 3;
       const float* cm = p.marker + gm * 3;
+      const bool ring_on = p.sm_ring != nullptr && p.rd_S > 0;
+      bool use_del = false;
+      float del[3] = {0.f, 0.f, 0.f};
+      float* ring_w = nullptr;
+      if (ring_on) {
+        const unsigned S = (unsigned)p.rd_S;
+        float* const ring = p.sm_ring + ((size_t)e * S * p.M + m) * 3;
+        const int delta = read_delay_steps(p, env, nstep, ep4);
+        use_del = delta > 0;
+        if (use_del && nstep >= (uint32_t)delta) {
+          const float* r = ring + (size_t)((nstep - (uint32_t)delta) % S) * p.M * 3;
+          del[0] = r[0]; del[1] = r[1]; del[2] = r[2];
+        }
+        ring_w = ring + (size_t)(nstep % S) * p.M * 3;
+      }
+      float rec[3];
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
         float ha = MODE != TS_HYST_OFF ? hp[c] : 0.f, hb = MODE == TS_HYST_MAXWELL ? hp[3 + c] : 0.f, dr = dp[c];
-        out[c] = scalar_chain<MODE>(p, 2, cm[c], gain, dead, u24(wsv[c]), zr[c], c == 0 ? zr[3] : zw[c - 1], ha, hb, dr);
+        out[c] = scalar_chain<MODE>(p, 2, cm[c], gain, dead, u24(wsv[c]), zr[c], c == 0 ? zr[3] : zw[c - 1], ha, hb, dr, use_del,
+                                    del[c], rec[c]);
         if (MODE != TS_HYST_OFF) hp[c] = ha;
         if (MODE == TS_HYST_MAXWELL) hp[3 + c] = hb;
         dp[c] = dr;
       }
+      if (ring_w) { ring_w[0] = rec[0]; ring_w[1] = rec[1]; ring_w[2] = rec[2]; }
     }
     float* o = p.marker_noisy + gm * 3;
     __stcs(o, out[0]); __stcs(o + 1, out[1]); __stcs(o + 2, out[2]);

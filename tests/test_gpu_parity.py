@@ -417,8 +417,8 @@ def test_two_objects_per_env():
 def test_noisy_scalar_readouts():
     """SURVEY 8(f-1) / DESIGN.md R10: noisy depth, prox and marker readouts (Table 3 P:346-359 gives them every knob of
     App. A.8 except crosstalk) with the Table 12 values and beyond: white noise, drift, bias, quantisation,
-    gain, dead probes with stuck values, both hysteresis modes, the Eq. 26 radius for the depth readout, over a reset,
-    with and without the clean outputs requested next to them."""
+    gain, dead probes with stuck values, both hysteresis modes, the Eq. 26 radius for the depth readout, the read delay
+    with jitter, over a reset, with and without the clean outputs requested next to them."""
     import torch
     from oracle import oracle as O
     from parity import Comparator
@@ -432,7 +432,10 @@ def test_noisy_scalar_readouts():
     only = ("contact", "ft", "ft_noisy", "dead", "depth_noisy", "prox_noisy", "marker_noisy")   # clean inputs from scratch buffers
     cases = ((dict(w.noise, hyst_mode="maxwell", beta=0.5, tau=0.05, **t12), full),
              (dict(w.noise, **t12, **more), full),
-             (dict(w.noise, hyst_mode="off", **more), only))
+             (dict(w.noise, hyst_mode="off", **more), only),
+             # Eq. 25 read delay with jitter on every readout (Table 3): rings of 3 slots, delays 0..3 steps
+             (dict(w.noise, read_delay=2, read_jitter=1, **t12, **more), full),
+             (dict(w.noise, hyst_mode="maxwell", beta=0.5, tau=0.05, read_delay=1, read_jitter=1, **t12), only))
     for noise, outs in cases:
         sim = TactileSim(w.patches, w.T, w.E, w.L, w.K, physics=w.physics, noise=noise, outputs=outs)
         sim.set_geometry(w.types, w.params, w.bank, w.voxel)
