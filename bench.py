@@ -148,8 +148,8 @@ def oracle_arm(w, ids, steps, warmup, threads):
 def time_extras(W, TactileSim, torch, dev, n_envs=4096, steps=20):
     """Device time per step (CUDA events on the launch stream, mean of `steps` after 3 warm-up steps) of the SURVEY 8(f)
     sensor kernels: a context that asks for the extra output next to `depth`, minus the same context without it.
-    Workload: config 4 (8 star objects, 1,000 taxels) at 4,096 envs; tracked clouds of 5,000 (proximity) / 1,000
-    (shear) surface points and 1,280-triangle meshes per object."""
+    Workload: config 4 (8 star objects, 1,000 taxels) at 4,096 envs; tracked clouds of 5,000 surface points (the
+    shear kernel also with 1,000) and 1,280-triangle meshes per object."""
     w = W.config(4, n_envs=n_envs)
     stream = torch.cuda.current_stream(dev)
     inputs = None
@@ -184,7 +184,8 @@ def time_extras(W, TactileSim, torch, dev, n_envs=4096, steps=20):
     res["base_depth_only_ms"] = base
     res["proxpc_ms"] = run(("depth", "proxpc"), setup=lambda s: s.set_pointclouds(pts5, cid)) - base
     res["raycast_ms"] = run(("depth", "depth_rc", "nrm_rc"), setup=lambda s: s.set_meshes(meshes, mid)) - base
-    res["shear_ms"] = run(("depth", "marker"), physics=dict(w.physics, shear_enable=1), setup=lambda s: s.set_pointclouds(pts1, cid)) - base_m
+    res["shear_ms"] = run(("depth", "marker"), physics=dict(w.physics, shear_enable=1), setup=lambda s: s.set_pointclouds(pts5, cid)) - base_m
+    res["shear_1000pts_ms"] = run(("depth", "marker"), physics=dict(w.physics, shear_enable=1), setup=lambda s: s.set_pointclouds(pts1, cid)) - base_m
     t12 = dict(w.noise, sigma_white_depth=2e-4, sigma_white_prox=1e-2, sigma_rw_prox=1e-3, quant_prox=1e-2, sigma_white_marker=1e-4,
                sigma_rw_marker=1e-5, quant_marker=1e-4, gain_min=0.85, gain_max=1.15)
     full = tuple(w.outputs)
@@ -201,7 +202,7 @@ def time_extras(W, TactileSim, torch, dev, n_envs=4096, steps=20):
                                         "frac": ach / peak, "peak_source": src},
                        "proxpc": {"bound": "latency (dependent loads: run bounds -> points)", "frac": None},
                        "raycast": {"bound": "latency (BVH node -> children / triangles)", "frac": None},
-                       "shear": {"bound": "latency (anchor flag -> anchor; one double transform per tracked point per pad)", "frac": None}}
+                       "shear": {"bound": "latency (per-pad phases: flag scan -> anchored points -> prism rows -> candidates)", "frac": None}}
     return res
 
 

@@ -59,7 +59,7 @@ struct ts_ctx {
   float4* pc_pts = nullptr; int32_t* pc_cell = nullptr; TsPcGrid* pc_grid = nullptr; int32_t* pc_id = nullptr;
   int32_t* tx_patch = nullptr;
   int pc_n = 0; bool have_pc = false;
-  uint8_t* sh_on = nullptr; float4* sh_e = nullptr; float4* pc_raw = nullptr;   // elastomer shear history (Eq. 22)
+  uint8_t* sh_on = nullptr; float4* sh_e = nullptr; float4* pc_raw = nullptr; int32_t* sh_cnt = nullptr;   // elastomer shear history (Eq. 22)
   // noisy scalar readouts (R10): state, the perturbed depth (Eq. 26), scratch copies of clean inputs the caller did not ask for
   float4* sn_h = nullptr; float2* sn_d = nullptr; float *sm_h = nullptr, *sm_d = nullptr;
   float *depth_pert = nullptr, *sc_depth = nullptr, *sc_prox = nullptr, *sc_marker = nullptr;
@@ -107,7 +107,7 @@ void free_all(ts_ctx* c) {
   cudaFree(c->g_type); cudaFree(c->g_params); cudaFree(c->env_perm); cudaFree(c->frames_g); cudaFree(c->patch_link); cudaFree(c->bank); cudaFree(c->bank_stage); cudaFree(c->st_flags); cudaFree(c->st_hyst);
   cudaFree(c->st_drift); cudaFree(c->reset_step); cudaFree(c->episode); cudaFree(c->ft_scratch); cudaFree(c->ft_scratch_r); cudaFree(c->st_ring);
   cudaFree(c->rc_nodes); cudaFree(c->rc_tri); cudaFree(c->rc_root); cudaFree(c->rc_id);
-  cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw);
+  cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw); cudaFree(c->sh_cnt);
   cudaFree(c->pc_pts); cudaFree(c->pc_cell); cudaFree(c->pc_grid); cudaFree(c->pc_id); cudaFree(c->tx_patch);
   cudaFree(c->sn_h); cudaFree(c->sn_d); cudaFree(c->sm_h); cudaFree(c->sm_d); cudaFree(c->depth_pert); cudaFree(c->sc_depth);
   cudaFree(c->sc_prox); cudaFree(c->sc_marker); cudaFree(c->sn_ring); cudaFree(c->sm_ring);
@@ -185,9 +185,9 @@ void fill_params(const ts_ctx* c, TsStepParams& p) {
     p.sn_quant[k] = g.sn_quant[k]; p.sn_stuck_min[k] = g.sn_stuck_min[k]; p.sn_stuck_max[k] = g.sn_stuck_max[k];
   }
   p.dead_thr = c->dead_thr;
-  p.pc_pts = c->pc_pts; p.pc_cell = c->pc_cell; p.pc_grid = c->pc_grid; p.pc_id = c->pc_id; p.pc_n = c->pc_n; p.tx_patch = c->tx_patch;
+  p.pc_pts = c->pc_pts; p.pc_cell = c->pc_cell; p.pc_grid = c->pc_grid; p.pc_id = c->pc_id; p.pc_n = c->pc_n; p.pc_np = (c->pc_n + 15) / 16 * 16; p.tx_patch = c->tx_patch;
   p.pc_radius = g.pc_radius; p.pc_k = g.pc_k; p.pc_ks = g.pc_ks; p.pc_density = g.pc_density;
-  p.sh_on = c->sh_on; p.sh_e = c->sh_e; p.pc_raw = c->pc_raw;
+  p.sh_on = c->sh_on; p.sh_e = c->sh_e; p.pc_raw = c->pc_raw; p.sh_cnt = c->sh_cnt;
   p.rc_nodes = c->rc_nodes; p.rc_tri = c->rc_tri; p.rc_root = c->rc_root; p.rc_id = c->rc_id;
   p.shear_enable = (g.shear_enable && c->sh_on) ? 1 : 0; p.s_s = g.s_s; p.lambda_s = g.lambda_s; p.eta_enter = g.eta_enter; p.eta_exit = g.eta_exit;
 }
@@ -735,15 +735,19 @@ ts_status ts_set_pointclouds(ts_ctx* c, const ts_pointclouds* pc, void* stream) 
     }
     for (long long k = 0; k < ncell; ++k) start[k + 1] += start[k];
     std::vector<int32_t> fill(start.begin(), start.end() - 1);
-    for (int i = 0; i < N; ++i) sorted[(size_t)g * N + fill[cidx[i]]++] = make_float4(P[3 * i], P[3 * i + 1], P[3 * i + 2], 0.f);
+    for (int i = 0; i < N; ++i) {   // .w carries the point's index in the caller's order (the shear anchors are indexed by it)
+      float wi;
+      std::memcpy(&wi, &i, sizeof(float));
+      sorted[(size_t)g * N + fill[cidx[i]]++] = make_float4(P[3 * i], P[3 * i + 1], P[3 * i + 2], wi);
+    }
     cells.insert(cells.end(), start.begin(), start.end());
   }
   DeviceGuard guard(c->device);
   cudaStream_t st = (cudaStream_t)stream;
   c->have_pc = false;
   TS_CUDA(c, cudaStreamSynchronize(st));   // steps in flight may still read the old index
-  cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw);
-  c->sh_on = nullptr; c->sh_e = nullptr; c->pc_raw = nullptr;
+  cudaFree(c->sh_on); cudaFree(c->sh_e); cudaFree(c->pc_raw); cudaFree(c->sh_cnt);
+  c->sh_on = nullptr; c->sh_e = nullptr; c->pc_raw = nullptr; c->sh_cnt = nullptr;
   cudaFree(c->pc_pts); cudaFree(c->pc_cell); cudaFree(c->pc_grid); cudaFree(c->pc_id);
   c->pc_pts = nullptr; c->pc_cell = nullptr; c->pc_grid = nullptr; c->pc_id = nullptr;
   TS_CUDA(c, cudaMalloc((void**)&c->pc_pts, sizeof(float4) * sorted.size()));
@@ -755,13 +759,16 @@ ts_status ts_set_pointclouds(ts_ctx* c, const ts_pointclouds* pc, void* stream) 
   TS_CUDA(c, cudaMemcpyAsync(c->pc_grid, grids.data(), sizeof(TsPcGrid) * G, cudaMemcpyHostToDevice, st));
   TS_CUDA(c, cudaMemcpyAsync(c->pc_id, pc->cloud_id, sizeof(int32_t) * EK, cudaMemcpyHostToDevice, st));
   if (c->cfg.shear_enable && c->M > 0) {   // Eq. 22 anchors: one per (env, patch, object, tracked point)
-    const size_t ns = (size_t)c->cfg.n_envs * c->P * c->cfg.objs_per_env * N;
+    const size_t ns = (size_t)c->cfg.n_envs * c->P * c->cfg.objs_per_env * (size_t)((N + 15) / 16 * 16);
     std::vector<float4> raw((size_t)G * N);
     for (size_t i = 0; i < raw.size(); ++i) raw[i] = make_float4(pc->points[3 * i], pc->points[3 * i + 1], pc->points[3 * i + 2], 0.f);
     TS_CUDA(c, cudaMalloc((void**)&c->sh_on, ns));
     TS_CUDA(c, cudaMalloc((void**)&c->sh_e, sizeof(float4) * ns));
     TS_CUDA(c, cudaMalloc((void**)&c->pc_raw, sizeof(float4) * raw.size()));
     TS_CUDA(c, cudaMemsetAsync(c->sh_on, 0, ns, st));
+    const size_t ncnt = (size_t)c->cfg.n_envs * c->P * c->cfg.objs_per_env;
+    TS_CUDA(c, cudaMalloc((void**)&c->sh_cnt, sizeof(int32_t) * ncnt));
+    TS_CUDA(c, cudaMemsetAsync(c->sh_cnt, 0, sizeof(int32_t) * ncnt, st));
     TS_CUDA(c, cudaMemcpyAsync(c->pc_raw, raw.data(), sizeof(float4) * raw.size(), cudaMemcpyHostToDevice, st));
   }
   TS_CUDA(c, cudaStreamSynchronize(st));
@@ -922,7 +929,7 @@ ts_status ts_depth_static(int32_t n_envs, int32_t n_links, int32_t n_taxels, con
 
 // ---- checkpoint / resume ----------------------------------------------------------------------------------------
 namespace {
-constexpr int kStateSections = 14;
+constexpr int kStateSections = 15;
 struct StateHeader {            // 160 bytes
   uint64_t magic, total;
   uint32_t version, n_envs, n_taxels, tp, nh, n_markers, ring_slots, pc_n, n_patches, objs, gstep, n_sections;
@@ -936,7 +943,7 @@ struct StateSection { void* dev; uint64_t bytes; };
 void state_sections(const ts_ctx* c, StateSection s[kStateSections], uint32_t* ring_slots) {
   const uint64_t E = (uint64_t)c->cfg.n_envs, T = (uint64_t)c->T, M = (uint64_t)c->M, Tp = (uint64_t)c->Tp;
   const uint32_t S = c->st_ring ? (uint32_t)(c->cfg.read_delay + c->cfg.read_jitter) : 0u;
-  const uint64_t nsh = c->sh_on ? E * (uint64_t)c->P * (uint64_t)c->cfg.objs_per_env * (uint64_t)c->pc_n : 0;
+  const uint64_t nsh = c->sh_on ? E * (uint64_t)c->P * (uint64_t)c->cfg.objs_per_env * (uint64_t)((c->pc_n + 15) / 16 * 16) : 0;
   *ring_slots = S;
   s[0] = {c->st_flags, E * T};
   s[1] = {c->reset_step, sizeof(uint32_t) * E};
@@ -953,6 +960,7 @@ void state_sections(const ts_ctx* c, StateSection s[kStateSections], uint32_t* r
   const uint64_t Sr = (uint64_t)(c->cfg.read_delay + c->cfg.read_jitter);
   s[12] = {c->sn_ring, c->sn_ring ? sizeof(float2) * E * Sr * T : 0};
   s[13] = {c->sm_ring, c->sm_ring ? sizeof(float) * E * Sr * M * 3 : 0};
+  s[14] = {c->sh_cnt, c->sh_cnt ? sizeof(int32_t) * E * (uint64_t)c->P * (uint64_t)c->cfg.objs_per_env : 0};
 }
 
 StateHeader state_header(const ts_ctx* c, const StateSection s[kStateSections], uint32_t ring_slots) {

@@ -144,6 +144,7 @@ struct TsStepParams {
   const struct TsPcGrid* pc_grid;  // [G]
   const int32_t* pc_id;       // [E,K] cloud of each object, -1 = none
   int32_t pc_n;               // points per cloud
+  int32_t pc_np;              // pc_n rounded up to 16: stride of the shear anchor rows (16-byte aligned flag rows)
   float pc_radius, pc_k, pc_ks, pc_density;
   // raycast depth backend (A.1): BVH nodes and leaf-ordered triangles of every mesh
   float* depth_rc;            // [E,T]
@@ -153,8 +154,9 @@ struct TsStepParams {
   const int32_t* rc_root;     // [G] root node of each mesh
   const int32_t* rc_id;       // [E,K] mesh of each object, -1 = none
   // elastomer shear history (Eq. 22): anchors per (env, patch, object, tracked point)
-  uint8_t* sh_on;             // [E,P,K,N] anchored?
-  float4* sh_e;               // [E,P,K,N] anchor relative to the pad centre (link frame); only read where sh_on is set
+  uint8_t* sh_on;             // [E,P,K,Np] anchored?  (Np = pc_np)
+  int32_t* sh_cnt;            // [E,P,K] number of anchored points (lets a pad with none skip the flag scan)
+  float4* sh_e;               // [E,P,K,Np] anchor relative to the pad centre (link frame); only read where sh_on is set
   const float4* pc_raw;       // [G,N] tracked points in their original order (the grid-sorted copy serves the proximity query)
   int32_t shear_enable;
   float s_s, lambda_s, eta_enter, eta_exit;

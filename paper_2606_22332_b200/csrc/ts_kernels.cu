@@ -1734,10 +1734,18 @@ __global__ void __launch_bounds__(128, TS_PC_MINB) ts_proxpc_kernel(const __grid
 #endif
 __global__ void __launch_bounds__(256, TS_SH_MINB) ts_shear_kernel(const __grid_constant__ TsStepParams p) {
   __shared__ double Rm[9], tv[3];
+  __shared__ float prism[12];         // the pad's frame in the object frame: u = a_u . p + b_u, v = a_v . p + b_v, phi_el = a_n . p + b_n
+  __shared__ int b2_on, dcnt;         // can any point of the cloud lie behind the pad plane?  change of the anchored count
   __shared__ float4 qd[TS_SHEAR_Q];   // (tangential slide x, y, z, h_p)
   __shared__ float4 qz[TS_SHEAR_Q];   // z_p relative to the pad centre
-  __shared__ int wcnt[2][8];          // anchored points per warp of the current pass (double-buffered by pass parity)
-  const int e = blockIdx.x / p.P, pi = blockIdx.x - e * p.P, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  __shared__ int wcnt[2][8];          // queued points per warp of the current pass (double-buffered by pass parity)
+  __shared__ uint4 fl[256];           // anchor flags of the current chunk, 16 per thread
+  __shared__ int pfx[257];            // exclusive prefix of the set flags per thread; [256] = total
+  __shared__ int wtot[8];
+  // Blocks run in the step kernel's env order: the relative poses of this step are still in frames_g (row bx = env
+  // env_perm[bx]), so no pose is rebuilt here (a one-thread rebuild was most of a block's life for pads that touch nothing).
+  const int bx = blockIdx.x / p.P, pi = blockIdx.x - bx * p.P, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int e = p.env_perm ? __ldg(p.env_perm + bx) : bx;
   const TsPatch& pt = p.patches[pi];
   const int mcount = __ldg(&pt.mnu) * __ldg(&pt.mnv), link = __ldg(&pt.link);
   if (mcount == 0 || link < 0) return;
@@ -1746,7 +1754,7 @@ __global__ void __launch_bounds__(256, TS_SH_MINB) ts_shear_kernel(const __grid_
   const D3 n = D3{(double)na.x, (double)na.y, (double)na.z}, uu = D3{(double)ua.x, (double)ua.y, (double)ua.z}, vv = D3{(double)va.x, (double)va.y, (double)va.z};
   const D3 xc = D3{(double)ctr.x, (double)ctr.y, (double)ctr.z};
   const double hu = 0.5 * (double)ua.w, hv = 0.5 * (double)va.w;
-  const int N = p.pc_n;
+  const int N = p.pc_n, Np = p.pc_np;
   float ax = 0.f, ay = 0.f, az = 0.f;   // this thread's marker (tid < mcount): shear sum
   float mx = 0.f, my = 0.f, mz = 0.f;
   if (tid < mcount) {
@@ -1765,79 +1773,219 @@ __global__ void __launch_bounds__(256, TS_SH_MINB) ts_shear_kernel(const __grid_
       ax = fmaf(wgt, d4.x, ax); ay = fmaf(wgt, d4.y, ay); az = fmaf(wgt, d4.z, az);
     }
   };
+  // pad SDF of a tracked point given in the object frame (R11): +inf beside the pad, n . (z - x_c) over it
+  auto pad_phi = [&](float4 po, D3& rel) {
+    const D3 z = D3{tv[0], tv[1], tv[2]} + mulR(Rm, D3{(double)po.x, (double)po.y, (double)po.z});
+    rel = z - xc;
+    double phi_el = __longlong_as_double(0x7ff0000000000000LL);
+    if (fabs(dot(rel, uu)) <= hu && fabs(dot(rel, vv)) <= hv) phi_el = dot(rel, n);
+    return phi_el;
+  };
   int pass = 0;
   for (int k = 0; k < p.K; ++k) {
     const int id = __ldg(p.pc_id + (size_t)e * p.K + k);   // block-uniform
     if (id < 0) continue;
     __syncthreads();
-    if (tid == 0) {
-      const size_t el = (size_t)e * p.L + link, ek = (size_t)e * p.K + k;
-      double RL[9], RO[9];
-      quat_Rd(p.link_quat + el * 4, RL);
-      quat_Rd(p.obj_quat + ek * 4, RO);
-      const D3 d = ld3d(p.obj_pos + ek * 3) - ld3d(p.link_pos + el * 3);
-      const D3 t = mulRT(RL, d);
-      tv[0] = t.x; tv[1] = t.y; tv[2] = t.z;
-      for (int r = 0; r < 3; ++r)
-        for (int c2 = 0; c2 < 3; ++c2) Rm[r * 3 + c2] = fma(RL[r], RO[c2], fma(RL[3 + r], RO[3 + c2], RL[6 + r] * RO[6 + c2]));   // R_L^T R_O
+    if (tid < 12) {   // R_L^T R_O = M^T and R_L^T (p_O - p_L) = -cbar of the frame (link of this pad, object k)
+      const FrameS* F = reinterpret_cast<const FrameS*>(p.frames_g) + ((size_t)bx * p.P + pi) * p.K + k;
+      if (tid < 9) Rm[tid] = F->M[(tid % 3) * 3 + tid / 3];
+      else tv[tid - 9] = -F->cbar[tid - 9];
     }
     __syncthreads();
-    const size_t sbase = (((size_t)e * p.P + pi) * p.K + k) * N;
-    for (int i0 = 0; i0 < N; i0 += 256, ++pass) {
-      if (qn > TS_SHEAR_Q - 256) {           // a pass queues at most 256 points: drain before the queue could overflow
-        __syncthreads();
-        shear_drain();
-        qn = 0;
-        __syncthreads();
+    if (tid == 0) {
+      const D3 t = D3{tv[0], tv[1], tv[2]};
+      const D3 au = mulRT(Rm, uu), av = mulRT(Rm, vv), tc = t - xc;
+      prism[0] = (float)au.x; prism[1] = (float)au.y; prism[2] = (float)au.z; prism[3] = (float)dot(uu, tc);
+      prism[4] = (float)av.x; prism[5] = (float)av.y; prism[6] = (float)av.z; prism[7] = (float)dot(vv, tc);
+      const D3 an = mulRT(Rm, n);
+      const double bn = dot(n, tc);
+      prism[8] = (float)an.x; prism[9] = (float)an.y; prism[10] = (float)an.z; prism[11] = (float)bn;
+      // smallest phi_el over the cloud's bounding box: if even that is not behind the pad plane, nothing can anchor
+      const TsPcGrid g = p.pc_grid[id];
+      const double w = 1.0 / (double)g.inv_cell;
+      const double lo3[3] = {(double)g.ox, (double)g.oy, (double)g.oz}, ext[3] = {g.nx * w, g.ny * w, g.nz * w}, a3[3] = {an.x, an.y, an.z};
+      double pmin = bn;
+      for (int ax2 = 0; ax2 < 3; ++ax2) pmin += fmin(a3[ax2] * lo3[ax2], a3[ax2] * (lo3[ax2] + ext[ax2]));
+      b2_on = pmin < -(double)p.eta_enter + 1e-6 ? 1 : 0;
+      dcnt = 0;
+    }
+    __syncthreads();
+    const size_t sbase = (((size_t)e * p.P + pi) * p.K + k) * (size_t)Np;   // a multiple of 16: the flag rows are 16-byte aligned
+    int* const cntp = p.sh_cnt + ((size_t)e * p.P + pi) * p.K + k;          // anchored points of this (env, pad, object)
+    const int cnt0 = *cntp;                                                  // block-uniform
+    const int NpB1 = cnt0 > 0 ? Np : 0;                                      // nothing anchored: no flag scan at all
+    // ---- phase B1: the points that are anchored, found by a scan of the flag bytes (16 per thread and chunk), taken in
+    // index order: exit test, and the penetrating ones go to the queue.  Work ~ N / 16 loads + the anchored points.
+    for (int c0 = 0; c0 < NpB1; c0 += 4096) {
+      __syncthreads();                     // fl / pfx of the previous chunk are no longer read
+      uint4 f = make_uint4(0u, 0u, 0u, 0u);
+      const int off = c0 + tid * 16;
+      if (off < Np) f = *reinterpret_cast<const uint4*>(p.sh_on + sbase + off);
+      fl[tid] = f;
+      const int cnt = __popc(f.x & 0x01010101u) + __popc(f.y & 0x01010101u) + __popc(f.z & 0x01010101u) + __popc(f.w & 0x01010101u);
+      int inc = cnt;                       // inclusive scan inside the warp
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(TS_FULL, inc, o);
+        if (lane >= o) inc += v;
       }
-      const int i = i0 + tid;
-      bool push = false;
-      float4 vd = make_float4(0.f, 0.f, 0.f, 0.f), vz = vd;
-      if (i < N) {
-        const float4 po = __ldg(p.pc_raw + (size_t)id * N + i);
-        const D3 z = D3{tv[0], tv[1], tv[2]} + mulR(Rm, D3{(double)po.x, (double)po.y, (double)po.z});
-        const D3 rel = z - xc;
-        double phi_el = __longlong_as_double(0x7ff0000000000000LL);
-        if (fabs(dot(rel, uu)) <= hu && fabs(dot(rel, vv)) <= hv) phi_el = dot(rel, n);
-        uint8_t on = p.sh_on[sbase + i];
-        float4 anc = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (!on && phi_el < -(double)p.eta_enter) {
-          on = 1; anc = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
-          p.sh_on[sbase + i] = 1; p.sh_e[sbase + i] = anc;
-        } else if (on && phi_el > (double)p.eta_exit) {
-          on = 0; p.sh_on[sbase + i] = 0;
-        } else if (on) {
-          anc = p.sh_e[sbase + i];
-        }
-        if (on && phi_el < 0.0) {
-          const D3 dz = D3{rel.x - (double)anc.x, rel.y - (double)anc.y, rel.z - (double)anc.z};
-          const D3 dzt = dz - dot(dz, n) * n;                          // Pi_n(z_p - e_p)
-          push = true;
-          vd = make_float4((float)dzt.x, (float)dzt.y, (float)dzt.z, (float)(-phi_el));
-          vz = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
-        }
-      }
-      // Ordered compaction: the queue holds the anchored points in index order, so the fp32 sums below are the same from
-      // run to run (a shared-memory atomic counter would enqueue in arrival order).
-      const unsigned bal = __ballot_sync(TS_FULL, push);
-      if (lane == 0) wcnt[pass & 1][warp] = __popc(bal);
+      if (lane == 31) wtot[warp] = inc;
       __syncthreads();
-      int base = qn, tot = 0;
+      int wb = 0, total = 0;
 #pragma unroll
       for (int w2 = 0; w2 < 8; ++w2) {
-        const int c2 = wcnt[pass & 1][w2];
-        if (w2 < warp) base += c2;
-        tot += c2;
+        const int c2 = wtot[w2];
+        if (w2 < warp) wb += c2;
+        total += c2;
       }
-      if (push) {
-        const int slot = base + __popc(bal & ((1u << lane) - 1u));     // < TS_SHEAR_Q by the drain rule above
-        qd[slot] = vd; qz[slot] = vz;
+      pfx[tid] = wb + inc - cnt;
+      if (tid == 0) pfx[256] = total;
+      __syncthreads();
+      for (int m0 = 0; m0 < total; m0 += 256, ++pass) {
+        if (qn > TS_SHEAR_Q - 256) {       // a pass queues at most 256 points: drain before the queue could overflow
+          __syncthreads();
+          shear_drain();
+          qn = 0;
+          __syncthreads();
+        }
+        const int m = m0 + tid;
+        bool push = false;
+        float4 vd = make_float4(0.f, 0.f, 0.f, 0.f), vz = vd;
+        if (m < total) {
+          int lo = 0, hi = 255;            // owner: the last thread whose prefix is <= m
+          while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (pfx[mid] <= m) lo = mid; else hi = mid - 1;
+          }
+          const uint4 g = fl[lo];
+          const unsigned wv[4] = {g.x, g.y, g.z, g.w};
+          int kth = m - pfx[lo], byte = 0;
+#pragma unroll
+          for (int b2 = 0; b2 < 16; ++b2) {
+            const int bit = (int)((wv[b2 >> 2] >> ((b2 & 3) * 8)) & 1u);
+            if (bit && kth == 0) byte = b2;
+            kth -= bit;
+          }
+          const int i = c0 + lo * 16 + byte;   // < N: flags past N are never set
+          D3 rel;
+          const double phi_el = pad_phi(__ldg(p.pc_raw + (size_t)id * N + i), rel);
+          if (phi_el > (double)p.eta_exit) {
+            p.sh_on[sbase + i] = 0;
+            atomicSub(&dcnt, 1);
+          } else if (phi_el < 0.0) {
+            const float4 anc = p.sh_e[sbase + i];
+            const D3 dz = D3{rel.x - (double)anc.x, rel.y - (double)anc.y, rel.z - (double)anc.z};
+            const D3 dzt = dz - dot(dz, n) * n;                          // Pi_n(z_p - e_p)
+            push = true;
+            vd = make_float4((float)dzt.x, (float)dzt.y, (float)dzt.z, (float)(-phi_el));
+            vz = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
+          }
+        }
+        // Ordered compaction: the queue holds the anchored points in index order, so the fp32 sums below are the same
+        // from run to run (a shared-memory atomic counter would enqueue in arrival order).
+        const unsigned bal = __ballot_sync(TS_FULL, push);
+        if (lane == 0) wcnt[pass & 1][warp] = __popc(bal);
+        __syncthreads();
+        int base = qn, tot = 0;
+#pragma unroll
+        for (int w2 = 0; w2 < 8; ++w2) {
+          const int c2 = wcnt[pass & 1][w2];
+          if (w2 < warp) base += c2;
+          tot += c2;
+        }
+        if (push) {
+          const int slot = base + __popc(bal & ((1u << lane) - 1u));     // < TS_SHEAR_Q by the drain rule above
+          qd[slot] = vd; qz[slot] = vz;
+        }
+        qn += tot;
       }
-      qn += tot;
     }
     __syncthreads();
     shear_drain();
     qn = 0;
+    // ---- phase B2: new anchors.  Only points inside the pad's prism can anchor, so the cloud's grid is walked by rows
+    // of cells (x fastest): per row the x-interval that can meet the prism, then the points of that run of cells that are
+    // not anchored yet.  A point anchored here contributes nothing this step (z_p = e_p), so it is not queued.
+    if (b2_on) {   // block-uniform
+      const TsPcGrid g = p.pc_grid[id];
+      const float cw = __frcp_rn(g.inv_cell), rc = 0.7072f * cw + 1e-5f;
+      const float Hu = (float)hu + rc, Hv = (float)hv + rc, Hn = rc - p.eta_enter;
+      const float4* pts = p.pc_pts + g.pt0;
+      const int nrows = g.ny * g.nz;
+      const float inv_ny = 1.0f / (float)g.ny;
+      int* const runb = reinterpret_cast<int*>(fl);   // first point of each thread's run (fl is free after phase B1)
+      for (int r0 = 0; r0 < nrows; r0 += 256) {
+        // one row of cells per thread: the run of points that can meet the prism behind the pad plane (possibly empty)
+        const int row = r0 + tid;
+        int rb = 0, rlen = 0;
+        if (row < nrows) {
+          const int kk = (int)(((float)row + 0.5f) * inv_ny), jj = row - kk * g.ny;   // exact: row, ny < 2^20
+          const float yc = g.oy + ((float)jj + 0.5f) * cw, zc = g.oz + ((float)kk + 0.5f) * cw;
+          float xlo = g.ox, xhi = g.ox + (float)g.nx * cw;
+          bool any = true;
+#pragma unroll
+          for (int s2 = 0; s2 < 3; ++s2) {   // slabs |u| <= Hu, |v| <= Hv and the half-space phi_el <= Hn along the line (x, yc, zc)
+            const float a = prism[4 * s2], c1 = fmaf(prism[4 * s2 + 1], yc, fmaf(prism[4 * s2 + 2], zc, prism[4 * s2 + 3]));
+            const float H = s2 == 0 ? Hu : (s2 == 1 ? Hv : Hn);
+            if (fabsf(a) < 1e-6f) {
+              any = any && c1 <= H + 1e-4f && (s2 == 2 || c1 >= -H - 1e-4f);
+            } else {
+              const float ia = __frcp_rn(a);
+              const float x1 = (H - c1) * ia, x0 = s2 == 2 ? (a > 0.f ? -3.0e38f : 3.0e38f) : (-H - c1) * ia;
+              xlo = fmaxf(xlo, fminf(x0, x1)); xhi = fminf(xhi, fmaxf(x0, x1));
+            }
+          }
+          if (any && xlo <= xhi) {           // +- one cell of slack covers the rounding of the interval ends
+            const int i0 = max((int)floorf((xlo - g.ox) * g.inv_cell) - 1, 0), i1 = min((int)floorf((xhi - g.ox) * g.inv_cell) + 1, g.nx - 1);
+            if (i0 <= i1) {
+              const int cell = g.cell0 + row * g.nx;
+              rb = __ldg(p.pc_cell + cell + i0);
+              rlen = __ldg(p.pc_cell + cell + i1 + 1) - rb;
+            }
+          }
+        }
+        // the candidates of all rows, dealt to the threads one point each (a row's thread walking its own run left 3 of 32
+        // lanes busy): block prefix of the run lengths, then point m belongs to the last row whose prefix is <= m
+        __syncthreads();                     // runb / pfx of the previous batch (or of phase B1) are no longer read
+        runb[tid] = rb;
+        int inc = rlen;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const int v = __shfl_up_sync(TS_FULL, inc, o);
+          if (lane >= o) inc += v;
+        }
+        if (lane == 31) wtot[warp] = inc;
+        __syncthreads();
+        int wb = 0, total = 0;
+#pragma unroll
+        for (int w2 = 0; w2 < 8; ++w2) {
+          const int c2 = wtot[w2];
+          if (w2 < warp) wb += c2;
+          total += c2;
+        }
+        pfx[tid] = wb + inc - rlen;
+        __syncthreads();
+        for (int m = tid; m < total; m += 256) {
+          int lo = 0, hi = 255;
+          while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (pfx[mid] <= m) lo = mid; else hi = mid - 1;
+          }
+          const float4 po = __ldg(pts + runb[lo] + (m - pfx[lo]));
+          const int i = __float_as_int(po.w);                            // index of the point in the caller's order
+          if (p.sh_on[sbase + i]) continue;
+          D3 rel;
+          const double phi_el = pad_phi(po, rel);
+          if (phi_el < -(double)p.eta_enter) {
+            p.sh_on[sbase + i] = 1;
+            p.sh_e[sbase + i] = make_float4((float)rel.x, (float)rel.y, (float)rel.z, 0.f);
+            atomicAdd(&dcnt, 1);
+          }
+        }
+      }
+    }
+    __syncthreads();
+    if (tid == 0 && dcnt != 0) *cntp = cnt0 + dcnt;
   }
   if (tid < mcount && (ax != 0.f || ay != 0.f || az != 0.f)) {
     float* o = p.marker + ((size_t)e * p.M + __ldg(&pt.mstart) + tid) * 3;
@@ -1846,12 +1994,14 @@ __global__ void __launch_bounds__(256, TS_SH_MINB) ts_shear_kernel(const __grid_
 }
 
 __global__ void ts_reset_shear_kernel(const __grid_constant__ TsStepParams p, const uint8_t* mask) {
-  const size_t per = (size_t)p.P * p.K * p.pc_n;
+  const size_t per = (size_t)p.P * p.K * p.pc_np;
   const size_t gt = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (gt >= (size_t)p.E * per) return;
   const int e = (int)(gt / per);
   if (mask && !mask[e]) return;
   p.sh_on[gt] = 0;
+  const size_t r = gt - (size_t)e * per;
+  if (r < (size_t)p.P * p.K) p.sh_cnt[(size_t)e * p.P * p.K + r] = 0;   // anchored-point counters of the env
 }
 
 // ---------------------------------------------------------------------------------------
@@ -2112,7 +2262,7 @@ int ts_launch_shear(const TsStepParams& p, void* stream) {
 }
 
 int ts_launch_reset_shear(const TsStepParams& p, const uint8_t* mask, void* stream) {
-  const size_t n = (size_t)p.E * p.P * p.K * p.pc_n;
+  const size_t n = (size_t)p.E * p.P * p.K * p.pc_np;
   ts_reset_shear_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(p, mask);
   return (int)cudaGetLastError();
 }
