@@ -65,7 +65,7 @@ __global__ void gather_kernel(const Patch* patches, int Q, int nu, int nv, float
   out[gt] = r_prox - t;
 }
 
-__device__ __forceinline__ uint32_t s32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+[[maybe_unused]] __device__ __forceinline__ uint32_t s32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 template <int B>
 __global__ void brick_kernel(const CUtensorMap* __restrict__ tmap_g, const float* lin, const Patch* patches, int Q, int nu, int nv, float pitch,
@@ -73,7 +73,8 @@ __global__ void brick_kernel(const CUtensorMap* __restrict__ tmap_g, const float
                              unsigned* fallbacks) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* brick = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);   // [B][B][B], x fastest; TMA wants 128-byte alignment
-  __shared__ __align__(8) uint64_t bar;
+  __shared__ __align__(8) uint64_t bar;   // unused in the -DBRICK_NO_TMA arm
+  (void)bar;
   __shared__ int org[3];
   const int q = blockIdx.x, tid = threadIdx.x, per = nu * nv;
   const Patch p = patches[q];
